@@ -1,0 +1,150 @@
+/*
+ * qmmm_field.h -- C ABI of the B200-native electrostatic potential / field library.
+ *
+ * Hot path of arxiv 1011.4687 ("Acceleration of a QM/MM-QMC simulation using GPU"):
+ * the electrostatic potential that an environment's fixed charge-density cells and
+ * nuclei produce at the QM electrons' positions,
+ *
+ *     V(r_i) = sum_{j<M} q_j / |r_i - R_j|  +  sum_{b<K} Z_b / |r_i - R_b|
+ *                                              (Eq. 4; V = -U_ES)
+ *     E(r_i) = -grad V(r_i) = sum_j q_j (r_i - R_j) / |r_i - R_j|^3   (north_star)
+ *
+ * an exact, open-boundary direct sum (no cutoff, no softening, no periodic images).
+ * Atomic units (bohr, hartree, elementary charge).  The paper uploads the cell
+ * positions / charges once per run and exchanges only r_new and U_ES per
+ * Monte-Carlo step; that is the create / eval split below.
+ *
+ * Sign: the paper's U_ES (energy of an electron) is -V with q_j = -rho(r_m) dV for
+ * the cells and +Z_b for the nuclei (readings 1-2).
+ *
+ * Precondition: no evaluation point coincides with a source (the paper has no
+ * softening); a coincident pair yields IEEE inf/NaN.  Inputs are not scanned for
+ * non-finite values.
+ *
+ * All entry points return a qmmm_status and never throw or abort; the message of
+ * the last failure on the calling thread is available from qmmm_last_error().
+ * Only sm_100 (B200) devices are supported; there is no CPU or other-GPU fallback.
+ *
+ * Determinism: identical inputs + same device + same library build give
+ * bitwise-identical outputs (fixed CTA -> partial-slot mapping, fixed reduction
+ * order, no floating-point atomics), independent of stream and earlier calls.
+ */
+#ifndef QMMM_FIELD_H
+#define QMMM_FIELD_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qmmm_field qmmm_field;     /* opaque; owned by the library */
+
+typedef enum {
+    QMMM_OK = 0,
+    QMMM_ERR_INVALID_ARG = 1,
+    QMMM_ERR_ALLOC = 2,
+    QMMM_ERR_CUDA = 3,
+    QMMM_ERR_UNSUPPORTED_DEVICE = 4
+} qmmm_status;
+
+/* Arithmetic of the pairwise kernel (kernel in single or double,
+ * everything around it in double).  I/O is FP64 in both modes.
+ *   QMMM_FP64       : FP64 throughout (rel. error <= 1e-12 on V and E).
+ *   QMMM_FP32_ACC64 : cell sources in FP32 arithmetic (MUFU rsqrt + one Newton
+ *                     step), running sums in FP64; nuclei always FP64
+ *                     (per-point rel. error <= 1e-5, energy within 1e-5 hartree). */
+typedef enum { QMMM_FP64 = 0, QMMM_FP32_ACC64 = 1 } qmmm_precision;
+
+/*
+ * qmmm_field_create -- upload and pack one environment (once per run).
+ *   src_xyz [M][3], src_q [M]   cell centres and cell CHARGES q_j (= -rho_j dV)
+ *   nuc_xyz [K][3], nuc_Z [K]   nuclei, enter with charge +Z
+ *   Each pointer may be a host pointer or a device pointer (detected); arrays are
+ *   C-contiguous FP64.  M = 0 and/or K = 0 are valid (then the pointers may be NULL).
+ *   max_points >= 1             largest W*N a later eval may pass (sizes the
+ *                               per-CTA partials workspace).
+ *   *out                        receives the handle.
+ * Ownership: everything needed is copied; the caller may free its arrays on return.
+ * The handle owns its device buffers.  Blocks until the packing has finished.
+ * Errors: INVALID_ARG (NULL out, NULL array with nonzero count, M < 0, K < 0,
+ * max_points < 1), UNSUPPORTED_DEVICE (current device is not compute capability
+ * 10.x), ALLOC, CUDA.
+ */
+qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_t M,
+                              const double *nuc_xyz, const double *nuc_Z, int64_t K,
+                              int64_t max_points, qmmm_field **out);
+
+/*
+ * qmmm_field_eval -- V and E at W*N evaluation points (once per step).
+ *   elec_xyz  DEVICE [W*N][3] FP64    electron positions, W walkers x N electrons
+ *   V         DEVICE [W*N]    FP64    out: potential (cells + nuclei)
+ *   E         DEVICE [W*N][3] FP64    out: field; NULL = potential only
+ *   prec      qmmm_precision
+ *   stream    cudaStream_t (as void*); all work is enqueued on it, the call never
+ *             synchronises.  One eval in flight per handle (shared workspace).
+ * Errors: INVALID_ARG (NULL handle/elec_xyz/V, W*N < 1 or > max_points, bad prec),
+ * CUDA (launch failure).  Outputs are unspecified after an error.
+ */
+qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t N,
+                            double *V, double *E, int prec, void *stream);
+
+/*
+ * qmmm_field_eval_host -- the paper's per-step loop: HOST buffers
+ * in and out.  Copies elec_xyz host->device, evaluates, copies V (and E) back on
+ * `stream`, and synchronises the stream before returning.  Buffers may be pageable
+ * or pinned.  Same argument meaning and errors as qmmm_field_eval.
+ */
+qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int64_t W,
+                                 int64_t N, double *V_host, double *E_host, int prec,
+                                 void *stream);
+
+/* qmmm_field_destroy -- frees the handle and its device buffers.  NULL is a no-op. */
+qmmm_status qmmm_field_destroy(qmmm_field *h);
+
+/* Launch plan of the pairwise kernel (Eq. 5-6: U = B[1]+...+B[N_B]).
+ * 0 in a field of qmmm_field_set_plan means "choose automatically". */
+typedef struct {
+    int32_t points_per_thread;   /* register blocking: 1, 2, 4 or 8 electrons per thread */
+    int32_t point_warps;         /* warps of a CTA that own different point groups: 1,2,4,8 */
+    int32_t slices;              /* N_B: CTAs the source sum is split over (per point block) */
+    int32_t stages;              /* TMA pipeline depth (shared-memory stages), 2..8 */
+} qmmm_plan;
+
+/* Override the automatic plan (testing partition independence, tuning).  Sticky
+ * until changed; pass zeros to restore automatic choice.  INVALID_ARG on bad values. */
+qmmm_status qmmm_field_set_plan(qmmm_field *h, const qmmm_plan *plan);
+
+typedef struct {
+    int64_t M, K, max_points;
+    int64_t n_chunks;            /* 128-source chunks after padding */
+    int64_t bytes_fp64, bytes_fp32, bytes_workspace;
+    qmmm_plan last_plan;         /* plan used by the most recent eval */
+    int32_t last_point_blocks;   /* grid.y of the most recent pair kernel */
+    int32_t last_launches;       /* kernels launched by the most recent eval */
+    int32_t sm_count;
+    int32_t reserved;
+} qmmm_field_info;
+
+qmmm_status qmmm_field_get_info(const qmmm_field *h, qmmm_field_info *info);
+
+/*
+ * qmmm_probe_peak -- same-run roofline denominators (north_star: "measured by a
+ * microbenchmark in the same run").  Runs a register-only kernel of independent
+ * dependent chains on every SM and reports the achieved rate.
+ *   kind 0: FP32 FFMA, 1: FP64 DFMA, 2: MUFU.RSQ (FP32), 3: empty-kernel launch+sync
+ *   iters      inner iterations (0 = default)
+ *   *rate      out: warp-lane operations per second (kind 0-2; an FMA counts 1),
+ *              or seconds per launch+sync (kind 3)
+ *   *seconds   out: device time of the timed launch (CUDA events), may be NULL
+ * Synchronises the stream.
+ */
+qmmm_status qmmm_probe_peak(int kind, int iters, double *rate, double *seconds, void *stream);
+
+/* Thread-local message of the last error returned on this thread ("" if none). */
+const char *qmmm_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QMMM_FIELD_H */

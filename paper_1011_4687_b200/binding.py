@@ -1,0 +1,185 @@
+"""Thin ctypes binding of include/qmmm_field.h (argument marshalling only).
+
+Every step of the path runs in the CUDA library; PyTorch is used here only for device
+memory and streams (tensor ``data_ptr()`` and ``torch.cuda.current_stream()``).  There is
+no CPU fallback: if ``libqmmm_field.so`` is missing the import of this module raises.
+Function names mirror the C ABI: ``qmmm_field_create``, ``qmmm_field_eval``,
+``qmmm_field_eval_host``, ``qmmm_field_destroy`` (PAPER.md:117 create/eval split).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Tuple
+
+import numpy as np
+
+QMMM_FP64 = 0
+QMMM_FP32_ACC64 = 1
+_PREC = {"fp64": QMMM_FP64, "fp32": QMMM_FP32_ACC64, QMMM_FP64: QMMM_FP64,
+         QMMM_FP32_ACC64: QMMM_FP32_ACC64}
+_STATUS = {0: "QMMM_OK", 1: "QMMM_ERR_INVALID_ARG", 2: "QMMM_ERR_ALLOC", 3: "QMMM_ERR_CUDA",
+           4: "QMMM_ERR_UNSUPPORTED_DEVICE"}
+
+LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libqmmm_field.so")
+EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_host",
+                    "qmmm_field_destroy", "qmmm_field_set_plan", "qmmm_field_get_info",
+                    "qmmm_probe_peak", "qmmm_last_error")
+
+
+class QmmmError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{_STATUS.get(status, status)}: {message}")
+        self.status = status
+
+
+class qmmm_plan(ctypes.Structure):
+    _fields_ = [("points_per_thread", ctypes.c_int32), ("point_warps", ctypes.c_int32),
+                ("slices", ctypes.c_int32), ("stages", ctypes.c_int32)]
+
+
+class qmmm_field_info(ctypes.Structure):
+    _fields_ = [("M", ctypes.c_int64), ("K", ctypes.c_int64), ("max_points", ctypes.c_int64),
+                ("n_chunks", ctypes.c_int64), ("bytes_fp64", ctypes.c_int64),
+                ("bytes_fp32", ctypes.c_int64), ("bytes_workspace", ctypes.c_int64),
+                ("last_plan", qmmm_plan), ("last_point_blocks", ctypes.c_int32),
+                ("last_launches", ctypes.c_int32), ("sm_count", ctypes.c_int32),
+                ("reserved", ctypes.c_int32)]
+
+
+def _load() -> ctypes.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_1011_4687_b200.build` "
+            "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i64, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int
+    lib.qmmm_field_create.restype = ci
+    lib.qmmm_field_create.argtypes = [vp, vp, i64, vp, vp, i64, i64, ctypes.POINTER(vp)]
+    lib.qmmm_field_eval.restype = ci
+    lib.qmmm_field_eval.argtypes = [vp, vp, i64, i64, vp, vp, ci, vp]
+    lib.qmmm_field_eval_host.restype = ci
+    lib.qmmm_field_eval_host.argtypes = [vp, vp, i64, i64, vp, vp, ci, vp]
+    lib.qmmm_field_destroy.restype = ci
+    lib.qmmm_field_destroy.argtypes = [vp]
+    lib.qmmm_field_set_plan.restype = ci
+    lib.qmmm_field_set_plan.argtypes = [vp, ctypes.POINTER(qmmm_plan)]
+    lib.qmmm_field_get_info.restype = ci
+    lib.qmmm_field_get_info.argtypes = [vp, ctypes.POINTER(qmmm_field_info)]
+    lib.qmmm_probe_peak.restype = ci
+    lib.qmmm_probe_peak.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double),
+                                    ctypes.POINTER(ctypes.c_double), vp]
+    lib.qmmm_last_error.restype = ctypes.c_char_p
+    lib.qmmm_last_error.argtypes = []
+    return lib
+
+
+_lib = _load()
+
+
+def _check(status: int) -> None:
+    if status != 0:
+        raise QmmmError(status, _lib.qmmm_last_error().decode())
+
+
+def _ptr(a) -> Optional[int]:
+    """Raw address of a numpy array (host) or torch tensor (host or device); None -> NULL."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        assert a.dtype == np.float64 and a.flags.c_contiguous
+        return a.ctypes.data if a.size else None
+    assert a.dtype.is_floating_point and a.element_size() == 8 and a.is_contiguous()
+    return a.data_ptr() if a.numel() else None
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream or None
+    return getattr(stream, "cuda_stream", stream) or None
+
+
+def qmmm_field_create(src_xyz, src_q, nuc_xyz, nuc_Z, max_points: int) -> int:
+    """Upload + pack one environment; arrays are FP64 numpy arrays or torch tensors (host
+    or device).  Returns the opaque handle."""
+    M = int(src_q.shape[0]) if src_q is not None else 0
+    K = int(nuc_Z.shape[0]) if nuc_Z is not None else 0
+    out = ctypes.c_void_p()
+    _check(_lib.qmmm_field_create(_ptr(src_xyz), _ptr(src_q), M, _ptr(nuc_xyz), _ptr(nuc_Z), K,
+                                  int(max_points), ctypes.byref(out)))
+    return out.value
+
+
+def qmmm_field_eval(handle: int, elec_xyz, W: int, N: int, V, E=None, precision="fp64",
+                    stream=None) -> None:
+    """Asynchronous evaluation on device tensors (elec_xyz [W*N,3], V [W*N], E [W*N,3])."""
+    _check(_lib.qmmm_field_eval(handle, _ptr(elec_xyz), int(W), int(N), _ptr(V), _ptr(E),
+                                _PREC[precision], _stream(stream)))
+
+
+def qmmm_field_eval_host(handle: int, elec_xyz, W: int, N: int, V, E=None, precision="fp64",
+                         stream=None) -> None:
+    """Per-step host loop of PAPER.md:117: host buffers in/out, synchronises the stream."""
+    _check(_lib.qmmm_field_eval_host(handle, _ptr(elec_xyz), int(W), int(N), _ptr(V), _ptr(E),
+                                     _PREC[precision], _stream(stream)))
+
+
+def qmmm_field_destroy(handle: Optional[int]) -> None:
+    _check(_lib.qmmm_field_destroy(handle))
+
+
+def qmmm_field_set_plan(handle: int, points_per_thread=0, point_warps=0, slices=0, stages=0):
+    pl = qmmm_plan(points_per_thread, point_warps, slices, stages)
+    _check(_lib.qmmm_field_set_plan(handle, ctypes.byref(pl)))
+
+
+def qmmm_field_get_info(handle: int) -> dict:
+    info = qmmm_field_info()
+    _check(_lib.qmmm_field_get_info(handle, ctypes.byref(info)))
+    d = {k: getattr(info, k) for k, _ in info._fields_ if k not in ("last_plan", "reserved")}
+    d["last_plan"] = {k: getattr(info.last_plan, k) for k, _ in qmmm_plan._fields_}
+    return d
+
+
+def qmmm_probe_peak(kind: int, iters: int = 0, stream=None) -> Tuple[float, float]:
+    """(rate, seconds): kind 0 FFMA, 1 DFMA, 2 MUFU.RSQ lane-ops/s; 3 launch+sync seconds."""
+    rate, secs = ctypes.c_double(), ctypes.c_double()
+    _check(_lib.qmmm_probe_peak(kind, iters, ctypes.byref(rate), ctypes.byref(secs),
+                                _stream(stream)))
+    return rate.value, secs.value
+
+
+class FieldEvaluator:
+    """Convenience owner of a handle (context manager); still argument marshalling only."""
+
+    def __init__(self, src_xyz, src_q, nuc_xyz, nuc_Z, max_points: int):
+        self.handle = qmmm_field_create(src_xyz, src_q, nuc_xyz, nuc_Z, max_points)
+
+    def eval(self, elec_xyz, precision="fp64", want_E=True, stream=None):
+        """elec_xyz: CUDA FP64 tensor [..., 3]; returns (V [...], E [..., 3] or None)."""
+        import torch
+        pts = elec_xyz.reshape(-1, 3).contiguous()
+        P = pts.shape[0]
+        V = torch.empty(P, dtype=torch.float64, device=pts.device)
+        E = torch.empty((P, 3), dtype=torch.float64, device=pts.device) if want_E else None
+        qmmm_field_eval(self.handle, pts, 1, P, V, E, precision, stream)
+        lead = elec_xyz.shape[:-1]
+        return V.reshape(lead), (E.reshape(*lead, 3) if want_E else None)
+
+    def close(self):
+        if self.handle is not None:
+            qmmm_field_destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

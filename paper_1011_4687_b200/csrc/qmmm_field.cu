@@ -1,0 +1,380 @@
+// qmmm_field.cu -- C ABI (include/qmmm_field.h) and host-side launch logic.
+//
+// create : upload + pack sources once ("required only once at the beginning
+//          of a run"), FP64 SoA chunks and FP32 tile-local SoA chunks, nuclei FP64.
+// eval   : pair kernel over (source slices x point blocks)  ->  per-slice partials
+//          (Eq. 5-6)  ->  finalize kernel (fixed-order sum + nuclei).
+// No torch types, no CPU fallback: every step of the path runs in the kernels of
+// qmmm_kernels.cuh.
+#include "qmmm_kernels.cuh"
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/qmmm_field.h"
+
+using namespace qmmm;
+
+namespace {
+
+thread_local std::string g_last_error;
+
+qmmm_status fail(qmmm_status st, const std::string &msg) {
+    g_last_error = msg;
+    return st;
+}
+qmmm_status cuda_fail(cudaError_t e, const char *what) {
+    return fail(QMMM_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CUDA_TRY(expr)                                          \
+    do {                                                        \
+        cudaError_t _e = (expr);                                \
+        if (_e != cudaSuccess) return cuda_fail(_e, #expr);     \
+    } while (0)
+
+int pow2_ceil(int64_t v) {
+    int p = 1;
+    while (p < v) p <<= 1;
+    return p;
+}
+int gcd_int(int a, int b) {
+    while (b) { int t = a % b; a = b; b = t; }
+    return a;
+}
+
+constexpr size_t stage_bytes(bool f32) {
+    return STAGE_HDR + static_cast<size_t>(BLOCK_CHUNKS) * 4 * CHUNK * (f32 ? 4 : 8);
+}
+size_t pair_smem_bytes(bool f32, int stages, int ept, int wp) {
+    return stages * stage_bytes(f32) + 16 * sizeof(uint64_t) +
+           static_cast<size_t>(COMPUTE_WARPS) * ept * 4 * sizeof(double) +
+           static_cast<size_t>(wp) * ept * 3 * sizeof(double);
+}
+
+}  // namespace
+
+struct qmmm_field {
+    int64_t M = 0, K = 0, max_points = 0;
+    int64_t n_chunks = 0, n_blocks = 0;
+    int device = 0, sm_count = 0;
+    double *chunks64 = nullptr;    // [n_chunks][4][128] double
+    float *chunks32 = nullptr;     // [n_chunks][4][128] float (offsets from block origin, q)
+    double *origins = nullptr;     // [n_blocks][4]
+    double *nuclei = nullptr;      // [K][4]
+    double *workspace = nullptr;   // partials [slices][P][4]
+    int64_t workspace_doubles = 0;
+    double *stage_elec = nullptr;  // eval_host staging: [max_points][3]
+    double *stage_out = nullptr;   // eval_host staging: V [max_points] then E [max_points][3]
+    qmmm_plan user_plan = {0, 0, 0, 0};
+    qmmm_plan last_plan = {0, 0, 0, 0};
+    int last_point_blocks = 0, last_launches = 0;
+};
+
+namespace {
+
+// Automatic plan: enough (point block x source slice) CTAs to fill the
+// SMs in whole waves; few points -> sources split across all warps and SMs.
+qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32) {
+    qmmm_plan pl = h->user_plan;
+    const int max_ept = f32 ? 8 : 4;
+    if (pl.points_per_thread == 0) pl.points_per_thread = std::min(max_ept, pow2_ceil(P));
+    const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
+    if (pl.point_warps == 0)
+        pl.point_warps = std::min<int>(COMPUTE_WARPS, pow2_ceil(groups));
+    const int64_t pb = (groups + pl.point_warps - 1) / pl.point_warps;
+    if (pl.slices == 0) {
+        const int g = gcd_int(static_cast<int>(pb % h->sm_count), h->sm_count);
+        pl.slices = h->sm_count / g;       // pb * slices is a multiple of the SM count
+    }
+    pl.slices = static_cast<int>(std::max<int64_t>(1, std::min<int64_t>(pl.slices, h->n_chunks)));
+    // the partials workspace bounds slices * P
+    const int64_t cap = h->workspace_doubles / (4 * P);
+    if (pl.slices > cap) pl.slices = static_cast<int>(std::max<int64_t>(1, cap));
+    if (pl.stages == 0) {
+        const bool bandwidth_bound = groups <= 2;
+        pl.stages = f32 ? (bandwidth_bound ? 8 : 4) : (bandwidth_bound ? 6 : 3);
+    }
+    return pl;
+}
+
+template <typename REAL, int EPT>
+cudaError_t launch_pair(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
+    auto kern = pair_kernel<REAL, EPT>;
+    static thread_local size_t configured = 0;
+    if (smem > configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             static_cast<int>(smem));
+        if (e != cudaSuccess) return e;
+        configured = smem;
+    }
+    kern<<<grid, CTA_THREADS, smem, st>>>(prm);
+    return cudaGetLastError();
+}
+
+template <typename REAL>
+cudaError_t launch_pair_ept(int ept, const PairParams &prm, dim3 grid, size_t smem,
+                            cudaStream_t st) {
+    switch (ept) {
+        case 1: return launch_pair<REAL, 1>(prm, grid, smem, st);
+        case 2: return launch_pair<REAL, 2>(prm, grid, smem, st);
+        case 4: return launch_pair<REAL, 4>(prm, grid, smem, st);
+        case 8: return launch_pair<REAL, 8>(prm, grid, smem, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+bool is_device_pointer(const void *p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+// Returns a device pointer holding n doubles of src (copying when src is a host pointer).
+cudaError_t to_device(const double *src, int64_t n, double **dev, bool *owned) {
+    *owned = false;
+    *dev = nullptr;
+    if (n == 0) return cudaSuccess;
+    if (is_device_pointer(src)) {
+        *dev = const_cast<double *>(src);
+        return cudaSuccess;
+    }
+    cudaError_t e = cudaMalloc(dev, n * sizeof(double));
+    if (e != cudaSuccess) return e;
+    *owned = true;
+    return cudaMemcpy(*dev, src, n * sizeof(double), cudaMemcpyHostToDevice);
+}
+
+}  // namespace
+
+// =============================================================================== C ABI
+extern "C" {
+
+const char *qmmm_last_error(void) { return g_last_error.c_str(); }
+
+qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_t M,
+                              const double *nuc_xyz, const double *nuc_Z, int64_t K,
+                              int64_t max_points, qmmm_field **out) {
+    if (!out) return fail(QMMM_ERR_INVALID_ARG, "create: out is NULL");
+    *out = nullptr;
+    if (M < 0 || K < 0) return fail(QMMM_ERR_INVALID_ARG, "create: negative M or K");
+    if (max_points < 1) return fail(QMMM_ERR_INVALID_ARG, "create: max_points < 1");
+    if (M > 0 && (!src_xyz || !src_q))
+        return fail(QMMM_ERR_INVALID_ARG, "create: NULL source array with M > 0");
+    if (K > 0 && (!nuc_xyz || !nuc_Z))
+        return fail(QMMM_ERR_INVALID_ARG, "create: NULL nuclear array with K > 0");
+    if (M > (int64_t(1) << 37)) return fail(QMMM_ERR_INVALID_ARG, "create: M too large");
+
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10)
+        return fail(QMMM_ERR_UNSUPPORTED_DEVICE,
+                    "create: device is sm_" + std::to_string(prop.major * 10 + prop.minor) +
+                        ", this library is built for sm_100a (B200) only");
+
+    qmmm_field *h = new (std::nothrow) qmmm_field();
+    if (!h) return fail(QMMM_ERR_ALLOC, "create: host allocation failed");
+    h->M = M; h->K = K; h->max_points = max_points;
+    h->device = dev; h->sm_count = prop.multiProcessorCount;
+    h->n_chunks = (M + CHUNK - 1) / CHUNK;
+    h->n_blocks = (h->n_chunks + BLOCK_CHUNKS - 1) / BLOCK_CHUNKS;
+
+    auto bail = [&](qmmm_status st) { qmmm_field_destroy(h); return st; };
+#define CREATE_TRY(expr)                                                               \
+    do {                                                                               \
+        cudaError_t _e = (expr);                                                       \
+        if (_e != cudaSuccess)                                                         \
+            return bail(_e == cudaErrorMemoryAllocation                                \
+                            ? fail(QMMM_ERR_ALLOC, std::string(#expr) + ": out of memory") \
+                            : cuda_fail(_e, #expr));                                   \
+    } while (0)
+
+    if (M > 0) {
+        const int64_t Mpad = h->n_chunks * CHUNK;
+        double *dxyz = nullptr, *dq = nullptr;
+        bool own_xyz = false, own_q = false;
+        CREATE_TRY(to_device(src_xyz, 3 * M, &dxyz, &own_xyz));
+        cudaError_t e = to_device(src_q, M, &dq, &own_q);
+        if (e == cudaSuccess) e = cudaMalloc(&h->chunks64, Mpad * 4 * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc(&h->chunks32, Mpad * 4 * sizeof(float));
+        if (e == cudaSuccess) e = cudaMalloc(&h->origins, h->n_blocks * 4 * sizeof(double));
+        if (e == cudaSuccess) {
+            const int T = 256;
+            const unsigned nb = static_cast<unsigned>((Mpad + T - 1) / T);
+            pack_f64_kernel<<<nb, T>>>(dxyz, dq, M, Mpad, h->chunks64);
+            origins_kernel<<<static_cast<unsigned>((h->n_blocks * 32 + T - 1) / T), T>>>(
+                dxyz, M, h->n_blocks, h->origins);
+            pack_f32_kernel<<<nb, T>>>(dxyz, dq, M, Mpad, h->origins, h->chunks32);
+            e = cudaGetLastError();
+            if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        }
+        if (own_xyz) cudaFree(dxyz);
+        if (own_q) cudaFree(dq);
+        CREATE_TRY(e);
+    }
+    if (K > 0) {
+        double *dxyz = nullptr, *dz = nullptr;
+        bool own_xyz = false, own_z = false;
+        CREATE_TRY(to_device(nuc_xyz, 3 * K, &dxyz, &own_xyz));
+        cudaError_t e = to_device(nuc_Z, K, &dz, &own_z);
+        if (e == cudaSuccess) e = cudaMalloc(&h->nuclei, K * 4 * sizeof(double));
+        if (e == cudaSuccess) {
+            pack_nuclei_kernel<<<static_cast<unsigned>((K + 255) / 256), 256>>>(dxyz, dz, K, h->nuclei);
+            e = cudaGetLastError();
+            if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        }
+        if (own_xyz) cudaFree(dxyz);
+        if (own_z) cudaFree(dz);
+        CREATE_TRY(e);
+    }
+    // Partials workspace: slices * P * 4 doubles.  With P = max_points the automatic plan
+    // uses at most sm_count slices; small P uses more slices but a smaller product.
+    h->workspace_doubles =
+        4 * std::max<int64_t>(static_cast<int64_t>(h->sm_count) * max_points, int64_t(1) << 16);
+    CREATE_TRY(cudaMalloc(&h->workspace, h->workspace_doubles * sizeof(double)));
+    CREATE_TRY(cudaMalloc(&h->stage_elec, max_points * 3 * sizeof(double)));
+    CREATE_TRY(cudaMalloc(&h->stage_out, max_points * 4 * sizeof(double)));
+#undef CREATE_TRY
+    *out = h;
+    return QMMM_OK;
+}
+
+qmmm_status qmmm_field_destroy(qmmm_field *h) {
+    if (!h) return QMMM_OK;
+    cudaFree(h->chunks64);
+    cudaFree(h->chunks32);
+    cudaFree(h->origins);
+    cudaFree(h->nuclei);
+    cudaFree(h->workspace);
+    cudaFree(h->stage_elec);
+    cudaFree(h->stage_out);
+    delete h;
+    return QMMM_OK;
+}
+
+qmmm_status qmmm_field_set_plan(qmmm_field *h, const qmmm_plan *plan) {
+    if (!h || !plan) return fail(QMMM_ERR_INVALID_ARG, "set_plan: NULL argument");
+    const int e = plan->points_per_thread, w = plan->point_warps;
+    if (!(e == 0 || e == 1 || e == 2 || e == 4 || e == 8))
+        return fail(QMMM_ERR_INVALID_ARG, "set_plan: points_per_thread must be 0,1,2,4,8");
+    if (!(w == 0 || w == 1 || w == 2 || w == 4 || w == 8))
+        return fail(QMMM_ERR_INVALID_ARG, "set_plan: point_warps must be 0,1,2,4,8");
+    if (plan->slices < 0 || plan->slices > 65535)
+        return fail(QMMM_ERR_INVALID_ARG, "set_plan: slices out of range");
+    if (plan->stages != 0 && (plan->stages < 2 || plan->stages > 8))
+        return fail(QMMM_ERR_INVALID_ARG, "set_plan: stages must be 0 or 2..8");
+    h->user_plan = *plan;
+    return QMMM_OK;
+}
+
+qmmm_status qmmm_field_get_info(const qmmm_field *h, qmmm_field_info *info) {
+    if (!h || !info) return fail(QMMM_ERR_INVALID_ARG, "get_info: NULL argument");
+    std::memset(info, 0, sizeof(*info));
+    info->M = h->M; info->K = h->K; info->max_points = h->max_points;
+    info->n_chunks = h->n_chunks;
+    info->bytes_fp64 = h->n_chunks * CHUNK * 4 * 8;
+    info->bytes_fp32 = h->n_chunks * CHUNK * 4 * 4 + h->n_blocks * 32;
+    info->bytes_workspace = h->workspace_doubles * 8;
+    info->last_plan = h->last_plan;
+    info->last_point_blocks = h->last_point_blocks;
+    info->last_launches = h->last_launches;
+    info->sm_count = h->sm_count;
+    return QMMM_OK;
+}
+
+qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t N,
+                            double *V, double *E, int prec, void *stream) {
+    if (!h) return fail(QMMM_ERR_INVALID_ARG, "eval: NULL handle");
+    if (!elec_xyz || !V) return fail(QMMM_ERR_INVALID_ARG, "eval: NULL elec_xyz or V");
+    if (W < 1 || N < 1 || W > h->max_points || N > h->max_points || W * N > h->max_points)
+        return fail(QMMM_ERR_INVALID_ARG, "eval: W*N must be in [1, max_points]");
+    if (prec != QMMM_FP64 && prec != QMMM_FP32_ACC64)
+        return fail(QMMM_ERR_INVALID_ARG, "eval: unknown precision");
+    const bool f32 = prec == QMMM_FP32_ACC64;
+    const int P = static_cast<int>(W * N);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+
+    qmmm_plan pl = choose_plan(h, P, f32);
+    const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
+    const int pb = static_cast<int>((groups + pl.point_warps - 1) / pl.point_warps);
+    int launches = 0;
+    const size_t smem = pair_smem_bytes(f32, pl.stages, pl.points_per_thread, pl.point_warps);
+    if (smem > 227 * 1024) return fail(QMMM_ERR_INVALID_ARG, "eval: plan exceeds shared memory");
+    if (pb > 65535) return fail(QMMM_ERR_INVALID_ARG, "eval: too many point blocks for this plan");
+
+    if (h->n_chunks > 0) {
+        PairParams prm;
+        prm.chunks = f32 ? reinterpret_cast<const char *>(h->chunks32)
+                         : reinterpret_cast<const char *>(h->chunks64);
+        prm.origins = h->origins;
+        prm.elec = elec_xyz;
+        prm.partial = h->workspace;
+        prm.P = P;
+        prm.n_chunks = static_cast<int>(h->n_chunks);
+        prm.slices = pl.slices;
+        prm.point_warps = pl.point_warps;
+        prm.stages = pl.stages;
+        const dim3 grid(pl.slices, pb);
+        cudaError_t e = f32 ? launch_pair_ept<float>(pl.points_per_thread, prm, grid, smem, st)
+                            : launch_pair_ept<double>(pl.points_per_thread, prm, grid, smem, st);
+        if (e != cudaSuccess) return cuda_fail(e, "pair_kernel launch");
+        ++launches;
+    }
+    FinalizeParams fp;
+    fp.partial = h->workspace;
+    fp.nuc = h->nuclei;
+    fp.elec = elec_xyz;
+    fp.V = V;
+    fp.E = E;
+    fp.P = P;
+    fp.slices = h->n_chunks > 0 ? pl.slices : 0;
+    fp.K = static_cast<int>(h->K);
+    fp.tpp = P <= 64 ? 256 : 32;
+    const int per_cta = 256 / fp.tpp;
+    finalize_kernel<<<(P + per_cta - 1) / per_cta, 256, 0, st>>>(fp);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "finalize_kernel launch");
+    ++launches;
+
+    h->last_plan = pl;
+    h->last_point_blocks = pb;
+    h->last_launches = launches;
+    return QMMM_OK;
+}
+
+qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int64_t W,
+                                 int64_t N, double *V_host, double *E_host, int prec,
+                                 void *stream) {
+    if (!h) return fail(QMMM_ERR_INVALID_ARG, "eval_host: NULL handle");
+    if (!elec_xyz_host || !V_host)
+        return fail(QMMM_ERR_INVALID_ARG, "eval_host: NULL elec_xyz or V");
+    if (W < 1 || N < 1 || W > h->max_points || N > h->max_points || W * N > h->max_points)
+        return fail(QMMM_ERR_INVALID_ARG, "eval_host: W*N must be in [1, max_points]");
+    const int64_t P = W * N;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    CUDA_TRY(cudaMemcpyAsync(h->stage_elec, elec_xyz_host, P * 3 * sizeof(double),
+                             cudaMemcpyHostToDevice, st));
+    double *dV = h->stage_out, *dE = E_host ? h->stage_out + P : nullptr;
+    qmmm_status s = qmmm_field_eval(h, h->stage_elec, W, N, dV, dE, prec, stream);
+    if (s != QMMM_OK) return s;
+    // V and E are adjacent in the staging buffer: one device->host copy when both are wanted
+    // and the host buffers are adjacent too, else two.
+    if (E_host && E_host == V_host + P) {
+        CUDA_TRY(cudaMemcpyAsync(V_host, dV, P * 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    } else {
+        CUDA_TRY(cudaMemcpyAsync(V_host, dV, P * sizeof(double), cudaMemcpyDeviceToHost, st));
+        if (E_host)
+            CUDA_TRY(cudaMemcpyAsync(E_host, dE, P * 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    }
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return QMMM_OK;
+}
+
+}  // extern "C"

