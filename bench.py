@@ -1,0 +1,399 @@
+#!/usr/bin/env python
+"""bench.py -- pair-interactions/s of the QM/MM electrostatic potential + field hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl reference]
+
+A "step" is one pass of the whole hot path (pair kernel + finalize kernel; SURVEY.md 8(a)
+rows a1-a6) over one batch of synthetic evaluation points of the chosen BASELINE.json
+configuration.  Rank 0 prints ONE JSON line.  See DESIGN.md "Measurement".
+
+* value      : whole-job pair-interactions/s (G/s), inputs resident in HBM, per-step CUDA
+               events on the launch stream, L2 flushed between steps, max over ranks.
+* e2e        : same metric through qmmm_field_eval_host (the paper's per-step loop,
+               PAPER.md:117): pinned HOST buffers, H2D + kernels + D2H + stream sync timed.
+* roofline   : pair kernel alone (events recorded by the library between its two kernels)
+               against the FMA-lane rate measured by the library's microbenchmark in the
+               same process ("bound": "alu").
+* cpu_baseline: the CPU oracle as it stands on a bounded sample of the same workload.
+* --impl reference : times the oracle (the only reference this tier has) on host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1011_4687_b200.workloads import CONFIG_SPECS, make_workload  # noqa: E402
+
+METRIC = "pair-interactions/s"
+UNIT = "Gpair/s"
+SLOTS = {"fp32": 17, "fp64": 18}      # algorithmic FMA-pipe slots per pair
+DTYPE = {"fp32": "f32 (f64 accumulation)", "fp64": "f64"}
+WORKLOAD_NAME = {i: f"configs[{i}] {s['name']}" for i, s in CONFIG_SPECS.items()}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (0-4)")
+    ap.add_argument("--precision", default=None, choices=["fp32", "fp64"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-sweep", action="store_true",
+                    help="skip the per-config table (all five configs) at N=1")
+    ap.add_argument("--cpu-sample-pairs", type=float, default=6e9,
+                    help="pairs in the cpu_baseline sample (about 10-30 s of host time)")
+    return ap.parse_args()
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+# ------------------------------------------------------------------------------ clocks
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML during the timed region."""
+
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown",
+               0x4: "sw_power_cap", 0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks",
+               0x100: "display_clock", 0x10: "sync_boost"}
+
+    def __init__(self, index: int, period: float = 0.02):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.power = [], set(), []
+        self.max_mhz = None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+                mask = self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                for bit, name in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+                self.power.append(self.nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self) -> dict:
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join()
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples),
+                "power_w_max": max(self.power) if self.power else None}
+
+
+# ------------------------------------------------------------------------ oracle timing
+def oracle_sample_rate(w, sample_pairs: float, seed: int = 99):
+    """Times the CPU oracle (as it stands) on a seeded subsample of the evaluation points."""
+    import oracle
+    oracle.build()
+    pts = w.elec_xyz.reshape(-1, 3)
+    per_point = w.M + w.K
+    n = int(max(1, min(len(pts), round(sample_pairs / per_point))))
+    rng = np.random.default_rng(seed)
+    idx = np.sort(rng.choice(len(pts), size=n, replace=False))
+    sub = np.ascontiguousarray(pts[idx])
+    t0 = time.perf_counter()
+    res = oracle.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, sub)
+    dt = time.perf_counter() - t0
+    pairs = n * per_point
+    return dict(pairs=pairs, seconds=dt, rate=pairs / dt, threads=res.threads, n_points=n,
+                n_total=len(pts))
+
+
+def run_reference(args):
+    """--impl reference: the oracle on host cores, same metric/config; rank 0 only."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    w = make_workload(args.config)
+    prec = args.precision or w.precisions[0]
+    # each step: a bounded sample sized so warmup+steps finish within a few minutes
+    per_step_pairs = min(args.cpu_sample_pairs / 4, 1.5e9)
+    for _ in range(args.warmup):
+        oracle_sample_rate(w, per_step_pairs / 8)
+    times, pairs, threads, npts = [], 0, 1, 0
+    for s in range(args.steps):
+        r = oracle_sample_rate(w, per_step_pairs, seed=1000 + s)
+        times.append(r["seconds"]); pairs += r["pairs"]; threads = r["threads"]; npts = r["n_points"]
+    total = sum(times)
+    value = pairs / total / 1e9
+    sample = f"{npts} of {w.P} evaluation points per step x all {w.M}+{w.K} sources"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD_NAME[args.config], "precision": "fp64 (oracle)",
+                   "M": w.M, "K": w.K, "W": w.W, "N": w.N,
+                   "note": "CPU oracle (plain FP64 Kahan double loop), bounded sample per step"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------ GPU arm
+class L2Flusher:
+    """Writes a buffer larger than the 126 MB L2 between timed steps."""
+
+    def __init__(self, torch, nbytes=256 << 20):
+        self.buf = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        self.k = 0
+
+    def __call__(self):
+        self.k = (self.k + 1) & 0x7F
+        self.buf.fill_(self.k)
+
+
+def probe_peaks(B):
+    ffma, _ = B.qmmm_probe_peak(0)
+    dfma, _ = B.qmmm_probe_peak(1)
+    mufu, _ = B.qmmm_probe_peak(2)
+    return {"ffma_lane_ops_per_s": ffma, "dfma_lane_ops_per_s": dfma, "mufu_lane_ops_per_s": mufu}
+
+
+def time_steps(torch, B, h, batches, W, N, prec, steps, warmup, flush, stream):
+    """Per-step CUDA events on the launch stream; returns (step_ms list, pair_ms list)."""
+    P = W * N
+    V = torch.empty(P, dtype=torch.float64, device="cuda")
+    E = torch.empty((P, 3), dtype=torch.float64, device="cuda")
+    for i in range(warmup):
+        B.qmmm_field_eval(h, batches[i % len(batches)], W, N, V, E, prec, stream)
+    torch.cuda.synchronize()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+           for _ in range(steps)]
+    pair_ms = []
+    for i in range(steps):
+        if flush is not None:
+            flush()
+        evs[i][0].record(stream)
+        B.qmmm_field_eval(h, batches[i % len(batches)], W, N, V, E, prec, stream)
+        evs[i][1].record(stream)
+        pair_ms.append(B.qmmm_field_last_timing(h)[0])      # waits for this eval
+    torch.cuda.synchronize()
+    return [a.elapsed_time(b) for a, b in evs], pair_ms, (V, E)
+
+
+def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
+    """Per-config table (N=1): ms per evaluation, Gpair/s and FMA-pipe fraction for every
+    BASELINE.json configuration and precision; config 2 also as the QMC host loop."""
+    out = []
+    stream = torch.cuda.current_stream()
+    flush = L2Flusher(torch)
+    for idx in sorted(CONFIG_SPECS):
+        w = make_workload(idx)
+        W, N = (1, 1) if w.sequential else (w.W, w.N)
+        P = W * N
+        h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, P)
+        try:
+            pts = torch.from_numpy(w.elec_xyz.reshape(-1, 3)).cuda()
+            batches = [pts[i:i + 1].contiguous() for i in range(8)] if w.sequential else [pts]
+            for prec in w.precisions:
+                reps = 5 if idx >= 3 else 30
+                B.qmmm_field_set_timing(h, True)
+                step_ms, pair_ms, _ = time_steps(torch, B, h, batches, W, N, prec, reps, 3, flush, stream)
+                pairs = P * (w.M + w.K)
+                peak = peaks["ffma_lane_ops_per_s" if prec == "fp32" else "dfma_lane_ops_per_s"]
+                row = {"config": idx, "name": w.name, "precision": prec, "points": P, "M": w.M,
+                       "K": w.K, "pairs_per_eval": pairs,
+                       "ms_per_eval_median": float(np.median(step_ms)),
+                       "ms_per_eval_min": float(np.min(step_ms)),
+                       "pair_kernel_ms_median": float(np.median(pair_ms)),
+                       "gpairs_per_s": pairs / np.median(step_ms) / 1e6,
+                       "fma_pipe_frac": pairs * SLOTS[prec] / (np.median(step_ms) * 1e-3) / peak,
+                       "plan": B.qmmm_field_get_info(h)["last_plan"]}
+                if w.sequential:
+                    # (i) 1,000 back-to-back evaluations, positions resident on the device
+                    B.qmmm_field_set_timing(h, False)
+                    V = torch.empty(1, dtype=torch.float64, device="cuda")
+                    E = torch.empty((1, 3), dtype=torch.float64, device="cuda")
+                    walk = [pts[i:i + 1].contiguous() for i in range(len(pts))]
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    torch.cuda.synchronize()
+                    e0.record(stream)
+                    for p in walk:
+                        B.qmmm_field_eval(h, p, 1, 1, V, E, prec, stream)
+                    e1.record(stream)
+                    torch.cuda.synchronize()
+                    row["us_per_eval_1000_back_to_back"] = e0.elapsed_time(e1) * 1e3 / len(walk)
+                    # (ii) the QMC loop of PAPER.md:117: r_new in (24 B), U out (32 B), sync
+                    hp = torch.from_numpy(w.elec_xyz.reshape(-1, 3).copy()).pin_memory()
+                    ho = torch.zeros(4, dtype=torch.float64).pin_memory()
+                    t0 = time.perf_counter()
+                    for i in range(len(hp)):
+                        B.qmmm_field_eval_host(h, hp[i:i + 1], 1, 1, ho[:1], ho[1:].reshape(1, 3), prec, stream)
+                    row["us_per_eval_host_loop"] = (time.perf_counter() - t0) * 1e6 / len(hp)
+                    bytes_eval = w.M * (16 if prec == "fp32" else 32)
+                    row["source_bytes_per_eval"] = bytes_eval
+                    row["source_GBps_back_to_back"] = bytes_eval / (row["us_per_eval_1000_back_to_back"] * 1e-6) / 1e9
+                out.append(row)
+        finally:
+            B.qmmm_field_destroy(h)
+        del w
+    return out
+
+
+def run_ours(args):
+    import torch
+    rank, world, local = dist_env()
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_1011_4687_b200 import binding as B     # raises if the CUDA library is missing
+    from paper_1011_4687_b200.workloads import draw_points
+
+    w = make_workload(args.config)
+    prec = args.precision or w.precisions[0]
+    W, N = (1, 1) if w.sequential else (w.W, w.N)
+    P = W * N
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # the environment is replicated on every GPU; each rank evaluates its own walkers
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, P)
+    B.qmmm_field_set_timing(h, True)
+    n_batches = 4
+    host_batches = [draw_points(args.config, W, N, seed=1 + 97 * rank + b).reshape(-1, 3)
+                    for b in range(n_batches)]
+    batches = [torch.from_numpy(b).cuda() for b in host_batches]
+    flush = L2Flusher(torch)
+    peaks0 = probe_peaks(B)
+
+    # ---- device-resident timing -------------------------------------------------------
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    step_ms, pair_ms, _ = time_steps(torch, B, h, batches, W, N, prec, args.steps, args.warmup,
+                                     flush, stream)
+    barrier()
+    clocks = sampler.stop()
+    peaks1 = probe_peaks(B)
+    total_ms = torch.tensor([sum(step_ms)], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
+    total_ms = float(total_ms.item())
+    pairs_step_rank = P * (w.M + w.K)
+    value = world * pairs_step_rank * args.steps / (total_ms * 1e-3) / 1e9
+    info = B.qmmm_field_get_info(h)
+
+    # ---- end to end: host buffers through the C ABI -----------------------------------
+    B.qmmm_field_set_timing(h, False)
+    pin_in = [torch.from_numpy(b.copy()).pin_memory() for b in host_batches]
+    pin_out = torch.zeros(P * 4, dtype=torch.float64).pin_memory()
+    hV, hE = pin_out[:P], pin_out[P:].reshape(P, 3)
+    for i in range(args.warmup):
+        B.qmmm_field_eval_host(h, pin_in[i % n_batches], W, N, hV, hE, prec, stream)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        B.qmmm_field_eval_host(h, pin_in[i % n_batches], W, N, hV, hE, prec, stream)
+    barrier()
+    e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    e2e_value = world * pairs_step_rank * args.steps / float(e2e_s.item()) / 1e9
+
+    if rank == 0:
+        peak_key = "ffma_lane_ops_per_s" if prec == "fp32" else "dfma_lane_ops_per_s"
+        peak_lane = 0.5 * (peaks0[peak_key] + peaks1[peak_key])
+        pair_s = float(np.mean(pair_ms)) * 1e-3
+        achieved = P * w.M * SLOTS[prec] * 2 / pair_s / 1e12
+        peak_tf = 2 * peak_lane / 1e12
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "pair_kernel_traffic.json")
+        if os.path.exists(tpath):
+            traffic = json.load(open(tpath)).get(f"config{args.config}_{prec}")
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": DTYPE[prec], "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAME[args.config], "precision": prec, "M": w.M,
+                       "M_nominal": w.M_nominal, "K": w.K, "W": W, "N": N,
+                       "pairs_per_step_per_gpu": pairs_step_rank,
+                       "parallelism": f"walkers sharded x{world}, sources replicated, no collective",
+                       "l2": "flushed between timed steps (256 MB write)", "plan": info["last_plan"],
+                       "point_blocks": info["last_point_blocks"]},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": P * 24,
+                    "d2h_bytes_per_step": P * 32},
+            "gpu_launches": info["last_launches"] * args.steps,
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
+                         "frac": achieved / peak_tf, "traffic": traffic,
+                         "kernel": "pair_kernel", "kernel_ms": pair_s * 1e3,
+                         "slots_per_pair": SLOTS[prec],
+                         "definition": "pairs x slots x 2 / pair-kernel time vs 2 x FMA lane rate of "
+                                       "the same-run microbenchmark (qmmm_probe_peak)",
+                         "peak_source": "measured, same process (mean of before/after)",
+                         "peak_nominal_tflops": 148 * (128 if prec == "fp32" else 64) * 2 * 1.965e-3,
+                         "mufu_lane_ops_per_s": peaks1["mufu_lane_ops_per_s"],
+                         "probe_before": peaks0, "probe_after": peaks1},
+        }
+        if world == 1:
+            cb = oracle_sample_rate(w, args.cpu_sample_pairs)
+            line["cpu_baseline"] = {
+                "value": cb["rate"] / 1e9, "unit": UNIT, "cores": cb["threads"], "kind": "oracle",
+                "sample": f"{cb['n_points']} of {cb['n_total']} evaluation points x all "
+                          f"{w.M}+{w.K} sources ({cb['pairs']:.3g} pairs, {cb['seconds']:.1f} s)"}
+            line["paper_context"] = "GTX 275 vs one i7-920 core: 23.6x (SP), 11.0x (DP), whole run (PAPER.md:13)"
+            if not args.no_sweep:
+                B.qmmm_field_destroy(h)
+                h = None
+                del batches
+                line["configs"] = sweep_all_configs(torch, B, peaks1, args.config, line)
+        print(json.dumps(line), flush=True)
+    if h is not None:
+        B.qmmm_field_destroy(h)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

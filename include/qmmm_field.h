@@ -129,6 +129,16 @@ typedef struct {
 qmmm_status qmmm_field_get_info(const qmmm_field *h, qmmm_field_info *info);
 
 /*
+ * Per-kernel device timing for roofline measurements.  When enabled, eval records CUDA
+ * events on its stream before the pair kernel, between the two kernels and after the
+ * finalize kernel (a few microseconds of overhead; off by default).
+ * qmmm_field_last_timing waits for the most recent eval to finish and returns the two
+ * kernel durations in milliseconds.  INVALID_ARG if timing is off or no eval has run.
+ */
+qmmm_status qmmm_field_set_timing(qmmm_field *h, int enable);
+qmmm_status qmmm_field_last_timing(qmmm_field *h, double *pair_ms, double *finalize_ms);
+
+/*
  * qmmm_probe_peak -- same-run roofline denominators (north_star: "measured by a
  * microbenchmark in the same run").  Runs a register-only kernel of independent
  * dependent chains on every SM and reports the achieved rate.

@@ -24,6 +24,7 @@ _STATUS = {0: "QMMM_OK", 1: "QMMM_ERR_INVALID_ARG", 2: "QMMM_ERR_ALLOC", 3: "QMM
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libqmmm_field.so")
 EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_host",
                     "qmmm_field_destroy", "qmmm_field_set_plan", "qmmm_field_get_info",
+                    "qmmm_field_set_timing", "qmmm_field_last_timing",
                     "qmmm_probe_peak", "qmmm_last_error")
 
 
@@ -66,6 +67,11 @@ def _load() -> ctypes.CDLL:
     lib.qmmm_field_set_plan.argtypes = [vp, ctypes.POINTER(qmmm_plan)]
     lib.qmmm_field_get_info.restype = ci
     lib.qmmm_field_get_info.argtypes = [vp, ctypes.POINTER(qmmm_field_info)]
+    lib.qmmm_field_set_timing.restype = ci
+    lib.qmmm_field_set_timing.argtypes = [vp, ci]
+    lib.qmmm_field_last_timing.restype = ci
+    lib.qmmm_field_last_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_double),
+                                           ctypes.POINTER(ctypes.c_double)]
     lib.qmmm_probe_peak.restype = ci
     lib.qmmm_probe_peak.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double),
                                     ctypes.POINTER(ctypes.c_double), vp]
@@ -140,6 +146,17 @@ def qmmm_field_get_info(handle: int) -> dict:
     d = {k: getattr(info, k) for k, _ in info._fields_ if k not in ("last_plan", "reserved")}
     d["last_plan"] = {k: getattr(info.last_plan, k) for k, _ in qmmm_plan._fields_}
     return d
+
+
+def qmmm_field_set_timing(handle: int, enable: bool) -> None:
+    _check(_lib.qmmm_field_set_timing(handle, int(bool(enable))))
+
+
+def qmmm_field_last_timing(handle: int) -> Tuple[float, float]:
+    """(pair_kernel_ms, finalize_kernel_ms) of the most recent eval (waits for it)."""
+    a, b = ctypes.c_double(), ctypes.c_double()
+    _check(_lib.qmmm_field_last_timing(handle, ctypes.byref(a), ctypes.byref(b)))
+    return a.value, b.value
 
 
 def qmmm_probe_peak(kind: int, iters: int = 0, stream=None) -> Tuple[float, float]:

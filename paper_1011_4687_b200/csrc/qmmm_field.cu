@@ -71,6 +71,8 @@ struct qmmm_field {
     qmmm_plan user_plan = {0, 0, 0, 0};
     qmmm_plan last_plan = {0, 0, 0, 0};
     int last_point_blocks = 0, last_launches = 0;
+    bool timing = false, timed = false;
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
 };
 
 namespace {
@@ -255,6 +257,8 @@ qmmm_status qmmm_field_destroy(qmmm_field *h) {
     cudaFree(h->workspace);
     cudaFree(h->stage_elec);
     cudaFree(h->stage_out);
+    for (cudaEvent_t e : h->ev)
+        if (e) cudaEventDestroy(e);
     delete h;
     return QMMM_OK;
 }
@@ -271,6 +275,28 @@ qmmm_status qmmm_field_set_plan(qmmm_field *h, const qmmm_plan *plan) {
     if (plan->stages != 0 && (plan->stages < 2 || plan->stages > 8))
         return fail(QMMM_ERR_INVALID_ARG, "set_plan: stages must be 0 or 2..8");
     h->user_plan = *plan;
+    return QMMM_OK;
+}
+
+qmmm_status qmmm_field_set_timing(qmmm_field *h, int enable) {
+    if (!h) return fail(QMMM_ERR_INVALID_ARG, "set_timing: NULL handle");
+    if (enable && !h->ev[0])
+        for (cudaEvent_t &e : h->ev) CUDA_TRY(cudaEventCreate(&e));
+    h->timing = enable != 0;
+    h->timed = false;
+    return QMMM_OK;
+}
+
+qmmm_status qmmm_field_last_timing(qmmm_field *h, double *pair_ms, double *finalize_ms) {
+    if (!h || !pair_ms || !finalize_ms) return fail(QMMM_ERR_INVALID_ARG, "last_timing: NULL argument");
+    if (!h->timing || !h->timed)
+        return fail(QMMM_ERR_INVALID_ARG, "last_timing: timing is off or no eval has run");
+    CUDA_TRY(cudaEventSynchronize(h->ev[2]));
+    float a = 0.f, b = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&a, h->ev[0], h->ev[1]));
+    CUDA_TRY(cudaEventElapsedTime(&b, h->ev[1], h->ev[2]));
+    *pair_ms = a;
+    *finalize_ms = b;
     return QMMM_OK;
 }
 
@@ -309,6 +335,7 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
     if (smem > 227 * 1024) return fail(QMMM_ERR_INVALID_ARG, "eval: plan exceeds shared memory");
     if (pb > 65535) return fail(QMMM_ERR_INVALID_ARG, "eval: too many point blocks for this plan");
 
+    if (h->timing) CUDA_TRY(cudaEventRecord(h->ev[0], st));
     if (h->n_chunks > 0) {
         PairParams prm;
         prm.chunks = f32 ? reinterpret_cast<const char *>(h->chunks32)
@@ -327,6 +354,7 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
         if (e != cudaSuccess) return cuda_fail(e, "pair_kernel launch");
         ++launches;
     }
+    if (h->timing) CUDA_TRY(cudaEventRecord(h->ev[1], st));
     FinalizeParams fp;
     fp.partial = h->workspace;
     fp.nuc = h->nuclei;
@@ -342,6 +370,10 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "finalize_kernel launch");
     ++launches;
+    if (h->timing) {
+        CUDA_TRY(cudaEventRecord(h->ev[2], st));
+        h->timed = true;
+    }
 
     h->last_plan = pl;
     h->last_point_blocks = pb;

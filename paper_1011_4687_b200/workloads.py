@@ -31,7 +31,7 @@ from typing import Optional, Tuple
 
 import numpy as np
 
-__all__ = ["Workload", "make_workload", "CONFIG_SPECS", "subsample_points"]
+__all__ = ["Workload", "make_workload", "CONFIG_SPECS", "subsample_points", "draw_points"]
 
 
 @dataclass
@@ -236,3 +236,16 @@ def subsample_points(P: int, fraction: float, seed: int) -> np.ndarray:
     rng = np.random.default_rng(seed)
     n = max(1, int(round(P * fraction)))
     return np.sort(rng.choice(P, size=n, replace=False))
+
+
+def draw_points(index: int, W: int, N: int, seed: int) -> np.ndarray:
+    """Another seeded batch of evaluation points [W][N][3] with configuration ``index``'s
+    distribution (bench.py: a different batch per step / per rank; the environment is not
+    redrawn)."""
+    spec = CONFIG_SPECS[index]
+    rng = np.random.default_rng([seed, index, 0x9E3779B9])
+    if spec.get("sequential"):
+        pts = _random_walk(rng, W * N, spec["walk_sigma"], spec["r_clip"])
+    else:
+        pts = _clipped_gaussian(rng, W * N, spec["sigma"], spec["r_clip"])
+    return np.ascontiguousarray(pts.reshape(W, N, 3))
