@@ -49,6 +49,10 @@ constexpr size_t stage_bytes(bool f32) {
     return STAGE_HDR + static_cast<size_t>(BLOCK_CHUNKS) * 4 * CHUNK * (f32 ? 4 : 8);
 }
 size_t pair_smem_bytes(bool f32, int stages, int ept, int wp) {
+    if (f32 && ept >= 2)      // pair_kernel_f32x2: electrons for 8 point warps + FP64 columns
+        return stages * stage_bytes(true) + 16 * sizeof(uint64_t) +
+               static_cast<size_t>(COMPUTE_WARPS) * ept * 3 * sizeof(double) +
+               static_cast<size_t>(ept) * 4 * 32 * COMPUTE_WARPS * sizeof(double);
     return stages * stage_bytes(f32) + 16 * sizeof(uint64_t) +
            static_cast<size_t>(COMPUTE_WARPS) * ept * 4 * sizeof(double) +
            static_cast<size_t>(wp) * ept * 3 * sizeof(double);
@@ -116,9 +120,30 @@ cudaError_t launch_pair(const PairParams &prm, dim3 grid, size_t smem, cudaStrea
     return cudaGetLastError();
 }
 
+template <int EP2>
+cudaError_t launch_pair_f32x2(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
+    auto kern = pair_kernel_f32x2<EP2>;
+    static thread_local size_t configured = 0;
+    if (smem > configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             static_cast<int>(smem));
+        if (e != cudaSuccess) return e;
+        configured = smem;
+    }
+    kern<<<grid, F32X2_THREADS, smem, st>>>(prm);
+    return cudaGetLastError();
+}
+
 template <typename REAL>
 cudaError_t launch_pair_ept(int ept, const PairParams &prm, dim3 grid, size_t smem,
                             cudaStream_t st) {
+    if constexpr (sizeof(REAL) == 4) {
+        switch (ept) {
+            case 2: return launch_pair_f32x2<1>(prm, grid, smem, st);
+            case 4: return launch_pair_f32x2<2>(prm, grid, smem, st);
+            case 8: return launch_pair_f32x2<4>(prm, grid, smem, st);
+        }
+    }
     switch (ept) {
         case 1: return launch_pair<REAL, 1>(prm, grid, smem, st);
         case 2: return launch_pair<REAL, 2>(prm, grid, smem, st);

@@ -338,6 +338,197 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
     }
 }
 
+// ----------------------------------------------------------------------------- FP32 packed
+// FP32-acc64 pair kernel for EPT >= 2: two evaluation points share one f32x2 register pair
+// (sm_100 FADD2 / FMUL2 / FFMA2; the source scalar is a broadcast operand), so the 17
+// FP32-pipe operations of a pair cost 8.5 issue slots and the issue port is no longer the
+// limiter.  The per-thread FP64 running sums live in shared memory (one conflict-free
+// column per thread) instead of 8*EPT registers, which leaves the register file to the
+// interleaved FP32 chains: ptxas serialises the pairs when the doubles stay in registers.
+__device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ float2 bc(float a) { return make_float2(a, a); }   // broadcast operand
+
+// One 128-source chunk: the lane's 4 sources x EP2 point pairs, written stage by stage so
+// that EP2 independent chains are in flight around every MUFU.
+template <int EP2>
+__device__ __forceinline__ void chunk_f32x2(const float *b, const float2 (&rx)[EP2],
+                                            const float2 (&ry)[EP2], const float2 (&rz)[EP2],
+                                            float2 (&V)[EP2], float2 (&Ex)[EP2],
+                                            float2 (&Ey)[EP2], float2 (&Ez)[EP2]) {
+    const float4 X = *reinterpret_cast<const float4 *>(b);
+    const float4 Y = *reinterpret_cast<const float4 *>(b + CHUNK);
+    const float4 Z = *reinterpret_cast<const float4 *>(b + 2 * CHUNK);
+    const float4 Q = *reinterpret_cast<const float4 *>(b + 3 * CHUNK);
+    const float xs[4] = {X.x, X.y, X.z, X.w}, ys[4] = {Y.x, Y.y, Y.z, Y.w};
+    const float zs[4] = {Z.x, Z.y, Z.z, Z.w}, qs[4] = {Q.x, Q.y, Q.z, Q.w};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        float2 dx[EP2], dy[EP2], dz[EP2], r2[EP2], y0[EP2];
+        const float2 nx = bc(-xs[k]), ny = bc(-ys[k]), nz = bc(-zs[k]), qq = bc(qs[k]);
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+            dx[e] = __fadd2_rn(rx[e], nx);
+            dy[e] = __fadd2_rn(ry[e], ny);
+            dz[e] = __fadd2_rn(rz[e], nz);
+            r2[e] = __ffma2_rn(dz[e], dz[e], __ffma2_rn(dy[e], dy[e], __fmul2_rn(dx[e], dx[e])));
+        }
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+            y0[e].x = rsqrt_mufu_f32(r2[e].x);
+            y0[e].y = rsqrt_mufu_f32(r2[e].y);
+        }
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {       // one Newton step, then V and E (17 FP32 ops/pair)
+            const float2 t = __fmul2_rn(r2[e], y0[e]);
+            const float2 err = __ffma2_rn(f2(-t.x, -t.y), y0[e], bc(1.0f));
+            const float2 h = __fmul2_rn(y0[e], bc(0.5f));
+            const float2 y = __ffma2_rn(h, err, y0[e]);
+            const float2 p = __fmul2_rn(y, qq);
+            V[e] = __fadd2_rn(V[e], p);
+            const float2 s = __fmul2_rn(p, __fmul2_rn(y, y));
+            Ex[e] = __ffma2_rn(s, dx[e], Ex[e]);
+            Ey[e] = __ffma2_rn(s, dy[e], Ey[e]);
+            Ez[e] = __ffma2_rn(s, dz[e], Ez[e]);
+        }
+    }
+}
+
+// grid = (slices, point_blocks); EPT = 2 * EP2 points per thread; 8 warps, no producer warp:
+// a 9th warp would put 3 warps on one SM sub-partition and cap every thread at 168
+// registers.  Warp 0 drives the TMA pipeline inline, one stage ahead of its own consumption.
+constexpr int F32X2_THREADS = 32 * COMPUTE_WARPS;
+
+template <int EP2>
+__global__ void __launch_bounds__(F32X2_THREADS, 1) pair_kernel_f32x2(const PairParams prm) {
+    constexpr int EPT = 2 * EP2;
+    constexpr int CHUNK_BYTES = 4 * CHUNK * sizeof(float);
+    constexpr int STAGE_BYTES = STAGE_HDR + BLOCK_CHUNKS * CHUNK_BYTES;
+    constexpr int NT = F32X2_THREADS;
+
+    extern __shared__ __align__(128) unsigned char smem[];
+    // layout: [stages x STAGE_BYTES] [full barriers] [empty barriers] [elec] [acc columns]
+    const int stages = prm.stages;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + static_cast<size_t>(stages) * STAGE_BYTES);
+    uint64_t *empty = full + 8;
+    double *elec_s = reinterpret_cast<double *>(empty + 8);   // [WP*EPT][3], WP <= 8
+    double *acc = elec_s + COMPUTE_WARPS * EPT * 3;            // [EPT*4][NT]
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int WP = prm.point_warps, WS = COMPUTE_WARPS / WP;
+    int lo, hi;
+    slice_range(prm.n_chunks, prm.slices, blockIdx.x, lo, hi);
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < stages; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], COMPUTE_WARPS);
+        }
+        fence_barrier_init();
+    }
+    const int ppb = WP * EPT;
+    for (int i = threadIdx.x; i < ppb * 3; i += NT) {
+        int p = blockIdx.y * ppb + i / 3;
+        p = p < prm.P ? p : prm.P - 1;
+        elec_s[i] = prm.elec[static_cast<int64_t>(p) * 3 + (i % 3)];
+    }
+    __syncthreads();
+
+    // producer cursor (used by warp 0 only): next pipeline step to load
+    int pc = lo, pk = 0;
+    auto produce = [&]() {
+        if (pc >= hi) return;
+        const int ce = stage_end(pc, hi);
+        const int slot = pk % stages;
+        if (pk >= stages) mbar_wait(&empty[slot], ((pk / stages) - 1) & 1);
+        if (lane == 0) {
+            unsigned char *dst = smem + static_cast<size_t>(slot) * STAGE_BYTES;
+            const uint32_t bytes = static_cast<uint32_t>(ce - pc) * CHUNK_BYTES;
+            mbar_expect_tx(&full[slot], bytes + 32);
+            tma_bulk_g2s(dst, prm.origins + 4 * (pc / BLOCK_CHUNKS), 32, &full[slot]);
+            tma_bulk_g2s(dst + STAGE_HDR, prm.chunks + static_cast<size_t>(pc) * CHUNK_BYTES, bytes,
+                         &full[slot]);
+        }
+        pc = ce;
+        ++pk;
+    };
+    if (warp == 0)
+        for (int i = 0; i < stages - 1; ++i) produce();
+
+    const int wp = warp % WP, ws = warp / WP;
+    double *my = acc + threadIdx.x;                 // column of this thread: my[i * NT]
+#pragma unroll
+    for (int i = 0; i < EPT * 4; ++i) my[i * NT] = 0.0;
+    const double *pe = elec_s + wp * EPT * 3;
+
+    int c = lo, k = 0;
+    while (c < hi) {
+        const int ce = stage_end(c, hi);
+        const int slot = k % stages;
+        if (warp == 0) produce();          // step k + stages - 1 into the slot freed by step k - 1
+        mbar_wait(&full[slot], (k / stages) & 1);
+        const unsigned char *st = smem + static_cast<size_t>(slot) * STAGE_BYTES;
+        const float *data = reinterpret_cast<const float *>(st + STAGE_HDR);
+        const int nch = ce - c;
+        // tile-local coordinates a = r_i - c_block, formed in FP64 and rounded once
+        const double *org = reinterpret_cast<const double *>(st);
+        const double cx = org[0], cy = org[1], cz = org[2];
+        float2 rx[EP2], ry[EP2], rz[EP2], v[EP2], ex[EP2], ey[EP2], ez[EP2];
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+            rx[e] = f2(static_cast<float>(pe[6 * e + 0] - cx), static_cast<float>(pe[6 * e + 3] - cx));
+            ry[e] = f2(static_cast<float>(pe[6 * e + 1] - cy), static_cast<float>(pe[6 * e + 4] - cy));
+            rz[e] = f2(static_cast<float>(pe[6 * e + 2] - cz), static_cast<float>(pe[6 * e + 5] - cz));
+            v[e] = ex[e] = ey[e] = ez[e] = f2(0.0f, 0.0f);
+        }
+        for (int ch = ws; ch < nch; ch += WS)
+            chunk_f32x2<EP2>(data + ch * 4 * CHUNK + 4 * lane, rx, ry, rz, v, ex, ey, ez);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[slot]);   // the stage's source data is consumed
+        // flush the FP32 run into the FP64 column; the rounding residual delta of a enters as
+        // the first-order correction V(a_hat + delta) = V(a_hat) - E(a_hat) . delta
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+#pragma unroll
+            for (int hlf = 0; hlf < 2; ++hlf) {
+                const int pi = 2 * e + hlf;
+                const float ax = hlf ? rx[e].y : rx[e].x, ay = hlf ? ry[e].y : ry[e].x;
+                const float az = hlf ? rz[e].y : rz[e].x;
+                const float fx = hlf ? ex[e].y : ex[e].x, fy = hlf ? ey[e].y : ey[e].x;
+                const float fz = hlf ? ez[e].y : ez[e].x, fv = hlf ? v[e].y : v[e].x;
+                const float ddx = static_cast<float>((pe[3 * pi + 0] - cx) - static_cast<double>(ax));
+                const float ddy = static_cast<float>((pe[3 * pi + 1] - cy) - static_cast<double>(ay));
+                const float ddz = static_cast<float>((pe[3 * pi + 2] - cz) - static_cast<double>(az));
+                const float corr = fmaf(fz, ddz, fmaf(fy, ddy, fx * ddx));
+                my[(4 * pi + 0) * NT] += static_cast<double>(fv) - static_cast<double>(corr);
+                my[(4 * pi + 1) * NT] += static_cast<double>(fx);
+                my[(4 * pi + 2) * NT] += static_cast<double>(fy);
+                my[(4 * pi + 3) * NT] += static_cast<double>(fz);
+            }
+        }
+        c = ce;
+        ++k;
+    }
+
+    // ---- in-CTA reduction: fixed-order butterfly per value, then the WS partners in order ----
+    double *red = acc;      // reuse: after the barrier, [COMPUTE_WARPS][EPT*4] at the front
+    double mine = 0.0;
+#pragma unroll
+    for (int i = 0; i < EPT * 4; ++i) {
+        const double t = warp_sum(my[i * NT]);
+        if (lane == i) mine = t;
+    }
+    __syncthreads();                                 // every column has been read
+    if (lane < EPT * 4) red[warp * EPT * 4 + lane] = mine;
+    __syncthreads();
+    if (ws == 0 && lane < EPT * 4) {
+        double a = 0.0;
+        for (int s = 0; s < WS; ++s) a += red[(s * WP + wp) * EPT * 4 + lane];
+        const int p = (blockIdx.y * WP + wp) * EPT + lane / 4;
+        if (p < prm.P)
+            prm.partial[(static_cast<int64_t>(blockIdx.x) * prm.P + p) * 4 + (lane & 3)] = a;
+    }
+}
+
 // ----------------------------------------------------------------------------- finalize
 // Adds the slice partials in index order, then the nuclear term (always FP64, PAPER.md:117
 // keeps U_nuc in double), and writes V, E.  TPP threads cooperate on one point.
