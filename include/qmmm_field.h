@@ -106,9 +106,9 @@ qmmm_status qmmm_field_destroy(qmmm_field *h);
  * 0 in a field of qmmm_field_set_plan means "choose automatically". */
 typedef struct {
     int32_t points_per_thread;   /* register blocking: 1, 2, 4 or 8 electrons per thread */
-    int32_t point_warps;         /* warps of a CTA that own different point groups: 1,2,4,8 */
+    int32_t point_warps;         /* warps of a CTA that own different point groups: 1..16 (clamped) */
     int32_t slices;              /* N_B: CTAs the source sum is split over (per point block) */
-    int32_t stages;              /* TMA pipeline depth (shared-memory stages), 2..8 */
+    int32_t stages;              /* TMA pipeline depth (shared-memory stages), 2..8; reduced if it does not fit */
 } qmmm_plan;
 
 /* Override the automatic plan (testing partition independence, tuning).  Sticky

@@ -21,7 +21,10 @@ _PREC = {"fp64": QMMM_FP64, "fp32": QMMM_FP32_ACC64, QMMM_FP64: QMMM_FP64,
 _STATUS = {0: "QMMM_OK", 1: "QMMM_ERR_INVALID_ARG", 2: "QMMM_ERR_ALLOC", 3: "QMMM_ERR_CUDA",
            4: "QMMM_ERR_UNSUPPORTED_DEVICE"}
 
-LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libqmmm_field.so")
+# QMMM_FIELD_LIB selects another build of the same library (a tuning variant made with
+# build.build(defines=..., out=...)); the default is the in-tree build.
+LIB_PATH = os.environ.get("QMMM_FIELD_LIB") or os.path.join(
+    os.path.dirname(os.path.abspath(__file__)), "libqmmm_field.so")
 EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_host",
                     "qmmm_field_destroy", "qmmm_field_set_plan", "qmmm_field_get_info",
                     "qmmm_field_set_timing", "qmmm_field_last_timing",

@@ -9,6 +9,7 @@
 #include "qmmm_kernels.cuh"
 
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -46,13 +47,16 @@ int gcd_int(int a, int b) {
 }
 
 constexpr size_t stage_bytes(bool f32) {
-    return STAGE_HDR + static_cast<size_t>(BLOCK_CHUNKS) * 4 * CHUNK * (f32 ? 4 : 8);
+    return STAGE_HDR + (f32 ? static_cast<size_t>(BLOCK_CHUNKS) * 4 * CHUNK * 4
+                            : static_cast<size_t>(STAGE_CHUNKS_F64) * 4 * CHUNK * 8);
 }
+// FP32 packed kernel variants: (points per thread, consumer warps)
+constexpr int F32X2_NW_EPT8 = 8, F32X2_NW_EPT4 = 16, F32X2_NW_EPT2 = 16;
+int f32x2_warps(int ept) { return ept == 8 ? F32X2_NW_EPT8 : (ept == 4 ? F32X2_NW_EPT4 : F32X2_NW_EPT2); }
 size_t pair_smem_bytes(bool f32, int stages, int ept, int wp) {
-    if (f32 && ept >= 2)      // pair_kernel_f32x2: electrons for 8 point warps + FP64 columns
-        return stages * stage_bytes(true) + 16 * sizeof(uint64_t) +
-               static_cast<size_t>(COMPUTE_WARPS) * ept * 3 * sizeof(double) +
-               static_cast<size_t>(ept) * 4 * 32 * COMPUTE_WARPS * sizeof(double);
+    if (f32 && ept == 8) return F32x2Layout<4, F32X2_NW_EPT8>::total(stages);
+    if (f32 && ept == 4) return F32x2Layout<2, F32X2_NW_EPT4>::total(stages);
+    if (f32 && ept == 2) return F32x2Layout<1, F32X2_NW_EPT2>::total(stages);
     return stages * stage_bytes(f32) + 16 * sizeof(uint64_t) +
            static_cast<size_t>(COMPUTE_WARPS) * ept * 4 * sizeof(double) +
            static_cast<size_t>(wp) * ept * 3 * sizeof(double);
@@ -67,6 +71,7 @@ struct qmmm_field {
     double *chunks64 = nullptr;    // [n_chunks][4][128] double
     float *chunks32 = nullptr;     // [n_chunks][4][128] float (offsets from block origin, q)
     double *origins = nullptr;     // [n_blocks][4]
+    double lattice = 1.0;          // FP32 coordinate quantum (power of two)
     double *nuclei = nullptr;      // [K][4]
     double *workspace = nullptr;   // partials [slices][P][4]
     int64_t workspace_doubles = 0;
@@ -75,6 +80,7 @@ struct qmmm_field {
     qmmm_plan user_plan = {0, 0, 0, 0};
     qmmm_plan last_plan = {0, 0, 0, 0};
     int last_point_blocks = 0, last_launches = 0;
+    double *workspace_bbox() const { return chunks64; }   // scratch before packing (>= 512 doubles)
     bool timing = false, timed = false;
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
 };
@@ -88,8 +94,9 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32) {
     const int max_ept = f32 ? 8 : 4;
     if (pl.points_per_thread == 0) pl.points_per_thread = std::min(max_ept, pow2_ceil(P));
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
-    if (pl.point_warps == 0)
-        pl.point_warps = std::min<int>(COMPUTE_WARPS, pow2_ceil(groups));
+    const int nw = (f32 && pl.points_per_thread >= 2) ? f32x2_warps(pl.points_per_thread) : COMPUTE_WARPS;
+    if (pl.point_warps == 0) pl.point_warps = std::min<int>(nw, pow2_ceil(groups));
+    if (pl.point_warps > nw) pl.point_warps = nw;
     const int64_t pb = (groups + pl.point_warps - 1) / pl.point_warps;
     if (pl.slices == 0) {
         const int g = gcd_int(static_cast<int>(pb % h->sm_count), h->sm_count);
@@ -101,7 +108,7 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32) {
     if (pl.slices > cap) pl.slices = static_cast<int>(std::max<int64_t>(1, cap));
     if (pl.stages == 0) {
         const bool bandwidth_bound = groups <= 2;
-        pl.stages = f32 ? (bandwidth_bound ? 8 : 4) : (bandwidth_bound ? 6 : 3);
+        pl.stages = f32 ? (pl.points_per_thread == 1 ? 6 : 4) : (bandwidth_bound ? 6 : 3);
     }
     return pl;
 }
@@ -120,9 +127,9 @@ cudaError_t launch_pair(const PairParams &prm, dim3 grid, size_t smem, cudaStrea
     return cudaGetLastError();
 }
 
-template <int EP2>
+template <int EP2, int NW>
 cudaError_t launch_pair_f32x2(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
-    auto kern = pair_kernel_f32x2<EP2>;
+    auto kern = pair_kernel_f32x2<EP2, NW>;
     static thread_local size_t configured = 0;
     if (smem > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -130,7 +137,7 @@ cudaError_t launch_pair_f32x2(const PairParams &prm, dim3 grid, size_t smem, cud
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    kern<<<grid, F32X2_THREADS, smem, st>>>(prm);
+    kern<<<grid, 32 * NW, smem, st>>>(prm);
     return cudaGetLastError();
 }
 
@@ -139,9 +146,9 @@ cudaError_t launch_pair_ept(int ept, const PairParams &prm, dim3 grid, size_t sm
                             cudaStream_t st) {
     if constexpr (sizeof(REAL) == 4) {
         switch (ept) {
-            case 2: return launch_pair_f32x2<1>(prm, grid, smem, st);
-            case 4: return launch_pair_f32x2<2>(prm, grid, smem, st);
-            case 8: return launch_pair_f32x2<4>(prm, grid, smem, st);
+            case 2: return launch_pair_f32x2<1, F32X2_NW_EPT2>(prm, grid, smem, st);
+            case 4: return launch_pair_f32x2<2, F32X2_NW_EPT4>(prm, grid, smem, st);
+            case 8: return launch_pair_f32x2<4, F32X2_NW_EPT8>(prm, grid, smem, st);
         }
     }
     switch (ept) {
@@ -233,12 +240,34 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
         if (e == cudaSuccess) e = cudaMalloc(&h->chunks32, Mpad * 4 * sizeof(float));
         if (e == cudaSuccess) e = cudaMalloc(&h->origins, h->n_blocks * 4 * sizeof(double));
         if (e == cudaSuccess) {
+            // coordinate lattice of the FP32 copy: the largest extent of the bounding box fits
+            // in 2^24 quanta, so d = a - o is exact for every point inside the box
+            const int nbb = static_cast<int>(std::min<int64_t>(256, (M + 255) / 256));
+            double hbb[256 * 6];
+            bbox_kernel<<<nbb, 256>>>(dxyz, M, h->workspace_bbox());
+            e = cudaMemcpy(hbb, h->workspace_bbox(), nbb * 6 * sizeof(double), cudaMemcpyDeviceToHost);
+            double ext = 0.0;
+            for (int k = 0; k < 3 && e == cudaSuccess; ++k) {
+                double lo = hbb[k], hi = hbb[3 + k];
+                for (int b = 1; b < nbb; ++b) {
+                    lo = std::min(lo, hbb[6 * b + k]);
+                    hi = std::max(hi, hbb[6 * b + 3 + k]);
+                }
+                ext = std::max(ext, hi - lo);
+            }
+            if (!(ext > 0.0) || !std::isfinite(ext)) ext = 1.0;
+            int ex2 = 0;
+            std::frexp(ext, &ex2);                       // ext = m * 2^ex2, 0.5 <= m < 1
+            h->lattice = std::ldexp(1.0, ex2 - 24);
+        }
+        if (e == cudaSuccess) {
             const int T = 256;
             const unsigned nb = static_cast<unsigned>((Mpad + T - 1) / T);
             pack_f64_kernel<<<nb, T>>>(dxyz, dq, M, Mpad, h->chunks64);
             origins_kernel<<<static_cast<unsigned>((h->n_blocks * 32 + T - 1) / T), T>>>(
-                dxyz, M, h->n_blocks, h->origins);
-            pack_f32_kernel<<<nb, T>>>(dxyz, dq, M, Mpad, h->origins, h->chunks32);
+                dxyz, M, h->n_blocks, h->lattice, h->origins);
+            pack_f32_kernel<<<static_cast<unsigned>((h->n_chunks + 63) / 64), 64>>>(
+                dxyz, dq, M, h->n_chunks, h->origins, h->lattice, h->chunks32);
             e = cudaGetLastError();
             if (e == cudaSuccess) e = cudaDeviceSynchronize();
         }
@@ -293,8 +322,8 @@ qmmm_status qmmm_field_set_plan(qmmm_field *h, const qmmm_plan *plan) {
     const int e = plan->points_per_thread, w = plan->point_warps;
     if (!(e == 0 || e == 1 || e == 2 || e == 4 || e == 8))
         return fail(QMMM_ERR_INVALID_ARG, "set_plan: points_per_thread must be 0,1,2,4,8");
-    if (!(w == 0 || w == 1 || w == 2 || w == 4 || w == 8))
-        return fail(QMMM_ERR_INVALID_ARG, "set_plan: point_warps must be 0,1,2,4,8");
+    if (!(w == 0 || w == 1 || w == 2 || w == 4 || w == 8 || w == 16))
+        return fail(QMMM_ERR_INVALID_ARG, "set_plan: point_warps must be 0,1,2,4,8,16");
     if (plan->slices < 0 || plan->slices > 65535)
         return fail(QMMM_ERR_INVALID_ARG, "set_plan: slices out of range");
     if (plan->stages != 0 && (plan->stages < 2 || plan->stages > 8))
@@ -356,7 +385,9 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
     const int pb = static_cast<int>((groups + pl.point_warps - 1) / pl.point_warps);
     int launches = 0;
-    const size_t smem = pair_smem_bytes(f32, pl.stages, pl.points_per_thread, pl.point_warps);
+    size_t smem = pair_smem_bytes(f32, pl.stages, pl.points_per_thread, pl.point_warps);
+    while (smem > 227 * 1024 && pl.stages > 2)           // a requested depth that does not fit is reduced
+        smem = pair_smem_bytes(f32, --pl.stages, pl.points_per_thread, pl.point_warps);
     if (smem > 227 * 1024) return fail(QMMM_ERR_INVALID_ARG, "eval: plan exceeds shared memory");
     if (pb > 65535) return fail(QMMM_ERR_INVALID_ARG, "eval: too many point blocks for this plan");
 
@@ -373,6 +404,8 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
         prm.slices = pl.slices;
         prm.point_warps = pl.point_warps;
         prm.stages = pl.stages;
+        prm.lattice = h->lattice;
+        prm.inv_lattice = 1.0 / h->lattice;
         const dim3 grid(pl.slices, pb);
         cudaError_t e = f32 ? launch_pair_ept<float>(pl.points_per_thread, prm, grid, smem, st)
                             : launch_pair_ept<double>(pl.points_per_thread, prm, grid, smem, st);

@@ -20,7 +20,11 @@
 namespace qmmm {
 
 constexpr int CHUNK = 128;          // sources per SoA chunk (4 per lane)
-constexpr int BLOCK_CHUNKS = 8;     // chunks per origin block (FP32 tile-local coordinates)
+#ifndef QMMM_BLOCK_CHUNKS
+#define QMMM_BLOCK_CHUNKS 16
+#endif
+constexpr int BLOCK_CHUNKS = QMMM_BLOCK_CHUNKS;    // chunks per origin block (FP32 tile-local coordinates) = FP32 stage
+constexpr int STAGE_CHUNKS_F64 = 8; // chunks per FP64 pipeline stage
 constexpr int COMPUTE_WARPS = 8;    // consumer warps per CTA; +1 producer warp
 constexpr int CTA_THREADS = 32 * (COMPUTE_WARPS + 1);
 constexpr int STAGE_HDR = 128;      // bytes reserved per stage for the block origin
@@ -35,6 +39,8 @@ struct PairParams {
     int slices;
     int point_warps;         // WP; source-split warps WS = COMPUTE_WARPS / WP
     int stages;
+    double lattice;          // FP32 only: coordinate quantum (power of two), and its inverse
+    double inv_lattice;
 };
 
 // ----------------------------------------------------------------------------- PTX helpers
@@ -91,6 +97,15 @@ __device__ __forceinline__ double rsqrt_mufu_f64(double x) {        // MUFU.RSQ6
     return y;
 }
 
+// Tile-local coordinate of an evaluation point on the handle's coordinate lattice: the FP32
+// offsets of the sources are multiples of the same power-of-two quantum, so the FP32
+// subtraction d = a - o is EXACT (no rounding) whenever |d| < 2^24 quanta, i.e. for every
+// point inside the environment's bounding box.  Plain FP32 rounding of d is coherent over
+// a regular grid and biases V by ~2e-8 hartree per point.
+__device__ __forceinline__ float lattice_round(double a64, double lattice, double inv_lattice) {
+    return static_cast<float>(rint(a64 * inv_lattice) * lattice);
+}
+
 // ----------------------------------------------------------------------------- pair math
 // FP64 reciprocal square root: hardware seed (about 20+ bits) + ONE cubically convergent
 // refinement  y <- y (1 + e/2 + 3 e^2/8),  e = 1 - x y^2  (relative error 2.5 eps0^3).
@@ -143,8 +158,9 @@ __device__ __host__ __forceinline__ void slice_range(int n_chunks, int S, int s,
     hi = static_cast<int>((static_cast<int64_t>(n_chunks) * (s + 1)) / S);
 }
 // A pipeline stage never straddles an origin block: [c, min(hi, next block boundary)).
+template <int BC = BLOCK_CHUNKS>
 __device__ __forceinline__ int stage_end(int c, int hi) {
-    int e = (c / BLOCK_CHUNKS + 1) * BLOCK_CHUNKS;
+    int e = (c / BC + 1) * BC;
     return e < hi ? e : hi;
 }
 
@@ -161,7 +177,8 @@ template <typename REAL, int EPT>
 __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams prm) {
     constexpr bool F32 = sizeof(REAL) == 4;
     constexpr int CHUNK_BYTES = 4 * CHUNK * sizeof(REAL);
-    constexpr int STAGE_BYTES = STAGE_HDR + BLOCK_CHUNKS * CHUNK_BYTES;
+    constexpr int SC = F32 ? BLOCK_CHUNKS : STAGE_CHUNKS_F64;     // chunks per stage
+    constexpr int STAGE_BYTES = STAGE_HDR + SC * CHUNK_BYTES;
 
     extern __shared__ __align__(128) unsigned char smem[];
     // layout: [stages x STAGE_BYTES] [full barriers] [empty barriers] [reduction scratch]
@@ -197,14 +214,14 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
         if (lane == 0) {
             int c = lo, k = 0;
             while (c < hi) {
-                const int ce = stage_end(c, hi);
+                const int ce = stage_end<SC>(c, hi);
                 const int slot = k % stages;
                 if (k >= stages) mbar_wait(&empty[slot], ((k / stages) - 1) & 1);
                 unsigned char *dst = smem + static_cast<size_t>(slot) * STAGE_BYTES;
                 const uint32_t bytes = static_cast<uint32_t>(ce - c) * CHUNK_BYTES;
                 if constexpr (F32) {
                     mbar_expect_tx(&full[slot], bytes + 32);
-                    tma_bulk_g2s(dst, prm.origins + 4 * (c / BLOCK_CHUNKS), 32, &full[slot]);
+                    tma_bulk_g2s(dst, prm.origins + 4 * (c / SC), 32, &full[slot]);
                 } else {
                     mbar_expect_tx(&full[slot], bytes);
                 }
@@ -235,7 +252,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
 
     int c = lo, k = 0;
     while (c < hi) {
-        const int ce = stage_end(c, hi);
+        const int ce = stage_end<SC>(c, hi);
         const int slot = k % stages;
         mbar_wait(&full[slot], (k / stages) & 1);
         const unsigned char *st = smem + static_cast<size_t>(slot) * STAGE_BYTES;
@@ -255,9 +272,9 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
                 const double a0 = elec_s[(wp * EPT + e) * 3 + 0] - cx;
                 const double a1 = elec_s[(wp * EPT + e) * 3 + 1] - cy;
                 const double a2 = elec_s[(wp * EPT + e) * 3 + 2] - cz;
-                rx[e] = static_cast<REAL>(a0);
-                ry[e] = static_cast<REAL>(a1);
-                rz[e] = static_cast<REAL>(a2);
+                rx[e] = lattice_round(a0, prm.lattice, prm.inv_lattice);
+                ry[e] = lattice_round(a1, prm.lattice, prm.inv_lattice);
+                rz[e] = lattice_round(a2, prm.lattice, prm.inv_lattice);
                 ddx[e] = static_cast<float>(a0 - static_cast<double>(rx[e]));
                 ddy[e] = static_cast<float>(a1 - static_cast<double>(ry[e]));
                 ddz[e] = static_cast<float>(a2 - static_cast<double>(rz[e]));
@@ -361,6 +378,10 @@ __device__ __forceinline__ void chunk_f32x2(const float *b, const float2 (&rx)[E
     const float4 Q = *reinterpret_cast<const float4 *>(b + 3 * CHUNK);
     const float xs[4] = {X.x, X.y, X.z, X.w}, ys[4] = {Y.x, Y.y, Y.z, Y.w};
     const float zs[4] = {Z.x, Z.y, Z.z, Z.w}, qs[4] = {Q.x, Q.y, Q.z, Q.w};
+    // V is summed as a tree of short FP32 runs (4 sources -> 4 chunks -> stage): a long FP32
+    // running sum of slowly varying same-sign terms drifts systematically (DESIGN.md "FP32
+    // path": +8e-8 hartree per point at 64 terms), a 4-term run does not.
+    float2 Vc[EP2];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         float2 dx[EP2], dy[EP2], dz[EP2], r2[EP2], y0[EP2];
@@ -384,138 +405,196 @@ __device__ __forceinline__ void chunk_f32x2(const float *b, const float2 (&rx)[E
             const float2 h = __fmul2_rn(y0[e], bc(0.5f));
             const float2 y = __ffma2_rn(h, err, y0[e]);
             const float2 p = __fmul2_rn(y, qq);
-            V[e] = __fadd2_rn(V[e], p);
+            Vc[e] = k == 0 ? p : __fadd2_rn(Vc[e], p);
             const float2 s = __fmul2_rn(p, __fmul2_rn(y, y));
             Ex[e] = __ffma2_rn(s, dx[e], Ex[e]);
             Ey[e] = __ffma2_rn(s, dy[e], Ey[e]);
             Ez[e] = __ffma2_rn(s, dz[e], Ez[e]);
         }
     }
+#pragma unroll
+    for (int e = 0; e < EP2; ++e) V[e] = __fadd2_rn(V[e], Vc[e]);
 }
 
-// grid = (slices, point_blocks); EPT = 2 * EP2 points per thread; 8 warps, no producer warp:
-// a 9th warp would put 3 warps on one SM sub-partition and cap every thread at 168
-// registers.  Warp 0 drives the TMA pipeline inline, one stage ahead of its own consumption.
-constexpr int F32X2_THREADS = 32 * COMPUTE_WARPS;
+// grid = (slices, point_blocks); EPT = 2 * EP2 points per thread; NW consumer warps and no
+// producer warp: a 9th warp would put 3 warps on one SM sub-partition and cap every thread
+// at 168 registers.  Warp 0 drives the TMA pipeline inline, stages-1 steps ahead.
+//   NW = 8,  EP2 = 4 : 2 warps per sub-partition, 8 points per thread (<= 255 registers)
+//   NW = 16, EP2 = 2 : 4 warps per sub-partition, 4 points per thread (<= 128 registers)
+// Shared memory: [stages x STAGE] [full/empty barriers] [elec FP64] [a/dd scratch per warp]
+//                [FP64 columns: EPT*4 doubles per thread, stored as double2 rows].
+template <int EP2, int NW>
+struct F32x2Layout {
+    static constexpr int EPT = 2 * EP2;
+    static constexpr int NT = 32 * NW;
+    static constexpr int CHUNK_BYTES = 4 * CHUNK * sizeof(float);
+    static constexpr int STAGE_BYTES = STAGE_HDR + BLOCK_CHUNKS * CHUNK_BYTES;
+    static constexpr int BAR_BYTES = 16 * sizeof(uint64_t);
+    static constexpr int ELEC_BYTES = NW * EPT * 3 * sizeof(double);
+    static constexpr int SCRATCH_BYTES = NW * 2 * 3 * EPT * sizeof(float);
+    static constexpr int ACC_BYTES = EPT * 4 * NT * sizeof(double);
+    __host__ __device__ static constexpr size_t total(int stages) {
+        return static_cast<size_t>(stages) * STAGE_BYTES + BAR_BYTES + ELEC_BYTES + SCRATCH_BYTES +
+               ACC_BYTES;
+    }
+};
 
-template <int EP2>
-__global__ void __launch_bounds__(F32X2_THREADS, 1) pair_kernel_f32x2(const PairParams prm) {
-    constexpr int EPT = 2 * EP2;
-    constexpr int CHUNK_BYTES = 4 * CHUNK * sizeof(float);
-    constexpr int STAGE_BYTES = STAGE_HDR + BLOCK_CHUNKS * CHUNK_BYTES;
-    constexpr int NT = F32X2_THREADS;
+template <int EP2, int NW>
+__global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams prm) {
+    using L = F32x2Layout<EP2, NW>;
+    constexpr int EPT = L::EPT, NT = L::NT;
+    constexpr int CHUNK_BYTES = L::CHUNK_BYTES, STAGE_BYTES = L::STAGE_BYTES;
 
     extern __shared__ __align__(128) unsigned char smem[];
-    // layout: [stages x STAGE_BYTES] [full barriers] [empty barriers] [elec] [acc columns]
     const int stages = prm.stages;
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem + static_cast<size_t>(stages) * STAGE_BYTES);
+    unsigned char *ptr = smem + static_cast<size_t>(stages) * STAGE_BYTES;
+    uint64_t *full = reinterpret_cast<uint64_t *>(ptr);
     uint64_t *empty = full + 8;
-    double *elec_s = reinterpret_cast<double *>(empty + 8);   // [WP*EPT][3], WP <= 8
-    double *acc = elec_s + COMPUTE_WARPS * EPT * 3;            // [EPT*4][NT]
+    ptr += L::BAR_BYTES;
+    double *elec_s = reinterpret_cast<double *>(ptr);          // [WP*EPT][3]
+    ptr += L::ELEC_BYTES;
+    float *scratch = reinterpret_cast<float *>(ptr);           // per warp: a[3][EPT], dd[3][EPT]
+    ptr += L::SCRATCH_BYTES;
+    double2 *acc = reinterpret_cast<double2 *>(ptr);           // [EPT*2][NT] double2
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int WP = prm.point_warps, WS = COMPUTE_WARPS / WP;
+    const int WP = prm.point_warps, WS = NW / WP;
     int lo, hi;
     slice_range(prm.n_chunks, prm.slices, blockIdx.x, lo, hi);
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < stages; ++s) {
             mbar_init(&full[s], 1);
-            mbar_init(&empty[s], COMPUTE_WARPS);
+            mbar_init(&empty[s], NW);
         }
         fence_barrier_init();
     }
     const int ppb = WP * EPT;
     for (int i = threadIdx.x; i < ppb * 3; i += NT) {
         int p = blockIdx.y * ppb + i / 3;
-        p = p < prm.P ? p : prm.P - 1;
+        p = p < prm.P ? p : prm.P - 1;                          // clamp: duplicates are not written
         elec_s[i] = prm.elec[static_cast<int64_t>(p) * 3 + (i % 3)];
     }
     __syncthreads();
 
-    // producer cursor (used by warp 0 only): next pipeline step to load
-    int pc = lo, pk = 0;
+    // ---- producer cursor (warp 0 only): next pipeline step to load -------------------------
+    int pc = lo, pslot = 0;
+    uint32_t pphase = 0;
+    bool pwrapped = false;
     auto produce = [&]() {
         if (pc >= hi) return;
         const int ce = stage_end(pc, hi);
-        const int slot = pk % stages;
-        if (pk >= stages) mbar_wait(&empty[slot], ((pk / stages) - 1) & 1);
+        if (pwrapped) mbar_wait(&empty[pslot], pphase);
         if (lane == 0) {
-            unsigned char *dst = smem + static_cast<size_t>(slot) * STAGE_BYTES;
+            unsigned char *dst = smem + static_cast<size_t>(pslot) * STAGE_BYTES;
             const uint32_t bytes = static_cast<uint32_t>(ce - pc) * CHUNK_BYTES;
-            mbar_expect_tx(&full[slot], bytes + 32);
-            tma_bulk_g2s(dst, prm.origins + 4 * (pc / BLOCK_CHUNKS), 32, &full[slot]);
+            mbar_expect_tx(&full[pslot], bytes + 32);
+            tma_bulk_g2s(dst, prm.origins + 4 * (pc / BLOCK_CHUNKS), 32, &full[pslot]);
             tma_bulk_g2s(dst + STAGE_HDR, prm.chunks + static_cast<size_t>(pc) * CHUNK_BYTES, bytes,
-                         &full[slot]);
+                         &full[pslot]);
         }
         pc = ce;
-        ++pk;
+        if (++pslot == stages) {
+            pslot = 0;
+            if (pwrapped) pphase ^= 1u;
+            pwrapped = true;
+        }
     };
     if (warp == 0)
         for (int i = 0; i < stages - 1; ++i) produce();
 
     const int wp = warp % WP, ws = warp / WP;
-    double *my = acc + threadIdx.x;                 // column of this thread: my[i * NT]
+    double2 *my = acc + threadIdx.x;                 // this thread's column: my[i * NT]
 #pragma unroll
-    for (int i = 0; i < EPT * 4; ++i) my[i * NT] = 0.0;
+    for (int i = 0; i < EPT * 2; ++i) my[i * NT] = make_double2(0.0, 0.0);
     const double *pe = elec_s + wp * EPT * 3;
+    float *a_s = scratch + warp * 6 * EPT;           // a[3][EPT]
+    float *dd_s = a_s + 3 * EPT;                     // dd[3][EPT]
 
-    int c = lo, k = 0;
-    while (c < hi) {
+    int slot = 0;
+    uint32_t phase = 0;
+    for (int c = lo; c < hi;) {
         const int ce = stage_end(c, hi);
-        const int slot = k % stages;
         if (warp == 0) produce();          // step k + stages - 1 into the slot freed by step k - 1
-        mbar_wait(&full[slot], (k / stages) & 1);
+        mbar_wait(&full[slot], phase);
         const unsigned char *st = smem + static_cast<size_t>(slot) * STAGE_BYTES;
         const float *data = reinterpret_cast<const float *>(st + STAGE_HDR);
         const int nch = ce - c;
-        // tile-local coordinates a = r_i - c_block, formed in FP64 and rounded once
-        const double *org = reinterpret_cast<const double *>(st);
-        const double cx = org[0], cy = org[1], cz = org[2];
+        // Tile-local coordinates a = r_i - c_block: formed in FP64 and rounded once, by the
+        // first 3*EPT lanes for the whole warp; dd = (r_i - c_block) - a is the rounding residual.
+        __syncwarp();
+        if (lane < 3 * EPT) {
+            const int comp = lane / EPT, pt = lane % EPT;
+            const double a64 = pe[3 * pt + comp] - reinterpret_cast<const double *>(st)[comp];
+            const float a32 = lattice_round(a64, prm.lattice, prm.inv_lattice);
+            a_s[lane] = a32;
+            dd_s[lane] = static_cast<float>(a64 - static_cast<double>(a32));
+        }
+        __syncwarp();
         float2 rx[EP2], ry[EP2], rz[EP2], v[EP2], ex[EP2], ey[EP2], ez[EP2];
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
-            rx[e] = f2(static_cast<float>(pe[6 * e + 0] - cx), static_cast<float>(pe[6 * e + 3] - cx));
-            ry[e] = f2(static_cast<float>(pe[6 * e + 1] - cy), static_cast<float>(pe[6 * e + 4] - cy));
-            rz[e] = f2(static_cast<float>(pe[6 * e + 2] - cz), static_cast<float>(pe[6 * e + 5] - cz));
+            rx[e] = *reinterpret_cast<const float2 *>(a_s + 2 * e);
+            ry[e] = *reinterpret_cast<const float2 *>(a_s + EPT + 2 * e);
+            rz[e] = *reinterpret_cast<const float2 *>(a_s + 2 * EPT + 2 * e);
             v[e] = ex[e] = ey[e] = ez[e] = f2(0.0f, 0.0f);
         }
-        for (int ch = ws; ch < nch; ch += WS)
-            chunk_f32x2<EP2>(data + ch * 4 * CHUNK + 4 * lane, rx, ry, rz, v, ex, ey, ez);
+        for (int ch = ws; ch < nch;) {
+            float2 v4[EP2];                           // middle level of the V tree: 4 chunks
+#pragma unroll
+            for (int e = 0; e < EP2; ++e) v4[e] = f2(0.0f, 0.0f);
+#pragma unroll 1
+            for (int g = 0; g < 4 && ch < nch; ++g, ch += WS)
+                chunk_f32x2<EP2>(data + ch * 4 * CHUNK + 4 * lane, rx, ry, rz, v4, ex, ey, ez);
+#pragma unroll
+            for (int e = 0; e < EP2; ++e) v[e] = __fadd2_rn(v[e], v4[e]);
+        }
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[slot]);   // the stage's source data is consumed
-        // flush the FP32 run into the FP64 column; the rounding residual delta of a enters as
-        // the first-order correction V(a_hat + delta) = V(a_hat) - E(a_hat) . delta
+        // Flush the FP32 run into the FP64 columns.  The residual dd enters as the first-order
+        // correction V(a + dd) = V(a) - E(a) . dd.
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
-#pragma unroll
-            for (int hlf = 0; hlf < 2; ++hlf) {
-                const int pi = 2 * e + hlf;
-                const float ax = hlf ? rx[e].y : rx[e].x, ay = hlf ? ry[e].y : ry[e].x;
-                const float az = hlf ? rz[e].y : rz[e].x;
-                const float fx = hlf ? ex[e].y : ex[e].x, fy = hlf ? ey[e].y : ey[e].x;
-                const float fz = hlf ? ez[e].y : ez[e].x, fv = hlf ? v[e].y : v[e].x;
-                const float ddx = static_cast<float>((pe[3 * pi + 0] - cx) - static_cast<double>(ax));
-                const float ddy = static_cast<float>((pe[3 * pi + 1] - cy) - static_cast<double>(ay));
-                const float ddz = static_cast<float>((pe[3 * pi + 2] - cz) - static_cast<double>(az));
-                const float corr = fmaf(fz, ddz, fmaf(fy, ddy, fx * ddx));
-                my[(4 * pi + 0) * NT] += static_cast<double>(fv) - static_cast<double>(corr);
-                my[(4 * pi + 1) * NT] += static_cast<double>(fx);
-                my[(4 * pi + 2) * NT] += static_cast<double>(fy);
-                my[(4 * pi + 3) * NT] += static_cast<double>(fz);
-            }
+            const float2 ddx = *reinterpret_cast<const float2 *>(dd_s + 2 * e);
+            const float2 ddy = *reinterpret_cast<const float2 *>(dd_s + EPT + 2 * e);
+            const float2 ddz = *reinterpret_cast<const float2 *>(dd_s + 2 * EPT + 2 * e);
+            const float2 corr = __ffma2_rn(ez[e], ddz, __ffma2_rn(ey[e], ddy, __fmul2_rn(ex[e], ddx)));
+            double2 t;                                // rows of the pair: V, Ex, Ey, Ez
+            t = my[(4 * e + 0) * NT];
+            t.x += static_cast<double>(v[e].x) - static_cast<double>(corr.x);
+            t.y += static_cast<double>(v[e].y) - static_cast<double>(corr.y);
+            my[(4 * e + 0) * NT] = t;
+            t = my[(4 * e + 1) * NT];
+            t.x += static_cast<double>(ex[e].x);
+            t.y += static_cast<double>(ex[e].y);
+            my[(4 * e + 1) * NT] = t;
+            t = my[(4 * e + 2) * NT];
+            t.x += static_cast<double>(ey[e].x);
+            t.y += static_cast<double>(ey[e].y);
+            my[(4 * e + 2) * NT] = t;
+            t = my[(4 * e + 3) * NT];
+            t.x += static_cast<double>(ez[e].x);
+            t.y += static_cast<double>(ez[e].y);
+            my[(4 * e + 3) * NT] = t;
         }
         c = ce;
-        ++k;
+        if (++slot == stages) {
+            slot = 0;
+            phase ^= 1u;
+        }
     }
 
     // ---- in-CTA reduction: fixed-order butterfly per value, then the WS partners in order ----
-    double *red = acc;      // reuse: after the barrier, [COMPUTE_WARPS][EPT*4] at the front
+    // column row 4e+comp holds {V,Ex,Ey,Ez}[comp] of points (2e, 2e+1); lane 4*point+comp of
+    // the warp keeps the reduced value.
+    double *red = reinterpret_cast<double *>(acc);   // reused after the barrier: [NW][EPT*4]
     double mine = 0.0;
 #pragma unroll
-    for (int i = 0; i < EPT * 4; ++i) {
-        const double t = warp_sum(my[i * NT]);
-        if (lane == i) mine = t;
+    for (int i = 0; i < EPT * 2; ++i) {
+        const double2 t = my[i * NT];
+        const double sx = warp_sum(t.x), sy = warp_sum(t.y);
+        if (lane == 8 * (i / 4) + (i & 3)) mine = sx;
+        if (lane == 8 * (i / 4) + 4 + (i & 3)) mine = sy;
     }
     __syncthreads();                                 // every column has been read
     if (lane < EPT * 4) red[warp * EPT * 4 + lane] = mine;
@@ -602,8 +681,38 @@ __global__ void pack_f64_kernel(const double *xyz, const double *q, int64_t M, i
     c[3 * CHUNK + i] = j < M ? q[src] : 0.0;
 }
 
+// Bounding box of all sources: CTA b writes {lo[3], hi[3]} to part[6b..]; the host finishes.
+__global__ void __launch_bounds__(256) bbox_kernel(const double *xyz, int64_t M, double *part) {
+    __shared__ double sh[8][6];
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    for (int64_t j = blockIdx.x * 256ll + threadIdx.x; j < M; j += 256ll * gridDim.x)
+        for (int k = 0; k < 3; ++k) {
+            const double v = xyz[3 * j + k];
+            lo[k] = fmin(lo[k], v);
+            hi[k] = fmax(hi[k], v);
+        }
+    for (int k = 0; k < 3; ++k)
+        for (int m = 16; m >= 1; m >>= 1) {
+            lo[k] = fmin(lo[k], __shfl_xor_sync(0xffffffffu, lo[k], m));
+            hi[k] = fmax(hi[k], __shfl_xor_sync(0xffffffffu, hi[k], m));
+        }
+    if ((threadIdx.x & 31) == 0)
+        for (int k = 0; k < 3; ++k) {
+            sh[threadIdx.x >> 5][k] = lo[k];
+            sh[threadIdx.x >> 5][3 + k] = hi[k];
+        }
+    __syncthreads();
+    if (threadIdx.x < 6) {
+        double v = sh[0][threadIdx.x];
+        for (int w = 1; w < 8; ++w)
+            v = threadIdx.x < 3 ? fmin(v, sh[w][threadIdx.x]) : fmax(v, sh[w][threadIdx.x]);
+        part[6 * blockIdx.x + threadIdx.x] = v;
+    }
+}
+
 // One warp per origin block: centre of the bounding box of the block's real sources.
-__global__ void origins_kernel(const double *xyz, int64_t M, int64_t n_blocks, double *origins) {
+__global__ void origins_kernel(const double *xyz, int64_t M, int64_t n_blocks, double lattice,
+                               double *origins) {
     const int64_t b = (blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (b >= n_blocks) return;
@@ -623,24 +732,63 @@ __global__ void origins_kernel(const double *xyz, int64_t M, int64_t n_blocks, d
             hi[k] = fmax(hi[k], __shfl_xor_sync(0xffffffffu, hi[k], m));
         }
     if (lane == 0) {
-        for (int k = 0; k < 3; ++k) origins[4 * b + k] = 0.5 * (lo[k] + hi[k]);
+        // centre of the bounding box, plus a deterministic sub-quantum jitter so that the
+        // lattice residuals of an evaluation point differ from block to block
+        for (int k = 0; k < 3; ++k) {
+            uint64_t hsh = (static_cast<uint64_t>(b) * 3 + k + 1) * 0x9E3779B97F4A7C15ull;
+            hsh ^= hsh >> 29; hsh *= 0xBF58476D1CE4E5B9ull; hsh ^= hsh >> 32;
+            const double u = static_cast<double>(hsh >> 11) * (1.0 / 9007199254740992.0) - 0.5;
+            origins[4 * b + k] = 0.5 * (lo[k] + hi[k]) + u * lattice;
+        }
         origins[4 * b + 3] = 0.0;
     }
 }
 
-__global__ void pack_f32_kernel(const double *xyz, const double *q, int64_t M, int64_t Mpad,
-                                const double *origins, float *chunks) {
-    const int64_t j = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x;
-    if (j >= Mpad) return;
-    const int64_t src = j < M ? j : M - 1;
-    const int64_t ch = j / CHUNK;
-    const int i = static_cast<int>(j % CHUNK);
+// FP32 copy: offsets from the block origin and charges, rounded with ERROR FEEDBACK along
+// memory order inside each 128-source chunk (one thread per chunk).  Plain round-to-nearest
+// of a regular grid's coordinates is a coherent pattern (the same residual at every node
+// with the same offset), which shifts V in the whole QM region by the same ~1e-8 hartree;
+// rounding errors of the charges do the same on a smaller scale.  Here every coordinate is
+// rounded to whichever of its two LATTICE neighbours keeps the running dipole residual
+// sum_j q_j (x_j - c - o_j) smallest, and every charge absorbs the residual of the previous
+// one, so the net monopole and dipole of the rounding errors of any run of neighbouring
+// sources stay below one rounding unit.
+__device__ __forceinline__ float round_feedback(double exact, double q, double &carry,
+                                                double lattice, double inv_lattice) {
+    const double n0 = rint(exact * inv_lattice);
+    const double v0 = n0 * lattice;
+    const float f0 = static_cast<float>(v0);          // exact: |offset| << 2^24 quanta
+    const double r0 = exact - v0;
+    if (r0 == 0.0 || q == 0.0) return f0;
+    const double v1 = (r0 > 0.0 ? n0 + 1.0 : n0 - 1.0) * lattice;
+    const float f1 = static_cast<float>(v1);
+    const double r1 = exact - v1;
+    const double c0 = carry + q * r0, c1 = carry + q * r1;
+    if (fabs(c0) <= fabs(c1)) { carry = c0; return f0; }
+    carry = c1;
+    return f1;
+}
+
+__global__ void pack_f32_kernel(const double *xyz, const double *q, int64_t M, int64_t n_chunks,
+                                const double *origins, double lattice, float *chunks) {
+    const double inv_lattice = 1.0 / lattice;
+    const int64_t ch = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x;
+    if (ch >= n_chunks) return;
     const double *o = origins + 4 * (ch / BLOCK_CHUNKS);
     float *c = chunks + ch * 4 * CHUNK;
-    c[i] = static_cast<float>(xyz[3 * src + 0] - o[0]);
-    c[CHUNK + i] = static_cast<float>(xyz[3 * src + 1] - o[1]);
-    c[2 * CHUNK + i] = static_cast<float>(xyz[3 * src + 2] - o[2]);
-    c[3 * CHUNK + i] = j < M ? static_cast<float>(q[src]) : 0.0f;
+    double cx = 0.0, cy = 0.0, cz = 0.0, cq = 0.0;       // running residuals
+    for (int i = 0; i < CHUNK; ++i) {
+        const int64_t j = ch * CHUNK + i;
+        const int64_t src = j < M ? j : M - 1;           // pads: last real source, charge 0
+        const double qj = j < M ? q[src] : 0.0;
+        c[i] = round_feedback(xyz[3 * src + 0] - o[0], qj, cx, lattice, inv_lattice);
+        c[CHUNK + i] = round_feedback(xyz[3 * src + 1] - o[1], qj, cy, lattice, inv_lattice);
+        c[2 * CHUNK + i] = round_feedback(xyz[3 * src + 2] - o[2], qj, cz, lattice, inv_lattice);
+        const double want = qj + cq;
+        const float q32 = static_cast<float>(want);
+        cq = j < M ? want - static_cast<double>(q32) : 0.0;
+        c[3 * CHUNK + i] = q32;
+    }
 }
 
 __global__ void pack_nuclei_kernel(const double *xyz, const double *Z, int64_t K, double *out) {
