@@ -341,10 +341,14 @@ def run_ours(args):
         pair_s = float(np.mean(pair_ms)) * 1e-3
         achieved = P * w.M * SLOTS[prec] * 2 / pair_s / 1e12
         peak_tf = 2 * peak_lane / 1e12
+        # DRAM bytes per pair-kernel launch from the committed ncu capture (profiles/), if any
         traffic = None
-        tpath = os.path.join(ROOT, "profiles", "pair_kernel_traffic.json")
+        tpath = os.path.join(ROOT, "profiles", "pair_kernel_traffic.csv")
         if os.path.exists(tpath):
-            traffic = json.load(open(tpath)).get(f"config{args.config}_{prec}")
+            for ln in open(tpath):
+                f = ln.strip().split(",")
+                if len(f) >= 2 and f[0] == f"config{args.config}_{prec}":
+                    traffic = float(f[1])
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,

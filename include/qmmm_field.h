@@ -120,7 +120,7 @@ typedef struct {
     int64_t n_chunks;            /* 128-source chunks after padding */
     int64_t bytes_fp64, bytes_fp32, bytes_workspace;
     qmmm_plan last_plan;         /* plan used by the most recent eval */
-    int32_t last_point_blocks;   /* grid.y of the most recent pair kernel */
+    int32_t last_point_blocks;   /* grid.x of the most recent pair kernel (grid.y = slices) */
     int32_t last_launches;       /* kernels launched by the most recent eval */
     int32_t sm_count;
     int32_t reserved;

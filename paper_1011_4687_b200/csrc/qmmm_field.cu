@@ -389,7 +389,6 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
     while (smem > 227 * 1024 && pl.stages > 2)           // a requested depth that does not fit is reduced
         smem = pair_smem_bytes(f32, --pl.stages, pl.points_per_thread, pl.point_warps);
     if (smem > 227 * 1024) return fail(QMMM_ERR_INVALID_ARG, "eval: plan exceeds shared memory");
-    if (pb > 65535) return fail(QMMM_ERR_INVALID_ARG, "eval: too many point blocks for this plan");
 
     if (h->timing) CUDA_TRY(cudaEventRecord(h->ev[0], st));
     if (h->n_chunks > 0) {
@@ -406,7 +405,9 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
         prm.stages = pl.stages;
         prm.lattice = h->lattice;
         prm.inv_lattice = 1.0 / h->lattice;
-        const dim3 grid(pl.slices, pb);
+        // point blocks vary fastest: the CTAs resident together read the same source slices,
+        // so a slice is fetched from HBM once and then served from L2
+        const dim3 grid(pb, pl.slices);
         cudaError_t e = f32 ? launch_pair_ept<float>(pl.points_per_thread, prm, grid, smem, st)
                             : launch_pair_ept<double>(pl.points_per_thread, prm, grid, smem, st);
         if (e != cudaSuccess) return cuda_fail(e, "pair_kernel launch");

@@ -172,7 +172,7 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 // ----------------------------------------------------------------------------- pair kernel
-// grid = (slices, point_blocks).  REAL = double (FP64 path) or float (FP32-acc64 path).
+// grid = (point_blocks, slices).  REAL = double (FP64 path) or float (FP32-acc64 path).
 template <typename REAL, int EPT>
 __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams prm) {
     constexpr bool F32 = sizeof(REAL) == 4;
@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int WP = prm.point_warps, WS = COMPUTE_WARPS / WP;
     int lo, hi;
-    slice_range(prm.n_chunks, prm.slices, blockIdx.x, lo, hi);
+    slice_range(prm.n_chunks, prm.slices, blockIdx.y, lo, hi);
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < stages; ++s) {
@@ -203,7 +203,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
     // stage the CTA's evaluation points (FP64) in shared memory
     const int ppb = WP * EPT;
     for (int i = threadIdx.x; i < ppb * 3; i += CTA_THREADS) {
-        int p = blockIdx.y * ppb + i / 3;
+        int p = blockIdx.x * ppb + i / 3;
         p = p < prm.P ? p : prm.P - 1;                       // clamp: duplicates are not written
         elec_s[i] = prm.elec[static_cast<int64_t>(p) * 3 + (i % 3)];
     }
@@ -349,9 +349,9 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
     if (ws == 0 && lane < EPT * 4) {
         double acc = 0.0;
         for (int s = 0; s < WS; ++s) acc += red[((s * WP + wp) * EPT) * 4 + lane];
-        const int p = (blockIdx.y * WP + wp) * EPT + lane / 4;
+        const int p = (blockIdx.x * WP + wp) * EPT + lane / 4;
         if (p < prm.P)
-            prm.partial[(static_cast<int64_t>(blockIdx.x) * prm.P + p) * 4 + (lane & 3)] = acc;
+            prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] = acc;
     }
 }
 
@@ -416,7 +416,7 @@ __device__ __forceinline__ void chunk_f32x2(const float *b, const float2 (&rx)[E
     for (int e = 0; e < EP2; ++e) V[e] = __fadd2_rn(V[e], Vc[e]);
 }
 
-// grid = (slices, point_blocks); EPT = 2 * EP2 points per thread; NW consumer warps and no
+// grid = (point_blocks, slices); EPT = 2 * EP2 points per thread; NW consumer warps and no
 // producer warp: a 9th warp would put 3 warps on one SM sub-partition and cap every thread
 // at 168 registers.  Warp 0 drives the TMA pipeline inline, stages-1 steps ahead.
 //   NW = 8,  EP2 = 4 : 2 warps per sub-partition, 8 points per thread (<= 255 registers)
@@ -460,7 +460,7 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int WP = prm.point_warps, WS = NW / WP;
     int lo, hi;
-    slice_range(prm.n_chunks, prm.slices, blockIdx.x, lo, hi);
+    slice_range(prm.n_chunks, prm.slices, blockIdx.y, lo, hi);
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < stages; ++s) {
@@ -471,7 +471,7 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
     }
     const int ppb = WP * EPT;
     for (int i = threadIdx.x; i < ppb * 3; i += NT) {
-        int p = blockIdx.y * ppb + i / 3;
+        int p = blockIdx.x * ppb + i / 3;
         p = p < prm.P ? p : prm.P - 1;                          // clamp: duplicates are not written
         elec_s[i] = prm.elec[static_cast<int64_t>(p) * 3 + (i % 3)];
     }
@@ -602,9 +602,9 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
     if (ws == 0 && lane < EPT * 4) {
         double a = 0.0;
         for (int s = 0; s < WS; ++s) a += red[(s * WP + wp) * EPT * 4 + lane];
-        const int p = (blockIdx.y * WP + wp) * EPT + lane / 4;
+        const int p = (blockIdx.x * WP + wp) * EPT + lane / 4;
         if (p < prm.P)
-            prm.partial[(static_cast<int64_t>(blockIdx.x) * prm.P + p) * 4 + (lane & 3)] = a;
+            prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] = a;
     }
 }
 
