@@ -3,15 +3,15 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl reference]
 
-A "step" is one pass of the whole hot path (pair kernel + finalize kernel; SURVEY.md 8(a)
-rows a1-a6) over one batch of synthetic evaluation points of the chosen BASELINE.json
+A "step" is one pass of the whole hot path (one fused launch: pair kernel incl. nuclei and the
+cross-CTA sum) over one batch of synthetic evaluation points of the chosen BASELINE.json
 configuration.  Rank 0 prints ONE JSON line.  See DESIGN.md "Measurement".
 
 * value      : whole-job pair-interactions/s (G/s), inputs resident in HBM, per-step CUDA
                events on the launch stream, L2 flushed between steps, max over ranks.
 * e2e        : same metric through qmmm_field_eval_host (the paper's per-step loop,
                PAPER.md:117): pinned HOST buffers, H2D + kernels + D2H + stream sync timed.
-* roofline   : pair kernel alone (events recorded by the library between its two kernels)
+* roofline   : the pair kernel (events recorded by the library around its launch)
                against the FMA-lane rate measured by the library's microbenchmark in the
                same process ("bound": "alu").
 * cpu_baseline: the CPU oracle as it stands on a bounded sample of the same workload.

@@ -130,10 +130,11 @@ qmmm_status qmmm_field_get_info(const qmmm_field *h, qmmm_field_info *info);
 
 /*
  * Per-kernel device timing for roofline measurements.  When enabled, eval records CUDA
- * events on its stream before the pair kernel, between the two kernels and after the
- * finalize kernel (a few microseconds of overhead; off by default).
- * qmmm_field_last_timing waits for the most recent eval to finish and returns the two
- * kernel durations in milliseconds.  INVALID_ARG if timing is off or no eval has run.
+ * events on its stream before and after the pair kernel (a few microseconds of overhead;
+ * off by default).  qmmm_field_last_timing waits for the most recent eval to finish and
+ * returns the kernel duration in milliseconds; *finalize_ms is always 0 (the cross-CTA sum
+ * and the nuclear term are fused into the pair kernel: one launch per evaluation).
+ * INVALID_ARG if timing is off or no eval has run.
  */
 qmmm_status qmmm_field_set_timing(qmmm_field *h, int enable);
 qmmm_status qmmm_field_last_timing(qmmm_field *h, double *pair_ms, double *finalize_ms);

@@ -156,7 +156,8 @@ def qmmm_field_set_timing(handle: int, enable: bool) -> None:
 
 
 def qmmm_field_last_timing(handle: int) -> Tuple[float, float]:
-    """(pair_kernel_ms, finalize_kernel_ms) of the most recent eval (waits for it)."""
+    """(pair_kernel_ms, 0.0) of the most recent eval (waits for it); the finalize step is
+    fused into the pair kernel."""
     a, b = ctypes.c_double(), ctypes.c_double()
     _check(_lib.qmmm_field_last_timing(handle, ctypes.byref(a), ctypes.byref(b)))
     return a.value, b.value

@@ -2,8 +2,9 @@
 //
 // create : upload + pack sources once ("required only once at the beginning
 //          of a run"), FP64 SoA chunks and FP32 tile-local SoA chunks, nuclei FP64.
-// eval   : pair kernel over (source slices x point blocks)  ->  per-slice partials
-//          (Eq. 5-6)  ->  finalize kernel (fixed-order sum + nuclei).
+// eval   : ONE launch: pair kernel over (point blocks x source slices) -> per-slice partials
+//          (Eq. 5-6) incl. the slice's share of the nuclei -> the last CTA
+//          of each point block adds the slices in a fixed order and writes V, E.
 // No torch types, no CPU fallback: every step of the path runs in the kernels of
 // qmmm_kernels.cuh.
 #include "qmmm_kernels.cuh"
@@ -57,8 +58,8 @@ size_t pair_smem_bytes(bool f32, int stages, int ept, int wp) {
     if (f32 && ept == 8) return F32x2Layout<4, F32X2_NW_EPT8>::total(stages);
     if (f32 && ept == 4) return F32x2Layout<2, F32X2_NW_EPT4>::total(stages);
     if (f32 && ept == 2) return F32x2Layout<1, F32X2_NW_EPT2>::total(stages);
-    return stages * stage_bytes(f32) + 16 * sizeof(uint64_t) +
-           static_cast<size_t>(COMPUTE_WARPS) * ept * 4 * sizeof(double) +
+    return stages * stage_bytes(f32) + 18 * sizeof(uint64_t) +
+           static_cast<size_t>(32) * COMPUTE_WARPS * sizeof(double) +
            static_cast<size_t>(wp) * ept * 3 * sizeof(double);
 }
 
@@ -66,9 +67,9 @@ size_t pair_smem_bytes(bool f32, int stages, int ept, int wp) {
 
 struct qmmm_field {
     int64_t M = 0, K = 0, max_points = 0;
-    int64_t n_chunks = 0, n_blocks = 0;
+    int64_t n_chunks = 0, n_chunks64 = 0, n_blocks = 0;
     int device = 0, sm_count = 0;
-    double *chunks64 = nullptr;    // [n_chunks][4][128] double
+    double *chunks64 = nullptr;    // [n_chunks64][4][128] double (cells, then nuclei)
     float *chunks32 = nullptr;     // [n_chunks][4][128] float (offsets from block origin, q)
     double *origins = nullptr;     // [n_blocks][4]
     double lattice = 1.0;          // FP32 coordinate quantum (power of two)
@@ -80,9 +81,9 @@ struct qmmm_field {
     qmmm_plan user_plan = {0, 0, 0, 0};
     qmmm_plan last_plan = {0, 0, 0, 0};
     int last_point_blocks = 0, last_launches = 0;
-    double *workspace_bbox() const { return chunks64; }   // scratch before packing (>= 512 doubles)
     bool timing = false, timed = false;
-    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    cudaEvent_t ev[2] = {nullptr, nullptr};
+    int *counters = nullptr;       // [max_points] arrival tickets of the point blocks (zero at rest)
 };
 
 namespace {
@@ -93,6 +94,7 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32) {
     qmmm_plan pl = h->user_plan;
     const int max_ept = f32 ? 8 : 4;
     if (pl.points_per_thread == 0) pl.points_per_thread = std::min(max_ept, pow2_ceil(P));
+    pl.points_per_thread = std::min(pl.points_per_thread, max_ept);
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
     const int nw = (f32 && pl.points_per_thread >= 2) ? f32x2_warps(pl.points_per_thread) : COMPUTE_WARPS;
     if (pl.point_warps == 0) pl.point_warps = std::min<int>(nw, pow2_ceil(groups));
@@ -102,7 +104,8 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32) {
         const int g = gcd_int(static_cast<int>(pb % h->sm_count), h->sm_count);
         pl.slices = h->sm_count / g;       // pb * slices is a multiple of the SM count
     }
-    pl.slices = static_cast<int>(std::max<int64_t>(1, std::min<int64_t>(pl.slices, h->n_chunks)));
+    const int64_t work_units = f32 ? std::max<int64_t>(h->n_chunks, (h->K + 31) / 32) : h->n_chunks64;
+    pl.slices = static_cast<int>(std::max<int64_t>(1, std::min<int64_t>(pl.slices, work_units)));
     // the partials workspace bounds slices * P
     const int64_t cap = h->workspace_doubles / (4 * P);
     if (pl.slices > cap) pl.slices = static_cast<int>(std::max<int64_t>(1, cap));
@@ -141,21 +144,23 @@ cudaError_t launch_pair_f32x2(const PairParams &prm, dim3 grid, size_t smem, cud
     return cudaGetLastError();
 }
 
-template <typename REAL>
-cudaError_t launch_pair_ept(int ept, const PairParams &prm, dim3 grid, size_t smem,
+// FP64: pair_kernel<double, 1|2|4>.  FP32-acc64: the scalar kernel for one point per
+// thread (bandwidth-bound), the packed f32x2 kernel for 2, 4 or 8.
+cudaError_t launch_pair_ept(bool f32, int ept, const PairParams &prm, dim3 grid, size_t smem,
                             cudaStream_t st) {
-    if constexpr (sizeof(REAL) == 4) {
+    if (f32) {
         switch (ept) {
+            case 1: return launch_pair<float, 1>(prm, grid, smem, st);
             case 2: return launch_pair_f32x2<1, F32X2_NW_EPT2>(prm, grid, smem, st);
             case 4: return launch_pair_f32x2<2, F32X2_NW_EPT4>(prm, grid, smem, st);
             case 8: return launch_pair_f32x2<4, F32X2_NW_EPT8>(prm, grid, smem, st);
         }
-    }
-    switch (ept) {
-        case 1: return launch_pair<REAL, 1>(prm, grid, smem, st);
-        case 2: return launch_pair<REAL, 2>(prm, grid, smem, st);
-        case 4: return launch_pair<REAL, 4>(prm, grid, smem, st);
-        case 8: return launch_pair<REAL, 8>(prm, grid, smem, st);
+    } else {
+        switch (ept) {
+            case 1: return launch_pair<double, 1>(prm, grid, smem, st);
+            case 2: return launch_pair<double, 2>(prm, grid, smem, st);
+            case 4: return launch_pair<double, 4>(prm, grid, smem, st);
+        }
     }
     return cudaErrorInvalidValue;
 }
@@ -217,7 +222,8 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
     if (!h) return fail(QMMM_ERR_ALLOC, "create: host allocation failed");
     h->M = M; h->K = K; h->max_points = max_points;
     h->device = dev; h->sm_count = prop.multiProcessorCount;
-    h->n_chunks = (M + CHUNK - 1) / CHUNK;
+    h->n_chunks = (M + CHUNK - 1) / CHUNK;                 // FP32 copy: cells only
+    h->n_chunks64 = (M + K + CHUNK - 1) / CHUNK;           // FP64 copy: cells + nuclei
     h->n_blocks = (h->n_chunks + BLOCK_CHUNKS - 1) / BLOCK_CHUNKS;
 
     auto bail = [&](qmmm_status st) { qmmm_field_destroy(h); return st; };
@@ -230,64 +236,69 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
                             : cuda_fail(_e, #expr));                                   \
     } while (0)
 
-    if (M > 0) {
-        const int64_t Mpad = h->n_chunks * CHUNK;
-        double *dxyz = nullptr, *dq = nullptr;
-        bool own_xyz = false, own_q = false;
-        CREATE_TRY(to_device(src_xyz, 3 * M, &dxyz, &own_xyz));
-        cudaError_t e = to_device(src_q, M, &dq, &own_q);
-        if (e == cudaSuccess) e = cudaMalloc(&h->chunks64, Mpad * 4 * sizeof(double));
-        if (e == cudaSuccess) e = cudaMalloc(&h->chunks32, Mpad * 4 * sizeof(float));
-        if (e == cudaSuccess) e = cudaMalloc(&h->origins, h->n_blocks * 4 * sizeof(double));
-        if (e == cudaSuccess) {
-            // coordinate lattice of the FP32 copy: the largest extent of the bounding box fits
-            // in 2^24 quanta, so d = a - o is exact for every point inside the box
-            const int nbb = static_cast<int>(std::min<int64_t>(256, (M + 255) / 256));
-            double hbb[256 * 6];
-            bbox_kernel<<<nbb, 256>>>(dxyz, M, h->workspace_bbox());
-            e = cudaMemcpy(hbb, h->workspace_bbox(), nbb * 6 * sizeof(double), cudaMemcpyDeviceToHost);
-            double ext = 0.0;
-            for (int k = 0; k < 3 && e == cudaSuccess; ++k) {
-                double lo = hbb[k], hi = hbb[3 + k];
-                for (int b = 1; b < nbb; ++b) {
-                    lo = std::min(lo, hbb[6 * b + k]);
-                    hi = std::max(hi, hbb[6 * b + 3 + k]);
+    {
+        // device copies of the caller's arrays (no copy when they already are device pointers)
+        double *dxyz = nullptr, *dq = nullptr, *dnxyz = nullptr, *dnz = nullptr;
+        bool own[4] = {false, false, false, false};
+        cudaError_t e = to_device(src_xyz, 3 * M, &dxyz, &own[0]);
+        if (e == cudaSuccess) e = to_device(src_q, M, &dq, &own[1]);
+        if (e == cudaSuccess) e = to_device(nuc_xyz, 3 * K, &dnxyz, &own[2]);
+        if (e == cudaSuccess) e = to_device(nuc_Z, K, &dnz, &own[3]);
+        const int T = 256;
+        if (e == cudaSuccess && M + K > 0) {
+            // FP64 copy: cells then nuclei, one SoA chunk array (the nuclei are ordinary FP64 sources)
+            const int64_t Mpad = h->n_chunks64 * CHUNK;
+            e = cudaMalloc(&h->chunks64, Mpad * 4 * sizeof(double));
+            if (e == cudaSuccess)
+                pack_f64_kernel<<<static_cast<unsigned>((Mpad + T - 1) / T), T>>>(
+                    dxyz, dq, M, dnxyz, dnz, K, Mpad, h->chunks64);
+        }
+        if (e == cudaSuccess && K > 0) {
+            // FP32 path: the nuclei stay FP64, packed x, y, z, Z
+            e = cudaMalloc(&h->nuclei, K * 4 * sizeof(double));
+            if (e == cudaSuccess)
+                pack_nuclei_kernel<<<static_cast<unsigned>((K + T - 1) / T), T>>>(dnxyz, dnz, K, h->nuclei);
+        }
+        if (e == cudaSuccess && M > 0) {
+            e = cudaMalloc(&h->chunks32, h->n_chunks * CHUNK * 4 * sizeof(float));
+            if (e == cudaSuccess) e = cudaMalloc(&h->origins, h->n_blocks * 4 * sizeof(double));
+            double *dbb = nullptr;
+            if (e == cudaSuccess) e = cudaMalloc(&dbb, 256 * 6 * sizeof(double));
+            if (e == cudaSuccess) {
+                // coordinate lattice of the FP32 copy: the largest extent of the cells' bounding
+                // box fits in 2^24 quanta, so d = a - o is exact for every point inside the box
+                const int nbb = static_cast<int>(std::min<int64_t>(256, (M + 255) / 256));
+                double hbb[256 * 6];
+                bbox_kernel<<<nbb, 256>>>(dxyz, M, dbb);
+                e = cudaMemcpy(hbb, dbb, nbb * 6 * sizeof(double), cudaMemcpyDeviceToHost);
+                double ext = 0.0;
+                for (int k = 0; k < 3 && e == cudaSuccess; ++k) {
+                    double lo = hbb[k], hi = hbb[3 + k];
+                    for (int b = 1; b < nbb; ++b) {
+                        lo = std::min(lo, hbb[6 * b + k]);
+                        hi = std::max(hi, hbb[6 * b + 3 + k]);
+                    }
+                    ext = std::max(ext, hi - lo);
                 }
-                ext = std::max(ext, hi - lo);
+                if (!(ext > 0.0) || !std::isfinite(ext)) ext = 1.0;
+                int ex2 = 0;
+                std::frexp(ext, &ex2);                       // ext = m * 2^ex2, 0.5 <= m < 1
+                h->lattice = std::ldexp(1.0, ex2 - 24);
             }
-            if (!(ext > 0.0) || !std::isfinite(ext)) ext = 1.0;
-            int ex2 = 0;
-            std::frexp(ext, &ex2);                       // ext = m * 2^ex2, 0.5 <= m < 1
-            h->lattice = std::ldexp(1.0, ex2 - 24);
+            if (dbb) cudaFree(dbb);
+            if (e == cudaSuccess) {
+                origins_kernel<<<static_cast<unsigned>((h->n_blocks * 32 + T - 1) / T), T>>>(
+                    dxyz, M, h->n_blocks, h->lattice, h->origins);
+                pack_f32_kernel<<<static_cast<unsigned>((h->n_chunks + 63) / 64), 64>>>(
+                    dxyz, dq, M, h->n_chunks, h->origins, h->lattice, h->chunks32);
+            }
         }
-        if (e == cudaSuccess) {
-            const int T = 256;
-            const unsigned nb = static_cast<unsigned>((Mpad + T - 1) / T);
-            pack_f64_kernel<<<nb, T>>>(dxyz, dq, M, Mpad, h->chunks64);
-            origins_kernel<<<static_cast<unsigned>((h->n_blocks * 32 + T - 1) / T), T>>>(
-                dxyz, M, h->n_blocks, h->lattice, h->origins);
-            pack_f32_kernel<<<static_cast<unsigned>((h->n_chunks + 63) / 64), 64>>>(
-                dxyz, dq, M, h->n_chunks, h->origins, h->lattice, h->chunks32);
-            e = cudaGetLastError();
-            if (e == cudaSuccess) e = cudaDeviceSynchronize();
-        }
-        if (own_xyz) cudaFree(dxyz);
-        if (own_q) cudaFree(dq);
-        CREATE_TRY(e);
-    }
-    if (K > 0) {
-        double *dxyz = nullptr, *dz = nullptr;
-        bool own_xyz = false, own_z = false;
-        CREATE_TRY(to_device(nuc_xyz, 3 * K, &dxyz, &own_xyz));
-        cudaError_t e = to_device(nuc_Z, K, &dz, &own_z);
-        if (e == cudaSuccess) e = cudaMalloc(&h->nuclei, K * 4 * sizeof(double));
-        if (e == cudaSuccess) {
-            pack_nuclei_kernel<<<static_cast<unsigned>((K + 255) / 256), 256>>>(dxyz, dz, K, h->nuclei);
-            e = cudaGetLastError();
-            if (e == cudaSuccess) e = cudaDeviceSynchronize();
-        }
-        if (own_xyz) cudaFree(dxyz);
-        if (own_z) cudaFree(dz);
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        if (own[0]) cudaFree(dxyz);
+        if (own[1]) cudaFree(dq);
+        if (own[2]) cudaFree(dnxyz);
+        if (own[3]) cudaFree(dnz);
         CREATE_TRY(e);
     }
     // Partials workspace: slices * P * 4 doubles.  With P = max_points the automatic plan
@@ -295,6 +306,8 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
     h->workspace_doubles =
         4 * std::max<int64_t>(static_cast<int64_t>(h->sm_count) * max_points, int64_t(1) << 16);
     CREATE_TRY(cudaMalloc(&h->workspace, h->workspace_doubles * sizeof(double)));
+    CREATE_TRY(cudaMalloc(&h->counters, max_points * sizeof(int)));
+    CREATE_TRY(cudaMemset(h->counters, 0, max_points * sizeof(int)));
     CREATE_TRY(cudaMalloc(&h->stage_elec, max_points * 3 * sizeof(double)));
     CREATE_TRY(cudaMalloc(&h->stage_out, max_points * 4 * sizeof(double)));
 #undef CREATE_TRY
@@ -309,6 +322,7 @@ qmmm_status qmmm_field_destroy(qmmm_field *h) {
     cudaFree(h->origins);
     cudaFree(h->nuclei);
     cudaFree(h->workspace);
+    cudaFree(h->counters);
     cudaFree(h->stage_elec);
     cudaFree(h->stage_out);
     for (cudaEvent_t e : h->ev)
@@ -345,12 +359,11 @@ qmmm_status qmmm_field_last_timing(qmmm_field *h, double *pair_ms, double *final
     if (!h || !pair_ms || !finalize_ms) return fail(QMMM_ERR_INVALID_ARG, "last_timing: NULL argument");
     if (!h->timing || !h->timed)
         return fail(QMMM_ERR_INVALID_ARG, "last_timing: timing is off or no eval has run");
-    CUDA_TRY(cudaEventSynchronize(h->ev[2]));
-    float a = 0.f, b = 0.f;
+    CUDA_TRY(cudaEventSynchronize(h->ev[1]));
+    float a = 0.f;
     CUDA_TRY(cudaEventElapsedTime(&a, h->ev[0], h->ev[1]));
-    CUDA_TRY(cudaEventElapsedTime(&b, h->ev[1], h->ev[2]));
     *pair_ms = a;
-    *finalize_ms = b;
+    *finalize_ms = 0.0;      // the cross-CTA sum is fused into the pair kernel
     return QMMM_OK;
 }
 
@@ -359,7 +372,7 @@ qmmm_status qmmm_field_get_info(const qmmm_field *h, qmmm_field_info *info) {
     std::memset(info, 0, sizeof(*info));
     info->M = h->M; info->K = h->K; info->max_points = h->max_points;
     info->n_chunks = h->n_chunks;
-    info->bytes_fp64 = h->n_chunks * CHUNK * 4 * 8;
+    info->bytes_fp64 = h->n_chunks64 * CHUNK * 4 * 8;
     info->bytes_fp32 = h->n_chunks * CHUNK * 4 * 4 + h->n_blocks * 32;
     info->bytes_workspace = h->workspace_doubles * 8;
     info->last_plan = h->last_plan;
@@ -391,7 +404,7 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
     if (smem > 227 * 1024) return fail(QMMM_ERR_INVALID_ARG, "eval: plan exceeds shared memory");
 
     if (h->timing) CUDA_TRY(cudaEventRecord(h->ev[0], st));
-    if (h->n_chunks > 0) {
+    {
         PairParams prm;
         prm.chunks = f32 ? reinterpret_cast<const char *>(h->chunks32)
                          : reinterpret_cast<const char *>(h->chunks64);
@@ -399,38 +412,26 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
         prm.elec = elec_xyz;
         prm.partial = h->workspace;
         prm.P = P;
-        prm.n_chunks = static_cast<int>(h->n_chunks);
+        prm.n_chunks = static_cast<int>(f32 ? h->n_chunks : h->n_chunks64);
         prm.slices = pl.slices;
         prm.point_warps = pl.point_warps;
         prm.stages = pl.stages;
         prm.lattice = h->lattice;
         prm.inv_lattice = 1.0 / h->lattice;
+        prm.nuc = h->nuclei;
+        prm.K = f32 ? static_cast<int>(h->K) : 0;     // FP64: nuclei are in the chunk array
+        prm.V = V;
+        prm.E = E;
+        prm.counters = h->counters;
         // point blocks vary fastest: the CTAs resident together read the same source slices,
         // so a slice is fetched from HBM once and then served from L2
         const dim3 grid(pb, pl.slices);
-        cudaError_t e = f32 ? launch_pair_ept<float>(pl.points_per_thread, prm, grid, smem, st)
-                            : launch_pair_ept<double>(pl.points_per_thread, prm, grid, smem, st);
+        cudaError_t e = launch_pair_ept(f32, pl.points_per_thread, prm, grid, smem, st);
         if (e != cudaSuccess) return cuda_fail(e, "pair_kernel launch");
         ++launches;
     }
-    if (h->timing) CUDA_TRY(cudaEventRecord(h->ev[1], st));
-    FinalizeParams fp;
-    fp.partial = h->workspace;
-    fp.nuc = h->nuclei;
-    fp.elec = elec_xyz;
-    fp.V = V;
-    fp.E = E;
-    fp.P = P;
-    fp.slices = h->n_chunks > 0 ? pl.slices : 0;
-    fp.K = static_cast<int>(h->K);
-    fp.tpp = P <= 64 ? 256 : 32;
-    const int per_cta = 256 / fp.tpp;
-    finalize_kernel<<<(P + per_cta - 1) / per_cta, 256, 0, st>>>(fp);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "finalize_kernel launch");
-    ++launches;
     if (h->timing) {
-        CUDA_TRY(cudaEventRecord(h->ev[2], st));
+        CUDA_TRY(cudaEventRecord(h->ev[1], st));
         h->timed = true;
     }
 

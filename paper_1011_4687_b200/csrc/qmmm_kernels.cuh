@@ -9,9 +9,10 @@
 //     producer warp stages up to 8 chunks per pipeline stage into shared memory with
 //     TMA bulk copies (cp.async.bulk + mbarrier complete_tx), consumers read them with
 //     conflict-free 128-bit LDS (lane l owns sources 4l..4l+3 of a chunk);
-//   * per-thread FP64 running sums, fixed-order warp-shuffle + shared-memory reduction,
-//     one partial {V,Ex,Ey,Ez} per (slice, point) in a workspace, and a second kernel
-//     that adds the slices in index order and the nuclear term (always FP64).
+//   * per-thread FP64 running sums (cells in FP64 or FP32-acc64, nuclei always FP64),
+//     fixed-order warp-shuffle + shared-memory reduction, one partial {V,Ex,Ey,Ez} per
+//     (slice, point) in a workspace; the last CTA of a point block to arrive (integer
+//     ticket) adds the slices in a fixed order and writes V, E: one launch per evaluation.
 // No floating-point atomics anywhere: results are bitwise reproducible.
 #pragma once
 #include <cuda_runtime.h>
@@ -41,6 +42,11 @@ struct PairParams {
     int stages;
     double lattice;          // FP32 only: coordinate quantum (power of two), and its inverse
     double inv_lattice;
+    const double *nuc;       // [K][4] packed x, y, z, Z (always FP64)
+    int K;
+    double *V;               // [P]       final outputs, written by the last CTA of a point block
+    double *E;               // [P][3] or NULL
+    int *counters;           // [point_blocks] arrival tickets, zero between evaluations
 };
 
 // ----------------------------------------------------------------------------- PTX helpers
@@ -171,6 +177,71 @@ __device__ __forceinline__ double warp_sum(double v) {
     return v;
 }
 
+// ----------------------------------------------------------------------------- epilogue
+// a5: the nuclear term, always FP64 (the paper keeps U_nuc in double on the
+// CPU).  The K nuclei are split over the source slices like the cells; inside
+// a CTA over the source-split warps and the lanes.  Every thread adds its share for its EPT
+// points to its FP64 sums before the in-CTA reduction.
+template <int EPT>
+__device__ __forceinline__ void nuclei_share(const PairParams &prm, const double *pe, int ws,
+                                             int WS, int lane, double (&V)[EPT], double (&Ex)[EPT],
+                                             double (&Ey)[EPT], double (&Ez)[EPT]) {
+    int klo, khi;
+    slice_range(prm.K, prm.slices, blockIdx.y, klo, khi);
+    for (int j = klo + ws * 32 + lane; j < khi; j += 32 * WS) {
+        const double2 a = *reinterpret_cast<const double2 *>(prm.nuc + 4 * static_cast<int64_t>(j));
+        const double2 b = *reinterpret_cast<const double2 *>(prm.nuc + 4 * static_cast<int64_t>(j) + 2);
+#pragma unroll
+        for (int e = 0; e < EPT; ++e)
+            pair_f64(pe[3 * e], pe[3 * e + 1], pe[3 * e + 2], a.x, a.y, b.x, b.y, V[e], Ex[e], Ey[e],
+                     Ez[e]);
+    }
+}
+
+// a4, cross-CTA part: the paper adds the block sums B[1..N_B] "by reduction" (PAPER.md:132,
+// Eq. 5).  Each CTA has stored its partial; the CTA that takes the LAST ticket of its point
+// block (an integer atomic; no floating-point atomics anywhere) adds the slices in a fixed
+// order -- lane-strided, then the butterfly -- so the result does not depend on which CTA
+// that is.  NT threads (whole warps) call this; sync() is their barrier.
+template <int NT, typename SYNC>
+__device__ __forceinline__ void finish_point_block(const PairParams &prm, int ppb, int tid,
+                                                   int *flag, double *scratch /*[NT]*/, SYNC sync) {
+    __threadfence();                                   // this CTA's partials are visible
+    sync();
+    if (tid == 0) *flag = atomicAdd(prm.counters + blockIdx.x, 1) == prm.slices - 1;
+    sync();
+    if (!*flag) return;
+    __threadfence();
+    // thread = (group g, value v): nval = 4*ppb values {V,Ex,Ey,Ez} x points (a power of two
+    // <= NT); group g adds slices g, g+G, g+2G, ... on four interleaved accumulators (all
+    // loads independent and coalesced over v), then the G groups are added in index order.
+    const int nval = 4 * ppb, G = NT / nval;
+    const int v = tid % nval, g = tid / nval;
+    const int p = blockIdx.x * ppb + v / 4;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    if (p < prm.P) {
+        const double *src = prm.partial + static_cast<int64_t>(p) * 4 + (v & 3);
+        const int64_t stride = static_cast<int64_t>(prm.P) * 4;
+        int sidx = g;
+        for (; sidx + 3 * G < prm.slices; sidx += 4 * G) {
+            a0 += __ldcg(src + (sidx) * stride);
+            a1 += __ldcg(src + (sidx + G) * stride);
+            a2 += __ldcg(src + (sidx + 2 * G) * stride);
+            a3 += __ldcg(src + (sidx + 3 * G) * stride);
+        }
+        for (; sidx < prm.slices; sidx += G) a0 += __ldcg(src + sidx * stride);
+    }
+    scratch[tid] = (a0 + a1) + (a2 + a3);
+    sync();
+    if (g == 0 && p < prm.P) {
+        double a = 0.0;
+        for (int k = 0; k < G; ++k) a += scratch[k * nval + v];
+        if ((v & 3) == 0) prm.V[p] = a;
+        else if (prm.E) prm.E[3 * static_cast<int64_t>(p) + (v & 3) - 1] = a;
+    }
+    if (tid == 0) prm.counters[blockIdx.x] = 0;        // ready for the next evaluation
+}
+
 // ----------------------------------------------------------------------------- pair kernel
 // grid = (point_blocks, slices).  REAL = double (FP64 path) or float (FP32-acc64 path).
 template <typename REAL, int EPT>
@@ -185,8 +256,9 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
     const int stages = prm.stages;
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + static_cast<size_t>(stages) * STAGE_BYTES);
     uint64_t *empty = full + 8;
-    double *red = reinterpret_cast<double *>(empty + 8);   // [COMPUTE_WARPS][EPT*4]
-    double *elec_s = red + COMPUTE_WARPS * EPT * 4;          // [WP*EPT][3]
+    int *flag = reinterpret_cast<int *>(empty + 8);        // last-CTA flag (16 bytes reserved)
+    double *red = reinterpret_cast<double *>(empty + 10);  // [COMPUTE_WARPS][EPT*4]
+    double *elec_s = red + 32 * COMPUTE_WARPS;               // [WP*EPT][3]; red has one double per thread
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int WP = prm.point_warps, WS = COMPUTE_WARPS / WP;
@@ -329,6 +401,9 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
         ++k;
     }
 
+    // FP64 path: the nuclei are ordinary sources at the end of the FP64 chunk array
+    if constexpr (F32) nuclei_share<EPT>(prm, elec_s + wp * EPT * 3, ws, WS, lane, V, Ex, Ey, Ez);
+
     // ---- in-CTA reduction (paper: shared memory; here shuffle + smem) ----
 #pragma unroll
     for (int e = 0; e < EPT; ++e) {
@@ -353,6 +428,8 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
         if (p < prm.P)
             prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] = acc;
     }
+    finish_point_block<32 * COMPUTE_WARPS>(prm, WP * EPT, threadIdx.x, flag, red,
+                                           [] { compute_warps_sync(); });
 }
 
 // ----------------------------------------------------------------------------- FP32 packed
@@ -429,7 +506,7 @@ struct F32x2Layout {
     static constexpr int NT = 32 * NW;
     static constexpr int CHUNK_BYTES = 4 * CHUNK * sizeof(float);
     static constexpr int STAGE_BYTES = STAGE_HDR + BLOCK_CHUNKS * CHUNK_BYTES;
-    static constexpr int BAR_BYTES = 16 * sizeof(uint64_t);
+    static constexpr int BAR_BYTES = 18 * sizeof(uint64_t);     // 8 full, 8 empty, last-CTA flag
     static constexpr int ELEC_BYTES = NW * EPT * 3 * sizeof(double);
     static constexpr int SCRATCH_BYTES = NW * 2 * 3 * EPT * sizeof(float);
     static constexpr int ACC_BYTES = EPT * 4 * NT * sizeof(double);
@@ -450,6 +527,7 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
     unsigned char *ptr = smem + static_cast<size_t>(stages) * STAGE_BYTES;
     uint64_t *full = reinterpret_cast<uint64_t *>(ptr);
     uint64_t *empty = full + 8;
+    int *flag = reinterpret_cast<int *>(empty + 8);
     ptr += L::BAR_BYTES;
     double *elec_s = reinterpret_cast<double *>(ptr);          // [WP*EPT][3]
     ptr += L::ELEC_BYTES;
@@ -584,6 +662,22 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
         }
     }
 
+    // nuclear term of this CTA's share, FP64, into the same columns
+    {
+        double nV[EPT], nEx[EPT], nEy[EPT], nEz[EPT];
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) nV[e] = nEx[e] = nEy[e] = nEz[e] = 0.0;
+        nuclei_share<EPT>(prm, pe, ws, WS, lane, nV, nEx, nEy, nEz);
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+            double2 t;
+            t = my[(4 * e + 0) * NT]; t.x += nV[2 * e]; t.y += nV[2 * e + 1]; my[(4 * e + 0) * NT] = t;
+            t = my[(4 * e + 1) * NT]; t.x += nEx[2 * e]; t.y += nEx[2 * e + 1]; my[(4 * e + 1) * NT] = t;
+            t = my[(4 * e + 2) * NT]; t.x += nEy[2 * e]; t.y += nEy[2 * e + 1]; my[(4 * e + 2) * NT] = t;
+            t = my[(4 * e + 3) * NT]; t.x += nEz[2 * e]; t.y += nEz[2 * e + 1]; my[(4 * e + 3) * NT] = t;
+        }
+    }
+
     // ---- in-CTA reduction: fixed-order butterfly per value, then the WS partners in order ----
     // column row 4e+comp holds {V,Ex,Ey,Ez}[comp] of points (2e, 2e+1); lane 4*point+comp of
     // the warp keeps the reduced value.
@@ -606,79 +700,29 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
         if (p < prm.P)
             prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] = a;
     }
-}
-
-// ----------------------------------------------------------------------------- finalize
-// Adds the slice partials in index order, then the nuclear term (always FP64, PAPER.md:117
-// keeps U_nuc in double), and writes V, E.  TPP threads cooperate on one point.
-struct FinalizeParams {
-    const double *partial;   // [slices][P][4]
-    const double *nuc;       // [K][4] packed x, y, z, Z
-    const double *elec;      // [P][3]
-    double *V;               // [P]
-    double *E;               // [P][3] or NULL
-    int P, slices, K, tpp;   // tpp: 32 or 256 threads per point
-};
-
-__global__ void __launch_bounds__(256) finalize_kernel(const FinalizeParams prm) {
-    __shared__ double red[8][4];
-    const int tpp = prm.tpp;
-    const int per_cta = 256 / tpp;
-    const int sub = threadIdx.x / tpp, t = threadIdx.x % tpp;
-    const int p = blockIdx.x * per_cta + sub;
-    const bool live = p < prm.P;
-    const int pc = live ? p : prm.P - 1;
-    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-    for (int s = t; s < prm.slices; s += tpp) {
-        const double4 v = *reinterpret_cast<const double4 *>(
-            prm.partial + (static_cast<int64_t>(s) * prm.P + pc) * 4);
-        a0 += v.x; a1 += v.y; a2 += v.z; a3 += v.w;
-    }
-    const double rx = prm.elec[3 * static_cast<int64_t>(pc) + 0];
-    const double ry = prm.elec[3 * static_cast<int64_t>(pc) + 1];
-    const double rz = prm.elec[3 * static_cast<int64_t>(pc) + 2];
-    for (int j = t; j < prm.K; j += tpp) {
-        const double4 n = *reinterpret_cast<const double4 *>(prm.nuc + 4 * static_cast<int64_t>(j));
-        pair_f64(rx, ry, rz, n.x, n.y, n.z, n.w, a0, a1, a2, a3);
-    }
-    a0 = warp_sum(a0); a1 = warp_sum(a1); a2 = warp_sum(a2); a3 = warp_sum(a3);
-    if (tpp == 256) {
-        const int w = threadIdx.x >> 5;
-        if ((threadIdx.x & 31) == 0) { red[w][0] = a0; red[w][1] = a1; red[w][2] = a2; red[w][3] = a3; }
-        __syncthreads();
-        if (threadIdx.x < 4) {
-            double acc = 0.0;
-            for (int i = 0; i < 8; ++i) acc += red[i][threadIdx.x];
-            if (threadIdx.x == 0) prm.V[p] = acc;
-            else if (prm.E) prm.E[3 * static_cast<int64_t>(p) + threadIdx.x - 1] = acc;
-        }
-    } else if (live && t == 0) {
-        prm.V[p] = a0;
-        if (prm.E) {
-            prm.E[3 * static_cast<int64_t>(p) + 0] = a1;
-            prm.E[3 * static_cast<int64_t>(p) + 1] = a2;
-            prm.E[3 * static_cast<int64_t>(p) + 2] = a3;
-        }
-    }
+    finish_point_block<NT>(prm, WP * EPT, threadIdx.x, flag, red, [] { __syncthreads(); });
 }
 
 // ----------------------------------------------------------------------------- packing
 // a0: pack {R_j, q_j} once per environment.
 // Pads (j >= M) replicate the last real source with charge 0: they contribute exactly 0.
-__global__ void pack_f64_kernel(const double *xyz, const double *q, int64_t M, int64_t Mpad,
+__global__ void pack_f64_kernel(const double *xyz, const double *q, int64_t M,
+                                const double *nuc_xyz, const double *nuc_Z, int64_t K, int64_t Mpad,
                                 double *chunks) {
     const int64_t j = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x;
     if (j >= Mpad) return;
-    const int64_t src = j < M ? j : M - 1;
-    const int64_t ch = j / CHUNK;
+    // FP64 copy: the M cells, then the K nuclei (charge +Z) as ordinary sources; pads replicate
+    // the last real entry with charge 0.
+    const int64_t jj = j < M + K ? j : M + K - 1;
+    const bool cell = jj < M;
+    const double *pos = cell ? xyz + 3 * jj : nuc_xyz + 3 * (jj - M);
+    const double charge = j < M + K ? (cell ? q[jj] : nuc_Z[jj - M]) : 0.0;
+    double *c = chunks + (j / CHUNK) * 4 * CHUNK;
     const int i = static_cast<int>(j % CHUNK);
-    // within a chunk the FP64 consumer reads element pairs (2l, 2l+1) and (64+2l, 64+2l+1):
-    // storage order is the natural one.
-    double *c = chunks + ch * 4 * CHUNK;
-    c[i] = xyz[3 * src + 0];
-    c[CHUNK + i] = xyz[3 * src + 1];
-    c[2 * CHUNK + i] = xyz[3 * src + 2];
-    c[3 * CHUNK + i] = j < M ? q[src] : 0.0;
+    c[i] = pos[0];
+    c[CHUNK + i] = pos[1];
+    c[2 * CHUNK + i] = pos[2];
+    c[3 * CHUNK + i] = charge;
 }
 
 // Bounding box of all sources: CTA b writes {lo[3], hi[3]} to part[6b..]; the host finishes.
