@@ -187,11 +187,11 @@ def probe_peaks(B):
     return {"ffma_lane_ops_per_s": ffma, "dfma_lane_ops_per_s": dfma, "mufu_lane_ops_per_s": mufu}
 
 
-def time_steps(torch, B, h, batches, W, N, prec, steps, warmup, flush, stream):
+def time_steps(torch, B, h, batches, W, N, prec, steps, warmup, flush, stream, want_E=True):
     """Per-step CUDA events on the launch stream; returns (step_ms list, pair_ms list)."""
     P = W * N
     V = torch.empty(P, dtype=torch.float64, device="cuda")
-    E = torch.empty((P, 3), dtype=torch.float64, device="cuda")
+    E = torch.empty((P, 3), dtype=torch.float64, device="cuda") if want_E else None
     for i in range(warmup):
         B.qmmm_field_eval(h, batches[i % len(batches)], W, N, V, E, prec, stream)
     torch.cuda.synchronize()
@@ -262,6 +262,20 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                     row["source_bytes_per_eval"] = bytes_eval
                     row["source_GBps_back_to_back"] = bytes_eval / (row["us_per_eval_1000_back_to_back"] * 1e-6) / 1e9
                 out.append(row)
+                if prec == "fp64" and not w.sequential and idx in (1, 4):
+                    # potential only (E = NULL): the paper's own computation, Eq. 4; 13 DP slots
+                    B.qmmm_field_set_timing(h, True)
+                    step_ms, pair_ms, _ = time_steps(torch, B, h, batches, W, N, prec, reps, 3, flush,
+                                                     stream, want_E=False)
+                    out.append({"config": idx, "name": w.name, "precision": "fp64 potential-only",
+                                "points": P, "M": w.M, "K": w.K, "pairs_per_eval": pairs,
+                                "ms_per_eval_median": float(np.median(step_ms)),
+                                "ms_per_eval_min": float(np.min(step_ms)),
+                                "pair_kernel_ms_median": float(np.median(pair_ms)),
+                                "gpairs_per_s": pairs / np.median(step_ms) / 1e6,
+                                "fma_pipe_frac": pairs * 13 / (np.median(step_ms) * 1e-3) / peak,
+                                "slots_per_pair": 13,
+                                "plan": B.qmmm_field_get_info(h)["last_plan"]})
         finally:
             B.qmmm_field_destroy(h)
         del w

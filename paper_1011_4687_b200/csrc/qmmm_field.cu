@@ -116,9 +116,9 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32) {
     return pl;
 }
 
-template <typename REAL, int EPT>
+template <typename REAL, int EPT, bool WITH_E = true>
 cudaError_t launch_pair(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
-    auto kern = pair_kernel<REAL, EPT>;
+    auto kern = pair_kernel<REAL, EPT, WITH_E>;
     static thread_local size_t configured = 0;
     if (smem > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -155,11 +155,17 @@ cudaError_t launch_pair_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
             case 4: return launch_pair_f32x2<2, F32X2_NW_EPT4>(prm, grid, smem, st);
             case 8: return launch_pair_f32x2<4, F32X2_NW_EPT8>(prm, grid, smem, st);
         }
-    } else {
+    } else if (prm.E) {
         switch (ept) {
             case 1: return launch_pair<double, 1>(prm, grid, smem, st);
             case 2: return launch_pair<double, 2>(prm, grid, smem, st);
             case 4: return launch_pair<double, 4>(prm, grid, smem, st);
+        }
+    } else {      // E == NULL: potential only (Eq. 4 is the potential alone)
+        switch (ept) {
+            case 1: return launch_pair<double, 1, false>(prm, grid, smem, st);
+            case 2: return launch_pair<double, 2, false>(prm, grid, smem, st);
+            case 4: return launch_pair<double, 4, false>(prm, grid, smem, st);
         }
     }
     return cudaErrorInvalidValue;

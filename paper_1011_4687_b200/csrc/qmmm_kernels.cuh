@@ -139,6 +139,14 @@ __device__ __forceinline__ void pair_f64(double rx, double ry, double rz, double
     Ez = fma(s, dz, Ez);
 }
 
+// Potential only (the paper's own computation, Eq. 4): 13 DP-pipe instructions + 1 MUFU.
+__device__ __forceinline__ void pair_f64_v(double rx, double ry, double rz, double sx, double sy,
+                                           double sz, double q, double &V) {
+    double dx = rx - sx, dy = ry - sy, dz = rz - sz;
+    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    V = fma(q, rsqrt_refined_f64(r2), V);
+}
+
 // One FP32 pair: 17 FP32-pipe instructions + 1 MUFU.RSQ (MUFU seed + one Newton step).
 __device__ __forceinline__ void pair_f32(float ax, float ay, float az, float ox, float oy,
                                          float oz, float q, float &V, float &Ex, float &Ey,
@@ -244,7 +252,7 @@ __device__ __forceinline__ void finish_point_block(const PairParams &prm, int pp
 
 // ----------------------------------------------------------------------------- pair kernel
 // grid = (point_blocks, slices).  REAL = double (FP64 path) or float (FP32-acc64 path).
-template <typename REAL, int EPT>
+template <typename REAL, int EPT, bool WITH_E = true>
 __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams prm) {
     constexpr bool F32 = sizeof(REAL) == 4;
     constexpr int CHUNK_BYTES = 4 * CHUNK * sizeof(REAL);
@@ -389,8 +397,13 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
                     const double2 Q = *reinterpret_cast<const double2 *>(b + 3 * CHUNK + half * 64);
 #pragma unroll
                     for (int e = 0; e < EPT; ++e) {
-                        pair_f64(rx[e], ry[e], rz[e], X.x, Y.x, Z.x, Q.x, V[e], Ex[e], Ey[e], Ez[e]);
-                        pair_f64(rx[e], ry[e], rz[e], X.y, Y.y, Z.y, Q.y, V[e], Ex[e], Ey[e], Ez[e]);
+                        if constexpr (WITH_E) {
+                            pair_f64(rx[e], ry[e], rz[e], X.x, Y.x, Z.x, Q.x, V[e], Ex[e], Ey[e], Ez[e]);
+                            pair_f64(rx[e], ry[e], rz[e], X.y, Y.y, Z.y, Q.y, V[e], Ex[e], Ey[e], Ez[e]);
+                        } else {
+                            pair_f64_v(rx[e], ry[e], rz[e], X.x, Y.x, Z.x, Q.x, V[e]);
+                            pair_f64_v(rx[e], ry[e], rz[e], X.y, Y.y, Z.y, Q.y, V[e]);
+                        }
                     }
                 }
             }
