@@ -97,7 +97,14 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32) {
     pl.points_per_thread = std::min(pl.points_per_thread, max_ept);
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
     const int nw = (f32 && pl.points_per_thread >= 2) ? f32x2_warps(pl.points_per_thread) : COMPUTE_WARPS;
-    if (pl.point_warps == 0) pl.point_warps = std::min<int>(nw, pow2_ceil(groups));
+    if (pl.point_warps == 0) {
+        // as many point warps as there are groups, but keep at least 4 point blocks when the
+        // points allow it: slices = SMs / 4 then, so every CTA streams a 4x longer source run
+        // through its TMA ring and the last CTA adds 4x fewer partials per point
+        int pw = std::min<int>(nw, pow2_ceil(groups));
+        while (pw > 1 && (groups + pw - 1) / pw < 4) pw >>= 1;
+        pl.point_warps = pw;
+    }
     if (pl.point_warps > nw) pl.point_warps = nw;
     const int64_t pb = (groups + pl.point_warps - 1) / pl.point_warps;
     if (pl.slices == 0) {
@@ -429,6 +436,9 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
         prm.V = V;
         prm.E = E;
         prm.counters = h->counters;
+#ifdef QMMM_PHASE_TIMING
+        prm.dbg = reinterpret_cast<long long *>(h->workspace + h->workspace_doubles - 16384);
+#endif
         // point blocks vary fastest: the CTAs resident together read the same source slices,
         // so a slice is fetched from HBM once and then served from L2
         const dim3 grid(pb, pl.slices);
@@ -474,5 +484,15 @@ qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int
     CUDA_TRY(cudaStreamSynchronize(st));
     return QMMM_OK;
 }
+
+#ifdef QMMM_PHASE_TIMING
+// Diagnostic build only: per-CTA phase clocks of the most recent packed-kernel launch.
+qmmm_status qmmm_debug_phases(qmmm_field *h, long long *out, int n) {
+    CUDA_TRY(cudaDeviceSynchronize());
+    CUDA_TRY(cudaMemcpy(out, h->workspace + h->workspace_doubles - 16384, n * sizeof(long long),
+                        cudaMemcpyDeviceToHost));
+    return QMMM_OK;
+}
+#endif
 
 }  // extern "C"

@@ -47,9 +47,30 @@ struct PairParams {
     double *V;               // [P]       final outputs, written by the last CTA of a point block
     double *E;               // [P][3] or NULL
     int *counters;           // [point_blocks] arrival tickets, zero between evaluations
+#ifdef QMMM_PHASE_TIMING
+    long long *dbg;          // [CTAs][10] clock64 at phase boundaries + globaltimer (diagnostic build)
+#endif
 };
 
 // ----------------------------------------------------------------------------- PTX helpers
+#ifdef QMMM_PHASE_TIMING
+#define QMMM_MARK(i)                                                                          \
+    do {                                                                                      \
+        if (threadIdx.x == 0)                                                                 \
+            prm.dbg[(blockIdx.y * gridDim.x + blockIdx.x) * 10 + (i)] = clock64();            \
+    } while (0)
+#define QMMM_MARK_GT(i)                                                                       \
+    do {                                                                                      \
+        if (threadIdx.x == 0) {                                                               \
+            long long t;                                                                      \
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));                             \
+            prm.dbg[(blockIdx.y * gridDim.x + blockIdx.x) * 10 + (i)] = t;                    \
+        }                                                                                     \
+    } while (0)
+#else
+#define QMMM_MARK(i) do {} while (0)
+#define QMMM_MARK_GT(i) do {} while (0)
+#endif
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
@@ -221,25 +242,26 @@ __device__ __forceinline__ void finish_point_block(const PairParams &prm, int pp
     if (!*flag) return;
     __threadfence();
     // thread = (group g, value v): nval = 4*ppb values {V,Ex,Ey,Ez} x points (a power of two
-    // <= NT); group g adds slices g, g+G, g+2G, ... on four interleaved accumulators (all
+    // <= NT); group g adds slices g, g+G, g+2G, ... on eight interleaved accumulators (all
     // loads independent and coalesced over v), then the G groups are added in index order.
     const int nval = 4 * ppb, G = NT / nval;
     const int v = tid % nval, g = tid / nval;
     const int p = blockIdx.x * ppb + v / 4;
-    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    double a[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};   // 8 loads in flight per thread
     if (p < prm.P) {
         const double *src = prm.partial + static_cast<int64_t>(p) * 4 + (v & 3);
         const int64_t stride = static_cast<int64_t>(prm.P) * 4;
         int sidx = g;
-        for (; sidx + 3 * G < prm.slices; sidx += 4 * G) {
-            a0 += __ldcg(src + (sidx) * stride);
-            a1 += __ldcg(src + (sidx + G) * stride);
-            a2 += __ldcg(src + (sidx + 2 * G) * stride);
-            a3 += __ldcg(src + (sidx + 3 * G) * stride);
+        for (; sidx + 7 * G < prm.slices; sidx += 8 * G) {
+            double t[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) t[k] = __ldcg(src + (sidx + k * G) * stride);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) a[k] += t[k];
         }
-        for (; sidx < prm.slices; sidx += G) a0 += __ldcg(src + sidx * stride);
+        for (int k = 0; sidx < prm.slices; sidx += G, ++k) a[k] += __ldcg(src + sidx * stride);
     }
-    scratch[tid] = (a0 + a1) + (a2 + a3);
+    scratch[tid] = ((a[0] + a[1]) + (a[2] + a[3])) + ((a[4] + a[5]) + (a[6] + a[7]));
     sync();
     if (g == 0 && p < prm.P) {
         double a = 0.0;
@@ -536,6 +558,8 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
     constexpr int CHUNK_BYTES = L::CHUNK_BYTES, STAGE_BYTES = L::STAGE_BYTES;
 
     extern __shared__ __align__(128) unsigned char smem[];
+    QMMM_MARK_GT(8);
+    QMMM_MARK(0);
     const int stages = prm.stages;
     unsigned char *ptr = smem + static_cast<size_t>(stages) * STAGE_BYTES;
     uint64_t *full = reinterpret_cast<uint64_t *>(ptr);
@@ -567,6 +591,7 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
         elec_s[i] = prm.elec[static_cast<int64_t>(p) * 3 + (i % 3)];
     }
     __syncthreads();
+    QMMM_MARK(1);
 
     // ---- producer cursor (warp 0 only): next pipeline step to load -------------------------
     int pc = lo, pslot = 0;
@@ -604,6 +629,7 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
 
     int slot = 0;
     uint32_t phase = 0;
+    QMMM_MARK(2);
     for (int c = lo; c < hi;) {
         const int ce = stage_end(c, hi);
         if (warp == 0) produce();          // step k + stages - 1 into the slot freed by step k - 1
@@ -675,6 +701,7 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
         }
     }
 
+    QMMM_MARK(3);
     // nuclear term of this CTA's share, FP64, into the same columns
     {
         double nV[EPT], nEx[EPT], nEy[EPT], nEz[EPT];
@@ -691,20 +718,29 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
         }
     }
 
-    // ---- in-CTA reduction: fixed-order butterfly per value, then the WS partners in order ----
-    // column row 4e+comp holds {V,Ex,Ey,Ez}[comp] of points (2e, 2e+1); lane 4*point+comp of
-    // the warp keeps the reduced value.
+    QMMM_MARK(4);
+    // ---- in-CTA reduction through shared memory (paper: PAPER.md:132) ------------------------
+    // Column row i = 4e+comp holds {V,Ex,Ey,Ez}[comp] of points (2e, 2e+1) for every thread.
+    // Lane r < 2*EPT of each warp adds row r over the warp's 32 columns, starting at column r
+    // (a rotation: the 32 lanes touch 32 different 16-byte slots, so the loads are conflict-
+    // free and the order is fixed).  10x fewer instructions than 64 butterflies of shuffles.
     double *red = reinterpret_cast<double *>(acc);   // reused after the barrier: [NW][EPT*4]
-    double mine = 0.0;
-#pragma unroll
-    for (int i = 0; i < EPT * 2; ++i) {
-        const double2 t = my[i * NT];
-        const double sx = warp_sum(t.x), sy = warp_sum(t.y);
-        if (lane == 8 * (i / 4) + (i & 3)) mine = sx;
-        if (lane == 8 * (i / 4) + 4 + (i & 3)) mine = sy;
+    double2 tot = make_double2(0.0, 0.0);
+    __syncwarp();
+    if (lane < 2 * EPT) {
+        const double2 *row = acc + lane * NT + warp * 32;
+#pragma unroll 8
+        for (int j = 0; j < 32; ++j) {
+            const double2 t = row[(j + lane) & 31];
+            tot.x += t.x;
+            tot.y += t.y;
+        }
     }
     __syncthreads();                                 // every column has been read
-    if (lane < EPT * 4) red[warp * EPT * 4 + lane] = mine;
+    if (lane < 2 * EPT) {                            // row 4e+comp -> values 8e+comp, 8e+4+comp
+        red[warp * EPT * 4 + 8 * (lane >> 2) + (lane & 3)] = tot.x;
+        red[warp * EPT * 4 + 8 * (lane >> 2) + 4 + (lane & 3)] = tot.y;
+    }
     __syncthreads();
     if (ws == 0 && lane < EPT * 4) {
         double a = 0.0;
@@ -713,7 +749,10 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
         if (p < prm.P)
             prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] = a;
     }
+    QMMM_MARK(5);
     finish_point_block<NT>(prm, WP * EPT, threadIdx.x, flag, red, [] { __syncthreads(); });
+    QMMM_MARK(6);
+    QMMM_MARK_GT(9);
 }
 
 // ----------------------------------------------------------------------------- packing
