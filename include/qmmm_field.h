@@ -90,14 +90,30 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
                             double *V, double *E, int prec, void *stream);
 
 /*
- * qmmm_field_eval_host -- the paper's per-step loop: HOST buffers
- * in and out.  Copies elec_xyz host->device, evaluates, copies V (and E) back on
- * `stream`, and synchronises the stream before returning.  Buffers may be pageable
- * or pinned.  Same argument meaning and errors as qmmm_field_eval.
+ * qmmm_field_eval_host -- the paper's per-step call: HOST buffers in and out;
+ * returns when V_host (and E_host) hold the result.  Buffers may be pageable or pinned.
+ * Up to 64 points go through a pinned, device-mapped mailbox owned by the handle: the kernel
+ * reads the points from it and the last CTA writes V, E and a sequence number back, which
+ * the host waits for -- no cudaMemcpy, no stream synchronisation.  More points: host->device
+ * copy, kernel, device->host copy on `stream`, stream synchronisation.
+ * Same argument meaning and errors as qmmm_field_eval.
  */
 qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int64_t W,
                                  int64_t N, double *V_host, double *E_host, int prec,
                                  void *stream);
+
+/*
+ * qmmm_field_eval_moves_host -- n successive single-configuration evaluations, the loop the
+ * paper deploys (every Monte-Carlo step sends r_new and receives U_ES).  Step s
+ * evaluates the N points elec_xyz_host[s][N][3] and writes V_host[s][N] (and E_host[s][N][3]
+ * unless NULL) through the same per-move path as qmmm_field_eval_host with W = 1; the steps
+ * are strictly sequential (step s+1 starts after the host has received step s), as in a
+ * Metropolis walk where the next proposal depends on the last result.  *seconds (may be
+ * NULL) receives the host wall-clock time of the whole loop.  Same errors as eval_host.
+ */
+qmmm_status qmmm_field_eval_moves_host(qmmm_field *h, const double *elec_xyz_host, int64_t n,
+                                       int64_t N, double *V_host, double *E_host, int prec,
+                                       void *stream, double *seconds);
 
 /* qmmm_field_destroy -- frees the handle and its device buffers.  NULL is a no-op. */
 qmmm_status qmmm_field_destroy(qmmm_field *h);

@@ -26,6 +26,7 @@ _STATUS = {0: "QMMM_OK", 1: "QMMM_ERR_INVALID_ARG", 2: "QMMM_ERR_ALLOC", 3: "QMM
 LIB_PATH = os.environ.get("QMMM_FIELD_LIB") or os.path.join(
     os.path.dirname(os.path.abspath(__file__)), "libqmmm_field.so")
 EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_host",
+                    "qmmm_field_eval_moves_host",
                     "qmmm_field_destroy", "qmmm_field_set_plan", "qmmm_field_get_info",
                     "qmmm_field_set_timing", "qmmm_field_last_timing",
                     "qmmm_probe_peak", "qmmm_last_error")
@@ -64,6 +65,9 @@ def _load() -> ctypes.CDLL:
     lib.qmmm_field_eval.argtypes = [vp, vp, i64, i64, vp, vp, ci, vp]
     lib.qmmm_field_eval_host.restype = ci
     lib.qmmm_field_eval_host.argtypes = [vp, vp, i64, i64, vp, vp, ci, vp]
+    lib.qmmm_field_eval_moves_host.restype = ci
+    lib.qmmm_field_eval_moves_host.argtypes = [vp, vp, i64, i64, vp, vp, ci, vp,
+                                               ctypes.POINTER(ctypes.c_double)]
     lib.qmmm_field_destroy.restype = ci
     lib.qmmm_field_destroy.argtypes = [vp]
     lib.qmmm_field_set_plan.restype = ci
@@ -132,6 +136,17 @@ def qmmm_field_eval_host(handle: int, elec_xyz, W: int, N: int, V, E=None, preci
     """Per-step host loop of PAPER.md:117: host buffers in/out, synchronises the stream."""
     _check(_lib.qmmm_field_eval_host(handle, _ptr(elec_xyz), int(W), int(N), _ptr(V), _ptr(E),
                                      _PREC[precision], _stream(stream)))
+
+
+def qmmm_field_eval_moves_host(handle: int, elec_xyz, n: int, N: int, V, E=None, precision="fp64",
+                               stream=None) -> float:
+    """n sequential single-configuration evaluations through the per-move path (the paper's
+    deployed loop); host arrays elec_xyz [n,N,3], V [n,N], E [n,N,3].  Returns
+    the host wall-clock seconds of the loop."""
+    secs = ctypes.c_double()
+    _check(_lib.qmmm_field_eval_moves_host(handle, _ptr(elec_xyz), int(n), int(N), _ptr(V), _ptr(E),
+                                           _PREC[precision], _stream(stream), ctypes.byref(secs)))
+    return secs.value
 
 
 def qmmm_field_destroy(handle: Optional[int]) -> None:

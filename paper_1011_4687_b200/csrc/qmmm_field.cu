@@ -10,9 +10,11 @@
 #include "qmmm_kernels.cuh"
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <ctime>
 #include <new>
 #include <string>
 
@@ -46,6 +48,8 @@ int gcd_int(int a, int b) {
     while (b) { int t = a % b; a = b; b = t; }
     return a;
 }
+
+constexpr int MAIL_POINTS = 64;   // eval_host uses the zero-copy mailbox up to this many points
 
 constexpr size_t stage_bytes(bool f32) {
     return STAGE_HDR + (f32 ? static_cast<size_t>(BLOCK_CHUNKS) * 4 * CHUNK * 4
@@ -83,6 +87,9 @@ struct qmmm_field {
     int last_point_blocks = 0, last_launches = 0;
     bool timing = false, timed = false;
     cudaEvent_t ev[2] = {nullptr, nullptr};
+    // per-move mailbox: pinned, device-mapped host memory (elec in; V, E and a sequence flag out)
+    double *mail_h = nullptr, *mail_d = nullptr;   // [MAIL_POINTS*3 | MAIL_POINTS*4 | flag]
+    unsigned long long seq = 0;
     int *counters = nullptr;       // [max_points] arrival tickets of the point blocks (zero at rest)
 };
 
@@ -319,8 +326,11 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
     h->workspace_doubles =
         4 * std::max<int64_t>(static_cast<int64_t>(h->sm_count) * max_points, int64_t(1) << 16);
     CREATE_TRY(cudaMalloc(&h->workspace, h->workspace_doubles * sizeof(double)));
-    CREATE_TRY(cudaMalloc(&h->counters, max_points * sizeof(int)));
-    CREATE_TRY(cudaMemset(h->counters, 0, max_points * sizeof(int)));
+    CREATE_TRY(cudaMalloc(&h->counters, (max_points + 1) * sizeof(int)));      // + 1: mailbox `done`
+    CREATE_TRY(cudaMemset(h->counters, 0, (max_points + 1) * sizeof(int)));
+    CREATE_TRY(cudaHostAlloc(&h->mail_h, (MAIL_POINTS * 7 + 1) * sizeof(double), cudaHostAllocMapped));
+    std::memset(h->mail_h, 0, (MAIL_POINTS * 7 + 1) * sizeof(double));
+    CREATE_TRY(cudaHostGetDevicePointer(&h->mail_d, h->mail_h, 0));
     CREATE_TRY(cudaMalloc(&h->stage_elec, max_points * 3 * sizeof(double)));
     CREATE_TRY(cudaMalloc(&h->stage_out, max_points * 4 * sizeof(double)));
 #undef CREATE_TRY
@@ -336,6 +346,7 @@ qmmm_status qmmm_field_destroy(qmmm_field *h) {
     cudaFree(h->nuclei);
     cudaFree(h->workspace);
     cudaFree(h->counters);
+    if (h->mail_h) cudaFreeHost(h->mail_h);
     cudaFree(h->stage_elec);
     cudaFree(h->stage_out);
     for (cudaEvent_t e : h->ev)
@@ -395,8 +406,11 @@ qmmm_status qmmm_field_get_info(const qmmm_field *h, qmmm_field_info *info) {
     return QMMM_OK;
 }
 
-qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t N,
-                            double *V, double *E, int prec, void *stream) {
+}  // extern "C"
+
+namespace {
+qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t N, double *V,
+                      double *E, int prec, void *stream, unsigned long long *host_flag) {
     if (!h) return fail(QMMM_ERR_INVALID_ARG, "eval: NULL handle");
     if (!elec_xyz || !V) return fail(QMMM_ERR_INVALID_ARG, "eval: NULL elec_xyz or V");
     if (W < 1 || N < 1 || W > h->max_points || N > h->max_points || W * N > h->max_points)
@@ -436,6 +450,9 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
         prm.V = V;
         prm.E = E;
         prm.counters = h->counters;
+        prm.host_flag = host_flag;
+        prm.seq = h->seq;
+        prm.done = h->counters + h->max_points;
 #ifdef QMMM_PHASE_TIMING
         prm.dbg = reinterpret_cast<long long *>(h->workspace + h->workspace_doubles - 16384);
 #endif
@@ -456,6 +473,14 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
     h->last_launches = launches;
     return QMMM_OK;
 }
+}  // namespace
+
+extern "C" {
+
+qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t N,
+                            double *V, double *E, int prec, void *stream) {
+    return eval_impl(h, elec_xyz, W, N, V, E, prec, stream, nullptr);
+}
 
 qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int64_t W,
                                  int64_t N, double *V_host, double *E_host, int prec,
@@ -467,10 +492,37 @@ qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int
         return fail(QMMM_ERR_INVALID_ARG, "eval_host: W*N must be in [1, max_points]");
     const int64_t P = W * N;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (P <= MAIL_POINTS) {
+        // Per-move path ("r_new" in, U_ES out, every Monte-Carlo step): no
+        // cudaMemcpy and no stream synchronisation.  The kernel reads the points from a
+        // pinned, device-mapped mailbox, the CTA that finishes last writes V, E and then a
+        // sequence number into it, and the host waits for that number.
+        double *in_h = h->mail_h, *out_h = h->mail_h + MAIL_POINTS * 3;
+        volatile unsigned long long *flag_h =
+            reinterpret_cast<volatile unsigned long long *>(h->mail_h + MAIL_POINTS * 7);
+        double *in_d = h->mail_d, *out_d = h->mail_d + MAIL_POINTS * 3;
+        std::memcpy(in_h, elec_xyz_host, P * 3 * sizeof(double));
+        ++h->seq;
+        qmmm_status s = eval_impl(h, in_d, W, N, out_d, E_host ? out_d + P : nullptr, prec, stream,
+                                  reinterpret_cast<unsigned long long *>(h->mail_d + MAIL_POINTS * 7));
+        if (s != QMMM_OK) return s;
+        for (uint64_t spin = 1; *flag_h != h->seq; ++spin) {
+            if ((spin & 0xFFFF) == 0) {                   // now and then: did the launch fail?
+                cudaError_t q = cudaStreamQuery(st);
+                if (q != cudaSuccess && q != cudaErrorNotReady) return cuda_fail(q, "eval_host: kernel");
+                if (q == cudaSuccess && *flag_h != h->seq)
+                    return fail(QMMM_ERR_CUDA, "eval_host: kernel finished without publishing its result");
+            }
+        }
+        std::atomic_thread_fence(std::memory_order_acquire);
+        std::memcpy(V_host, out_h, P * sizeof(double));
+        if (E_host) std::memcpy(E_host, out_h + P, P * 3 * sizeof(double));
+        return QMMM_OK;
+    }
     CUDA_TRY(cudaMemcpyAsync(h->stage_elec, elec_xyz_host, P * 3 * sizeof(double),
                              cudaMemcpyHostToDevice, st));
     double *dV = h->stage_out, *dE = E_host ? h->stage_out + P : nullptr;
-    qmmm_status s = qmmm_field_eval(h, h->stage_elec, W, N, dV, dE, prec, stream);
+    qmmm_status s = eval_impl(h, h->stage_elec, W, N, dV, dE, prec, stream, nullptr);
     if (s != QMMM_OK) return s;
     // V and E are adjacent in the staging buffer: one device->host copy when both are wanted
     // and the host buffers are adjacent too, else two.
@@ -494,5 +546,21 @@ qmmm_status qmmm_debug_phases(qmmm_field *h, long long *out, int n) {
     return QMMM_OK;
 }
 #endif
+
+qmmm_status qmmm_field_eval_moves_host(qmmm_field *h, const double *elec_xyz_host, int64_t n,
+                                       int64_t N, double *V_host, double *E_host, int prec,
+                                       void *stream, double *seconds) {
+    if (n < 0) return fail(QMMM_ERR_INVALID_ARG, "eval_moves_host: n < 0");
+    struct timespec t0, t1;
+    clock_gettime(CLOCK_MONOTONIC, &t0);
+    for (int64_t s = 0; s < n; ++s) {
+        qmmm_status st = qmmm_field_eval_host(h, elec_xyz_host + s * N * 3, 1, N, V_host + s * N,
+                                              E_host ? E_host + s * N * 3 : nullptr, prec, stream);
+        if (st != QMMM_OK) return st;
+    }
+    clock_gettime(CLOCK_MONOTONIC, &t1);
+    if (seconds) *seconds = (t1.tv_sec - t0.tv_sec) + 1e-9 * (t1.tv_nsec - t0.tv_nsec);
+    return QMMM_OK;
+}
 
 }  // extern "C"

@@ -47,6 +47,11 @@ struct PairParams {
     double *V;               // [P]       final outputs, written by the last CTA of a point block
     double *E;               // [P][3] or NULL
     int *counters;           // [point_blocks] arrival tickets, zero between evaluations
+    // per-move mailbox (qmmm_field_eval_host with few points): when host_flag is set, the CTA
+    // that completes the LAST point block publishes seq to pinned host memory
+    unsigned long long *host_flag;
+    unsigned long long seq;
+    int *done;               // point blocks finished (zero between evaluations)
 #ifdef QMMM_PHASE_TIMING
     long long *dbg;          // [CTAs][10] clock64 at phase boundaries + globaltimer (diagnostic build)
 #endif
@@ -270,6 +275,15 @@ __device__ __forceinline__ void finish_point_block(const PairParams &prm, int pp
         else if (prm.E) prm.E[3 * static_cast<int64_t>(p) + (v & 3) - 1] = a;
     }
     if (tid == 0) prm.counters[blockIdx.x] = 0;        // ready for the next evaluation
+    if (prm.host_flag) {
+        __threadfence_system();                        // V, E (mapped host memory) before the flag
+        sync();
+        if (tid == 0 && atomicAdd(prm.done, 1) == static_cast<int>(gridDim.x) - 1) {
+            *prm.done = 0;
+            __threadfence_system();
+            *reinterpret_cast<volatile unsigned long long *>(prm.host_flag) = prm.seq;
+        }
+    }
 }
 
 // ----------------------------------------------------------------------------- pair kernel
@@ -295,14 +309,35 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
     int lo, hi;
     slice_range(prm.n_chunks, prm.slices, blockIdx.y, lo, hi);
 
-    if (threadIdx.x == 0) {
+    // The producer lane initialises the barriers itself and sends the first `stages` loads at
+    // once; everybody else meanwhile stages the CTA's evaluation points (FP64) in shared memory.
+    const bool producer = warp == COMPUTE_WARPS && lane == 0;
+    int pc = lo, pk = 0;                                     // producer cursor
+    auto load_step = [&]() {                                 // one pipeline step: [pc, stage end)
+        const int ce = stage_end<SC>(pc, hi);
+        const int slot = pk % stages;
+        if (pk >= stages) mbar_wait(&empty[slot], ((pk / stages) - 1) & 1);
+        unsigned char *dst = smem + static_cast<size_t>(slot) * STAGE_BYTES;
+        const uint32_t bytes = static_cast<uint32_t>(ce - pc) * CHUNK_BYTES;
+        if constexpr (F32) {
+            mbar_expect_tx(&full[slot], bytes + 32);
+            tma_bulk_g2s(dst, prm.origins + 4 * (pc / SC), 32, &full[slot]);
+        } else {
+            mbar_expect_tx(&full[slot], bytes);
+        }
+        tma_bulk_g2s(dst + STAGE_HDR, prm.chunks + static_cast<size_t>(pc) * CHUNK_BYTES, bytes,
+                     &full[slot]);
+        pc = ce;
+        ++pk;
+    };
+    if (producer) {
         for (int s = 0; s < stages; ++s) {
             mbar_init(&full[s], 1);
             mbar_init(&empty[s], COMPUTE_WARPS);
         }
         fence_barrier_init();
+        while (pc < hi && pk < stages) load_step();
     }
-    // stage the CTA's evaluation points (FP64) in shared memory
     const int ppb = WP * EPT;
     for (int i = threadIdx.x; i < ppb * 3; i += CTA_THREADS) {
         int p = blockIdx.x * ppb + i / 3;
@@ -313,26 +348,8 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
 
     if (warp == COMPUTE_WARPS) {
         // ===================== producer warp: one lane drives the TMA pipeline ==========
-        if (lane == 0) {
-            int c = lo, k = 0;
-            while (c < hi) {
-                const int ce = stage_end<SC>(c, hi);
-                const int slot = k % stages;
-                if (k >= stages) mbar_wait(&empty[slot], ((k / stages) - 1) & 1);
-                unsigned char *dst = smem + static_cast<size_t>(slot) * STAGE_BYTES;
-                const uint32_t bytes = static_cast<uint32_t>(ce - c) * CHUNK_BYTES;
-                if constexpr (F32) {
-                    mbar_expect_tx(&full[slot], bytes + 32);
-                    tma_bulk_g2s(dst, prm.origins + 4 * (c / SC), 32, &full[slot]);
-                } else {
-                    mbar_expect_tx(&full[slot], bytes);
-                }
-                tma_bulk_g2s(dst + STAGE_HDR, prm.chunks + static_cast<size_t>(c) * CHUNK_BYTES,
-                             bytes, &full[slot]);
-                c = ce;
-                ++k;
-            }
-        }
+        if (lane == 0)
+            while (pc < hi) load_step();
         return;
     }
 
@@ -584,15 +601,6 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
         }
         fence_barrier_init();
     }
-    const int ppb = WP * EPT;
-    for (int i = threadIdx.x; i < ppb * 3; i += NT) {
-        int p = blockIdx.x * ppb + i / 3;
-        p = p < prm.P ? p : prm.P - 1;                          // clamp: duplicates are not written
-        elec_s[i] = prm.elec[static_cast<int64_t>(p) * 3 + (i % 3)];
-    }
-    __syncthreads();
-    QMMM_MARK(1);
-
     // ---- producer cursor (warp 0 only): next pipeline step to load -------------------------
     int pc = lo, pslot = 0;
     uint32_t pphase = 0;
@@ -616,8 +624,20 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
             pwrapped = true;
         }
     };
-    if (warp == 0)
+    // The first loads go out before anything else: they need only the barriers, which the
+    // issuing thread has just initialised itself.
+    if (warp == 0) {
+        __syncwarp();
         for (int i = 0; i < stages - 1; ++i) produce();
+    }
+    const int ppb = WP * EPT;
+    for (int i = threadIdx.x; i < ppb * 3; i += NT) {
+        int p = blockIdx.x * ppb + i / 3;
+        p = p < prm.P ? p : prm.P - 1;                          // clamp: duplicates are not written
+        elec_s[i] = prm.elec[static_cast<int64_t>(p) * 3 + (i % 3)];
+    }
+    __syncthreads();
+    QMMM_MARK(1);
 
     const int wp = warp % WP, ws = warp / WP;
     double2 *my = acc + threadIdx.x;                 // this thread's column: my[i * NT]

@@ -259,3 +259,64 @@ def test_config4_large_environment_fp64(torch_cuda, B, oracle_mod):
     ref = oracle_of(oracle_mod, w, pts[idx])
     check(ref, V[idx], E[idx], TOL64)
     assert np.all(np.isfinite(V)) and np.all(np.isfinite(E))
+
+
+# ------------------------------------------------- per-move mailbox path
+@pytest.mark.parametrize("precision,tol", [("fp64", TOL64), ("fp32", TOL32)])
+def test_moves_host_loop_matches_oracle(torch_cuda, B, oracle_mod, precision, tol):
+    """qmmm_field_eval_moves_host: 40 sequential single-electron moves of config 2's walk
+    through the pinned mailbox; every move against the oracle."""
+    w = make_workload(2, n_points=(40, 1))
+    pts = np.ascontiguousarray(w.elec_xyz.reshape(-1, 3))
+    ref = oracle_of(oracle_mod, w, pts)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 1)
+    try:
+        V = np.full(len(pts), np.nan); E = np.full((len(pts), 3), np.nan)
+        secs = B.qmmm_field_eval_moves_host(h, pts, len(pts), 1, V, E, precision)
+        assert secs > 0
+        check(ref, V, E, tol)
+        V2 = np.full(len(pts), np.nan)
+        B.qmmm_field_eval_moves_host(h, pts, len(pts), 1, V2, None, precision)   # potential only
+        assert np.max(np.abs(V2 - V) / np.abs(V)) <= 1e-13
+    finally:
+        B.qmmm_field_destroy(h)
+
+
+@pytest.mark.parametrize("P", [1, 7, 64, 65, 200])
+def test_eval_host_mailbox_and_copy_paths_agree_with_device_path(torch_cuda, B, P):
+    """eval_host uses the zero-copy mailbox up to 64 points and staged copies above; both
+    must give bitwise the device-path result (same kernels, same plan)."""
+    w = make_workload(0)
+    rng = np.random.default_rng(P)
+    pts = rng.normal(size=(P, 3))
+    pts *= (rng.random((P, 1)) * 2.5) / np.linalg.norm(pts, axis=1, keepdims=True)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, P)
+    try:
+        for prec in ("fp64", "fp32"):
+            Vd, Ed = gpu_eval(torch_cuda, B, w, pts, prec, handle=h)
+            for rep in range(3):                      # the sequence flag must advance correctly
+                V = np.full(P, np.nan); E = np.full((P, 3), np.nan)
+                B.qmmm_field_eval_host(h, np.ascontiguousarray(pts), 1, P, V, E, prec)
+                assert np.array_equal(V, Vd) and np.array_equal(E, Ed)
+    finally:
+        B.qmmm_field_destroy(h)
+
+
+def test_repeatability_stress_all_kernel_variants(torch_cuda, B):
+    """compute-sanitizer is closed on this GPU pool, so races are hunted statistically: every
+    kernel variant and several partitions, 25 evaluations each on one handle, must be bitwise
+    identical (shared-memory reuse in the reduction, the ticket of the last CTA, the mailbox)."""
+    w = make_workload(1, n_points=(3, 11))
+    pts = w.elec_xyz.reshape(-1, 3)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, len(pts))
+    try:
+        for prec in ("fp64", "fp32"):
+            for plan in (dict(), dict(points_per_thread=1, slices=148), dict(points_per_thread=2, slices=37),
+                         dict(points_per_thread=4, point_warps=1, slices=74),
+                         dict(points_per_thread=8, point_warps=2, slices=296, stages=2)):
+                V0, E0 = gpu_eval(torch_cuda, B, w, pts, prec, plan=plan, handle=h)
+                for _ in range(25):
+                    V, E = gpu_eval(torch_cuda, B, w, pts, prec, plan=plan, handle=h)
+                    assert np.array_equal(V, V0) and np.array_equal(E, E0), (prec, plan)
+    finally:
+        B.qmmm_field_destroy(h)
