@@ -242,10 +242,13 @@ __device__ __forceinline__ void finish_point_block(const PairParams &prm, int pp
                                                    int *flag, double *scratch /*[NT]*/, SYNC sync) {
     __threadfence();                                   // this CTA's partials are visible
     sync();
-    if (tid == 0) *flag = atomicAdd(prm.counters + blockIdx.x, 1) == prm.slices - 1;
+    if (tid == 0) {
+        *flag = atomicAdd(prm.counters + blockIdx.x, 1) == prm.slices - 1;
+        __threadfence();                               // the other CTAs' partials, seen through the ticket
+    }
     sync();
     if (!*flag) return;
-    __threadfence();
+    QMMM_MARK(7);
     // thread = (group g, value v): nval = 4*ppb values {V,Ex,Ey,Ez} x points (a power of two
     // <= NT); group g adds slices g, g+G, g+2G, ... on eight interleaved accumulators (all
     // loads independent and coalesced over v), then the G groups are added in index order.
@@ -296,6 +299,8 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
     constexpr int STAGE_BYTES = STAGE_HDR + SC * CHUNK_BYTES;
 
     extern __shared__ __align__(128) unsigned char smem[];
+    QMMM_MARK_GT(8);
+    QMMM_MARK(0);
     // layout: [stages x STAGE_BYTES] [full barriers] [empty barriers] [reduction scratch]
     const int stages = prm.stages;
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + static_cast<size_t>(stages) * STAGE_BYTES);
@@ -345,6 +350,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
         elec_s[i] = prm.elec[static_cast<int64_t>(p) * 3 + (i % 3)];
     }
     __syncthreads();
+    QMMM_MARK(1);
 
     if (warp == COMPUTE_WARPS) {
         // ===================== producer warp: one lane drives the TMA pipeline ==========
@@ -369,6 +375,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
         }
     }
 
+    QMMM_MARK(2);
     int c = lo, k = 0;
     while (c < hi) {
         const int ce = stage_end<SC>(c, hi);
@@ -453,9 +460,11 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
         ++k;
     }
 
+    QMMM_MARK(3);
     // FP64 path: the nuclei are ordinary sources at the end of the FP64 chunk array
     if constexpr (F32) nuclei_share<EPT>(prm, elec_s + wp * EPT * 3, ws, WS, lane, V, Ex, Ey, Ez);
 
+    QMMM_MARK(4);
     // ---- in-CTA reduction (paper: shared memory; here shuffle + smem) ----
 #pragma unroll
     for (int e = 0; e < EPT; ++e) {
@@ -480,8 +489,11 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
         if (p < prm.P)
             prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] = acc;
     }
+    QMMM_MARK(5);
     finish_point_block<32 * COMPUTE_WARPS>(prm, WP * EPT, threadIdx.x, flag, red,
                                            [] { compute_warps_sync(); });
+    QMMM_MARK(6);
+    QMMM_MARK_GT(9);
 }
 
 // ----------------------------------------------------------------------------- FP32 packed
