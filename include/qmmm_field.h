@@ -92,10 +92,16 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
 /*
  * qmmm_field_eval_host -- the paper's per-step call: HOST buffers in and out;
  * returns when V_host (and E_host) hold the result.  Buffers may be pageable or pinned.
- * Up to 64 points go through a pinned, device-mapped mailbox owned by the handle: the kernel
- * reads the points from it and the last CTA writes V, E and a sequence number back, which
- * the host waits for -- no cudaMemcpy, no stream synchronisation.  More points: host->device
- * copy, kernel, device->host copy on `stream`, stream synchronisation.
+ *   W*N == 1  : served by a resident "move server": one cooperative kernel (one CTA per SM)
+ *               that stays on the GPU, polls a pinned mailbox for r_new, evaluates, and
+ *               writes {V, E} back -- no kernel launch, copy or synchronisation per move.
+ *               It retires by itself after 2 ms without a request (and after 1 s in any
+ *               case) and is restarted transparently; any other call on the handle retires
+ *               it first.  While it is resident it occupies every SM.  `stream` is not used.
+ *   W*N <= 64 : one kernel launch on `stream`; points read from and results written to a
+ *               pinned, device-mapped mailbox, completion signalled by a sequence number.
+ *   otherwise : host->device copy, kernel, device->host copy on `stream`, synchronisation.
+ * All three give bitwise the result of qmmm_field_eval with the same plan.
  * Same argument meaning and errors as qmmm_field_eval.
  */
 qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int64_t W,

@@ -8,6 +8,7 @@
 // No torch types, no CPU fallback: every step of the path runs in the kernels of
 // qmmm_kernels.cuh.
 #include "qmmm_kernels.cuh"
+#include "qmmm_server.cuh"
 
 #include <algorithm>
 #include <atomic>
@@ -90,6 +91,13 @@ struct qmmm_field {
     // per-move mailbox: pinned, device-mapped host memory (elec in; V, E and a sequence flag out)
     double *mail_h = nullptr, *mail_d = nullptr;   // [MAIL_POINTS*3 | MAIL_POINTS*4 | flag]
     unsigned long long seq = 0;
+    // resident move server (qmmm_server.cuh): serves single-point eval_host calls
+    ServerMailbox *srv_mail_h = nullptr, *srv_mail_d = nullptr;
+    ServerDevice *srv_dev = nullptr;
+    cudaStream_t srv_stream = nullptr;
+    bool srv_alive = false, srv_ok = true;     // srv_ok: cooperative launch available
+    int srv_prec = -1;
+    unsigned long long srv_launch_id = 0, srv_seq = 0;
     int *counters = nullptr;       // [max_points] arrival tickets of the point blocks (zero at rest)
 };
 
@@ -207,6 +215,164 @@ cudaError_t to_device(const double *src, int64_t n, double **dev, bool *owned) {
     if (e != cudaSuccess) return e;
     *owned = true;
     return cudaMemcpy(*dev, src, n * sizeof(double), cudaMemcpyHostToDevice);
+}
+
+}  // namespace
+
+namespace {
+
+// ------------------------------------------------------------------ resident move server
+double now_seconds() {
+    struct timespec t;
+    clock_gettime(CLOCK_MONOTONIC, &t);
+    return t.tv_sec + 1e-9 * t.tv_nsec;
+}
+
+// Host side of the request seqlock: seq_a, then r, then seq_b (program order = store order on x86).
+void post_request(ServerMailbox *m, unsigned long long s, const double *r) {
+    m->req[0] = s;
+    std::atomic_thread_fence(std::memory_order_release);
+    if (r)
+        for (int i = 0; i < 3; ++i) {
+            unsigned long long bits;
+            std::memcpy(&bits, r + i, 8);
+            m->req[1 + i] = bits;
+        }
+    std::atomic_thread_fence(std::memory_order_release);
+    m->req[4] = s;
+}
+
+// Waits until the server launch `h->srv_launch_id` has retired, then joins its stream.
+qmmm_status server_join(qmmm_field *h) {
+    const double t0 = now_seconds();
+    while (h->srv_mail_h->exited != h->srv_launch_id) {
+        if (cudaStreamQuery(h->srv_stream) != cudaErrorNotReady) break;     // ended (or failed)
+        if (now_seconds() - t0 > 10.0) return fail(QMMM_ERR_CUDA, "move server did not retire");
+    }
+    CUDA_TRY(cudaStreamSynchronize(h->srv_stream));
+    h->srv_alive = false;
+    return QMMM_OK;
+}
+
+// Retires a running server (any other use of the handle's workspace must do this first).
+qmmm_status server_stop(qmmm_field *h) {
+    if (!h->srv_alive) return QMMM_OK;
+    post_request(h->srv_mail_h, SERVER_EXIT, nullptr);
+    qmmm_status st = server_join(h);
+    post_request(h->srv_mail_h, h->srv_seq, nullptr);
+    return st;
+}
+
+template <typename REAL>
+cudaError_t server_launch(const ServerParams &sp, int slices, size_t smem, cudaStream_t st) {
+    auto kern = move_server_kernel<REAL>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         static_cast<int>(smem));
+    if (e != cudaSuccess) return e;
+    void *args[] = {const_cast<ServerParams *>(&sp)};
+    return cudaLaunchCooperativeKernel(reinterpret_cast<void *>(kern), dim3(1, slices),
+                                       dim3(CTA_THREADS), args, smem, st);
+}
+
+// Starts the server for `prec`; *usable = false when this problem cannot be served (the
+// caller then uses the launch path).
+qmmm_status server_start(qmmm_field *h, int prec, bool *usable) {
+    const bool f32 = prec == QMMM_FP32_ACC64;
+    *usable = false;
+    const int64_t n_chunks = f32 ? h->n_chunks : h->n_chunks64;
+    if (!h->srv_ok || n_chunks < 1 || h->timing) return QMMM_OK;
+    qmmm_plan pl = choose_plan(h, 1, f32);
+    if (pl.points_per_thread != 1 || pl.point_warps != 1 || pl.slices > h->sm_count) return QMMM_OK;
+    size_t smem = pair_smem_bytes(f32, pl.stages, 1, 1) + 64;
+    while (smem > 227 * 1024 && pl.stages > 2) smem = pair_smem_bytes(f32, --pl.stages, 1, 1) + 64;
+
+    ServerParams sp;
+    std::memset(&sp, 0, sizeof(sp));
+    PairParams &prm = sp.pair;
+    prm.chunks = f32 ? reinterpret_cast<const char *>(h->chunks32)
+                     : reinterpret_cast<const char *>(h->chunks64);
+    prm.origins = h->origins;
+    prm.partial = h->workspace;
+    prm.P = 1;
+    prm.n_chunks = static_cast<int>(n_chunks);
+    prm.slices = pl.slices;
+    prm.point_warps = 1;
+    prm.stages = pl.stages;
+    prm.lattice = h->lattice;
+    prm.inv_lattice = 1.0 / h->lattice;
+    prm.nuc = h->nuclei;
+    prm.K = f32 ? static_cast<int>(h->K) : 0;
+    prm.counters = h->counters;
+    sp.mail = h->srv_mail_d;
+    sp.dev = h->srv_dev;
+    sp.start_seq = h->srv_seq;
+    sp.launch_id = ++h->srv_launch_id;
+    post_request(h->srv_mail_h, h->srv_seq, nullptr);
+    ServerDevice init;
+    std::memset(&init, 0, sizeof(init));
+    init.cmd = h->srv_seq;
+    CUDA_TRY(cudaMemcpy(h->srv_dev, &init, sizeof(init), cudaMemcpyHostToDevice));
+    cudaError_t e = f32 ? server_launch<float>(sp, pl.slices, smem, h->srv_stream)
+                        : server_launch<double>(sp, pl.slices, smem, h->srv_stream);
+    if (e != cudaSuccess) {                    // e.g. the GPU is shared and cannot hold the grid
+        cudaGetLastError();
+        h->srv_ok = false;
+        return QMMM_OK;
+    }
+    h->srv_alive = true;
+    h->srv_prec = prec;
+    h->last_plan = pl;
+    h->last_point_blocks = 1;
+    h->last_launches = 0;
+    *usable = true;
+    return QMMM_OK;
+}
+
+// One move through the server.  *served = false: the caller must use the launch path.
+qmmm_status server_move(qmmm_field *h, const double *r, double *V, double *E, int prec,
+                        bool *served) {
+    *served = false;
+    if (h->srv_alive && h->srv_prec != prec) {
+        qmmm_status st = server_stop(h);
+        if (st != QMMM_OK) return st;
+    }
+    if (!h->srv_alive) {
+        bool usable = false;
+        qmmm_status st = server_start(h, prec, &usable);
+        if (st != QMMM_OK) return st;
+        if (!usable) return QMMM_OK;
+    }
+    ServerMailbox *m = h->srv_mail_h;
+    const unsigned long long s = ++h->srv_seq;
+    post_request(m, s, r);
+    const double t0 = now_seconds();
+    auto answered = [&]() { return m->ans[0] == s && m->ans[5] == s; };
+    for (uint64_t spin = 1; !answered(); ++spin) {
+        if (m->exited == h->srv_launch_id) {
+            // the server retired (idle / lifetime) before taking this move: start a new one,
+            // the request stays posted
+            CUDA_TRY(cudaStreamSynchronize(h->srv_stream));
+            h->srv_alive = false;
+            if (answered()) break;
+            --h->srv_seq;                              // server_start reposts seq_req = srv_seq
+            bool usable = false;
+            qmmm_status st = server_start(h, prec, &usable);
+            ++h->srv_seq;
+            if (st != QMMM_OK) return st;
+            if (!usable) return QMMM_OK;               // fall back to the launch path
+            post_request(m, s, r);
+        }
+        if ((spin & 0xFFFFF) == 0 && now_seconds() - t0 > 10.0)
+            return fail(QMMM_ERR_CUDA, "move server did not answer");
+    }
+    std::atomic_thread_fence(std::memory_order_acquire);
+    unsigned long long bits[4] = {m->ans[1], m->ans[2], m->ans[3], m->ans[4]};
+    if (m->ans[0] != s || m->ans[5] != s)
+        return fail(QMMM_ERR_CUDA, "move server: answer line changed while it was read");
+    std::memcpy(V, &bits[0], 8);
+    if (E) std::memcpy(E, &bits[1], 24);
+    *served = true;
+    return QMMM_OK;
 }
 
 }  // namespace
@@ -331,6 +497,16 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
     CREATE_TRY(cudaHostAlloc(&h->mail_h, (MAIL_POINTS * 7 + 1) * sizeof(double), cudaHostAllocMapped));
     std::memset(h->mail_h, 0, (MAIL_POINTS * 7 + 1) * sizeof(double));
     CREATE_TRY(cudaHostGetDevicePointer(&h->mail_d, h->mail_h, 0));
+    CREATE_TRY(cudaHostAlloc(&h->srv_mail_h, sizeof(ServerMailbox), cudaHostAllocMapped));
+    std::memset(h->srv_mail_h, 0, sizeof(ServerMailbox));
+    CREATE_TRY(cudaHostGetDevicePointer(&h->srv_mail_d, h->srv_mail_h, 0));
+    CREATE_TRY(cudaMalloc(&h->srv_dev, sizeof(ServerDevice)));
+    CREATE_TRY(cudaStreamCreateWithFlags(&h->srv_stream, cudaStreamNonBlocking));
+    {
+        int coop = 0;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        h->srv_ok = coop != 0;
+    }
     CREATE_TRY(cudaMalloc(&h->stage_elec, max_points * 3 * sizeof(double)));
     CREATE_TRY(cudaMalloc(&h->stage_out, max_points * 4 * sizeof(double)));
 #undef CREATE_TRY
@@ -340,6 +516,10 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
 
 qmmm_status qmmm_field_destroy(qmmm_field *h) {
     if (!h) return QMMM_OK;
+    server_stop(h);
+    if (h->srv_stream) cudaStreamDestroy(h->srv_stream);
+    if (h->srv_mail_h) cudaFreeHost(h->srv_mail_h);
+    cudaFree(h->srv_dev);
     cudaFree(h->chunks64);
     cudaFree(h->chunks32);
     cudaFree(h->origins);
@@ -366,6 +546,7 @@ qmmm_status qmmm_field_set_plan(qmmm_field *h, const qmmm_plan *plan) {
         return fail(QMMM_ERR_INVALID_ARG, "set_plan: slices out of range");
     if (plan->stages != 0 && (plan->stages < 2 || plan->stages > 8))
         return fail(QMMM_ERR_INVALID_ARG, "set_plan: stages must be 0 or 2..8");
+    server_stop(h);
     h->user_plan = *plan;
     return QMMM_OK;
 }
@@ -374,6 +555,7 @@ qmmm_status qmmm_field_set_timing(qmmm_field *h, int enable) {
     if (!h) return fail(QMMM_ERR_INVALID_ARG, "set_timing: NULL handle");
     if (enable && !h->ev[0])
         for (cudaEvent_t &e : h->ev) CUDA_TRY(cudaEventCreate(&e));
+    server_stop(h);
     h->timing = enable != 0;
     h->timed = false;
     return QMMM_OK;
@@ -420,6 +602,10 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
     const bool f32 = prec == QMMM_FP32_ACC64;
     const int P = static_cast<int>(W * N);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (h->srv_alive) {                    // the resident server owns the workspace: retire it
+        qmmm_status ss = server_stop(h);
+        if (ss != QMMM_OK) return ss;
+    }
 
     qmmm_plan pl = choose_plan(h, P, f32);
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
@@ -492,6 +678,12 @@ qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int
         return fail(QMMM_ERR_INVALID_ARG, "eval_host: W*N must be in [1, max_points]");
     const int64_t P = W * N;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (P == 1 && (prec == QMMM_FP64 || prec == QMMM_FP32_ACC64)) {
+        // one point per call is the paper's own loop: served by the resident move server
+        bool served = false;
+        qmmm_status s = server_move(h, elec_xyz_host, V_host, E_host, prec, &served);
+        if (s != QMMM_OK || served) return s;
+    }
     if (P <= MAIL_POINTS) {
         // Per-move path ("r_new" in, U_ES out, every Monte-Carlo step): no
         // cudaMemcpy and no stream synchronisation.  The kernel reads the points from a

@@ -239,7 +239,8 @@ __device__ __forceinline__ void nuclei_share(const PairParams &prm, const double
 // that is.  NT threads (whole warps) call this; sync() is their barrier.
 template <int NT, typename SYNC>
 __device__ __forceinline__ void finish_point_block(const PairParams &prm, int ppb, int tid,
-                                                   int *flag, double *scratch /*[NT]*/, SYNC sync) {
+                                                   int *flag, double *scratch /*[NT]*/, SYNC sync,
+                                                   unsigned long long seq) {
     __threadfence();                                   // this CTA's partials are visible
     sync();
     if (tid == 0) {
@@ -284,7 +285,7 @@ __device__ __forceinline__ void finish_point_block(const PairParams &prm, int pp
         if (tid == 0 && atomicAdd(prm.done, 1) == static_cast<int>(gridDim.x) - 1) {
             *prm.done = 0;
             __threadfence_system();
-            *reinterpret_cast<volatile unsigned long long *>(prm.host_flag) = prm.seq;
+            *reinterpret_cast<volatile unsigned long long *>(prm.host_flag) = seq;
         }
     }
 }
@@ -491,7 +492,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
     }
     QMMM_MARK(5);
     finish_point_block<32 * COMPUTE_WARPS>(prm, WP * EPT, threadIdx.x, flag, red,
-                                           [] { compute_warps_sync(); });
+                                           [] { compute_warps_sync(); }, prm.seq);
     QMMM_MARK(6);
     QMMM_MARK_GT(9);
 }
@@ -782,7 +783,7 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
             prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] = a;
     }
     QMMM_MARK(5);
-    finish_point_block<NT>(prm, WP * EPT, threadIdx.x, flag, red, [] { __syncthreads(); });
+    finish_point_block<NT>(prm, WP * EPT, threadIdx.x, flag, red, [] { __syncthreads(); }, prm.seq);
     QMMM_MARK(6);
     QMMM_MARK_GT(9);
 }

@@ -320,3 +320,34 @@ def test_repeatability_stress_all_kernel_variants(torch_cuda, B):
                     assert np.array_equal(V, V0) and np.array_equal(E, E0), (prec, plan)
     finally:
         B.qmmm_field_destroy(h)
+
+
+def test_move_server_bitwise_equals_launch_path_and_survives_idle_and_switches(torch_cuda, B):
+    """Single-point eval_host calls are served by the resident move server (one cooperative
+    launch, pinned mailbox).  Its results must be bitwise those of the launch path (same
+    partition), across idle retirement (2 ms) and relaunch, precision switches, interleaved
+    device-path evaluations and potential-only calls."""
+    import time
+    w = make_workload(2, n_points=(12, 1))
+    pts = np.ascontiguousarray(w.elec_xyz.reshape(-1, 3))
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 4)
+    try:
+        ref = {}
+        for prec in ("fp64", "fp32"):
+            ref[prec] = [gpu_eval(torch_cuda, B, w, pts[i:i + 1], prec, handle=h) for i in range(len(pts))]
+        order = ["fp64", "fp64", "fp32", "fp64", "fp32", "fp32"] * 2
+        for i, prec in enumerate(order):
+            V = np.full(1, np.nan); E = np.full((1, 3), np.nan)
+            B.qmmm_field_eval_host(h, pts[i:i + 1], 1, 1, V, E, prec)
+            assert np.array_equal(V, ref[prec][i][0]) and np.array_equal(E, ref[prec][i][1]), (i, prec)
+            if i == 3:
+                time.sleep(0.02)                         # the server retires after 2 ms idle
+            if i == 5:                                    # a device-path call in between
+                Vd, Ed = gpu_eval(torch_cuda, B, w, pts[:3], "fp32", handle=h)
+                assert np.all(np.isfinite(Vd))
+            if i == 7:                                    # potential only
+                V2 = np.full(1, np.nan)
+                B.qmmm_field_eval_host(h, pts[i:i + 1], 1, 1, V2, None, prec)
+                assert np.array_equal(V2, V)
+    finally:
+        B.qmmm_field_destroy(h)
