@@ -283,8 +283,9 @@ qmmm_status server_start(qmmm_field *h, int prec, bool *usable) {
     if (!h->srv_ok || n_chunks < 1 || h->timing) return QMMM_OK;
     qmmm_plan pl = choose_plan(h, 1, f32);
     if (pl.points_per_thread != 1 || pl.point_warps != 1 || pl.slices > h->sm_count) return QMMM_OK;
-    size_t smem = pair_smem_bytes(f32, pl.stages, 1, 1) + 64;
-    while (smem > 227 * 1024 && pl.stages > 2) smem = pair_smem_bytes(f32, --pl.stages, 1, 1) + 64;
+    const size_t extra = 128 + static_cast<size_t>(pl.slices) * 4 * sizeof(double);   // cmd, go, collected partials
+    size_t smem = pair_smem_bytes(f32, pl.stages, 1, 1) + extra;
+    while (smem > 227 * 1024 && pl.stages > 2) smem = pair_smem_bytes(f32, --pl.stages, 1, 1) + extra;
 
     ServerParams sp;
     std::memset(&sp, 0, sizeof(sp));
@@ -312,6 +313,7 @@ qmmm_status server_start(qmmm_field *h, int prec, bool *usable) {
     std::memset(&init, 0, sizeof(init));
     init.cmd = h->srv_seq;
     CUDA_TRY(cudaMemcpy(h->srv_dev, &init, sizeof(init), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemset(h->workspace, 0, static_cast<size_t>(pl.slices) * SLOT_WORDS * 8));   // untagged slots
     cudaError_t e = f32 ? server_launch<float>(sp, pl.slices, smem, h->srv_stream)
                         : server_launch<double>(sp, pl.slices, smem, h->srv_stream);
     if (e != cudaSuccess) {                    // e.g. the GPU is shared and cannot hold the grid

@@ -59,36 +59,67 @@ __device__ __forceinline__ long long global_ns() {
     return t;
 }
 
-// Cross-CTA sum of one move (finish_point_block for P = 1) with the answer going straight to
-// the host: threads 0..3 of the last CTA hold V, Ex, Ey, Ez in registers, and lanes 0..5 of
-// warp 0 store {seq, V, Ex, Ey, Ez, seq} to the mapped answer line in one transaction -- no
-// system-scope fence (a PCIe round trip each) on the critical path.
+// Cross-CTA sum of one move, push model.  Every CTA stores its partial as one tagged 48-byte
+// record {s, V, Ex, Ey, Ez, s} (six lanes, one store instruction, one L2 write packet) into
+// its own slot -- no fence, no atomic ticket, and it is free for the next move at once.  The
+// leader CTA collects: thread t polls slot t with three 16-byte volatile loads until both tags
+// carry s, the records go to shared memory, and the slices are added in exactly the order of
+// finish_point_block (so the result is bitwise that of the launch path).  Threads 0..3 then
+// hold V, Ex, Ey, Ez and lanes 0..5 of warp 0 store {s, V, E, s} to the mapped answer line in
+// one transaction -- no system-scope fence (a PCIe round trip each) on the critical path.
+constexpr int SLOT_WORDS = 8;              // 64-byte slots in the partials workspace
+
+__device__ __forceinline__ void server_push(unsigned long long *slots, int lane, double acc,
+                                            unsigned long long seq) {
+    // lanes 0..3 hold V, Ex, Ey, Ez; shift them to lanes 1..4, tags in lanes 0 and 5
+    const double up = __shfl_up_sync(0xffffffffu, acc, 1);
+    unsigned long long w = static_cast<unsigned long long>(__double_as_longlong(up));
+    if (lane == 0 || lane == 5) w = seq;
+    if (lane < 6)
+        *reinterpret_cast<volatile unsigned long long *>(slots + blockIdx.y * SLOT_WORDS + lane) = w;
+}
+
+struct u64x2 { unsigned long long x, y; };
+__device__ __forceinline__ u64x2 ld_volatile_v2(const unsigned long long *p) {
+    u64x2 r;
+    asm volatile("ld.volatile.global.v2.u64 {%0, %1}, [%2];" : "=l"(r.x), "=l"(r.y) : "l"(p));
+    return r;
+}
+
+// Leader CTA only; all 256 consumer threads call it.  part_s: [slices][4] doubles of shared
+// memory.  Returns false if a slot never arrived (hard timeout): the caller retires the server.
 template <typename SYNC>
-__device__ __forceinline__ void server_finish(const PairParams &prm, ServerMailbox *mail, int tid,
-                                              int *flag, double *scratch, SYNC sync,
-                                              unsigned long long seq) {
+__device__ __forceinline__ bool server_collect(const PairParams &prm, ServerMailbox *mail,
+                                               const unsigned long long *slots, int tid,
+                                               double *part_s, double *scratch, int *flag, SYNC sync,
+                                               unsigned long long seq, long long t_start) {
     constexpr int NT = 32 * COMPUTE_WARPS;
-    __threadfence();
+    if (tid == 0) *flag = 1;
     sync();
-    if (tid == 0) {
-        *flag = atomicAdd(prm.counters, 1) == prm.slices - 1;
-        __threadfence();
+    for (int sl = tid; sl < prm.slices; sl += NT) {
+        const unsigned long long *p = slots + sl * SLOT_WORDS;
+        for (;;) {
+            const u64x2 a = ld_volatile_v2(p), b = ld_volatile_v2(p + 2), c = ld_volatile_v2(p + 4);
+            if (a.x == seq && c.y == seq) {
+                part_s[4 * sl + 0] = __longlong_as_double(static_cast<long long>(a.y));
+                part_s[4 * sl + 1] = __longlong_as_double(static_cast<long long>(b.x));
+                part_s[4 * sl + 2] = __longlong_as_double(static_cast<long long>(b.y));
+                part_s[4 * sl + 3] = __longlong_as_double(static_cast<long long>(c.x));
+                break;
+            }
+            if (global_ns() - t_start > SERVER_HARD_NS) { *flag = 0; break; }
+        }
     }
     sync();
-    if (!*flag) return;
+    if (!*flag) return false;
     const int G = NT / 4, v = tid & 3, g = tid >> 2;      // same association as finish_point_block
     double a[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     {
-        const double *src = prm.partial + v;
         int sidx = g;
-        for (; sidx + 7 * G < prm.slices; sidx += 8 * G) {
-            double t[8];
+        for (; sidx + 7 * G < prm.slices; sidx += 8 * G)
 #pragma unroll
-            for (int k = 0; k < 8; ++k) t[k] = __ldcg(src + (sidx + k * G) * 4);
-#pragma unroll
-            for (int k = 0; k < 8; ++k) a[k] += t[k];
-        }
-        for (int k = 0; sidx < prm.slices; sidx += G, ++k) a[k] += __ldcg(src + sidx * 4);
+            for (int k = 0; k < 8; ++k) a[k] += part_s[4 * (sidx + k * G) + v];
+        for (int k = 0; sidx < prm.slices; sidx += G, ++k) a[k] += part_s[4 * sidx + v];
     }
     scratch[tid] = ((a[0] + a[1]) + (a[2] + a[3])) + ((a[4] + a[5]) + (a[6] + a[7]));
     sync();
@@ -96,13 +127,12 @@ __device__ __forceinline__ void server_finish(const PairParams &prm, ServerMailb
         double r = 0.0;
         if (tid < 4)
             for (int k = 0; k < G; ++k) r += scratch[k * 4 + tid];
-        // lanes 1..4 <- values of lanes 0..3; lanes 0 and 5 carry the sequence number
         const double up = __shfl_up_sync(0xffffffffu, r, 1);
         unsigned long long w = static_cast<unsigned long long>(__double_as_longlong(up));
         if (tid == 0 || tid == 5) w = seq;
-        if (tid == 0) *prm.counters = 0;               // ready for the next move
         if (tid < 6) mail->ans[tid] = w;
     }
+    return true;
 }
 
 // grid = (1, slices) with slices <= SM count, launched cooperatively (all CTAs resident).
@@ -124,6 +154,8 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) move_server_kernel(const Serve
     double *elec_s = red + 32 * COMPUTE_WARPS;               // [3]
     volatile unsigned long long *cmd_s = reinterpret_cast<volatile unsigned long long *>(elec_s + 4);
     volatile unsigned long long *go_s = cmd_s + 1;           // moves released to the producer, or EXIT
+    double *part_s = elec_s + 8;                             // leader: [slices][4] collected partials
+    unsigned long long *slots = reinterpret_cast<unsigned long long *>(prm.partial);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int lo, hi;
@@ -302,12 +334,25 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) move_server_kernel(const Serve
             r[0] = sV; r[1] = sEx; r[2] = sEy; r[3] = sEz;
         }
         compute_warps_sync();
-        if (warp == 0 && lane < 4) {
+        if (warp == 0) {
             double acc = 0.0;
-            for (int s = 0; s < WS; ++s) acc += red[s * 4 + lane];
-            prm.partial[static_cast<int64_t>(blockIdx.y) * 4 + lane] = acc;
+            if (lane < 4)
+                for (int s = 0; s < WS; ++s) acc += red[s * 4 + lane];
+            server_push(slots, lane, acc, cmd);
         }
-        server_finish(prm, sp.mail, threadIdx.x, flag, red, [] { compute_warps_sync(); }, cmd);
+        if (leader &&
+            !server_collect(prm, sp.mail, slots, threadIdx.x, part_s, red, flag,
+                            [] { compute_warps_sync(); }, cmd, t_start)) {
+            // a slot never arrived (not expected): retire everybody
+            if (threadIdx.x == 0) {
+                *reinterpret_cast<volatile unsigned long long *>(&sp.dev->cmd) = SERVER_EXIT;
+                *go_s = SERVER_EXIT;
+            }
+            compute_warps_sync();
+            for (int s = 0; s < npre; ++s, ++k)
+                mbar_wait(&full[k % stages], static_cast<uint32_t>(k / stages) & 1u);
+            break;
+        }
     }
     if (leader && threadIdx.x == 0) {
         __threadfence_system();
