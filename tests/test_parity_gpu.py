@@ -351,3 +351,61 @@ def test_move_server_bitwise_equals_launch_path_and_survives_idle_and_switches(t
                 assert np.array_equal(V2, V)
     finally:
         B.qmmm_field_destroy(h)
+
+
+def test_config1_neutral_density_model(torch_cuda, B, oracle_mod):
+    """DESIGN.md reading 15, alternative weights w_k = Z_k (a neutral environment like the
+    paper's 84-electron / 19-atom MM part): V is a difference of two large sums
+    (kappa_V ~ 40), the harder case for both precisions."""
+    w = make_workload(1, neutral=True)
+    pts = w.elec_xyz.reshape(-1, 3)
+    ref = oracle_of(oracle_mod, w, pts)
+    kV = (ref.absV / np.abs(ref.V)).max()
+    V, E = gpu_eval(torch_cuda, B, w, pts, "fp64")
+    check(ref, V, E, TOL64)
+    V32, E32 = gpu_eval(torch_cuda, B, w, pts, "fp32")
+    # FP32: the per-point bound is relative to the size of the terms, |dV| <= 1e-5 * sum|q|/r
+    assert np.all(np.abs(V32 - ref.V) <= TOL32 * ref.absV), f"kappa_V {kV:.1f}"
+    assert np.all(np.linalg.norm(E32 - ref.E, axis=1) <= TOL32 * ref.absE)
+    dE = abs(V32.sum() - ref.V.sum())
+    print(f"config1 neutral: kappa_V max {kV:.1f}, fp32 energy deviation {dE:.3e} hartree")
+    assert dE <= E_TOL
+
+
+def test_random_shapes_and_plans(torch_cuda, B, oracle_mod):
+    """Seeded random (M, K, P, plan, precision) combinations: ragged chunk tails, slices that
+    exceed the chunk count, every points-per-thread variant, host and device paths."""
+    rng = np.random.default_rng(2024)
+    w0 = make_workload(0)
+    for trial in range(40):
+        M = int(rng.choice([1, 3, 127, 128, 129, 500, 2047, 2049, 4096]))
+        K = int(rng.choice([0, 1, 5, 16]))
+        P = int(rng.choice([1, 2, 3, 7, 8, 9, 31, 64, 65, 100]))
+        sel = rng.permutation(w0.M)[:M]
+
+        class W:
+            src_xyz = np.ascontiguousarray(w0.src_xyz[sel]); src_q = np.ascontiguousarray(w0.src_q[sel])
+            nuc_xyz = np.ascontiguousarray(w0.nuc_xyz[:K]); nuc_Z = np.ascontiguousarray(w0.nuc_Z[:K])
+        pts = rng.normal(size=(P, 3))
+        pts *= (rng.random((P, 1)) * 2.8) / np.linalg.norm(pts, axis=1, keepdims=True)
+        prec = str(rng.choice(["fp64", "fp32"]))
+        plan = dict(points_per_thread=int(rng.choice([0, 1, 2, 4, 8])), point_warps=int(rng.choice([0, 1, 2, 8])),
+                    slices=int(rng.choice([0, 1, 2, 5, 37, 148, 300])), stages=int(rng.choice([0, 2, 3, 6])))
+        ref = oracle_of(oracle_mod, W, pts)
+
+        def ok(V, E):
+            # random subsets mix +Z nuclei and negative cells, so V can cancel (kappa > 1000):
+            # errors are bounded against the size of the terms, sum|q|/r and sum|q|/r^2
+            tol = TOL64 if prec == "fp64" else TOL32
+            assert np.all(np.abs(V - ref.V) <= tol * ref.absV), (trial, M, K, P, prec, plan)
+            assert np.all(np.linalg.norm(E - ref.E, axis=1) <= tol * ref.absE), (trial, M, K, P, prec, plan)
+
+        V, E = gpu_eval(torch_cuda, B, W, pts, prec, plan=plan)
+        ok(V, E)
+        h = B.qmmm_field_create(W.src_xyz, W.src_q, W.nuc_xyz, W.nuc_Z, P)
+        try:
+            Vh = np.zeros(P); Eh = np.zeros((P, 3))
+            B.qmmm_field_eval_host(h, np.ascontiguousarray(pts), 1, P, Vh, Eh, prec)
+            ok(Vh, Eh)
+        finally:
+            B.qmmm_field_destroy(h)
