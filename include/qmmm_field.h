@@ -121,6 +121,57 @@ qmmm_status qmmm_field_eval_moves_host(qmmm_field *h, const double *elec_xyz_hos
                                        int64_t N, double *V_host, double *E_host, int prec,
                                        void *stream, double *seconds);
 
+/*
+ * Grid-aware compact source format.  The paper's sources are "spatially
+ * discretized cells": nodes of a regular grid.  When the cells are the nodes
+ *     R(ix, iy, iz) = origin + spacing * (ix, iy, iz),   0 <= i_k < n[k]   (cubic cells)
+ * the library keeps a second copy that stores only the charges (4 B FP32 / 8 B FP64 per cell
+ * instead of 16 / 32 B) and regenerates the coordinates from the indices.  Its kernels walk
+ * the z rows of the grid, where dx, dy and dx^2 + dy^2 are row constants: 12 FP32 (13 FP64)
+ * lane operations per pair instead of 17 (18).  Same V and E as the list kernels up to
+ * rounding (FP64: node coordinates are origin + i*spacing, within 16 ulp of the listed
+ * positions; tolerances as for the list).  Empty (masked) cells are zero charges.
+ *
+ * qmmm_field_create detects the structure by itself (every source must lie on a node within
+ * 16 ulp of the largest coordinate, no node twice, at least half of the bounding grid
+ * occupied, M >= 4096); qmmm_field_create_grid takes the grid directly:
+ *   origin [3]                  position of node (0,0,0), bohr (host pointer)
+ *   spacing                     cell edge h > 0, bohr
+ *   n [3]                       nodes per axis, 1..65536 each, at most 2e9 cells (host pointer)
+ *   cell_q [n0][n1][n2]         cell CHARGES, C order (z fastest), host or device pointer;
+ *                               0 = no cell there
+ *   nuclei, max_points, out     as qmmm_field_create
+ * A handle made by qmmm_field_create_grid has no source list (layout LIST is refused; the
+ * single-point move server is not used).  Precondition of the grid layout: no evaluation
+ * point coincides with a node that carries charge (empty nodes are harmless).
+ * Errors as qmmm_field_create.
+ */
+qmmm_status qmmm_field_create_grid(const double *origin, double spacing, const int64_t *n,
+                                   const double *cell_q, const double *nuc_xyz,
+                                   const double *nuc_Z, int64_t K, int64_t max_points,
+                                   qmmm_field **out);
+
+/* Which copy qmmm_field_eval uses.  AUTO (default): the grid kernels when the handle has a
+ * grid and the launch plan leaves every source-split warp group at least 4 work units of
+ * 32 rows x 64 nodes (many points per evaluation); otherwise the list.  LIST / GRID force one
+ * (INVALID_ARG if the handle does not have that copy).  Sticky. */
+typedef enum { QMMM_LAYOUT_AUTO = 0, QMMM_LAYOUT_LIST = 1, QMMM_LAYOUT_GRID = 2 } qmmm_layout;
+qmmm_status qmmm_field_set_layout(qmmm_field *h, int layout);
+
+typedef struct {
+    int32_t present;             /* 1 if the handle has a grid copy */
+    int32_t has_list;            /* 1 if the handle has a source list */
+    int32_t layout;              /* qmmm_layout set by qmmm_field_set_layout */
+    int32_t last_layout;         /* LIST or GRID: what the most recent eval used */
+    int32_t n[3];                /* nodes per axis */
+    int32_t reserved;
+    double origin[3];            /* node (0,0,0), bohr */
+    double spacing;              /* h, bohr */
+    int64_t n_gchunks;           /* work units of 32 rows x 64 z nodes (after padding) */
+    int64_t bytes_fp32, bytes_fp64;
+} qmmm_grid_info;
+qmmm_status qmmm_field_get_grid_info(const qmmm_field *h, qmmm_grid_info *info);
+
 /* qmmm_field_destroy -- frees the handle and its device buffers.  NULL is a no-op. */
 qmmm_status qmmm_field_destroy(qmmm_field *h);
 

@@ -26,7 +26,8 @@ _STATUS = {0: "QMMM_OK", 1: "QMMM_ERR_INVALID_ARG", 2: "QMMM_ERR_ALLOC", 3: "QMM
 LIB_PATH = os.environ.get("QMMM_FIELD_LIB") or os.path.join(
     os.path.dirname(os.path.abspath(__file__)), "libqmmm_field.so")
 EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_host",
-                    "qmmm_field_eval_moves_host",
+                    "qmmm_field_eval_moves_host", "qmmm_field_create_grid",
+                    "qmmm_field_set_layout", "qmmm_field_get_grid_info",
                     "qmmm_field_destroy", "qmmm_field_set_plan", "qmmm_field_get_info",
                     "qmmm_field_set_timing", "qmmm_field_last_timing",
                     "qmmm_probe_peak", "qmmm_last_error")
@@ -52,6 +53,19 @@ class qmmm_field_info(ctypes.Structure):
                 ("reserved", ctypes.c_int32)]
 
 
+class qmmm_grid_info(ctypes.Structure):
+    _fields_ = [("present", ctypes.c_int32), ("has_list", ctypes.c_int32),
+                ("layout", ctypes.c_int32), ("last_layout", ctypes.c_int32),
+                ("n", ctypes.c_int32 * 3), ("reserved", ctypes.c_int32),
+                ("origin", ctypes.c_double * 3), ("spacing", ctypes.c_double),
+                ("n_gchunks", ctypes.c_int64), ("bytes_fp32", ctypes.c_int64),
+                ("bytes_fp64", ctypes.c_int64)]
+
+
+QMMM_LAYOUT_AUTO, QMMM_LAYOUT_LIST, QMMM_LAYOUT_GRID = 0, 1, 2
+_LAYOUT = {"auto": 0, "list": 1, "grid": 2, 0: 0, 1: 1, 2: 2}
+
+
 def _load() -> ctypes.CDLL:
     if not os.path.exists(LIB_PATH):
         raise ImportError(
@@ -68,6 +82,14 @@ def _load() -> ctypes.CDLL:
     lib.qmmm_field_eval_moves_host.restype = ci
     lib.qmmm_field_eval_moves_host.argtypes = [vp, vp, i64, i64, vp, vp, ci, vp,
                                                ctypes.POINTER(ctypes.c_double)]
+    lib.qmmm_field_create_grid.restype = ci
+    lib.qmmm_field_create_grid.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.c_double,
+                                           ctypes.POINTER(i64), vp, vp, vp, i64, i64,
+                                           ctypes.POINTER(vp)]
+    lib.qmmm_field_set_layout.restype = ci
+    lib.qmmm_field_set_layout.argtypes = [vp, ci]
+    lib.qmmm_field_get_grid_info.restype = ci
+    lib.qmmm_field_get_grid_info.argtypes = [vp, ctypes.POINTER(qmmm_grid_info)]
     lib.qmmm_field_destroy.restype = ci
     lib.qmmm_field_destroy.argtypes = [vp]
     lib.qmmm_field_set_plan.restype = ci
@@ -122,6 +144,36 @@ def qmmm_field_create(src_xyz, src_q, nuc_xyz, nuc_Z, max_points: int) -> int:
     _check(_lib.qmmm_field_create(_ptr(src_xyz), _ptr(src_q), M, _ptr(nuc_xyz), _ptr(nuc_Z), K,
                                   int(max_points), ctypes.byref(out)))
     return out.value
+
+
+def qmmm_field_create_grid(origin, spacing: float, n, cell_q, nuc_xyz, nuc_Z,
+                           max_points: int) -> int:
+    """Environment given as a cubic grid: node (0,0,0) at ``origin``, edge ``spacing``,
+    ``cell_q`` [n0,n1,n2] FP64 cell charges (C order; 0 = no cell), host or device."""
+    org = (ctypes.c_double * 3)(*[float(v) for v in origin])
+    dims = (ctypes.c_int64 * 3)(*[int(v) for v in n])
+    assert cell_q is not None and tuple(cell_q.shape) == tuple(int(v) for v in n)
+    K = int(nuc_Z.shape[0]) if nuc_Z is not None else 0
+    out = ctypes.c_void_p()
+    _check(_lib.qmmm_field_create_grid(org, float(spacing), dims, _ptr(cell_q), _ptr(nuc_xyz),
+                                       _ptr(nuc_Z), K, int(max_points), ctypes.byref(out)))
+    return out.value
+
+
+def qmmm_field_set_layout(handle: int, layout="auto") -> None:
+    """"auto" | "list" | "grid": which copy of the sources eval uses."""
+    _check(_lib.qmmm_field_set_layout(handle, _LAYOUT[layout]))
+
+
+def qmmm_field_get_grid_info(handle: int) -> dict:
+    info = qmmm_grid_info()
+    _check(_lib.qmmm_field_get_grid_info(handle, ctypes.byref(info)))
+    names = {0: "auto", 1: "list", 2: "grid"}
+    return {"present": bool(info.present), "has_list": bool(info.has_list),
+            "layout": names[info.layout], "last_layout": names[info.last_layout],
+            "n": tuple(info.n), "origin": tuple(info.origin), "spacing": info.spacing,
+            "n_gchunks": info.n_gchunks, "bytes_fp32": info.bytes_fp32,
+            "bytes_fp64": info.bytes_fp64}
 
 
 def qmmm_field_eval(handle: int, elec_xyz, W: int, N: int, V, E=None, precision="fp64",

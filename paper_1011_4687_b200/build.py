@@ -15,7 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libqmmm_field.so")
 SOURCES = ["qmmm_field.cu", "qmmm_probe.cu"]
-HEADERS = [os.path.join(CSRC, "qmmm_kernels.cuh"),
+HEADERS = [os.path.join(CSRC, "qmmm_kernels.cuh"), os.path.join(CSRC, "qmmm_grid.cuh"),
+           os.path.join(CSRC, "qmmm_server.cuh"),
            os.path.join(os.path.dirname(HERE), "include", "qmmm_field.h")]
 # No --use_fast_math: the approximate instructions the kernels want are called
 # explicitly.  -lineinfo keeps ncu's source page usable.

@@ -8,6 +8,7 @@
 // No torch types, no CPU fallback: every step of the path runs in the kernels of
 // qmmm_kernels.cuh.
 #include "qmmm_kernels.cuh"
+#include "qmmm_grid.cuh"
 #include "qmmm_server.cuh"
 
 #include <algorithm>
@@ -68,6 +69,15 @@ size_t pair_smem_bytes(bool f32, int stages, int ept, int wp) {
            static_cast<size_t>(wp) * ept * 3 * sizeof(double);
 }
 
+size_t grid_smem_bytes(bool f32, int stages, int ept, int wp) {
+    if (f32 && ept == 8) return GridF32Layout<4>::total(stages);
+    if (f32 && ept == 4) return GridF32Layout<2>::total(stages);
+    if (f32) return GridF32Layout<1>::total(stages);
+    return static_cast<size_t>(stages) * GRID_STAGE_BYTES_F64 + 18 * sizeof(uint64_t) +
+           static_cast<size_t>(32) * COMPUTE_WARPS * sizeof(double) +
+           static_cast<size_t>(wp) * ept * 3 * sizeof(double);
+}
+
 }  // namespace
 
 struct qmmm_field {
@@ -99,19 +109,30 @@ struct qmmm_field {
     int srv_prec = -1;
     unsigned long long srv_launch_id = 0, srv_seq = 0;
     int *counters = nullptr;       // [max_points] arrival tickets of the point blocks (zero at rest)
+    // grid layout (qmmm_grid.cuh): present when the cells are nodes of a cubic grid
+    bool has_list = true, has_grid = false;
+    GridGeom grid = {{0, 0, 0}, 1.0, {0, 0, 0}, 0.0};
+    int64_t g_rows = 0, g_tiles = 0, g_segs = 0, n_g = 0;
+    float *gcells32 = nullptr;     // [n_g][ZS/4][32][4]
+    double *gcells64 = nullptr;    // [n_g][ZS/2][32][2]
+    double *nuclei_u = nullptr;    // [K][4] nuclei in grid units
+    int layout = QMMM_LAYOUT_AUTO, last_layout = QMMM_LAYOUT_LIST;
+    double bb_lo[3] = {0, 0, 0}, bb_hi[3] = {0, 0, 0};   // bounding box of the cells
 };
 
 namespace {
 
 // Automatic plan: enough (point block x source slice) CTAs to fill the
 // SMs in whole waves; few points -> sources split across all warps and SMs.
-qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32) {
+qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32, bool grid = false) {
     qmmm_plan pl = h->user_plan;
     const int max_ept = f32 ? 8 : 4;
     if (pl.points_per_thread == 0) pl.points_per_thread = std::min(max_ept, pow2_ceil(P));
     pl.points_per_thread = std::min(pl.points_per_thread, max_ept);
+    if (grid && f32) pl.points_per_thread = std::max(pl.points_per_thread, 2);   // packed pairs only
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
-    const int nw = (f32 && pl.points_per_thread >= 2) ? f32x2_warps(pl.points_per_thread) : COMPUTE_WARPS;
+    const int nw = grid ? COMPUTE_WARPS
+                        : ((f32 && pl.points_per_thread >= 2) ? f32x2_warps(pl.points_per_thread) : COMPUTE_WARPS);
     if (pl.point_warps == 0) {
         // as many point warps as there are groups, but keep at least 4 point blocks when the
         // points allow it: slices = SMs / 4 then, so every CTA streams a 4x longer source run
@@ -126,16 +147,30 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32) {
         const int g = gcd_int(static_cast<int>(pb % h->sm_count), h->sm_count);
         pl.slices = h->sm_count / g;       // pb * slices is a multiple of the SM count
     }
-    const int64_t work_units = f32 ? std::max<int64_t>(h->n_chunks, (h->K + 31) / 32) : h->n_chunks64;
+    const int64_t work_units = grid ? std::max<int64_t>(h->n_g, (h->K + 31) / 32)
+                               : f32 ? std::max<int64_t>(h->n_chunks, (h->K + 31) / 32) : h->n_chunks64;
     pl.slices = static_cast<int>(std::max<int64_t>(1, std::min<int64_t>(pl.slices, work_units)));
     // the partials workspace bounds slices * P
     const int64_t cap = h->workspace_doubles / (4 * P);
     if (pl.slices > cap) pl.slices = static_cast<int>(std::max<int64_t>(1, cap));
     if (pl.stages == 0) {
         const bool bandwidth_bound = groups <= 2;
-        pl.stages = f32 ? (pl.points_per_thread == 1 ? 6 : 4) : (bandwidth_bound ? 6 : 3);
+        if (grid)        // the source-split warp groups take the stages round-robin: one each + 1
+            pl.stages = std::min(8, std::max(f32 ? 6 : 4, nw / pl.point_warps + 1));
+        else
+            pl.stages = f32 ? (pl.points_per_thread == 1 ? 6 : 4) : (bandwidth_bound ? 6 : 3);
     }
     return pl;
+}
+
+// AUTO layout: the grid kernels when the handle has a grid and every source-split warp group
+// of every slice gets at least a few gchunks (32 rows x 64 nodes each); else the source list.
+bool auto_uses_grid(const qmmm_field *h, int64_t P, bool f32) {
+    if (!h->has_grid) return false;
+    if (!h->has_list) return true;
+    const qmmm_plan pl = choose_plan(h, P, f32, true);
+    const int ws = COMPUTE_WARPS / pl.point_warps;
+    return h->n_g >= static_cast<int64_t>(4) * pl.slices * ws;
 }
 
 template <typename REAL, int EPT, bool WITH_E = true>
@@ -193,6 +228,57 @@ cudaError_t launch_pair_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
     return cudaErrorInvalidValue;
 }
 
+template <int EP2>
+cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
+    auto kern = grid_kernel_f32x2<EP2>;
+    static thread_local size_t configured = 0;
+    if (smem > configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             static_cast<int>(smem));
+        if (e != cudaSuccess) return e;
+        configured = smem;
+    }
+    kern<<<grid, CTA_THREADS, smem, st>>>(prm);
+    return cudaGetLastError();
+}
+template <int EPT, bool WITH_E>
+cudaError_t launch_grid_f64(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
+    auto kern = grid_kernel_f64<EPT, WITH_E>;
+    static thread_local size_t configured = 0;
+    if (smem > configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             static_cast<int>(smem));
+        if (e != cudaSuccess) return e;
+        configured = smem;
+    }
+    kern<<<grid, CTA_THREADS, smem, st>>>(prm);
+    return cudaGetLastError();
+}
+// Grid layout: FP32-acc64 packed kernel for 2, 4, 8 points per thread; FP64 for 1, 2, 4.
+cudaError_t launch_grid_ept(bool f32, int ept, const PairParams &prm, dim3 grid, size_t smem,
+                            cudaStream_t st) {
+    if (f32) {
+        switch (ept) {
+            case 2: return launch_grid_f32<1>(prm, grid, smem, st);
+            case 4: return launch_grid_f32<2>(prm, grid, smem, st);
+            case 8: return launch_grid_f32<4>(prm, grid, smem, st);
+        }
+    } else if (prm.E) {
+        switch (ept) {
+            case 1: return launch_grid_f64<1, true>(prm, grid, smem, st);
+            case 2: return launch_grid_f64<2, true>(prm, grid, smem, st);
+            case 4: return launch_grid_f64<4, true>(prm, grid, smem, st);
+        }
+    } else {
+        switch (ept) {
+            case 1: return launch_grid_f64<1, false>(prm, grid, smem, st);
+            case 2: return launch_grid_f64<2, false>(prm, grid, smem, st);
+            case 4: return launch_grid_f64<4, false>(prm, grid, smem, st);
+        }
+    }
+    return cudaErrorInvalidValue;
+}
+
 bool is_device_pointer(const void *p) {
     cudaPointerAttributes a;
     if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
@@ -215,6 +301,105 @@ cudaError_t to_device(const double *src, int64_t n, double **dev, bool *owned) {
     if (e != cudaSuccess) return e;
     *owned = true;
     return cudaMemcpy(*dev, src, n * sizeof(double), cudaMemcpyHostToDevice);
+}
+
+
+// ------------------------------------------------------------------ grid layout (8(f)-1)
+// Packs dense charges [nx][ny][nz] (device) into the FP32 and FP64 gchunk copies and converts
+// the packed nuclei (h->nuclei) to grid units.
+cudaError_t build_grid(qmmm_field *h, const double *ddense, const GridGeom &gg) {
+    h->grid = gg;
+    h->g_rows = static_cast<int64_t>(gg.n[0]) * gg.n[1];
+    h->g_tiles = (h->g_rows + 31) / 32;
+    h->g_segs = (gg.n[2] + GRID_ZS - 1) / GRID_ZS;
+    h->n_g = h->g_tiles * h->g_segs;
+    if (h->n_g < 1 || h->n_g > (int64_t(1) << 30)) return cudaErrorInvalidValue;
+    const int64_t rows_padded = h->g_tiles * 32;
+    cudaError_t e = cudaMalloc(&h->gcells32, h->n_g * GRID_NODES * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&h->gcells64, h->n_g * GRID_NODES * sizeof(double));
+    if (e != cudaSuccess) return e;
+    const unsigned nb = static_cast<unsigned>((rows_padded + 63) / 64);
+    grid_pack_kernel<float><<<nb, 64>>>(ddense, h->g_rows, gg.n[2], static_cast<int>(h->g_segs),
+                                        rows_padded, h->gcells32);
+    grid_pack_kernel<double><<<nb, 64>>>(ddense, h->g_rows, gg.n[2], static_cast<int>(h->g_segs),
+                                         rows_padded, h->gcells64);
+    if (h->K > 0) {
+        e = cudaMalloc(&h->nuclei_u, h->K * 4 * sizeof(double));
+        if (e != cudaSuccess) return e;
+        grid_nuclei_kernel<<<static_cast<unsigned>((h->K + 255) / 256), 256>>>(h->nuclei, h->K, gg,
+                                                                              h->nuclei_u);
+    }
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) h->has_grid = true;
+    return e;
+}
+
+// Are the cells nodes of a cubic grid ("spatially discretized cell")?  Candidate
+// spacing from the smallest positive coordinate step between consecutive sources, node
+// counts from the bounding box, then EVERY source is checked against its node (within a few
+// ulp of the coordinates) and no node may hold two sources.  Anything else keeps the list.
+cudaError_t detect_grid(qmmm_field *h, const double *dxyz, const double *dq, int64_t M) {
+    if (M < 4096) return cudaSuccess;
+    const int nb = static_cast<int>(std::min<int64_t>(256, (M + 255) / 256));
+    double *dpart = nullptr;
+    cudaError_t e = cudaMalloc(&dpart, 256 * 3 * sizeof(double));
+    if (e != cudaSuccess) return e;
+    double hpart[256 * 3];
+    grid_spacing_kernel<<<nb, 256>>>(dxyz, M, dpart);
+    e = cudaMemcpy(hpart, dpart, nb * 3 * sizeof(double), cudaMemcpyDeviceToHost);
+    cudaFree(dpart);
+    if (e != cudaSuccess) return e;
+    GridGeom gg;
+    double hcand[3], ext[3], maxabs = 0.0;
+    int best = -1;
+    for (int k = 0; k < 3; ++k) {
+        hcand[k] = 1e300;
+        for (int b = 0; b < nb; ++b) hcand[k] = std::min(hcand[k], hpart[3 * b + k]);
+        ext[k] = h->bb_hi[k] - h->bb_lo[k];
+        maxabs = std::max({maxabs, std::fabs(h->bb_lo[k]), std::fabs(h->bb_hi[k]), ext[k]});
+        gg.org[k] = h->bb_lo[k];
+        gg.n[k] = 1;
+        if (ext[k] > 0.0) {
+            if (!(hcand[k] < 1e299)) return cudaSuccess;
+            const double nn = std::rint(ext[k] / hcand[k]) + 1.0;
+            if (!(nn >= 2.0 && nn <= 65536.0)) return cudaSuccess;
+            gg.n[k] = static_cast<int>(nn);
+            if (best < 0 || gg.n[k] > gg.n[best]) best = k;
+        }
+    }
+    if (best < 0) return cudaSuccess;
+    gg.h = ext[best] / (gg.n[best] - 1);
+    gg.tol = 16.0 * 2.220446049250313e-16 * maxabs;
+    const double total = static_cast<double>(gg.n[0]) * gg.n[1] * gg.n[2];
+    if (total > 2.0 * static_cast<double>(M) + 65536.0 || total > 2.0e9) return cudaSuccess;   // too sparse
+    for (int k = 0; k < 3; ++k)
+        if (std::fabs(ext[k] - (gg.n[k] - 1) * gg.h) > gg.tol) return cudaSuccess;           // not cubic cells
+    const int64_t ntot = static_cast<int64_t>(total);
+    double *ddense = nullptr;
+    int *dcount = nullptr;
+    e = cudaMalloc(&ddense, ntot * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&dcount, (ntot + 2) * sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(ddense, 0, ntot * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemset(dcount, 0, (ntot + 2) * sizeof(int));
+    int bad[2] = {1, 1};
+    if (e == cudaSuccess) {
+        grid_scatter_kernel<<<static_cast<unsigned>((M + 255) / 256), 256>>>(dxyz, dq, M, gg, ddense,
+                                                                            dcount + 2, dcount);
+        e = cudaMemcpy(bad, dcount, sizeof(bad), cudaMemcpyDeviceToHost);
+    }
+    if (e == cudaSuccess && bad[0] == 0 && bad[1] == 0) e = build_grid(h, ddense, gg);
+    cudaFree(ddense);
+    cudaFree(dcount);
+    if (e == cudaErrorMemoryAllocation) {      // no room for the extra copies: keep the list only
+        cudaGetLastError();
+        cudaFree(h->gcells32); h->gcells32 = nullptr;
+        cudaFree(h->gcells64); h->gcells64 = nullptr;
+        cudaFree(h->nuclei_u); h->nuclei_u = nullptr;
+        h->has_grid = false;
+        return cudaSuccess;
+    }
+    return e;
 }
 
 }  // namespace
@@ -280,7 +465,7 @@ qmmm_status server_start(qmmm_field *h, int prec, bool *usable) {
     const bool f32 = prec == QMMM_FP32_ACC64;
     *usable = false;
     const int64_t n_chunks = f32 ? h->n_chunks : h->n_chunks64;
-    if (!h->srv_ok || n_chunks < 1 || h->timing) return QMMM_OK;
+    if (!h->srv_ok || n_chunks < 1 || h->timing || !h->has_list || h->layout == QMMM_LAYOUT_GRID) return QMMM_OK;
     qmmm_plan pl = choose_plan(h, 1, f32);
     if (pl.points_per_thread != 1 || pl.point_warps != 1 || pl.slices > h->sm_count) return QMMM_OK;
     const size_t extra = 128 + static_cast<size_t>(pl.slices) * 4 * sizeof(double);   // cmd, go, collected partials
@@ -379,6 +564,45 @@ qmmm_status server_move(qmmm_field *h, const double *r, double *V, double *E, in
 
 }  // namespace
 
+namespace {
+// Per-handle buffers that do not depend on the source format: partials workspace, tickets,
+// mailboxes, move-server state, eval_host staging.
+qmmm_status alloc_runtime(qmmm_field *h) {
+#define RT_TRY(expr)                                                                       \
+    do {                                                                                   \
+        cudaError_t _e = (expr);                                                           \
+        if (_e == cudaErrorMemoryAllocation)                                               \
+            return fail(QMMM_ERR_ALLOC, std::string(#expr) + ": out of memory");           \
+        if (_e != cudaSuccess) return cuda_fail(_e, #expr);                                \
+    } while (0)
+    // Partials workspace: slices * P * 4 doubles.  With P = h->max_points the automatic plan
+    // uses at most sm_count slices; small P uses more slices but a smaller product.
+    h->workspace_doubles =
+        4 * std::max<int64_t>(static_cast<int64_t>(h->sm_count) * h->max_points, int64_t(1) << 16);
+    RT_TRY(cudaMalloc(&h->workspace, h->workspace_doubles * sizeof(double)));
+    RT_TRY(cudaMalloc(&h->counters, (h->max_points + 1) * sizeof(int)));      // + 1: mailbox `done`
+    RT_TRY(cudaMemset(h->counters, 0, (h->max_points + 1) * sizeof(int)));
+    RT_TRY(cudaHostAlloc(&h->mail_h, (MAIL_POINTS * 7 + 1) * sizeof(double), cudaHostAllocMapped));
+    std::memset(h->mail_h, 0, (MAIL_POINTS * 7 + 1) * sizeof(double));
+    RT_TRY(cudaHostGetDevicePointer(&h->mail_d, h->mail_h, 0));
+    RT_TRY(cudaHostAlloc(&h->srv_mail_h, sizeof(ServerMailbox), cudaHostAllocMapped));
+    std::memset(h->srv_mail_h, 0, sizeof(ServerMailbox));
+    RT_TRY(cudaHostGetDevicePointer(&h->srv_mail_d, h->srv_mail_h, 0));
+    RT_TRY(cudaMalloc(&h->srv_dev, sizeof(ServerDevice)));
+    RT_TRY(cudaStreamCreateWithFlags(&h->srv_stream, cudaStreamNonBlocking));
+    {
+        int coop = 0;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device);
+        h->srv_ok = coop != 0;
+    }
+    RT_TRY(cudaMalloc(&h->stage_elec, h->max_points * 3 * sizeof(double)));
+    RT_TRY(cudaMalloc(&h->stage_out, h->max_points * 4 * sizeof(double)));
+#undef RT_TRY
+    return QMMM_OK;
+}
+
+}  // namespace
+
 // =============================================================================== C ABI
 extern "C" {
 
@@ -466,6 +690,8 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
                         lo = std::min(lo, hbb[6 * b + k]);
                         hi = std::max(hi, hbb[6 * b + 3 + k]);
                     }
+                    h->bb_lo[k] = lo;
+                    h->bb_hi[k] = hi;
                     ext = std::max(ext, hi - lo);
                 }
                 if (!(ext > 0.0) || !std::isfinite(ext)) ext = 1.0;
@@ -483,36 +709,129 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
         }
         if (e == cudaSuccess) e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        // grid-aware compact copies when the cells are nodes of a cubic grid (8(f)-1)
+        if (e == cudaSuccess && M > 0) e = detect_grid(h, dxyz, dq, M);
         if (own[0]) cudaFree(dxyz);
         if (own[1]) cudaFree(dq);
         if (own[2]) cudaFree(dnxyz);
         if (own[3]) cudaFree(dnz);
         CREATE_TRY(e);
     }
-    // Partials workspace: slices * P * 4 doubles.  With P = max_points the automatic plan
-    // uses at most sm_count slices; small P uses more slices but a smaller product.
-    h->workspace_doubles =
-        4 * std::max<int64_t>(static_cast<int64_t>(h->sm_count) * max_points, int64_t(1) << 16);
-    CREATE_TRY(cudaMalloc(&h->workspace, h->workspace_doubles * sizeof(double)));
-    CREATE_TRY(cudaMalloc(&h->counters, (max_points + 1) * sizeof(int)));      // + 1: mailbox `done`
-    CREATE_TRY(cudaMemset(h->counters, 0, (max_points + 1) * sizeof(int)));
-    CREATE_TRY(cudaHostAlloc(&h->mail_h, (MAIL_POINTS * 7 + 1) * sizeof(double), cudaHostAllocMapped));
-    std::memset(h->mail_h, 0, (MAIL_POINTS * 7 + 1) * sizeof(double));
-    CREATE_TRY(cudaHostGetDevicePointer(&h->mail_d, h->mail_h, 0));
-    CREATE_TRY(cudaHostAlloc(&h->srv_mail_h, sizeof(ServerMailbox), cudaHostAllocMapped));
-    std::memset(h->srv_mail_h, 0, sizeof(ServerMailbox));
-    CREATE_TRY(cudaHostGetDevicePointer(&h->srv_mail_d, h->srv_mail_h, 0));
-    CREATE_TRY(cudaMalloc(&h->srv_dev, sizeof(ServerDevice)));
-    CREATE_TRY(cudaStreamCreateWithFlags(&h->srv_stream, cudaStreamNonBlocking));
     {
-        int coop = 0;
-        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-        h->srv_ok = coop != 0;
+        qmmm_status rs = alloc_runtime(h);
+        if (rs != QMMM_OK) return bail(rs);
     }
-    CREATE_TRY(cudaMalloc(&h->stage_elec, max_points * 3 * sizeof(double)));
-    CREATE_TRY(cudaMalloc(&h->stage_out, max_points * 4 * sizeof(double)));
 #undef CREATE_TRY
     *out = h;
+    return QMMM_OK;
+}
+
+qmmm_status qmmm_field_create_grid(const double *origin, double spacing, const int64_t *n,
+                                   const double *cell_q, const double *nuc_xyz,
+                                   const double *nuc_Z, int64_t K, int64_t max_points,
+                                   qmmm_field **out) {
+    if (!out) return fail(QMMM_ERR_INVALID_ARG, "create_grid: out is NULL");
+    *out = nullptr;
+    if (!origin || !n || !cell_q) return fail(QMMM_ERR_INVALID_ARG, "create_grid: NULL origin, n or cell_q");
+    if (!(spacing > 0.0) || !std::isfinite(spacing))
+        return fail(QMMM_ERR_INVALID_ARG, "create_grid: spacing must be positive and finite");
+    for (int k = 0; k < 3; ++k)
+        if (n[k] < 1 || n[k] > 65536) return fail(QMMM_ERR_INVALID_ARG, "create_grid: n[k] must be in [1, 65536]");
+    const double total = static_cast<double>(n[0]) * n[1] * n[2];
+    if (total > 2.0e9) return fail(QMMM_ERR_INVALID_ARG, "create_grid: more than 2e9 cells");
+    if (K < 0) return fail(QMMM_ERR_INVALID_ARG, "create_grid: negative K");
+    if (max_points < 1) return fail(QMMM_ERR_INVALID_ARG, "create_grid: max_points < 1");
+    if (K > 0 && (!nuc_xyz || !nuc_Z))
+        return fail(QMMM_ERR_INVALID_ARG, "create_grid: NULL nuclear array with K > 0");
+
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10)
+        return fail(QMMM_ERR_UNSUPPORTED_DEVICE,
+                    "create_grid: device is sm_" + std::to_string(prop.major * 10 + prop.minor) +
+                        ", this library is built for sm_100a (B200) only");
+    qmmm_field *h = new (std::nothrow) qmmm_field();
+    if (!h) return fail(QMMM_ERR_ALLOC, "create_grid: host allocation failed");
+    h->K = K; h->max_points = max_points;
+    h->device = dev; h->sm_count = prop.multiProcessorCount;
+    h->has_list = false;
+    auto bail = [&](qmmm_status st) { qmmm_field_destroy(h); return st; };
+
+    const int64_t ntot = static_cast<int64_t>(total);
+    GridGeom gg;
+    for (int k = 0; k < 3; ++k) {
+        gg.org[k] = origin[k];
+        gg.n[k] = static_cast<int>(n[k]);
+        h->bb_lo[k] = origin[k];
+        h->bb_hi[k] = origin[k] + (n[k] - 1) * spacing;
+    }
+    gg.h = spacing;
+    gg.tol = 0.0;
+    double *dq = nullptr, *dnxyz = nullptr, *dnz = nullptr;
+    unsigned long long *dcnt = nullptr, cnt = 0;
+    bool own[3] = {false, false, false};
+    cudaError_t e = to_device(cell_q, ntot, &dq, &own[0]);
+    if (e == cudaSuccess) e = to_device(nuc_xyz, 3 * K, &dnxyz, &own[1]);
+    if (e == cudaSuccess) e = to_device(nuc_Z, K, &dnz, &own[2]);
+    if (e == cudaSuccess && K > 0) {
+        e = cudaMalloc(&h->nuclei, K * 4 * sizeof(double));
+        if (e == cudaSuccess)
+            pack_nuclei_kernel<<<static_cast<unsigned>((K + 255) / 256), 256>>>(dnxyz, dnz, K, h->nuclei);
+    }
+    if (e == cudaSuccess) e = cudaMalloc(&dcnt, sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(dcnt, 0, sizeof(unsigned long long));
+    if (e == cudaSuccess) {
+        grid_count_kernel<<<1024, 256>>>(dq, ntot, dcnt);
+        e = cudaMemcpy(&cnt, dcnt, sizeof(cnt), cudaMemcpyDeviceToHost);
+    }
+    if (e == cudaSuccess) e = build_grid(h, dq, gg);
+    cudaFree(dcnt);
+    if (own[0]) cudaFree(dq);
+    if (own[1]) cudaFree(dnxyz);
+    if (own[2]) cudaFree(dnz);
+    if (e == cudaErrorMemoryAllocation) return bail(fail(QMMM_ERR_ALLOC, "create_grid: out of device memory"));
+    if (e != cudaSuccess) return bail(cuda_fail(e, "create_grid"));
+    h->M = static_cast<int64_t>(cnt);            // non-empty cells
+    {
+        qmmm_status rs = alloc_runtime(h);
+        if (rs != QMMM_OK) return bail(rs);
+    }
+    *out = h;
+    return QMMM_OK;
+}
+
+qmmm_status qmmm_field_set_layout(qmmm_field *h, int layout) {
+    if (!h) return fail(QMMM_ERR_INVALID_ARG, "set_layout: NULL handle");
+    if (layout != QMMM_LAYOUT_AUTO && layout != QMMM_LAYOUT_LIST && layout != QMMM_LAYOUT_GRID)
+        return fail(QMMM_ERR_INVALID_ARG, "set_layout: unknown layout");
+    if (layout == QMMM_LAYOUT_GRID && !h->has_grid)
+        return fail(QMMM_ERR_INVALID_ARG, "set_layout: this environment has no grid copy (the cells are not nodes of a cubic grid)");
+    if (layout == QMMM_LAYOUT_LIST && !h->has_list)
+        return fail(QMMM_ERR_INVALID_ARG, "set_layout: this environment was created from a grid and has no source list");
+    server_stop(h);
+    h->layout = layout;
+    return QMMM_OK;
+}
+
+qmmm_status qmmm_field_get_grid_info(const qmmm_field *h, qmmm_grid_info *info) {
+    if (!h || !info) return fail(QMMM_ERR_INVALID_ARG, "get_grid_info: NULL argument");
+    std::memset(info, 0, sizeof(*info));
+    info->present = h->has_grid ? 1 : 0;
+    info->has_list = h->has_list ? 1 : 0;
+    info->layout = h->layout;
+    info->last_layout = h->last_layout;
+    if (h->has_grid) {
+        for (int k = 0; k < 3; ++k) {
+            info->n[k] = h->grid.n[k];
+            info->origin[k] = h->grid.org[k];
+        }
+        info->spacing = h->grid.h;
+        info->n_gchunks = h->n_g;
+        info->bytes_fp32 = h->n_g * GRID_NODES * 4;
+        info->bytes_fp64 = h->n_g * GRID_NODES * 8;
+    }
     return QMMM_OK;
 }
 
@@ -526,6 +845,9 @@ qmmm_status qmmm_field_destroy(qmmm_field *h) {
     cudaFree(h->chunks32);
     cudaFree(h->origins);
     cudaFree(h->nuclei);
+    cudaFree(h->gcells32);
+    cudaFree(h->gcells64);
+    cudaFree(h->nuclei_u);
     cudaFree(h->workspace);
     cudaFree(h->counters);
     if (h->mail_h) cudaFreeHost(h->mail_h);
@@ -609,48 +931,72 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
         if (ss != QMMM_OK) return ss;
     }
 
-    qmmm_plan pl = choose_plan(h, P, f32);
+    const bool grid = h->layout == QMMM_LAYOUT_GRID ||
+                      (h->layout == QMMM_LAYOUT_AUTO && auto_uses_grid(h, P, f32));
+    qmmm_plan pl = choose_plan(h, P, f32, grid);
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
     const int pb = static_cast<int>((groups + pl.point_warps - 1) / pl.point_warps);
     int launches = 0;
-    size_t smem = pair_smem_bytes(f32, pl.stages, pl.points_per_thread, pl.point_warps);
+    auto smem_of = [&](int stages) {
+        return grid ? grid_smem_bytes(f32, stages, pl.points_per_thread, pl.point_warps)
+                    : pair_smem_bytes(f32, stages, pl.points_per_thread, pl.point_warps);
+    };
+    size_t smem = smem_of(pl.stages);
     while (smem > 227 * 1024 && pl.stages > 2)           // a requested depth that does not fit is reduced
-        smem = pair_smem_bytes(f32, --pl.stages, pl.points_per_thread, pl.point_warps);
+        smem = smem_of(--pl.stages);
     if (smem > 227 * 1024) return fail(QMMM_ERR_INVALID_ARG, "eval: plan exceeds shared memory");
 
     if (h->timing) CUDA_TRY(cudaEventRecord(h->ev[0], st));
     {
         PairParams prm;
-        prm.chunks = f32 ? reinterpret_cast<const char *>(h->chunks32)
-                         : reinterpret_cast<const char *>(h->chunks64);
-        prm.origins = h->origins;
+        std::memset(&prm, 0, sizeof(prm));
         prm.elec = elec_xyz;
         prm.partial = h->workspace;
         prm.P = P;
-        prm.n_chunks = static_cast<int>(f32 ? h->n_chunks : h->n_chunks64);
         prm.slices = pl.slices;
         prm.point_warps = pl.point_warps;
         prm.stages = pl.stages;
-        prm.lattice = h->lattice;
-        prm.inv_lattice = 1.0 / h->lattice;
-        prm.nuc = h->nuclei;
-        prm.K = f32 ? static_cast<int>(h->K) : 0;     // FP64: nuclei are in the chunk array
         prm.V = V;
         prm.E = E;
         prm.counters = h->counters;
         prm.host_flag = host_flag;
         prm.seq = h->seq;
         prm.done = h->counters + h->max_points;
+        if (grid) {
+            // cells: charges only, coordinates from the indices; everything in grid units
+            prm.chunks = f32 ? reinterpret_cast<const char *>(h->gcells32)
+                             : reinterpret_cast<const char *>(h->gcells64);
+            prm.n_chunks = static_cast<int>(h->n_g);
+            prm.nuc = h->nuclei_u;
+            prm.K = static_cast<int>(h->K);
+            for (int k = 0; k < 3; ++k) prm.g_org[k] = h->grid.org[k];
+            prm.g_inv_h = 1.0 / h->grid.h;
+            prm.g_scaleV = 1.0 / h->grid.h;
+            prm.g_scaleE = 1.0 / (h->grid.h * h->grid.h);
+            prm.g_ny = h->grid.n[1];
+            prm.g_segs = static_cast<int>(h->g_segs);
+        } else {
+            prm.chunks = f32 ? reinterpret_cast<const char *>(h->chunks32)
+                             : reinterpret_cast<const char *>(h->chunks64);
+            prm.origins = h->origins;
+            prm.n_chunks = static_cast<int>(f32 ? h->n_chunks : h->n_chunks64);
+            prm.lattice = h->lattice;
+            prm.inv_lattice = 1.0 / h->lattice;
+            prm.nuc = h->nuclei;
+            prm.K = f32 ? static_cast<int>(h->K) : 0;     // FP64: nuclei are in the chunk array
+        }
 #ifdef QMMM_PHASE_TIMING
         prm.dbg = reinterpret_cast<long long *>(h->workspace + h->workspace_doubles - 16384);
 #endif
         // point blocks vary fastest: the CTAs resident together read the same source slices,
         // so a slice is fetched from HBM once and then served from L2
-        const dim3 grid(pb, pl.slices);
-        cudaError_t e = launch_pair_ept(f32, pl.points_per_thread, prm, grid, smem, st);
+        const dim3 grid_dim(pb, pl.slices);
+        cudaError_t e = grid ? launch_grid_ept(f32, pl.points_per_thread, prm, grid_dim, smem, st)
+                             : launch_pair_ept(f32, pl.points_per_thread, prm, grid_dim, smem, st);
         if (e != cudaSuccess) return cuda_fail(e, "pair_kernel launch");
         ++launches;
     }
+    h->last_layout = grid ? QMMM_LAYOUT_GRID : QMMM_LAYOUT_LIST;
     if (h->timing) {
         CUDA_TRY(cudaEventRecord(h->ev[1], st));
         h->timed = true;

@@ -1,0 +1,556 @@
+// qmmm_grid.cuh -- grid-aware compact source format.
+//
+// The paper's sources ARE "spatially discretized cells": nodes of a regular
+// grid.  When the cells of an environment are nodes origin + (ix, iy, iz) h of a cubic grid,
+// only the charges are stored (4 B FP32 / 8 B FP64 per cell instead of 16 / 32 B) and the
+// coordinates are regenerated from the indices.  Everything is computed in GRID UNITS
+// (u = (r - origin) / h, nodes at integer coordinates; V = sum / h, E = sum / h^2 at the end).
+//
+// Mapping: a "row" is the nz nodes of one (ix, iy); the 32 lanes of a warp own 32 DIFFERENT
+// rows of a row tile and walk along z together.  For a point i and a row, dx, dy and
+// dx^2 + dy^2 are constants of the row walk, and so is the x, y part of the field:
+//     r^2  = (dx^2 + dy^2) + dz^2                       1 add (dz) + 1 fma per pair
+//     Ex  += dx * sum_k s_k,  Ey += dy * sum_k s_k      1 add per pair (sum s), not 2 fma
+//     Ez  += sum_k s_k dz_k                             1 fma per pair
+// which leaves 12 FP32 (13 FP64) lane operations per pair instead of 17 (18) for a source
+// list: dz, r^2, the 4 (5) refinement operations, p = q y, V += p,
+// y^2, s = p y^2, sum s, sum s dz.
+//
+// Work unit ("gchunk"): 32 rows x ZS = 64 consecutive z nodes, stored [ZS/4][32][4] (FP32) or
+// [ZS/2][32][2] (FP64) so that a lane's 128-bit shared-memory loads are conflict-free.  One
+// TMA bulk copy per gchunk and pipeline stage.  Slices (Eq. 5-6) are
+// ranges of gchunks; the source-split warp groups of a CTA take the stages round-robin.
+// Masked-out cells are zero charges (they contribute exactly 0: r^2 carries a tiny positive
+// offset so that a coincident zero-charge node cannot produce 0 * inf).
+#pragma once
+#include "qmmm_kernels.cuh"
+
+namespace qmmm {
+
+constexpr int GRID_ZS = 64;                         // z nodes per gchunk
+constexpr int GRID_NODES = 32 * GRID_ZS;            // cells per gchunk
+
+// ----------------------------------------------------------------------------- FP32 packed
+template <int EP2>
+struct GridF32Layout {
+    static constexpr int EPT = 2 * EP2;
+    static constexpr int NT = 32 * COMPUTE_WARPS;
+    static constexpr int STAGE_BYTES = GRID_NODES * sizeof(float);          // 8 KB
+    static constexpr int BAR_BYTES = 18 * sizeof(uint64_t);                 // 8 full, 8 empty, flag
+    static constexpr int ELEC_BYTES = COMPUTE_WARPS * EPT * 3 * sizeof(double);
+    static constexpr int SCRATCH_BYTES = COMPUTE_WARPS * 2 * EPT * sizeof(float);
+    static constexpr int ACC_BYTES = EPT * 4 * NT * sizeof(double);
+    __host__ __device__ static constexpr size_t total(int stages) {
+        return static_cast<size_t>(stages) * STAGE_BYTES + BAR_BYTES + ELEC_BYTES + SCRATCH_BYTES +
+               ACC_BYTES;
+    }
+};
+
+// z coordinate of a point relative to the first node of a z segment, on a power-of-two
+// lattice fine enough that every dz = azb - k (k = 0..ZS-1) is EXACT in FP32: the quantum is
+// 2^-24 of the power of two above the farthest node of the segment.  dd is the residual
+// that enters as the first-order correction V(a + dd) = V(a) - Ez(a) dd at the flush.
+__device__ __forceinline__ void z_on_lattice(double zb, float &azb, float &dd) {
+    const double far = fmax(fabs(zb), fabs(zb - (GRID_ZS - 1)));
+    const int ex = ilogb(far) + 1;                             // far < 2^ex
+    const double lam = scalbn(1.0, ex - 24);
+    const double a = rint(zb * scalbn(1.0, 24 - ex)) * lam;
+    azb = static_cast<float>(a);                               // exact
+    dd = static_cast<float>(zb - a);
+}
+
+// One gchunk for EP2 packed point pairs: the lane's row, ZS nodes along z.
+// 12 FP32 lane operations + 1 MUFU.RSQ per pair, + 1/4 (dz base step) + 5/16 (V tree).
+template <int EP2>
+__device__ __forceinline__ void gchunk_f32x2(const float *b, float2 (&azb)[EP2],
+                                             const float2 (&rxy2)[EP2], float2 (&v)[EP2],
+                                             float2 (&S)[EP2], float2 (&SZ)[EP2]) {
+#pragma unroll 1
+    for (int g = 0; g < GRID_ZS / 16; ++g) {
+        float2 v16[EP2];                          // middle level of the V tree: 16 nodes
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) v16[e] = f2(0.0f, 0.0f);
+#pragma unroll 1
+        for (int k4 = 0; k4 < 4; ++k4) {
+            const float4 Q = *reinterpret_cast<const float4 *>(b + (4 * g + k4) * 128);
+            const float qs[4] = {Q.x, Q.y, Q.z, Q.w};
+            // V is summed as a tree of short FP32 runs (4 nodes -> 16 -> gchunk): a long FP32
+            // running sum of slowly varying same-sign terms drifts
+            float2 Vc[EP2];
+#pragma unroll
+            for (int t = 0; t < 4; ++t) {
+                float2 dz[EP2], r2[EP2], y0[EP2];
+                const float2 qq = bc(qs[t]);
+#pragma unroll
+                for (int e = 0; e < EP2; ++e) {
+                    dz[e] = t == 0 ? azb[e] : __fadd2_rn(azb[e], bc(-static_cast<float>(t)));
+                    r2[e] = __ffma2_rn(dz[e], dz[e], rxy2[e]);
+                }
+#pragma unroll
+                for (int e = 0; e < EP2; ++e) {
+                    y0[e].x = rsqrt_mufu_f32(r2[e].x);
+                    y0[e].y = rsqrt_mufu_f32(r2[e].y);
+                }
+#pragma unroll
+                for (int e = 0; e < EP2; ++e) {       // one Newton step, then V and the E sums
+                    const float2 tt = __fmul2_rn(r2[e], y0[e]);
+                    const float2 err = __ffma2_rn(f2(-tt.x, -tt.y), y0[e], bc(1.0f));
+                    const float2 hh = __fmul2_rn(y0[e], bc(0.5f));
+                    const float2 y = __ffma2_rn(hh, err, y0[e]);
+                    const float2 p = __fmul2_rn(y, qq);
+                    Vc[e] = t == 0 ? p : __fadd2_rn(Vc[e], p);
+                    const float2 s = __fmul2_rn(p, __fmul2_rn(y, y));
+                    S[e] = __fadd2_rn(S[e], s);
+                    SZ[e] = __ffma2_rn(s, dz[e], SZ[e]);
+                }
+            }
+#pragma unroll
+            for (int e = 0; e < EP2; ++e) {
+                azb[e] = __fadd2_rn(azb[e], bc(-4.0f));           // exact (lattice multiples)
+                v16[e] = __fadd2_rn(v16[e], Vc[e]);
+            }
+        }
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) v[e] = __fadd2_rn(v[e], v16[e]);
+    }
+}
+
+// grid = (point_blocks, slices); EPT = 2 * EP2 points per thread; 8 consumer warps + 1 TMA
+// producer warp.  The FP64 running sums live in shared-memory columns as in
+// pair_kernel_f32x2.  prm.chunks = gchunks [n_chunks][ZS/4][32][4] float; prm.nuc = nuclei in
+// grid units; prm.elec in bohr (converted to grid units when staged).
+template <int EP2>
+__global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f32x2(const PairParams prm) {
+    using L = GridF32Layout<EP2>;
+    constexpr int EPT = L::EPT, NT = L::NT, STAGE_BYTES = L::STAGE_BYTES;
+
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int stages = prm.stages;
+    unsigned char *ptr = smem + static_cast<size_t>(stages) * STAGE_BYTES;
+    uint64_t *full = reinterpret_cast<uint64_t *>(ptr);
+    uint64_t *empty = full + 8;
+    int *flag = reinterpret_cast<int *>(empty + 8);
+    ptr += L::BAR_BYTES;
+    double *elec_s = reinterpret_cast<double *>(ptr);          // [WP*EPT][3], grid units
+    ptr += L::ELEC_BYTES;
+    float *scratch = reinterpret_cast<float *>(ptr);           // per warp: azb[EPT], ddz[EPT]
+    ptr += L::SCRATCH_BYTES;
+    double2 *acc = reinterpret_cast<double2 *>(ptr);           // [EPT*2][NT] double2
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int WP = prm.point_warps, WS = COMPUTE_WARPS / WP;
+    int lo, hi;
+    slice_range(prm.n_chunks, prm.slices, blockIdx.y, lo, hi);
+    const int nk = hi - lo;
+
+    const bool producer = warp == COMPUTE_WARPS && lane == 0;
+    int pk = 0;
+    auto load_step = [&]() {
+        const int slot = pk % stages;
+        if (pk >= stages) mbar_wait(&empty[slot], ((pk / stages) - 1) & 1);
+        mbar_expect_tx(&full[slot], STAGE_BYTES);
+        tma_bulk_g2s(smem + static_cast<size_t>(slot) * STAGE_BYTES,
+                     prm.chunks + static_cast<size_t>(lo + pk) * STAGE_BYTES, STAGE_BYTES,
+                     &full[slot]);
+        ++pk;
+    };
+    if (producer) {
+        for (int s = 0; s < stages; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], WP);          // stage k is consumed by the WP warps of group k % WS
+        }
+        fence_barrier_init();
+        while (pk < nk && pk < stages) load_step();
+    }
+    const int ppb = WP * EPT;
+    for (int i = threadIdx.x; i < ppb * 3; i += CTA_THREADS) {
+        int p = blockIdx.x * ppb + i / 3;
+        p = p < prm.P ? p : prm.P - 1;                          // clamp: duplicates are not written
+        const int comp = i % 3;
+        elec_s[i] = (prm.elec[static_cast<int64_t>(p) * 3 + comp] - prm.g_org[comp]) * prm.g_inv_h;
+    }
+    __syncthreads();
+
+    if (warp == COMPUTE_WARPS) {
+        if (lane == 0)
+            while (pk < nk) load_step();
+        return;
+    }
+
+    const int wp = warp % WP, ws = warp / WP;
+    double2 *my = acc + threadIdx.x;                 // this thread's column: my[i * NT]
+#pragma unroll
+    for (int i = 0; i < EPT * 2; ++i) my[i * NT] = make_double2(0.0, 0.0);
+    const double *pe = elec_s + wp * EPT * 3;
+    float *az_s = scratch + warp * 2 * EPT;          // azb[EPT]
+    float *dd_s = az_s + EPT;                        // ddz[EPT]
+
+    for (int k = ws; k < nk; k += WS) {
+        const int g = lo + k;
+        const int tile = g / prm.g_segs, seg = g - tile * prm.g_segs;
+        const int row = tile * 32 + lane;
+        const int ix = row / prm.g_ny;
+        const double fx = static_cast<double>(ix), fy = static_cast<double>(row - ix * prm.g_ny);
+        // z: the same for all lanes -> the first EPT lanes compute it for the warp
+        __syncwarp();
+        if (lane < EPT) {
+            float a, d;
+            z_on_lattice(pe[3 * lane + 2] - static_cast<double>(seg * GRID_ZS), a, d);
+            az_s[lane] = a;
+            dd_s[lane] = d;
+        }
+        __syncwarp();
+        float2 dx[EP2], dy[EP2], rxy2[EP2], azb[EP2], v[EP2], S[EP2], SZ[EP2];
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+            // x, y: the difference is formed in FP64 and rounded once (relative error 2^-24)
+            dx[e] = f2(static_cast<float>(pe[6 * e + 0] - fx), static_cast<float>(pe[6 * e + 3] - fx));
+            dy[e] = f2(static_cast<float>(pe[6 * e + 1] - fy), static_cast<float>(pe[6 * e + 4] - fy));
+            rxy2[e] = __ffma2_rn(dy[e], dy[e], __ffma2_rn(dx[e], dx[e], bc(1e-30f)));
+            azb[e] = *reinterpret_cast<const float2 *>(az_s + 2 * e);
+            v[e] = S[e] = SZ[e] = f2(0.0f, 0.0f);
+        }
+        const int slot = k % stages;
+        mbar_wait(&full[slot], (k / stages) & 1);
+        const float *data = reinterpret_cast<const float *>(smem + static_cast<size_t>(slot) * STAGE_BYTES);
+        gchunk_f32x2<EP2>(data + 4 * lane, azb, rxy2, v, S, SZ);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[slot]);
+        // flush the FP32 run into the FP64 columns; Ex = dx sum(s), Ey = dy sum(s), Ez = sum(s dz)
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+            const float2 ddz = *reinterpret_cast<const float2 *>(dd_s + 2 * e);
+            const float2 ex = __fmul2_rn(dx[e], S[e]), ey = __fmul2_rn(dy[e], S[e]);
+            const float2 corr = __fmul2_rn(SZ[e], ddz);
+            double2 t;
+            t = my[(4 * e + 0) * NT];
+            t.x += static_cast<double>(v[e].x) - static_cast<double>(corr.x);
+            t.y += static_cast<double>(v[e].y) - static_cast<double>(corr.y);
+            my[(4 * e + 0) * NT] = t;
+            t = my[(4 * e + 1) * NT];
+            t.x += static_cast<double>(ex.x);
+            t.y += static_cast<double>(ex.y);
+            my[(4 * e + 1) * NT] = t;
+            t = my[(4 * e + 2) * NT];
+            t.x += static_cast<double>(ey.x);
+            t.y += static_cast<double>(ey.y);
+            my[(4 * e + 2) * NT] = t;
+            t = my[(4 * e + 3) * NT];
+            t.x += static_cast<double>(SZ[e].x);
+            t.y += static_cast<double>(SZ[e].y);
+            my[(4 * e + 3) * NT] = t;
+        }
+    }
+
+    // nuclear term of this CTA's share, FP64, grid units, into the same columns
+    {
+        double nV[EPT], nEx[EPT], nEy[EPT], nEz[EPT];
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) nV[e] = nEx[e] = nEy[e] = nEz[e] = 0.0;
+        nuclei_share<EPT>(prm, pe, ws, WS, lane, nV, nEx, nEy, nEz);
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+            double2 t;
+            t = my[(4 * e + 0) * NT]; t.x += nV[2 * e]; t.y += nV[2 * e + 1]; my[(4 * e + 0) * NT] = t;
+            t = my[(4 * e + 1) * NT]; t.x += nEx[2 * e]; t.y += nEx[2 * e + 1]; my[(4 * e + 1) * NT] = t;
+            t = my[(4 * e + 2) * NT]; t.x += nEy[2 * e]; t.y += nEy[2 * e + 1]; my[(4 * e + 2) * NT] = t;
+            t = my[(4 * e + 3) * NT]; t.x += nEz[2 * e]; t.y += nEz[2 * e + 1]; my[(4 * e + 3) * NT] = t;
+        }
+    }
+
+    // ---- in-CTA reduction through shared memory, as in pair_kernel_f32x2 ----------------------
+    double *red = reinterpret_cast<double *>(acc);   // reused after the barrier: [8][EPT*4]
+    double2 tot = make_double2(0.0, 0.0);
+    __syncwarp();
+    if (lane < 2 * EPT) {
+        const double2 *rowp = acc + lane * NT + warp * 32;
+#pragma unroll 8
+        for (int j = 0; j < 32; ++j) {
+            const double2 t = rowp[(j + lane) & 31];
+            tot.x += t.x;
+            tot.y += t.y;
+        }
+    }
+    compute_warps_sync();                            // every column has been read
+    if (lane < 2 * EPT) {                            // row 4e+comp -> values 8e+comp, 8e+4+comp
+        red[warp * EPT * 4 + 8 * (lane >> 2) + (lane & 3)] = tot.x;
+        red[warp * EPT * 4 + 8 * (lane >> 2) + 4 + (lane & 3)] = tot.y;
+    }
+    compute_warps_sync();
+    if (ws == 0 && lane < EPT * 4) {
+        double a = 0.0;
+        for (int s = 0; s < WS; ++s) a += red[(s * WP + wp) * EPT * 4 + lane];
+        const int p = (blockIdx.x * WP + wp) * EPT + lane / 4;
+        if (p < prm.P)                               // grid units -> hartree, hartree / bohr
+            prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] =
+                a * ((lane & 3) ? prm.g_scaleE : prm.g_scaleV);
+    }
+    finish_point_block<NT>(prm, WP * EPT, threadIdx.x, flag, red, [] { compute_warps_sync(); },
+                           prm.seq);
+}
+
+// ----------------------------------------------------------------------------- FP64
+// gchunk layout [ZS/2][32][2] double (16 KB).  13 DP lane operations + 1 MUFU.RSQ64H per pair
+// (+ 1/4 for the dz base step); potential only: 8.
+constexpr int GRID_STAGE_BYTES_F64 = GRID_NODES * sizeof(double);
+
+template <int EPT, bool WITH_E>
+__global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f64(const PairParams prm) {
+    constexpr int STAGE_BYTES = GRID_STAGE_BYTES_F64;
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int stages = prm.stages;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + static_cast<size_t>(stages) * STAGE_BYTES);
+    uint64_t *empty = full + 8;
+    int *flag = reinterpret_cast<int *>(empty + 8);
+    double *red = reinterpret_cast<double *>(empty + 10);  // one double per consumer thread
+    double *elec_s = red + 32 * COMPUTE_WARPS;             // [WP*EPT][3], grid units
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int WP = prm.point_warps, WS = COMPUTE_WARPS / WP;
+    int lo, hi;
+    slice_range(prm.n_chunks, prm.slices, blockIdx.y, lo, hi);
+    const int nk = hi - lo;
+
+    const bool producer = warp == COMPUTE_WARPS && lane == 0;
+    int pk = 0;
+    auto load_step = [&]() {
+        const int slot = pk % stages;
+        if (pk >= stages) mbar_wait(&empty[slot], ((pk / stages) - 1) & 1);
+        mbar_expect_tx(&full[slot], STAGE_BYTES);
+        tma_bulk_g2s(smem + static_cast<size_t>(slot) * STAGE_BYTES,
+                     prm.chunks + static_cast<size_t>(lo + pk) * STAGE_BYTES, STAGE_BYTES,
+                     &full[slot]);
+        ++pk;
+    };
+    if (producer) {
+        for (int s = 0; s < stages; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], WP);
+        }
+        fence_barrier_init();
+        while (pk < nk && pk < stages) load_step();
+    }
+    const int ppb = WP * EPT;
+    for (int i = threadIdx.x; i < ppb * 3; i += CTA_THREADS) {
+        int p = blockIdx.x * ppb + i / 3;
+        p = p < prm.P ? p : prm.P - 1;
+        const int comp = i % 3;
+        elec_s[i] = (prm.elec[static_cast<int64_t>(p) * 3 + comp] - prm.g_org[comp]) * prm.g_inv_h;
+    }
+    __syncthreads();
+
+    if (warp == COMPUTE_WARPS) {
+        if (lane == 0)
+            while (pk < nk) load_step();
+        return;
+    }
+
+    const int wp = warp % WP, ws = warp / WP;
+    const double *pe = elec_s + wp * EPT * 3;
+    double V[EPT], Ex[EPT], Ey[EPT], Ez[EPT];
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) V[e] = Ex[e] = Ey[e] = Ez[e] = 0.0;
+
+    for (int k = ws; k < nk; k += WS) {
+        const int g = lo + k;
+        const int tile = g / prm.g_segs, seg = g - tile * prm.g_segs;
+        const int row = tile * 32 + lane;
+        const int ix = row / prm.g_ny;
+        const double fx = static_cast<double>(ix), fy = static_cast<double>(row - ix * prm.g_ny);
+        const double fz = static_cast<double>(seg * GRID_ZS);
+        double dx[EPT], dy[EPT], rxy2[EPT], azb[EPT], S[EPT], SZ[EPT];
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {
+            dx[e] = pe[3 * e + 0] - fx;
+            dy[e] = pe[3 * e + 1] - fy;
+            rxy2[e] = fma(dy[e], dy[e], fma(dx[e], dx[e], 1e-200));
+            azb[e] = pe[3 * e + 2] - fz;
+            S[e] = SZ[e] = 0.0;
+        }
+        const int slot = k % stages;
+        mbar_wait(&full[slot], (k / stages) & 1);
+        const double *b =
+            reinterpret_cast<const double *>(smem + static_cast<size_t>(slot) * STAGE_BYTES) + 2 * lane;
+#pragma unroll 1
+        for (int k4 = 0; k4 < GRID_ZS / 4; ++k4) {
+            const double2 Qa = *reinterpret_cast<const double2 *>(b + (2 * k4) * 64);
+            const double2 Qb = *reinterpret_cast<const double2 *>(b + (2 * k4 + 1) * 64);
+            const double qs[4] = {Qa.x, Qa.y, Qb.x, Qb.y};
+#pragma unroll
+            for (int t = 0; t < 4; ++t) {
+#pragma unroll
+                for (int e = 0; e < EPT; ++e) {
+                    const double dz = t == 0 ? azb[e] : azb[e] - static_cast<double>(t);
+                    const double r2 = fma(dz, dz, rxy2[e]);
+                    const double y = rsqrt_refined_f64(r2);
+                    if constexpr (WITH_E) {
+                        const double p = qs[t] * y;
+                        V[e] += p;
+                        const double s = p * (y * y);
+                        S[e] += s;
+                        SZ[e] = fma(s, dz, SZ[e]);
+                    } else {
+                        V[e] = fma(qs[t], y, V[e]);
+                    }
+                }
+            }
+#pragma unroll
+            for (int e = 0; e < EPT; ++e) azb[e] -= 4.0;
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[slot]);
+        if constexpr (WITH_E) {
+#pragma unroll
+            for (int e = 0; e < EPT; ++e) {
+                Ex[e] = fma(dx[e], S[e], Ex[e]);
+                Ey[e] = fma(dy[e], S[e], Ey[e]);
+                Ez[e] += SZ[e];
+            }
+        }
+    }
+
+    // nuclei (grid units), FP64
+    if constexpr (WITH_E) {
+        nuclei_share<EPT>(prm, pe, ws, WS, lane, V, Ex, Ey, Ez);
+    } else {
+        double nEx[EPT], nEy[EPT], nEz[EPT];
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) nEx[e] = nEy[e] = nEz[e] = 0.0;
+        nuclei_share<EPT>(prm, pe, ws, WS, lane, V, nEx, nEy, nEz);
+    }
+
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+        V[e] = warp_sum(V[e]);
+        Ex[e] = warp_sum(Ex[e]);
+        Ey[e] = warp_sum(Ey[e]);
+        Ez[e] = warp_sum(Ez[e]);
+    }
+    if (lane == 0) {
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {
+            double *r = red + (warp * EPT + e) * 4;
+            r[0] = V[e]; r[1] = Ex[e]; r[2] = Ey[e]; r[3] = Ez[e];
+        }
+    }
+    compute_warps_sync();
+    if (ws == 0 && lane < EPT * 4) {
+        double a = 0.0;
+        for (int s = 0; s < WS; ++s) a += red[((s * WP + wp) * EPT) * 4 + lane];
+        const int p = (blockIdx.x * WP + wp) * EPT + lane / 4;
+        if (p < prm.P)
+            prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] =
+                a * ((lane & 3) ? prm.g_scaleE : prm.g_scaleV);
+    }
+    finish_point_block<32 * COMPUTE_WARPS>(prm, WP * EPT, threadIdx.x, flag, red,
+                                           [] { compute_warps_sync(); }, prm.seq);
+}
+
+// ----------------------------------------------------------------------------- create: detect
+// Smallest positive difference between consecutive sources per axis (a candidate spacing):
+// CTA b writes part[3b..3b+2].
+__global__ void __launch_bounds__(256) grid_spacing_kernel(const double *xyz, int64_t M, double *part) {
+    __shared__ double sh[8][3];
+    double mn[3] = {1e300, 1e300, 1e300};
+    for (int64_t j = blockIdx.x * 256ll + threadIdx.x; j + 1 < M; j += 256ll * gridDim.x)
+        for (int k = 0; k < 3; ++k) {
+            const double d = fabs(xyz[3 * (j + 1) + k] - xyz[3 * j + k]);
+            if (d > 0.0) mn[k] = fmin(mn[k], d);
+        }
+    for (int k = 0; k < 3; ++k)
+        for (int m = 16; m >= 1; m >>= 1) mn[k] = fmin(mn[k], __shfl_xor_sync(0xffffffffu, mn[k], m));
+    if ((threadIdx.x & 31) == 0)
+        for (int k = 0; k < 3; ++k) sh[threadIdx.x >> 5][k] = mn[k];
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        double v = sh[0][threadIdx.x];
+        for (int w = 1; w < 8; ++w) v = fmin(v, sh[w][threadIdx.x]);
+        part[3 * blockIdx.x + threadIdx.x] = v;
+    }
+}
+
+struct GridGeom {
+    double org[3];      // node (0,0,0)
+    double h;
+    int n[3];           // nodes per axis
+    double tol;         // accepted distance of a source from its node, per axis (bohr)
+};
+
+// Every source must sit on a node (within tol) and no node may hold two sources; the charges
+// go to the dense array dense[nx][ny][nz] (zero elsewhere).  bad[0] counts off-node sources,
+// bad[1] duplicates.
+__global__ void grid_scatter_kernel(const double *xyz, const double *q, int64_t M, GridGeom gg,
+                                    double *dense, int *count, int *bad) {
+    const int64_t j = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x;
+    if (j >= M) return;
+    int idx[3];
+    bool ok = true;
+    for (int k = 0; k < 3; ++k) {
+        const double x = xyz[3 * j + k];
+        const double fi = rint((x - gg.org[k]) / gg.h);
+        ok = ok && fi >= 0.0 && fi < static_cast<double>(gg.n[k]) &&
+             fabs(fma(fi, gg.h, gg.org[k]) - x) <= gg.tol;
+        idx[k] = static_cast<int>(fmin(fmax(fi, 0.0), static_cast<double>(gg.n[k] - 1)));
+    }
+    if (!ok) {
+        atomicAdd(bad, 1);
+        return;
+    }
+    const int64_t at = (static_cast<int64_t>(idx[0]) * gg.n[1] + idx[1]) * gg.n[2] + idx[2];
+    if (atomicAdd(count + at, 1) != 0) {
+        atomicAdd(bad + 1, 1);
+        return;
+    }
+    dense[at] = q[j];
+}
+
+// Pack the dense charges into gchunks: one thread per (padded) row.  REAL = float: each
+// charge absorbs the rounding residual of the previous one along the row (running monopole
+// residual below one rounding unit).  Cells beyond the grid are 0.
+template <typename REAL>
+__global__ void grid_pack_kernel(const double *dense, int64_t rows, int nz, int segs,
+                                 int64_t rows_padded, REAL *out) {
+    constexpr int PER = sizeof(REAL) == 4 ? 4 : 2;       // nodes per 128-bit load
+    const int64_t row = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x;
+    if (row >= rows_padded) return;
+    const int64_t tile = row / 32;
+    const int lane = static_cast<int>(row % 32);
+    double carry = 0.0;
+    for (int seg = 0; seg < segs; ++seg) {
+        REAL *o = out + (tile * segs + seg) * GRID_NODES;
+        for (int k = 0; k < GRID_ZS; ++k) {
+            const int iz = seg * GRID_ZS + k;
+            const double qd = (row < rows && iz < nz) ? dense[row * nz + iz] : 0.0;
+            REAL v;
+            if constexpr (sizeof(REAL) == 4) {
+                const double want = qd + carry;
+                v = static_cast<float>(want);
+                carry = qd != 0.0 ? want - static_cast<double>(v) : carry;
+                if (qd == 0.0) v = 0.0f;                 // empty cells stay exactly empty
+            } else {
+                v = qd;
+            }
+            o[(k / PER) * 32 * PER + lane * PER + (k % PER)] = v;
+        }
+    }
+}
+
+// number of non-empty cells of a dense charge array (qmmm_field_create_grid reports it as M)
+__global__ void grid_count_kernel(const double *dense, int64_t n, unsigned long long *out) {
+    unsigned long long c = 0;
+    for (int64_t j = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x; j < n;
+         j += static_cast<int64_t>(blockDim.x) * gridDim.x)
+        c += dense[j] != 0.0;
+    for (int m = 16; m >= 1; m >>= 1) c += __shfl_xor_sync(0xffffffffu, c, m);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(out, c);
+}
+
+// nuclei in grid units: {(x - org) / h, ..., Z}
+__global__ void grid_nuclei_kernel(const double *nuc, int64_t K, GridGeom gg, double *out) {
+    const int64_t j = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x;
+    if (j >= K) return;
+    for (int k = 0; k < 3; ++k) out[4 * j + k] = (nuc[4 * j + k] - gg.org[k]) / gg.h;
+    out[4 * j + 3] = nuc[4 * j + 3];
+}
+
+}  // namespace qmmm

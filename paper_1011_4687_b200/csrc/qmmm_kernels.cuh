@@ -52,6 +52,12 @@ struct PairParams {
     unsigned long long *host_flag;
     unsigned long long seq;
     int *done;               // point blocks finished (zero between evaluations)
+    // grid layout (qmmm_grid.cuh): chunks = gchunks of charges only, n_chunks = their number,
+    // nuc = nuclei in grid units; sums are formed in grid units and scaled at the partial store
+    double g_org[3];         // position of node (0,0,0), bohr
+    double g_inv_h;          // 1 / spacing
+    double g_scaleV, g_scaleE;   // 1/h, 1/h^2
+    int g_ny, g_segs;        // row = ix * ny + iy; z segments (gchunks) per row tile
 #ifdef QMMM_PHASE_TIMING
     long long *dbg;          // [CTAs][10] clock64 at phase boundaries + globaltimer (diagnostic build)
 #endif

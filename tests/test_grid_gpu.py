@@ -1,0 +1,335 @@
+"""GPU parity of the grid-aware compact format (include/qmmm_field.h
+"Grid-aware compact source format") against the CPU oracle, through the C ABI.
+
+The oracle knows nothing of grids: it gets the list of occupied nodes (positions and charges)
+and runs the plain Eq. 4 double loop.  Tolerances as for the list kernels.
+"""
+import numpy as np
+import pytest
+
+from paper_1011_4687_b200.workloads import make_workload, subsample_points
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-12
+TOL32 = 1e-5
+E_TOL = 1e-5          # hartree
+NO_XYZ, NO_Z = np.zeros((0, 3)), np.zeros(0)
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1011_4687_b200 import binding
+    return binding
+
+
+def run(torch, B, handle, pts, precision, want_E=True, layout=None, plan=None):
+    if layout is not None:
+        B.qmmm_field_set_layout(handle, layout)
+    B.qmmm_field_set_plan(handle, **(plan or {}))
+    d = torch.from_numpy(np.ascontiguousarray(pts)).cuda()
+    V = torch.full((len(pts),), float("nan"), dtype=torch.float64, device="cuda")
+    E = torch.full((len(pts), 3), float("nan"), dtype=torch.float64, device="cuda") if want_E else None
+    B.qmmm_field_eval(handle, d, 1, len(pts), V, E, precision)
+    torch.cuda.synchronize()
+    return V.cpu().numpy(), (E.cpu().numpy() if want_E else None)
+
+
+def rel_errors(ref, V, E):
+    eV = np.abs(V - ref.V) / np.abs(ref.V)
+    eE = None
+    if E is not None:
+        eE = np.linalg.norm(E - ref.E, axis=1) / np.linalg.norm(ref.E, axis=1)
+    return eV, eE
+
+
+def check(ref, V, E, tol):
+    eV, eE = rel_errors(ref, V, E)
+    kV = ref.absV / np.abs(ref.V)
+    assert np.all((eV <= tol) | ((kV > 1e3) & (eV / kV <= tol * 1e-3))), f"V: max rel err {eV.max():.3e}"
+    if E is not None:
+        kE = ref.absE / np.linalg.norm(ref.E, axis=1)
+        assert np.all((eE <= tol) | ((kE > 1e3) & (eE / kE <= tol * 1e-3))), f"E: max rel err {eE.max():.3e}"
+
+
+def random_grid(rng, n, h, origin, fill=0.8, hole=None, signed=False):
+    """Dense charges on an n[0] x n[1] x n[2] grid and the list of its occupied nodes."""
+    q = -rng.random(n) * 1e-2
+    if signed:
+        q *= rng.choice([-1.0, 1.0], size=n)
+    q[rng.random(n) > fill] = 0.0
+    idx = np.stack(np.meshgrid(*[np.arange(k) for k in n], indexing="ij"), axis=-1)
+    pos = np.asarray(origin) + h * idx
+    if hole is not None:                       # masked sphere (the QM region)
+        c, r = hole
+        q[np.linalg.norm(pos - np.asarray(c), axis=-1) < r] = 0.0
+    keep = q != 0.0
+    return np.ascontiguousarray(q), np.ascontiguousarray(pos[keep]), np.ascontiguousarray(q[keep])
+
+
+# ------------------------------------------------------------------------------ detection
+def test_detection_on_the_baseline_configs(torch_cuda, B):
+    w = make_workload(1)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 64)
+    try:
+        gi = B.qmmm_field_get_grid_info(h)
+        assert gi["present"] and gi["has_list"]
+        assert gi["n"] == (64, 64, 64)
+        assert abs(gi["spacing"] - 0.3) < 1e-13
+        assert np.allclose(gi["origin"], [-9.45] * 3, atol=1e-13)
+        assert gi["n_gchunks"] == 64 * 64 // 32
+    finally:
+        B.qmmm_field_destroy(h)
+    w0 = make_workload(0)                      # random positions in a shell: no grid
+    h = B.qmmm_field_create(w0.src_xyz, w0.src_q, w0.nuc_xyz, w0.nuc_Z, 8)
+    try:
+        gi = B.qmmm_field_get_grid_info(h)
+        assert not gi["present"]
+        with pytest.raises(B.QmmmError):
+            B.qmmm_field_set_layout(h, "grid")
+    finally:
+        B.qmmm_field_destroy(h)
+
+
+def test_detection_refuses_off_node_and_duplicate_sources(torch_cuda, B):
+    rng = np.random.default_rng(5)
+    _, pos, q = random_grid(rng, (20, 24, 40), 0.25, (-2.0, 1.0, 3.0), fill=1.0)
+    for kind in ("off-node", "duplicate", "anisotropic"):
+        p, c = pos.copy(), q.copy()
+        if kind == "off-node":
+            p[len(p) // 2, 1] += 1e-9
+        elif kind == "duplicate":
+            p[7] = p[8]
+        else:
+            p[:, 2] *= 1.5
+        h = B.qmmm_field_create(p, c, None, None, 4)
+        try:
+            assert not B.qmmm_field_get_grid_info(h)["present"], kind
+        finally:
+            B.qmmm_field_destroy(h)
+    h = B.qmmm_field_create(pos, q, None, None, 4)
+    try:
+        assert B.qmmm_field_get_grid_info(h)["present"]
+    finally:
+        B.qmmm_field_destroy(h)
+
+
+# ------------------------------------------------------------------------------ parity
+@pytest.mark.parametrize("precision,tol", [("fp64", TOL64), ("fp32", TOL32)])
+def test_config1_grid_layout(torch_cuda, B, oracle_mod, precision, tol):
+    """Config 1 (64^3 grid, masked sphere, 256 nuclei, 32 points) with the grid layout forced;
+    the list layout on the same handle must agree to rounding."""
+    w = make_workload(1)
+    pts = w.elec_xyz.reshape(-1, 3)
+    ref = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, pts, want_abs=True)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, len(pts))
+    try:
+        V, E = run(torch_cuda, B, h, pts, precision, layout="grid")
+        assert B.qmmm_field_get_grid_info(h)["last_layout"] == "grid"
+        check(ref, V, E, tol)
+        dE = abs(V.sum() - ref.V.sum())
+        assert dE <= (E_TOL if precision == "fp32" else 1e-9), f"energy deviation {dE:.3e} hartree"
+        Vl, El = run(torch_cuda, B, h, pts, precision, layout="list")
+        assert B.qmmm_field_get_grid_info(h)["last_layout"] == "list"
+        assert np.max(np.abs(V - Vl) / np.abs(Vl)) <= 2 * tol
+        V2, E2 = run(torch_cuda, B, h, pts, precision, layout="grid")
+        assert np.array_equal(V, V2) and np.array_equal(E, E2)          # bitwise repeatable
+        if precision == "fp64":
+            Vp, none = run(torch_cuda, B, h, pts, precision, want_E=False, layout="grid")
+            assert none is None
+            check(ref, Vp, None, tol)
+    finally:
+        B.qmmm_field_destroy(h)
+
+
+@pytest.mark.parametrize("n,h,P", [((20, 13, 70), 0.3, 33), ((5, 7, 9), 0.5, 3), ((33, 32, 64), 0.2, 100),
+                                   ((1, 40, 129), 0.25, 8), ((40, 1, 1), 0.4, 1), ((64, 3, 200), 0.1, 17)])
+@pytest.mark.parametrize("precision,tol", [("fp64", TOL64), ("fp32", TOL32)])
+def test_create_grid_ragged_shapes(torch_cuda, B, oracle_mod, n, h, P, precision, tol):
+    """qmmm_field_create_grid with row counts that are not multiples of 32, z extents that are
+    not multiples of 64, empty cells, nuclei, and point counts with ragged tails."""
+    rng = np.random.default_rng(hash((n, P)) % (2 ** 32))
+    origin = rng.normal(size=3) * 2.0
+    centre = origin + 0.5 * h * (np.array(n) - 1)
+    dense, pos, q = random_grid(rng, n, h, origin, fill=0.7, hole=(centre, 1.6))
+    K = 5
+    nuc = centre + rng.normal(size=(K, 3)) * 4.0 + 6.0
+    Z = rng.choice([1.0, 6.0, 8.0], size=K)
+    pts = centre + rng.normal(size=(P, 3)) * 0.5
+    pts = centre + (pts - centre) * np.minimum(1.0, 1.2 / np.linalg.norm(pts - centre, axis=1))[:, None]
+    ref = oracle_mod.field(pos, q, nuc, Z, pts, want_abs=True)
+    hnd = B.qmmm_field_create_grid(origin, h, n, dense, nuc, Z, P)
+    try:
+        gi = B.qmmm_field_get_grid_info(hnd)
+        assert gi["present"] and not gi["has_list"] and gi["n"] == tuple(n)
+        assert B.qmmm_field_get_info(hnd)["M"] == len(q)
+        with pytest.raises(B.QmmmError):
+            B.qmmm_field_set_layout(hnd, "list")
+        V, E = run(torch_cuda, B, hnd, pts, precision)
+        check(ref, V, E, tol)
+        # the same through a device pointer and through the per-move host path
+        hd = B.qmmm_field_create_grid(origin, h, n, torch_cuda.from_numpy(dense).cuda(),
+                                      torch_cuda.from_numpy(nuc).cuda(), torch_cuda.from_numpy(Z).cuda(), P)
+        try:
+            V2, E2 = run(torch_cuda, B, hd, pts, precision)
+            assert np.array_equal(V, V2) and np.array_equal(E, E2)
+            Vh = np.zeros(P); Eh = np.zeros((P, 3))
+            B.qmmm_field_eval_host(hd, np.ascontiguousarray(pts), 1, P, Vh, Eh, precision)
+            assert np.array_equal(V, Vh) and np.array_equal(E, Eh)
+        finally:
+            B.qmmm_field_destroy(hd)
+    finally:
+        B.qmmm_field_destroy(hnd)
+
+
+@pytest.mark.parametrize("precision,tol", [("fp64", TOL64), ("fp32", TOL32)])
+def test_grid_partition_independence_and_source_order(torch_cuda, B, oracle_mod, precision, tol):
+    """Eq. 5-6: any partition of the sum gives the result to rounding; the
+    order of the source LIST does not matter at all (the dense grid is the same: bitwise)."""
+    rng = np.random.default_rng(11)
+    n, h, origin = (32, 48, 128), 0.25, (-4.0, -6.0, -16.0)
+    centre = np.asarray(origin) + 0.5 * h * (np.array(n) - 1)
+    _, pos, q = random_grid(rng, n, h, origin, fill=0.95, hole=(centre, 2.5))
+    pts = centre + rng.normal(size=(70, 3)) * 0.7
+    ref = oracle_mod.field(pos, q, NO_XYZ, NO_Z, pts, want_abs=True)
+    h1 = B.qmmm_field_create(pos, q, None, None, len(pts))
+    perm = rng.permutation(len(q))
+    h2 = B.qmmm_field_create(np.ascontiguousarray(pos[perm]), np.ascontiguousarray(q[perm]), None, None, len(pts))
+    try:
+        assert B.qmmm_field_get_grid_info(h1)["present"] and B.qmmm_field_get_grid_info(h2)["present"]
+        base = run(torch_cuda, B, h1, pts, precision, layout="grid")
+        check(ref, *base, tol)
+        shuf = run(torch_cuda, B, h2, pts, precision, layout="grid")
+        assert np.array_equal(base[0], shuf[0]) and np.array_equal(base[1], shuf[1])
+        epts = (2, 4, 8) if precision == "fp32" else (1, 2, 4)
+        for ept in epts:
+            for pw in (1, 2, 8):
+                for slices in (1, 5, 37):
+                    V, E = run(torch_cuda, B, h1, pts, precision,
+                               plan=dict(points_per_thread=ept, point_warps=pw, slices=slices, stages=3))
+                    check(ref, V, E, tol)
+                    bound = 1e-13 if precision == "fp64" else 1e-6
+                    assert np.max(np.abs(V - base[0]) / np.abs(base[0])) <= bound
+        # batched walkers = one walker at a time, bitwise, under the same plan
+        plan = dict(points_per_thread=epts[-1], point_warps=2, slices=7, stages=4)
+        Vb, Eb = run(torch_cuda, B, h1, pts[:64], precision, plan=plan)
+        for wlk in range(4):
+            Vw, Ew = run(torch_cuda, B, h1, pts[16 * wlk:16 * wlk + 16], precision, plan=plan)
+            assert np.array_equal(Vw, Vb[16 * wlk:16 * wlk + 16]) and np.array_equal(Ew, Eb[16 * wlk:16 * wlk + 16])
+    finally:
+        B.qmmm_field_destroy(h1)
+        B.qmmm_field_destroy(h2)
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_point_on_an_empty_node_is_harmless(torch_cuda, B, oracle_mod, precision):
+    """Masked-out cells are zero charges in the grid copy; an evaluation point that coincides
+    with one must not produce 0 * inf."""
+    rng = np.random.default_rng(3)
+    n, h, origin = (16, 32, 64), 0.5, (-4.0, -8.0, -16.0)
+    centre = np.asarray(origin) + h * np.array([8, 16, 32])          # a node, inside the hole
+    dense, pos, q = random_grid(rng, n, h, origin, fill=1.0, hole=(centre, 2.0))
+    pts = np.stack([centre, centre + [h, 0, 0], centre + [0.1, 0.2, -0.3]])
+    ref = oracle_mod.field(pos, q, NO_XYZ, NO_Z, pts, want_abs=True)
+    hnd = B.qmmm_field_create_grid(origin, h, n, dense, None, None, len(pts))
+    try:
+        V, E = run(torch_cuda, B, hnd, pts, precision)
+        assert np.all(np.isfinite(V)) and np.all(np.isfinite(E))
+        eV, _ = rel_errors(ref, V, None)
+        assert eV.max() <= (TOL64 if precision == "fp64" else TOL32)
+        # E at the centre of a symmetric hole is a small difference of large terms: absolute bound
+        scale = ref.absE.max()
+        assert np.max(np.linalg.norm(E - ref.E, axis=1)) <= (1e-12 if precision == "fp64" else 1e-5) * scale
+    finally:
+        B.qmmm_field_destroy(hnd)
+
+
+def test_grid_symmetry_pins_without_the_oracle(torch_cuda, B):
+    """Closed forms the grid kernels must hit by themselves: one charged node (V = q/d,
+    E = q d/d^3) and a full symmetric cube of equal charges (E = 0 at its centre)."""
+    n, h, origin = (9, 9, 9), 0.5, (-2.0, -2.0, -2.0)
+    dense = np.zeros(n)
+    dense[6, 2, 7] = -0.75
+    node = np.asarray(origin) + h * np.array([6, 2, 7])
+    pts = np.array([[0.1, 0.2, -0.3], [1.0, -1.0, 0.25]])
+    hnd = B.qmmm_field_create_grid(origin, h, n, dense, None, None, 2)
+    try:
+        for precision, tol in (("fp64", 1e-14), ("fp32", 3e-7)):
+            V, E = run(torch_cuda, B, hnd, pts, precision)
+            d = pts - node
+            r = np.linalg.norm(d, axis=1)
+            assert np.max(np.abs(V - (-0.75 / r)) / (0.75 / r)) <= tol
+            assert np.max(np.linalg.norm(E - (-0.75 * d / r[:, None] ** 3), axis=1) * r ** 2 / 0.75) <= tol
+    finally:
+        B.qmmm_field_destroy(hnd)
+    cube = np.full(n, 0.01)
+    cube[4, 4, 4] = 0.0                        # the point sits on the (empty) centre node
+    hnd = B.qmmm_field_create_grid(origin, h, n, cube, None, None, 1)
+    try:
+        for precision, tol in (("fp64", 1e-13), ("fp32", 1e-6)):
+            V, E = run(torch_cuda, B, hnd, np.zeros((1, 3)), precision)
+            assert np.linalg.norm(E) <= tol * abs(V[0])
+    finally:
+        B.qmmm_field_destroy(hnd)
+
+
+# ------------------------------------------------------------ the bench configurations
+def test_config3_grid_fp32_full_energy(torch_cuda, B, oracle_mod):
+    """Config 3 in the launch configuration bench.py times (AUTO -> grid kernels): V and E on a
+    seeded 1 % subsample, the total energy per walker and whole batch against the oracle on
+    all 16,384 points; the list layout on the same handle for comparison."""
+    w = make_workload(3)
+    pts = w.elec_xyz.reshape(-1, 3)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, len(pts))
+    try:
+        V, E = run(torch_cuda, B, h, pts, "fp32")
+        assert B.qmmm_field_get_grid_info(h)["last_layout"] == "grid"
+        Vl, El = run(torch_cuda, B, h, pts, "fp32", layout="list")
+    finally:
+        B.qmmm_field_destroy(h)
+    idx = subsample_points(w.P, 0.01, seed=3)
+    ref = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, pts[idx], want_abs=True)
+    check(ref, V[idx], E[idx], TOL32)
+    full = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, pts, want_E=False)
+    for name, v in (("grid", V), ("list", Vl)):
+        per_walker = np.abs(v.reshape(w.W, w.N).sum(1) - full.V.reshape(w.W, w.N).sum(1))
+        batch = abs(v.sum() - full.V.sum())
+        d = v - full.V
+        print(f"config3 fp32 {name}: per-walker max |dE| = {per_walker.max():.3e}, batch |dE| = {batch:.3e} "
+              f"hartree, per point mean {d.mean():.3e} rms {d.std():.3e} max {np.abs(d).max():.3e}")
+        assert per_walker.max() <= E_TOL
+        assert batch / w.W <= E_TOL
+        assert batch <= 1e-4
+    eE = np.linalg.norm(E[idx] - ref.E, axis=1) / np.linalg.norm(ref.E, axis=1)
+    print(f"config3 fp32 grid: max rel err of |E| on the subsample {eE.max():.3e}")
+
+
+def test_config4_grid_fp64(torch_cuda, B, oracle_mod):
+    """Config 4 (16.7 M cells x 2,048 points, FP64) in bench.py's launch configuration
+    (AUTO -> grid kernels); oracle on 24 sampled points; list layout for comparison."""
+    w = make_workload(4)
+    pts = w.elec_xyz.reshape(-1, 3)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, len(pts))
+    try:
+        gi = B.qmmm_field_get_grid_info(h)
+        assert gi["present"] and gi["n"] == (256, 256, 256)
+        V, E = run(torch_cuda, B, h, pts, "fp64")
+        assert B.qmmm_field_get_grid_info(h)["last_layout"] == "grid"
+        Vp, _ = run(torch_cuda, B, h, pts, "fp64", want_E=False)
+        Vl, El = run(torch_cuda, B, h, pts, "fp64", layout="list")
+    finally:
+        B.qmmm_field_destroy(h)
+    idx = subsample_points(w.P, 24 / w.P, seed=4)
+    ref = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, pts[idx], want_abs=True)
+    check(ref, V[idx], E[idx], TOL64)
+    check(ref, Vp[idx], None, TOL64)
+    assert np.all(np.isfinite(V)) and np.all(np.isfinite(E))
+    assert np.max(np.abs(V - Vl) / np.abs(Vl)) <= 1e-12
+    assert np.max(np.linalg.norm(E - El, axis=1) / np.linalg.norm(El, axis=1)) <= 1e-11
