@@ -69,10 +69,16 @@ size_t pair_smem_bytes(bool f32, int stages, int ept, int wp) {
            static_cast<size_t>(wp) * ept * 3 * sizeof(double);
 }
 
+// FP32 grid kernel variants: (points per thread -> warps per CTA)
+#ifndef QMMM_GRID_F32_MAXEPT
+#define QMMM_GRID_F32_MAXEPT 4
+#endif
+constexpr int GRID_NW_EPT8 = 8, GRID_NW_EPT4 = 16, GRID_NW_EPT2 = 16;
+int grid_f32_warps(int ept) { return ept == 8 ? GRID_NW_EPT8 : (ept == 4 ? GRID_NW_EPT4 : GRID_NW_EPT2); }
 size_t grid_smem_bytes(bool f32, int stages, int ept, int wp) {
-    if (f32 && ept == 8) return GridF32Layout<4>::total(stages);
-    if (f32 && ept == 4) return GridF32Layout<2>::total(stages);
-    if (f32) return GridF32Layout<1>::total(stages);
+    if (f32 && ept == 8) return GridF32Layout<4, GRID_NW_EPT8>::total(stages);
+    if (f32 && ept == 4) return GridF32Layout<2, GRID_NW_EPT4>::total(stages);
+    if (f32) return GridF32Layout<1, GRID_NW_EPT2>::total(stages);
     return static_cast<size_t>(stages) * GRID_STAGE_BYTES_F64 + 18 * sizeof(uint64_t) +
            static_cast<size_t>(32) * COMPUTE_WARPS * sizeof(double) +
            static_cast<size_t>(wp) * ept * 3 * sizeof(double);
@@ -126,12 +132,12 @@ namespace {
 // SMs in whole waves; few points -> sources split across all warps and SMs.
 qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32, bool grid = false) {
     qmmm_plan pl = h->user_plan;
-    const int max_ept = f32 ? 8 : 4;
+    const int max_ept = f32 ? (grid ? QMMM_GRID_F32_MAXEPT : 8) : 4;
     if (pl.points_per_thread == 0) pl.points_per_thread = std::min(max_ept, pow2_ceil(P));
     pl.points_per_thread = std::min(pl.points_per_thread, max_ept);
     if (grid && f32) pl.points_per_thread = std::max(pl.points_per_thread, 2);   // packed pairs only
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
-    const int nw = grid ? COMPUTE_WARPS
+    const int nw = grid ? (f32 ? grid_f32_warps(pl.points_per_thread) : COMPUTE_WARPS)
                         : ((f32 && pl.points_per_thread >= 2) ? f32x2_warps(pl.points_per_thread) : COMPUTE_WARPS);
     if (pl.point_warps == 0) {
         // as many point warps as there are groups, but keep at least 4 point blocks when the
@@ -155,22 +161,21 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32, bool grid = fals
     if (pl.slices > cap) pl.slices = static_cast<int>(std::max<int64_t>(1, cap));
     if (pl.stages == 0) {
         const bool bandwidth_bound = groups <= 2;
-        if (grid)        // the source-split warp groups take the stages round-robin: one each + 1
-            pl.stages = std::min(8, std::max(f32 ? 6 : 4, nw / pl.point_warps + 1));
-        else
-            pl.stages = f32 ? (pl.points_per_thread == 1 ? 6 : 4) : (bandwidth_bound ? 6 : 3);
+        if (!grid) pl.stages = f32 ? (pl.points_per_thread == 1 ? 6 : 4) : (bandwidth_bound ? 6 : 3);
     }
+    if (grid && pl.stages == 0) pl.stages = f32 ? 6 : 4;     // one gchunk (8 / 16 KB) per stage
     return pl;
 }
 
-// AUTO layout: the grid kernels when the handle has a grid and every source-split warp group
-// of every slice gets at least a few gchunks (32 rows x 64 nodes each); else the source list.
+// AUTO layout: the grid kernels when the handle has a grid, every warp of a CTA owns its own
+// point group (no z split) and every slice gets at least a few gchunks (32 rows x 64 nodes
+// each); else the source list.
 bool auto_uses_grid(const qmmm_field *h, int64_t P, bool f32) {
     if (!h->has_grid) return false;
     if (!h->has_list) return true;
     const qmmm_plan pl = choose_plan(h, P, f32, true);
-    const int ws = COMPUTE_WARPS / pl.point_warps;
-    return h->n_g >= static_cast<int64_t>(4) * pl.slices * ws;
+    const int nw = f32 ? grid_f32_warps(pl.points_per_thread) : COMPUTE_WARPS;
+    return pl.point_warps == nw && h->n_g >= static_cast<int64_t>(4) * pl.slices;
 }
 
 template <typename REAL, int EPT, bool WITH_E = true>
@@ -228,9 +233,9 @@ cudaError_t launch_pair_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
     return cudaErrorInvalidValue;
 }
 
-template <int EP2>
+template <int EP2, int NW>
 cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
-    auto kern = grid_kernel_f32x2<EP2>;
+    auto kern = grid_kernel_f32x2<EP2, NW>;
     static thread_local size_t configured = 0;
     if (smem > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -238,7 +243,7 @@ cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaS
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    kern<<<grid, CTA_THREADS, smem, st>>>(prm);
+    kern<<<grid, 32 * NW, smem, st>>>(prm);
     return cudaGetLastError();
 }
 template <int EPT, bool WITH_E>
@@ -259,9 +264,9 @@ cudaError_t launch_grid_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
                             cudaStream_t st) {
     if (f32) {
         switch (ept) {
-            case 2: return launch_grid_f32<1>(prm, grid, smem, st);
-            case 4: return launch_grid_f32<2>(prm, grid, smem, st);
-            case 8: return launch_grid_f32<4>(prm, grid, smem, st);
+            case 2: return launch_grid_f32<1, GRID_NW_EPT2>(prm, grid, smem, st);
+            case 4: return launch_grid_f32<2, GRID_NW_EPT4>(prm, grid, smem, st);
+            case 8: return launch_grid_f32<4, GRID_NW_EPT8>(prm, grid, smem, st);
         }
     } else if (prm.E) {
         switch (ept) {
@@ -973,7 +978,7 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
             prm.g_inv_h = 1.0 / h->grid.h;
             prm.g_scaleV = 1.0 / h->grid.h;
             prm.g_scaleE = 1.0 / (h->grid.h * h->grid.h);
-            prm.g_ny = h->grid.n[1];
+            for (int k = 0; k < 3; ++k) prm.g_n[k] = h->grid.n[k];
             prm.g_segs = static_cast<int>(h->g_segs);
         } else {
             prm.chunks = f32 ? reinterpret_cast<const char *>(h->chunks32)

@@ -14,12 +14,12 @@
 //     Ez  += sum_k s_k dz_k                             1 fma per pair
 // which leaves 12 FP32 (13 FP64) lane operations per pair instead of 17 (18) for a source
 // list: dz, r^2, the 4 (5) refinement operations, p = q y, V += p,
-// y^2, s = p y^2, sum s, sum s dz.
+// y^2, s = p y^2, sum s, sum s dz.  (FP32: one of the 12, y0 / 2, runs on the integer pipe.)
 //
 // Work unit ("gchunk"): 32 rows x ZS = 64 consecutive z nodes, stored [ZS/4][32][4] (FP32) or
 // [ZS/2][32][2] (FP64) so that a lane's 128-bit shared-memory loads are conflict-free.  One
 // TMA bulk copy per gchunk and pipeline stage.  Slices (Eq. 5-6) are
-// ranges of gchunks; the source-split warp groups of a CTA take the stages round-robin.
+// ranges of gchunks; the source-split warps of a CTA take different z runs of every gchunk.
 // Masked-out cells are zero charges (they contribute exactly 0: r^2 carries a tiny positive
 // offset so that a coincident zero-charge node cannot produce 0 * inf).
 #pragma once
@@ -31,14 +31,14 @@ constexpr int GRID_ZS = 64;                         // z nodes per gchunk
 constexpr int GRID_NODES = 32 * GRID_ZS;            // cells per gchunk
 
 // ----------------------------------------------------------------------------- FP32 packed
-template <int EP2>
+template <int EP2, int NW>
 struct GridF32Layout {
     static constexpr int EPT = 2 * EP2;
-    static constexpr int NT = 32 * COMPUTE_WARPS;
+    static constexpr int NT = 32 * NW;
     static constexpr int STAGE_BYTES = GRID_NODES * sizeof(float);          // 8 KB
     static constexpr int BAR_BYTES = 18 * sizeof(uint64_t);                 // 8 full, 8 empty, flag
-    static constexpr int ELEC_BYTES = COMPUTE_WARPS * EPT * 3 * sizeof(double);
-    static constexpr int SCRATCH_BYTES = COMPUTE_WARPS * 2 * EPT * sizeof(float);
+    static constexpr int ELEC_BYTES = NW * EPT * 3 * sizeof(double);
+    static constexpr int SCRATCH_BYTES = NW * 2 * 3 * EPT * sizeof(float);     // lattice a, dd
     static constexpr int ACC_BYTES = EPT * 4 * NT * sizeof(double);
     __host__ __device__ static constexpr size_t total(int stages) {
         return static_cast<size_t>(stages) * STAGE_BYTES + BAR_BYTES + ELEC_BYTES + SCRATCH_BYTES +
@@ -46,82 +46,140 @@ struct GridF32Layout {
     }
 };
 
-// z coordinate of a point relative to the first node of a z segment, on a power-of-two
-// lattice fine enough that every dz = azb - k (k = 0..ZS-1) is EXACT in FP32: the quantum is
-// 2^-24 of the power of two above the farthest node of the segment.  dd is the residual
-// that enters as the first-order correction V(a + dd) = V(a) - Ez(a) dd at the flush.
-__device__ __forceinline__ void z_on_lattice(double zb, float &azb, float &dd) {
-    const double far = fmax(fabs(zb), fabs(zb - (GRID_ZS - 1)));
-    const int ex = ilogb(far) + 1;                             // far < 2^ex
-    const double lam = scalbn(1.0, ex - 24);
-    const double a = rint(zb * scalbn(1.0, 24 - ex)) * lam;
-    azb = static_cast<float>(a);                               // exact
-    dd = static_cast<float>(zb - a);
+// Coordinate of an evaluation point along one axis (grid units) on a power-of-two lattice
+// fine enough that every difference a - k to a node index k = 0..n-1 is EXACT in FP32: the
+// quantum is 2^-24 of the power of two above the farthest node.  dd = u - a is the residual;
+// it enters once, at the end, as the first-order correction V(a + dd) = V(a) - E(a) . dd
+// (DESIGN.md "FP32 path").  Plain FP32 rounding of the differences would be coherent over a
+// regular grid and bias V.
+__device__ __forceinline__ void on_lattice(double u, int n, float &a, float &dd) {
+    const double far = fmax(fmax(fabs(u), fabs(u - (n - 1))), 1.0);
+    const int ex = ((__double2hiint(far) >> 20) & 0x7ff) - 1022;          // far < 2^ex
+    const double lam = __hiloint2double((ex - 24 + 1023) << 20, 0);
+    const double inv = __hiloint2double((24 - ex + 1023) << 20, 0);
+    const double al = rint(u * inv) * lam;
+    a = static_cast<float>(al);                                // exact: |al| <= 2^24 quanta
+    dd = static_cast<float>(u - al);
 }
 
-// One gchunk for EP2 packed point pairs: the lane's row, ZS nodes along z.
-// 12 FP32 lane operations + 1 MUFU.RSQ per pair, + 1/4 (dz base step) + 5/16 (V tree).
+// y0 / 2 on the integer pipe (exponent - 1; y0 is a normal number): one FMA-pipe operation
+// of the Newton step moved to the idle ALU pipe.
+__device__ __forceinline__ float2 half_f32x2(float2 y) {
+    return f2(__int_as_float(__float_as_int(y.x) - 0x00800000),
+              __int_as_float(__float_as_int(y.y) - 0x00800000));
+}
+
+// A run of z nodes of the lane's row for EP2 packed point pairs, software-pipelined: while
+// the FMA pipe works on node n (Newton step, V, field sums) the MUFU.RSQ of node n + 1 is
+// already in flight (two register sets A / B in turn).  Per pair: dz (1 add: the running dz
+// steps by -1, exact on the lattice), r^2 (1 fma), 3 FMA-pipe operations + 1 integer
+// operation for the Newton step, p = q y, V += p, y^2, s = p y^2, sum s, sum s dz = 11
+// FMA-pipe lane operations + 1 MUFU.RSQ (+ 5/16 for the V tree).
 template <int EP2>
-__device__ __forceinline__ void gchunk_f32x2(const float *b, float2 (&azb)[EP2],
-                                             const float2 (&rxy2)[EP2], float2 (&v)[EP2],
-                                             float2 (&S)[EP2], float2 (&SZ)[EP2]) {
-#pragma unroll 1
-    for (int g = 0; g < GRID_ZS / 16; ++g) {
-        float2 v16[EP2];                          // middle level of the V tree: 16 nodes
+struct GridRowF32 {
+    float2 dzA[EP2], r2A[EP2], y0A[EP2], dzB[EP2], r2B[EP2], y0B[EP2];
+    float2 rxy2[EP2], S[EP2], SZ[EP2];
+
+    __device__ __forceinline__ void start(const float2 (&azb)[EP2], const float2 (&rxy2_)[EP2]) {
 #pragma unroll
-        for (int e = 0; e < EP2; ++e) v16[e] = f2(0.0f, 0.0f);
-#pragma unroll 1
-        for (int k4 = 0; k4 < 4; ++k4) {
-            const float4 Q = *reinterpret_cast<const float4 *>(b + (4 * g + k4) * 128);
-            const float qs[4] = {Q.x, Q.y, Q.z, Q.w};
-            // V is summed as a tree of short FP32 runs (4 nodes -> 16 -> gchunk): a long FP32
-            // running sum of slowly varying same-sign terms drifts
-            float2 Vc[EP2];
-#pragma unroll
-            for (int t = 0; t < 4; ++t) {
-                float2 dz[EP2], r2[EP2], y0[EP2];
-                const float2 qq = bc(qs[t]);
-#pragma unroll
-                for (int e = 0; e < EP2; ++e) {
-                    dz[e] = t == 0 ? azb[e] : __fadd2_rn(azb[e], bc(-static_cast<float>(t)));
-                    r2[e] = __ffma2_rn(dz[e], dz[e], rxy2[e]);
-                }
-#pragma unroll
-                for (int e = 0; e < EP2; ++e) {
-                    y0[e].x = rsqrt_mufu_f32(r2[e].x);
-                    y0[e].y = rsqrt_mufu_f32(r2[e].y);
-                }
-#pragma unroll
-                for (int e = 0; e < EP2; ++e) {       // one Newton step, then V and the E sums
-                    const float2 tt = __fmul2_rn(r2[e], y0[e]);
-                    const float2 err = __ffma2_rn(f2(-tt.x, -tt.y), y0[e], bc(1.0f));
-                    const float2 hh = __fmul2_rn(y0[e], bc(0.5f));
-                    const float2 y = __ffma2_rn(hh, err, y0[e]);
-                    const float2 p = __fmul2_rn(y, qq);
-                    Vc[e] = t == 0 ? p : __fadd2_rn(Vc[e], p);
-                    const float2 s = __fmul2_rn(p, __fmul2_rn(y, y));
-                    S[e] = __fadd2_rn(S[e], s);
-                    SZ[e] = __ffma2_rn(s, dz[e], SZ[e]);
-                }
-            }
-#pragma unroll
-            for (int e = 0; e < EP2; ++e) {
-                azb[e] = __fadd2_rn(azb[e], bc(-4.0f));           // exact (lattice multiples)
-                v16[e] = __fadd2_rn(v16[e], Vc[e]);
-            }
+        for (int e = 0; e < EP2; ++e) {
+            rxy2[e] = rxy2_[e];
+            S[e] = SZ[e] = f2(0.0f, 0.0f);
+            dzA[e] = azb[e];
+            r2A[e] = __ffma2_rn(dzA[e], dzA[e], rxy2[e]);
         }
 #pragma unroll
-        for (int e = 0; e < EP2; ++e) v[e] = __fadd2_rn(v[e], v16[e]);
+        for (int e = 0; e < EP2; ++e) {
+            y0A[e].x = rsqrt_mufu_f32(r2A[e].x);
+            y0A[e].y = rsqrt_mufu_f32(r2A[e].y);
+        }
     }
-}
+    // next node from the current one: dz - 1, r^2, MUFU
+    __device__ __forceinline__ void step(const float2 (&dzc)[EP2], float2 (&dzn)[EP2],
+                                         float2 (&r2n)[EP2], float2 (&y0n)[EP2]) {
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+            dzn[e] = __fadd2_rn(dzc[e], bc(-1.0f));
+            r2n[e] = __ffma2_rn(dzn[e], dzn[e], rxy2[e]);
+        }
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+            y0n[e].x = rsqrt_mufu_f32(r2n[e].x);
+            y0n[e].y = rsqrt_mufu_f32(r2n[e].y);
+        }
+    }
+    // one Newton step, then V and the field sums of the node
+    __device__ __forceinline__ void acc(const float2 (&dz)[EP2], const float2 (&r2)[EP2],
+                                        const float2 (&y0)[EP2], float q, float2 (&Vc)[EP2],
+                                        bool first) {
+        const float2 qq = bc(q);
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+            const float2 tt = __fmul2_rn(r2[e], y0[e]);
+            const float2 err = __ffma2_rn(f2(-tt.x, -tt.y), y0[e], bc(1.0f));
+            const float2 y = __ffma2_rn(half_f32x2(y0[e]), err, y0[e]);
+            const float2 p = __fmul2_rn(y, qq);
+            Vc[e] = first ? p : __fadd2_rn(Vc[e], p);
+            const float2 s = __fmul2_rn(p, __fmul2_rn(y, y));
+            S[e] = __fadd2_rn(S[e], s);
+            SZ[e] = __ffma2_rn(s, dz[e], SZ[e]);
+        }
+    }
+    // 4 nodes (one 128-bit load of charges); their V sum goes to Vc
+    __device__ __forceinline__ void four(const float *q4, float2 (&Vc)[EP2]) {
+        const float4 Q = *reinterpret_cast<const float4 *>(q4);
+        step(dzA, dzB, r2B, y0B);
+        acc(dzA, r2A, y0A, Q.x, Vc, true);
+        step(dzB, dzA, r2A, y0A);
+        acc(dzB, r2B, y0B, Q.y, Vc, false);
+        step(dzA, dzB, r2B, y0B);
+        acc(dzA, r2A, y0A, Q.z, Vc, false);
+        step(dzB, dzA, r2A, y0A);           // the last one looks one node past the run: unused
+        acc(dzB, r2B, y0B, Q.w, Vc, false);
+    }
+    // n4 * 4 nodes starting at b ([k4][32][4] floats); V is summed as a tree of short FP32
+    // runs (4 nodes -> 16 -> run): a long FP32 running sum of slowly varying same-sign terms
+    // drifts
+    __device__ __forceinline__ void run(const float *b, int n4, float2 (&v)[EP2]) {
+        if ((n4 & 3) == 0) {
+#pragma unroll 1
+            for (int g = 0; g < n4; g += 4) {
+                float2 v16[EP2], Vc[EP2];
+                four(b + g * 128, v16);
+#pragma unroll
+                for (int k4 = 1; k4 < 4; ++k4) {
+                    four(b + (g + k4) * 128, Vc);
+#pragma unroll
+                    for (int e = 0; e < EP2; ++e) v16[e] = __fadd2_rn(v16[e], Vc[e]);
+                }
+#pragma unroll
+                for (int e = 0; e < EP2; ++e) v[e] = __fadd2_rn(v[e], v16[e]);
+            }
+        } else {
+#pragma unroll 1
+            for (int k4 = 0; k4 < n4; ++k4) {
+                float2 Vc[EP2];
+                four(b + k4 * 128, Vc);
+#pragma unroll
+                for (int e = 0; e < EP2; ++e) v[e] = __fadd2_rn(v[e], Vc[e]);
+            }
+        }
+    }
+};
 
-// grid = (point_blocks, slices); EPT = 2 * EP2 points per thread; 8 consumer warps + 1 TMA
-// producer warp.  The FP64 running sums live in shared-memory columns as in
-// pair_kernel_f32x2.  prm.chunks = gchunks [n_chunks][ZS/4][32][4] float; prm.nuc = nuclei in
-// grid units; prm.elec in bohr (converted to grid units when staged).
-template <int EP2>
-__global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f32x2(const PairParams prm) {
-    using L = GridF32Layout<EP2>;
+// grid = (point_blocks, slices); EPT = 2 * EP2 points per thread; NW warps (8 x 8 points or
+// 16 x 4 points), warp 0 drives the TMA ring inline (a producer warp would cost registers).
+// A pipeline stage is one gchunk, consumed by all warps: the WP point warps own different
+// point groups, the WS source-split warps different z runs (ZS / WS nodes) of the same 32
+// rows.  Per gchunk a thread only forms dx, dy (exact FP32 differences on the point's
+// lattice) and adds the row's sums into FP32 accumulators, flushed to the FP64 columns in
+// shared memory every 4th gchunk.  prm.chunks = gchunks [n_chunks][ZS/4][32][4] float;
+// prm.nuc = nuclei in grid units; prm.elec in bohr (converted to grid units when staged).
+constexpr int GRID_FLUSH = 4;                       // gchunks per FP32 -> FP64 flush
+
+template <int EP2, int NW>
+__global__ void __launch_bounds__(32 * NW, 1) grid_kernel_f32x2(const PairParams prm) {
+    using L = GridF32Layout<EP2, NW>;
     constexpr int EPT = L::EPT, NT = L::NT, STAGE_BYTES = L::STAGE_BYTES;
 
     extern __shared__ __align__(128) unsigned char smem[];
@@ -133,113 +191,166 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f32x2(const PairPa
     ptr += L::BAR_BYTES;
     double *elec_s = reinterpret_cast<double *>(ptr);          // [WP*EPT][3], grid units
     ptr += L::ELEC_BYTES;
-    float *scratch = reinterpret_cast<float *>(ptr);           // per warp: azb[EPT], ddz[EPT]
+    float *lat_s = reinterpret_cast<float *>(ptr);             // a[WP*EPT][3], then dd[WP*EPT][3]
     ptr += L::SCRATCH_BYTES;
     double2 *acc = reinterpret_cast<double2 *>(ptr);           // [EPT*2][NT] double2
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int WP = prm.point_warps, WS = COMPUTE_WARPS / WP;
+    const int WP = prm.point_warps, WS = NW / WP;
     int lo, hi;
     slice_range(prm.n_chunks, prm.slices, blockIdx.y, lo, hi);
-    const int nk = hi - lo;
 
-    const bool producer = warp == COMPUTE_WARPS && lane == 0;
-    int pk = 0;
-    auto load_step = [&]() {
-        const int slot = pk % stages;
-        if (pk >= stages) mbar_wait(&empty[slot], ((pk / stages) - 1) & 1);
-        mbar_expect_tx(&full[slot], STAGE_BYTES);
-        tma_bulk_g2s(smem + static_cast<size_t>(slot) * STAGE_BYTES,
-                     prm.chunks + static_cast<size_t>(lo + pk) * STAGE_BYTES, STAGE_BYTES,
-                     &full[slot]);
-        ++pk;
-    };
-    if (producer) {
+    if (threadIdx.x == 0) {
         for (int s = 0; s < stages; ++s) {
             mbar_init(&full[s], 1);
-            mbar_init(&empty[s], WP);          // stage k is consumed by the WP warps of group k % WS
+            mbar_init(&empty[s], NW);
         }
         fence_barrier_init();
-        while (pk < nk && pk < stages) load_step();
+    }
+    // ---- producer cursor (warp 0 only): next gchunk to load ---------------------------------
+    int pc = lo, pslot = 0;
+    uint32_t pphase = 0;
+    bool pwrapped = false;
+    auto produce = [&]() {
+        if (pc >= hi) return;
+        if (pwrapped) mbar_wait(&empty[pslot], pphase);
+        if (lane == 0) {
+            mbar_expect_tx(&full[pslot], STAGE_BYTES);
+            tma_bulk_g2s(smem + static_cast<size_t>(pslot) * STAGE_BYTES,
+                         prm.chunks + static_cast<size_t>(pc) * STAGE_BYTES, STAGE_BYTES, &full[pslot]);
+        }
+        ++pc;
+        if (++pslot == stages) {
+            pslot = 0;
+            if (pwrapped) pphase ^= 1u;
+            pwrapped = true;
+        }
+    };
+    if (warp == 0) {
+        __syncwarp();
+        for (int i = 0; i < stages - 1; ++i) produce();
     }
     const int ppb = WP * EPT;
-    for (int i = threadIdx.x; i < ppb * 3; i += CTA_THREADS) {
+    float *dd_all = lat_s + NW * EPT * 3;
+    for (int i = threadIdx.x; i < ppb * 3; i += NT) {
         int p = blockIdx.x * ppb + i / 3;
         p = p < prm.P ? p : prm.P - 1;                          // clamp: duplicates are not written
         const int comp = i % 3;
-        elec_s[i] = (prm.elec[static_cast<int64_t>(p) * 3 + comp] - prm.g_org[comp]) * prm.g_inv_h;
+        const double u = (prm.elec[static_cast<int64_t>(p) * 3 + comp] - prm.g_org[comp]) * prm.g_inv_h;
+        elec_s[i] = u;
+        on_lattice(u, prm.g_n[comp], lat_s[i], dd_all[i]);
     }
     __syncthreads();
 
-    if (warp == COMPUTE_WARPS) {
-        if (lane == 0)
-            while (pk < nk) load_step();
-        return;
-    }
-
     const int wp = warp % WP, ws = warp / WP;
+    const int ZL = GRID_ZS / WS, z0 = ws * ZL;       // this warp's z run inside every gchunk
     double2 *my = acc + threadIdx.x;                 // this thread's column: my[i * NT]
 #pragma unroll
     for (int i = 0; i < EPT * 2; ++i) my[i * NT] = make_double2(0.0, 0.0);
     const double *pe = elec_s + wp * EPT * 3;
-    float *az_s = scratch + warp * 2 * EPT;          // azb[EPT]
-    float *dd_s = az_s + EPT;                        // ddz[EPT]
-
-    for (int k = ws; k < nk; k += WS) {
-        const int g = lo + k;
-        const int tile = g / prm.g_segs, seg = g - tile * prm.g_segs;
-        const int row = tile * 32 + lane;
-        const int ix = row / prm.g_ny;
-        const double fx = static_cast<double>(ix), fy = static_cast<double>(row - ix * prm.g_ny);
-        // z: the same for all lanes -> the first EPT lanes compute it for the warp
-        __syncwarp();
-        if (lane < EPT) {
-            float a, d;
-            z_on_lattice(pe[3 * lane + 2] - static_cast<double>(seg * GRID_ZS), a, d);
-            az_s[lane] = a;
-            dd_s[lane] = d;
-        }
-        __syncwarp();
-        float2 dx[EP2], dy[EP2], rxy2[EP2], azb[EP2], v[EP2], S[EP2], SZ[EP2];
+    // lattice coordinates of this thread's points, packed two points per register pair
+    float2 ax[EP2], ay[EP2], az[EP2];
+#pragma unroll
+    for (int e = 0; e < EP2; ++e) {
+        const float *a0 = lat_s + (wp * EPT + 2 * e) * 3;
+        ax[e] = f2(a0[0], a0[3]);
+        ay[e] = f2(a0[1], a0[4]);
+        az[e] = f2(a0[2], a0[5]);
+    }
+    // FP32 accumulators over up to GRID_FLUSH gchunks, then FP64 columns
+    float2 vv[EP2], ex[EP2], ey[EP2], ez[EP2];
+#pragma unroll
+    for (int e = 0; e < EP2; ++e) vv[e] = ex[e] = ey[e] = ez[e] = f2(0.0f, 0.0f);
+    auto flush = [&]() {
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
-            // x, y: the difference is formed in FP64 and rounded once (relative error 2^-24)
-            dx[e] = f2(static_cast<float>(pe[6 * e + 0] - fx), static_cast<float>(pe[6 * e + 3] - fx));
-            dy[e] = f2(static_cast<float>(pe[6 * e + 1] - fy), static_cast<float>(pe[6 * e + 4] - fy));
-            rxy2[e] = __ffma2_rn(dy[e], dy[e], __ffma2_rn(dx[e], dx[e], bc(1e-30f)));
-            azb[e] = *reinterpret_cast<const float2 *>(az_s + 2 * e);
-            v[e] = S[e] = SZ[e] = f2(0.0f, 0.0f);
-        }
-        const int slot = k % stages;
-        mbar_wait(&full[slot], (k / stages) & 1);
-        const float *data = reinterpret_cast<const float *>(smem + static_cast<size_t>(slot) * STAGE_BYTES);
-        gchunk_f32x2<EP2>(data + 4 * lane, azb, rxy2, v, S, SZ);
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[slot]);
-        // flush the FP32 run into the FP64 columns; Ex = dx sum(s), Ey = dy sum(s), Ez = sum(s dz)
-#pragma unroll
-        for (int e = 0; e < EP2; ++e) {
-            const float2 ddz = *reinterpret_cast<const float2 *>(dd_s + 2 * e);
-            const float2 ex = __fmul2_rn(dx[e], S[e]), ey = __fmul2_rn(dy[e], S[e]);
-            const float2 corr = __fmul2_rn(SZ[e], ddz);
             double2 t;
             t = my[(4 * e + 0) * NT];
-            t.x += static_cast<double>(v[e].x) - static_cast<double>(corr.x);
-            t.y += static_cast<double>(v[e].y) - static_cast<double>(corr.y);
+            t.x += static_cast<double>(vv[e].x);
+            t.y += static_cast<double>(vv[e].y);
             my[(4 * e + 0) * NT] = t;
             t = my[(4 * e + 1) * NT];
-            t.x += static_cast<double>(ex.x);
-            t.y += static_cast<double>(ex.y);
+            t.x += static_cast<double>(ex[e].x);
+            t.y += static_cast<double>(ex[e].y);
             my[(4 * e + 1) * NT] = t;
             t = my[(4 * e + 2) * NT];
-            t.x += static_cast<double>(ey.x);
-            t.y += static_cast<double>(ey.y);
+            t.x += static_cast<double>(ey[e].x);
+            t.y += static_cast<double>(ey[e].y);
             my[(4 * e + 2) * NT] = t;
             t = my[(4 * e + 3) * NT];
-            t.x += static_cast<double>(SZ[e].x);
-            t.y += static_cast<double>(SZ[e].y);
+            t.x += static_cast<double>(ez[e].x);
+            t.y += static_cast<double>(ez[e].y);
             my[(4 * e + 3) * NT] = t;
+            vv[e] = ex[e] = ey[e] = ez[e] = f2(0.0f, 0.0f);
         }
+    };
+
+    // (tile, seg) of gchunk g = tile * segs + seg, and the lane's row (ix, iy) of that tile
+    const int segs = prm.g_segs, ny = prm.g_n[1];
+    int tile = lo / segs, seg = lo - tile * segs;
+    int ix = (tile * 32 + lane) / ny, iy = tile * 32 + lane - ix * ny;
+
+    int slot = 0, pending = 0;
+    uint32_t phase = 0;
+    for (int g = lo; g < hi; ++g) {
+        if (warp == 0) produce();          // gchunk g + stages - 1 into the slot freed by g - 1
+        const float2 fx = bc(static_cast<float>(ix)), fy = bc(static_cast<float>(iy));
+        const float2 fz = bc(static_cast<float>(seg * GRID_ZS + z0));
+        float2 dx[EP2], dy[EP2], rxy2[EP2], azb[EP2], v[EP2];
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+            dx[e] = __fadd2_rn(ax[e], f2(-fx.x, -fx.y));          // exact (lattice)
+            dy[e] = __fadd2_rn(ay[e], f2(-fy.x, -fy.y));
+            azb[e] = __fadd2_rn(az[e], f2(-fz.x, -fz.y));
+            rxy2[e] = __ffma2_rn(dy[e], dy[e], __ffma2_rn(dx[e], dx[e], bc(1e-30f)));
+            v[e] = f2(0.0f, 0.0f);
+        }
+        GridRowF32<EP2> row;
+        row.start(azb, rxy2);
+        mbar_wait(&full[slot], phase);
+        const float *data = reinterpret_cast<const float *>(smem + static_cast<size_t>(slot) * STAGE_BYTES);
+        row.run(data + (z0 / 4) * 128 + 4 * lane, ZL / 4, v);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[slot]);
+        // Ex = dx sum(s), Ey = dy sum(s), Ez = sum(s dz)
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+            vv[e] = __fadd2_rn(vv[e], v[e]);
+            ex[e] = __ffma2_rn(dx[e], row.S[e], ex[e]);
+            ey[e] = __ffma2_rn(dy[e], row.S[e], ey[e]);
+            ez[e] = __fadd2_rn(ez[e], row.SZ[e]);
+        }
+        if (++pending == GRID_FLUSH) {
+            flush();
+            pending = 0;
+        }
+        if (++slot == stages) {
+            slot = 0;
+            phase ^= 1u;
+        }
+        if (++seg == segs) {               // next row tile
+            seg = 0;
+            ++tile;
+            iy += 32;
+            if (ny >= 32) {
+                if (iy >= ny) { iy -= ny; ++ix; }
+            } else {
+                ix = (tile * 32 + lane) / ny;
+                iy = tile * 32 + lane - ix * ny;
+            }
+        }
+    }
+    if (pending) flush();
+    // the cells were seen from the lattice point a = u - dd: V(u) = V(a) - E(a) . dd, applied to
+    // this thread's FP64 sums (before the nuclei, which are evaluated at u itself)
+#pragma unroll
+    for (int e = 0; e < EP2; ++e) {
+        const float *d0 = dd_all + (wp * EPT + 2 * e) * 3;
+        double2 t = my[(4 * e + 0) * NT];
+        const double2 tx = my[(4 * e + 1) * NT], ty = my[(4 * e + 2) * NT], tz = my[(4 * e + 3) * NT];
+        t.x -= tx.x * static_cast<double>(d0[0]) + ty.x * static_cast<double>(d0[1]) + tz.x * static_cast<double>(d0[2]);
+        t.y -= tx.y * static_cast<double>(d0[3]) + ty.y * static_cast<double>(d0[4]) + tz.y * static_cast<double>(d0[5]);
+        my[(4 * e + 0) * NT] = t;
     }
 
     // nuclear term of this CTA's share, FP64, grid units, into the same columns
@@ -259,7 +370,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f32x2(const PairPa
     }
 
     // ---- in-CTA reduction through shared memory, as in pair_kernel_f32x2 ----------------------
-    double *red = reinterpret_cast<double *>(acc);   // reused after the barrier: [8][EPT*4]
+    double *red = reinterpret_cast<double *>(acc);   // reused after the barrier: [NW][EPT*4]
     double2 tot = make_double2(0.0, 0.0);
     __syncwarp();
     if (lane < 2 * EPT) {
@@ -271,12 +382,12 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f32x2(const PairPa
             tot.y += t.y;
         }
     }
-    compute_warps_sync();                            // every column has been read
+    __syncthreads();                                 // every column has been read
     if (lane < 2 * EPT) {                            // row 4e+comp -> values 8e+comp, 8e+4+comp
         red[warp * EPT * 4 + 8 * (lane >> 2) + (lane & 3)] = tot.x;
         red[warp * EPT * 4 + 8 * (lane >> 2) + 4 + (lane & 3)] = tot.y;
     }
-    compute_warps_sync();
+    __syncthreads();
     if (ws == 0 && lane < EPT * 4) {
         double a = 0.0;
         for (int s = 0; s < WS; ++s) a += red[(s * WP + wp) * EPT * 4 + lane];
@@ -285,8 +396,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f32x2(const PairPa
             prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] =
                 a * ((lane & 3) ? prm.g_scaleE : prm.g_scaleV);
     }
-    finish_point_block<NT>(prm, WP * EPT, threadIdx.x, flag, red, [] { compute_warps_sync(); },
-                           prm.seq);
+    finish_point_block<NT>(prm, WP * EPT, threadIdx.x, flag, red, [] { __syncthreads(); }, prm.seq);
 }
 
 // ----------------------------------------------------------------------------- FP64
@@ -325,7 +435,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f64(const PairPara
     if (producer) {
         for (int s = 0; s < stages; ++s) {
             mbar_init(&full[s], 1);
-            mbar_init(&empty[s], WP);
+            mbar_init(&empty[s], COMPUTE_WARPS);
         }
         fence_barrier_init();
         while (pk < nk && pk < stages) load_step();
@@ -351,13 +461,14 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f64(const PairPara
 #pragma unroll
     for (int e = 0; e < EPT; ++e) V[e] = Ex[e] = Ey[e] = Ez[e] = 0.0;
 
-    for (int k = ws; k < nk; k += WS) {
+    const int ZL = GRID_ZS / WS, z0 = ws * ZL;       // this warp's z run inside every gchunk
+    for (int k = 0; k < nk; ++k) {
         const int g = lo + k;
         const int tile = g / prm.g_segs, seg = g - tile * prm.g_segs;
         const int row = tile * 32 + lane;
-        const int ix = row / prm.g_ny;
-        const double fx = static_cast<double>(ix), fy = static_cast<double>(row - ix * prm.g_ny);
-        const double fz = static_cast<double>(seg * GRID_ZS);
+        const int ix = row / prm.g_n[1];
+        const double fx = static_cast<double>(ix), fy = static_cast<double>(row - ix * prm.g_n[1]);
+        const double fz = static_cast<double>(seg * GRID_ZS + z0);
         double dx[EPT], dy[EPT], rxy2[EPT], azb[EPT], S[EPT], SZ[EPT];
 #pragma unroll
         for (int e = 0; e < EPT; ++e) {
@@ -369,10 +480,10 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f64(const PairPara
         }
         const int slot = k % stages;
         mbar_wait(&full[slot], (k / stages) & 1);
-        const double *b =
-            reinterpret_cast<const double *>(smem + static_cast<size_t>(slot) * STAGE_BYTES) + 2 * lane;
+        const double *b = reinterpret_cast<const double *>(smem + static_cast<size_t>(slot) * STAGE_BYTES) +
+                          (z0 / 2) * 64 + 2 * lane;
 #pragma unroll 1
-        for (int k4 = 0; k4 < GRID_ZS / 4; ++k4) {
+        for (int k4 = 0; k4 < ZL / 4; ++k4) {
             const double2 Qa = *reinterpret_cast<const double2 *>(b + (2 * k4) * 64);
             const double2 Qb = *reinterpret_cast<const double2 *>(b + (2 * k4 + 1) * 64);
             const double qs[4] = {Qa.x, Qa.y, Qb.x, Qb.y};

@@ -57,7 +57,7 @@ struct PairParams {
     double g_org[3];         // position of node (0,0,0), bohr
     double g_inv_h;          // 1 / spacing
     double g_scaleV, g_scaleE;   // 1/h, 1/h^2
-    int g_ny, g_segs;        // row = ix * ny + iy; z segments (gchunks) per row tile
+    int g_n[3], g_segs;      // nodes per axis (row = ix * ny + iy); z segments (gchunks) per row tile
 #ifdef QMMM_PHASE_TIMING
     long long *dbg;          // [CTAs][10] clock64 at phase boundaries + globaltimer (diagnostic build)
 #endif
