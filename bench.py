@@ -36,7 +36,14 @@ from paper_1011_4687_b200.workloads import CONFIG_SPECS, make_workload  # noqa: 
 
 METRIC = "pair-interactions/s"
 UNIT = "Gpair/s"
-SLOTS = {"fp32": 17, "fp64": 18}      # algorithmic FMA-pipe slots per pair
+# Algorithmic FMA-pipe lane operations per pair.  Source list: SURVEY.md
+# 8(a).  Grid layout: dx, dy and dx^2 + dy^2 are constants of a z row, which leaves dz, r^2, the
+# refinement, p, V, y^2, s, sum s, sum s dz = 12 (FP32; the y0/2 of the Newton step is an exact
+# exponent decrement on the integer pipe, so 11 need the FMA pipe) or 13 (FP64).
+SLOTS = {("list", "fp32"): 17, ("list", "fp64"): 18, ("grid", "fp32"): 11, ("grid", "fp64"): 13}
+SLOTS_V_ONLY = {"list": 13, "grid": 8}     # FP64 potential only (E = NULL)
+KERNEL = {("list", "fp32"): "pair_kernel_f32x2", ("list", "fp64"): "pair_kernel<double>",
+          ("grid", "fp32"): "grid_kernel_f32x2", ("grid", "fp64"): "grid_kernel_f64"}
 DTYPE = {"fp32": "f32 (f64 accumulation)", "fp64": "f64"}
 WORKLOAD_NAME = {i: f"configs[{i}] {s['name']}" for i, s in CONFIG_SPECS.items()}
 
@@ -48,6 +55,10 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (0-4)")
     ap.add_argument("--precision", default=None, choices=["fp32", "fp64"])
+    ap.add_argument("--layout", default="auto", choices=["auto", "list", "grid"],
+                    help="source copy the kernels read: list of positions, or the grid-aware "
+                         "compact format (auto: grid when the cells are grid nodes and the "
+                         "batch has many points)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-sweep", action="store_true",
                     help="skip the per-config table (all five configs) at N=1")
@@ -225,19 +236,32 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
         try:
             pts = torch.from_numpy(w.elec_xyz.reshape(-1, 3)).cuda()
             batches = [pts[i:i + 1].contiguous() for i in range(8)] if w.sequential else [pts]
-            for prec in w.precisions:
+            has_grid = B.qmmm_field_get_grid_info(h)["present"]
+            # the automatic layout, then the other one for comparison where a grid copy exists
+            runs = [(prec, "auto") for prec in w.precisions]
+            if has_grid and not w.sequential:
+                runs += [(prec, "other") for prec in w.precisions]
+            for prec, which in runs:
                 reps = 5 if idx >= 3 else 30
+                B.qmmm_field_set_layout(h, "auto")
                 B.qmmm_field_set_timing(h, True)
+                if which == "other":
+                    used = [r["layout"] for r in out if r["config"] == idx and r["precision"] == prec][0]
+                    B.qmmm_field_set_layout(h, "list" if used == "grid" else "grid")
                 step_ms, pair_ms, _ = time_steps(torch, B, h, batches, W, N, prec, reps, 3, flush, stream)
+                layout = B.qmmm_field_get_grid_info(h)["last_layout"]
                 pairs = P * (w.M + w.K)
                 peak = peaks["ffma_lane_ops_per_s" if prec == "fp32" else "dfma_lane_ops_per_s"]
-                row = {"config": idx, "name": w.name, "precision": prec, "points": P, "M": w.M,
+                row = {"config": idx, "name": w.name, "precision": prec, "layout": layout,
+                       "layout_choice": "auto" if which == "auto" else "forced",
+                       "points": P, "M": w.M,
                        "K": w.K, "pairs_per_eval": pairs,
                        "ms_per_eval_median": float(np.median(step_ms)),
                        "ms_per_eval_min": float(np.min(step_ms)),
                        "pair_kernel_ms_median": float(np.median(pair_ms)),
                        "gpairs_per_s": pairs / np.median(step_ms) / 1e6,
-                       "fma_pipe_frac": pairs * SLOTS[prec] / (np.median(step_ms) * 1e-3) / peak,
+                       "slots_per_pair": SLOTS[(layout, prec)],
+                       "fma_pipe_frac": pairs * SLOTS[(layout, prec)] / (np.median(step_ms) * 1e-3) / peak,
                        "plan": B.qmmm_field_get_info(h)["last_plan"]}
                 if w.sequential:
                     # (i) 1,000 back-to-back evaluations, positions resident on the device
@@ -265,18 +289,21 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                     row["source_GBps_back_to_back"] = bytes_eval / (row["us_per_eval_1000_back_to_back"] * 1e-6) / 1e9
                 out.append(row)
                 if prec == "fp64" and not w.sequential and idx in (1, 4):
-                    # potential only (E = NULL): the paper's own computation, Eq. 4; 13 DP slots
+                    # potential only (E = NULL): the paper's own computation, Eq. 4; 13 (list) or
+                    # 8 (grid) DP slots
                     B.qmmm_field_set_timing(h, True)
                     step_ms, pair_ms, _ = time_steps(torch, B, h, batches, W, N, prec, reps, 3, flush,
                                                      stream, want_E=False)
+                    layout = B.qmmm_field_get_grid_info(h)["last_layout"]
                     out.append({"config": idx, "name": w.name, "precision": "fp64 potential-only",
+                                "layout": layout, "layout_choice": "auto" if which == "auto" else "forced",
                                 "points": P, "M": w.M, "K": w.K, "pairs_per_eval": pairs,
                                 "ms_per_eval_median": float(np.median(step_ms)),
                                 "ms_per_eval_min": float(np.min(step_ms)),
                                 "pair_kernel_ms_median": float(np.median(pair_ms)),
                                 "gpairs_per_s": pairs / np.median(step_ms) / 1e6,
-                                "fma_pipe_frac": pairs * 13 / (np.median(step_ms) * 1e-3) / peak,
-                                "slots_per_pair": 13,
+                                "fma_pipe_frac": pairs * SLOTS_V_ONLY[layout] / (np.median(step_ms) * 1e-3) / peak,
+                                "slots_per_pair": SLOTS_V_ONLY[layout],
                                 "plan": B.qmmm_field_get_info(h)["last_plan"]})
         finally:
             B.qmmm_field_destroy(h)
@@ -315,6 +342,7 @@ def run_ours(args):
 
     # the environment is replicated on every GPU; each rank evaluates its own walkers
     h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, P)
+    B.qmmm_field_set_layout(h, args.layout)
     B.qmmm_field_set_timing(h, True)
     n_batches = 4
     host_batches = [draw_points(args.config, W, N, seed=1 + 97 * rank + b).reshape(-1, 3)
@@ -339,6 +367,7 @@ def run_ours(args):
     pairs_step_rank = P * (w.M + w.K)
     value = world * pairs_step_rank * args.steps / (total_ms * 1e-3) / 1e9
     info = B.qmmm_field_get_info(h)
+    layout = B.qmmm_field_get_grid_info(h)["last_layout"]
 
     # ---- end to end: host buffers through the C ABI -----------------------------------
     B.qmmm_field_set_timing(h, False)
@@ -361,7 +390,8 @@ def run_ours(args):
         peak_key = "ffma_lane_ops_per_s" if prec == "fp32" else "dfma_lane_ops_per_s"
         peak_lane = 0.5 * (peaks0[peak_key] + peaks1[peak_key])
         pair_s = float(np.mean(pair_ms)) * 1e-3
-        achieved = P * w.M * SLOTS[prec] * 2 / pair_s / 1e12
+        slots = SLOTS[(layout, prec)]
+        achieved = P * w.M * slots * 2 / pair_s / 1e12
         peak_tf = 2 * peak_lane / 1e12
         # DRAM bytes per pair-kernel launch from the committed ncu capture (profiles/), if any
         traffic = None
@@ -369,7 +399,7 @@ def run_ours(args):
         if os.path.exists(tpath):
             for ln in open(tpath):
                 f = ln.strip().split(",")
-                if len(f) >= 2 and f[0] == f"config{args.config}_{prec}":
+                if len(f) >= 2 and f[0] == f"config{args.config}_{prec}_{layout}":
                     traffic = float(f[1])
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
@@ -380,6 +410,7 @@ def run_ours(args):
                        "M_nominal": w.M_nominal, "K": w.K, "W": W, "N": N,
                        "pairs_per_step_per_gpu": pairs_step_rank,
                        "parallelism": f"walkers sharded x{world}, sources replicated, no collective",
+                       "layout": layout,
                        "l2": "flushed between timed steps (256 MB write)", "plan": info["last_plan"],
                        "point_blocks": info["last_point_blocks"]},
             "clocks": clocks,
@@ -388,8 +419,8 @@ def run_ours(args):
             "gpu_launches": info["last_launches"] * args.steps,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
                          "frac": achieved / peak_tf, "traffic": traffic,
-                         "kernel": "pair_kernel", "kernel_ms": pair_s * 1e3,
-                         "slots_per_pair": SLOTS[prec],
+                         "kernel": KERNEL[(layout, prec)], "kernel_ms": pair_s * 1e3,
+                         "slots_per_pair": slots,
                          "definition": "pairs x slots x 2 / pair-kernel time vs 2 x FMA lane rate of "
                                        "the same-run microbenchmark (qmmm_probe_peak)",
                          "peak_source": "measured, same process (mean of before/after)",

@@ -73,14 +73,23 @@ size_t pair_smem_bytes(bool f32, int stages, int ept, int wp) {
 #ifndef QMMM_GRID_F32_MAXEPT
 #define QMMM_GRID_F32_MAXEPT 4
 #endif
-constexpr int GRID_NW_EPT8 = 8, GRID_NW_EPT4 = 16, GRID_NW_EPT2 = 16;
+#ifndef QMMM_GRID_NW_EPT4
+#define QMMM_GRID_NW_EPT4 8
+#endif
+constexpr int GRID_NW_EPT8 = 8, GRID_NW_EPT4 = QMMM_GRID_NW_EPT4, GRID_NW_EPT2 = 16;
+// FP64 grid kernel variants: 8 warps x 4 points, 16 warps x 2 (or 1) points
+#ifndef QMMM_GRID_F64_MAXEPT
+#define QMMM_GRID_F64_MAXEPT 4
+#endif
+constexpr int GRID64_NW_EPT4 = 8, GRID64_NW_EPT2 = 16, GRID64_NW_EPT1 = 16;
+int grid_f64_warps(int ept) { return ept == 4 ? GRID64_NW_EPT4 : (ept == 2 ? GRID64_NW_EPT2 : GRID64_NW_EPT1); }
 int grid_f32_warps(int ept) { return ept == 8 ? GRID_NW_EPT8 : (ept == 4 ? GRID_NW_EPT4 : GRID_NW_EPT2); }
 size_t grid_smem_bytes(bool f32, int stages, int ept, int wp) {
     if (f32 && ept == 8) return GridF32Layout<4, GRID_NW_EPT8>::total(stages);
     if (f32 && ept == 4) return GridF32Layout<2, GRID_NW_EPT4>::total(stages);
     if (f32) return GridF32Layout<1, GRID_NW_EPT2>::total(stages);
     return static_cast<size_t>(stages) * GRID_STAGE_BYTES_F64 + 18 * sizeof(uint64_t) +
-           static_cast<size_t>(32) * COMPUTE_WARPS * sizeof(double) +
+           static_cast<size_t>(32) * grid_f64_warps(ept) * sizeof(double) +
            static_cast<size_t>(wp) * ept * 3 * sizeof(double);
 }
 
@@ -132,12 +141,14 @@ namespace {
 // SMs in whole waves; few points -> sources split across all warps and SMs.
 qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32, bool grid = false) {
     qmmm_plan pl = h->user_plan;
-    const int max_ept = f32 ? (grid ? QMMM_GRID_F32_MAXEPT : 8) : 4;
-    if (pl.points_per_thread == 0) pl.points_per_thread = std::min(max_ept, pow2_ceil(P));
+    const int max_ept = f32 ? 8 : 4;
+    // automatic choice: FP32 grid kernel 16 warps x 4 points (measured faster than 8 x 8)
+    const int auto_ept = grid ? (f32 ? QMMM_GRID_F32_MAXEPT : QMMM_GRID_F64_MAXEPT) : max_ept;
+    if (pl.points_per_thread == 0) pl.points_per_thread = std::min(auto_ept, pow2_ceil(P));
     pl.points_per_thread = std::min(pl.points_per_thread, max_ept);
     if (grid && f32) pl.points_per_thread = std::max(pl.points_per_thread, 2);   // packed pairs only
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
-    const int nw = grid ? (f32 ? grid_f32_warps(pl.points_per_thread) : COMPUTE_WARPS)
+    const int nw = grid ? (f32 ? grid_f32_warps(pl.points_per_thread) : grid_f64_warps(pl.points_per_thread))
                         : ((f32 && pl.points_per_thread >= 2) ? f32x2_warps(pl.points_per_thread) : COMPUTE_WARPS);
     if (pl.point_warps == 0) {
         // as many point warps as there are groups, but keep at least 4 point blocks when the
@@ -163,19 +174,20 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32, bool grid = fals
         const bool bandwidth_bound = groups <= 2;
         if (!grid) pl.stages = f32 ? (pl.points_per_thread == 1 ? 6 : 4) : (bandwidth_bound ? 6 : 3);
     }
-    if (grid && pl.stages == 0) pl.stages = f32 ? 6 : 4;     // one gchunk (8 / 16 KB) per stage
+    if (grid && pl.stages == 0) pl.stages = 4;             // one gchunk (8 / 16 KB) per stage
     return pl;
 }
 
-// AUTO layout: the grid kernels when the handle has a grid, every warp of a CTA owns its own
-// point group (no z split) and every slice gets at least a few gchunks (32 rows x 64 nodes
-// each); else the source list.
+// AUTO layout: the grid kernels when the handle has a grid, the source-split warps of a CTA
+// keep z runs of at least 16 nodes (at most 4 of them share a gchunk) and every slice gets at
+// least two gchunks (32 rows x 64 nodes each); else the source list, whose kernels split the
+// source range more finely (single points, a handful of points).
 bool auto_uses_grid(const qmmm_field *h, int64_t P, bool f32) {
     if (!h->has_grid) return false;
     if (!h->has_list) return true;
     const qmmm_plan pl = choose_plan(h, P, f32, true);
-    const int nw = f32 ? grid_f32_warps(pl.points_per_thread) : COMPUTE_WARPS;
-    return pl.point_warps == nw && h->n_g >= static_cast<int64_t>(4) * pl.slices;
+    const int nw = f32 ? grid_f32_warps(pl.points_per_thread) : grid_f64_warps(pl.points_per_thread);
+    return nw / pl.point_warps <= 4 && h->n_g >= static_cast<int64_t>(2) * pl.slices;
 }
 
 template <typename REAL, int EPT, bool WITH_E = true>
@@ -246,9 +258,9 @@ cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaS
     kern<<<grid, 32 * NW, smem, st>>>(prm);
     return cudaGetLastError();
 }
-template <int EPT, bool WITH_E>
+template <int EPT, bool WITH_E, int NW>
 cudaError_t launch_grid_f64(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
-    auto kern = grid_kernel_f64<EPT, WITH_E>;
+    auto kern = grid_kernel_f64<EPT, WITH_E, NW>;
     static thread_local size_t configured = 0;
     if (smem > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -256,7 +268,7 @@ cudaError_t launch_grid_f64(const PairParams &prm, dim3 grid, size_t smem, cudaS
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    kern<<<grid, CTA_THREADS, smem, st>>>(prm);
+    kern<<<grid, 32 * (NW + 1), smem, st>>>(prm);
     return cudaGetLastError();
 }
 // Grid layout: FP32-acc64 packed kernel for 2, 4, 8 points per thread; FP64 for 1, 2, 4.
@@ -270,15 +282,15 @@ cudaError_t launch_grid_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
         }
     } else if (prm.E) {
         switch (ept) {
-            case 1: return launch_grid_f64<1, true>(prm, grid, smem, st);
-            case 2: return launch_grid_f64<2, true>(prm, grid, smem, st);
-            case 4: return launch_grid_f64<4, true>(prm, grid, smem, st);
+            case 1: return launch_grid_f64<1, true, GRID64_NW_EPT1>(prm, grid, smem, st);
+            case 2: return launch_grid_f64<2, true, GRID64_NW_EPT2>(prm, grid, smem, st);
+            case 4: return launch_grid_f64<4, true, GRID64_NW_EPT4>(prm, grid, smem, st);
         }
     } else {
         switch (ept) {
-            case 1: return launch_grid_f64<1, false>(prm, grid, smem, st);
-            case 2: return launch_grid_f64<2, false>(prm, grid, smem, st);
-            case 4: return launch_grid_f64<4, false>(prm, grid, smem, st);
+            case 1: return launch_grid_f64<1, false, GRID64_NW_EPT1>(prm, grid, smem, st);
+            case 2: return launch_grid_f64<2, false, GRID64_NW_EPT2>(prm, grid, smem, st);
+            case 4: return launch_grid_f64<4, false, GRID64_NW_EPT4>(prm, grid, smem, st);
         }
     }
     return cudaErrorInvalidValue;

@@ -178,7 +178,7 @@ struct GridRowF32 {
 constexpr int GRID_FLUSH = 4;                       // gchunks per FP32 -> FP64 flush
 
 template <int EP2, int NW>
-__global__ void __launch_bounds__(32 * NW, 1) grid_kernel_f32x2(const PairParams prm) {
+__global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) grid_kernel_f32x2(const PairParams prm) {
     using L = GridF32Layout<EP2, NW>;
     constexpr int EPT = L::EPT, NT = L::NT, STAGE_BYTES = L::STAGE_BYTES;
 
@@ -404,8 +404,14 @@ __global__ void __launch_bounds__(32 * NW, 1) grid_kernel_f32x2(const PairParams
 // (+ 1/4 for the dz base step); potential only: 8.
 constexpr int GRID_STAGE_BYTES_F64 = GRID_NODES * sizeof(double);
 
-template <int EPT, bool WITH_E>
-__global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f64(const PairParams prm) {
+template <int N>
+__device__ __forceinline__ void consumer_sync() {     // named barrier 1: the N consumer warps only
+    asm volatile("bar.sync 1, %0;" ::"n"(32 * N) : "memory");
+}
+
+// NW consumer warps (8 x 4 points or 16 x 2 points) + 1 TMA producer warp.
+template <int EPT, bool WITH_E, int NW>
+__global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairParams prm) {
     constexpr int STAGE_BYTES = GRID_STAGE_BYTES_F64;
     extern __shared__ __align__(128) unsigned char smem[];
     const int stages = prm.stages;
@@ -413,15 +419,15 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f64(const PairPara
     uint64_t *empty = full + 8;
     int *flag = reinterpret_cast<int *>(empty + 8);
     double *red = reinterpret_cast<double *>(empty + 10);  // one double per consumer thread
-    double *elec_s = red + 32 * COMPUTE_WARPS;             // [WP*EPT][3], grid units
+    double *elec_s = red + 32 * NW;             // [WP*EPT][3], grid units
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int WP = prm.point_warps, WS = COMPUTE_WARPS / WP;
+    const int WP = prm.point_warps, WS = NW / WP;
     int lo, hi;
     slice_range(prm.n_chunks, prm.slices, blockIdx.y, lo, hi);
     const int nk = hi - lo;
 
-    const bool producer = warp == COMPUTE_WARPS && lane == 0;
+    const bool producer = warp == NW && lane == 0;
     int pk = 0;
     auto load_step = [&]() {
         const int slot = pk % stages;
@@ -435,13 +441,13 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f64(const PairPara
     if (producer) {
         for (int s = 0; s < stages; ++s) {
             mbar_init(&full[s], 1);
-            mbar_init(&empty[s], COMPUTE_WARPS);
+            mbar_init(&empty[s], NW);
         }
         fence_barrier_init();
         while (pk < nk && pk < stages) load_step();
     }
     const int ppb = WP * EPT;
-    for (int i = threadIdx.x; i < ppb * 3; i += CTA_THREADS) {
+    for (int i = threadIdx.x; i < ppb * 3; i += 32 * (NW + 1)) {
         int p = blockIdx.x * ppb + i / 3;
         p = p < prm.P ? p : prm.P - 1;
         const int comp = i % 3;
@@ -449,7 +455,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f64(const PairPara
     }
     __syncthreads();
 
-    if (warp == COMPUTE_WARPS) {
+    if (warp == NW) {
         if (lane == 0)
             while (pk < nk) load_step();
         return;
@@ -544,7 +550,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f64(const PairPara
             r[0] = V[e]; r[1] = Ex[e]; r[2] = Ey[e]; r[3] = Ez[e];
         }
     }
-    compute_warps_sync();
+    consumer_sync<NW>();
     if (ws == 0 && lane < EPT * 4) {
         double a = 0.0;
         for (int s = 0; s < WS; ++s) a += red[((s * WP + wp) * EPT) * 4 + lane];
@@ -553,8 +559,8 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) grid_kernel_f64(const PairPara
             prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] =
                 a * ((lane & 3) ? prm.g_scaleE : prm.g_scaleV);
     }
-    finish_point_block<32 * COMPUTE_WARPS>(prm, WP * EPT, threadIdx.x, flag, red,
-                                           [] { compute_warps_sync(); }, prm.seq);
+    finish_point_block<32 * NW>(prm, WP * EPT, threadIdx.x, flag, red, [] { consumer_sync<NW>(); },
+                                prm.seq);
 }
 
 // ----------------------------------------------------------------------------- create: detect

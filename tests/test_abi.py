@@ -62,3 +62,29 @@ def test_argument_errors_without_gpu(lib_path):
     assert lib.qmmm_field_create(None, None, 0, None, None, 0, 8, None) == 1
     assert lib.qmmm_field_eval(None, None, 1, 1, None, None, 0, None) == 1
     assert lib.qmmm_field_destroy(None) == 0
+
+
+def test_grid_argument_errors_without_gpu(lib_path):
+    """qmmm_field_create_grid / set_layout validate their arguments before any CUDA call."""
+    from paper_1011_4687_b200 import binding
+    lib = binding._lib
+    out = ctypes.c_void_p()
+    org = (ctypes.c_double * 3)(0.0, 0.0, 0.0)
+    n = (ctypes.c_int64 * 3)(4, 4, 4)
+    q = (ctypes.c_double * 64)()
+    qp = ctypes.cast(q, ctypes.c_void_p)
+    assert lib.qmmm_field_create_grid(None, 0.3, n, qp, None, None, 0, 8, ctypes.byref(out)) == 1
+    assert lib.qmmm_field_create_grid(org, 0.0, n, qp, None, None, 0, 8, ctypes.byref(out)) == 1
+    assert b"spacing" in lib.qmmm_last_error()
+    assert lib.qmmm_field_create_grid(org, float("nan"), n, qp, None, None, 0, 8, ctypes.byref(out)) == 1
+    bad = (ctypes.c_int64 * 3)(4, 0, 4)
+    assert lib.qmmm_field_create_grid(org, 0.3, bad, qp, None, None, 0, 8, ctypes.byref(out)) == 1
+    huge = (ctypes.c_int64 * 3)(65536, 65536, 2)
+    assert lib.qmmm_field_create_grid(org, 0.3, huge, qp, None, None, 0, 8, ctypes.byref(out)) == 1
+    assert lib.qmmm_field_create_grid(org, 0.3, n, None, None, None, 0, 8, ctypes.byref(out)) == 1
+    assert lib.qmmm_field_create_grid(org, 0.3, n, qp, None, None, 2, 8, ctypes.byref(out)) == 1   # K > 0, NULL nuclei
+    assert lib.qmmm_field_create_grid(org, 0.3, n, qp, None, None, 0, 0, ctypes.byref(out)) == 1   # max_points < 1
+    assert lib.qmmm_field_create_grid(org, 0.3, n, qp, None, None, 0, 8, None) == 1
+    assert out.value is None
+    assert lib.qmmm_field_set_layout(None, 0) == 1
+    assert lib.qmmm_field_get_grid_info(None, None) == 1
