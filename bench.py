@@ -36,11 +36,13 @@ from paper_1011_4687_b200.workloads import CONFIG_SPECS, make_workload  # noqa: 
 
 METRIC = "pair-interactions/s"
 UNIT = "Gpair/s"
-# Algorithmic FMA-pipe lane operations per pair.  Source list: SURVEY.md
-# 8(a).  Grid layout: dx, dy and dx^2 + dy^2 are constants of a z row, which leaves dz, r^2, the
-# refinement, p, V, y^2, s, sum s, sum s dz = 12 (FP32; the y0/2 of the Newton step is an exact
-# exponent decrement on the integer pipe, so 11 need the FMA pipe) or 13 (FP64).
-SLOTS = {("list", "fp32"): 17, ("list", "fp64"): 18, ("grid", "fp32"): 11, ("grid", "fp64"): 13}
+# Algorithmic FMA-pipe lane operations per pair (DESIGN.md sections 5, 5b).  Source list, FP64:
+# SURVEY.md 8(a), 18.  FP32: the Newton step is applied to the sum (V = (3 sum a - sum c r^2) / 2,
+# one fma per pair), which leaves 3 sub, 3 for r^2, a, V0, y0^2, c, T, 3 fma for E = 14 (the
+# per-pair step of SURVEY.md 8(a) costs 17).  Grid layout: dx, dy and dx^2 + dy^2 are constants
+# of a z row: dz, r^2, a, V0, y0^2, c, sum c, sum c dz, T = 9 (FP32) or, with the per-pair cubic
+# refinement, 13 (FP64).
+SLOTS = {("list", "fp32"): 14, ("list", "fp64"): 18, ("grid", "fp32"): 9, ("grid", "fp64"): 13}
 SLOTS_V_ONLY = {"list": 13, "grid": 8}     # FP64 potential only (E = NULL)
 KERNEL = {("list", "fp32"): "pair_kernel_f32x2", ("list", "fp64"): "pair_kernel<double>",
           ("grid", "fp32"): "grid_kernel_f32x2", ("grid", "fp64"): "grid_kernel_f64"}

@@ -62,19 +62,23 @@ __device__ __forceinline__ void on_lattice(double u, int n, float &a, float &dd)
     dd = static_cast<float>(u - al);
 }
 
-// y0 / 2 on the integer pipe (exponent - 1; y0 is a normal number): one FMA-pipe operation
-// of the Newton step moved to the idle ALU pipe.
-__device__ __forceinline__ float2 half_f32x2(float2 y) {
-    return f2(__int_as_float(__float_as_int(y.x) - 0x00800000),
-              __int_as_float(__float_as_int(y.y) - 0x00800000));
-}
-
 // A run of z nodes of the lane's row for EP2 packed point pairs, software-pipelined: while
-// the FMA pipe works on node n (Newton step, V, field sums) the MUFU.RSQ of node n + 1 is
-// already in flight (two register sets A / B in turn).  Per pair: dz (1 add: the running dz
-// steps by -1, exact on the lattice), r^2 (1 fma), 3 FMA-pipe operations + 1 integer
-// operation for the Newton step, p = q y, V += p, y^2, s = p y^2, sum s, sum s dz = 11
-// FMA-pipe lane operations + 1 MUFU.RSQ (+ 5/16 for the V tree).
+// the FMA pipe works on node n the MUFU.RSQ of node n + 1 is already in flight (two register
+// sets A / B in turn).
+//
+// The Newton step is applied to the SUM, not to every pair.  With y0 = MUFU.RSQ(r^2),
+// a = q y0 and c = q y0^3 (needed for the field anyway), the refined term is
+//     q y1 = q y0 (3 - r^2 y0^2) / 2 = (3 a - c r^2) / 2,
+// so V = (3 sum a - sum c r^2) / 2: ONE extra fma per pair (T += c r^2) instead of the three
+// FMA-pipe operations + one integer operation of a per-pair step, and algebraically the same
+// value.  (Evaluating y0 (3 - r^2 y0^2) / 2 per pair would round the correction away: the
+// bracket is ~2, its ulp 2.4e-7 is the size of the MUFU error.  Raw MUFU.RSQ values have a
+// mean relative error of +5.5e-9 on these inputs -- measured: 1.2e-5 hartree per 64-electron
+// walker, over the tolerance -- hence the refinement.)  The FIELD uses y0 itself: its
+// tolerance is 1e-5 relative per point, the raw values give 4e-7.
+// Per pair: dz (the running dz steps by -1, exact on the lattice), r^2, a = q y0, V0 += a,
+// y0^2, c = a y0^2, sum c, sum c dz, T += c r^2 = 9 FMA-pipe lane operations + 1 MUFU.RSQ
+// (+ 10/16 for the two summation trees).
 template <int EP2>
 struct GridRowF32 {
     float2 dzA[EP2], r2A[EP2], y0A[EP2], dzB[EP2], r2B[EP2], y0B[EP2];
@@ -108,60 +112,67 @@ struct GridRowF32 {
             y0n[e].y = rsqrt_mufu_f32(r2n[e].y);
         }
     }
-    // one Newton step, then V and the field sums of the node
+    // the sums of one node: V0 += a, T += c r^2, S += c, SZ += c dz
     __device__ __forceinline__ void acc(const float2 (&dz)[EP2], const float2 (&r2)[EP2],
                                         const float2 (&y0)[EP2], float q, float2 (&Vc)[EP2],
-                                        bool first) {
+                                        float2 (&Tc)[EP2], bool first) {
         const float2 qq = bc(q);
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
-            const float2 tt = __fmul2_rn(r2[e], y0[e]);
-            const float2 err = __ffma2_rn(f2(-tt.x, -tt.y), y0[e], bc(1.0f));
-            const float2 y = __ffma2_rn(half_f32x2(y0[e]), err, y0[e]);
-            const float2 p = __fmul2_rn(y, qq);
-            Vc[e] = first ? p : __fadd2_rn(Vc[e], p);
-            const float2 s = __fmul2_rn(p, __fmul2_rn(y, y));
-            S[e] = __fadd2_rn(S[e], s);
-            SZ[e] = __ffma2_rn(s, dz[e], SZ[e]);
+            const float2 a = __fmul2_rn(y0[e], qq);
+            Vc[e] = first ? a : __fadd2_rn(Vc[e], a);
+            const float2 c = __fmul2_rn(a, __fmul2_rn(y0[e], y0[e]));
+            Tc[e] = first ? __fmul2_rn(c, r2[e]) : __ffma2_rn(c, r2[e], Tc[e]);
+            S[e] = __fadd2_rn(S[e], c);
+            SZ[e] = __ffma2_rn(c, dz[e], SZ[e]);
         }
     }
-    // 4 nodes (one 128-bit load of charges); their V sum goes to Vc
-    __device__ __forceinline__ void four(const float *q4, float2 (&Vc)[EP2]) {
+    // 4 nodes (one 128-bit load of charges); their V0 and T sums go to Vc, Tc
+    __device__ __forceinline__ void four(const float *q4, float2 (&Vc)[EP2], float2 (&Tc)[EP2]) {
         const float4 Q = *reinterpret_cast<const float4 *>(q4);
         step(dzA, dzB, r2B, y0B);
-        acc(dzA, r2A, y0A, Q.x, Vc, true);
+        acc(dzA, r2A, y0A, Q.x, Vc, Tc, true);
         step(dzB, dzA, r2A, y0A);
-        acc(dzB, r2B, y0B, Q.y, Vc, false);
+        acc(dzB, r2B, y0B, Q.y, Vc, Tc, false);
         step(dzA, dzB, r2B, y0B);
-        acc(dzA, r2A, y0A, Q.z, Vc, false);
+        acc(dzA, r2A, y0A, Q.z, Vc, Tc, false);
         step(dzB, dzA, r2A, y0A);           // the last one looks one node past the run: unused
-        acc(dzB, r2B, y0B, Q.w, Vc, false);
+        acc(dzB, r2B, y0B, Q.w, Vc, Tc, false);
     }
-    // n4 * 4 nodes starting at b ([k4][32][4] floats); V is summed as a tree of short FP32
-    // runs (4 nodes -> 16 -> run): a long FP32 running sum of slowly varying same-sign terms
-    // drifts
-    __device__ __forceinline__ void run(const float *b, int n4, float2 (&v)[EP2]) {
+    // n4 * 4 nodes starting at b ([k4][32][4] floats); V0 and T are summed as trees of short
+    // FP32 runs (4 nodes -> 16 -> run): a long FP32 running sum of slowly varying same-sign
+    // terms drifts
+    __device__ __forceinline__ void run(const float *b, int n4, float2 (&v)[EP2], float2 (&t)[EP2]) {
         if ((n4 & 3) == 0) {
 #pragma unroll 1
             for (int g = 0; g < n4; g += 4) {
-                float2 v16[EP2], Vc[EP2];
-                four(b + g * 128, v16);
+                float2 v16[EP2], t16[EP2], Vc[EP2], Tc[EP2];
+                four(b + g * 128, v16, t16);
 #pragma unroll
                 for (int k4 = 1; k4 < 4; ++k4) {
-                    four(b + (g + k4) * 128, Vc);
+                    four(b + (g + k4) * 128, Vc, Tc);
 #pragma unroll
-                    for (int e = 0; e < EP2; ++e) v16[e] = __fadd2_rn(v16[e], Vc[e]);
+                    for (int e = 0; e < EP2; ++e) {
+                        v16[e] = __fadd2_rn(v16[e], Vc[e]);
+                        t16[e] = __fadd2_rn(t16[e], Tc[e]);
+                    }
                 }
 #pragma unroll
-                for (int e = 0; e < EP2; ++e) v[e] = __fadd2_rn(v[e], v16[e]);
+                for (int e = 0; e < EP2; ++e) {
+                    v[e] = __fadd2_rn(v[e], v16[e]);
+                    t[e] = __fadd2_rn(t[e], t16[e]);
+                }
             }
         } else {
 #pragma unroll 1
             for (int k4 = 0; k4 < n4; ++k4) {
-                float2 Vc[EP2];
-                four(b + k4 * 128, Vc);
+                float2 Vc[EP2], Tc[EP2];
+                four(b + k4 * 128, Vc, Tc);
 #pragma unroll
-                for (int e = 0; e < EP2; ++e) v[e] = __fadd2_rn(v[e], Vc[e]);
+                for (int e = 0; e < EP2; ++e) {
+                    v[e] = __fadd2_rn(v[e], Vc[e]);
+                    t[e] = __fadd2_rn(t[e], Tc[e]);
+                }
             }
         }
     }
@@ -258,16 +269,16 @@ __global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) 
         az[e] = f2(a0[2], a0[5]);
     }
     // FP32 accumulators over up to GRID_FLUSH gchunks, then FP64 columns
-    float2 vv[EP2], ex[EP2], ey[EP2], ez[EP2];
+    float2 vv[EP2], tt[EP2], ex[EP2], ey[EP2], ez[EP2];
 #pragma unroll
-    for (int e = 0; e < EP2; ++e) vv[e] = ex[e] = ey[e] = ez[e] = f2(0.0f, 0.0f);
+    for (int e = 0; e < EP2; ++e) vv[e] = tt[e] = ex[e] = ey[e] = ez[e] = f2(0.0f, 0.0f);
     auto flush = [&]() {
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
             double2 t;
-            t = my[(4 * e + 0) * NT];
-            t.x += static_cast<double>(vv[e].x);
-            t.y += static_cast<double>(vv[e].y);
+            t = my[(4 * e + 0) * NT];            // V = (3 sum a - sum c r^2) / 2: the Newton step
+            t.x += 1.5 * static_cast<double>(vv[e].x) - 0.5 * static_cast<double>(tt[e].x);
+            t.y += 1.5 * static_cast<double>(vv[e].y) - 0.5 * static_cast<double>(tt[e].y);
             my[(4 * e + 0) * NT] = t;
             t = my[(4 * e + 1) * NT];
             t.x += static_cast<double>(ex[e].x);
@@ -281,7 +292,7 @@ __global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) 
             t.x += static_cast<double>(ez[e].x);
             t.y += static_cast<double>(ez[e].y);
             my[(4 * e + 3) * NT] = t;
-            vv[e] = ex[e] = ey[e] = ez[e] = f2(0.0f, 0.0f);
+            vv[e] = tt[e] = ex[e] = ey[e] = ez[e] = f2(0.0f, 0.0f);
         }
     };
 
@@ -296,26 +307,27 @@ __global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) 
         if (warp == 0) produce();          // gchunk g + stages - 1 into the slot freed by g - 1
         const float2 fx = bc(static_cast<float>(ix)), fy = bc(static_cast<float>(iy));
         const float2 fz = bc(static_cast<float>(seg * GRID_ZS + z0));
-        float2 dx[EP2], dy[EP2], rxy2[EP2], azb[EP2], v[EP2];
+        float2 dx[EP2], dy[EP2], rxy2[EP2], azb[EP2], v[EP2], tq[EP2];
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
             dx[e] = __fadd2_rn(ax[e], f2(-fx.x, -fx.y));          // exact (lattice)
             dy[e] = __fadd2_rn(ay[e], f2(-fy.x, -fy.y));
             azb[e] = __fadd2_rn(az[e], f2(-fz.x, -fz.y));
             rxy2[e] = __ffma2_rn(dy[e], dy[e], __ffma2_rn(dx[e], dx[e], bc(1e-30f)));
-            v[e] = f2(0.0f, 0.0f);
+            v[e] = tq[e] = f2(0.0f, 0.0f);
         }
         GridRowF32<EP2> row;
         row.start(azb, rxy2);
         mbar_wait(&full[slot], phase);
         const float *data = reinterpret_cast<const float *>(smem + static_cast<size_t>(slot) * STAGE_BYTES);
-        row.run(data + (z0 / 4) * 128 + 4 * lane, ZL / 4, v);
+        row.run(data + (z0 / 4) * 128 + 4 * lane, ZL / 4, v, tq);
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[slot]);
         // Ex = dx sum(s), Ey = dy sum(s), Ez = sum(s dz)
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
             vv[e] = __fadd2_rn(vv[e], v[e]);
+            tt[e] = __fadd2_rn(tt[e], tq[e]);
             ex[e] = __ffma2_rn(dx[e], row.S[e], ex[e]);
             ey[e] = __ffma2_rn(dy[e], row.S[e], ey[e]);
             ez[e] = __fadd2_rn(ez[e], row.SZ[e]);

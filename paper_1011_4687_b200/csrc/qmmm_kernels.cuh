@@ -505,8 +505,8 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
 
 // ----------------------------------------------------------------------------- FP32 packed
 // FP32-acc64 pair kernel for EPT >= 2: two evaluation points share one f32x2 register pair
-// (sm_100 FADD2 / FMUL2 / FFMA2; the source scalar is a broadcast operand), so the 17
-// FP32-pipe operations of a pair cost 8.5 issue slots and the issue port is no longer the
+// (sm_100 FADD2 / FMUL2 / FFMA2; the source scalar is a broadcast operand), so the 14
+// FP32-pipe operations of a pair cost 7 issue slots and the issue port is no longer the
 // limiter.  The per-thread FP64 running sums live in shared memory (one conflict-free
 // column per thread) instead of 8*EPT registers, which leaves the register file to the
 // interleaved FP32 chains: ptxas serialises the pairs when the doubles stay in registers.
@@ -515,10 +515,18 @@ __device__ __forceinline__ float2 bc(float a) { return make_float2(a, a); }   //
 
 // One 128-source chunk: the lane's 4 sources x EP2 point pairs, written stage by stage so
 // that EP2 independent chains are in flight around every MUFU.
+//
+// The Newton step is applied to the SUM, not to every pair.  With y0 = MUFU.RSQ(r^2),
+// a = q y0 and c = q y0^3 (needed for the field anyway) the refined term is
+//     q y1 = q y0 (3 - r^2 y0^2) / 2 = (3 a - c r^2) / 2,
+// so V = (3 sum a - sum c r^2) / 2: one extra fma per pair (T += c r^2) instead of the four
+// operations of a per-pair step, algebraically the same value.  The field uses y0 itself
+// (tolerance 1e-5 relative per point; the raw MUFU values give 4e-7).  14 FP32-pipe
+// operations per pair: 3 sub, mul + 2 fma (r^2), a, V0 += a, y0^2, c, T, 3 fma (E).
 template <int EP2>
 __device__ __forceinline__ void chunk_f32x2(const float *b, const float2 (&rx)[EP2],
                                             const float2 (&ry)[EP2], const float2 (&rz)[EP2],
-                                            float2 (&V)[EP2], float2 (&Ex)[EP2],
+                                            float2 (&V)[EP2], float2 (&T)[EP2], float2 (&Ex)[EP2],
                                             float2 (&Ey)[EP2], float2 (&Ez)[EP2]) {
     const float4 X = *reinterpret_cast<const float4 *>(b);
     const float4 Y = *reinterpret_cast<const float4 *>(b + CHUNK);
@@ -526,10 +534,10 @@ __device__ __forceinline__ void chunk_f32x2(const float *b, const float2 (&rx)[E
     const float4 Q = *reinterpret_cast<const float4 *>(b + 3 * CHUNK);
     const float xs[4] = {X.x, X.y, X.z, X.w}, ys[4] = {Y.x, Y.y, Y.z, Y.w};
     const float zs[4] = {Z.x, Z.y, Z.z, Z.w}, qs[4] = {Q.x, Q.y, Q.z, Q.w};
-    // V is summed as a tree of short FP32 runs (4 sources -> 4 chunks -> stage): a long FP32
-    // running sum of slowly varying same-sign terms drifts systematically (DESIGN.md "FP32
-    // path": +8e-8 hartree per point at 64 terms), a 4-term run does not.
-    float2 Vc[EP2];
+    // V0 and T are summed as trees of short FP32 runs (4 sources -> 4 chunks -> stage): a long
+    // FP32 running sum of slowly varying same-sign terms drifts systematically (DESIGN.md
+    // "FP32 path": +8e-8 hartree per point at 64 terms), a 4-term run does not.
+    float2 Vc[EP2], Tc[EP2];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         float2 dx[EP2], dy[EP2], dz[EP2], r2[EP2], y0[EP2];
@@ -547,21 +555,21 @@ __device__ __forceinline__ void chunk_f32x2(const float *b, const float2 (&rx)[E
             y0[e].y = rsqrt_mufu_f32(r2[e].y);
         }
 #pragma unroll
-        for (int e = 0; e < EP2; ++e) {       // one Newton step, then V and E (17 FP32 ops/pair)
-            const float2 t = __fmul2_rn(r2[e], y0[e]);
-            const float2 err = __ffma2_rn(f2(-t.x, -t.y), y0[e], bc(1.0f));
-            const float2 h = __fmul2_rn(y0[e], bc(0.5f));
-            const float2 y = __ffma2_rn(h, err, y0[e]);
-            const float2 p = __fmul2_rn(y, qq);
-            Vc[e] = k == 0 ? p : __fadd2_rn(Vc[e], p);
-            const float2 s = __fmul2_rn(p, __fmul2_rn(y, y));
-            Ex[e] = __ffma2_rn(s, dx[e], Ex[e]);
-            Ey[e] = __ffma2_rn(s, dy[e], Ey[e]);
-            Ez[e] = __ffma2_rn(s, dz[e], Ez[e]);
+        for (int e = 0; e < EP2; ++e) {
+            const float2 a = __fmul2_rn(y0[e], qq);
+            Vc[e] = k == 0 ? a : __fadd2_rn(Vc[e], a);
+            const float2 c = __fmul2_rn(a, __fmul2_rn(y0[e], y0[e]));
+            Tc[e] = k == 0 ? __fmul2_rn(c, r2[e]) : __ffma2_rn(c, r2[e], Tc[e]);
+            Ex[e] = __ffma2_rn(c, dx[e], Ex[e]);
+            Ey[e] = __ffma2_rn(c, dy[e], Ey[e]);
+            Ez[e] = __ffma2_rn(c, dz[e], Ez[e]);
         }
     }
 #pragma unroll
-    for (int e = 0; e < EP2; ++e) V[e] = __fadd2_rn(V[e], Vc[e]);
+    for (int e = 0; e < EP2; ++e) {
+        V[e] = __fadd2_rn(V[e], Vc[e]);
+        T[e] = __fadd2_rn(T[e], Tc[e]);
+    }
 }
 
 // grid = (point_blocks, slices); EPT = 2 * EP2 points per thread; NW consumer warps and no
@@ -687,23 +695,26 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
             dd_s[lane] = static_cast<float>(a64 - static_cast<double>(a32));
         }
         __syncwarp();
-        float2 rx[EP2], ry[EP2], rz[EP2], v[EP2], ex[EP2], ey[EP2], ez[EP2];
+        float2 rx[EP2], ry[EP2], rz[EP2], v[EP2], tq[EP2], ex[EP2], ey[EP2], ez[EP2];
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
             rx[e] = *reinterpret_cast<const float2 *>(a_s + 2 * e);
             ry[e] = *reinterpret_cast<const float2 *>(a_s + EPT + 2 * e);
             rz[e] = *reinterpret_cast<const float2 *>(a_s + 2 * EPT + 2 * e);
-            v[e] = ex[e] = ey[e] = ez[e] = f2(0.0f, 0.0f);
+            v[e] = tq[e] = ex[e] = ey[e] = ez[e] = f2(0.0f, 0.0f);
         }
         for (int ch = ws; ch < nch;) {
-            float2 v4[EP2];                           // middle level of the V tree: 4 chunks
+            float2 v4[EP2], t4[EP2];                  // middle level of the trees: 4 chunks
 #pragma unroll
-            for (int e = 0; e < EP2; ++e) v4[e] = f2(0.0f, 0.0f);
+            for (int e = 0; e < EP2; ++e) v4[e] = t4[e] = f2(0.0f, 0.0f);
 #pragma unroll 1
             for (int g = 0; g < 4 && ch < nch; ++g, ch += WS)
-                chunk_f32x2<EP2>(data + ch * 4 * CHUNK + 4 * lane, rx, ry, rz, v4, ex, ey, ez);
+                chunk_f32x2<EP2>(data + ch * 4 * CHUNK + 4 * lane, rx, ry, rz, v4, t4, ex, ey, ez);
 #pragma unroll
-            for (int e = 0; e < EP2; ++e) v[e] = __fadd2_rn(v[e], v4[e]);
+            for (int e = 0; e < EP2; ++e) {
+                v[e] = __fadd2_rn(v[e], v4[e]);
+                tq[e] = __fadd2_rn(tq[e], t4[e]);
+            }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[slot]);   // the stage's source data is consumed
@@ -716,9 +727,11 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
             const float2 ddz = *reinterpret_cast<const float2 *>(dd_s + 2 * EPT + 2 * e);
             const float2 corr = __ffma2_rn(ez[e], ddz, __ffma2_rn(ey[e], ddy, __fmul2_rn(ex[e], ddx)));
             double2 t;                                // rows of the pair: V, Ex, Ey, Ez
-            t = my[(4 * e + 0) * NT];
-            t.x += static_cast<double>(v[e].x) - static_cast<double>(corr.x);
-            t.y += static_cast<double>(v[e].y) - static_cast<double>(corr.y);
+            t = my[(4 * e + 0) * NT];                // V = (3 sum a - sum c r^2) / 2: the Newton step
+            t.x += 1.5 * static_cast<double>(v[e].x) - 0.5 * static_cast<double>(tq[e].x) -
+                   static_cast<double>(corr.x);
+            t.y += 1.5 * static_cast<double>(v[e].y) - 0.5 * static_cast<double>(tq[e].y) -
+                   static_cast<double>(corr.y);
             my[(4 * e + 0) * NT] = t;
             t = my[(4 * e + 1) * NT];
             t.x += static_cast<double>(ex[e].x);
