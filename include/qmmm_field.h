@@ -90,6 +90,19 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
                             double *V, double *E, int prec, void *stream);
 
 /*
+ * qmmm_field_eval_energy -- the paper's own output (Eq. 4): the electrostatic
+ * energy of each configuration's electrons in the environment's field,
+ *     U_ES[w] = - sum_{i<N} V(r_{w,i})          (electrons carry charge -1),
+ * without writing V or E back ("energy-fused variant").
+ *   elec_xyz  DEVICE [W][N][3] FP64;   U  DEVICE [W] FP64 out;   prec, stream as eval.
+ * The field is not formed in FP64 (potential-only kernel); the per-walker sum runs in a
+ * fixed order (deterministic).  Two launches on `stream`, never synchronises.
+ * Errors as qmmm_field_eval (U takes the place of V).
+ */
+qmmm_status qmmm_field_eval_energy(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t N,
+                                   double *U, int prec, void *stream);
+
+/*
  * qmmm_field_eval_host -- the paper's per-step call: HOST buffers in and out;
  * returns when V_host (and E_host) hold the result.  Buffers may be pageable or pinned.
  *   W*N == 1  : served by a resident "move server": one cooperative kernel (one CTA per SM)

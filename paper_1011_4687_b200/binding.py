@@ -26,7 +26,7 @@ _STATUS = {0: "QMMM_OK", 1: "QMMM_ERR_INVALID_ARG", 2: "QMMM_ERR_ALLOC", 3: "QMM
 LIB_PATH = os.environ.get("QMMM_FIELD_LIB") or os.path.join(
     os.path.dirname(os.path.abspath(__file__)), "libqmmm_field.so")
 EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_host",
-                    "qmmm_field_eval_moves_host", "qmmm_field_create_grid",
+                    "qmmm_field_eval_moves_host", "qmmm_field_create_grid", "qmmm_field_eval_energy",
                     "qmmm_field_set_layout", "qmmm_field_get_grid_info",
                     "qmmm_field_destroy", "qmmm_field_set_plan", "qmmm_field_get_info",
                     "qmmm_field_set_timing", "qmmm_field_last_timing",
@@ -77,6 +77,8 @@ def _load() -> ctypes.CDLL:
     lib.qmmm_field_create.argtypes = [vp, vp, i64, vp, vp, i64, i64, ctypes.POINTER(vp)]
     lib.qmmm_field_eval.restype = ci
     lib.qmmm_field_eval.argtypes = [vp, vp, i64, i64, vp, vp, ci, vp]
+    lib.qmmm_field_eval_energy.restype = ci
+    lib.qmmm_field_eval_energy.argtypes = [vp, vp, i64, i64, vp, ci, vp]
     lib.qmmm_field_eval_host.restype = ci
     lib.qmmm_field_eval_host.argtypes = [vp, vp, i64, i64, vp, vp, ci, vp]
     lib.qmmm_field_eval_moves_host.restype = ci
@@ -181,6 +183,13 @@ def qmmm_field_eval(handle: int, elec_xyz, W: int, N: int, V, E=None, precision=
     """Asynchronous evaluation on device tensors (elec_xyz [W*N,3], V [W*N], E [W*N,3])."""
     _check(_lib.qmmm_field_eval(handle, _ptr(elec_xyz), int(W), int(N), _ptr(V), _ptr(E),
                                 _PREC[precision], _stream(stream)))
+
+
+def qmmm_field_eval_energy(handle: int, elec_xyz, W: int, N: int, U, precision="fp64",
+                           stream=None) -> None:
+    """U[w] = -sum_i V(r_{w,i}) per walker (Eq. 4), device tensors, asynchronous."""
+    _check(_lib.qmmm_field_eval_energy(handle, _ptr(elec_xyz), int(W), int(N), _ptr(U),
+                                       _PREC[precision], _stream(stream)))
 
 
 def qmmm_field_eval_host(handle: int, elec_xyz, W: int, N: int, V, E=None, precision="fp64",

@@ -163,6 +163,11 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32, bool grid = fals
     if (pl.slices == 0) {
         const int g = gcd_int(static_cast<int>(pb % h->sm_count), h->sm_count);
         pl.slices = h->sm_count / g;       // pb * slices is a multiple of the SM count
+        // Many waves: a CTA costs about 5 us of launch, pipeline fill, reduction and ticket
+        // whatever its length, while a partly filled last wave costs less and less.  Halve
+        // the slices (longer CTAs) as long as 32 or more waves remain.
+        while (pl.slices > 1 && pb * ((pl.slices + 1) / 2) >= 32 * static_cast<int64_t>(h->sm_count))
+            pl.slices = (pl.slices + 1) / 2;
     }
     const int64_t work_units = grid ? std::max<int64_t>(h->n_g, (h->K + 31) / 32)
                                : f32 ? std::max<int64_t>(h->n_chunks, (h->K + 31) / 32) : h->n_chunks64;
@@ -1031,6 +1036,22 @@ extern "C" {
 qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t N,
                             double *V, double *E, int prec, void *stream) {
     return eval_impl(h, elec_xyz, W, N, V, E, prec, stream, nullptr);
+}
+
+qmmm_status qmmm_field_eval_energy(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t N,
+                                   double *U, int prec, void *stream) {
+    if (!h) return fail(QMMM_ERR_INVALID_ARG, "eval_energy: NULL handle");
+    if (!U) return fail(QMMM_ERR_INVALID_ARG, "eval_energy: NULL U");
+    // V goes to the handle's staging buffer (sized for max_points), E is not formed (FP64:
+    // the potential-only kernel, Eq. 4 proper), then one small fixed-order sum per walker
+    qmmm_status s = eval_impl(h, elec_xyz, W, N, h->stage_out, nullptr, prec, stream, nullptr);
+    if (s != QMMM_OK) return s;
+    walker_energy_kernel<<<static_cast<unsigned>((W + 7) / 8), 256, 0, static_cast<cudaStream_t>(stream)>>>(
+        h->stage_out, W, N, U);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "walker_energy_kernel launch");
+    ++h->last_launches;
+    return QMMM_OK;
 }
 
 qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int64_t W,

@@ -807,6 +807,26 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
     QMMM_MARK_GT(9);
 }
 
+// ----------------------------------------------------------------------------- walker energy
+// U_ES of one configuration (Eq. 4: the energy of the electrons in the
+// environment's field, U = -sum_i V(r_i) with the library's sign convention): one warp per
+// walker, lane-strided fixed-order sums, then the butterfly.  Deterministic.
+__global__ void __launch_bounds__(256) walker_energy_kernel(const double *V, int64_t W, int64_t N,
+                                                            double *U) {
+    const int64_t w = blockIdx.x * 8ll + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (w >= W) return;
+    const double *v = V + w * N;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    int64_t i = lane;
+    for (; i + 96 < N; i += 128) {
+        a0 += v[i]; a1 += v[i + 32]; a2 += v[i + 64]; a3 += v[i + 96];
+    }
+    for (; i < N; i += 32) a0 += v[i];
+    const double s = warp_sum((a0 + a1) + (a2 + a3));
+    if (lane == 0) U[w] = -s;
+}
+
 // ----------------------------------------------------------------------------- packing
 // a0: pack {R_j, q_j} once per environment.
 // Pads (j >= M) replicate the last real source with charge 0: they contribute exactly 0.

@@ -333,3 +333,32 @@ def test_config4_grid_fp64(torch_cuda, B, oracle_mod):
     assert np.all(np.isfinite(V)) and np.all(np.isfinite(E))
     assert np.max(np.abs(V - Vl) / np.abs(Vl)) <= 1e-12
     assert np.max(np.linalg.norm(E - El, axis=1) / np.linalg.norm(El, axis=1)) <= 1e-11
+
+
+# ------------------------------------------------------------------ per-walker energy (Eq. 4)
+@pytest.mark.parametrize("precision,tol", [("fp64", 1e-11), ("fp32", E_TOL)])
+@pytest.mark.parametrize("layout", ["list", "grid"])
+def test_eval_energy_per_walker(torch_cuda, B, oracle_mod, precision, tol, layout):
+    """qmmm_field_eval_energy: U_ES[w] = -sum_i V(r_wi) for 6 walkers x 37
+    electrons on config 1's environment, against the oracle's per-walker sums."""
+    w = make_workload(1, n_points=(6, 37))
+    pts = w.elec_xyz.reshape(-1, 3)
+    ref = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, pts, want_E=False)
+    want = -ref.V.reshape(6, 37).sum(1)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, len(pts))
+    try:
+        B.qmmm_field_set_layout(h, layout)
+        d = torch_cuda.from_numpy(pts).cuda()
+        U = torch_cuda.full((6,), float("nan"), dtype=torch_cuda.float64, device="cuda")
+        B.qmmm_field_eval_energy(h, d, 6, 37, U, precision)
+        torch_cuda.cuda.synchronize()
+        got = U.cpu().numpy()
+        assert np.max(np.abs(got - want)) <= tol, f"max |dU| = {np.max(np.abs(got - want)):.3e} hartree"
+        U2 = torch_cuda.zeros(6, dtype=torch_cuda.float64, device="cuda")
+        B.qmmm_field_eval_energy(h, d, 6, 37, U2, precision)
+        torch_cuda.cuda.synchronize()
+        assert np.array_equal(got, U2.cpu().numpy())                     # deterministic
+        V, _ = run(torch_cuda, B, h, pts, precision, want_E=False)
+        assert np.max(np.abs(got + V.reshape(6, 37).sum(1))) <= 1e-11    # = -sum of eval's V
+    finally:
+        B.qmmm_field_destroy(h)
