@@ -362,3 +362,54 @@ def test_eval_energy_per_walker(torch_cuda, B, oracle_mod, precision, tol, layou
         assert np.max(np.abs(got + V.reshape(6, 37).sum(1))) <= 1e-11    # = -sum of eval's V
     finally:
         B.qmmm_field_destroy(h)
+
+
+# --------------------------------------------------------------------- seeded random sweep
+def test_random_grids_plans_and_precisions(torch_cuda, B, oracle_mod):
+    """40 seeded random combinations of grid shape, spacing, fill, point count, launch plan,
+    precision and entry point (list + detection, or qmmm_field_create_grid), each against the
+    oracle on the list of occupied nodes."""
+    rng = np.random.default_rng(20261104)
+    for case in range(40):
+        n = tuple(int(v) for v in rng.integers(1, 70, size=3))
+        if rng.random() < 0.5:
+            n = (n[0], int(rng.choice([32, 64, 96])), int(rng.choice([64, 128])))
+        h = float(rng.choice([0.1, 0.25, 0.3, 0.5]))
+        origin = rng.normal(size=3) * 3.0
+        centre = origin + 0.5 * h * (np.array(n) - 1)
+        dense, pos, q = random_grid(rng, n, h, origin, fill=float(rng.uniform(0.55, 1.0)),
+                                    hole=(centre, 1.5), signed=bool(rng.random() < 0.3))
+        if len(q) == 0:
+            continue
+        K = int(rng.integers(0, 9))
+        nuc = centre + rng.normal(size=(K, 3)) * 3.0 + 5.0
+        Z = rng.choice([1.0, 6.0, 7.0, 8.0], size=K)
+        P = int(rng.choice([1, 2, 3, 5, 8, 17, 32, 33, 64, 100, 257]))
+        pts = centre + rng.normal(size=(P, 3)) * 0.4
+        pts = centre + (pts - centre) * np.minimum(1.0, 1.1 / np.linalg.norm(pts - centre, axis=1))[:, None]
+        precision = "fp32" if rng.random() < 0.5 else "fp64"
+        tol = TOL32 if precision == "fp32" else TOL64
+        ref = oracle_mod.field(pos, q, nuc if K else NO_XYZ, Z if K else NO_Z, pts, want_abs=True)
+        use_list = len(q) >= 4096 and rng.random() < 0.5
+        if use_list:
+            hnd = B.qmmm_field_create(pos, q, nuc if K else None, Z if K else None, P)
+        else:
+            hnd = B.qmmm_field_create_grid(origin, h, n, dense, nuc if K else None, Z if K else None, P)
+        try:
+            gi = B.qmmm_field_get_grid_info(hnd)
+            if not gi["present"]:       # a sparse random grid may fail the fill criterion
+                continue
+            plan = dict(points_per_thread=int(rng.choice([0, 1, 2, 4, 8])),
+                        point_warps=int(rng.choice([0, 1, 2, 4, 8, 16])),
+                        slices=int(rng.choice([0, 1, 3, 37, 200])), stages=int(rng.choice([0, 2, 5, 8])))
+            want_E = bool(rng.random() < 0.8)
+            V, E = run(torch_cuda, B, hnd, pts, precision, want_E=want_E, layout="grid", plan=plan)
+            eV, eE = rel_errors(ref, V, E)
+            kV = ref.absV / np.abs(ref.V)
+            kE = ref.absE / np.linalg.norm(ref.E, axis=1)
+            msg = f"case {case}: n={n} h={h} P={P} {precision} plan={plan} list={use_list}"
+            assert np.all(eV <= tol * np.maximum(1.0, kV)), f"{msg}: V rel err {eV.max():.3e}"
+            if want_E:
+                assert np.all(eE <= tol * np.maximum(1.0, kE)), f"{msg}: E rel err {eE.max():.3e}"
+        finally:
+            B.qmmm_field_destroy(hnd)
