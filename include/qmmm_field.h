@@ -82,7 +82,8 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
  *   E         DEVICE [W*N][3] FP64    out: field; NULL = potential only
  *   prec      qmmm_precision
  *   stream    cudaStream_t (as void*); all work is enqueued on it, the call never
- *             synchronises.  One eval in flight per handle (shared workspace).
+ *             synchronises.  One eval in flight per handle (its workspace); for concurrent
+ *             streams or host threads use qmmm_field_share.
  * Errors: INVALID_ARG (NULL handle/elec_xyz/V, W*N < 1 or > max_points, bad prec),
  * CUDA (launch failure).  Outputs are unspecified after an error.
  */
@@ -185,6 +186,20 @@ typedef struct {
     int64_t bytes_fp32, bytes_fp64;
 } qmmm_grid_info;
 qmmm_status qmmm_field_get_grid_info(const qmmm_field *h, qmmm_grid_info *info);
+
+/*
+ * qmmm_field_share -- a second handle on the SAME environment for concurrent use.
+ * The paper suggests OpenMP on the host code and one GPU shared by the node's MPI ranks
+ * (PAPER.md:23, :242); one eval may be in flight per handle (its partials workspace, tickets
+ * and mailboxes are per handle), so every host thread / stream gets its own handle.  The new
+ * handle shares the parent's packed source copies (immutable after create; no copy, no
+ * packing) and owns only its runtime buffers sized by max_points; plan, layout choice,
+ * timing and the move server are per handle.  Handles may be destroyed in any order: the
+ * source copies are freed with the last one.  Results are bitwise those of the parent.
+ * Errors: INVALID_ARG (NULL argument, max_points < 1, current device differs from the
+ * parent's), ALLOC, CUDA.
+ */
+qmmm_status qmmm_field_share(const qmmm_field *parent, int64_t max_points, qmmm_field **out);
 
 /* qmmm_field_destroy -- frees the handle and its device buffers.  NULL is a no-op. */
 qmmm_status qmmm_field_destroy(qmmm_field *h);

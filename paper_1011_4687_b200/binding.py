@@ -27,6 +27,7 @@ LIB_PATH = os.environ.get("QMMM_FIELD_LIB") or os.path.join(
     os.path.dirname(os.path.abspath(__file__)), "libqmmm_field.so")
 EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_host",
                     "qmmm_field_eval_moves_host", "qmmm_field_create_grid", "qmmm_field_eval_energy",
+                    "qmmm_field_share",
                     "qmmm_field_set_layout", "qmmm_field_get_grid_info",
                     "qmmm_field_destroy", "qmmm_field_set_plan", "qmmm_field_get_info",
                     "qmmm_field_set_timing", "qmmm_field_last_timing",
@@ -88,6 +89,8 @@ def _load() -> ctypes.CDLL:
     lib.qmmm_field_create_grid.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.c_double,
                                            ctypes.POINTER(i64), vp, vp, vp, i64, i64,
                                            ctypes.POINTER(vp)]
+    lib.qmmm_field_share.restype = ci
+    lib.qmmm_field_share.argtypes = [vp, i64, ctypes.POINTER(vp)]
     lib.qmmm_field_set_layout.restype = ci
     lib.qmmm_field_set_layout.argtypes = [vp, ci]
     lib.qmmm_field_get_grid_info.restype = ci
@@ -159,6 +162,14 @@ def qmmm_field_create_grid(origin, spacing: float, n, cell_q, nuc_xyz, nuc_Z,
     out = ctypes.c_void_p()
     _check(_lib.qmmm_field_create_grid(org, float(spacing), dims, _ptr(cell_q), _ptr(nuc_xyz),
                                        _ptr(nuc_Z), K, int(max_points), ctypes.byref(out)))
+    return out.value
+
+
+def qmmm_field_share(parent: int, max_points: int) -> int:
+    """A second handle on the same environment (shares the packed sources, own workspace):
+    one per stream / host thread for concurrent evaluations."""
+    out = ctypes.c_void_p()
+    _check(_lib.qmmm_field_share(parent, int(max_points), ctypes.byref(out)))
     return out.value
 
 

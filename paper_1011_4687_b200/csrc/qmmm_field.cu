@@ -17,6 +17,7 @@
 #include <cstdio>
 #include <cstring>
 #include <ctime>
+#include <memory>
 #include <new>
 #include <string>
 
@@ -95,7 +96,18 @@ size_t grid_smem_bytes(bool f32, int stages, int ept, int wp) {
 
 }  // namespace
 
+// The packed source copies of one environment.  They are immutable after create and may be
+// shared by several handles (qmmm_field_share): the last handle to go frees them.
+struct SourceOwner {
+    void *ptr[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    ~SourceOwner() {
+        for (void *p : ptr)
+            if (p) cudaFree(p);
+    }
+};
+
 struct qmmm_field {
+    std::shared_ptr<SourceOwner> keep;   // owns chunks64/32, origins, nuclei, gcells32/64, nuclei_u
     int64_t M = 0, K = 0, max_points = 0;
     int64_t n_chunks = 0, n_chunks64 = 0, n_blocks = 0;
     int device = 0, sm_count = 0;
@@ -587,6 +599,13 @@ qmmm_status server_move(qmmm_field *h, const double *r, double *V, double *E, in
 }  // namespace
 
 namespace {
+// From here on the source copies are owned by a shared SourceOwner (qmmm_field_share).
+void adopt_sources(qmmm_field *h) {
+    h->keep = std::make_shared<SourceOwner>();
+    void *p[7] = {h->chunks64, h->chunks32, h->origins, h->nuclei, h->gcells32, h->gcells64, h->nuclei_u};
+    for (int i = 0; i < 7; ++i) h->keep->ptr[i] = p[i];
+}
+
 // Per-handle buffers that do not depend on the source format: partials workspace, tickets,
 // mailboxes, move-server state, eval_host staging.
 qmmm_status alloc_runtime(qmmm_field *h) {
@@ -744,6 +763,7 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
         if (rs != QMMM_OK) return bail(rs);
     }
 #undef CREATE_TRY
+    adopt_sources(h);
     *out = h;
     return QMMM_OK;
 }
@@ -820,6 +840,40 @@ qmmm_status qmmm_field_create_grid(const double *origin, double spacing, const i
         qmmm_status rs = alloc_runtime(h);
         if (rs != QMMM_OK) return bail(rs);
     }
+    adopt_sources(h);
+    *out = h;
+    return QMMM_OK;
+}
+
+qmmm_status qmmm_field_share(const qmmm_field *parent, int64_t max_points, qmmm_field **out) {
+    if (!out) return fail(QMMM_ERR_INVALID_ARG, "share: out is NULL");
+    *out = nullptr;
+    if (!parent || !parent->keep) return fail(QMMM_ERR_INVALID_ARG, "share: NULL or incomplete parent handle");
+    if (max_points < 1) return fail(QMMM_ERR_INVALID_ARG, "share: max_points < 1");
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != parent->device)
+        return fail(QMMM_ERR_INVALID_ARG, "share: the current device is not the parent handle's device");
+    qmmm_field *h = new (std::nothrow) qmmm_field();
+    if (!h) return fail(QMMM_ERR_ALLOC, "share: host allocation failed");
+    // the immutable part: source copies, their geometry and sizes
+    h->keep = parent->keep;
+    h->M = parent->M; h->K = parent->K; h->max_points = max_points;
+    h->n_chunks = parent->n_chunks; h->n_chunks64 = parent->n_chunks64; h->n_blocks = parent->n_blocks;
+    h->device = parent->device; h->sm_count = parent->sm_count;
+    h->chunks64 = parent->chunks64; h->chunks32 = parent->chunks32; h->origins = parent->origins;
+    h->lattice = parent->lattice; h->nuclei = parent->nuclei;
+    h->has_list = parent->has_list; h->has_grid = parent->has_grid; h->grid = parent->grid;
+    h->g_rows = parent->g_rows; h->g_tiles = parent->g_tiles; h->g_segs = parent->g_segs; h->n_g = parent->n_g;
+    h->gcells32 = parent->gcells32; h->gcells64 = parent->gcells64; h->nuclei_u = parent->nuclei_u;
+    h->layout = parent->layout;
+    for (int k = 0; k < 3; ++k) { h->bb_lo[k] = parent->bb_lo[k]; h->bb_hi[k] = parent->bb_hi[k]; }
+    // its own mutable part: workspace, tickets, mailboxes, move server, staging, plan
+    qmmm_status rs = alloc_runtime(h);
+    if (rs != QMMM_OK) {
+        qmmm_field_destroy(h);
+        return rs;
+    }
     *out = h;
     return QMMM_OK;
 }
@@ -863,13 +917,16 @@ qmmm_status qmmm_field_destroy(qmmm_field *h) {
     if (h->srv_stream) cudaStreamDestroy(h->srv_stream);
     if (h->srv_mail_h) cudaFreeHost(h->srv_mail_h);
     cudaFree(h->srv_dev);
-    cudaFree(h->chunks64);
-    cudaFree(h->chunks32);
-    cudaFree(h->origins);
-    cudaFree(h->nuclei);
-    cudaFree(h->gcells32);
-    cudaFree(h->gcells64);
-    cudaFree(h->nuclei_u);
+    if (!h->keep) {                 // a handle that failed before its sources were adopted
+        cudaFree(h->chunks64);
+        cudaFree(h->chunks32);
+        cudaFree(h->origins);
+        cudaFree(h->nuclei);
+        cudaFree(h->gcells32);
+        cudaFree(h->gcells64);
+        cudaFree(h->nuclei_u);
+    }
+    h->keep.reset();                // shared copies: freed with the last handle
     cudaFree(h->workspace);
     cudaFree(h->counters);
     if (h->mail_h) cudaFreeHost(h->mail_h);

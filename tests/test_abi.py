@@ -87,4 +87,6 @@ def test_grid_argument_errors_without_gpu(lib_path):
     assert lib.qmmm_field_create_grid(org, 0.3, n, qp, None, None, 0, 8, None) == 1
     assert out.value is None
     assert lib.qmmm_field_set_layout(None, 0) == 1
+    assert lib.qmmm_field_share(None, 8, ctypes.byref(out)) == 1
+    assert lib.qmmm_field_eval_energy(None, None, 1, 1, None, 0, None) == 1
     assert lib.qmmm_field_get_grid_info(None, None) == 1

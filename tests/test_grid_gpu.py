@@ -413,3 +413,45 @@ def test_random_grids_plans_and_precisions(torch_cuda, B, oracle_mod):
                 assert np.all(eE <= tol * np.maximum(1.0, kE)), f"{msg}: E rel err {eE.max():.3e}"
         finally:
             B.qmmm_field_destroy(hnd)
+
+
+# ------------------------------------------------- shared handles
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_shared_handles_on_concurrent_streams(torch_cuda, B, precision):
+    """qmmm_field_share: two handles on one environment (shared packed sources, own
+    workspaces) evaluate different point sets concurrently on two streams; results are bitwise
+    those of one handle used sequentially, also after the parent has been destroyed."""
+    torch = torch_cuda
+    w = make_workload(1)
+    rng = np.random.default_rng(8)
+    pa = rng.normal(size=(48, 3)) * 0.8
+    pb = rng.normal(size=(200, 3)) * 0.8
+    parent = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 48)
+    child = B.qmmm_field_share(parent, 200)
+    try:
+        Va, Ea = run(torch, B, parent, pa, precision)
+        gi_p, gi_c = B.qmmm_field_get_grid_info(parent), B.qmmm_field_get_grid_info(child)
+        assert gi_c["present"] == gi_p["present"] and gi_c["n"] == gi_p["n"]
+        Vb, Eb = run(torch, B, child, pb, precision)
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        da, db = torch.from_numpy(pa).cuda(), torch.from_numpy(pb).cuda()
+        oa = (torch.zeros(48, dtype=torch.float64, device="cuda"), torch.zeros((48, 3), dtype=torch.float64, device="cuda"))
+        ob = (torch.zeros(200, dtype=torch.float64, device="cuda"), torch.zeros((200, 3), dtype=torch.float64, device="cuda"))
+        torch.cuda.synchronize()
+        for _ in range(60):                      # interleaved launches, no synchronisation
+            B.qmmm_field_eval(parent, da, 1, 48, oa[0], oa[1], precision, s1)
+            B.qmmm_field_eval(child, db, 1, 200, ob[0], ob[1], precision, s2)
+        torch.cuda.synchronize()
+        assert np.array_equal(oa[0].cpu().numpy(), Va) and np.array_equal(oa[1].cpu().numpy(), Ea)
+        assert np.array_equal(ob[0].cpu().numpy(), Vb) and np.array_equal(ob[1].cpu().numpy(), Eb)
+        B.qmmm_field_destroy(parent)             # the child keeps the source copies alive
+        parent = None
+        Vb2, Eb2 = run(torch, B, child, pb, precision)
+        assert np.array_equal(Vb2, Vb) and np.array_equal(Eb2, Eb)
+        hv = np.zeros(1); he = np.zeros((1, 3))  # the child's own move server
+        B.qmmm_field_eval_host(child, np.ascontiguousarray(pb[:1]), 1, 1, hv, he, precision)
+        assert np.all(np.isfinite(hv)) and abs(hv[0] - Vb[0]) <= 1e-5 * abs(Vb[0])
+    finally:
+        if parent is not None:
+            B.qmmm_field_destroy(parent)
+        B.qmmm_field_destroy(child)
