@@ -194,6 +194,8 @@ __global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) 
     constexpr int EPT = L::EPT, NT = L::NT, STAGE_BYTES = L::STAGE_BYTES;
 
     extern __shared__ __align__(128) unsigned char smem[];
+    QMMM_MARK_GT(8);
+    QMMM_MARK(0);
     const int stages = prm.stages;
     unsigned char *ptr = smem + static_cast<size_t>(stages) * STAGE_BYTES;
     uint64_t *full = reinterpret_cast<uint64_t *>(ptr);
@@ -252,6 +254,7 @@ __global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) 
         on_lattice(u, prm.g_n[comp], lat_s[i], dd_all[i]);
     }
     __syncthreads();
+    QMMM_MARK(1);
 
     const int wp = warp % WP, ws = warp / WP;
     const int ZL = GRID_ZS / WS, z0 = ws * ZL;       // this warp's z run inside every gchunk
@@ -301,6 +304,7 @@ __global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) 
     int tile = lo / segs, seg = lo - tile * segs;
     int ix = (tile * 32 + lane) / ny, iy = tile * 32 + lane - ix * ny;
 
+    QMMM_MARK(2);
     int slot = 0, pending = 0;
     uint32_t phase = 0;
     for (int g = lo; g < hi; ++g) {
@@ -353,6 +357,7 @@ __global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) 
         }
     }
     if (pending) flush();
+    QMMM_MARK(3);
     // the cells were seen from the lattice point a = u - dd: V(u) = V(a) - E(a) . dd, applied to
     // this thread's FP64 sums (before the nuclei, which are evaluated at u itself)
 #pragma unroll
@@ -381,6 +386,7 @@ __global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) 
         }
     }
 
+    QMMM_MARK(4);
     // ---- in-CTA reduction through shared memory, as in pair_kernel_f32x2 ----------------------
     double *red = reinterpret_cast<double *>(acc);   // reused after the barrier: [NW][EPT*4]
     double2 tot = make_double2(0.0, 0.0);
@@ -408,7 +414,10 @@ __global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) 
             prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] =
                 a * ((lane & 3) ? prm.g_scaleE : prm.g_scaleV);
     }
+    QMMM_MARK(5);
     finish_point_block<NT>(prm, WP * EPT, threadIdx.x, flag, red, [] { __syncthreads(); }, prm.seq);
+    QMMM_MARK(6);
+    QMMM_MARK_GT(9);
 }
 
 // ----------------------------------------------------------------------------- FP64
