@@ -279,6 +279,21 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                     e1.record(stream)
                     torch.cuda.synchronize()
                     row["us_per_eval_1000_back_to_back"] = e0.elapsed_time(e1) * 1e3 / len(walk)
+                    # (i') the same 1,000 launches captured once in a CUDA graph and replayed: no
+                    # host launch cost per evaluation (the Python / ctypes call is ~12 us)
+                    gr = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(gr):
+                        for p in walk:
+                            B.qmmm_field_eval(h, p, 1, 1, V, E, prec)
+                    gr.replay()
+                    torch.cuda.synchronize()
+                    cs = torch.cuda.current_stream()
+                    e0.record(cs)
+                    gr.replay()
+                    e1.record(cs)
+                    torch.cuda.synchronize()
+                    row["us_per_eval_1000_cuda_graph"] = e0.elapsed_time(e1) * 1e3 / len(walk)
+                    del gr
                     # (ii) the QMC loop of PAPER.md:117: r_new in (24 B), U out (32 B), every move;
                     # the loop itself runs inside the library (qmmm_field_eval_moves_host)
                     hp = np.ascontiguousarray(w.elec_xyz.reshape(-1, 3))
@@ -289,6 +304,7 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                     bytes_eval = w.M * (16 if prec == "fp32" else 32)
                     row["source_bytes_per_eval"] = bytes_eval
                     row["source_GBps_back_to_back"] = bytes_eval / (row["us_per_eval_1000_back_to_back"] * 1e-6) / 1e9
+                    row["source_GBps_cuda_graph"] = bytes_eval / (row["us_per_eval_1000_cuda_graph"] * 1e-6) / 1e9
                 out.append(row)
                 if prec == "fp64" and not w.sequential and idx in (1, 4):
                     # potential only (E = NULL): the paper's own computation, Eq. 4; 13 (list) or

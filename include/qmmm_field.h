@@ -82,7 +82,7 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
  *   E         DEVICE [W*N][3] FP64    out: field; NULL = potential only
  *   prec      qmmm_precision
  *   stream    cudaStream_t (as void*); all work is enqueued on it, the call never
- *             synchronises.  One eval in flight per handle (its workspace); for concurrent
+ *             synchronises or allocates, so it may be captured into a CUDA graph.  One eval in flight per handle (its workspace); for concurrent
  *             streams or host threads use qmmm_field_share.
  * Errors: INVALID_ARG (NULL handle/elec_xyz/V, W*N < 1 or > max_points, bad prec),
  * CUDA (launch failure).  Outputs are unspecified after an error.

@@ -455,3 +455,51 @@ def test_shared_handles_on_concurrent_streams(torch_cuda, B, precision):
         if parent is not None:
             B.qmmm_field_destroy(parent)
         B.qmmm_field_destroy(child)
+
+
+# ----------------------------------------------------------------------- CUDA graphs
+@pytest.mark.parametrize("layout,precision", [("grid", "fp32"), ("grid", "fp64"), ("list", "fp32"), ("list", "fp64")])
+def test_eval_is_cuda_graph_capturable(torch_cuda, B, layout, precision):
+    """qmmm_field_eval only enqueues work on the caller's stream (no allocation, no
+    synchronisation), so a sequence of evaluations can be captured into a CUDA graph and
+    replayed; the replay gives bitwise the eager results, also after the inputs change."""
+    torch = torch_cuda
+    w = make_workload(1)
+    rng = np.random.default_rng(4)
+    P = 32
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, P)
+    try:
+        B.qmmm_field_set_layout(h, layout)
+        pts = [torch.from_numpy(rng.normal(size=(P, 3)) * 0.8).cuda() for _ in range(3)]
+        outs = [(torch.zeros(P, dtype=torch.float64, device="cuda"),
+                 torch.zeros((P, 3), dtype=torch.float64, device="cuda")) for _ in range(3)]
+        eager = []
+        for p in pts:                                   # eager reference (also warms up)
+            V = torch.zeros(P, dtype=torch.float64, device="cuda")
+            E = torch.zeros((P, 3), dtype=torch.float64, device="cuda")
+            B.qmmm_field_eval(h, p, 1, P, V, E, precision)
+            torch.cuda.synchronize()
+            eager.append((V.cpu().numpy(), E.cpu().numpy()))
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            for p, (V, E) in zip(pts, outs):
+                B.qmmm_field_eval(h, p, 1, P, V, E, precision)      # current (capturing) stream
+        for rep in range(3):
+            for V, E in outs:
+                V.zero_(); E.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            for (V, E), (Ve, Ee) in zip(outs, eager):
+                assert np.array_equal(V.cpu().numpy(), Ve) and np.array_equal(E.cpu().numpy(), Ee)
+        # new positions in the same buffers: the graph re-reads them
+        new = torch.from_numpy(rng.normal(size=(P, 3)) * 0.8).cuda()
+        Vn = torch.zeros(P, dtype=torch.float64, device="cuda"); En = torch.zeros((P, 3), dtype=torch.float64, device="cuda")
+        B.qmmm_field_eval(h, new, 1, P, Vn, En, precision)
+        torch.cuda.synchronize()
+        pts[1].copy_(new)
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(outs[1][0].cpu().numpy(), Vn.cpu().numpy())
+        assert np.array_equal(outs[1][1].cpu().numpy(), En.cpu().numpy())
+    finally:
+        B.qmmm_field_destroy(h)
