@@ -52,7 +52,7 @@ typedef enum {
  * everything around it in double).  I/O is FP64 in both modes.
  *   QMMM_FP64       : FP64 throughout (rel. error <= 1e-12 on V and E).
  *   QMMM_FP32_ACC64 : cell sources in FP32 arithmetic (MUFU rsqrt + one Newton
- *                     step), running sums in FP64; nuclei always FP64
+ *                     step, applied to the sum), running sums in FP64; nuclei always FP64
  *                     (per-point rel. error <= 1e-5, energy within 1e-5 hartree). */
 typedef enum { QMMM_FP64 = 0, QMMM_FP32_ACC64 = 1 } qmmm_precision;
 
@@ -141,8 +141,8 @@ qmmm_status qmmm_field_eval_moves_host(qmmm_field *h, const double *elec_xyz_hos
  *     R(ix, iy, iz) = origin + spacing * (ix, iy, iz),   0 <= i_k < n[k]   (cubic cells)
  * the library keeps a second copy that stores only the charges (4 B FP32 / 8 B FP64 per cell
  * instead of 16 / 32 B) and regenerates the coordinates from the indices.  Its kernels walk
- * the z rows of the grid, where dx, dy and dx^2 + dy^2 are row constants: 12 FP32 (13 FP64)
- * lane operations per pair instead of 17 (18).  Same V and E as the list kernels up to
+ * the z rows of the grid, where dx, dy and dx^2 + dy^2 are row constants: 9 FP32 (13 FP64)
+ * lane operations per pair instead of 14 (18).  Same V and E as the list kernels up to
  * rounding (FP64: node coordinates are origin + i*spacing, within 16 ulp of the listed
  * positions; tolerances as for the list).  Empty (masked) cells are zero charges.
  *

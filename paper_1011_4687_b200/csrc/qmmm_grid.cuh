@@ -12,9 +12,9 @@
 //     r^2  = (dx^2 + dy^2) + dz^2                       1 add (dz) + 1 fma per pair
 //     Ex  += dx * sum_k s_k,  Ey += dy * sum_k s_k      1 add per pair (sum s), not 2 fma
 //     Ez  += sum_k s_k dz_k                             1 fma per pair
-// which leaves 12 FP32 (13 FP64) lane operations per pair instead of 17 (18) for a source
-// list: dz, r^2, the 4 (5) refinement operations, p = q y, V += p,
-// y^2, s = p y^2, sum s, sum s dz.  (FP32: one of the 12, y0 / 2, runs on the integer pipe.)
+// which, with the Newton step applied to the sum (GridRowF32 below), leaves 9 FP32 lane
+// operations per pair instead of 14 for a source list, and 13 FP64 instead of 18
+// (DESIGN.md section 5b).
 //
 // Work unit ("gchunk"): 32 rows x ZS = 64 consecutive z nodes, stored [ZS/4][32][4] (FP32) or
 // [ZS/2][32][2] (FP64) so that a lane's 128-bit shared-memory loads are conflict-free.  One
