@@ -489,12 +489,12 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
     for (int e = 0; e < EPT; ++e) V[e] = Ex[e] = Ey[e] = Ez[e] = 0.0;
 
     const int ZL = GRID_ZS / WS, z0 = ws * ZL;       // this warp's z run inside every gchunk
+    // (tile, seg) of gchunk g = tile * segs + seg, and the lane's row (ix, iy) of that tile
+    const int segs = prm.g_segs, ny = prm.g_n[1];
+    int tile = lo / segs, seg = lo - tile * segs;
+    int ix = (tile * 32 + lane) / ny, iy = tile * 32 + lane - ix * ny;
     for (int k = 0; k < nk; ++k) {
-        const int g = lo + k;
-        const int tile = g / prm.g_segs, seg = g - tile * prm.g_segs;
-        const int row = tile * 32 + lane;
-        const int ix = row / prm.g_n[1];
-        const double fx = static_cast<double>(ix), fy = static_cast<double>(row - ix * prm.g_n[1]);
+        const double fx = static_cast<double>(ix), fy = static_cast<double>(iy);
         const double fz = static_cast<double>(seg * GRID_ZS + z0);
         double dx[EPT], dy[EPT], rxy2[EPT], azb[EPT], S[EPT], SZ[EPT];
 #pragma unroll
@@ -543,6 +543,17 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
                 Ex[e] = fma(dx[e], S[e], Ex[e]);
                 Ey[e] = fma(dy[e], S[e], Ey[e]);
                 Ez[e] += SZ[e];
+            }
+        }
+        if (++seg == segs) {               // next row tile
+            seg = 0;
+            ++tile;
+            iy += 32;
+            if (ny >= 32) {
+                if (iy >= ny) { iy -= ny; ++ix; }
+            } else {
+                ix = (tile * 32 + lane) / ny;
+                iy = tile * 32 + lane - ix * ny;
             }
         }
     }
