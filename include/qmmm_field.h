@@ -115,7 +115,8 @@ qmmm_status qmmm_field_eval_energy(qmmm_field *h, const double *elec_xyz, int64_
  *   W*N <= 64 : one kernel launch on `stream`; points read from and results written to a
  *               pinned, device-mapped mailbox, completion signalled by a sequence number.
  *   otherwise : host->device copy, kernel, device->host copy on `stream`, synchronisation.
- * All three give bitwise the result of qmmm_field_eval with the same plan.
+ * All three give bitwise the result of qmmm_field_eval with the same plan and layout (the
+ * move server always reads the source list: layout LIST).
  * Same argument meaning and errors as qmmm_field_eval.
  */
 qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int64_t W,

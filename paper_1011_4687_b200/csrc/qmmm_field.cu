@@ -84,10 +84,18 @@ constexpr int GRID_NW_EPT8 = 8, GRID_NW_EPT4 = QMMM_GRID_NW_EPT4, GRID_NW_EPT2 =
 #endif
 constexpr int GRID64_NW_EPT4 = 8, GRID64_NW_EPT2 = 16, GRID64_NW_EPT1 = 16;
 int grid_f64_warps(int ept) { return ept == 4 ? GRID64_NW_EPT4 : (ept == 2 ? GRID64_NW_EPT2 : GRID64_NW_EPT1); }
-int grid_f32_warps(int ept) { return ept == 8 ? GRID_NW_EPT8 : (ept == 4 ? GRID_NW_EPT4 : GRID_NW_EPT2); }
-size_t grid_smem_bytes(bool f32, int stages, int ept, int wp) {
+// one or two points per evaluation: the node-packed kernel, 8 warps, two CTAs per SM
+constexpr int GRID_NW_NODEPACK = 8;
+bool grid_f32_nodepack(int ept, int64_t P) { return ept == 2 && P <= 2; }
+int grid_f32_warps(int ept, int64_t P) {
+    if (grid_f32_nodepack(ept, P)) return GRID_NW_NODEPACK;
+    return ept == 8 ? GRID_NW_EPT8 : (ept == 4 ? GRID_NW_EPT4 : GRID_NW_EPT2);
+}
+size_t grid_smem_bytes(bool f32, int stages, int ept, int wp, int64_t P) {
     if (f32 && ept == 8) return GridF32Layout<4, GRID_NW_EPT8>::total(stages);
     if (f32 && ept == 4) return GridF32Layout<2, GRID_NW_EPT4>::total(stages);
+    if (f32 && grid_f32_nodepack(ept, P))       // warp-private pipelines: two slots per warp
+        return GridF32Layout<1, GRID_NW_NODEPACK>::total(2 * GRID_NW_NODEPACK);
     if (f32) return GridF32Layout<1, GRID_NW_EPT2>::total(stages);
     return static_cast<size_t>(stages) * GRID_STAGE_BYTES_F64 + 18 * sizeof(uint64_t) +
            static_cast<size_t>(32) * grid_f64_warps(ept) * sizeof(double) +
@@ -160,7 +168,7 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32, bool grid = fals
     pl.points_per_thread = std::min(pl.points_per_thread, max_ept);
     if (grid && f32) pl.points_per_thread = std::max(pl.points_per_thread, 2);   // packed pairs only
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
-    const int nw = grid ? (f32 ? grid_f32_warps(pl.points_per_thread) : grid_f64_warps(pl.points_per_thread))
+    const int nw = grid ? (f32 ? grid_f32_warps(pl.points_per_thread, P) : grid_f64_warps(pl.points_per_thread))
                         : ((f32 && pl.points_per_thread >= 2) ? f32x2_warps(pl.points_per_thread) : COMPUTE_WARPS);
     if (pl.point_warps == 0) {
         // as many point warps as there are groups, but keep at least 4 point blocks when the
@@ -192,6 +200,10 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32, bool grid = fals
         if (!grid) pl.stages = f32 ? (pl.points_per_thread == 1 ? 6 : 4) : (bandwidth_bound ? 6 : 3);
     }
     if (grid && pl.stages == 0) pl.stages = 4;             // one gchunk (8 / 16 KB) per stage
+    if (grid && f32 && grid_f32_nodepack(pl.points_per_thread, P)) {
+        pl.point_warps = 1;                                // every warp walks whole gchunks of its own
+        pl.stages = 2;                                     // two private slots per warp
+    }
     return pl;
 }
 
@@ -203,8 +215,10 @@ bool auto_uses_grid(const qmmm_field *h, int64_t P, bool f32) {
     if (!h->has_grid) return false;
     if (!h->has_list) return true;
     const qmmm_plan pl = choose_plan(h, P, f32, true);
-    const int nw = f32 ? grid_f32_warps(pl.points_per_thread) : grid_f64_warps(pl.points_per_thread);
-    return nw / pl.point_warps <= 4 && h->n_g >= static_cast<int64_t>(2) * pl.slices;
+    if (h->n_g < static_cast<int64_t>(2) * pl.slices) return false;
+    if (f32 && grid_f32_nodepack(pl.points_per_thread, P)) return true;     // single-point walk
+    const int nw = f32 ? grid_f32_warps(pl.points_per_thread, P) : grid_f64_warps(pl.points_per_thread);
+    return nw / pl.point_warps <= 4;
 }
 
 template <typename REAL, int EPT, bool WITH_E = true>
@@ -262,9 +276,9 @@ cudaError_t launch_pair_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
     return cudaErrorInvalidValue;
 }
 
-template <int EP2, int NW>
+template <int EP2, int NW, bool NODEPACK = false>
 cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
-    auto kern = grid_kernel_f32x2<EP2, NW>;
+    auto kern = grid_kernel_f32x2<EP2, NW, NODEPACK>;
     static thread_local size_t configured = 0;
     if (smem > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -293,7 +307,9 @@ cudaError_t launch_grid_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
                             cudaStream_t st) {
     if (f32) {
         switch (ept) {
-            case 2: return launch_grid_f32<1, GRID_NW_EPT2>(prm, grid, smem, st);
+            case 2:
+                if (grid_f32_nodepack(2, prm.P)) return launch_grid_f32<1, GRID_NW_NODEPACK, true>(prm, grid, smem, st);
+                return launch_grid_f32<1, GRID_NW_EPT2>(prm, grid, smem, st);
             case 4: return launch_grid_f32<2, GRID_NW_EPT4>(prm, grid, smem, st);
             case 8: return launch_grid_f32<4, GRID_NW_EPT8>(prm, grid, smem, st);
         }
@@ -1017,7 +1033,7 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
     const int pb = static_cast<int>((groups + pl.point_warps - 1) / pl.point_warps);
     int launches = 0;
     auto smem_of = [&](int stages) {
-        return grid ? grid_smem_bytes(f32, stages, pl.points_per_thread, pl.point_warps)
+        return grid ? grid_smem_bytes(f32, stages, pl.points_per_thread, pl.point_warps, P)
                     : pair_smem_bytes(f32, stages, pl.points_per_thread, pl.point_warps);
     };
     size_t smem = smem_of(pl.stages);

@@ -178,6 +178,86 @@ struct GridRowF32 {
     }
 };
 
+// The same walk for ONE evaluation point (single-electron moves): the two
+// halves of a register pair hold two consecutive z NODES instead of two points, so the
+// packed instructions stay full with a single point.  Two chains (4 nodes = one 128-bit
+// charge load) x two register sets; same 9 operations per pair.  The halves are added at
+// the end of the run.
+struct GridRowF32N {
+    float2 dzA[2], r2A[2], y0A[2], dzB[2], r2B[2], y0B[2];
+    float2 rxy2, S, SZ;
+
+    __device__ __forceinline__ void start(float azb, float rxy2s) {
+        rxy2 = bc(rxy2s);
+        S = SZ = f2(0.0f, 0.0f);
+        dzA[0] = f2(azb, azb - 1.0f);                  // exact (lattice)
+        dzA[1] = f2(azb - 2.0f, azb - 3.0f);
+#pragma unroll
+        for (int e = 0; e < 2; ++e) r2A[e] = __ffma2_rn(dzA[e], dzA[e], rxy2);
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            y0A[e].x = rsqrt_mufu_f32(r2A[e].x);
+            y0A[e].y = rsqrt_mufu_f32(r2A[e].y);
+        }
+    }
+    __device__ __forceinline__ void step(const float2 (&dzc)[2], float2 (&dzn)[2], float2 (&r2n)[2],
+                                         float2 (&y0n)[2]) {
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            dzn[e] = __fadd2_rn(dzc[e], bc(-4.0f));
+            r2n[e] = __ffma2_rn(dzn[e], dzn[e], rxy2);
+        }
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            y0n[e].x = rsqrt_mufu_f32(r2n[e].x);
+            y0n[e].y = rsqrt_mufu_f32(r2n[e].y);
+        }
+    }
+    __device__ __forceinline__ void acc(const float2 (&dz)[2], const float2 (&r2)[2],
+                                        const float2 (&y0)[2], const float *q4, float2 &Vc,
+                                        float2 &Tc, bool first) {
+        const float4 Q = *reinterpret_cast<const float4 *>(q4);
+        const float2 q[2] = {f2(Q.x, Q.y), f2(Q.z, Q.w)};
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const float2 a = __fmul2_rn(y0[e], q[e]);
+            const float2 c = __fmul2_rn(a, __fmul2_rn(y0[e], y0[e]));
+            if (first && e == 0) {
+                Vc = a;
+                Tc = __fmul2_rn(c, r2[e]);
+            } else {
+                Vc = __fadd2_rn(Vc, a);
+                Tc = __ffma2_rn(c, r2[e], Tc);
+            }
+            S = __fadd2_rn(S, c);
+            SZ = __ffma2_rn(c, dz[e], SZ);
+        }
+    }
+    // n4 * 4 nodes starting at b; v, t receive the sums of V0 and T (both halves added)
+    __device__ __forceinline__ void run(const float *b, int n4, float &v, float &t) {
+        float2 vs = f2(0.0f, 0.0f), ts = f2(0.0f, 0.0f);
+        int k4 = 0;
+#pragma unroll 1
+        for (; k4 + 1 < n4; k4 += 2) {               // 8 nodes: sets A then B
+            float2 Vc, Tc;
+            step(dzA, dzB, r2B, y0B);
+            acc(dzA, r2A, y0A, b + k4 * 128, Vc, Tc, true);
+            step(dzB, dzA, r2A, y0A);                 // the last one looks past the run: unused
+            acc(dzB, r2B, y0B, b + (k4 + 1) * 128, Vc, Tc, false);
+            vs = __fadd2_rn(vs, Vc);
+            ts = __fadd2_rn(ts, Tc);
+        }
+        if (k4 < n4) {                                // odd tail: 4 nodes
+            float2 Vc, Tc;
+            acc(dzA, r2A, y0A, b + k4 * 128, Vc, Tc, true);
+            vs = __fadd2_rn(vs, Vc);
+            ts = __fadd2_rn(ts, Tc);
+        }
+        v = vs.x + vs.y;
+        t = ts.x + ts.y;
+    }
+};
+
 // grid = (point_blocks, slices); EPT = 2 * EP2 points per thread; NW warps (8 x 8 points or
 // 16 x 4 points), warp 0 drives the TMA ring inline (a producer warp would cost registers).
 // A pipeline stage is one gchunk, consumed by all warps: the WP point warps own different
@@ -188,17 +268,22 @@ struct GridRowF32 {
 // prm.nuc = nuclei in grid units; prm.elec in bohr (converted to grid units when staged).
 constexpr int GRID_FLUSH = 4;                       // gchunks per FP32 -> FP64 flush
 
-template <int EP2, int NW>
-__global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) grid_kernel_f32x2(const PairParams prm) {
+// NODEPACK (EP2 = 1 only): each of the thread's two points is walked on its own with two NODES
+// per register pair (GridRowF32N); a second point beyond P is skipped.  For one or two points
+// per evaluation.
+template <int EP2, int NW, bool NODEPACK = false>
+__global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 16 / NW : 1) grid_kernel_f32x2(const PairParams prm) {
+    static_assert(!NODEPACK || EP2 == 1, "node packing walks single points");
     using L = GridF32Layout<EP2, NW>;
     constexpr int EPT = L::EPT, NT = L::NT, STAGE_BYTES = L::STAGE_BYTES;
 
     extern __shared__ __align__(128) unsigned char smem[];
     QMMM_MARK_GT(8);
     QMMM_MARK(0);
-    const int stages = prm.stages;
+    // NODEPACK: warp-private pipelines, two slots per warp (prm.stages is not used)
+    const int stages = NODEPACK ? 2 * NW : prm.stages;
     unsigned char *ptr = smem + static_cast<size_t>(stages) * STAGE_BYTES;
-    uint64_t *full = reinterpret_cast<uint64_t *>(ptr);
+    uint64_t *full = reinterpret_cast<uint64_t *>(ptr);        // NODEPACK: 16 full barriers
     uint64_t *empty = full + 8;
     int *flag = reinterpret_cast<int *>(empty + 8);
     ptr += L::BAR_BYTES;
@@ -209,17 +294,10 @@ __global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) 
     double2 *acc = reinterpret_cast<double2 *>(ptr);           // [EPT*2][NT] double2
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int WP = prm.point_warps, WS = NW / WP;
+    const int WP = NODEPACK ? 1 : prm.point_warps, WS = NW / WP;
     int lo, hi;
     slice_range(prm.n_chunks, prm.slices, blockIdx.y, lo, hi);
 
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < stages; ++s) {
-            mbar_init(&full[s], 1);
-            mbar_init(&empty[s], NW);
-        }
-        fence_barrier_init();
-    }
     // ---- producer cursor (warp 0 only): next gchunk to load ---------------------------------
     int pc = lo, pslot = 0;
     uint32_t pphase = 0;
@@ -239,9 +317,34 @@ __global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) 
             pwrapped = true;
         }
     };
-    if (warp == 0) {
+    // NODEPACK: warp w walks gchunks lo + w, lo + w + NW, ... whole (all 64 z nodes) and loads
+    // them itself into its own two slots: no waiting on other warps anywhere in the loop
+    auto load_own = [&](int g, int sl) {           // lane 0 of the owning warp
+        mbar_expect_tx(&full[sl], STAGE_BYTES);
+        tma_bulk_g2s(smem + static_cast<size_t>(sl) * STAGE_BYTES,
+                     prm.chunks + static_cast<size_t>(g) * STAGE_BYTES, STAGE_BYTES, &full[sl]);
+    };
+    if constexpr (NODEPACK) {
+        if (lane == 0) {
+            mbar_init(&full[2 * warp], 1);
+            mbar_init(&full[2 * warp + 1], 1);
+            fence_barrier_init();
+            for (int i = 0; i < 2; ++i)
+                if (lo + warp + i * NW < hi) load_own(lo + warp + i * NW, 2 * warp + i);
+        }
         __syncwarp();
-        for (int i = 0; i < stages - 1; ++i) produce();
+    } else {
+        if (threadIdx.x == 0) {
+            for (int s = 0; s < stages; ++s) {
+                mbar_init(&full[s], 1);
+                mbar_init(&empty[s], NW);
+            }
+            fence_barrier_init();
+        }
+        if (warp == 0) {
+            __syncwarp();
+            for (int i = 0; i < stages - 1; ++i) produce();
+        }
     }
     const int ppb = WP * EPT;
     float *dd_all = lat_s + NW * EPT * 3;
@@ -305,7 +408,47 @@ __global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) 
     int ix = (tile * 32 + lane) / ny, iy = tile * 32 + lane - ix * ny;
 
     QMMM_MARK(2);
-    int slot = 0, pending = 0;
+    int pending = 0;
+    if constexpr (NODEPACK) {
+        // one point at a time, two NODES per register pair, whole gchunks per warp
+        const bool second = blockIdx.x * ppb + 1 < prm.P;
+        int it = 0;
+        for (int g = lo + warp; g < hi; g += NW, ++it) {
+            const int sl = 2 * warp + (it & 1);
+            const int tl = g / segs, sg = g - tl * segs;
+            const int rw = tl * 32 + lane, rx = rw / ny;
+            const float fxs = static_cast<float>(rx), fys = static_cast<float>(rw - rx * ny);
+            const float fzs = static_cast<float>(sg * GRID_ZS);
+            mbar_wait(&full[sl], (it >> 1) & 1);
+            const float *data = reinterpret_cast<const float *>(smem + static_cast<size_t>(sl) * STAGE_BYTES);
+            auto one_point = [&](float axs, float ays, float azs, float &vvc, float &ttc, float &exc,
+                                 float &eyc, float &ezc) {
+                const float dxs = axs - fxs, dys = ays - fys;         // exact (lattice)
+                GridRowF32N row;
+                row.start(azs - fzs, fmaf(dys, dys, fmaf(dxs, dxs, 1e-30f)));
+                float v1, t1;
+                row.run(data + 4 * lane, GRID_ZS / 4, v1, t1);
+                const float s1 = row.S.x + row.S.y;
+                vvc += v1;
+                ttc += t1;
+                exc = fmaf(dxs, s1, exc);
+                eyc = fmaf(dys, s1, eyc);
+                ezc += row.SZ.x + row.SZ.y;
+            };
+            one_point(ax[0].x, ay[0].x, az[0].x, vv[0].x, tt[0].x, ex[0].x, ey[0].x, ez[0].x);
+            if (second) one_point(ax[0].y, ay[0].y, az[0].y, vv[0].y, tt[0].y, ex[0].y, ey[0].y, ez[0].y);
+            __syncwarp();                          // every lane has read the slot
+            if (lane == 0 && g + 2 * NW < hi) {    // refill it with the gchunk after next
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                load_own(g + 2 * NW, sl);
+            }
+            if (++pending == GRID_FLUSH) {
+                flush();
+                pending = 0;
+            }
+        }
+    } else {
+    int slot = 0;
     uint32_t phase = 0;
     for (int g = lo; g < hi; ++g) {
         if (warp == 0) produce();          // gchunk g + stages - 1 into the slot freed by g - 1
@@ -355,6 +498,7 @@ __global__ void __launch_bounds__(32 * NW, (NW <= 8 && EP2 <= 2) ? 16 / NW : 1) 
                 iy = tile * 32 + lane - ix * ny;
             }
         }
+    }
     }
     if (pending) flush();
     QMMM_MARK(3);

@@ -333,8 +333,12 @@ def test_move_server_bitwise_equals_launch_path_and_survives_idle_and_switches(t
     h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 4)
     try:
         ref = {}
+        # the move server reads the source LIST: its launch-path twin is eval with that layout
+        # (AUTO sends single-point FP32 device evaluations to the grid kernel)
+        B.qmmm_field_set_layout(h, "list")
         for prec in ("fp64", "fp32"):
             ref[prec] = [gpu_eval(torch_cuda, B, w, pts[i:i + 1], prec, handle=h) for i in range(len(pts))]
+        B.qmmm_field_set_layout(h, "auto")
         order = ["fp64", "fp64", "fp32", "fp64", "fp32", "fp32"] * 2
         for i, prec in enumerate(order):
             V = np.full(1, np.nan); E = np.full((1, 3), np.nan)
