@@ -301,7 +301,11 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                     B.qmmm_field_eval_moves_host(h, hp[:50], 50, 1, hV, hE, prec, stream)
                     secs = B.qmmm_field_eval_moves_host(h, hp, len(hp), 1, hV, hE, prec, stream)
                     row["us_per_eval_host_loop"] = secs * 1e6 / len(hp)
-                    bytes_eval = w.M * (16 if prec == "fp32" else 32)
+                    if layout == "grid":        # charges only, empty cells included
+                        gi = B.qmmm_field_get_grid_info(h)
+                        bytes_eval = gi["bytes_fp32" if prec == "fp32" else "bytes_fp64"]
+                    else:
+                        bytes_eval = w.M * (16 if prec == "fp32" else 32)
                     row["source_bytes_per_eval"] = bytes_eval
                     row["source_GBps_back_to_back"] = bytes_eval / (row["us_per_eval_1000_back_to_back"] * 1e-6) / 1e9
                     row["source_GBps_cuda_graph"] = bytes_eval / (row["us_per_eval_1000_cuda_graph"] * 1e-6) / 1e9

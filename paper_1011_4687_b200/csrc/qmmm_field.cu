@@ -83,7 +83,13 @@ constexpr int GRID_NW_EPT8 = 8, GRID_NW_EPT4 = QMMM_GRID_NW_EPT4, GRID_NW_EPT2 =
 #define QMMM_GRID_F64_MAXEPT 4
 #endif
 constexpr int GRID64_NW_EPT4 = 8, GRID64_NW_EPT2 = 16, GRID64_NW_EPT1 = 16;
-int grid_f64_warps(int ept) { return ept == 4 ? GRID64_NW_EPT4 : (ept == 2 ? GRID64_NW_EPT2 : GRID64_NW_EPT1); }
+// a handful of points (one point group): every warp loads and walks whole gchunks of its own
+constexpr int GRID64_NW_WARPOWN = 8;
+bool grid_f64_warpown(int ept, int64_t P) { return P <= ept; }
+int grid_f64_warps(int ept, int64_t P) {
+    if (grid_f64_warpown(ept, P)) return GRID64_NW_WARPOWN;
+    return ept == 4 ? GRID64_NW_EPT4 : (ept == 2 ? GRID64_NW_EPT2 : GRID64_NW_EPT1);
+}
 // one or two points per evaluation: the node-packed kernel, 8 warps, two CTAs per SM
 constexpr int GRID_NW_NODEPACK = 8;
 bool grid_f32_nodepack(int ept, int64_t P) { return ept == 2 && P <= 2; }
@@ -97,8 +103,9 @@ size_t grid_smem_bytes(bool f32, int stages, int ept, int wp, int64_t P) {
     if (f32 && grid_f32_nodepack(ept, P))       // warp-private pipelines: two slots per warp
         return GridF32Layout<1, GRID_NW_NODEPACK>::total(2 * GRID_NW_NODEPACK);
     if (f32) return GridF32Layout<1, GRID_NW_EPT2>::total(stages);
+    if (grid_f64_warpown(ept, P)) stages = GRID64_NW_WARPOWN;      // one private slot per warp
     return static_cast<size_t>(stages) * GRID_STAGE_BYTES_F64 + 18 * sizeof(uint64_t) +
-           static_cast<size_t>(32) * grid_f64_warps(ept) * sizeof(double) +
+           static_cast<size_t>(32) * grid_f64_warps(ept, P) * sizeof(double) +
            static_cast<size_t>(wp) * ept * 3 * sizeof(double);
 }
 
@@ -168,7 +175,7 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32, bool grid = fals
     pl.points_per_thread = std::min(pl.points_per_thread, max_ept);
     if (grid && f32) pl.points_per_thread = std::max(pl.points_per_thread, 2);   // packed pairs only
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
-    const int nw = grid ? (f32 ? grid_f32_warps(pl.points_per_thread, P) : grid_f64_warps(pl.points_per_thread))
+    const int nw = grid ? (f32 ? grid_f32_warps(pl.points_per_thread, P) : grid_f64_warps(pl.points_per_thread, P))
                         : ((f32 && pl.points_per_thread >= 2) ? f32x2_warps(pl.points_per_thread) : COMPUTE_WARPS);
     if (pl.point_warps == 0) {
         // as many point warps as there are groups, but keep at least 4 point blocks when the
@@ -204,6 +211,10 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32, bool grid = fals
         pl.point_warps = 1;                                // every warp walks whole gchunks of its own
         pl.stages = 2;                                     // two private slots per warp
     }
+    if (grid && !f32 && grid_f64_warpown(pl.points_per_thread, P)) {
+        pl.point_warps = 1;
+        pl.stages = 1;                                     // one private slot per warp
+    }
     return pl;
 }
 
@@ -217,7 +228,8 @@ bool auto_uses_grid(const qmmm_field *h, int64_t P, bool f32) {
     const qmmm_plan pl = choose_plan(h, P, f32, true);
     if (h->n_g < static_cast<int64_t>(2) * pl.slices) return false;
     if (f32 && grid_f32_nodepack(pl.points_per_thread, P)) return true;     // single-point walk
-    const int nw = f32 ? grid_f32_warps(pl.points_per_thread, P) : grid_f64_warps(pl.points_per_thread);
+    if (!f32 && grid_f64_warpown(pl.points_per_thread, P)) return true;     // warp-private gchunks
+    const int nw = f32 ? grid_f32_warps(pl.points_per_thread, P) : grid_f64_warps(pl.points_per_thread, P);
     return nw / pl.point_warps <= 4;
 }
 
@@ -289,9 +301,9 @@ cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaS
     kern<<<grid, 32 * NW, smem, st>>>(prm);
     return cudaGetLastError();
 }
-template <int EPT, bool WITH_E, int NW>
+template <int EPT, bool WITH_E, int NW, bool WARPOWN = false>
 cudaError_t launch_grid_f64(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
-    auto kern = grid_kernel_f64<EPT, WITH_E, NW>;
+    auto kern = grid_kernel_f64<EPT, WITH_E, NW, WARPOWN>;
     static thread_local size_t configured = 0;
     if (smem > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -315,15 +327,27 @@ cudaError_t launch_grid_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
         }
     } else if (prm.E) {
         switch (ept) {
-            case 1: return launch_grid_f64<1, true, GRID64_NW_EPT1>(prm, grid, smem, st);
-            case 2: return launch_grid_f64<2, true, GRID64_NW_EPT2>(prm, grid, smem, st);
-            case 4: return launch_grid_f64<4, true, GRID64_NW_EPT4>(prm, grid, smem, st);
+            case 1:
+                if (grid_f64_warpown(1, prm.P)) return launch_grid_f64<1, true, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
+                return launch_grid_f64<1, true, GRID64_NW_EPT1>(prm, grid, smem, st);
+            case 2:
+                if (grid_f64_warpown(2, prm.P)) return launch_grid_f64<2, true, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
+                return launch_grid_f64<2, true, GRID64_NW_EPT2>(prm, grid, smem, st);
+            case 4:
+                if (grid_f64_warpown(4, prm.P)) return launch_grid_f64<4, true, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
+                return launch_grid_f64<4, true, GRID64_NW_EPT4>(prm, grid, smem, st);
         }
     } else {
         switch (ept) {
-            case 1: return launch_grid_f64<1, false, GRID64_NW_EPT1>(prm, grid, smem, st);
-            case 2: return launch_grid_f64<2, false, GRID64_NW_EPT2>(prm, grid, smem, st);
-            case 4: return launch_grid_f64<4, false, GRID64_NW_EPT4>(prm, grid, smem, st);
+            case 1:
+                if (grid_f64_warpown(1, prm.P)) return launch_grid_f64<1, false, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
+                return launch_grid_f64<1, false, GRID64_NW_EPT1>(prm, grid, smem, st);
+            case 2:
+                if (grid_f64_warpown(2, prm.P)) return launch_grid_f64<2, false, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
+                return launch_grid_f64<2, false, GRID64_NW_EPT2>(prm, grid, smem, st);
+            case 4:
+                if (grid_f64_warpown(4, prm.P)) return launch_grid_f64<4, false, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
+                return launch_grid_f64<4, false, GRID64_NW_EPT4>(prm, grid, smem, st);
         }
     }
     return cudaErrorInvalidValue;

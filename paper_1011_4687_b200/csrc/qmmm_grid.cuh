@@ -575,11 +575,14 @@ __device__ __forceinline__ void consumer_sync() {     // named barrier 1: the N 
 }
 
 // NW consumer warps (8 x 4 points or 16 x 2 points) + 1 TMA producer warp.
-template <int EPT, bool WITH_E, int NW>
+// WARPOWN (a handful of points, all owned by every warp): warp w loads and walks whole gchunks
+// lo + w, lo + w + NW, ... by itself (one private slot per warp, no producer warp, no waiting
+// on other warps), as the node-packed FP32 kernel does.
+template <int EPT, bool WITH_E, int NW, bool WARPOWN = false>
 __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairParams prm) {
     constexpr int STAGE_BYTES = GRID_STAGE_BYTES_F64;
     extern __shared__ __align__(128) unsigned char smem[];
-    const int stages = prm.stages;
+    const int stages = WARPOWN ? NW : prm.stages;
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + static_cast<size_t>(stages) * STAGE_BYTES);
     uint64_t *empty = full + 8;
     int *flag = reinterpret_cast<int *>(empty + 8);
@@ -587,12 +590,12 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
     double *elec_s = red + 32 * NW;             // [WP*EPT][3], grid units
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int WP = prm.point_warps, WS = NW / WP;
+    const int WP = WARPOWN ? 1 : prm.point_warps, WS = NW / WP;
     int lo, hi;
     slice_range(prm.n_chunks, prm.slices, blockIdx.y, lo, hi);
     const int nk = hi - lo;
 
-    const bool producer = warp == NW && lane == 0;
+    const bool producer = !WARPOWN && warp == NW && lane == 0;
     int pk = 0;
     auto load_step = [&]() {
         const int slot = pk % stages;
@@ -603,6 +606,11 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
                      &full[slot]);
         ++pk;
     };
+    auto load_own = [&](int g) {                   // WARPOWN: lane 0 of the owning warp
+        mbar_expect_tx(&full[warp], STAGE_BYTES);
+        tma_bulk_g2s(smem + static_cast<size_t>(warp) * STAGE_BYTES,
+                     prm.chunks + static_cast<size_t>(g) * STAGE_BYTES, STAGE_BYTES, &full[warp]);
+    };
     if (producer) {
         for (int s = 0; s < stages; ++s) {
             mbar_init(&full[s], 1);
@@ -610,6 +618,13 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
         }
         fence_barrier_init();
         while (pk < nk && pk < stages) load_step();
+    }
+    if constexpr (WARPOWN) {
+        if (warp < NW && lane == 0) {
+            mbar_init(&full[warp], 1);
+            fence_barrier_init();
+            if (lo + warp < hi) load_own(lo + warp);
+        }
     }
     const int ppb = WP * EPT;
     for (int i = threadIdx.x; i < ppb * 3; i += 32 * (NW + 1)) {
@@ -621,9 +636,11 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
     __syncthreads();
 
     if (warp == NW) {
-        if (lane == 0)
-            while (pk < nk) load_step();
-        return;
+        if constexpr (!WARPOWN) {
+            if (lane == 0)
+                while (pk < nk) load_step();
+        }
+        return;                                    // WARPOWN: the consumer warps load for themselves
     }
 
     const int wp = warp % WP, ws = warp / WP;
@@ -632,14 +649,9 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
 #pragma unroll
     for (int e = 0; e < EPT; ++e) V[e] = Ex[e] = Ey[e] = Ez[e] = 0.0;
 
-    const int ZL = GRID_ZS / WS, z0 = ws * ZL;       // this warp's z run inside every gchunk
-    // (tile, seg) of gchunk g = tile * segs + seg, and the lane's row (ix, iy) of that tile
-    const int segs = prm.g_segs, ny = prm.g_n[1];
-    int tile = lo / segs, seg = lo - tile * segs;
-    int ix = (tile * 32 + lane) / ny, iy = tile * 32 + lane - ix * ny;
-    for (int k = 0; k < nk; ++k) {
-        const double fx = static_cast<double>(ix), fy = static_cast<double>(iy);
-        const double fz = static_cast<double>(seg * GRID_ZS + z0);
+    // one z run (n4 * 4 nodes at b, [k/2][32][2] doubles) of the lane's row (fx, fy), first
+    // node at z = fz, for the thread's EPT points
+    auto walk = [&](const double *b, int n4, double fx, double fy, double fz) {
         double dx[EPT], dy[EPT], rxy2[EPT], azb[EPT], S[EPT], SZ[EPT];
 #pragma unroll
         for (int e = 0; e < EPT; ++e) {
@@ -649,12 +661,8 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
             azb[e] = pe[3 * e + 2] - fz;
             S[e] = SZ[e] = 0.0;
         }
-        const int slot = k % stages;
-        mbar_wait(&full[slot], (k / stages) & 1);
-        const double *b = reinterpret_cast<const double *>(smem + static_cast<size_t>(slot) * STAGE_BYTES) +
-                          (z0 / 2) * 64 + 2 * lane;
 #pragma unroll 1
-        for (int k4 = 0; k4 < ZL / 4; ++k4) {
+        for (int k4 = 0; k4 < n4; ++k4) {
             const double2 Qa = *reinterpret_cast<const double2 *>(b + (2 * k4) * 64);
             const double2 Qb = *reinterpret_cast<const double2 *>(b + (2 * k4 + 1) * 64);
             const double qs[4] = {Qa.x, Qa.y, Qb.x, Qb.y};
@@ -679,8 +687,6 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
 #pragma unroll
             for (int e = 0; e < EPT; ++e) azb[e] -= 4.0;
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[slot]);
         if constexpr (WITH_E) {
 #pragma unroll
             for (int e = 0; e < EPT; ++e) {
@@ -689,15 +695,48 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
                 Ez[e] += SZ[e];
             }
         }
-        if (++seg == segs) {               // next row tile
-            seg = 0;
-            ++tile;
-            iy += 32;
-            if (ny >= 32) {
-                if (iy >= ny) { iy -= ny; ++ix; }
-            } else {
-                ix = (tile * 32 + lane) / ny;
-                iy = tile * 32 + lane - ix * ny;
+    };
+
+    const int segs = prm.g_segs, ny = prm.g_n[1];
+    if constexpr (WARPOWN) {
+        int it = 0;
+        for (int g = lo + warp; g < hi; g += NW, ++it) {
+            const int tl = g / segs, sg = g - tl * segs;
+            const int rw = tl * 32 + lane, rx = rw / ny;
+            mbar_wait(&full[warp], it & 1);
+            walk(reinterpret_cast<const double *>(smem + static_cast<size_t>(warp) * STAGE_BYTES) + 2 * lane,
+                 GRID_ZS / 4, static_cast<double>(rx), static_cast<double>(rw - rx * ny),
+                 static_cast<double>(sg * GRID_ZS));
+            __syncwarp();                          // every lane has read the slot
+            if (lane == 0 && g + NW < hi) {        // refill it with the warp's next gchunk
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                load_own(g + NW);
+            }
+        }
+    } else {
+        const int ZL = GRID_ZS / WS, z0 = ws * ZL;       // this warp's z run inside every gchunk
+        // (tile, seg) of gchunk g = tile * segs + seg, and the lane's row (ix, iy) of that tile
+        int tile = lo / segs, seg = lo - tile * segs;
+        int ix = (tile * 32 + lane) / ny, iy = tile * 32 + lane - ix * ny;
+        for (int k = 0; k < nk; ++k) {
+            const int slot = k % stages;
+            mbar_wait(&full[slot], (k / stages) & 1);
+            walk(reinterpret_cast<const double *>(smem + static_cast<size_t>(slot) * STAGE_BYTES) +
+                     (z0 / 2) * 64 + 2 * lane,
+                 ZL / 4, static_cast<double>(ix), static_cast<double>(iy),
+                 static_cast<double>(seg * GRID_ZS + z0));
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[slot]);
+            if (++seg == segs) {               // next row tile
+                seg = 0;
+                ++tile;
+                iy += 32;
+                if (ny >= 32) {
+                    if (iy >= ny) { iy -= ny; ++ix; }
+                } else {
+                    ix = (tile * 32 + lane) / ny;
+                    iy = tile * 32 + lane - ix * ny;
+                }
             }
         }
     }
