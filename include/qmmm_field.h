@@ -167,8 +167,9 @@ qmmm_status qmmm_field_create_grid(const double *origin, double spacing, const i
                                    qmmm_field **out);
 
 /* Which copy qmmm_field_eval uses.  AUTO (default): the grid kernels when the handle has a
- * grid and the launch plan keeps z runs of >= 16 nodes per warp and >= 2 work units (32 rows
- * x 64 nodes) per slice -- in practice from a few dozen points per evaluation; otherwise
+ * grid with >= 2 work units (32 rows x 64 nodes) per slice and the batch is either a handful
+ * of points (FP32 <= 2, FP64 <= 4: warp-private walks) or large enough to keep z runs of
+ * >= 16 nodes per warp -- in practice one or two points, or a few dozen and more; otherwise
  * the list.  LIST / GRID force one (INVALID_ARG if the handle does not have that copy).
  * Sticky. */
 typedef enum { QMMM_LAYOUT_AUTO = 0, QMMM_LAYOUT_LIST = 1, QMMM_LAYOUT_GRID = 2 } qmmm_layout;
