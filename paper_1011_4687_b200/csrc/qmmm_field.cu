@@ -288,9 +288,12 @@ cudaError_t launch_pair_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
     return cudaErrorInvalidValue;
 }
 
-template <int EP2, int NW, bool NODEPACK = false>
+template <int EP2, int NW, bool NODEPACK = false, bool FULL = false>
 cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
-    auto kern = grid_kernel_f32x2<EP2, NW, NODEPACK>;
+    if constexpr (!NODEPACK && !FULL) {            // every warp its own point group: no z split
+        if (prm.point_warps == NW) return launch_grid_f32<EP2, NW, false, true>(prm, grid, smem, st);
+    }
+    auto kern = grid_kernel_f32x2<EP2, NW, NODEPACK, FULL>;
     static thread_local size_t configured = 0;
     if (smem > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,

@@ -271,9 +271,13 @@ constexpr int GRID_FLUSH = 4;                       // gchunks per FP32 -> FP64 
 // NODEPACK (EP2 = 1 only): each of the thread's two points is walked on its own with two NODES
 // per register pair (GridRowF32N); a second point beyond P is skipped.  For one or two points
 // per evaluation.
-template <int EP2, int NW, bool NODEPACK = false>
+// FULL: every warp owns its own point group (WP = NW, no z split): the z run is the whole
+// gchunk, a compile-time constant (1.3 % on config 3; the same switch made the FP64 kernel
+// slower and is not used there).
+template <int EP2, int NW, bool NODEPACK = false, bool FULL = false>
 __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 16 / NW : 1) grid_kernel_f32x2(const PairParams prm) {
     static_assert(!NODEPACK || EP2 == 1, "node packing walks single points");
+    static_assert(!(NODEPACK && FULL), "FULL is a mode of the point-packed walk");
     using L = GridF32Layout<EP2, NW>;
     constexpr int EPT = L::EPT, NT = L::NT, STAGE_BYTES = L::STAGE_BYTES;
 
@@ -294,7 +298,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     double2 *acc = reinterpret_cast<double2 *>(ptr);           // [EPT*2][NT] double2
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int WP = NODEPACK ? 1 : prm.point_warps, WS = NW / WP;
+    const int WP = NODEPACK ? 1 : (FULL ? NW : prm.point_warps), WS = NW / WP;
     int lo, hi;
     slice_range(prm.n_chunks, prm.slices, blockIdx.y, lo, hi);
 
@@ -360,7 +364,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     QMMM_MARK(1);
 
     const int wp = warp % WP, ws = warp / WP;
-    const int ZL = GRID_ZS / WS, z0 = ws * ZL;       // this warp's z run inside every gchunk
+    const int ZL = FULL ? GRID_ZS : GRID_ZS / WS, z0 = FULL ? 0 : ws * ZL;   // this warp's z run inside every gchunk
     double2 *my = acc + threadIdx.x;                 // this thread's column: my[i * NT]
 #pragma unroll
     for (int i = 0; i < EPT * 2; ++i) my[i * NT] = make_double2(0.0, 0.0);
@@ -467,7 +471,10 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
         row.start(azb, rxy2);
         mbar_wait(&full[slot], phase);
         const float *data = reinterpret_cast<const float *>(smem + static_cast<size_t>(slot) * STAGE_BYTES);
-        row.run(data + (z0 / 4) * 128 + 4 * lane, ZL / 4, v, tq);
+        if constexpr (FULL)
+            row.run(data + 4 * lane, GRID_ZS / 4, v, tq);
+        else
+            row.run(data + (z0 / 4) * 128 + 4 * lane, ZL / 4, v, tq);
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[slot]);
         // Ex = dx sum(s), Ey = dy sum(s), Ez = sum(s dz)
