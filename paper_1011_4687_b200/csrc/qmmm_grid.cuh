@@ -266,7 +266,10 @@ struct GridRowF32N {
 // lattice) and adds the row's sums into FP32 accumulators, flushed to the FP64 columns in
 // shared memory every 4th gchunk.  prm.chunks = gchunks [n_chunks][ZS/4][32][4] float;
 // prm.nuc = nuclei in grid units; prm.elec in bohr (converted to grid units when staged).
-constexpr int GRID_FLUSH = 4;                       // gchunks per FP32 -> FP64 flush
+#ifndef QMMM_GRID_FLUSH
+#define QMMM_GRID_FLUSH 4
+#endif
+constexpr int GRID_FLUSH = QMMM_GRID_FLUSH;                       // gchunks per FP32 -> FP64 flush
 
 // NODEPACK (EP2 = 1 only): each of the thread's two points is walked on its own with two NODES
 // per register pair (GridRowF32N); a second point beyond P is skipped.  For one or two points
