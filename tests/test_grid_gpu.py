@@ -503,3 +503,31 @@ def test_eval_is_cuda_graph_capturable(torch_cuda, B, layout, precision):
         assert np.array_equal(outs[1][1].cpu().numpy(), En.cpu().numpy())
     finally:
         B.qmmm_field_destroy(h)
+
+
+# ------------------------------------------ config 2 on the device: warp-private grid walks
+@pytest.mark.parametrize("precision,tol", [("fp64", TOL64), ("fp32", TOL32)])
+def test_config2_single_point_device_evaluations(torch_cuda, B, oracle_mod, precision, tol):
+    """Config 2 (one electron, 2.08 M cells + 1,024 nuclei) evaluated point by point with
+    qmmm_field_eval in bench.py's launch configuration: AUTO picks the grid kernels' single-point
+    modes (FP32: node-packed walk, FP64: warp-own walk).  24 positions of the seeded random
+    walk against the oracle; a two-point and a four-point batch as well."""
+    w = make_workload(2, n_points=(24, 1))
+    pts = w.elec_xyz.reshape(-1, 3)
+    ref = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, pts, want_abs=True)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 4)
+    try:
+        V = np.zeros(len(pts)); E = np.zeros((len(pts), 3))
+        for i in range(len(pts)):
+            V[i:i + 1], E[i:i + 1] = run(torch_cuda, B, h, pts[i:i + 1], precision)
+            assert B.qmmm_field_get_grid_info(h)["last_layout"] == "grid"
+        check(ref, V, E, tol)
+        assert B.qmmm_field_get_info(h)["last_plan"]["point_warps"] == 1
+        for n in (2, 4):
+            Vn, En = run(torch_cuda, B, h, pts[:n], precision)
+            eV, eE = rel_errors(ref, np.concatenate([Vn, V[n:]]), np.concatenate([En, E[n:]]))
+            assert eV.max() <= tol and eE.max() <= tol
+        Vl, El = run(torch_cuda, B, h, pts[:1], precision, layout="list")
+        assert abs(Vl[0] - V[0]) <= 2 * tol * abs(V[0])
+    finally:
+        B.qmmm_field_destroy(h)
