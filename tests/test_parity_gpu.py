@@ -310,14 +310,22 @@ def test_repeatability_stress_all_kernel_variants(torch_cuda, B):
     pts = w.elec_xyz.reshape(-1, 3)
     h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, len(pts))
     try:
-        for prec in ("fp64", "fp32"):
-            for plan in (dict(), dict(points_per_thread=1, slices=148), dict(points_per_thread=2, slices=37),
-                         dict(points_per_thread=4, point_warps=1, slices=74),
-                         dict(points_per_thread=8, point_warps=2, slices=296, stages=2)):
-                V0, E0 = gpu_eval(torch_cuda, B, w, pts, prec, plan=plan, handle=h)
-                for _ in range(25):
-                    V, E = gpu_eval(torch_cuda, B, w, pts, prec, plan=plan, handle=h)
-                    assert np.array_equal(V, V0) and np.array_equal(E, E0), (prec, plan)
+        for layout in ("list", "grid"):             # source-list kernels, grid kernels
+            B.qmmm_field_set_layout(h, layout)
+            for prec in ("fp64", "fp32"):
+                for plan in (dict(), dict(points_per_thread=1, slices=148), dict(points_per_thread=2, slices=37),
+                             dict(points_per_thread=4, point_warps=1, slices=74),
+                             dict(points_per_thread=8, point_warps=2, slices=296, stages=2)):
+                    V0, E0 = gpu_eval(torch_cuda, B, w, pts, prec, plan=plan, handle=h)
+                    for _ in range(25):
+                        V, E = gpu_eval(torch_cuda, B, w, pts, prec, plan=plan, handle=h)
+                        assert np.array_equal(V, V0) and np.array_equal(E, E0), (layout, prec, plan)
+                # one, two and four points: the warp-private walks of the grid kernels
+                for n in (1, 2, 4):
+                    V0, E0 = gpu_eval(torch_cuda, B, w, pts[:n], prec, plan=dict(), handle=h)
+                    for _ in range(25):
+                        V, E = gpu_eval(torch_cuda, B, w, pts[:n], prec, plan=dict(), handle=h)
+                        assert np.array_equal(V, V0) and np.array_equal(E, E0), (layout, prec, n)
     finally:
         B.qmmm_field_destroy(h)
 
