@@ -139,7 +139,7 @@ qmmm_status qmmm_field_eval_moves_host(qmmm_field *h, const double *elec_xyz_hos
 /*
  * Grid-aware compact source format.  The paper's sources are "spatially
  * discretized cells": nodes of a regular grid.  When the cells are the nodes
- *     R(ix, iy, iz) = origin + spacing * (ix, iy, iz),   0 <= i_k < n[k]   (cubic cells)
+ *     R(ix, iy, iz) = origin + (ix hx, iy hy, iz hz),   0 <= i_k < n[k]   (cubic or orthorhombic cells)
  * the library keeps a second copy that stores only the charges (4 B FP32 / 8 B FP64 per cell
  * instead of 16 / 32 B) and regenerates the coordinates from the indices.  Its kernels walk
  * the z rows of the grid, where dx, dy and dx^2 + dy^2 are row constants: 9 FP32 (13 FP64)
@@ -149,7 +149,7 @@ qmmm_status qmmm_field_eval_moves_host(qmmm_field *h, const double *elec_xyz_hos
  *
  * qmmm_field_create detects the structure by itself (every source must lie on a node within
  * 16 ulp of the largest coordinate, no node twice, at least half of the bounding grid
- * occupied, M >= 4096); qmmm_field_create_grid takes the grid directly:
+ * occupied, M >= 4096, cell edges within a factor 16 of each other); qmmm_field_create_grid takes the grid directly:
  *   origin [3]                  position of node (0,0,0), bohr (host pointer)
  *   spacing                     cell edge h > 0, bohr
  *   n [3]                       nodes per axis, 1..65536 each, at most 2e9 cells (host pointer)
@@ -165,6 +165,13 @@ qmmm_status qmmm_field_create_grid(const double *origin, double spacing, const i
                                    const double *cell_q, const double *nuc_xyz,
                                    const double *nuc_Z, int64_t K, int64_t max_points,
                                    qmmm_field **out);
+/* The same for orthorhombic cells: spacing [3] = (hx, hy, hz) (host pointer), nodes at
+ * origin + (ix hx, iy hy, iz hz).  The row walk is unchanged (lengths are measured in units of
+ * hz; dx, dy take the factors hx/hz, hy/hz once per row). */
+qmmm_status qmmm_field_create_grid3(const double *origin, const double *spacing, const int64_t *n,
+                                    const double *cell_q, const double *nuc_xyz,
+                                    const double *nuc_Z, int64_t K, int64_t max_points,
+                                    qmmm_field **out);
 
 /* Which copy qmmm_field_eval uses.  AUTO (default): the grid kernels when the handle has a
  * grid with >= 2 work units (32 rows x 64 nodes) per slice and the batch is either a handful
@@ -183,9 +190,10 @@ typedef struct {
     int32_t n[3];                /* nodes per axis */
     int32_t reserved;
     double origin[3];            /* node (0,0,0), bohr */
-    double spacing;              /* h, bohr */
+    double spacing;              /* hz, bohr (= hx = hy for cubic cells) */
     int64_t n_gchunks;           /* work units of 32 rows x 64 z nodes (after padding) */
     int64_t bytes_fp32, bytes_fp64;
+    double spacing3[3];          /* hx, hy, hz, bohr */
 } qmmm_grid_info;
 qmmm_status qmmm_field_get_grid_info(const qmmm_field *h, qmmm_grid_info *info);
 

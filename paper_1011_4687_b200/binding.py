@@ -27,7 +27,7 @@ LIB_PATH = os.environ.get("QMMM_FIELD_LIB") or os.path.join(
     os.path.dirname(os.path.abspath(__file__)), "libqmmm_field.so")
 EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_host",
                     "qmmm_field_eval_moves_host", "qmmm_field_create_grid", "qmmm_field_eval_energy",
-                    "qmmm_field_share",
+                    "qmmm_field_share", "qmmm_field_create_grid3",
                     "qmmm_field_set_layout", "qmmm_field_get_grid_info",
                     "qmmm_field_destroy", "qmmm_field_set_plan", "qmmm_field_get_info",
                     "qmmm_field_set_timing", "qmmm_field_last_timing",
@@ -60,7 +60,7 @@ class qmmm_grid_info(ctypes.Structure):
                 ("n", ctypes.c_int32 * 3), ("reserved", ctypes.c_int32),
                 ("origin", ctypes.c_double * 3), ("spacing", ctypes.c_double),
                 ("n_gchunks", ctypes.c_int64), ("bytes_fp32", ctypes.c_int64),
-                ("bytes_fp64", ctypes.c_int64)]
+                ("bytes_fp64", ctypes.c_int64), ("spacing3", ctypes.c_double * 3)]
 
 
 QMMM_LAYOUT_AUTO, QMMM_LAYOUT_LIST, QMMM_LAYOUT_GRID = 0, 1, 2
@@ -91,6 +91,10 @@ def _load() -> ctypes.CDLL:
                                            ctypes.POINTER(vp)]
     lib.qmmm_field_share.restype = ci
     lib.qmmm_field_share.argtypes = [vp, i64, ctypes.POINTER(vp)]
+    lib.qmmm_field_create_grid3.restype = ci
+    lib.qmmm_field_create_grid3.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double),
+                                            ctypes.POINTER(i64), vp, vp, vp, i64, i64,
+                                            ctypes.POINTER(vp)]
     lib.qmmm_field_set_layout.restype = ci
     lib.qmmm_field_set_layout.argtypes = [vp, ci]
     lib.qmmm_field_get_grid_info.restype = ci
@@ -153,15 +157,21 @@ def qmmm_field_create(src_xyz, src_q, nuc_xyz, nuc_Z, max_points: int) -> int:
 
 def qmmm_field_create_grid(origin, spacing: float, n, cell_q, nuc_xyz, nuc_Z,
                            max_points: int) -> int:
-    """Environment given as a cubic grid: node (0,0,0) at ``origin``, edge ``spacing``,
+    """Environment given as a regular grid: node (0,0,0) at ``origin``, edge ``spacing`` (a
+    number, or (hx, hy, hz) for orthorhombic cells),
     ``cell_q`` [n0,n1,n2] FP64 cell charges (C order; 0 = no cell), host or device."""
     org = (ctypes.c_double * 3)(*[float(v) for v in origin])
     dims = (ctypes.c_int64 * 3)(*[int(v) for v in n])
     assert cell_q is not None and tuple(cell_q.shape) == tuple(int(v) for v in n)
     K = int(nuc_Z.shape[0]) if nuc_Z is not None else 0
     out = ctypes.c_void_p()
-    _check(_lib.qmmm_field_create_grid(org, float(spacing), dims, _ptr(cell_q), _ptr(nuc_xyz),
-                                       _ptr(nuc_Z), K, int(max_points), ctypes.byref(out)))
+    if np.ndim(spacing) == 0:
+        _check(_lib.qmmm_field_create_grid(org, float(spacing), dims, _ptr(cell_q), _ptr(nuc_xyz),
+                                           _ptr(nuc_Z), K, int(max_points), ctypes.byref(out)))
+    else:                                       # (hx, hy, hz): orthorhombic cells
+        sp = (ctypes.c_double * 3)(*[float(v) for v in spacing])
+        _check(_lib.qmmm_field_create_grid3(org, sp, dims, _ptr(cell_q), _ptr(nuc_xyz),
+                                            _ptr(nuc_Z), K, int(max_points), ctypes.byref(out)))
     return out.value
 
 
@@ -185,6 +195,7 @@ def qmmm_field_get_grid_info(handle: int) -> dict:
     return {"present": bool(info.present), "has_list": bool(info.has_list),
             "layout": names[info.layout], "last_layout": names[info.last_layout],
             "n": tuple(info.n), "origin": tuple(info.origin), "spacing": info.spacing,
+            "spacing3": tuple(info.spacing3),
             "n_gchunks": info.n_gchunks, "bytes_fp32": info.bytes_fp32,
             "bytes_fp64": info.bytes_fp64}
 

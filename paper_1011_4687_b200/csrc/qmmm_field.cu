@@ -153,7 +153,7 @@ struct qmmm_field {
     int *counters = nullptr;       // [max_points] arrival tickets of the point blocks (zero at rest)
     // grid layout (qmmm_grid.cuh): present when the cells are nodes of a cubic grid
     bool has_list = true, has_grid = false;
-    GridGeom grid = {{0, 0, 0}, 1.0, {0, 0, 0}, 0.0};
+    GridGeom grid = {{0, 0, 0}, {1.0, 1.0, 1.0}, {0, 0, 0}, 0.0};
     int64_t g_rows = 0, g_tiles = 0, g_segs = 0, n_g = 0;
     float *gcells32 = nullptr;     // [n_g][ZS/4][32][4]
     double *gcells64 = nullptr;    // [n_g][ZS/2][32][2]
@@ -412,9 +412,9 @@ cudaError_t build_grid(qmmm_field *h, const double *ddense, const GridGeom &gg) 
     return e;
 }
 
-// Are the cells nodes of a cubic grid ("spatially discretized cell")?  Candidate
-// spacing from the smallest positive coordinate step between consecutive sources, node
-// counts from the bounding box, then EVERY source is checked against its node (within a few
+// Are the cells nodes of a regular (orthorhombic) grid ("spatially discretized
+// cell")?  Candidate spacing per axis from the smallest positive coordinate step between
+// consecutive sources, node counts from the bounding box, then EVERY source is checked against its node (within a few
 // ulp of the coordinates) and no node may hold two sources.  Anything else keeps the list.
 cudaError_t detect_grid(qmmm_field *h, const double *dxyz, const double *dq, int64_t M) {
     if (M < 4096) return cudaSuccess;
@@ -446,12 +446,18 @@ cudaError_t detect_grid(qmmm_field *h, const double *dxyz, const double *dq, int
         }
     }
     if (best < 0) return cudaSuccess;
-    gg.h = ext[best] / (gg.n[best] - 1);
+    // spacing per axis (orthorhombic cells; a flat axis takes the spacing of the finest one)
+    for (int k = 0; k < 3; ++k)
+        gg.h[k] = gg.n[k] > 1 ? ext[k] / (gg.n[k] - 1) : ext[best] / (gg.n[best] - 1);
+    for (int k = 0; k < 3; ++k)             // cubic cells: one spacing, bit for bit
+        if (std::fabs(gg.h[k] - gg.h[best]) <= 1e-14 * gg.h[best]) gg.h[k] = gg.h[best];
     gg.tol = 16.0 * 2.220446049250313e-16 * maxabs;
     const double total = static_cast<double>(gg.n[0]) * gg.n[1] * gg.n[2];
     if (total > 2.0 * static_cast<double>(M) + 65536.0 || total > 2.0e9) return cudaSuccess;   // too sparse
-    for (int k = 0; k < 3; ++k)
-        if (std::fabs(ext[k] - (gg.n[k] - 1) * gg.h) > gg.tol) return cudaSuccess;           // not cubic cells
+    {
+        const double hmin = std::min({gg.h[0], gg.h[1], gg.h[2]}), hmax = std::max({gg.h[0], gg.h[1], gg.h[2]});
+        if (hmax > 16.0 * hmin) return cudaSuccess;     // needle-shaped cells: keep the list
+    }
     const int64_t ntot = static_cast<int64_t>(total);
     double *ddense = nullptr;
     int *dcount = nullptr;
@@ -811,15 +817,17 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
     return QMMM_OK;
 }
 
-qmmm_status qmmm_field_create_grid(const double *origin, double spacing, const int64_t *n,
-                                   const double *cell_q, const double *nuc_xyz,
-                                   const double *nuc_Z, int64_t K, int64_t max_points,
-                                   qmmm_field **out) {
+qmmm_status qmmm_field_create_grid3(const double *origin, const double *spacing, const int64_t *n,
+                                    const double *cell_q, const double *nuc_xyz,
+                                    const double *nuc_Z, int64_t K, int64_t max_points,
+                                    qmmm_field **out) {
     if (!out) return fail(QMMM_ERR_INVALID_ARG, "create_grid: out is NULL");
     *out = nullptr;
-    if (!origin || !n || !cell_q) return fail(QMMM_ERR_INVALID_ARG, "create_grid: NULL origin, n or cell_q");
-    if (!(spacing > 0.0) || !std::isfinite(spacing))
-        return fail(QMMM_ERR_INVALID_ARG, "create_grid: spacing must be positive and finite");
+    if (!origin || !n || !cell_q || !spacing)
+        return fail(QMMM_ERR_INVALID_ARG, "create_grid: NULL origin, spacing, n or cell_q");
+    for (int k = 0; k < 3; ++k)
+        if (!(spacing[k] > 0.0) || !std::isfinite(spacing[k]))
+            return fail(QMMM_ERR_INVALID_ARG, "create_grid: spacing must be positive and finite");
     for (int k = 0; k < 3; ++k)
         if (n[k] < 1 || n[k] > 65536) return fail(QMMM_ERR_INVALID_ARG, "create_grid: n[k] must be in [1, 65536]");
     const double total = static_cast<double>(n[0]) * n[1] * n[2];
@@ -850,9 +858,9 @@ qmmm_status qmmm_field_create_grid(const double *origin, double spacing, const i
         gg.org[k] = origin[k];
         gg.n[k] = static_cast<int>(n[k]);
         h->bb_lo[k] = origin[k];
-        h->bb_hi[k] = origin[k] + (n[k] - 1) * spacing;
+        h->bb_hi[k] = origin[k] + (n[k] - 1) * spacing[k];
+        gg.h[k] = spacing[k];
     }
-    gg.h = spacing;
     gg.tol = 0.0;
     double *dq = nullptr, *dnxyz = nullptr, *dnz = nullptr;
     unsigned long long *dcnt = nullptr, cnt = 0;
@@ -886,6 +894,14 @@ qmmm_status qmmm_field_create_grid(const double *origin, double spacing, const i
     adopt_sources(h);
     *out = h;
     return QMMM_OK;
+}
+
+qmmm_status qmmm_field_create_grid(const double *origin, double spacing, const int64_t *n,
+                                   const double *cell_q, const double *nuc_xyz,
+                                   const double *nuc_Z, int64_t K, int64_t max_points,
+                                   qmmm_field **out) {
+    const double s3[3] = {spacing, spacing, spacing};
+    return qmmm_field_create_grid3(origin, s3, n, cell_q, nuc_xyz, nuc_Z, K, max_points, out);
 }
 
 qmmm_status qmmm_field_share(const qmmm_field *parent, int64_t max_points, qmmm_field **out) {
@@ -946,7 +962,8 @@ qmmm_status qmmm_field_get_grid_info(const qmmm_field *h, qmmm_grid_info *info) 
             info->n[k] = h->grid.n[k];
             info->origin[k] = h->grid.org[k];
         }
-        info->spacing = h->grid.h;
+        info->spacing = h->grid.h[2];
+        for (int k = 0; k < 3; ++k) info->spacing3[k] = h->grid.h[k];
         info->n_gchunks = h->n_g;
         info->bytes_fp32 = h->n_g * GRID_NODES * 4;
         info->bytes_fp64 = h->n_g * GRID_NODES * 8;
@@ -1092,9 +1109,12 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
             prm.nuc = h->nuclei_u;
             prm.K = static_cast<int>(h->K);
             for (int k = 0; k < 3; ++k) prm.g_org[k] = h->grid.org[k];
-            prm.g_inv_h = 1.0 / h->grid.h;
-            prm.g_scaleV = 1.0 / h->grid.h;
-            prm.g_scaleE = 1.0 / (h->grid.h * h->grid.h);
+            for (int k = 0; k < 3; ++k) prm.g_inv_h[k] = 1.0 / h->grid.h[k];
+            prm.g_sx = h->grid.h[0] / h->grid.h[2];        // exactly 1 for cubic cells
+            prm.g_sy = h->grid.h[1] / h->grid.h[2];
+            prm.g_ortho = (prm.g_sx != 1.0 || prm.g_sy != 1.0) ? 1 : 0;
+            prm.g_scaleV = 1.0 / h->grid.h[2];
+            prm.g_scaleE = 1.0 / (h->grid.h[2] * h->grid.h[2]);
             for (int k = 0; k < 3; ++k) prm.g_n[k] = h->grid.n[k];
             prm.g_segs = static_cast<int>(h->g_segs);
         } else {

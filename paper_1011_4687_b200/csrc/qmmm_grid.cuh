@@ -4,7 +4,9 @@
 // grid.  When the cells of an environment are nodes origin + (ix, iy, iz) h of a cubic grid,
 // only the charges are stored (4 B FP32 / 8 B FP64 per cell instead of 16 / 32 B) and the
 // coordinates are regenerated from the indices.  Everything is computed in GRID UNITS
-// (u = (r - origin) / h, nodes at integer coordinates; V = sum / h, E = sum / h^2 at the end).
+// (u = (r - origin) / h per axis, nodes at integer coordinates; lengths in units of hz, so
+// for cells that are not cubic dx, dy carry the factors hx/hz, hy/hz from the row setup on;
+// V = sum / hz, E = sum / hz^2 at the end).
 //
 // Mapping: a "row" is the nz nodes of one (ix, iy); the 32 lanes of a warp own 32 DIFFERENT
 // rows of a row tile and walk along z together.  For a point i and a row, dx, dy and
@@ -359,9 +361,12 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
         int p = blockIdx.x * ppb + i / 3;
         p = p < prm.P ? p : prm.P - 1;                          // clamp: duplicates are not written
         const int comp = i % 3;
-        const double u = (prm.elec[static_cast<int64_t>(p) * 3 + comp] - prm.g_org[comp]) * prm.g_inv_h;
-        elec_s[i] = u;
-        on_lattice(u, prm.g_n[comp], lat_s[i], dd_all[i]);
+        const double u = (prm.elec[static_cast<int64_t>(p) * 3 + comp] - prm.g_org[comp]) * prm.g_inv_h[comp];
+        const double sc = comp == 0 ? prm.g_sx : (comp == 1 ? prm.g_sy : 1.0);
+        elec_s[i] = u * sc;                                     // units of hz (for the nuclei)
+        float dd;
+        on_lattice(u, prm.g_n[comp], lat_s[i], dd);             // node index units of this axis
+        dd_all[i] = dd * static_cast<float>(sc);                // residual in units of hz
     }
     __syncthreads();
     QMMM_MARK(1);
@@ -430,7 +435,8 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
             const float *data = reinterpret_cast<const float *>(smem + static_cast<size_t>(sl) * STAGE_BYTES);
             auto one_point = [&](float axs, float ays, float azs, float &vvc, float &ttc, float &exc,
                                  float &eyc, float &ezc) {
-                const float dxs = axs - fxs, dys = ays - fys;         // exact (lattice)
+                const float dxs = (axs - fxs) * static_cast<float>(prm.g_sx);   // exact difference (lattice), then hx/hz
+                const float dys = (ays - fys) * static_cast<float>(prm.g_sy);
                 GridRowF32N row;
                 row.start(azs - fzs, fmaf(dys, dys, fmaf(dxs, dxs, 1e-30f)));
                 float v1, t1;
@@ -466,6 +472,10 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
         for (int e = 0; e < EP2; ++e) {
             dx[e] = __fadd2_rn(ax[e], f2(-fx.x, -fx.y));          // exact (lattice)
             dy[e] = __fadd2_rn(ay[e], f2(-fy.x, -fy.y));
+            if (prm.g_ortho) {                                    // cells that are not cubic: hx/hz, hy/hz
+                dx[e] = __fmul2_rn(dx[e], bc(static_cast<float>(prm.g_sx)));
+                dy[e] = __fmul2_rn(dy[e], bc(static_cast<float>(prm.g_sy)));
+            }
             azb[e] = __fadd2_rn(az[e], f2(-fz.x, -fz.y));
             rxy2[e] = __ffma2_rn(dy[e], dy[e], __ffma2_rn(dx[e], dx[e], bc(1e-30f)));
             v[e] = tq[e] = f2(0.0f, 0.0f);
@@ -641,7 +651,8 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
         int p = blockIdx.x * ppb + i / 3;
         p = p < prm.P ? p : prm.P - 1;
         const int comp = i % 3;
-        elec_s[i] = (prm.elec[static_cast<int64_t>(p) * 3 + comp] - prm.g_org[comp]) * prm.g_inv_h;
+        // units of hz on every axis: (r - org) / hz; node (ix, iy, iz) sits at (ix sx, iy sy, iz)
+        elec_s[i] = (prm.elec[static_cast<int64_t>(p) * 3 + comp] - prm.g_org[comp]) * prm.g_scaleV;
     }
     __syncthreads();
 
@@ -659,8 +670,8 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
 #pragma unroll
     for (int e = 0; e < EPT; ++e) V[e] = Ex[e] = Ey[e] = Ez[e] = 0.0;
 
-    // one z run (n4 * 4 nodes at b, [k/2][32][2] doubles) of the lane's row (fx, fy), first
-    // node at z = fz, for the thread's EPT points
+    // one z run (n4 * 4 nodes at b, [k/2][32][2] doubles) of the lane's row at (fx, fy) (units
+    // of hz: ix hx/hz, iy hy/hz), first node at z = fz, for the thread's EPT points
     auto walk = [&](const double *b, int n4, double fx, double fy, double fz) {
         double dx[EPT], dy[EPT], rxy2[EPT], azb[EPT], S[EPT], SZ[EPT];
 #pragma unroll
@@ -715,7 +726,7 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
             const int rw = tl * 32 + lane, rx = rw / ny;
             mbar_wait(&full[warp], it & 1);
             walk(reinterpret_cast<const double *>(smem + static_cast<size_t>(warp) * STAGE_BYTES) + 2 * lane,
-                 GRID_ZS / 4, static_cast<double>(rx), static_cast<double>(rw - rx * ny),
+                 GRID_ZS / 4, static_cast<double>(rx) * prm.g_sx, static_cast<double>(rw - rx * ny) * prm.g_sy,
                  static_cast<double>(sg * GRID_ZS));
             __syncwarp();                          // every lane has read the slot
             if (lane == 0 && g + NW < hi) {        // refill it with the warp's next gchunk
@@ -733,7 +744,7 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
             mbar_wait(&full[slot], (k / stages) & 1);
             walk(reinterpret_cast<const double *>(smem + static_cast<size_t>(slot) * STAGE_BYTES) +
                      (z0 / 2) * 64 + 2 * lane,
-                 ZL / 4, static_cast<double>(ix), static_cast<double>(iy),
+                 ZL / 4, static_cast<double>(ix) * prm.g_sx, static_cast<double>(iy) * prm.g_sy,
                  static_cast<double>(seg * GRID_ZS + z0));
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[slot]);
@@ -751,7 +762,7 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
         }
     }
 
-    // nuclei (grid units), FP64
+    // nuclei (units of hz), FP64
     if constexpr (WITH_E) {
         nuclei_share<EPT>(prm, pe, ws, WS, lane, V, Ex, Ey, Ez);
     } else {
@@ -813,7 +824,7 @@ __global__ void __launch_bounds__(256) grid_spacing_kernel(const double *xyz, in
 
 struct GridGeom {
     double org[3];      // node (0,0,0)
-    double h;
+    double h[3];        // spacing per axis (orthorhombic cells; cubic: all equal)
     int n[3];           // nodes per axis
     double tol;         // accepted distance of a source from its node, per axis (bohr)
 };
@@ -829,9 +840,9 @@ __global__ void grid_scatter_kernel(const double *xyz, const double *q, int64_t 
     bool ok = true;
     for (int k = 0; k < 3; ++k) {
         const double x = xyz[3 * j + k];
-        const double fi = rint((x - gg.org[k]) / gg.h);
+        const double fi = rint((x - gg.org[k]) / gg.h[k]);
         ok = ok && fi >= 0.0 && fi < static_cast<double>(gg.n[k]) &&
-             fabs(fma(fi, gg.h, gg.org[k]) - x) <= gg.tol;
+             fabs(fma(fi, gg.h[k], gg.org[k]) - x) <= gg.tol;
         idx[k] = static_cast<int>(fmin(fmax(fi, 0.0), static_cast<double>(gg.n[k] - 1)));
     }
     if (!ok) {
@@ -887,11 +898,11 @@ __global__ void grid_count_kernel(const double *dense, int64_t n, unsigned long 
     if ((threadIdx.x & 31) == 0 && c) atomicAdd(out, c);
 }
 
-// nuclei in grid units: {(x - org) / h, ..., Z}
+// nuclei in units of hz: {(x - org) / hz, ..., Z}
 __global__ void grid_nuclei_kernel(const double *nuc, int64_t K, GridGeom gg, double *out) {
     const int64_t j = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x;
     if (j >= K) return;
-    for (int k = 0; k < 3; ++k) out[4 * j + k] = (nuc[4 * j + k] - gg.org[k]) / gg.h;
+    for (int k = 0; k < 3; ++k) out[4 * j + k] = (nuc[4 * j + k] - gg.org[k]) / gg.h[2];
     out[4 * j + 3] = nuc[4 * j + 3];
 }
 

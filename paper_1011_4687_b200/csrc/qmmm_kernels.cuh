@@ -55,8 +55,10 @@ struct PairParams {
     // grid layout (qmmm_grid.cuh): chunks = gchunks of charges only, n_chunks = their number,
     // nuc = nuclei in grid units; sums are formed in grid units and scaled at the partial store
     double g_org[3];         // position of node (0,0,0), bohr
-    double g_inv_h;          // 1 / spacing
-    double g_scaleV, g_scaleE;   // 1/h, 1/h^2
+    double g_inv_h[3];       // 1 / spacing per axis: u = (r - org) * inv_h puts the nodes at integers
+    double g_sx, g_sy;       // hx / hz, hy / hz: distances are measured in units of hz
+    int g_ortho;             // cells are not cubic (g_sx or g_sy differs from 1)
+    double g_scaleV, g_scaleE;   // 1/hz, 1/hz^2
     int g_n[3], g_segs;      // nodes per axis (row = ix * ny + iy); z segments (gchunks) per row tile
 #ifdef QMMM_PHASE_TIMING
     long long *dbg;          // [CTAs][10] clock64 at phase boundaries + globaltimer (diagnostic build)

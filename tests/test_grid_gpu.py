@@ -101,14 +101,14 @@ def test_detection_on_the_baseline_configs(torch_cuda, B):
 def test_detection_refuses_off_node_and_duplicate_sources(torch_cuda, B):
     rng = np.random.default_rng(5)
     _, pos, q = random_grid(rng, (20, 24, 40), 0.25, (-2.0, 1.0, 3.0), fill=1.0)
-    for kind in ("off-node", "duplicate", "anisotropic"):
+    for kind in ("off-node", "duplicate", "needles"):
         p, c = pos.copy(), q.copy()
         if kind == "off-node":
             p[len(p) // 2, 1] += 1e-9
         elif kind == "duplicate":
             p[7] = p[8]
         else:
-            p[:, 2] *= 1.5
+            p[:, 2] *= 40.0                      # cell edges 1 : 1 : 40
         h = B.qmmm_field_create(p, c, None, None, 4)
         try:
             assert not B.qmmm_field_get_grid_info(h)["present"], kind
@@ -116,7 +116,16 @@ def test_detection_refuses_off_node_and_duplicate_sources(torch_cuda, B):
             B.qmmm_field_destroy(h)
     h = B.qmmm_field_create(pos, q, None, None, 4)
     try:
-        assert B.qmmm_field_get_grid_info(h)["present"]
+        gi = B.qmmm_field_get_grid_info(h)
+        assert gi["present"] and gi["spacing3"] == (0.25, 0.25, 0.25)
+    finally:
+        B.qmmm_field_destroy(h)
+    p = pos.copy()
+    p[:, 2] = 3.0 + (p[:, 2] - 3.0) * 1.5        # orthorhombic cells 0.25 x 0.25 x 0.375: accepted
+    h = B.qmmm_field_create(p, q, None, None, 4)
+    try:
+        gi = B.qmmm_field_get_grid_info(h)
+        assert gi["present"] and np.allclose(gi["spacing3"], (0.25, 0.25, 0.375), rtol=1e-13)
     finally:
         B.qmmm_field_destroy(h)
 
@@ -150,15 +159,17 @@ def test_config1_grid_layout(torch_cuda, B, oracle_mod, precision, tol):
 
 
 @pytest.mark.parametrize("n,h,P", [((20, 13, 70), 0.3, 33), ((5, 7, 9), 0.5, 3), ((33, 32, 64), 0.2, 100),
-                                   ((1, 40, 129), 0.25, 8), ((40, 1, 1), 0.4, 1), ((64, 3, 200), 0.1, 17)])
+                                   ((1, 40, 129), 0.25, 8), ((40, 1, 1), 0.4, 1), ((64, 3, 200), 0.1, 17),
+                                   ((24, 40, 70), (0.3, 0.2, 0.25), 50), ((40, 33, 64), (0.17, 0.31, 0.23), 1),
+                                   ((16, 16, 130), (0.5, 0.45, 0.1), 4)])
 @pytest.mark.parametrize("precision,tol", [("fp64", TOL64), ("fp32", TOL32)])
 def test_create_grid_ragged_shapes(torch_cuda, B, oracle_mod, n, h, P, precision, tol):
     """qmmm_field_create_grid with row counts that are not multiples of 32, z extents that are
     not multiples of 64, empty cells, nuclei, and point counts with ragged tails."""
     rng = np.random.default_rng(hash((n, P)) % (2 ** 32))
     origin = rng.normal(size=3) * 2.0
-    centre = origin + 0.5 * h * (np.array(n) - 1)
-    dense, pos, q = random_grid(rng, n, h, origin, fill=0.7, hole=(centre, 1.6))
+    centre = origin + 0.5 * np.asarray(h) * (np.array(n) - 1)
+    dense, pos, q = random_grid(rng, n, np.asarray(h), origin, fill=0.7, hole=(centre, 1.6))
     K = 5
     nuc = centre + rng.normal(size=(K, 3)) * 4.0 + 6.0
     Z = rng.choice([1.0, 6.0, 8.0], size=K)
