@@ -309,6 +309,29 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                     row["source_bytes_per_eval"] = bytes_eval
                     row["source_GBps_back_to_back"] = bytes_eval / (row["us_per_eval_1000_back_to_back"] * 1e-6) / 1e9
                     row["source_GBps_cuda_graph"] = bytes_eval / (row["us_per_eval_1000_cuda_graph"] * 1e-6) / 1e9
+                if not w.sequential and idx <= 1:
+                    # launch-free figure for the small configurations (an evaluation is of the
+                    # size of one kernel launch): 200 evaluations captured once in a CUDA graph
+                    # and replayed, sources warm in L2 as in a running QMC job
+                    B.qmmm_field_set_timing(h, False)
+                    V = torch.empty(P, dtype=torch.float64, device="cuda")
+                    E = torch.empty((P, 3), dtype=torch.float64, device="cuda")
+                    gr = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(gr):
+                        for _ in range(200):
+                            B.qmmm_field_eval(h, pts, W, N, V, E, prec)
+                    gr.replay()
+                    torch.cuda.synchronize()
+                    cs = torch.cuda.current_stream()
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(cs)
+                    gr.replay()
+                    e1.record(cs)
+                    torch.cuda.synchronize()
+                    us = e0.elapsed_time(e1) * 1e3 / 200
+                    row["us_per_eval_200_cuda_graph"] = us
+                    row["fma_pipe_frac_cuda_graph"] = pairs * SLOTS[(layout, prec)] / (us * 1e-6) / peak
+                    del gr
                 out.append(row)
                 if prec == "fp64" and not w.sequential and idx in (1, 4):
                     # potential only (E = NULL): the paper's own computation, Eq. 4; 13 (list) or

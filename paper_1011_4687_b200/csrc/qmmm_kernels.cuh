@@ -276,7 +276,14 @@ __device__ __forceinline__ void finish_point_block(const PairParams &prm, int pp
 #pragma unroll
             for (int k = 0; k < 8; ++k) a[k] += t[k];
         }
-        for (int k = 0; sidx < prm.slices; sidx += G, ++k) a[k] += __ldcg(src + sidx * stride);
+        // tail (< 8 G slices left): same accumulator order, compile-time indices (a[] stays in
+        // registers) and all loads in flight together
+        double t[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+            t[k] = sidx + k * G < prm.slices ? __ldcg(src + (sidx + k * G) * stride) : 0.0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) a[k] += t[k];
     }
     scratch[tid] = ((a[0] + a[1]) + (a[2] + a[3])) + ((a[4] + a[5]) + (a[6] + a[7]));
     sync();

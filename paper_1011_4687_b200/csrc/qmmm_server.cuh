@@ -119,7 +119,9 @@ __device__ __forceinline__ bool server_collect(const PairParams &prm, ServerMail
         for (; sidx + 7 * G < prm.slices; sidx += 8 * G)
 #pragma unroll
             for (int k = 0; k < 8; ++k) a[k] += part_s[4 * (sidx + k * G) + v];
-        for (int k = 0; sidx < prm.slices; sidx += G, ++k) a[k] += part_s[4 * sidx + v];
+#pragma unroll
+        for (int k = 0; k < 8; ++k)                         // tail, compile-time indices
+            if (sidx + k * G < prm.slices) a[k] += part_s[4 * (sidx + k * G) + v];
     }
     scratch[tid] = ((a[0] + a[1]) + (a[2] + a[3])) + ((a[4] + a[5]) + (a[6] + a[7]));
     sync();
