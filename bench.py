@@ -42,8 +42,18 @@ UNIT = "Gpair/s"
 # per-pair step of SURVEY.md 8(a) costs 17).  Grid layout: dx, dy and dx^2 + dy^2 are constants
 # of a z row: dz, r^2, a, V0, y0^2, c, sum c, sum c dz, T = 9 (FP32) or, with the per-pair cubic
 # refinement, 13 (FP64).
+# Grid kernels that tabulate dz = u_z - k in shared memory (it depends on the point and the z
+# node only; qmmm_field_info.last_dz_table says whether the last launch did) load it instead of
+# stepping it: one operation less, 8 (FP32) / 12 (FP64).
 SLOTS = {("list", "fp32"): 14, ("list", "fp64"): 18, ("grid", "fp32"): 9, ("grid", "fp64"): 13}
 SLOTS_V_ONLY = {"list": 13, "grid": 8}     # FP64 potential only (E = NULL)
+
+
+def slots_for(layout, prec, info, v_only=False):
+    """Algorithmic FMA-pipe lane operations per pair of the kernel the last launch ran."""
+    n = SLOTS_V_ONLY[layout] if v_only else SLOTS[(layout, prec)]
+    return n - 1 if (layout == "grid" and info.get("last_dz_table")) else n
+
 KERNEL = {("list", "fp32"): "pair_kernel_f32x2", ("list", "fp64"): "pair_kernel<double>",
           ("grid", "fp32"): "grid_kernel_f32x2", ("grid", "fp64"): "grid_kernel_f64"}
 DTYPE = {"fp32": "f32 (f64 accumulation)", "fp64": "f64"}
@@ -254,6 +264,8 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                 layout = B.qmmm_field_get_grid_info(h)["last_layout"]
                 pairs = P * (w.M + w.K)
                 peak = peaks["ffma_lane_ops_per_s" if prec == "fp32" else "dfma_lane_ops_per_s"]
+                info = B.qmmm_field_get_info(h)
+                slots = slots_for(layout, prec, info)
                 row = {"config": idx, "name": w.name, "precision": prec, "layout": layout,
                        "layout_choice": "auto" if which == "auto" else "forced",
                        "points": P, "M": w.M,
@@ -262,9 +274,9 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                        "ms_per_eval_min": float(np.min(step_ms)),
                        "pair_kernel_ms_median": float(np.median(pair_ms)),
                        "gpairs_per_s": pairs / np.median(step_ms) / 1e6,
-                       "slots_per_pair": SLOTS[(layout, prec)],
-                       "fma_pipe_frac": pairs * SLOTS[(layout, prec)] / (np.median(step_ms) * 1e-3) / peak,
-                       "plan": B.qmmm_field_get_info(h)["last_plan"]}
+                       "slots_per_pair": slots, "dz_table": bool(info["last_dz_table"]),
+                       "fma_pipe_frac": pairs * slots / (np.median(step_ms) * 1e-3) / peak,
+                       "plan": info["last_plan"]}
                 if w.sequential:
                     # (i) 1,000 back-to-back evaluations, positions resident on the device
                     B.qmmm_field_set_timing(h, False)
@@ -330,7 +342,7 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                     torch.cuda.synchronize()
                     us = e0.elapsed_time(e1) * 1e3 / 200
                     row["us_per_eval_200_cuda_graph"] = us
-                    row["fma_pipe_frac_cuda_graph"] = pairs * SLOTS[(layout, prec)] / (us * 1e-6) / peak
+                    row["fma_pipe_frac_cuda_graph"] = pairs * slots / (us * 1e-6) / peak
                     del gr
                 out.append(row)
                 if prec == "fp64" and not w.sequential and idx in (1, 4):
@@ -340,6 +352,8 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                     step_ms, pair_ms, _ = time_steps(torch, B, h, batches, W, N, prec, reps, 3, flush,
                                                      stream, want_E=False)
                     layout = B.qmmm_field_get_grid_info(h)["last_layout"]
+                    info = B.qmmm_field_get_info(h)
+                    vslots = slots_for(layout, prec, info, v_only=True)
                     out.append({"config": idx, "name": w.name, "precision": "fp64 potential-only",
                                 "layout": layout, "layout_choice": "auto" if which == "auto" else "forced",
                                 "points": P, "M": w.M, "K": w.K, "pairs_per_eval": pairs,
@@ -347,9 +361,9 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                                 "ms_per_eval_min": float(np.min(step_ms)),
                                 "pair_kernel_ms_median": float(np.median(pair_ms)),
                                 "gpairs_per_s": pairs / np.median(step_ms) / 1e6,
-                                "fma_pipe_frac": pairs * SLOTS_V_ONLY[layout] / (np.median(step_ms) * 1e-3) / peak,
-                                "slots_per_pair": SLOTS_V_ONLY[layout],
-                                "plan": B.qmmm_field_get_info(h)["last_plan"]})
+                                "fma_pipe_frac": pairs * vslots / (np.median(step_ms) * 1e-3) / peak,
+                                "slots_per_pair": vslots, "dz_table": bool(info["last_dz_table"]),
+                                "plan": info["last_plan"]})
         finally:
             B.qmmm_field_destroy(h)
         del w
@@ -435,7 +449,7 @@ def run_ours(args):
         peak_key = "ffma_lane_ops_per_s" if prec == "fp32" else "dfma_lane_ops_per_s"
         peak_lane = 0.5 * (peaks0[peak_key] + peaks1[peak_key])
         pair_s = float(np.mean(pair_ms)) * 1e-3
-        slots = SLOTS[(layout, prec)]
+        slots = slots_for(layout, prec, info)
         achieved = P * w.M * slots * 2 / pair_s / 1e12
         peak_tf = 2 * peak_lane / 1e12
         # DRAM bytes per pair-kernel launch from the committed ncu capture (profiles/), if any

@@ -51,7 +51,7 @@ class qmmm_field_info(ctypes.Structure):
                 ("bytes_fp32", ctypes.c_int64), ("bytes_workspace", ctypes.c_int64),
                 ("last_plan", qmmm_plan), ("last_point_blocks", ctypes.c_int32),
                 ("last_launches", ctypes.c_int32), ("sm_count", ctypes.c_int32),
-                ("reserved", ctypes.c_int32)]
+                ("last_dz_table", ctypes.c_int32)]
 
 
 class qmmm_grid_info(ctypes.Structure):

@@ -97,6 +97,22 @@ int grid_f32_warps(int ept, int64_t P) {
     if (grid_f32_nodepack(ept, P)) return GRID_NW_NODEPACK;
     return ept == 8 ? GRID_NW_EPT8 : (ept == 4 ? GRID_NW_EPT4 : GRID_NW_EPT2);
 }
+// dz table of the FP64 grid kernel (4 points per thread, shared stages): [z nodes padded to
+// whole gchunks][points of the CTA] doubles; 0 when the variant has none
+#ifndef QMMM_GRID_F64_DZT
+#define QMMM_GRID_F64_DZT 1
+#endif
+#ifndef QMMM_GRID_F32_DZT
+#define QMMM_GRID_F32_DZT 1
+#endif
+size_t grid_dzt_bytes(bool f32, int ept, int wp, int64_t P, int64_t g_segs) {
+    if (f32) {      // 4 points per thread, every warp its own point group (the FULL kernel)
+        if (!QMMM_GRID_F32_DZT || ept != 4 || wp != GRID_NW_EPT4 || g_segs > 4096) return 0;
+        return GridF32Layout<2, GRID_NW_EPT4>::dzt_bytes(static_cast<int>(g_segs));
+    }
+    if (!QMMM_GRID_F64_DZT || ept != 4 || grid_f64_warpown(ept, P)) return 0;
+    return static_cast<size_t>(g_segs) * GRID_ZS * wp * ept * sizeof(double);
+}
 size_t grid_smem_bytes(bool f32, int stages, int ept, int wp, int64_t P) {
     if (f32 && ept == 8) return GridF32Layout<4, GRID_NW_EPT8>::total(stages);
     if (f32 && ept == 4) return GridF32Layout<2, GRID_NW_EPT4>::total(stages);
@@ -137,7 +153,7 @@ struct qmmm_field {
     double *stage_out = nullptr;   // eval_host staging: V [max_points] then E [max_points][3]
     qmmm_plan user_plan = {0, 0, 0, 0};
     qmmm_plan last_plan = {0, 0, 0, 0};
-    int last_point_blocks = 0, last_launches = 0;
+    int last_point_blocks = 0, last_launches = 0, last_dz_table = 0;
     bool timing = false, timed = false;
     cudaEvent_t ev[2] = {nullptr, nullptr};
     // per-move mailbox: pinned, device-mapped host memory (elec in; V, E and a sequence flag out)
@@ -288,12 +304,16 @@ cudaError_t launch_pair_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
     return cudaErrorInvalidValue;
 }
 
-template <int EP2, int NW, bool NODEPACK = false, bool FULL = false>
+template <int EP2, int NW, bool NODEPACK = false, bool FULL = false, bool DZT = false>
 cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
     if constexpr (!NODEPACK && !FULL) {            // every warp its own point group: no z split
+        if constexpr (EP2 == 2 && NW == GRID_NW_EPT4) {
+            if (prm.point_warps == NW && prm.g_dzt)
+                return launch_grid_f32<EP2, NW, false, true, true>(prm, grid, smem, st);
+        }
         if (prm.point_warps == NW) return launch_grid_f32<EP2, NW, false, true>(prm, grid, smem, st);
     }
-    auto kern = grid_kernel_f32x2<EP2, NW, NODEPACK, FULL>;
+    auto kern = grid_kernel_f32x2<EP2, NW, NODEPACK, FULL, DZT>;
     static thread_local size_t configured = 0;
     if (smem > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -304,9 +324,9 @@ cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaS
     kern<<<grid, 32 * NW, smem, st>>>(prm);
     return cudaGetLastError();
 }
-template <int EPT, bool WITH_E, int NW, bool WARPOWN = false>
+template <int EPT, bool WITH_E, int NW, bool WARPOWN = false, bool DZT = false>
 cudaError_t launch_grid_f64(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
-    auto kern = grid_kernel_f64<EPT, WITH_E, NW, WARPOWN>;
+    auto kern = grid_kernel_f64<EPT, WITH_E, NW, WARPOWN, DZT>;
     static thread_local size_t configured = 0;
     if (smem > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -338,6 +358,7 @@ cudaError_t launch_grid_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
                 return launch_grid_f64<2, true, GRID64_NW_EPT2>(prm, grid, smem, st);
             case 4:
                 if (grid_f64_warpown(4, prm.P)) return launch_grid_f64<4, true, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
+                if (prm.g_dzt) return launch_grid_f64<4, true, GRID64_NW_EPT4, false, true>(prm, grid, smem, st);
                 return launch_grid_f64<4, true, GRID64_NW_EPT4>(prm, grid, smem, st);
         }
     } else {
@@ -350,6 +371,7 @@ cudaError_t launch_grid_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
                 return launch_grid_f64<2, false, GRID64_NW_EPT2>(prm, grid, smem, st);
             case 4:
                 if (grid_f64_warpown(4, prm.P)) return launch_grid_f64<4, false, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
+                if (prm.g_dzt) return launch_grid_f64<4, false, GRID64_NW_EPT4, false, true>(prm, grid, smem, st);
                 return launch_grid_f64<4, false, GRID64_NW_EPT4>(prm, grid, smem, st);
         }
     }
@@ -1048,6 +1070,7 @@ qmmm_status qmmm_field_get_info(const qmmm_field *h, qmmm_field_info *info) {
     info->last_point_blocks = h->last_point_blocks;
     info->last_launches = h->last_launches;
     info->sm_count = h->sm_count;
+    info->last_dz_table = h->last_dz_table;
     return QMMM_OK;
 }
 
@@ -1084,6 +1107,11 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
     while (smem > 227 * 1024 && pl.stages > 2)           // a requested depth that does not fit is reduced
         smem = smem_of(--pl.stages);
     if (smem > 227 * 1024) return fail(QMMM_ERR_INVALID_ARG, "eval: plan exceeds shared memory");
+    // grid kernels: dz table when it fits beside the stages (long z axes keep the stepped dz)
+    const size_t dzt = grid ? grid_dzt_bytes(f32, pl.points_per_thread, pl.point_warps, P, h->g_segs) : 0;
+    // (the FP32 kernel runs two CTAs per SM: half the budget each)
+    const bool use_dzt = dzt > 0 && smem + dzt <= (f32 ? 110 : 200) * 1024;
+    if (use_dzt) smem += dzt;
 
     if (h->timing) CUDA_TRY(cudaEventRecord(h->ev[0], st));
     {
@@ -1117,6 +1145,7 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
             prm.g_scaleE = 1.0 / (h->grid.h[2] * h->grid.h[2]);
             for (int k = 0; k < 3; ++k) prm.g_n[k] = h->grid.n[k];
             prm.g_segs = static_cast<int>(h->g_segs);
+            prm.g_dzt = use_dzt ? 1 : 0;
         } else {
             prm.chunks = f32 ? reinterpret_cast<const char *>(h->chunks32)
                              : reinterpret_cast<const char *>(h->chunks64);
@@ -1147,6 +1176,7 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
     h->last_plan = pl;
     h->last_point_blocks = pb;
     h->last_launches = launches;
+    h->last_dz_table = use_dzt ? 1 : 0;
     return QMMM_OK;
 }
 }  // namespace

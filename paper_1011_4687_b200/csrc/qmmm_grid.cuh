@@ -46,6 +46,10 @@ struct GridF32Layout {
         return static_cast<size_t>(stages) * STAGE_BYTES + BAR_BYTES + ELEC_BYTES + SCRATCH_BYTES +
                ACC_BYTES;
     }
+    // dz table (DZT kernels), after everything else: [z nodes padded to whole gchunks + 1][NW][EPT]
+    __host__ __device__ static constexpr size_t dzt_bytes(int segs) {
+        return static_cast<size_t>(segs * 64 + 1) * NW * EPT * sizeof(float);
+    }
 };
 
 // Coordinate of an evaluation point along one axis (grid units) on a power-of-two lattice
@@ -81,11 +85,43 @@ __device__ __forceinline__ void on_lattice(double u, int n, float &a, float &dd)
 // Per pair: dz (the running dz steps by -1, exact on the lattice), r^2, a = q y0, V0 += a,
 // y0^2, c = a y0^2, sum c, sum c dz, T += c r^2 = 9 FMA-pipe lane operations + 1 MUFU.RSQ
 // (+ 10/16 for the two summation trees).
-template <int EP2>
+//
+// TS > 0 (dz table): dz = a_z - k depends on the point and the z node only, not on the row, so
+// the CTA tabulates it once in shared memory ([z node][warp][EPT] floats, TS = float2 per z
+// node) and a node's dz is ONE broadcast 128-bit load for both point pairs instead of a packed
+// add per pair: 8 FMA-pipe lane operations per pair instead of 9.
+template <int EP2, int TS = 0>
 struct GridRowF32 {
     float2 dzA[EP2], r2A[EP2], y0A[EP2], dzB[EP2], r2B[EP2], y0B[EP2];
     float2 rxy2[EP2], S[EP2], SZ[EP2];
+    const float2 *tp;                  // TS > 0: table entry of the node held in the current set
 
+    __device__ __forceinline__ void load_dz(const float2 *t, float2 (&dz)[EP2]) {
+        if constexpr (EP2 == 2) {
+            const float4 d = *reinterpret_cast<const float4 *>(t);
+            dz[0] = f2(d.x, d.y);
+            dz[1] = f2(d.z, d.w);
+        } else {
+#pragma unroll
+            for (int e = 0; e < EP2; ++e) dz[e] = t[e];
+        }
+    }
+    // table variant: the run starts at the node whose entry is t
+    __device__ __forceinline__ void start(const float2 *t, const float2 (&rxy2_)[EP2]) {
+        tp = t;
+        load_dz(t, dzA);
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+            rxy2[e] = rxy2_[e];
+            S[e] = SZ[e] = f2(0.0f, 0.0f);
+            r2A[e] = __ffma2_rn(dzA[e], dzA[e], rxy2[e]);
+        }
+#pragma unroll
+        for (int e = 0; e < EP2; ++e) {
+            y0A[e].x = rsqrt_mufu_f32(r2A[e].x);
+            y0A[e].y = rsqrt_mufu_f32(r2A[e].y);
+        }
+    }
     __device__ __forceinline__ void start(const float2 (&azb)[EP2], const float2 (&rxy2_)[EP2]) {
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
@@ -102,10 +138,11 @@ struct GridRowF32 {
     }
     // next node from the current one: dz - 1, r^2, MUFU
     __device__ __forceinline__ void step(const float2 (&dzc)[EP2], float2 (&dzn)[EP2],
-                                         float2 (&r2n)[EP2], float2 (&y0n)[EP2]) {
+                                         float2 (&r2n)[EP2], float2 (&y0n)[EP2], int j = 0) {
+        if constexpr (TS > 0) load_dz(tp + j * TS, dzn);      // j-th node after the one at tp
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
-            dzn[e] = __fadd2_rn(dzc[e], bc(-1.0f));
+            if constexpr (TS == 0) dzn[e] = __fadd2_rn(dzc[e], bc(-1.0f));
             r2n[e] = __ffma2_rn(dzn[e], dzn[e], rxy2[e]);
         }
 #pragma unroll
@@ -132,14 +169,15 @@ struct GridRowF32 {
     // 4 nodes (one 128-bit load of charges); their V0 and T sums go to Vc, Tc
     __device__ __forceinline__ void four(const float *q4, float2 (&Vc)[EP2], float2 (&Tc)[EP2]) {
         const float4 Q = *reinterpret_cast<const float4 *>(q4);
-        step(dzA, dzB, r2B, y0B);
+        step(dzA, dzB, r2B, y0B, 1);
         acc(dzA, r2A, y0A, Q.x, Vc, Tc, true);
-        step(dzB, dzA, r2A, y0A);
+        step(dzB, dzA, r2A, y0A, 2);
         acc(dzB, r2B, y0B, Q.y, Vc, Tc, false);
-        step(dzA, dzB, r2B, y0B);
+        step(dzA, dzB, r2B, y0B, 3);
         acc(dzA, r2A, y0A, Q.z, Vc, Tc, false);
-        step(dzB, dzA, r2A, y0A);           // the last one looks one node past the run: unused
+        step(dzB, dzA, r2A, y0A, 4);        // the last one looks one node past the run: unused
         acc(dzB, r2B, y0B, Q.w, Vc, Tc, false);
+        if constexpr (TS > 0) tp += 4 * TS;
     }
     // n4 * 4 nodes starting at b ([k4][32][4] floats); V0 and T are summed as trees of short
     // FP32 runs (4 nodes -> 16 -> run): a long FP32 running sum of slowly varying same-sign
@@ -279,8 +317,11 @@ constexpr int GRID_FLUSH = QMMM_GRID_FLUSH;                       // gchunks per
 // FULL: every warp owns its own point group (WP = NW, no z split): the z run is the whole
 // gchunk, a compile-time constant (1.3 % on config 3; the same switch made the FP64 kernel
 // slower and is not used there).
-template <int EP2, int NW, bool NODEPACK = false, bool FULL = false>
+// DZT (FULL only): dz from a per-CTA table in shared memory (GridRowF32<EP2, TS>), chosen by
+// the launcher when the table fits beside two CTAs per SM.
+template <int EP2, int NW, bool NODEPACK = false, bool FULL = false, bool DZT = false>
 __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 16 / NW : 1) grid_kernel_f32x2(const PairParams prm) {
+    static_assert(!DZT || (FULL && !NODEPACK), "dz table: every warp walks whole gchunks of its own points");
     static_assert(!NODEPACK || EP2 == 1, "node packing walks single points");
     static_assert(!(NODEPACK && FULL), "FULL is a mode of the point-packed walk");
     using L = GridF32Layout<EP2, NW>;
@@ -369,6 +410,16 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
         dd_all[i] = dd * static_cast<float>(sc);                // residual in units of hz
     }
     __syncthreads();
+    constexpr int TS = DZT ? NW * EP2 : 0;                      // float2 per z node of the table
+    float *dzt = reinterpret_cast<float *>(acc + EPT * 2 * NT); // [segs * ZS + 1][NW][EPT]
+    if constexpr (DZT) {                                        // a_z - k: exact on the lattice
+        const int nent = (prm.g_segs * GRID_ZS + 1) * NW * EPT;
+        for (int i = threadIdx.x; i < nent; i += NT) {
+            const int kz = i / (NW * EPT), pp = i - kz * (NW * EPT);
+            dzt[i] = lat_s[pp * 3 + 2] - static_cast<float>(kz);
+        }
+        __syncthreads();
+    }
     QMMM_MARK(1);
 
     const int wp = warp % WP, ws = warp / WP;
@@ -476,12 +527,15 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
                 dx[e] = __fmul2_rn(dx[e], bc(static_cast<float>(prm.g_sx)));
                 dy[e] = __fmul2_rn(dy[e], bc(static_cast<float>(prm.g_sy)));
             }
-            azb[e] = __fadd2_rn(az[e], f2(-fz.x, -fz.y));
+            if constexpr (!DZT) azb[e] = __fadd2_rn(az[e], f2(-fz.x, -fz.y));
             rxy2[e] = __ffma2_rn(dy[e], dy[e], __ffma2_rn(dx[e], dx[e], bc(1e-30f)));
             v[e] = tq[e] = f2(0.0f, 0.0f);
         }
-        GridRowF32<EP2> row;
-        row.start(azb, rxy2);
+        GridRowF32<EP2, TS> row;
+        if constexpr (DZT)
+            row.start(reinterpret_cast<const float2 *>(dzt) + (seg * GRID_ZS) * TS + wp * EP2, rxy2);
+        else
+            row.start(azb, rxy2);
         mbar_wait(&full[slot], phase);
         const float *data = reinterpret_cast<const float *>(smem + static_cast<size_t>(slot) * STAGE_BYTES);
         if constexpr (FULL)
@@ -598,8 +652,14 @@ __device__ __forceinline__ void consumer_sync() {     // named barrier 1: the N 
 // WARPOWN (a handful of points, all owned by every warp): warp w loads and walks whole gchunks
 // lo + w, lo + w + NW, ... by itself (one private slot per warp, no producer warp, no waiting
 // on other warps), as the node-packed FP32 kernel does.
-template <int EPT, bool WITH_E, int NW, bool WARPOWN = false>
+// DZT (EPT = 4, not WARPOWN; chosen by the launcher when the table fits): dz = u_z - k depends
+// on the point and the z node only, not on the row, so the CTA tabulates it once in shared
+// memory ([nz padded][WP * EPT] doubles) and the walk loads it with two broadcast LDS.128 per
+// node instead of stepping it on the DP pipe: 12 DP lane operations per pair instead of 13
+// (potential only: 7 instead of 8).
+template <int EPT, bool WITH_E, int NW, bool WARPOWN = false, bool DZT = false>
 __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairParams prm) {
+    static_assert(!DZT || (EPT == 4 && !WARPOWN), "dz table: 4 points per thread, shared stages");
     constexpr int STAGE_BYTES = GRID_STAGE_BYTES_F64;
     extern __shared__ __align__(128) unsigned char smem[];
     const int stages = WARPOWN ? NW : prm.stages;
@@ -611,6 +671,7 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int WP = WARPOWN ? 1 : prm.point_warps, WS = NW / WP;
+    double *dzt = elec_s + WP * EPT * 3;        // DZT: [g_segs * ZS][WP*EPT], 16-byte aligned (EPT = 4)
     int lo, hi;
     slice_range(prm.n_chunks, prm.slices, blockIdx.y, lo, hi);
     const int nk = hi - lo;
@@ -654,6 +715,16 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
         // units of hz on every axis: (r - org) / hz; node (ix, iy, iz) sits at (ix sx, iy sy, iz)
         elec_s[i] = (prm.elec[static_cast<int64_t>(p) * 3 + comp] - prm.g_org[comp]) * prm.g_scaleV;
     }
+    if constexpr (DZT) {                           // dz of every (z node, point of this CTA)
+        const int nzp = prm.g_segs * GRID_ZS;
+        for (int i = threadIdx.x; i < nzp * ppb; i += 32 * (NW + 1)) {
+            const int kz = i / ppb, pp = i - kz * ppb;
+            int p = blockIdx.x * ppb + pp;
+            p = p < prm.P ? p : prm.P - 1;
+            const double uz = (prm.elec[static_cast<int64_t>(p) * 3 + 2] - prm.g_org[2]) * prm.g_scaleV;
+            dzt[i] = uz - static_cast<double>(kz);
+        }
+    }
     __syncthreads();
 
     if (warp == NW) {
@@ -672,14 +743,15 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
 
     // one z run (n4 * 4 nodes at b, [k/2][32][2] doubles) of the lane's row at (fx, fy) (units
     // of hz: ix hx/hz, iy hy/hz), first node at z = fz, for the thread's EPT points
-    auto walk = [&](const double *b, int n4, double fx, double fy, double fz) {
+    const int tstride = WP * EPT;                  // DZT: doubles per z node in the table
+    auto walk = [&](const double *b, int n4, double fx, double fy, double fz, const double *tz) {
         double dx[EPT], dy[EPT], rxy2[EPT], azb[EPT], S[EPT], SZ[EPT];
 #pragma unroll
         for (int e = 0; e < EPT; ++e) {
             dx[e] = pe[3 * e + 0] - fx;
             dy[e] = pe[3 * e + 1] - fy;
             rxy2[e] = fma(dy[e], dy[e], fma(dx[e], dx[e], 1e-200));
-            azb[e] = pe[3 * e + 2] - fz;
+            if constexpr (!DZT) azb[e] = pe[3 * e + 2] - fz;
             S[e] = SZ[e] = 0.0;
         }
 #pragma unroll 1
@@ -689,9 +761,19 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
             const double qs[4] = {Qa.x, Qa.y, Qb.x, Qb.y};
 #pragma unroll
             for (int t = 0; t < 4; ++t) {
+                double dzs[EPT];
+                if constexpr (DZT) {               // EPT = 4: two broadcast 128-bit loads
+                    const double2 d01 = *reinterpret_cast<const double2 *>(tz + t * tstride);
+                    const double2 d23 = *reinterpret_cast<const double2 *>(tz + t * tstride + 2);
+                    dzs[0] = d01.x; dzs[1] = d01.y; dzs[EPT - 2] = d23.x; dzs[EPT - 1] = d23.y;
+                } else {
+#pragma unroll
+                    for (int e = 0; e < EPT; ++e)
+                        dzs[e] = t == 0 ? azb[e] : azb[e] - static_cast<double>(t);
+                }
 #pragma unroll
                 for (int e = 0; e < EPT; ++e) {
-                    const double dz = t == 0 ? azb[e] : azb[e] - static_cast<double>(t);
+                    const double dz = dzs[e];
                     const double r2 = fma(dz, dz, rxy2[e]);
                     const double y = rsqrt_refined_f64(r2);
                     if constexpr (WITH_E) {
@@ -705,8 +787,12 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
                     }
                 }
             }
+            if constexpr (DZT) {
+                tz += 4 * tstride;
+            } else {
 #pragma unroll
-            for (int e = 0; e < EPT; ++e) azb[e] -= 4.0;
+                for (int e = 0; e < EPT; ++e) azb[e] -= 4.0;
+            }
         }
         if constexpr (WITH_E) {
 #pragma unroll
@@ -727,7 +813,7 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
             mbar_wait(&full[warp], it & 1);
             walk(reinterpret_cast<const double *>(smem + static_cast<size_t>(warp) * STAGE_BYTES) + 2 * lane,
                  GRID_ZS / 4, static_cast<double>(rx) * prm.g_sx, static_cast<double>(rw - rx * ny) * prm.g_sy,
-                 static_cast<double>(sg * GRID_ZS));
+                 static_cast<double>(sg * GRID_ZS), nullptr);
             __syncwarp();                          // every lane has read the slot
             if (lane == 0 && g + NW < hi) {        // refill it with the warp's next gchunk
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -745,7 +831,8 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
             walk(reinterpret_cast<const double *>(smem + static_cast<size_t>(slot) * STAGE_BYTES) +
                      (z0 / 2) * 64 + 2 * lane,
                  ZL / 4, static_cast<double>(ix) * prm.g_sx, static_cast<double>(iy) * prm.g_sy,
-                 static_cast<double>(seg * GRID_ZS + z0));
+                 static_cast<double>(seg * GRID_ZS + z0),
+                 dzt + (seg * GRID_ZS + z0) * tstride + wp * EPT);
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[slot]);
             if (++seg == segs) {               // next row tile

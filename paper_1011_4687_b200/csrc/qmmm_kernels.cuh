@@ -60,6 +60,7 @@ struct PairParams {
     int g_ortho;             // cells are not cubic (g_sx or g_sy differs from 1)
     double g_scaleV, g_scaleE;   // 1/hz, 1/hz^2
     int g_n[3], g_segs;      // nodes per axis (row = ix * ny + iy); z segments (gchunks) per row tile
+    int g_dzt;               // grid kernels: dz table in shared memory (qmmm_grid.cuh, DZT)
 #ifdef QMMM_PHASE_TIMING
     long long *dbg;          // [CTAs][10] clock64 at phase boundaries + globaltimer (diagnostic build)
 #endif
