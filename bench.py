@@ -306,6 +306,22 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                     torch.cuda.synchronize()
                     row["us_per_eval_1000_cuda_graph"] = e0.elapsed_time(e1) * 1e3 / len(walk)
                     del gr
+                    # (i'') the same graph with overlapped evaluations (qmmm_field_set_overlap:
+                    # programmatic dependent launch, evaluation n + 1 starts while n finishes)
+                    B.qmmm_field_set_overlap(h, True)
+                    gr = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(gr):
+                        for p in walk:
+                            B.qmmm_field_eval(h, p, 1, 1, V, E, prec)
+                    gr.replay()
+                    torch.cuda.synchronize()
+                    e0.record(cs)
+                    gr.replay()
+                    e1.record(cs)
+                    torch.cuda.synchronize()
+                    row["us_per_eval_1000_cuda_graph_overlap"] = e0.elapsed_time(e1) * 1e3 / len(walk)
+                    del gr
+                    B.qmmm_field_set_overlap(h, False)
                     # (ii) the QMC loop of PAPER.md:117: r_new in (24 B), U out (32 B), every move;
                     # the loop itself runs inside the library (qmmm_field_eval_moves_host)
                     hp = np.ascontiguousarray(w.elec_xyz.reshape(-1, 3))
@@ -321,6 +337,7 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                     row["source_bytes_per_eval"] = bytes_eval
                     row["source_GBps_back_to_back"] = bytes_eval / (row["us_per_eval_1000_back_to_back"] * 1e-6) / 1e9
                     row["source_GBps_cuda_graph"] = bytes_eval / (row["us_per_eval_1000_cuda_graph"] * 1e-6) / 1e9
+                    row["source_GBps_cuda_graph_overlap"] = bytes_eval / (row["us_per_eval_1000_cuda_graph_overlap"] * 1e-6) / 1e9
                 if not w.sequential and idx <= 1:
                     # launch-free figure for the small configurations (an evaluation is of the
                     # size of one kernel launch): 200 evaluations captured once in a CUDA graph
@@ -343,6 +360,23 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                     us = e0.elapsed_time(e1) * 1e3 / 200
                     row["us_per_eval_200_cuda_graph"] = us
                     row["fma_pipe_frac_cuda_graph"] = pairs * slots / (us * 1e-6) / peak
+                    del gr
+                    # the same with overlapped evaluations (programmatic dependent launch)
+                    B.qmmm_field_set_overlap(h, True)
+                    gr = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(gr):
+                        for _ in range(200):
+                            B.qmmm_field_eval(h, pts, W, N, V, E, prec)
+                    gr.replay()
+                    torch.cuda.synchronize()
+                    e0.record(cs)
+                    gr.replay()
+                    e1.record(cs)
+                    torch.cuda.synchronize()
+                    B.qmmm_field_set_overlap(h, False)
+                    us = e0.elapsed_time(e1) * 1e3 / 200
+                    row["us_per_eval_200_cuda_graph_overlap"] = us
+                    row["fma_pipe_frac_cuda_graph_overlap"] = pairs * slots / (us * 1e-6) / peak
                     del gr
                 out.append(row)
                 if prec == "fp64" and not w.sequential and idx in (1, 4):

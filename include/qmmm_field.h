@@ -250,6 +250,23 @@ qmmm_status qmmm_field_get_info(const qmmm_field *h, qmmm_field_info *info);
  * INVALID_ARG if timing is off or no eval has run.
  */
 qmmm_status qmmm_field_set_timing(qmmm_field *h, int enable);
+
+/*
+ * Overlap of back-to-back evaluations on one stream (off by default).  The paper's use is a
+ * long sequence of single-point evaluations, one per Monte-Carlo move; each is
+ * a few microseconds, of which the launch, the prologue (barrier set-up, first bulk copies)
+ * and the tail (fence, ticket, cross-CTA sum) are the larger part.  When enabled, eval
+ * launches its kernel with programmatic stream serialization: it may START while the previous
+ * kernel in the stream -- the previous evaluation -- is still running, does its prologue,
+ * source walk and in-CTA reduction, and waits for the predecessor to finish (griddepcontrol)
+ * only before it touches the partials workspace, the tickets or V / E.  Results are bitwise
+ * the same as without overlap.
+ * Precondition while enabled: elec_xyz of an evaluation is not produced by the evaluation
+ * immediately before it on the same stream (it is read before the wait); work of other
+ * libraries in between serialises as usual.  Ignored (plain serialization) while timing is on
+ * and by the host-buffer paths.  Works inside CUDA-graph capture.
+ */
+qmmm_status qmmm_field_set_overlap(qmmm_field *h, int enable);
 qmmm_status qmmm_field_last_timing(qmmm_field *h, double *pair_ms, double *finalize_ms);
 
 /*

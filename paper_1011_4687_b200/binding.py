@@ -30,7 +30,7 @@ EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_hos
                     "qmmm_field_share", "qmmm_field_create_grid3",
                     "qmmm_field_set_layout", "qmmm_field_get_grid_info",
                     "qmmm_field_destroy", "qmmm_field_set_plan", "qmmm_field_get_info",
-                    "qmmm_field_set_timing", "qmmm_field_last_timing",
+                    "qmmm_field_set_timing", "qmmm_field_last_timing", "qmmm_field_set_overlap",
                     "qmmm_probe_peak", "qmmm_last_error")
 
 
@@ -107,6 +107,8 @@ def _load() -> ctypes.CDLL:
     lib.qmmm_field_get_info.argtypes = [vp, ctypes.POINTER(qmmm_field_info)]
     lib.qmmm_field_set_timing.restype = ci
     lib.qmmm_field_set_timing.argtypes = [vp, ci]
+    lib.qmmm_field_set_overlap.restype = ci
+    lib.qmmm_field_set_overlap.argtypes = [vp, ci]
     lib.qmmm_field_last_timing.restype = ci
     lib.qmmm_field_last_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_double),
                                            ctypes.POINTER(ctypes.c_double)]
@@ -251,6 +253,12 @@ def qmmm_field_get_info(handle: int) -> dict:
 
 def qmmm_field_set_timing(handle: int, enable: bool) -> None:
     _check(_lib.qmmm_field_set_timing(handle, int(bool(enable))))
+
+
+def qmmm_field_set_overlap(handle: int, enable: bool) -> None:
+    """Back-to-back evaluations on one stream may overlap (programmatic dependent launch); see
+    include/qmmm_field.h for the precondition on elec_xyz."""
+    _check(_lib.qmmm_field_set_overlap(handle, int(bool(enable))))
 
 
 def qmmm_field_last_timing(handle: int) -> Tuple[float, float]:

@@ -155,6 +155,7 @@ struct qmmm_field {
     qmmm_plan last_plan = {0, 0, 0, 0};
     int last_point_blocks = 0, last_launches = 0, last_dz_table = 0;
     bool timing = false, timed = false;
+    bool overlap = false;          // qmmm_field_set_overlap: back-to-back evaluations may overlap
     cudaEvent_t ev[2] = {nullptr, nullptr};
     // per-move mailbox: pinned, device-mapped host memory (elec in; V, E and a sequence flag out)
     double *mail_h = nullptr, *mail_d = nullptr;   // [MAIL_POINTS*3 | MAIL_POINTS*4 | flag]
@@ -249,6 +250,24 @@ bool auto_uses_grid(const qmmm_field *h, int64_t P, bool f32) {
     return nw / pl.point_warps <= 4;
 }
 
+// One evaluation kernel launch.  prm.pdl: programmatic stream serialization -- the kernel may
+// start while its predecessor in the stream is still running (qmmm_field_set_overlap; the
+// kernels order themselves with griddepcontrol, qmmm_kernels.cuh).
+cudaError_t launch_eval_kernel(void (*kern)(const PairParams), dim3 grid, unsigned threads, size_t smem,
+                               cudaStream_t st, const PairParams &prm) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = dim3(threads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = prm.pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, prm);
+}
+
 template <typename REAL, int EPT, bool WITH_E = true>
 cudaError_t launch_pair(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
     auto kern = pair_kernel<REAL, EPT, WITH_E>;
@@ -259,8 +278,7 @@ cudaError_t launch_pair(const PairParams &prm, dim3 grid, size_t smem, cudaStrea
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    kern<<<grid, CTA_THREADS, smem, st>>>(prm);
-    return cudaGetLastError();
+    return launch_eval_kernel(kern, grid, CTA_THREADS, smem, st, prm);
 }
 
 template <int EP2, int NW>
@@ -273,8 +291,7 @@ cudaError_t launch_pair_f32x2(const PairParams &prm, dim3 grid, size_t smem, cud
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    kern<<<grid, 32 * NW, smem, st>>>(prm);
-    return cudaGetLastError();
+    return launch_eval_kernel(kern, grid, 32 * NW, smem, st, prm);
 }
 
 // FP64: pair_kernel<double, 1|2|4>.  FP32-acc64: the scalar kernel for one point per
@@ -321,8 +338,7 @@ cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaS
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    kern<<<grid, 32 * NW, smem, st>>>(prm);
-    return cudaGetLastError();
+    return launch_eval_kernel(kern, grid, 32 * NW, smem, st, prm);
 }
 template <int EPT, bool WITH_E, int NW, bool WARPOWN = false, bool DZT = false>
 cudaError_t launch_grid_f64(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
@@ -334,8 +350,7 @@ cudaError_t launch_grid_f64(const PairParams &prm, dim3 grid, size_t smem, cudaS
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    kern<<<grid, 32 * (NW + 1), smem, st>>>(prm);
-    return cudaGetLastError();
+    return launch_eval_kernel(kern, grid, 32 * (NW + 1), smem, st, prm);
 }
 // Grid layout: FP32-acc64 packed kernel for 2, 4, 8 points per thread; FP64 for 1, 2, 4.
 cudaError_t launch_grid_ept(bool f32, int ept, const PairParams &prm, dim3 grid, size_t smem,
@@ -1046,6 +1061,12 @@ qmmm_status qmmm_field_set_timing(qmmm_field *h, int enable) {
     return QMMM_OK;
 }
 
+qmmm_status qmmm_field_set_overlap(qmmm_field *h, int enable) {
+    if (!h) return fail(QMMM_ERR_INVALID_ARG, "set_overlap: NULL handle");
+    h->overlap = enable != 0;
+    return QMMM_OK;
+}
+
 qmmm_status qmmm_field_last_timing(qmmm_field *h, double *pair_ms, double *finalize_ms) {
     if (!h || !pair_ms || !finalize_ms) return fail(QMMM_ERR_INVALID_ARG, "last_timing: NULL argument");
     if (!h->timing || !h->timed)
@@ -1129,6 +1150,9 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
         prm.host_flag = host_flag;
         prm.seq = h->seq;
         prm.done = h->counters + h->max_points;
+        // overlap with the previous evaluation on this stream (not with the timing events in
+        // between, and not for the mailbox path, whose host reads V and E behind a flag)
+        prm.pdl = (h->overlap && !h->timing && !host_flag) ? 1 : 0;
         if (grid) {
             // cells: charges only, coordinates from the indices; everything in grid units
             prm.chunks = f32 ? reinterpret_cast<const char *>(h->gcells32)

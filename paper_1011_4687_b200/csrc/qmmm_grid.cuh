@@ -328,6 +328,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     constexpr int EPT = L::EPT, NT = L::NT, STAGE_BYTES = L::STAGE_BYTES;
 
     extern __shared__ __align__(128) unsigned char smem[];
+    pdl_launch_dependents();
     QMMM_MARK_GT(8);
     QMMM_MARK(0);
     // NODEPACK: warp-private pipelines, two slots per warp (prm.stages is not used)
@@ -624,6 +625,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
         red[warp * EPT * 4 + 8 * (lane >> 2) + 4 + (lane & 3)] = tot.y;
     }
     __syncthreads();
+    pdl_wait();                                  // the previous evaluation is done with the workspace
     if (ws == 0 && lane < EPT * 4) {
         double a = 0.0;
         for (int s = 0; s < WS; ++s) a += red[(s * WP + wp) * EPT * 4 + lane];
@@ -662,6 +664,7 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
     static_assert(!DZT || (EPT == 4 && !WARPOWN), "dz table: 4 points per thread, shared stages");
     constexpr int STAGE_BYTES = GRID_STAGE_BYTES_F64;
     extern __shared__ __align__(128) unsigned char smem[];
+    pdl_launch_dependents();
     const int stages = WARPOWN ? NW : prm.stages;
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + static_cast<size_t>(stages) * STAGE_BYTES);
     uint64_t *empty = full + 8;
@@ -874,6 +877,7 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
         }
     }
     consumer_sync<NW>();
+    pdl_wait();                                  // the previous evaluation is done with the workspace
     if (ws == 0 && lane < EPT * 4) {
         double a = 0.0;
         for (int s = 0; s < WS; ++s) a += red[((s * WP + wp) * EPT) * 4 + lane];

@@ -61,6 +61,7 @@ struct PairParams {
     double g_scaleV, g_scaleE;   // 1/hz, 1/hz^2
     int g_n[3], g_segs;      // nodes per axis (row = ix * ny + iy); z segments (gchunks) per row tile
     int g_dzt;               // grid kernels: dz table in shared memory (qmmm_grid.cuh, DZT)
+    int pdl;                 // host side only: launch with programmatic stream serialization
 #ifdef QMMM_PHASE_TIMING
     long long *dbg;          // [CTAs][10] clock64 at phase boundaries + globaltimer (diagnostic build)
 #endif
@@ -99,6 +100,17 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+// Programmatic dependent launch (qmmm_field_set_overlap).  Every evaluation kernel lets its
+// successor in the stream start at once (launch_dependents, first instruction) and touches
+// what a predecessor may still be using -- the partials workspace, the tickets, V and E --
+// only after pdl_wait(): prologue, source walk, nuclear term and in-CTA reduction of evaluation
+// n + 1 overlap the tail (fence, ticket, last-CTA sum) of evaluation n.  Both instructions are
+// no-ops for launches without the attribute.
+__device__ __forceinline__ void pdl_launch_dependents() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
     asm volatile(
         "{\n\t"
@@ -316,6 +328,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
     constexpr int STAGE_BYTES = STAGE_HDR + SC * CHUNK_BYTES;
 
     extern __shared__ __align__(128) unsigned char smem[];
+    pdl_launch_dependents();
     QMMM_MARK_GT(8);
     QMMM_MARK(0);
     // layout: [stages x STAGE_BYTES] [full barriers] [empty barriers] [reduction scratch]
@@ -498,6 +511,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
         }
     }
     compute_warps_sync();
+    pdl_wait();                                  // the previous evaluation is done with the workspace
     // warps with ws == 0 add the WS source-split partners in index order and store
     if (ws == 0 && lane < EPT * 4) {
         double acc = 0.0;
@@ -612,6 +626,7 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
     constexpr int CHUNK_BYTES = L::CHUNK_BYTES, STAGE_BYTES = L::STAGE_BYTES;
 
     extern __shared__ __align__(128) unsigned char smem[];
+    pdl_launch_dependents();
     QMMM_MARK_GT(8);
     QMMM_MARK(0);
     const int stages = prm.stages;
@@ -804,6 +819,7 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
         red[warp * EPT * 4 + 8 * (lane >> 2) + 4 + (lane & 3)] = tot.y;
     }
     __syncthreads();
+    pdl_wait();                                  // the previous evaluation is done with the workspace
     if (ws == 0 && lane < EPT * 4) {
         double a = 0.0;
         for (int s = 0; s < WS; ++s) a += red[(s * WP + wp) * EPT * 4 + lane];

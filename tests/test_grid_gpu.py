@@ -516,6 +516,54 @@ def test_eval_is_cuda_graph_capturable(torch_cuda, B, layout, precision):
         B.qmmm_field_destroy(h)
 
 
+# ----------------------------------------------- overlapped back-to-back evaluations (PDL)
+@pytest.mark.parametrize("layout,precision", [("grid", "fp32"), ("grid", "fp64"), ("list", "fp32"), ("list", "fp64")])
+@pytest.mark.parametrize("P", [1, 4, 32])
+def test_overlapped_back_to_back_evaluations_are_bitwise_the_same(torch_cuda, B, oracle_mod, layout,
+                                                                  precision, P):
+    """qmmm_field_set_overlap: evaluation n + 1 starts while evaluation n is still running
+    (programmatic dependent launch) and waits for it only before it touches the workspace, the
+    tickets and the outputs.  300 evaluations of changing batch size in one stream -- every one
+    reuses the same workspace and tickets -- give bitwise the results of the serial launches,
+    eagerly and replayed from a CUDA graph; a sample is checked against the oracle."""
+    torch = torch_cuda
+    w = make_workload(1)
+    rng = np.random.default_rng(11)
+    n = 300
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, P)
+    try:
+        B.qmmm_field_set_layout(h, layout)
+        sizes = [P if i % 3 else max(1, P // 2) for i in range(n)]      # the plan changes too
+        pts = [torch.from_numpy(rng.normal(size=(sz, 3)) * 0.8).cuda() for sz in sizes]
+        res = {}
+        for mode in ("serial", "overlap", "graph"):
+            B.qmmm_field_set_overlap(h, mode != "serial")
+            V = torch.full((n, P), float("nan"), dtype=torch.float64, device="cuda")
+            E = torch.full((n, P, 3), float("nan"), dtype=torch.float64, device="cuda")
+            if mode == "graph":
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g):
+                    for i, p in enumerate(pts):
+                        B.qmmm_field_eval(h, p, 1, sizes[i], V[i, :sizes[i]], E[i, :sizes[i]], precision)
+                g.replay()
+                g.replay()
+            else:
+                for i, p in enumerate(pts):
+                    B.qmmm_field_eval(h, p, 1, sizes[i], V[i, :sizes[i]], E[i, :sizes[i]], precision)
+            torch.cuda.synchronize()
+            res[mode] = (V.cpu().numpy(), E.cpu().numpy())
+        for mode in ("overlap", "graph"):
+            assert np.array_equal(res[mode][0], res["serial"][0], equal_nan=True), mode
+            assert np.array_equal(res[mode][1], res["serial"][1], equal_nan=True), mode
+        tol = TOL64 if precision == "fp64" else TOL32
+        for i in (0, 1, 150, n - 1):
+            q = pts[i].cpu().numpy()
+            ref = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, q, want_abs=True)
+            check(ref, res["overlap"][0][i, :sizes[i]], res["overlap"][1][i, :sizes[i]], tol)
+    finally:
+        B.qmmm_field_destroy(h)
+
+
 # ------------------------------------------ config 2 on the device: warp-private grid walks
 @pytest.mark.parametrize("precision,tol", [("fp64", TOL64), ("fp32", TOL32)])
 def test_config2_single_point_device_evaluations(torch_cuda, B, oracle_mod, precision, tol):
