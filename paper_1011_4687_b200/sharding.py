@@ -1,12 +1,20 @@
-"""Walker sharding across GPUs (the paper's own scaling, PAPER.md:203-205,
-Table V: independent walkers on MPI ranks, one GPU each, no communication in the data path).
+"""Sharding across GPUs.
 
-Every rank holds a replica of the environment (<= 802 MB for the largest configuration) and
-evaluates a contiguous block of walkers.  There is NO collective in the hot path; the only
-communication is the optional gather of the results (4 doubles per point), done with
-``torch.distributed`` (NCCL on GPUs, gloo in the CPU tests).  This module holds none of the
-method's arithmetic: the evaluation itself is the callable passed in (on a GPU:
-``FieldEvaluator.eval``).
+By walkers (the paper's own scaling, Table V: independent walkers on MPI
+ranks, one GPU each, no communication in the data path): every rank holds a replica of the
+environment (<= 802 MB for the largest configuration) and evaluates a contiguous block of
+walkers.  There is NO collective in the hot path; the only communication is the optional
+gather of the results (4 doubles per point).
+
+By sources (Eq. 5-6 across devices: U = B[1] + ... + B[N_B] with one block
+per GPU), for environments that do not fit one GPU: every rank holds a contiguous range of the
+cells (the nuclei go to rank 0), evaluates ALL points against it, and the per-rank partial
+{V, E} are exchanged once (4 doubles per point) and added in RANK ORDER on every rank, so the
+result is deterministic and identical on all ranks (a tree all-reduce would not fix the order).
+
+Communication is ``torch.distributed`` (NCCL on GPUs, gloo in the CPU tests).  This module
+holds none of the method's arithmetic beyond that fixed-order sum of partials: the evaluation
+itself is the callable passed in (on a GPU: ``FieldEvaluator.eval``).
 """
 from __future__ import annotations
 
@@ -56,3 +64,32 @@ def eval_sharded(evaluate: Callable, elec_xyz: torch.Tensor, rank: int, world: i
     parts = [out[r][:walker_shard(W, r, world)[1]] for r in range(world)]
     full = torch.cat(parts, dim=0)
     return full[..., 0].contiguous(), full[..., 1:].contiguous()
+
+
+def source_shard(M: int, rank: int, world: int) -> Tuple[int, int]:
+    """(first cell, number of cells) of ``rank``: contiguous, balanced to within one."""
+    return walker_shard(M, rank, world)
+
+
+def eval_source_sharded(evaluate_local: Callable, elec_xyz: torch.Tensor, rank: int, world: int,
+                        group=None):
+    """V, E at ``elec_xyz`` [P, 3] from an environment whose cells are split over the ranks.
+
+    ``evaluate_local(pts [P, 3]) -> (V [P], E [P, 3])`` is this rank's partial: the sum over
+    ITS cells (rank 0 also owns the nuclei).  Every rank returns the full sums, bitwise the
+    same on all ranks: the partials are gathered and added in rank order 0, 1, 2, ...
+    """
+    V_loc, E_loc = evaluate_local(elec_xyz)
+    if world == 1:
+        return V_loc, E_loc
+    import torch.distributed as dist
+    P = int(elec_xyz.shape[0])
+    buf = elec_xyz.new_empty((P, 4))
+    buf[:, 0] = V_loc
+    buf[:, 1:] = E_loc
+    out = [torch.empty_like(buf) for _ in range(world)]
+    dist.all_gather(out, buf, group=group)
+    total = out[0].clone()
+    for r in range(1, world):              # fixed order: deterministic, identical everywhere
+        total += out[r]
+    return total[:, 0].contiguous(), total[:, 1:].contiguous()
