@@ -513,7 +513,14 @@ def run_ours(args):
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
                          "frac": achieved / peak_tf, "traffic": traffic,
                          "kernel": KERNEL[(layout, prec)], "kernel_ms": pair_s * 1e3,
-                         "slots_per_pair": slots,
+                         "slots_per_pair": slots, "dz_table": bool(info.get("last_dz_table")),
+                         # the same launch against SURVEY.md 8(d)'s fixed per-pair figure (17 FP32 /
+                         # 18 FP64 slots: list of positions, per-pair refinement); above 1 when the
+                         # kernel needs fewer operations than that formulation
+                         "frac_at_survey_slots": P * w.M * (17 if prec == "fp32" else 18) / pair_s / peak_lane,
+                         # one MUFU (RSQ / RSQ64H) per pair against the measured MUFU rate: the
+                         # co-limiter of the FP32 grid kernel
+                         "xu_frac": P * w.M / pair_s / (0.5 * (peaks0["mufu_lane_ops_per_s"] + peaks1["mufu_lane_ops_per_s"])),
                          "definition": "pairs x slots x 2 / pair-kernel time vs 2 x FMA lane rate of "
                                        "the same-run microbenchmark (qmmm_probe_peak)",
                          "peak_source": "measured, same process (mean of before/after)",
