@@ -516,6 +516,42 @@ def test_eval_is_cuda_graph_capturable(torch_cuda, B, layout, precision):
         B.qmmm_field_destroy(h)
 
 
+# --------------------------------------------------------- dz table and its fallback
+@pytest.mark.parametrize("nz,P,precision,tol,table", [
+    (64, 128, "fp32", TOL32, True), (130, 128, "fp32", TOL32, True), (400, 128, "fp32", TOL32, False),
+    (64, 128, "fp64", TOL64, True), (300, 128, "fp64", TOL64, True), (600, 128, "fp64", TOL64, False),
+    (64, 8, "fp32", TOL32, False), (64, 3, "fp64", TOL64, False)])
+def test_dz_table_and_stepped_dz_kernels(torch_cuda, B, oracle_mod, nz, P, precision, tol, table):
+    """The batched grid kernels tabulate dz = u_z - k per CTA in shared memory when the table
+    fits (qmmm_field_info.last_dz_table) and step it per pair otherwise (long z axes; few-point
+    plans): both against the oracle, on z extents with ragged last gchunks."""
+    n = (9, 8, nz)
+    h = 0.25
+    rng = np.random.default_rng(1000 + nz + P)
+    origin = np.array([-1.0, -0.9, -0.5 * h * (nz - 1)]) + rng.normal(size=3) * 0.1
+    centre = origin + 0.5 * h * (np.array(n) - 1)
+    # FP32: the point coordinates live on a lattice of 2^-24 of the axis extent and only V gets
+    # the first-order correction for the residual (DESIGN.md section 6), so the relative error
+    # of E grows with (nodes along the axis) / (distance to the nearest cell in nodes): keep
+    # the points four cells away from the cells, as the BASELINE configurations do
+    dense, pos, q = random_grid(rng, n, h, origin, fill=0.8, hole=(centre, 1.6))
+    nuc = centre + np.array([3.0, -2.5, 4.0]) + rng.normal(size=(4, 3))
+    Z = np.array([1.0, 6.0, 7.0, 8.0])
+    pts = centre + rng.normal(size=(P, 3)) * 0.3
+    pts = centre + (pts - centre) * np.minimum(1.0, 0.6 / np.linalg.norm(pts - centre, axis=1))[:, None]
+    ref = oracle_mod.field(pos, q, nuc, Z, pts, want_abs=True)
+    hnd = B.qmmm_field_create_grid(origin, h, n, dense, nuc, Z, P)
+    try:
+        V, E = run(torch_cuda, B, hnd, pts, precision)
+        assert bool(B.qmmm_field_get_info(hnd)["last_dz_table"]) == table
+        check(ref, V, E, tol)
+        if precision == "fp64":                                   # potential only
+            V0, _ = run(torch_cuda, B, hnd, pts, precision, want_E=False)
+            check(ref, V0, None, tol)
+    finally:
+        B.qmmm_field_destroy(hnd)
+
+
 # ----------------------------------------------- overlapped back-to-back evaluations (PDL)
 @pytest.mark.parametrize("layout,precision", [("grid", "fp32"), ("grid", "fp64"), ("list", "fp32"), ("list", "fp64")])
 @pytest.mark.parametrize("P", [1, 4, 32])
