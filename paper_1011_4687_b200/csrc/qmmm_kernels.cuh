@@ -61,6 +61,7 @@ struct PairParams {
     double g_scaleV, g_scaleE;   // 1/hz, 1/hz^2
     int g_n[3], g_segs;      // nodes per axis (row = ix * ny + iy); z segments (gchunks) per row tile
     int g_dzt;               // grid kernels: dz table in shared memory (qmmm_grid.cuh, DZT)
+    int g_light;             // host side only: FP64 grid kernel with 4 consumer warps (overlapped few-point evaluations)
     int pdl;                 // host side only: launch with programmatic stream serialization
 #ifdef QMMM_PHASE_TIMING
     long long *dbg;          // [CTAs][10] clock64 at phase boundaries + globaltimer (diagnostic build)

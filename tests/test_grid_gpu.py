@@ -560,8 +560,8 @@ def test_overlapped_back_to_back_evaluations_are_bitwise_the_same(torch_cuda, B,
     """qmmm_field_set_overlap: evaluation n + 1 starts while evaluation n is still running
     (programmatic dependent launch) and waits for it only before it touches the workspace, the
     tickets and the outputs.  300 evaluations of changing batch size in one stream -- every one
-    reuses the same workspace and tickets -- give bitwise the results of the serial launches,
-    eagerly and replayed from a CUDA graph; a sample is checked against the oracle."""
+    reuses the same workspace and tickets -- give bitwise the results of the serial launches
+    (same plan), eagerly and replayed from a CUDA graph; a sample is checked against the oracle."""
     torch = torch_cuda
     w = make_workload(1)
     rng = np.random.default_rng(11)
@@ -588,9 +588,16 @@ def test_overlapped_back_to_back_evaluations_are_bitwise_the_same(torch_cuda, B,
                     B.qmmm_field_eval(h, p, 1, sizes[i], V[i, :sizes[i]], E[i, :sizes[i]], precision)
             torch.cuda.synchronize()
             res[mode] = (V.cpu().numpy(), E.cpu().numpy())
-        for mode in ("overlap", "graph"):
-            assert np.array_equal(res[mode][0], res["serial"][0], equal_nan=True), mode
-            assert np.array_equal(res[mode][1], res["serial"][1], equal_nan=True), mode
+        assert np.array_equal(res["graph"][0], res["overlap"][0], equal_nan=True)
+        assert np.array_equal(res["graph"][1], res["overlap"][1], equal_nan=True)
+        if layout == "grid" and precision == "fp64" and P == 32:
+            # overlapped few-point FP64 grid evaluations run 4-warp CTAs (two evaluations share
+            # an SM): another split of the z runs, so the sums agree to rounding, not bitwise
+            assert np.allclose(res["overlap"][0], res["serial"][0], rtol=1e-12, atol=0, equal_nan=True)
+            assert np.allclose(res["overlap"][1], res["serial"][1], rtol=0, atol=1e-12 * np.nanmax(np.abs(res["serial"][1])), equal_nan=True)
+        else:
+            assert np.array_equal(res["overlap"][0], res["serial"][0], equal_nan=True)
+            assert np.array_equal(res["overlap"][1], res["serial"][1], equal_nan=True)
         tol = TOL64 if precision == "fp64" else TOL32
         for i in (0, 1, 150, n - 1):
             q = pts[i].cpu().numpy()
