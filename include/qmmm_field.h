@@ -260,9 +260,11 @@ qmmm_status qmmm_field_set_timing(qmmm_field *h, int enable);
  * kernel in the stream -- the previous evaluation -- is still running, does its prologue,
  * source walk and in-CTA reduction, and waits for the predecessor to finish (griddepcontrol)
  * only before it touches the partials workspace, the tickets or V / E.  Results are bitwise
- * the same as without overlap for the same launch plan; the one plan that changes is the FP64
- * grid kernel for 5..64 points, which runs 4-warp instead of 8-warp CTAs so that two
- * evaluations share an SM (another association of the same sums: equal to rounding).
+ * the same as without overlap for the same launch plan.  The plans that change are the
+ * few-point grid kernels (up to 64 points), which run 4-warp instead of
+ * 8-warp CTAs so that several evaluations share an SM -- the period of a sequence is a CTA's
+ * lifetime divided by the CTAs an SM holds -- i.e. another association of the same sums:
+ * equal to rounding, and still deterministic from run to run.
  * Precondition while enabled: elec_xyz of an evaluation is not produced by the evaluation
  * immediately before it on the same stream (it is read before the wait); work of other
  * libraries in between serialises as usual.  Ignored (plain serialization) while timing is on

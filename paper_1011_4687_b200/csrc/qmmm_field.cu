@@ -87,26 +87,39 @@ constexpr int GRID_NW_EPT8 = 8, GRID_NW_EPT4 = QMMM_GRID_NW_EPT4, GRID_NW_EPT2 =
 #endif
 constexpr int GRID64_NW_EPT4 = QMMM_GRID64_NW_EPT4, GRID64_NW_EPT2 = 16, GRID64_NW_EPT1 = 16;
 // a handful of points (one point group): every warp loads and walks whole gchunks of its own
-constexpr int GRID64_NW_WARPOWN = 8;
+#ifndef QMMM_GRID64_NW_WARPOWN
+#define QMMM_GRID64_NW_WARPOWN 8
+#endif
+constexpr int GRID64_NW_WARPOWN = QMMM_GRID64_NW_WARPOWN;
 bool grid_f64_warpown(int ept, int64_t P) { return P <= ept; }
-// "light" CTAs for overlapped few-point evaluations (qmmm_field_set_overlap): 4 consumer warps
-// + producer = 160 threads x <= 168 registers, so that the CTAs of two consecutive evaluations
-// share an SM (the 8-warp CTA fills the register file alone and the next evaluation could not
-// start before it exits).  Config 1 FP64, 200 overlapped evaluations: 13.8 -> 9.5 us each.
-constexpr int GRID64_NW_LIGHT = 4;
+// "Light" CTAs for overlapped few-point evaluations (qmmm_field_set_overlap).  With overlap,
+// the CTAs of consecutive evaluations share the SMs and the steady-state period of a sequence
+// is (lifetime of a CTA, waiting included) / (CTAs an SM holds), until the serial tail bounds
+// it: smaller CTAs win although a single evaluation gets slower.  4 warps instead of 8
+// (measured per overlapped evaluation, 1,000 replayed from one graph): config 2 FP32
+// 5.7 -> 3.7 us, FP64 6.9 -> 3.6 us; config 1 FP64 13.8 -> 9.5 us (2 warps: 3.5 / 3.8 us).
+constexpr int GRID64_NW_LIGHT = 4, GRID64_NW_WARPOWN_LIGHT = 4, GRID_NW_NODEPACK_LIGHT = 4;
 bool grid_f64_light(bool overlap, int ept, int64_t P) {
-    return overlap && ept == 4 && !grid_f64_warpown(ept, P) && P <= 64;
+    return overlap && (grid_f64_warpown(ept, P) || (ept == 4 && P <= 64));
 }
 int grid_f64_warps(int ept, int64_t P, bool light) {
-    if (grid_f64_warpown(ept, P)) return GRID64_NW_WARPOWN;
+    if (grid_f64_warpown(ept, P)) return light ? GRID64_NW_WARPOWN_LIGHT : GRID64_NW_WARPOWN;
     if (light) return GRID64_NW_LIGHT;
     return ept == 4 ? GRID64_NW_EPT4 : (ept == 2 ? GRID64_NW_EPT2 : GRID64_NW_EPT1);
 }
 // one or two points per evaluation: the node-packed kernel, 8 warps, two CTAs per SM
-constexpr int GRID_NW_NODEPACK = 8;
+#ifndef QMMM_GRID_NW_NODEPACK
+#define QMMM_GRID_NW_NODEPACK 8
+#endif
+constexpr int GRID_NW_NODEPACK = QMMM_GRID_NW_NODEPACK;
 bool grid_f32_nodepack(int ept, int64_t P) { return ept == 2 && P <= 2; }
-int grid_f32_warps(int ept, int64_t P) {
-    if (grid_f32_nodepack(ept, P)) return GRID_NW_NODEPACK;
+constexpr int GRID_NW_EPT4_LIGHT = 4;
+bool grid_f32_light(bool overlap, int ept, int64_t P) {
+    return overlap && (grid_f32_nodepack(ept, P) || (ept == 4 && P <= 64));
+}
+int grid_f32_warps(int ept, int64_t P, bool light) {
+    if (grid_f32_nodepack(ept, P)) return light ? GRID_NW_NODEPACK_LIGHT : GRID_NW_NODEPACK;
+    if (light && ept == 4) return GRID_NW_EPT4_LIGHT;
     return ept == 8 ? GRID_NW_EPT8 : (ept == 4 ? GRID_NW_EPT4 : GRID_NW_EPT2);
 }
 // dz table of the FP64 grid kernel (4 points per thread, shared stages): [z nodes padded to
@@ -119,7 +132,7 @@ int grid_f32_warps(int ept, int64_t P) {
 #endif
 size_t grid_dzt_bytes(bool f32, int ept, int wp, int64_t P, int64_t g_segs) {
     if (f32) {      // 4 points per thread, every warp its own point group (the FULL kernel)
-        if (!QMMM_GRID_F32_DZT || ept != 4 || wp != GRID_NW_EPT4 || g_segs > 4096) return 0;
+        if (!QMMM_GRID_F32_DZT || ept != 4 || wp != GRID_NW_EPT4 || g_segs > 4096) return 0;   // (light CTAs: wp <= 4)
         return GridF32Layout<2, GRID_NW_EPT4>::dzt_bytes(static_cast<int>(g_segs));
     }
     if (!QMMM_GRID_F64_DZT || ept != 4 || grid_f64_warpown(ept, P)) return 0;
@@ -127,11 +140,13 @@ size_t grid_dzt_bytes(bool f32, int ept, int wp, int64_t P, int64_t g_segs) {
 }
 size_t grid_smem_bytes(bool f32, int stages, int ept, int wp, int64_t P, bool light) {
     if (f32 && ept == 8) return GridF32Layout<4, GRID_NW_EPT8>::total(stages);
-    if (f32 && ept == 4) return GridF32Layout<2, GRID_NW_EPT4>::total(stages);
+    if (f32 && ept == 4)
+        return light ? GridF32Layout<2, GRID_NW_EPT4_LIGHT>::total(stages) : GridF32Layout<2, GRID_NW_EPT4>::total(stages);
     if (f32 && grid_f32_nodepack(ept, P))       // warp-private pipelines: two slots per warp
-        return GridF32Layout<1, GRID_NW_NODEPACK>::total(2 * GRID_NW_NODEPACK);
+        return light ? GridF32Layout<1, GRID_NW_NODEPACK_LIGHT>::total(2 * GRID_NW_NODEPACK_LIGHT)
+                     : GridF32Layout<1, GRID_NW_NODEPACK>::total(2 * GRID_NW_NODEPACK);
     if (f32) return GridF32Layout<1, GRID_NW_EPT2>::total(stages);
-    if (grid_f64_warpown(ept, P)) stages = GRID64_NW_WARPOWN;      // one private slot per warp
+    if (grid_f64_warpown(ept, P)) stages = grid_f64_warps(ept, P, light);   // one private slot per warp
     return static_cast<size_t>(stages) * GRID_STAGE_BYTES_F64 + 18 * sizeof(uint64_t) +
            static_cast<size_t>(32) * grid_f64_warps(ept, P, light) * sizeof(double) +
            static_cast<size_t>(wp) * ept * 3 * sizeof(double);
@@ -204,8 +219,9 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32, bool grid = fals
     pl.points_per_thread = std::min(pl.points_per_thread, max_ept);
     if (grid && f32) pl.points_per_thread = std::max(pl.points_per_thread, 2);   // packed pairs only
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
-    const bool light = grid && !f32 && grid_f64_light(h->overlap, pl.points_per_thread, P);
-    const int nw = grid ? (f32 ? grid_f32_warps(pl.points_per_thread, P) : grid_f64_warps(pl.points_per_thread, P, light))
+    const bool light = grid && (f32 ? grid_f32_light(h->overlap, pl.points_per_thread, P)
+                                    : grid_f64_light(h->overlap, pl.points_per_thread, P));
+    const int nw = grid ? (f32 ? grid_f32_warps(pl.points_per_thread, P, light) : grid_f64_warps(pl.points_per_thread, P, light))
                         : ((f32 && pl.points_per_thread >= 2) ? f32x2_warps(pl.points_per_thread) : COMPUTE_WARPS);
     if (pl.point_warps == 0) {
         // as many point warps as there are groups, but keep at least 4 point blocks when the
@@ -259,7 +275,7 @@ bool auto_uses_grid(const qmmm_field *h, int64_t P, bool f32) {
     if (h->n_g < static_cast<int64_t>(2) * pl.slices) return false;
     if (f32 && grid_f32_nodepack(pl.points_per_thread, P)) return true;     // single-point walk
     if (!f32 && grid_f64_warpown(pl.points_per_thread, P)) return true;     // warp-private gchunks
-    const int nw = f32 ? grid_f32_warps(pl.points_per_thread, P)
+    const int nw = f32 ? grid_f32_warps(pl.points_per_thread, P, grid_f32_light(h->overlap, pl.points_per_thread, P))
                        : grid_f64_warps(pl.points_per_thread, P, grid_f64_light(h->overlap, pl.points_per_thread, P));
     return nw / pl.point_warps <= 4;
 }
@@ -372,21 +388,31 @@ cudaError_t launch_grid_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
     if (f32) {
         switch (ept) {
             case 2:
-                if (grid_f32_nodepack(2, prm.P)) return launch_grid_f32<1, GRID_NW_NODEPACK, true>(prm, grid, smem, st);
+                if (grid_f32_nodepack(2, prm.P))
+                    return prm.g_light ? launch_grid_f32<1, GRID_NW_NODEPACK_LIGHT, true>(prm, grid, smem, st)
+                                       : launch_grid_f32<1, GRID_NW_NODEPACK, true>(prm, grid, smem, st);
                 return launch_grid_f32<1, GRID_NW_EPT2>(prm, grid, smem, st);
-            case 4: return launch_grid_f32<2, GRID_NW_EPT4>(prm, grid, smem, st);
+            case 4:
+                if (prm.g_light) return launch_grid_f32<2, GRID_NW_EPT4_LIGHT>(prm, grid, smem, st);
+                return launch_grid_f32<2, GRID_NW_EPT4>(prm, grid, smem, st);
             case 8: return launch_grid_f32<4, GRID_NW_EPT8>(prm, grid, smem, st);
         }
     } else if (prm.E) {
         switch (ept) {
             case 1:
-                if (grid_f64_warpown(1, prm.P)) return launch_grid_f64<1, true, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
+                if (grid_f64_warpown(1, prm.P))
+                    return prm.g_light ? launch_grid_f64<1, true, GRID64_NW_WARPOWN_LIGHT, true>(prm, grid, smem, st)
+                                       : launch_grid_f64<1, true, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
                 return launch_grid_f64<1, true, GRID64_NW_EPT1>(prm, grid, smem, st);
             case 2:
-                if (grid_f64_warpown(2, prm.P)) return launch_grid_f64<2, true, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
+                if (grid_f64_warpown(2, prm.P))
+                    return prm.g_light ? launch_grid_f64<2, true, GRID64_NW_WARPOWN_LIGHT, true>(prm, grid, smem, st)
+                                       : launch_grid_f64<2, true, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
                 return launch_grid_f64<2, true, GRID64_NW_EPT2>(prm, grid, smem, st);
             case 4:
-                if (grid_f64_warpown(4, prm.P)) return launch_grid_f64<4, true, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
+                if (grid_f64_warpown(4, prm.P))
+                    return prm.g_light ? launch_grid_f64<4, true, GRID64_NW_WARPOWN_LIGHT, true>(prm, grid, smem, st)
+                                       : launch_grid_f64<4, true, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
                 if (prm.g_light)
                     return prm.g_dzt ? launch_grid_f64<4, true, GRID64_NW_LIGHT, false, true>(prm, grid, smem, st)
                                      : launch_grid_f64<4, true, GRID64_NW_LIGHT>(prm, grid, smem, st);
@@ -396,13 +422,19 @@ cudaError_t launch_grid_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
     } else {
         switch (ept) {
             case 1:
-                if (grid_f64_warpown(1, prm.P)) return launch_grid_f64<1, false, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
+                if (grid_f64_warpown(1, prm.P))
+                    return prm.g_light ? launch_grid_f64<1, false, GRID64_NW_WARPOWN_LIGHT, true>(prm, grid, smem, st)
+                                       : launch_grid_f64<1, false, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
                 return launch_grid_f64<1, false, GRID64_NW_EPT1>(prm, grid, smem, st);
             case 2:
-                if (grid_f64_warpown(2, prm.P)) return launch_grid_f64<2, false, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
+                if (grid_f64_warpown(2, prm.P))
+                    return prm.g_light ? launch_grid_f64<2, false, GRID64_NW_WARPOWN_LIGHT, true>(prm, grid, smem, st)
+                                       : launch_grid_f64<2, false, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
                 return launch_grid_f64<2, false, GRID64_NW_EPT2>(prm, grid, smem, st);
             case 4:
-                if (grid_f64_warpown(4, prm.P)) return launch_grid_f64<4, false, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
+                if (grid_f64_warpown(4, prm.P))
+                    return prm.g_light ? launch_grid_f64<4, false, GRID64_NW_WARPOWN_LIGHT, true>(prm, grid, smem, st)
+                                       : launch_grid_f64<4, false, GRID64_NW_WARPOWN, true>(prm, grid, smem, st);
                 if (prm.g_light)
                     return prm.g_dzt ? launch_grid_f64<4, false, GRID64_NW_LIGHT, false, true>(prm, grid, smem, st)
                                      : launch_grid_f64<4, false, GRID64_NW_LIGHT>(prm, grid, smem, st);
@@ -1140,7 +1172,8 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
     const int pb = static_cast<int>((groups + pl.point_warps - 1) / pl.point_warps);
     int launches = 0;
-    const bool light = grid && !f32 && grid_f64_light(h->overlap, pl.points_per_thread, P);
+    const bool light = grid && (f32 ? grid_f32_light(h->overlap, pl.points_per_thread, P)
+                                    : grid_f64_light(h->overlap, pl.points_per_thread, P));
     auto smem_of = [&](int stages) {
         return grid ? grid_smem_bytes(f32, stages, pl.points_per_thread, pl.point_warps, P, light)
                     : pair_smem_bytes(f32, stages, pl.points_per_thread, pl.point_warps);

@@ -590,11 +590,14 @@ def test_overlapped_back_to_back_evaluations_are_bitwise_the_same(torch_cuda, B,
             res[mode] = (V.cpu().numpy(), E.cpu().numpy())
         assert np.array_equal(res["graph"][0], res["overlap"][0], equal_nan=True)
         assert np.array_equal(res["graph"][1], res["overlap"][1], equal_nan=True)
-        if layout == "grid" and precision == "fp64" and P == 32:
-            # overlapped few-point FP64 grid evaluations run 4-warp CTAs (two evaluations share
-            # an SM): another split of the z runs, so the sums agree to rounding, not bitwise
-            assert np.allclose(res["overlap"][0], res["serial"][0], rtol=1e-12, atol=0, equal_nan=True)
-            assert np.allclose(res["overlap"][1], res["serial"][1], rtol=0, atol=1e-12 * np.nanmax(np.abs(res["serial"][1])), equal_nan=True)
+        if layout == "grid":
+            # overlapped few-point grid evaluations run 4-warp CTAs (several evaluations share an
+            # SM): another split of the z runs / gchunks over the warps, so the sums agree with
+            # the serial launches to rounding (of the arithmetic type), not bitwise
+            rt = 1e-12 if precision == "fp64" else 2e-6
+            assert np.allclose(res["overlap"][0], res["serial"][0], rtol=rt, atol=0, equal_nan=True)
+            assert np.allclose(res["overlap"][1], res["serial"][1], rtol=0,
+                               atol=rt * np.nanmax(np.abs(res["serial"][1])), equal_nan=True)
         else:
             assert np.array_equal(res["overlap"][0], res["serial"][0], equal_nan=True)
             assert np.array_equal(res["overlap"][1], res["serial"][1], equal_nan=True)
