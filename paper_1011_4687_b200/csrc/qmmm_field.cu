@@ -130,10 +130,12 @@ int grid_f32_warps(int ept, int64_t P, bool light) {
 #ifndef QMMM_GRID_F32_DZT
 #define QMMM_GRID_F32_DZT 1
 #endif
-size_t grid_dzt_bytes(bool f32, int ept, int wp, int64_t P, int64_t g_segs) {
+size_t grid_dzt_bytes(bool f32, int ept, int wp, int64_t P, int64_t g_segs, bool light) {
     if (f32) {      // 4 points per thread, every warp its own point group (the FULL kernel)
-        if (!QMMM_GRID_F32_DZT || ept != 4 || wp != GRID_NW_EPT4 || g_segs > 4096) return 0;   // (light CTAs: wp <= 4)
-        return GridF32Layout<2, GRID_NW_EPT4>::dzt_bytes(static_cast<int>(g_segs));
+        if (!QMMM_GRID_F32_DZT || ept != 4 || g_segs > 4096) return 0;
+        if (wp != (light ? GRID_NW_EPT4_LIGHT : GRID_NW_EPT4)) return 0;
+        return light ? GridF32Layout<2, GRID_NW_EPT4_LIGHT>::dzt_bytes(static_cast<int>(g_segs))
+                     : GridF32Layout<2, GRID_NW_EPT4>::dzt_bytes(static_cast<int>(g_segs));
     }
     if (!QMMM_GRID_F64_DZT || ept != 4 || grid_f64_warpown(ept, P)) return 0;
     return static_cast<size_t>(g_segs) * GRID_ZS * wp * ept * sizeof(double);
@@ -228,11 +230,21 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32, bool grid = fals
         // points allow it: slices = SMs / 4 then, so every CTA streams a 4x longer source run
         // through its TMA ring and the last CTA adds 4x fewer partials per point
         int pw = std::min<int>(nw, pow2_ceil(groups));
-        while (pw > 1 && (groups + pw - 1) / pw < 4) pw >>= 1;
+        // (overlapped few-point evaluations: the SMs are filled by several evaluations in
+        // flight, not by one, so a CTA takes as many point groups as it has warps)
+        while (!light && pw > 1 && (groups + pw - 1) / pw < 4) pw >>= 1;
         pl.point_warps = pw;
     }
     if (pl.point_warps > nw) pl.point_warps = nw;
     const int64_t pb = (groups + pl.point_warps - 1) / pl.point_warps;
+    if (pl.slices == 0 && light) {
+        // Overlapped evaluations: fewer, longer CTAs -- half an SM count per evaluation for
+        // the single-group walks, a quarter otherwise (measured, 200-1,000 evaluations replayed
+        // from one graph: config 2 3.6 -> 3.0 us FP32, 3.7 -> 3.4 us FP64; config 1 4.0 -> 3.4 us
+        // FP32, 9.4 -> 7.3 us FP64 = 73 % of the DFMA peak); a single evaluation gets slower.
+        const bool single = f32 ? grid_f32_nodepack(pl.points_per_thread, P) : grid_f64_warpown(pl.points_per_thread, P);
+        pl.slices = static_cast<int>(std::max<int64_t>(1, (h->sm_count / (single ? 2 : 4)) / pb));
+    }
     if (pl.slices == 0) {
         const int g = gcd_int(static_cast<int>(pb % h->sm_count), h->sm_count);
         pl.slices = h->sm_count / g;       // pb * slices is a multiple of the SM count
@@ -354,7 +366,7 @@ cudaError_t launch_pair_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
 template <int EP2, int NW, bool NODEPACK = false, bool FULL = false, bool DZT = false>
 cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
     if constexpr (!NODEPACK && !FULL) {            // every warp its own point group: no z split
-        if constexpr (EP2 == 2 && NW == GRID_NW_EPT4) {
+        if constexpr (EP2 == 2 && (NW == GRID_NW_EPT4 || NW == GRID_NW_EPT4_LIGHT)) {
             if (prm.point_warps == NW && prm.g_dzt)
                 return launch_grid_f32<EP2, NW, false, true, true>(prm, grid, smem, st);
         }
@@ -1183,9 +1195,9 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
         smem = smem_of(--pl.stages);
     if (smem > 227 * 1024) return fail(QMMM_ERR_INVALID_ARG, "eval: plan exceeds shared memory");
     // grid kernels: dz table when it fits beside the stages (long z axes keep the stepped dz)
-    const size_t dzt = grid ? grid_dzt_bytes(f32, pl.points_per_thread, pl.point_warps, P, h->g_segs) : 0;
+    const size_t dzt = grid ? grid_dzt_bytes(f32, pl.points_per_thread, pl.point_warps, P, h->g_segs, light) : 0;
     // (the FP32 kernel runs two CTAs per SM: half the budget each)
-    const bool use_dzt = dzt > 0 && smem + dzt <= (f32 ? 110 : 200) * 1024;
+    const bool use_dzt = dzt > 0 && smem + dzt <= (f32 ? (light ? 56 : 110) : 200) * 1024;
     if (use_dzt) smem += dzt;
 
     if (h->timing) CUDA_TRY(cudaEventRecord(h->ev[0], st));
