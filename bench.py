@@ -375,8 +375,12 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                     torch.cuda.synchronize()
                     B.qmmm_field_set_overlap(h, False)
                     us = e0.elapsed_time(e1) * 1e3 / 200
+                    info_o = B.qmmm_field_get_info(h)       # the overlapped plan (light CTAs) and its kernel
+                    slots_o = slots_for(layout, prec, info_o)
                     row["us_per_eval_200_cuda_graph_overlap"] = us
-                    row["fma_pipe_frac_cuda_graph_overlap"] = pairs * slots / (us * 1e-6) / peak
+                    row["slots_per_pair_overlap"] = slots_o
+                    row["plan_overlap"] = info_o["last_plan"]
+                    row["fma_pipe_frac_cuda_graph_overlap"] = pairs * slots_o / (us * 1e-6) / peak
                     del gr
                 out.append(row)
                 if prec == "fp64" and not w.sequential and idx in (1, 4):

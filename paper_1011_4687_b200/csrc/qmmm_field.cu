@@ -185,6 +185,7 @@ struct qmmm_field {
     int last_point_blocks = 0, last_launches = 0, last_dz_table = 0;
     bool timing = false, timed = false;
     bool overlap = false;          // qmmm_field_set_overlap: back-to-back evaluations may overlap
+    bool overlap_now = false;      // ... and this evaluation is launched that way (not timed, no mailbox)
     cudaEvent_t ev[2] = {nullptr, nullptr};
     // per-move mailbox: pinned, device-mapped host memory (elec in; V, E and a sequence flag out)
     double *mail_h = nullptr, *mail_d = nullptr;   // [MAIL_POINTS*3 | MAIL_POINTS*4 | flag]
@@ -221,8 +222,8 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32, bool grid = fals
     pl.points_per_thread = std::min(pl.points_per_thread, max_ept);
     if (grid && f32) pl.points_per_thread = std::max(pl.points_per_thread, 2);   // packed pairs only
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
-    const bool light = grid && (f32 ? grid_f32_light(h->overlap, pl.points_per_thread, P)
-                                    : grid_f64_light(h->overlap, pl.points_per_thread, P));
+    const bool light = grid && (f32 ? grid_f32_light(h->overlap_now, pl.points_per_thread, P)
+                                    : grid_f64_light(h->overlap_now, pl.points_per_thread, P));
     const int nw = grid ? (f32 ? grid_f32_warps(pl.points_per_thread, P, light) : grid_f64_warps(pl.points_per_thread, P, light))
                         : ((f32 && pl.points_per_thread >= 2) ? f32x2_warps(pl.points_per_thread) : COMPUTE_WARPS);
     if (pl.point_warps == 0) {
@@ -287,8 +288,8 @@ bool auto_uses_grid(const qmmm_field *h, int64_t P, bool f32) {
     if (h->n_g < static_cast<int64_t>(2) * pl.slices) return false;
     if (f32 && grid_f32_nodepack(pl.points_per_thread, P)) return true;     // single-point walk
     if (!f32 && grid_f64_warpown(pl.points_per_thread, P)) return true;     // warp-private gchunks
-    const int nw = f32 ? grid_f32_warps(pl.points_per_thread, P, grid_f32_light(h->overlap, pl.points_per_thread, P))
-                       : grid_f64_warps(pl.points_per_thread, P, grid_f64_light(h->overlap, pl.points_per_thread, P));
+    const int nw = f32 ? grid_f32_warps(pl.points_per_thread, P, grid_f32_light(h->overlap_now, pl.points_per_thread, P))
+                       : grid_f64_warps(pl.points_per_thread, P, grid_f64_light(h->overlap_now, pl.points_per_thread, P));
     return nw / pl.point_warps <= 4;
 }
 
@@ -1178,14 +1179,17 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
         if (ss != QMMM_OK) return ss;
     }
 
+    // overlapped launch (and the few-point plans that go with it): not between timing events,
+    // not for the mailbox path, whose host reads V and E behind a flag
+    h->overlap_now = h->overlap && !h->timing && !host_flag;
     const bool grid = h->layout == QMMM_LAYOUT_GRID ||
                       (h->layout == QMMM_LAYOUT_AUTO && auto_uses_grid(h, P, f32));
     qmmm_plan pl = choose_plan(h, P, f32, grid);
     const int64_t groups = (P + pl.points_per_thread - 1) / pl.points_per_thread;
     const int pb = static_cast<int>((groups + pl.point_warps - 1) / pl.point_warps);
     int launches = 0;
-    const bool light = grid && (f32 ? grid_f32_light(h->overlap, pl.points_per_thread, P)
-                                    : grid_f64_light(h->overlap, pl.points_per_thread, P));
+    const bool light = grid && (f32 ? grid_f32_light(h->overlap_now, pl.points_per_thread, P)
+                                    : grid_f64_light(h->overlap_now, pl.points_per_thread, P));
     auto smem_of = [&](int stages) {
         return grid ? grid_smem_bytes(f32, stages, pl.points_per_thread, pl.point_warps, P, light)
                     : pair_smem_bytes(f32, stages, pl.points_per_thread, pl.point_warps);
@@ -1218,7 +1222,7 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
         prm.done = h->counters + h->max_points;
         // overlap with the previous evaluation on this stream (not with the timing events in
         // between, and not for the mailbox path, whose host reads V and E behind a flag)
-        prm.pdl = (h->overlap && !h->timing && !host_flag) ? 1 : 0;
+        prm.pdl = h->overlap_now ? 1 : 0;
         if (grid) {
             // cells: charges only, coordinates from the indices; everything in grid units
             prm.chunks = f32 ? reinterpret_cast<const char *>(h->gcells32)
