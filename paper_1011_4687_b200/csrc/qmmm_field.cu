@@ -198,6 +198,9 @@ struct qmmm_field {
     int srv_prec = -1;
     unsigned long long srv_launch_id = 0, srv_seq = 0;
     int *counters = nullptr;       // [max_points] arrival tickets of the point blocks (zero at rest)
+    // push-model collection for overlapped few-point evaluations (qmmm_kernels.cuh): tagged records
+    unsigned long long *push_slots = nullptr;      // [PUSH_MAX_RECORDS][8] words, zero at create
+    unsigned long long push_seq = 0;               // tag of the last pushing evaluation
     // grid layout (qmmm_grid.cuh): present when the cells are nodes of a cubic grid
     bool has_list = true, has_grid = false;
     GridGeom grid = {{0, 0, 0}, {1.0, 1.0, 1.0}, {0, 0, 0}, 0.0};
@@ -292,6 +295,11 @@ bool auto_uses_grid(const qmmm_field *h, int64_t P, bool f32) {
                        : grid_f64_warps(pl.points_per_thread, P, grid_f64_light(h->overlap_now, pl.points_per_thread, P));
     return nw / pl.point_warps <= 4;
 }
+
+// records (slices x P) the push-model collection of a handle can hold; the collecting CTA
+// keeps slices x (points of a CTA) records of 32 bytes in its idle stage buffers
+constexpr int64_t PUSH_MAX_RECORDS = 4096;
+constexpr int64_t PUSH_MAX_CTA_RECORD_BYTES = 16384;
 
 // One evaluation kernel launch.  prm.pdl: programmatic stream serialization -- the kernel may
 // start while its predecessor in the stream is still running (qmmm_field_set_overlap; the
@@ -774,6 +782,8 @@ qmmm_status alloc_runtime(qmmm_field *h) {
     RT_TRY(cudaMalloc(&h->workspace, h->workspace_doubles * sizeof(double)));
     RT_TRY(cudaMalloc(&h->counters, (h->max_points + 1) * sizeof(int)));      // + 1: mailbox `done`
     RT_TRY(cudaMemset(h->counters, 0, (h->max_points + 1) * sizeof(int)));
+    RT_TRY(cudaMalloc(&h->push_slots, PUSH_MAX_RECORDS * PUSH_SLOT_WORDS * sizeof(unsigned long long)));
+    RT_TRY(cudaMemset(h->push_slots, 0, PUSH_MAX_RECORDS * PUSH_SLOT_WORDS * sizeof(unsigned long long)));
     RT_TRY(cudaHostAlloc(&h->mail_h, (MAIL_POINTS * 7 + 1) * sizeof(double), cudaHostAllocMapped));
     std::memset(h->mail_h, 0, (MAIL_POINTS * 7 + 1) * sizeof(double));
     RT_TRY(cudaHostGetDevicePointer(&h->mail_d, h->mail_h, 0));
@@ -1091,6 +1101,7 @@ qmmm_status qmmm_field_destroy(qmmm_field *h) {
     h->keep.reset();                // shared copies: freed with the last handle
     cudaFree(h->workspace);
     cudaFree(h->counters);
+    cudaFree(h->push_slots);
     if (h->mail_h) cudaFreeHost(h->mail_h);
     cudaFree(h->stage_elec);
     cudaFree(h->stage_out);
@@ -1223,6 +1234,13 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
         // overlap with the previous evaluation on this stream (not with the timing events in
         // between, and not for the mailbox path, whose host reads V and E behind a flag)
         prm.pdl = h->overlap_now ? 1 : 0;
+        // light (overlapped, few points, grid): collect the CTA partials by tagged records
+        // instead of fence + ticket -- the serial tail that bounds the period of a sequence
+        if (light && pl.points_per_thread <= 4 && static_cast<int64_t>(pl.slices) * P <= PUSH_MAX_RECORDS &&
+            static_cast<int64_t>(pl.slices) * pl.point_warps * pl.points_per_thread * 32 <= PUSH_MAX_CTA_RECORD_BYTES) {
+            prm.push_slots = h->push_slots;
+            prm.push_seq = ++h->push_seq;
+        }
         if (grid) {
             // cells: charges only, coordinates from the indices; everything in grid units
             prm.chunks = f32 ? reinterpret_cast<const char *>(h->gcells32)

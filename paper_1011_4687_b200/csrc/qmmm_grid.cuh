@@ -626,15 +626,26 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     }
     __syncthreads();
     pdl_wait();                                  // the previous evaluation is done with the workspace
-    if (ws == 0 && lane < EPT * 4) {
+    if (ws == 0) {
         double a = 0.0;
-        for (int s = 0; s < WS; ++s) a += red[(s * WP + wp) * EPT * 4 + lane];
+        if (lane < EPT * 4)
+            for (int s = 0; s < WS; ++s) a += red[(s * WP + wp) * EPT * 4 + lane];
+        a *= (lane & 3) ? prm.g_scaleE : prm.g_scaleV;   // grid units -> hartree, hartree / bohr
         const int p = (blockIdx.x * WP + wp) * EPT + lane / 4;
-        if (p < prm.P)                               // grid units -> hartree, hartree / bohr
-            prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] =
-                a * ((lane & 3) ? prm.g_scaleE : prm.g_scaleV);
+        if constexpr (EPT <= 4) {
+            if (prm.push_slots) push_records<EPT>(prm, a, (blockIdx.x * WP + wp) * EPT, lane);
+        }
+        if (!(EPT <= 4 && prm.push_slots) && lane < EPT * 4 && p < prm.P)
+            prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] = a;
     }
     QMMM_MARK(5);
+    if constexpr (EPT <= 4) {
+        if (prm.push_slots) {                    // (uniform over the grid)
+            finish_point_block_push<NT>(prm, WP * EPT, threadIdx.x, flag, reinterpret_cast<double *>(smem), red,
+                                        [] { __syncthreads(); });
+            return;
+        }
+    }
     finish_point_block<NT>(prm, WP * EPT, threadIdx.x, flag, red, [] { __syncthreads(); }, prm.seq);
     QMMM_MARK(6);
     QMMM_MARK_GT(9);
@@ -878,13 +889,21 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
     }
     consumer_sync<NW>();
     pdl_wait();                                  // the previous evaluation is done with the workspace
-    if (ws == 0 && lane < EPT * 4) {
+    if (ws == 0) {
         double a = 0.0;
-        for (int s = 0; s < WS; ++s) a += red[((s * WP + wp) * EPT) * 4 + lane];
+        if (lane < EPT * 4)
+            for (int s = 0; s < WS; ++s) a += red[((s * WP + wp) * EPT) * 4 + lane];
+        a *= (lane & 3) ? prm.g_scaleE : prm.g_scaleV;
         const int p = (blockIdx.x * WP + wp) * EPT + lane / 4;
-        if (p < prm.P)
-            prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] =
-                a * ((lane & 3) ? prm.g_scaleE : prm.g_scaleV);
+        if (prm.push_slots)
+            push_records<EPT>(prm, a, (blockIdx.x * WP + wp) * EPT, lane);
+        else if (lane < EPT * 4 && p < prm.P)
+            prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] = a;
+    }
+    if (prm.push_slots) {                        // (uniform over the grid)
+        finish_point_block_push<32 * NW>(prm, WP * EPT, threadIdx.x, flag, reinterpret_cast<double *>(smem), red,
+                                         [] { consumer_sync<NW>(); });
+        return;
     }
     finish_point_block<32 * NW>(prm, WP * EPT, threadIdx.x, flag, red, [] { consumer_sync<NW>(); },
                                 prm.seq);

@@ -62,6 +62,10 @@ struct PairParams {
     int g_n[3], g_segs;      // nodes per axis (row = ix * ny + iy); z segments (gchunks) per row tile
     int g_dzt;               // grid kernels: dz table in shared memory (qmmm_grid.cuh, DZT)
     int g_light;             // host side only: FP64 grid kernel with 4 consumer warps (overlapped few-point evaluations)
+    // push-model collection (overlapped few-point evaluations): tagged 64-byte records instead
+    // of partials + fence + ticket; NULL = the ticket path
+    unsigned long long *push_slots;   // [slices][P][8] words
+    unsigned long long push_seq;      // tag of this evaluation (never 0, never reused)
     int pdl;                 // host side only: launch with programmatic stream serialization
 #ifdef QMMM_PHASE_TIMING
     long long *dbg;          // [CTAs][10] clock64 at phase boundaries + globaltimer (diagnostic build)
@@ -316,6 +320,103 @@ __device__ __forceinline__ void finish_point_block(const PairParams &prm, int pp
             __threadfence_system();
             *reinterpret_cast<volatile unsigned long long *>(prm.host_flag) = seq;
         }
+    }
+}
+
+// ---------------------------------------------------------------- push-model cross-CTA sum
+// For overlapped few-point evaluations (qmmm_field_set_overlap) the serial tail of an
+// evaluation -- partial store, fence, ticket atomic, fence, last-CTA loads -- is what bounds
+// the period of a sequence (measured in isolation: 2.6 us at 37 CTAs, 3.4 us at 148).  Here
+// every CTA instead stores each of its points' partials as ONE tagged 64-byte record
+// {tag, V, Ex, Ey, Ez, tag} (no fence, no atomic) and the CTA of slice 0 collects: its threads
+// poll the records with volatile 16-byte loads until both tags carry this evaluation's tag
+// (1.4 us at 37 CTAs, 2.5 us at 148), then add the slices in exactly the order of
+// finish_point_block.  Tags are unique per evaluation, so nothing is reset; a record is
+// overwritten only by a later evaluation, which pushes after its griddepcontrol.wait, i.e.
+// after this evaluation has completed.  A record that never arrives (cannot happen: every CTA
+// of the grid pushes unconditionally) ends the poll after PUSH_HARD_NS with NaN results
+// instead of a hang.
+constexpr int PUSH_SLOT_WORDS = 8;
+constexpr long long PUSH_HARD_NS = 2000000000ll;
+__device__ __forceinline__ long long push_global_ns() {
+    long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+// Warps with ws == 0 call this with all 32 lanes: lane 4 e + c holds value c of the warp's
+// point e (first point pbase); EPT <= 4.
+template <int EPT>
+__device__ __forceinline__ void push_records(const PairParams &prm, double a, int pbase, int lane) {
+    static_assert(EPT <= 4, "six record words per point in one warp");
+    const int e = lane / 6, w = lane - 6 * e;
+    const int src = e < EPT ? 4 * e + (w == 0 || w == 5 ? 0 : w - 1) : 0;
+    const double v = __shfl_sync(0xffffffffu, a, src);
+    const unsigned long long word = (w == 0 || w == 5) ? prm.push_seq
+                                                       : static_cast<unsigned long long>(__double_as_longlong(v));
+    const int p = pbase + e;
+    if (e < EPT && p < prm.P)
+        *reinterpret_cast<volatile unsigned long long *>(
+            prm.push_slots + (static_cast<int64_t>(blockIdx.y) * prm.P + p) * PUSH_SLOT_WORDS + w) = word;
+}
+struct push_u64x2 { unsigned long long x, y; };
+__device__ __forceinline__ push_u64x2 push_ld_v2(const unsigned long long *p) {
+    push_u64x2 r;
+    asm volatile("ld.volatile.global.v2.u64 {%0, %1}, [%2];" : "=l"(r.x), "=l"(r.y) : "l"(p));
+    return r;
+}
+// All NT threads of every CTA call this after the records are pushed.  rec_s: shared memory
+// for slices * ppb * 4 doubles (the idle stage buffers), scratch: NT doubles, flag: one int.
+template <int NT, typename SYNC>
+__device__ __forceinline__ void finish_point_block_push(const PairParams &prm, int ppb, int tid, int *flag,
+                                                        double *rec_s, double *scratch, SYNC sync) {
+    if (blockIdx.y != 0) return;                       // slice 0 of each point block collects
+    if (tid == 0) *flag = 1;
+    sync();
+    const long long t0 = push_global_ns();
+    const int nrec = prm.slices * ppb;
+    for (int r = tid; r < nrec; r += NT) {
+        const int sl = r / ppb, pp = r - sl * ppb;
+        const int p = blockIdx.x * ppb + pp;
+        double *dst = rec_s + 4 * r;
+        if (p >= prm.P) { dst[0] = dst[1] = dst[2] = dst[3] = 0.0; continue; }
+        const unsigned long long *q = prm.push_slots + (static_cast<int64_t>(sl) * prm.P + p) * PUSH_SLOT_WORDS;
+        for (;;) {
+            const push_u64x2 a = push_ld_v2(q), b = push_ld_v2(q + 2), c = push_ld_v2(q + 4);
+            if (a.x == prm.push_seq && c.y == prm.push_seq) {
+                dst[0] = __longlong_as_double(static_cast<long long>(a.y));
+                dst[1] = __longlong_as_double(static_cast<long long>(b.x));
+                dst[2] = __longlong_as_double(static_cast<long long>(b.y));
+                dst[3] = __longlong_as_double(static_cast<long long>(c.x));
+                break;
+            }
+            if (push_global_ns() - t0 > PUSH_HARD_NS) { *flag = 0; break; }
+        }
+    }
+    sync();
+    const bool ok = *flag != 0;
+    // same association as finish_point_block: thread = (group g, value v)
+    const int nval = 4 * ppb, G = NT / nval;
+    const int v = tid % nval, g = tid / nval;
+    const int p = blockIdx.x * ppb + v / 4;
+    double a[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    if (p < prm.P && g < G) {
+        const double *src = rec_s + v;                 // record (sl, pp): rec_s[(sl * ppb + pp) * 4 + c]
+        int sidx = g;
+        for (; sidx + 7 * G < prm.slices; sidx += 8 * G)
+#pragma unroll
+            for (int k = 0; k < 8; ++k) a[k] += src[(sidx + k * G) * nval];
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+            if (sidx + k * G < prm.slices) a[k] += src[(sidx + k * G) * nval];
+    }
+    scratch[tid] = ((a[0] + a[1]) + (a[2] + a[3])) + ((a[4] + a[5]) + (a[6] + a[7]));
+    sync();
+    if (g == 0 && p < prm.P) {
+        double r = 0.0;
+        for (int k = 0; k < G; ++k) r += scratch[k * nval + v];
+        if (!ok) r = __longlong_as_double(0x7ff8000000000000ll);
+        if ((v & 3) == 0) prm.V[p] = r;
+        else if (prm.E) prm.E[3 * static_cast<int64_t>(p) + (v & 3) - 1] = r;
     }
 }
 
