@@ -242,12 +242,12 @@ qmmm_plan choose_plan(const qmmm_field *h, int64_t P, bool f32, bool grid = fals
     if (pl.point_warps > nw) pl.point_warps = nw;
     const int64_t pb = (groups + pl.point_warps - 1) / pl.point_warps;
     if (pl.slices == 0 && light) {
-        // Overlapped evaluations: fewer, longer CTAs -- half an SM count per evaluation for
-        // the single-group walks, a quarter otherwise (measured, 200-1,000 evaluations replayed
-        // from one graph: config 2 3.6 -> 3.0 us FP32, 3.7 -> 3.4 us FP64; config 1 4.0 -> 3.4 us
-        // FP32, 9.4 -> 7.3 us FP64 = 73 % of the DFMA peak); a single evaluation gets slower.
-        const bool single = f32 ? grid_f32_nodepack(pl.points_per_thread, P) : grid_f64_warpown(pl.points_per_thread, P);
-        pl.slices = static_cast<int>(std::max<int64_t>(1, (h->sm_count / (single ? 2 : 4)) / pb));
+        // Overlapped evaluations: fewer, longer CTAs -- a quarter of an SM count per evaluation
+        // (measured, 200-1,000 evaluations replayed from one graph, with the push-model
+        // collection: config 2 FP32 148 / 74 / 37 / 18 CTAs: 2.67 / 2.17 / 1.87 / 1.81 us, FP64
+        // 2.58 / 2.24 / 2.22 / 2.28 us; config 1 FP32 74 / 36 / 18 CTAs: 3.42 / 3.00 / 2.91 us,
+        // FP64 8.60 / 7.27 / 7.21 us); a single evaluation gets slower.
+        pl.slices = static_cast<int>(std::max<int64_t>(1, (h->sm_count / 4) / pb));
     }
     if (pl.slices == 0) {
         const int g = gcd_int(static_cast<int>(pb % h->sm_count), h->sm_count);
