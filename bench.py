@@ -322,6 +322,18 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                     row["us_per_eval_1000_cuda_graph_overlap"] = e0.elapsed_time(e1) * 1e3 / len(walk)
                     del gr
                     B.qmmm_field_set_overlap(h, False)
+                    # (i-3) no graph: ONE library call (qmmm_field_eval_moves) issues the 1,000
+                    # overlapped launches from C
+                    nm = len(pts)
+                    Vm = torch.empty(nm, dtype=torch.float64, device="cuda")
+                    Em = torch.empty((nm, 3), dtype=torch.float64, device="cuda")
+                    B.qmmm_field_eval_moves(h, pts, nm, 1, Vm, Em, prec, stream)
+                    torch.cuda.synchronize()
+                    e0.record(stream)
+                    B.qmmm_field_eval_moves(h, pts, nm, 1, Vm, Em, prec, stream)
+                    e1.record(stream)
+                    torch.cuda.synchronize()
+                    row["us_per_eval_1000_eval_moves_call"] = e0.elapsed_time(e1) * 1e3 / nm
                     # (ii) the QMC loop of PAPER.md:117: r_new in (24 B), U out (32 B), every move;
                     # the loop itself runs inside the library (qmmm_field_eval_moves_host)
                     hp = np.ascontiguousarray(w.elec_xyz.reshape(-1, 3))

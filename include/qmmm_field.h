@@ -137,6 +137,19 @@ qmmm_status qmmm_field_eval_moves_host(qmmm_field *h, const double *elec_xyz_hos
                                        void *stream, double *seconds);
 
 /*
+ * qmmm_field_eval_moves -- n INDEPENDENT single-configuration evaluations whose positions are
+ * all known up front, on the device (BASELINE configs[2]: 1,000 evaluations along a given
+ * random walk): move s evaluates the N points elec_xyz[s][N][3] (device) into V[s][N] and
+ * E[s][N][3] (device; E may be NULL).  Equivalent to n calls of qmmm_field_eval with W = 1,
+ * issued from C (no per-call binding cost) and always with overlapped launches
+ * (qmmm_field_set_overlap, whose precondition holds by construction here): each move is its
+ * own kernel, move s + 1 starts while move s finishes.  Asynchronous on `stream`; capturable
+ * into a CUDA graph.  Errors as qmmm_field_eval.
+ */
+qmmm_status qmmm_field_eval_moves(qmmm_field *h, const double *elec_xyz, int64_t n, int64_t N,
+                                  double *V, double *E, int prec, void *stream);
+
+/*
  * Grid-aware compact source format.  The paper's sources are "spatially
  * discretized cells": nodes of a regular grid.  When the cells are the nodes
  *     R(ix, iy, iz) = origin + (ix hx, iy hy, iz hz),   0 <= i_k < n[k]   (cubic or orthorhombic cells)

@@ -27,6 +27,7 @@ LIB_PATH = os.environ.get("QMMM_FIELD_LIB") or os.path.join(
     os.path.dirname(os.path.abspath(__file__)), "libqmmm_field.so")
 EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_host",
                     "qmmm_field_eval_moves_host", "qmmm_field_create_grid", "qmmm_field_eval_energy",
+                    "qmmm_field_eval_moves",
                     "qmmm_field_share", "qmmm_field_create_grid3",
                     "qmmm_field_set_layout", "qmmm_field_get_grid_info",
                     "qmmm_field_destroy", "qmmm_field_set_plan", "qmmm_field_get_info",
@@ -85,6 +86,8 @@ def _load() -> ctypes.CDLL:
     lib.qmmm_field_eval_moves_host.restype = ci
     lib.qmmm_field_eval_moves_host.argtypes = [vp, vp, i64, i64, vp, vp, ci, vp,
                                                ctypes.POINTER(ctypes.c_double)]
+    lib.qmmm_field_eval_moves.restype = ci
+    lib.qmmm_field_eval_moves.argtypes = [vp, vp, i64, i64, vp, vp, ci, vp]
     lib.qmmm_field_create_grid.restype = ci
     lib.qmmm_field_create_grid.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.c_double,
                                            ctypes.POINTER(i64), vp, vp, vp, i64, i64,
@@ -232,6 +235,15 @@ def qmmm_field_eval_moves_host(handle: int, elec_xyz, n: int, N: int, V, E=None,
     _check(_lib.qmmm_field_eval_moves_host(handle, _ptr(elec_xyz), int(n), int(N), _ptr(V), _ptr(E),
                                            _PREC[precision], _stream(stream), ctypes.byref(secs)))
     return secs.value
+
+
+def qmmm_field_eval_moves(handle: int, elec_xyz, n: int, N: int, V, E=None, precision="fp64",
+                          stream=None) -> None:
+    """n independent single-configuration evaluations with all positions known up front
+    (device tensors elec_xyz [n,N,3], V [n,N], E [n,N,3]): one overlapped kernel per move,
+    issued from C.  Asynchronous on the stream."""
+    _check(_lib.qmmm_field_eval_moves(handle, _ptr(elec_xyz), int(n), int(N), _ptr(V), _ptr(E),
+                                      _PREC[precision], _stream(stream)))
 
 
 def qmmm_field_destroy(handle: Optional[int]) -> None:

@@ -1301,6 +1301,22 @@ qmmm_status qmmm_field_eval(qmmm_field *h, const double *elec_xyz, int64_t W, in
     return eval_impl(h, elec_xyz, W, N, V, E, prec, stream, nullptr);
 }
 
+qmmm_status qmmm_field_eval_moves(qmmm_field *h, const double *elec_xyz, int64_t n, int64_t N,
+                                  double *V, double *E, int prec, void *stream) {
+    if (!h) return fail(QMMM_ERR_INVALID_ARG, "eval_moves: NULL handle");
+    if (n < 0) return fail(QMMM_ERR_INVALID_ARG, "eval_moves: n < 0");
+    if (n > 0 && (!elec_xyz || !V)) return fail(QMMM_ERR_INVALID_ARG, "eval_moves: NULL elec_xyz or V");
+    // independent evaluations (all positions are known up front): let them overlap
+    const bool was = h->overlap;
+    h->overlap = true;
+    qmmm_status s = QMMM_OK;
+    for (int64_t i = 0; i < n && s == QMMM_OK; ++i)
+        s = eval_impl(h, elec_xyz + i * N * 3, 1, N, V + i * N, E ? E + i * N * 3 : nullptr, prec, stream,
+                      nullptr);
+    h->overlap = was;
+    return s;
+}
+
 qmmm_status qmmm_field_eval_energy(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t N,
                                    double *U, int prec, void *stream) {
     if (!h) return fail(QMMM_ERR_INVALID_ARG, "eval_energy: NULL handle");

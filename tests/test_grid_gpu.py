@@ -610,6 +610,44 @@ def test_overlapped_back_to_back_evaluations_are_bitwise_the_same(torch_cuda, B,
         B.qmmm_field_destroy(h)
 
 
+@pytest.mark.parametrize("precision,tol", [("fp64", TOL64), ("fp32", TOL32)])
+@pytest.mark.parametrize("layout", ["grid", "list"])
+def test_eval_moves_device_sequence(torch_cuda, B, oracle_mod, precision, tol, layout):
+    """qmmm_field_eval_moves: 200 independent single-electron moves of config 2's random walk
+    (and a 3-point variant) issued from C as overlapped launches; every move against the
+    oracle, twice bitwise the same, and the handle's overlap setting is left as it was."""
+    torch = torch_cuda
+    w = make_workload(2, n_points=(200, 1))
+    pts = w.elec_xyz.reshape(-1, 3)
+    ref = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, pts, want_abs=True)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 4)
+    try:
+        B.qmmm_field_set_layout(h, layout)
+        d = torch.from_numpy(pts).cuda()
+        out = []
+        for rep in range(2):
+            V = torch.full((200,), float("nan"), dtype=torch.float64, device="cuda")
+            E = torch.full((200, 3), float("nan"), dtype=torch.float64, device="cuda")
+            B.qmmm_field_eval_moves(h, d, 200, 1, V, E, precision)
+            torch.cuda.synchronize()
+            out.append((V.cpu().numpy(), E.cpu().numpy()))
+        assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+        check(ref, out[0][0], out[0][1], tol)
+        # three points per move (66 moves), potential only
+        V3 = torch.full((198,), float("nan"), dtype=torch.float64, device="cuda")
+        B.qmmm_field_eval_moves(h, d, 66, 3, V3, None, precision)
+        torch.cuda.synchronize()
+        eV = np.abs(V3.cpu().numpy() - ref.V[:198]) / np.abs(ref.V[:198])
+        assert eV.max() <= tol
+        # a plain eval afterwards is serial again (same result as a fresh serial evaluation)
+        V1, E1 = run(torch, B, h, pts[:1], precision)
+        assert abs(V1[0] - ref.V[0]) <= tol * abs(ref.V[0])
+        with pytest.raises(B.QmmmError):
+            B.qmmm_field_eval_moves(h, d, -1, 1, V, E, precision)
+    finally:
+        B.qmmm_field_destroy(h)
+
+
 # ------------------------------------------ config 2 on the device: warp-private grid walks
 @pytest.mark.parametrize("precision,tol", [("fp64", TOL64), ("fp32", TOL32)])
 def test_config2_single_point_device_evaluations(torch_cuda, B, oracle_mod, precision, tol):
