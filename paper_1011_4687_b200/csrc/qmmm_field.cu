@@ -1234,13 +1234,13 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
         // overlap with the previous evaluation on this stream (not with the timing events in
         // between, and not for the mailbox path, whose host reads V and E behind a flag)
         prm.pdl = h->overlap_now ? 1 : 0;
-        // Few points on the grid kernels, all CTAs of the launch resident together (at most
+        // Few points, all CTAs of the launch resident together (at most
         // one per SM, so the collecting CTAs cannot keep the pushing ones from starting):
         // collect the CTA partials by tagged records instead of fence + ticket -- about 1 us
         // less per evaluation, and the serial tail that bounds the period of an overlapped
         // sequence.  Same summation order, bitwise the same result.  (Not for the mailbox
         // path, whose last CTA also publishes the host flag.)
-        if (grid && !host_flag && pl.points_per_thread <= 4 &&
+        if (!host_flag && pl.points_per_thread <= 4 &&
             static_cast<int64_t>(pb) * pl.slices <= h->sm_count &&
             static_cast<int64_t>(pl.slices) * P <= PUSH_MAX_RECORDS &&
             static_cast<int64_t>(pl.slices) * pl.point_warps * pl.points_per_thread * 32 <= PUSH_MAX_CTA_RECORD_BYTES) {

@@ -615,14 +615,23 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
     compute_warps_sync();
     pdl_wait();                                  // the previous evaluation is done with the workspace
     // warps with ws == 0 add the WS source-split partners in index order and store
-    if (ws == 0 && lane < EPT * 4) {
+    if (ws == 0) {
         double acc = 0.0;
-        for (int s = 0; s < WS; ++s) acc += red[((s * WP + wp) * EPT) * 4 + lane];
+        if (lane < EPT * 4)
+            for (int s = 0; s < WS; ++s) acc += red[((s * WP + wp) * EPT) * 4 + lane];
         const int p = (blockIdx.x * WP + wp) * EPT + lane / 4;
-        if (p < prm.P)
+        if (prm.push_slots)                      // few points, single wave: tagged records
+            push_records<EPT>(prm, acc, (blockIdx.x * WP + wp) * EPT, lane);
+        else if (lane < EPT * 4 && p < prm.P)
             prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] = acc;
     }
     QMMM_MARK(5);
+    if (prm.push_slots) {                        // (uniform over the grid)
+        finish_point_block_push<32 * COMPUTE_WARPS>(prm, WP * EPT, threadIdx.x, flag,
+                                                    reinterpret_cast<double *>(smem), red,
+                                                    [] { compute_warps_sync(); });
+        return;
+    }
     finish_point_block<32 * COMPUTE_WARPS>(prm, WP * EPT, threadIdx.x, flag, red,
                                            [] { compute_warps_sync(); }, prm.seq);
     QMMM_MARK(6);
@@ -922,14 +931,25 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
     }
     __syncthreads();
     pdl_wait();                                  // the previous evaluation is done with the workspace
-    if (ws == 0 && lane < EPT * 4) {
+    if (ws == 0) {
         double a = 0.0;
-        for (int s = 0; s < WS; ++s) a += red[(s * WP + wp) * EPT * 4 + lane];
+        if (lane < EPT * 4)
+            for (int s = 0; s < WS; ++s) a += red[(s * WP + wp) * EPT * 4 + lane];
         const int p = (blockIdx.x * WP + wp) * EPT + lane / 4;
-        if (p < prm.P)
+        if constexpr (EPT <= 4) {
+            if (prm.push_slots) push_records<EPT>(prm, a, (blockIdx.x * WP + wp) * EPT, lane);
+        }
+        if (!(EPT <= 4 && prm.push_slots) && lane < EPT * 4 && p < prm.P)
             prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] = a;
     }
     QMMM_MARK(5);
+    if constexpr (EPT <= 4) {
+        if (prm.push_slots) {                    // (uniform over the grid)
+            finish_point_block_push<NT>(prm, WP * EPT, threadIdx.x, flag, reinterpret_cast<double *>(smem), red,
+                                        [] { __syncthreads(); });
+            return;
+        }
+    }
     finish_point_block<NT>(prm, WP * EPT, threadIdx.x, flag, red, [] { __syncthreads(); }, prm.seq);
     QMMM_MARK(6);
     QMMM_MARK_GT(9);
