@@ -648,6 +648,63 @@ def test_eval_moves_device_sequence(torch_cuda, B, oracle_mod, precision, tol, l
         B.qmmm_field_destroy(h)
 
 
+def test_overlap_stress_two_streams_mixed_shapes(torch_cuda, B):
+    """Overlapped launches, light CTAs and tagged-record collection under stress: two handles on
+    the same environment (qmmm_field_share) run 250 evaluations each on two concurrent streams,
+    batch size, precision, layout and E / no E changing from one evaluation to the next (so
+    ticket and push collections, light and batched plans, grid and list kernels alternate on
+    the same workspace).  Every result must equal a serial reference of the same call to
+    rounding; a stale or torn record would be off by orders of magnitude."""
+    torch = torch_cuda
+    w = make_workload(1)
+    rng = np.random.default_rng(77)
+    sizes = [1, 2, 3, 4, 5, 8, 17, 32, 64, 100, 257]
+    Pmax = max(sizes)
+    parent = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, Pmax)
+    child = B.qmmm_field_share(parent, Pmax)
+    try:
+        n = 250
+        calls = []
+        for i in range(n):
+            P = int(rng.choice(sizes))
+            calls.append((P, str(rng.choice(["fp32", "fp64"])), str(rng.choice(["auto", "list"])),
+                          bool(rng.random() < 0.8),
+                          torch.from_numpy(rng.normal(size=(P, 3)) * 0.8).cuda()))
+        # serial reference on the parent
+        ref = []
+        B.qmmm_field_set_overlap(parent, False)
+        for P, prec, lay, wantE, pts in calls:
+            B.qmmm_field_set_layout(parent, lay)
+            V = torch.zeros(P, dtype=torch.float64, device="cuda")
+            E = torch.zeros((P, 3), dtype=torch.float64, device="cuda") if wantE else None
+            B.qmmm_field_eval(parent, pts, 1, P, V, E, prec)
+            ref.append((V, E))
+        torch.cuda.synchronize()
+        # overlapped, both handles at once on two streams
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        outs = [[], []]
+        for k, hnd in enumerate((parent, child)):
+            B.qmmm_field_set_overlap(hnd, True)
+        for (P, prec, lay, wantE, pts) in calls:
+            for k, hnd in enumerate((parent, child)):
+                B.qmmm_field_set_layout(hnd, lay)
+                with torch.cuda.stream(streams[k]):          # (the NaN fill on the same stream)
+                    V = torch.full((P,), float("nan"), dtype=torch.float64, device="cuda")
+                    E = torch.full((P, 3), float("nan"), dtype=torch.float64, device="cuda") if wantE else None
+                    B.qmmm_field_eval(hnd, pts, 1, P, V, E, prec, streams[k])
+                outs[k].append((V, E))
+        torch.cuda.synchronize()
+        for k in range(2):
+            for (P, prec, lay, wantE, pts), (Vr, Er), (V, E) in zip(calls, ref, outs[k]):
+                rt = 1e-12 if prec == "fp64" else 2e-6
+                assert torch.allclose(V, Vr, rtol=rt, atol=0), (k, P, prec, lay)
+                if wantE:
+                    assert float((E - Er).abs().max()) <= rt * float(Er.abs().max()), (k, P, prec, lay)
+    finally:
+        B.qmmm_field_destroy(child)
+        B.qmmm_field_destroy(parent)
+
+
 # ------------------------------------------ config 2 on the device: warp-private grid walks
 @pytest.mark.parametrize("precision,tol", [("fp64", TOL64), ("fp32", TOL32)])
 def test_config2_single_point_device_evaluations(torch_cuda, B, oracle_mod, precision, tol):
