@@ -53,6 +53,7 @@ int gcd_int(int a, int b) {
 }
 
 constexpr int MAIL_POINTS = 64;   // eval_host uses the zero-copy mailbox up to this many points
+constexpr int MAIL_REC_OFFSET = MAIL_POINTS * 8;   // doubles before the tagged answer records (4 KB: 64-byte aligned)
 
 constexpr size_t stage_bytes(bool f32) {
     return STAGE_HDR + (f32 ? static_cast<size_t>(BLOCK_CHUNKS) * 4 * CHUNK * 4
@@ -188,7 +189,8 @@ struct qmmm_field {
     bool overlap_now = false;      // ... and this evaluation is launched that way (not timed, no mailbox)
     cudaEvent_t ev[2] = {nullptr, nullptr};
     // per-move mailbox: pinned, device-mapped host memory (elec in; V, E and a sequence flag out)
-    double *mail_h = nullptr, *mail_d = nullptr;   // [MAIL_POINTS*3 | MAIL_POINTS*4 | flag]
+    double *mail_h = nullptr, *mail_d = nullptr;   // [MAIL_POINTS*3 | MAIL_POINTS*4 | flag | pad | records MAIL_POINTS*8]
+    bool last_mail_push = false;                   // the last mailbox evaluation answered with tagged records
     unsigned long long seq = 0;
     // resident move server (qmmm_server.cuh): serves single-point eval_host calls
     ServerMailbox *srv_mail_h = nullptr, *srv_mail_d = nullptr;
@@ -299,7 +301,7 @@ bool auto_uses_grid(const qmmm_field *h, int64_t P, bool f32) {
 // records (slices x P) the push-model collection of a handle can hold; the collecting CTA
 // keeps slices x (points of a CTA) records of 32 bytes in its idle stage buffers
 constexpr int64_t PUSH_MAX_RECORDS = 4096;
-constexpr int64_t PUSH_MAX_CTA_RECORD_BYTES = 16384;
+constexpr int64_t PUSH_MAX_CTA_RECORD_BYTES = 32768;   // and never more than the stage buffers hold
 
 // One evaluation kernel launch.  prm.pdl: programmatic stream serialization -- the kernel may
 // start while its predecessor in the stream is still running (qmmm_field_set_overlap; the
@@ -784,8 +786,8 @@ qmmm_status alloc_runtime(qmmm_field *h) {
     RT_TRY(cudaMemset(h->counters, 0, (h->max_points + 1) * sizeof(int)));
     RT_TRY(cudaMalloc(&h->push_slots, PUSH_MAX_RECORDS * PUSH_SLOT_WORDS * sizeof(unsigned long long)));
     RT_TRY(cudaMemset(h->push_slots, 0, PUSH_MAX_RECORDS * PUSH_SLOT_WORDS * sizeof(unsigned long long)));
-    RT_TRY(cudaHostAlloc(&h->mail_h, (MAIL_POINTS * 7 + 1) * sizeof(double), cudaHostAllocMapped));
-    std::memset(h->mail_h, 0, (MAIL_POINTS * 7 + 1) * sizeof(double));
+    RT_TRY(cudaHostAlloc(&h->mail_h, (MAIL_REC_OFFSET + MAIL_POINTS * 8) * sizeof(double), cudaHostAllocMapped));
+    std::memset(h->mail_h, 0, (MAIL_REC_OFFSET + MAIL_POINTS * 8) * sizeof(double));
     RT_TRY(cudaHostGetDevicePointer(&h->mail_d, h->mail_h, 0));
     RT_TRY(cudaHostAlloc(&h->srv_mail_h, sizeof(ServerMailbox), cudaHostAllocMapped));
     std::memset(h->srv_mail_h, 0, sizeof(ServerMailbox));
@@ -1240,12 +1242,20 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
         // less per evaluation, and the serial tail that bounds the period of an overlapped
         // sequence.  Same summation order, bitwise the same result.  (Not for the mailbox
         // path, whose last CTA also publishes the host flag.)
-        if (!host_flag && pl.points_per_thread <= 4 &&
+        h->last_mail_push = false;
+        if (pl.points_per_thread <= 4 &&
             static_cast<int64_t>(pb) * pl.slices <= h->sm_count &&
             static_cast<int64_t>(pl.slices) * P <= PUSH_MAX_RECORDS &&
-            static_cast<int64_t>(pl.slices) * pl.point_warps * pl.points_per_thread * 32 <= PUSH_MAX_CTA_RECORD_BYTES) {
+            static_cast<int64_t>(pl.slices) * pl.point_warps * pl.points_per_thread * 32 <=
+                std::min<int64_t>(PUSH_MAX_CTA_RECORD_BYTES,
+                                  static_cast<int64_t>(pl.stages) * (grid ? (f32 ? 8192 : 16384) : 32768))) {
             prm.push_slots = h->push_slots;
             prm.push_seq = ++h->push_seq;
+            if (host_flag) {               // mailbox: the collecting CTAs answer with tagged records
+                prm.host_flag = nullptr;
+                prm.host_records = reinterpret_cast<unsigned long long *>(h->mail_d + MAIL_REC_OFFSET);
+                h->last_mail_push = true;
+            }
         }
         if (grid) {
             // cells: charges only, coordinates from the indices; everything in grid units
@@ -1369,6 +1379,33 @@ qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int
         qmmm_status s = eval_impl(h, in_d, W, N, out_d, E_host ? out_d + P : nullptr, prec, stream,
                                   reinterpret_cast<unsigned long long *>(h->mail_d + MAIL_POINTS * 7));
         if (s != QMMM_OK) return s;
+        if (h->last_mail_push) {
+            // answered by tagged records {tag, V, Ex, Ey, Ez, tag}, one per point, written by the
+            // collecting CTAs without fences: wait until every record carries this call's tag
+            const volatile unsigned long long *rec =
+                reinterpret_cast<const volatile unsigned long long *>(h->mail_h + MAIL_REC_OFFSET);
+            const unsigned long long tag = h->push_seq;
+            uint64_t spin = 1;
+            for (int64_t p = 0; p < P; ++p) {
+                const volatile unsigned long long *r = rec + p * 8;
+                for (;;) {
+                    if (r[0] == tag && r[5] == tag) {         // both ends of the 48-byte record (one
+                        std::atomic_thread_fence(std::memory_order_acquire);   // store, one line)
+                        const unsigned long long bits[4] = {r[1], r[2], r[3], r[4]};
+                        std::memcpy(V_host + p, &bits[0], 8);
+                        if (E_host) std::memcpy(E_host + 3 * p, &bits[1], 24);
+                        break;
+                    }
+                    if ((++spin & 0xFFFF) == 0) {             // now and then: did the launch fail?
+                        cudaError_t q = cudaStreamQuery(st);
+                        if (q != cudaSuccess && q != cudaErrorNotReady) return cuda_fail(q, "eval_host: kernel");
+                        if (q == cudaSuccess && !(r[0] == tag && r[5] == tag))
+                            return fail(QMMM_ERR_CUDA, "eval_host: kernel finished without publishing its result");
+                    }
+                }
+            }
+            return QMMM_OK;
+        }
         for (uint64_t spin = 1; *flag_h != h->seq; ++spin) {
             if ((spin & 0xFFFF) == 0) {                   // now and then: did the launch fail?
                 cudaError_t q = cudaStreamQuery(st);

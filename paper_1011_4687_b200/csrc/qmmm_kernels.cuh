@@ -66,6 +66,10 @@ struct PairParams {
     // of partials + fence + ticket; NULL = the ticket path
     unsigned long long *push_slots;   // [slices][P][8] words
     unsigned long long push_seq;      // tag of this evaluation (never 0, never reused)
+    // per-move mailbox with the push collection: the collecting CTA writes one tagged record
+    // {tag, V, Ex, Ey, Ez, tag} per point straight into pinned host memory (no system-scope
+    // fence, no flag); NULL = V / E as usual
+    unsigned long long *host_records; // [P][8] words, device-mapped host memory
     int pdl;                 // host side only: launch with programmatic stream serialization
 #ifdef QMMM_PHASE_TIMING
     long long *dbg;          // [CTAs][10] clock64 at phase boundaries + globaltimer (diagnostic build)
@@ -411,10 +415,31 @@ __device__ __forceinline__ void finish_point_block_push(const PairParams &prm, i
     }
     scratch[tid] = ((a[0] + a[1]) + (a[2] + a[3])) + ((a[4] + a[5]) + (a[6] + a[7]));
     sync();
-    if (g == 0 && p < prm.P) {
-        double r = 0.0;
+    const bool mine = g == 0 && p < prm.P;
+    double r = 0.0;
+    if (mine) {
         for (int k = 0; k < G; ++k) r += scratch[k * nval + v];
         if (!ok) r = __longlong_as_double(0x7ff8000000000000ll);
+    }
+    if (prm.host_records) {
+        // threads 0 .. nval-1 hold value (tid & 3) of the CTA's point tid >> 2: eight points per
+        // warp, written as two groups of four records (six lanes each, one store instruction)
+        if (tid < ((nval + 31) & ~31)) {
+            const int lane = tid & 31, wbase = (tid >> 5) * 8;
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                const int e = lane / 6, w = lane - 6 * e;
+                const int src = (4 * half + (e < 4 ? e : 0)) * 4 + ((w == 0 || w == 5) ? 0 : w - 1);
+                const double val = __shfl_sync(0xffffffffu, r, src);
+                const unsigned long long word =
+                    (w == 0 || w == 5) ? prm.push_seq : static_cast<unsigned long long>(__double_as_longlong(val));
+                const int lp = wbase + 4 * half + e, gp = blockIdx.x * ppb + lp;
+                if (e < 4 && lp < ppb && gp < prm.P)
+                    *reinterpret_cast<volatile unsigned long long *>(
+                        prm.host_records + static_cast<int64_t>(gp) * PUSH_SLOT_WORDS + w) = word;
+            }
+        }
+    } else if (mine) {
         if ((v & 3) == 0) prm.V[p] = r;
         else if (prm.E) prm.E[3 * static_cast<int64_t>(p) + (v & 3) - 1] = r;
     }
