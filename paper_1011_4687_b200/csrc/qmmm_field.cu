@@ -1243,6 +1243,10 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
         // sequence.  Same summation order, bitwise the same result.  (Not for the mailbox
         // path, whose last CTA also publishes the host flag.)
         h->last_mail_push = false;
+        if (host_flag && P <= INLINE_POINTS) {     // mailbox call: the points as kernel parameters
+            std::memcpy(prm.pts, h->mail_h, static_cast<size_t>(P) * 3 * sizeof(double));
+            prm.inline_pts = 1;
+        }
         if (pl.points_per_thread <= 4 &&
             static_cast<int64_t>(pb) * pl.slices <= h->sm_count &&
             static_cast<int64_t>(pl.slices) * P <= PUSH_MAX_RECORDS &&

@@ -403,7 +403,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
         int p = blockIdx.x * ppb + i / 3;
         p = p < prm.P ? p : prm.P - 1;                          // clamp: duplicates are not written
         const int comp = i % 3;
-        const double u = (prm.elec[static_cast<int64_t>(p) * 3 + comp] - prm.g_org[comp]) * prm.g_inv_h[comp];
+        const double u = (point_coord(prm, static_cast<int64_t>(p) * 3 + comp) - prm.g_org[comp]) * prm.g_inv_h[comp];
         const double sc = comp == 0 ? prm.g_sx : (comp == 1 ? prm.g_sy : 1.0);
         elec_s[i] = u * sc;                                     // units of hz (for the nuclei)
         float dd;
@@ -727,7 +727,7 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
         p = p < prm.P ? p : prm.P - 1;
         const int comp = i % 3;
         // units of hz on every axis: (r - org) / hz; node (ix, iy, iz) sits at (ix sx, iy sy, iz)
-        elec_s[i] = (prm.elec[static_cast<int64_t>(p) * 3 + comp] - prm.g_org[comp]) * prm.g_scaleV;
+        elec_s[i] = (point_coord(prm, static_cast<int64_t>(p) * 3 + comp) - prm.g_org[comp]) * prm.g_scaleV;
     }
     if constexpr (DZT) {                           // dz of every (z node, point of this CTA)
         const int nzp = prm.g_segs * GRID_ZS;
@@ -735,7 +735,7 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
             const int kz = i / ppb, pp = i - kz * ppb;
             int p = blockIdx.x * ppb + pp;
             p = p < prm.P ? p : prm.P - 1;
-            const double uz = (prm.elec[static_cast<int64_t>(p) * 3 + 2] - prm.g_org[2]) * prm.g_scaleV;
+            const double uz = (point_coord(prm, static_cast<int64_t>(p) * 3 + 2) - prm.g_org[2]) * prm.g_scaleV;
             dzt[i] = uz - static_cast<double>(kz);
         }
     }

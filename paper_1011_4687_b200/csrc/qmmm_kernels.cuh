@@ -70,11 +70,21 @@ struct PairParams {
     // {tag, V, Ex, Ey, Ez, tag} per point straight into pinned host memory (no system-scope
     // fence, no flag); NULL = V / E as usual
     unsigned long long *host_records; // [P][8] words, device-mapped host memory
+    // per-move mailbox, up to INLINE_POINTS points: the coordinates travel as kernel parameters
+    // (constant bank) instead of being read from pinned host memory over PCIe by every CTA
+    int inline_pts;
+    double pts[3 * 32];
     int pdl;                 // host side only: launch with programmatic stream serialization
 #ifdef QMMM_PHASE_TIMING
     long long *dbg;          // [CTAs][10] clock64 at phase boundaries + globaltimer (diagnostic build)
 #endif
 };
+
+constexpr int INLINE_POINTS = 32;
+// coordinate idx (= 3 p + component) of the evaluation points
+__device__ __forceinline__ double point_coord(const PairParams &prm, int64_t idx) {
+    return prm.inline_pts ? prm.pts[idx] : prm.elec[idx];
+}
 
 // ----------------------------------------------------------------------------- PTX helpers
 #ifdef QMMM_PHASE_TIMING
@@ -504,7 +514,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
     for (int i = threadIdx.x; i < ppb * 3; i += CTA_THREADS) {
         int p = blockIdx.x * ppb + i / 3;
         p = p < prm.P ? p : prm.P - 1;                       // clamp: duplicates are not written
-        elec_s[i] = prm.elec[static_cast<int64_t>(p) * 3 + (i % 3)];
+        elec_s[i] = point_coord(prm, static_cast<int64_t>(p) * 3 + (i % 3));
     }
     __syncthreads();
     QMMM_MARK(1);
@@ -822,7 +832,7 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
     for (int i = threadIdx.x; i < ppb * 3; i += NT) {
         int p = blockIdx.x * ppb + i / 3;
         p = p < prm.P ? p : prm.P - 1;                          // clamp: duplicates are not written
-        elec_s[i] = prm.elec[static_cast<int64_t>(p) * 3 + (i % 3)];
+        elec_s[i] = point_coord(prm, static_cast<int64_t>(p) * 3 + (i % 3));
     }
     __syncthreads();
     QMMM_MARK(1);
