@@ -112,8 +112,12 @@ qmmm_status qmmm_field_eval_energy(qmmm_field *h, const double *elec_xyz, int64_
  *               It retires by itself after 2 ms without a request (and after 1 s in any
  *               case) and is restarted transparently; any other call on the handle retires
  *               it first.  While it is resident it occupies every SM.  `stream` is not used.
- *   W*N <= 64 : one kernel launch on `stream`; points read from and results written to a
- *               pinned, device-mapped mailbox, completion signalled by a sequence number.
+ *   W*N <= 64 : one kernel launch on `stream`, no copies and no stream synchronisation: up to
+ *               32 points travel as kernel parameters (more are read by the kernel from a
+ *               pinned, device-mapped mailbox), and the results come back as one tagged
+ *               record {tag, V, E, tag} per point written by the kernel straight into pinned
+ *               host memory, which the call polls (or, for launch shapes the record
+ *               collection does not cover, as V, E followed by a sequence number).
  *   otherwise : host->device copy, kernel, device->host copy on `stream`, synchronisation.
  * All three give bitwise the result of qmmm_field_eval with the same plan and layout (the
  * move server always reads the source list: layout LIST).
