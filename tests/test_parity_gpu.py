@@ -302,6 +302,39 @@ def test_eval_host_mailbox_and_copy_paths_agree_with_device_path(torch_cuda, B, 
         B.qmmm_field_destroy(h)
 
 
+def test_mailbox_tagged_record_answers_stress(torch_cuda, B):
+    """Per-move mailbox path of qmmm_field_eval_host (2..64 points): the points travel as kernel
+    parameters (<= 32) or through the pinned mailbox, the answers come back as tagged records
+    written by the collecting CTAs into pinned host memory.  1,200 calls with changing point
+    count, precision and layout: every answer finite and non-zero, every 20th bitwise the
+    device path's (a torn or stale record would show at once)."""
+    torch = torch_cuda
+    w = make_workload(1)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 64)
+    rng = np.random.default_rng(5)
+    try:
+        for it in range(1200):
+            P = int(rng.integers(2, 65))
+            prec = "fp32" if it % 2 else "fp64"
+            B.qmmm_field_set_layout(h, "auto" if (it // 2) % 2 else "list")
+            x = np.ascontiguousarray(rng.normal(size=(P, 3)) * 0.8)
+            V = np.zeros(P); E = np.zeros((P, 3))
+            want_E = it % 7 != 0
+            B.qmmm_field_eval_host(h, x, 1, P, V, E if want_E else None, prec)
+            assert np.all(np.isfinite(V)) and np.all(V != 0.0), (it, P, prec)
+            if it % 20 == 0:
+                d = torch.from_numpy(x).cuda()
+                Vd = torch.zeros(P, dtype=torch.float64, device="cuda")
+                Ed = torch.zeros((P, 3), dtype=torch.float64, device="cuda")
+                B.qmmm_field_eval(h, d, 1, P, Vd, Ed if want_E else None, prec)
+                torch.cuda.synchronize()
+                assert np.array_equal(V, Vd.cpu().numpy()), (it, P, prec)
+                if want_E:
+                    assert np.array_equal(E, Ed.cpu().numpy()), (it, P, prec)
+    finally:
+        B.qmmm_field_destroy(h)
+
+
 def test_repeatability_stress_all_kernel_variants(torch_cuda, B):
     """compute-sanitizer is closed on this GPU pool, so races are hunted statistically: every
     kernel variant and several partitions, 25 evaluations each on one handle, must be bitwise
