@@ -31,7 +31,9 @@
  * math.fsum of the terms, mpmath 50-digit brute force, scipy cdist restatement,
  * superposition, power-of-two scaling (bitwise), permutation, dyadic-lattice
  * translation (bitwise), 90-degree rotation, E = -grad V by central differences,
- * mean-value property and Gauss's law.  Nothing here is "parity unpinned".
+ * mean-value property and Gauss's law; the absolute sums absV, absE (condition
+ * numbers) against |q|/d, |q|/d^2, math.fsum of numpy-formed terms and mpmath.
+ * Nothing here is "parity unpinned".
  */
 #include <math.h>
 #include <stddef.h>

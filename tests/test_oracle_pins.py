@@ -138,6 +138,56 @@ def test_summation_vs_fsum(oracle_mod):
         assert res.absV[i] == pytest.approx(math.fsum(np.abs(t)), rel=1e-15)
 
 
+
+def test_absolute_sums_absV_absE_are_pinned(oracle_mod):
+    """The oracle's condition-number sums absV = sum_j |q_j|/r_ij and absE = sum_j |q_j|/r_ij^2
+    (SURVEY.md 8(c) "Error metrics") scale every kappa-aware GPU assertion, so they are pinned
+    like V itself: one source (closed form |q|/d and |q|/d^2: catches dividing by r once
+    instead of twice, a signed instead of an absolute term), and on config 0 against the
+    exactly rounded math.fsum of terms formed here with numpy from the positions (not from the
+    oracle's own term routine), and against 50-digit mpmath on a mixed-sign tiny case."""
+    R = np.array([[1.0, -2.0, 0.5]])
+    r = np.array([[3.0, 1.0, -1.5]])
+    d2 = float(((r[0] - R[0]) ** 2).sum())
+    for q in (-0.75, 0.75):
+        res = oracle_mod.field(R, np.array([q]), EMPTY3, EMPTY, r, want_abs=True)
+        assert res.absV[0] == pytest.approx(0.75 / math.sqrt(d2), rel=4e-16)
+        assert res.absE[0] == pytest.approx(0.75 / d2, rel=4e-16)
+    # one cell and one nucleus of opposite sign: the absolute sums add, V and E cancel partly
+    res = oracle_mod.field(R, np.array([-2.0]), np.array([[1.0, -2.0, 2.5]]), np.array([2.0]), r,
+                           want_abs=True)
+    d2n = float(((r[0] - np.array([1.0, -2.0, 2.5])) ** 2).sum())
+    assert res.absV[0] == pytest.approx(2.0 / math.sqrt(d2) + 2.0 / math.sqrt(d2n), rel=4e-16)
+    assert res.absE[0] == pytest.approx(2.0 / d2 + 2.0 / d2n, rel=4e-16)
+    assert abs(res.V[0]) < res.absV[0] and np.linalg.norm(res.E[0]) < res.absE[0]
+
+    w = make_workload(0)
+    pts = w.elec_xyz.reshape(-1, 3)
+    allx = np.vstack([w.src_xyz, w.nuc_xyz])
+    allq = np.abs(np.concatenate([w.src_q, w.nuc_Z]))
+    res = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, pts, want_abs=True)
+    for i in range(w.P):
+        r2 = ((pts[i] - allx) ** 2).sum(1)
+        assert res.absV[i] == pytest.approx(math.fsum(allq / np.sqrt(r2)), rel=4e-15)
+        assert res.absE[i] == pytest.approx(math.fsum(allq / r2), rel=4e-15)
+
+    import mpmath as mp
+    mp.mp.dps = 50
+    rng = np.random.default_rng(12)
+    src = rng.uniform(-6, 6, (48, 3)); src = src[np.linalg.norm(src, axis=1) > 2.5]
+    q = rng.normal(size=len(src))
+    pts = rng.uniform(-1, 1, (3, 3))
+    res = oracle_mod.field(src, q, EMPTY3, EMPTY, pts, want_abs=True)
+    for i, p in enumerate(pts):
+        aV = mp.mpf(0); aE = mp.mpf(0)
+        for Rj, qj in zip(src, q):
+            r2 = sum((mp.mpf(float(p[k])) - mp.mpf(float(Rj[k]))) ** 2 for k in range(3))
+            aV += abs(mp.mpf(float(qj))) / mp.sqrt(r2)
+            aE += abs(mp.mpf(float(qj))) / r2
+        assert res.absV[i] == pytest.approx(float(aV), rel=1e-15)
+        assert res.absE[i] == pytest.approx(float(aE), rel=1e-15)
+
+
 def _mp_field(src_xyz, src_q, nuc_xyz, nuc_Z, pts):
     import mpmath as mp
     mp.mp.dps = 50
