@@ -228,6 +228,18 @@ qmmm_status qmmm_field_get_grid_info(const qmmm_field *h, qmmm_grid_info *info);
  */
 qmmm_status qmmm_field_share(const qmmm_field *parent, int64_t max_points, qmmm_field **out);
 
+/*
+ * qmmm_sum_rank_partials -- the cross-device step of sharding by SOURCES (Eq. 5 of the paper,
+ * PAPER.md:119-128, with one block B[m] per GPU): every rank evaluates all
+ * points against its own cells, the per-rank partials {V, E} are gathered (NCCL all-gather of
+ * 4 doubles per point), and this call adds them in RANK ORDER, out[i] = ((parts[0][i] +
+ * parts[1][i]) + parts[2][i]) + ..., so that every rank holds bitwise the same sums (a tree
+ * all-reduce would not fix the order).
+ *   parts  DEVICE [R][n] FP64,  out  DEVICE [n] FP64 (may alias parts[0]),  1 <= R <= 65536.
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA (launch failure).
+ */
+qmmm_status qmmm_sum_rank_partials(const double *parts, int64_t R, int64_t n, double *out, void *stream);
+
 /* qmmm_field_destroy -- frees the handle and its device buffers.  NULL is a no-op. */
 qmmm_status qmmm_field_destroy(qmmm_field *h);
 
@@ -254,6 +266,12 @@ typedef struct {
     int32_t sm_count;
     int32_t last_dz_table;       /* 1: the most recent eval ran a grid kernel that tabulates dz in shared
                                   * memory (8 / 12 instead of 9 / 13 lane operations per pair) */
+    int32_t device_errors;       /* nonzero: a kernel of this handle gave up a bounded wait (a cross-CTA
+                                  * record never arrived; never expected) and wrote NaN results.  Read
+                                  * without synchronising; the host-buffer calls return QMMM_ERR_CUDA. */
+    int32_t reserved;
+    char last_kernel[192];       /* mangled name of the kernel the most recent evaluation launched (or of
+                                  * the move server it started): which template instantiation ran */
 } qmmm_field_info;
 
 qmmm_status qmmm_field_get_info(const qmmm_field *h, qmmm_field_info *info);
@@ -294,12 +312,16 @@ qmmm_status qmmm_field_last_timing(qmmm_field *h, double *pair_ms, double *final
  * qmmm_probe_peak -- same-run roofline denominators (north_star: "measured by a
  * microbenchmark in the same run").  Runs a register-only kernel of independent
  * dependent chains on every SM and reports the achieved rate.
- *   kind 0: FP32 FFMA, 1: FP64 DFMA, 2: MUFU.RSQ (FP32), 3: empty-kernel launch+sync
- *   iters      inner iterations (0 = default)
+ *   kind 0: FP32 FFMA, 1: FP64 DFMA, 2: MUFU.RSQ (FP32), 3: empty-kernel launch+sync,
+ *        4: read bandwidth over a 33 MB buffer (resident in L2 after the warm-up pass),
+ *        5: read bandwidth over a 537 MB buffer (HBM)   (the rooflines of the
+ *           single-electron path, whose sources are 8-67 MB per evaluation)
+ *   iters      inner iterations / passes over the buffer (0 = default)
  *   *rate      out: warp-lane operations per second (kind 0-2; an FMA counts 1),
- *              or seconds per launch+sync (kind 3)
+ *              seconds per launch+sync (kind 3), or bytes per second (kind 4, 5)
  *   *seconds   out: device time of the timed launch (CUDA events), may be NULL
- * Synchronises the stream.
+ * Synchronises the stream.  Kinds 4 and 5 allocate (and free) their buffer on the current
+ * device.  Errors: INVALID_ARG (NULL rate, unknown kind), ALLOC, CUDA; qmmm_last_error() is set.
  */
 qmmm_status qmmm_probe_peak(int kind, int iters, double *rate, double *seconds, void *stream);
 

@@ -32,7 +32,7 @@ EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_hos
                     "qmmm_field_set_layout", "qmmm_field_get_grid_info",
                     "qmmm_field_destroy", "qmmm_field_set_plan", "qmmm_field_get_info",
                     "qmmm_field_set_timing", "qmmm_field_last_timing", "qmmm_field_set_overlap",
-                    "qmmm_probe_peak", "qmmm_last_error")
+                    "qmmm_sum_rank_partials", "qmmm_probe_peak", "qmmm_last_error")
 
 
 class QmmmError(RuntimeError):
@@ -52,7 +52,8 @@ class qmmm_field_info(ctypes.Structure):
                 ("bytes_fp32", ctypes.c_int64), ("bytes_workspace", ctypes.c_int64),
                 ("last_plan", qmmm_plan), ("last_point_blocks", ctypes.c_int32),
                 ("last_launches", ctypes.c_int32), ("sm_count", ctypes.c_int32),
-                ("last_dz_table", ctypes.c_int32)]
+                ("last_dz_table", ctypes.c_int32), ("device_errors", ctypes.c_int32),
+                ("reserved", ctypes.c_int32), ("last_kernel", ctypes.c_char * 192)]
 
 
 class qmmm_grid_info(ctypes.Structure):
@@ -118,6 +119,8 @@ def _load() -> ctypes.CDLL:
     lib.qmmm_probe_peak.restype = ci
     lib.qmmm_probe_peak.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double),
                                     ctypes.POINTER(ctypes.c_double), vp]
+    lib.qmmm_sum_rank_partials.restype = ci
+    lib.qmmm_sum_rank_partials.argtypes = [vp, i64, i64, vp, vp]
     lib.qmmm_last_error.restype = ctypes.c_char_p
     lib.qmmm_last_error.argtypes = []
     return lib
@@ -246,6 +249,14 @@ def qmmm_field_eval_moves(handle: int, elec_xyz, n: int, N: int, V, E=None, prec
                                       _PREC[precision], _stream(stream)))
 
 
+def qmmm_sum_rank_partials(parts, out, stream=None) -> None:
+    """out[i] = parts[0][i] + parts[1][i] + ... in rank order (device tensors: parts [R, n]
+    contiguous FP64, out [n]); sharding by sources, Eq. 5 across GPUs."""
+    R = int(parts.shape[0])
+    n = int(parts.numel() // R) if R else 0
+    _check(_lib.qmmm_sum_rank_partials(_ptr(parts), R, n, _ptr(out), _stream(stream)))
+
+
 def qmmm_field_destroy(handle: Optional[int]) -> None:
     _check(_lib.qmmm_field_destroy(handle))
 
@@ -259,6 +270,7 @@ def qmmm_field_get_info(handle: int) -> dict:
     info = qmmm_field_info()
     _check(_lib.qmmm_field_get_info(handle, ctypes.byref(info)))
     d = {k: getattr(info, k) for k, _ in info._fields_ if k not in ("last_plan", "reserved")}
+    d["last_kernel"] = info.last_kernel.decode()
     d["last_plan"] = {k: getattr(info.last_plan, k) for k, _ in qmmm_plan._fields_}
     return d
 
@@ -282,7 +294,8 @@ def qmmm_field_last_timing(handle: int) -> Tuple[float, float]:
 
 
 def qmmm_probe_peak(kind: int, iters: int = 0, stream=None) -> Tuple[float, float]:
-    """(rate, seconds): kind 0 FFMA, 1 DFMA, 2 MUFU.RSQ lane-ops/s; 3 launch+sync seconds."""
+    """(rate, seconds): kind 0 FFMA, 1 DFMA, 2 MUFU.RSQ lane-ops/s; 3 launch+sync seconds;
+    4 / 5 read bandwidth in bytes/s over a 33 MB (L2) / 537 MB (HBM) buffer."""
     rate, secs = ctypes.c_double(), ctypes.c_double()
     _check(_lib.qmmm_probe_peak(kind, iters, ctypes.byref(rate), ctypes.byref(secs),
                                 _stream(stream)))

@@ -17,7 +17,9 @@
 #include <cstdio>
 #include <cstring>
 #include <ctime>
+#include <climits>
 #include <memory>
+#include <mutex>
 #include <new>
 #include <string>
 
@@ -41,6 +43,12 @@ qmmm_status cuda_fail(cudaError_t e, const char *what) {
         cudaError_t _e = (expr);                                \
         if (_e != cudaSuccess) return cuda_fail(_e, #expr);     \
     } while (0)
+
+}  // namespace
+namespace qmmm {
+void set_last_error(const char *msg) { g_last_error = msg ? msg : ""; }    // for qmmm_probe.cu
+}
+namespace {
 
 int pow2_ceil(int64_t v) {
     int p = 1;
@@ -212,6 +220,12 @@ struct qmmm_field {
     double *nuclei_u = nullptr;    // [K][4] nuclei in grid units
     int layout = QMMM_LAYOUT_AUTO, last_layout = QMMM_LAYOUT_LIST;
     double bb_lo[3] = {0, 0, 0}, bb_hi[3] = {0, 0, 0};   // bounding box of the cells
+    const char *last_kernel = "";  // mangled name of the kernel the most recent evaluation ran
+    // device error word (pinned, device-mapped): set by a kernel whose bounded wait gave up
+    int *dev_err_h = nullptr, *dev_err_d = nullptr;
+    // first evaluation of a qmmm_field_eval_moves sequence: launched WITHOUT programmatic
+    // serialization, so that it orders after whatever produced the positions
+    bool pdl_hold = false;
 };
 
 namespace {
@@ -306,6 +320,37 @@ constexpr int64_t PUSH_MAX_CTA_RECORD_BYTES = 32768;   // and never more than th
 // One evaluation kernel launch.  prm.pdl: programmatic stream serialization -- the kernel may
 // start while its predecessor in the stream is still running (qmmm_field_set_overlap; the
 // kernels order themselves with griddepcontrol, qmmm_kernels.cuh).
+constexpr int MAX_DEVICES = 64;
+thread_local int g_device = 0;                    // device of the handle being evaluated (checked current)
+thread_local const char *g_launched = "";         // mangled name of the kernel launched last on this thread
+
+const char *kernel_name(const void *kern) {
+    const char *name = nullptr;
+    if (cudaFuncGetName(&name, kern) != cudaSuccess || !name) {
+        cudaGetLastError();
+        return "?";
+    }
+    return name;
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a property of (function, device): one record
+// per device, shared by all host threads.
+struct SmemConfig {
+    std::atomic<size_t> bytes[MAX_DEVICES];
+    SmemConfig() { for (auto &b : bytes) b.store(0); }
+    template <typename K>
+    cudaError_t ensure(K kern, size_t smem) {
+        std::atomic<size_t> &cur = bytes[g_device];
+        if (smem <= cur.load(std::memory_order_acquire)) return cudaSuccess;
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             static_cast<int>(smem));
+        if (e != cudaSuccess) return e;
+        size_t seen = cur.load();
+        while (seen < smem && !cur.compare_exchange_weak(seen, smem)) {}
+        return cudaSuccess;
+    }
+};
+
 cudaError_t launch_eval_kernel(void (*kern)(const PairParams), dim3 grid, unsigned threads, size_t smem,
                                cudaStream_t st, const PairParams &prm) {
     cudaLaunchConfig_t cfg = {};
@@ -324,26 +369,22 @@ cudaError_t launch_eval_kernel(void (*kern)(const PairParams), dim3 grid, unsign
 template <typename REAL, int EPT, bool WITH_E = true>
 cudaError_t launch_pair(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
     auto kern = pair_kernel<REAL, EPT, WITH_E>;
-    static thread_local size_t configured = 0;
-    if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             static_cast<int>(smem));
-        if (e != cudaSuccess) return e;
-        configured = smem;
-    }
+    static SmemConfig configured;
+    static const char *const name = kernel_name(reinterpret_cast<const void *>(kern));
+    g_launched = name;
+    cudaError_t e = configured.ensure(kern, smem);
+    if (e != cudaSuccess) return e;
     return launch_eval_kernel(kern, grid, CTA_THREADS, smem, st, prm);
 }
 
 template <int EP2, int NW>
 cudaError_t launch_pair_f32x2(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
     auto kern = pair_kernel_f32x2<EP2, NW>;
-    static thread_local size_t configured = 0;
-    if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             static_cast<int>(smem));
-        if (e != cudaSuccess) return e;
-        configured = smem;
-    }
+    static SmemConfig configured;
+    static const char *const name = kernel_name(reinterpret_cast<const void *>(kern));
+    g_launched = name;
+    cudaError_t e = configured.ensure(kern, smem);
+    if (e != cudaSuccess) return e;
     return launch_eval_kernel(kern, grid, 32 * NW, smem, st, prm);
 }
 
@@ -384,25 +425,21 @@ cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaS
         if (prm.point_warps == NW) return launch_grid_f32<EP2, NW, false, true>(prm, grid, smem, st);
     }
     auto kern = grid_kernel_f32x2<EP2, NW, NODEPACK, FULL, DZT>;
-    static thread_local size_t configured = 0;
-    if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             static_cast<int>(smem));
-        if (e != cudaSuccess) return e;
-        configured = smem;
-    }
+    static SmemConfig configured;
+    static const char *const name = kernel_name(reinterpret_cast<const void *>(kern));
+    g_launched = name;
+    cudaError_t e = configured.ensure(kern, smem);
+    if (e != cudaSuccess) return e;
     return launch_eval_kernel(kern, grid, 32 * NW, smem, st, prm);
 }
 template <int EPT, bool WITH_E, int NW, bool WARPOWN = false, bool DZT = false>
 cudaError_t launch_grid_f64(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
     auto kern = grid_kernel_f64<EPT, WITH_E, NW, WARPOWN, DZT>;
-    static thread_local size_t configured = 0;
-    if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             static_cast<int>(smem));
-        if (e != cudaSuccess) return e;
-        configured = smem;
-    }
+    static SmemConfig configured;
+    static const char *const name = kernel_name(reinterpret_cast<const void *>(kern));
+    g_launched = name;
+    cudaError_t e = configured.ensure(kern, smem);
+    if (e != cudaSuccess) return e;
     return launch_eval_kernel(kern, grid, 32 * (NW + 1), smem, st, prm);
 }
 // Grid layout: FP32-acc64 packed kernel for 2, 4, 8 points per thread; FP64 for 1, 2, 4.
@@ -622,6 +659,56 @@ void post_request(ServerMailbox *m, unsigned long long s, const double *r) {
     m->req[4] = s;
 }
 
+// One resident move server per device, and only while a single handle is making host-path
+// evaluations there: a server occupies every SM, so the servers (and the launch-path kernels)
+// of other handles on the same device would queue behind it for up to its lifetime.  A handle
+// that finds another handle's server resident asks it to yield (request word 5; the leader
+// retires after the move in flight), marks the device contended for a while, and uses the
+// launch path; contended handles do not start servers.
+struct DeviceServers {
+    std::mutex mu;
+    std::atomic<qmmm_field *> owner{nullptr};   // handle whose server is resident (or starting)
+    qmmm_field *last_host = nullptr;    // handle of the most recent host-path evaluation
+    double last_host_t = 0.0, contended_until = 0.0;
+};
+DeviceServers g_servers[MAX_DEVICES];
+constexpr double CONTENDED_S = 0.05;
+
+// Called by every evaluation that launches kernels: a resident server of ANOTHER handle on
+// this device is asked to retire (its owner restarts it when the device is quiet again).
+void yield_foreign_server(qmmm_field *h) {
+    DeviceServers &ds = g_servers[h->device];
+    qmmm_field *o = ds.owner.load(std::memory_order_acquire);
+    if (o == nullptr || o == h) return;                      // re-checked under the lock
+    std::lock_guard<std::mutex> lk(ds.mu);
+    o = ds.owner.load();
+    if (o && o != h && o->srv_mail_h) {
+        o->srv_mail_h->req[5] = 1;
+        ds.contended_until = now_seconds() + CONTENDED_S;
+    }
+}
+// Host-path evaluation by h: two different handles within CONTENDED_S = contention.
+void note_host_eval(qmmm_field *h) {
+    DeviceServers &ds = g_servers[h->device];
+    std::lock_guard<std::mutex> lk(ds.mu);
+    const double t = now_seconds();
+    if (ds.last_host && ds.last_host != h && t - ds.last_host_t < CONTENDED_S) ds.contended_until = t + CONTENDED_S;
+    ds.last_host = h;
+    ds.last_host_t = t;
+}
+void server_retired(qmmm_field *h) {
+    DeviceServers &ds = g_servers[h->device];
+    std::lock_guard<std::mutex> lk(ds.mu);
+    if (ds.owner.load() == h) ds.owner = nullptr;
+    h->srv_alive = false;
+}
+void forget_handle(qmmm_field *h) {              // destroy
+    DeviceServers &ds = g_servers[h->device];
+    std::lock_guard<std::mutex> lk(ds.mu);
+    if (ds.owner.load() == h) ds.owner = nullptr;
+    if (ds.last_host == h) ds.last_host = nullptr;
+}
+
 // Waits until the server launch `h->srv_launch_id` has retired, then joins its stream.
 qmmm_status server_join(qmmm_field *h) {
     const double t0 = now_seconds();
@@ -630,7 +717,7 @@ qmmm_status server_join(qmmm_field *h) {
         if (now_seconds() - t0 > 10.0) return fail(QMMM_ERR_CUDA, "move server did not retire");
     }
     CUDA_TRY(cudaStreamSynchronize(h->srv_stream));
-    h->srv_alive = false;
+    server_retired(h);
     return QMMM_OK;
 }
 
@@ -646,8 +733,10 @@ qmmm_status server_stop(qmmm_field *h) {
 template <typename REAL>
 cudaError_t server_launch(const ServerParams &sp, int slices, size_t smem, cudaStream_t st) {
     auto kern = move_server_kernel<REAL>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         static_cast<int>(smem));
+    static SmemConfig configured;
+    static const char *const name = kernel_name(reinterpret_cast<const void *>(kern));
+    g_launched = name;
+    cudaError_t e = configured.ensure(kern, smem);
     if (e != cudaSuccess) return e;
     void *args[] = {const_cast<ServerParams *>(&sp)};
     return cudaLaunchCooperativeKernel(reinterpret_cast<void *>(kern), dim3(1, slices),
@@ -667,6 +756,21 @@ qmmm_status server_start(qmmm_field *h, int prec, bool *usable) {
     size_t smem = pair_smem_bytes(f32, pl.stages, 1, 1) + extra;
     while (smem > 227 * 1024 && pl.stages > 2) smem = pair_smem_bytes(f32, --pl.stages, 1, 1) + extra;
 
+    {
+        // one resident server per device, and none while several handles make host-path calls
+        DeviceServers &ds = g_servers[h->device];
+        std::lock_guard<std::mutex> lk(ds.mu);
+        qmmm_field *o = ds.owner.load();
+        if (o && o != h) {
+            if (o->srv_mail_h) o->srv_mail_h->req[5] = 1;
+            ds.contended_until = now_seconds() + CONTENDED_S;
+            return QMMM_OK;
+        }
+        if (now_seconds() < ds.contended_until) return QMMM_OK;
+        ds.owner = h;
+        h->srv_mail_h->req[5] = 0;
+    }
+    g_device = h->device;
     ServerParams sp;
     std::memset(&sp, 0, sizeof(sp));
     PairParams &prm = sp.pair;
@@ -692,16 +796,25 @@ qmmm_status server_start(qmmm_field *h, int prec, bool *usable) {
     ServerDevice init;
     std::memset(&init, 0, sizeof(init));
     init.cmd = h->srv_seq;
-    CUDA_TRY(cudaMemcpy(h->srv_dev, &init, sizeof(init), cudaMemcpyHostToDevice));
-    CUDA_TRY(cudaMemset(h->workspace, 0, static_cast<size_t>(pl.slices) * SLOT_WORDS * 8));   // untagged slots
+    {
+        cudaError_t e0 = cudaMemcpy(h->srv_dev, &init, sizeof(init), cudaMemcpyHostToDevice);
+        if (e0 == cudaSuccess)
+            e0 = cudaMemset(h->workspace, 0, static_cast<size_t>(pl.slices) * SLOT_WORDS * 8);   // untagged slots
+        if (e0 != cudaSuccess) {
+            server_retired(h);
+            return cuda_fail(e0, "move server set-up");
+        }
+    }
     cudaError_t e = f32 ? server_launch<float>(sp, pl.slices, smem, h->srv_stream)
                         : server_launch<double>(sp, pl.slices, smem, h->srv_stream);
     if (e != cudaSuccess) {                    // e.g. the GPU is shared and cannot hold the grid
         cudaGetLastError();
         h->srv_ok = false;
+        server_retired(h);
         return QMMM_OK;
     }
     h->srv_alive = true;
+    h->last_kernel = g_launched;
     h->srv_prec = prec;
     h->last_plan = pl;
     h->last_point_blocks = 1;
@@ -728,13 +841,13 @@ qmmm_status server_move(qmmm_field *h, const double *r, double *V, double *E, in
     const unsigned long long s = ++h->srv_seq;
     post_request(m, s, r);
     const double t0 = now_seconds();
-    auto answered = [&]() { return m->ans[0] == s && m->ans[5] == s; };
+    auto answered = [&]() { return m->ans[0] == s && m->ans[2] == s && m->ans[4] == s && m->ans[6] == s; };
     for (uint64_t spin = 1; !answered(); ++spin) {
         if (m->exited == h->srv_launch_id) {
             // the server retired (idle / lifetime) before taking this move: start a new one,
             // the request stays posted
             CUDA_TRY(cudaStreamSynchronize(h->srv_stream));
-            h->srv_alive = false;
+            server_retired(h);
             if (answered()) break;
             --h->srv_seq;                              // server_start reposts seq_req = srv_seq
             bool usable = false;
@@ -748,8 +861,9 @@ qmmm_status server_move(qmmm_field *h, const double *r, double *V, double *E, in
             return fail(QMMM_ERR_CUDA, "move server did not answer");
     }
     std::atomic_thread_fence(std::memory_order_acquire);
-    unsigned long long bits[4] = {m->ans[1], m->ans[2], m->ans[3], m->ans[4]};
-    if (m->ans[0] != s || m->ans[5] != s)
+    unsigned long long bits[4] = {m->ans[1], m->ans[3], m->ans[5], m->ans[7]};
+    std::atomic_thread_fence(std::memory_order_acquire);
+    if (!answered())
         return fail(QMMM_ERR_CUDA, "move server: answer line changed while it was read");
     std::memcpy(V, &bits[0], 8);
     if (E) std::memcpy(E, &bits[1], 24);
@@ -799,6 +913,9 @@ qmmm_status alloc_runtime(qmmm_field *h) {
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device);
         h->srv_ok = coop != 0;
     }
+    RT_TRY(cudaHostAlloc(&h->dev_err_h, 64, cudaHostAllocMapped));
+    std::memset(h->dev_err_h, 0, 64);
+    RT_TRY(cudaHostGetDevicePointer(&h->dev_err_d, h->dev_err_h, 0));
     RT_TRY(cudaMalloc(&h->stage_elec, h->max_points * 3 * sizeof(double)));
     RT_TRY(cudaMalloc(&h->stage_out, h->max_points * 4 * sizeof(double)));
 #undef RT_TRY
@@ -818,7 +935,8 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
     if (!out) return fail(QMMM_ERR_INVALID_ARG, "create: out is NULL");
     *out = nullptr;
     if (M < 0 || K < 0) return fail(QMMM_ERR_INVALID_ARG, "create: negative M or K");
-    if (max_points < 1) return fail(QMMM_ERR_INVALID_ARG, "create: max_points < 1");
+    if (max_points < 1 || max_points > INT_MAX)
+        return fail(QMMM_ERR_INVALID_ARG, "create: max_points must be in [1, 2^31 - 1]");
     if (M > 0 && (!src_xyz || !src_q))
         return fail(QMMM_ERR_INVALID_ARG, "create: NULL source array with M > 0");
     if (K > 0 && (!nuc_xyz || !nuc_Z))
@@ -947,7 +1065,8 @@ qmmm_status qmmm_field_create_grid3(const double *origin, const double *spacing,
     const double total = static_cast<double>(n[0]) * n[1] * n[2];
     if (total > 2.0e9) return fail(QMMM_ERR_INVALID_ARG, "create_grid: more than 2e9 cells");
     if (K < 0) return fail(QMMM_ERR_INVALID_ARG, "create_grid: negative K");
-    if (max_points < 1) return fail(QMMM_ERR_INVALID_ARG, "create_grid: max_points < 1");
+    if (max_points < 1 || max_points > INT_MAX)
+        return fail(QMMM_ERR_INVALID_ARG, "create_grid: max_points must be in [1, 2^31 - 1]");
     if (K > 0 && (!nuc_xyz || !nuc_Z))
         return fail(QMMM_ERR_INVALID_ARG, "create_grid: NULL nuclear array with K > 0");
 
@@ -1022,7 +1141,8 @@ qmmm_status qmmm_field_share(const qmmm_field *parent, int64_t max_points, qmmm_
     if (!out) return fail(QMMM_ERR_INVALID_ARG, "share: out is NULL");
     *out = nullptr;
     if (!parent || !parent->keep) return fail(QMMM_ERR_INVALID_ARG, "share: NULL or incomplete parent handle");
-    if (max_points < 1) return fail(QMMM_ERR_INVALID_ARG, "share: max_points < 1");
+    if (max_points < 1 || max_points > INT_MAX)
+        return fail(QMMM_ERR_INVALID_ARG, "share: max_points must be in [1, 2^31 - 1]");
     int dev = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     if (dev != parent->device)
@@ -1088,6 +1208,8 @@ qmmm_status qmmm_field_get_grid_info(const qmmm_field *h, qmmm_grid_info *info) 
 qmmm_status qmmm_field_destroy(qmmm_field *h) {
     if (!h) return QMMM_OK;
     server_stop(h);
+    forget_handle(h);
+    if (h->dev_err_h) cudaFreeHost(h->dev_err_h);
     if (h->srv_stream) cudaStreamDestroy(h->srv_stream);
     if (h->srv_mail_h) cudaFreeHost(h->srv_mail_h);
     cudaFree(h->srv_dev);
@@ -1170,6 +1292,8 @@ qmmm_status qmmm_field_get_info(const qmmm_field *h, qmmm_field_info *info) {
     info->last_launches = h->last_launches;
     info->sm_count = h->sm_count;
     info->last_dz_table = h->last_dz_table;
+    info->device_errors = h->dev_err_h ? *reinterpret_cast<volatile int *>(h->dev_err_h) : 0;
+    std::strncpy(info->last_kernel, h->last_kernel ? h->last_kernel : "", sizeof(info->last_kernel) - 1);
     return QMMM_OK;
 }
 
@@ -1187,14 +1311,24 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
     const bool f32 = prec == QMMM_FP32_ACC64;
     const int P = static_cast<int>(W * N);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    {
+        // launches, the shared-memory attribute and the handle's buffers belong to h->device
+        int cur = -1;
+        CUDA_TRY(cudaGetDevice(&cur));
+        if (cur != h->device)
+            return fail(QMMM_ERR_INVALID_ARG, "eval: the current device is not the handle's device");
+        g_device = cur;
+    }
     if (h->srv_alive) {                    // the resident server owns the workspace: retire it
         qmmm_status ss = server_stop(h);
         if (ss != QMMM_OK) return ss;
     }
+    yield_foreign_server(h);               // another handle's resident server would hold every SM
 
     // overlapped launch (and the few-point plans that go with it): not between timing events,
     // not for the mailbox path, whose host reads V and E behind a flag
     h->overlap_now = h->overlap && !h->timing && !host_flag;
+    const bool pdl_attr = h->overlap_now && !h->pdl_hold;
     const bool grid = h->layout == QMMM_LAYOUT_GRID ||
                       (h->layout == QMMM_LAYOUT_AUTO && auto_uses_grid(h, P, f32));
     qmmm_plan pl = choose_plan(h, P, f32, grid);
@@ -1235,7 +1369,8 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
         prm.done = h->counters + h->max_points;
         // overlap with the previous evaluation on this stream (not with the timing events in
         // between, and not for the mailbox path, whose host reads V and E behind a flag)
-        prm.pdl = h->overlap_now ? 1 : 0;
+        prm.pdl = pdl_attr ? 1 : 0;
+        prm.dev_err = h->dev_err_d;
         // Few points, all CTAs of the launch resident together (at most
         // one per SM, so the collecting CTAs cannot keep the pushing ones from starting):
         // collect the CTA partials by tagged records instead of fence + ticket -- about 1 us
@@ -1301,6 +1436,7 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
         ++launches;
     }
     h->last_layout = grid ? QMMM_LAYOUT_GRID : QMMM_LAYOUT_LIST;
+    h->last_kernel = g_launched;
     if (h->timing) {
         CUDA_TRY(cudaEventRecord(h->ev[1], st));
         h->timed = true;
@@ -1330,9 +1466,15 @@ qmmm_status qmmm_field_eval_moves(qmmm_field *h, const double *elec_xyz, int64_t
     const bool was = h->overlap;
     h->overlap = true;
     qmmm_status s = QMMM_OK;
-    for (int64_t i = 0; i < n && s == QMMM_OK; ++i)
+    for (int64_t i = 0; i < n && s == QMMM_OK; ++i) {
+        // the first move is launched with plain stream serialization (it reads elec_xyz, which
+        // whatever precedes the call on the stream may have produced); moves 1.. overlap with
+        // their predecessor, which is this library's own evaluation
+        h->pdl_hold = i == 0;
         s = eval_impl(h, elec_xyz + i * N * 3, 1, N, V + i * N, E ? E + i * N * 3 : nullptr, prec, stream,
                       nullptr);
+    }
+    h->pdl_hold = false;
     h->overlap = was;
     return s;
 }
@@ -1353,6 +1495,17 @@ qmmm_status qmmm_field_eval_energy(qmmm_field *h, const double *elec_xyz, int64_
     return QMMM_OK;
 }
 
+qmmm_status qmmm_sum_rank_partials(const double *parts, int64_t R, int64_t n, double *out, void *stream) {
+    if (!parts || !out) return fail(QMMM_ERR_INVALID_ARG, "sum_rank_partials: NULL pointer");
+    if (R < 1 || R > 65536 || n < 0) return fail(QMMM_ERR_INVALID_ARG, "sum_rank_partials: need 1 <= R <= 65536, n >= 0");
+    if (n == 0) return QMMM_OK;
+    sum_rank_partials_kernel<<<static_cast<unsigned>((n + 255) / 256), 256, 0, static_cast<cudaStream_t>(stream)>>>(
+        parts, static_cast<int>(R), n, out);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "sum_rank_partials_kernel launch");
+    return QMMM_OK;
+}
+
 qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int64_t W,
                                  int64_t N, double *V_host, double *E_host, int prec,
                                  void *stream) {
@@ -1363,6 +1516,8 @@ qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int
         return fail(QMMM_ERR_INVALID_ARG, "eval_host: W*N must be in [1, max_points]");
     const int64_t P = W * N;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    note_host_eval(h);
+    auto device_error = [&]() -> bool { return *reinterpret_cast<volatile int *>(h->dev_err_h) != 0; };
     if (P == 1 && (prec == QMMM_FP64 || prec == QMMM_FP32_ACC64)) {
         // one point per call is the paper's own loop: served by the resident move server
         bool served = false;
@@ -1392,10 +1547,15 @@ qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int
             uint64_t spin = 1;
             for (int64_t p = 0; p < P; ++p) {
                 const volatile unsigned long long *r = rec + p * 8;
+                // four self-validating 16-byte units {tag, value}: each is one aligned 16-byte
+                // store of the device, so a value is read after (and re-checked against) its tag
+                auto complete = [&]() { return r[0] == tag && r[2] == tag && r[4] == tag && r[6] == tag; };
                 for (;;) {
-                    if (r[0] == tag && r[5] == tag) {         // both ends of the 48-byte record (one
-                        std::atomic_thread_fence(std::memory_order_acquire);   // store, one line)
-                        const unsigned long long bits[4] = {r[1], r[2], r[3], r[4]};
+                    if (complete()) {
+                        std::atomic_thread_fence(std::memory_order_acquire);
+                        const unsigned long long bits[4] = {r[1], r[3], r[5], r[7]};
+                        std::atomic_thread_fence(std::memory_order_acquire);
+                        if (!complete()) continue;
                         std::memcpy(V_host + p, &bits[0], 8);
                         if (E_host) std::memcpy(E_host + 3 * p, &bits[1], 24);
                         break;
@@ -1403,11 +1563,13 @@ qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int
                     if ((++spin & 0xFFFF) == 0) {             // now and then: did the launch fail?
                         cudaError_t q = cudaStreamQuery(st);
                         if (q != cudaSuccess && q != cudaErrorNotReady) return cuda_fail(q, "eval_host: kernel");
-                        if (q == cudaSuccess && !(r[0] == tag && r[5] == tag))
+                        if (q == cudaSuccess && !complete())
                             return fail(QMMM_ERR_CUDA, "eval_host: kernel finished without publishing its result");
                     }
                 }
             }
+            if (device_error())
+                return fail(QMMM_ERR_CUDA, "eval_host: a cross-CTA collection timed out on the device (results are NaN)");
             return QMMM_OK;
         }
         for (uint64_t spin = 1; *flag_h != h->seq; ++spin) {
@@ -1421,6 +1583,8 @@ qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int
         std::atomic_thread_fence(std::memory_order_acquire);
         std::memcpy(V_host, out_h, P * sizeof(double));
         if (E_host) std::memcpy(E_host, out_h + P, P * 3 * sizeof(double));
+        if (device_error())
+            return fail(QMMM_ERR_CUDA, "eval_host: a cross-CTA collection timed out on the device (results are NaN)");
         return QMMM_OK;
     }
     CUDA_TRY(cudaMemcpyAsync(h->stage_elec, elec_xyz_host, P * 3 * sizeof(double),
@@ -1438,6 +1602,8 @@ qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int
             CUDA_TRY(cudaMemcpyAsync(E_host, dE, P * 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
     }
     CUDA_TRY(cudaStreamSynchronize(st));
+    if (device_error())
+        return fail(QMMM_ERR_CUDA, "eval_host: a cross-CTA collection timed out on the device (results are NaN)");
     return QMMM_OK;
 }
 

@@ -75,6 +75,8 @@ struct PairParams {
     int inline_pts;
     double pts[3 * 32];
     int pdl;                 // host side only: launch with programmatic stream serialization
+    int *dev_err;            // device-mapped host word: set when a bounded wait gave up (never expected)
+    int kernel_id;           // host side only: which instantiation was launched (qmmm_field_info.last_kernel)
 #ifdef QMMM_PHASE_TIMING
     long long *dbg;          // [CTAs][10] clock64 at phase boundaries + globaltimer (diagnostic build)
 #endif
@@ -341,15 +343,28 @@ __device__ __forceinline__ void finish_point_block(const PairParams &prm, int pp
 // For overlapped few-point evaluations (qmmm_field_set_overlap) the serial tail of an
 // evaluation -- partial store, fence, ticket atomic, fence, last-CTA loads -- is what bounds
 // the period of a sequence (measured in isolation: 2.6 us at 37 CTAs, 3.4 us at 148).  Here
-// every CTA instead stores each of its points' partials as ONE tagged 64-byte record
-// {tag, V, Ex, Ey, Ez, tag} (no fence, no atomic) and the CTA of slice 0 collects: its threads
-// poll the records with volatile 16-byte loads until both tags carry this evaluation's tag
-// (1.4 us at 37 CTAs, 2.5 us at 148), then add the slices in exactly the order of
-// finish_point_block.  Tags are unique per evaluation, so nothing is reset; a record is
-// overwritten only by a later evaluation, which pushes after its griddepcontrol.wait, i.e.
-// after this evaluation has completed.  A record that never arrives (cannot happen: every CTA
-// of the grid pushes unconditionally) ends the poll after PUSH_HARD_NS with NaN results
-// instead of a hang.
+// every CTA instead stores each of its points' partials as ONE tagged 64-byte record of four
+// self-validating 16-byte units {tag, V} {tag, Ex} {tag, Ey} {tag, Ez} (no fence, no atomic)
+// and the CTA of slice 0 collects: its threads poll the records with volatile 16-byte loads
+// until all four units carry this evaluation's tag (1.4 us at 37 CTAs, 2.5 us at 148), then add
+// the slices in exactly the order of finish_point_block.
+//
+// What the protocol rests on: a naturally aligned 16-byte vector store / load of one thread
+// (st.v2.u64 / ld.v2.u64) is performed as one access, so a unit is seen whole or not at all;
+// nothing is assumed about the order in which the four units of a record, or different
+// records, become visible.  (An earlier layout -- six 8-byte stores, tags at both ends of a
+// 48-byte record -- assumed that a 32-byte sector is written atomically.)
+//
+// Tags.  A record is taken when its tags equal prm.push_seq, which is unique per evaluation
+// ISSUED by the host -- but a kernel parameter, so a CUDA graph replays an evaluation with the
+// same tag.  The collector therefore CLEARS the tags of every record it has consumed: when the
+// same graph node runs again, its slots are untagged until this replay's CTAs push.  The
+// clearing stores cannot race with the next evaluation's pushes: those are issued after its
+// griddepcontrol.wait (overlapped launches) or after the kernel boundary (serial launches),
+// i.e. after this grid has completed and its memory operations are visible.  A record that
+// never arrives (cannot happen: every CTA of the grid pushes unconditionally) ends the poll
+// after PUSH_HARD_NS with NaN results and sets the handle's device error word
+// (qmmm_field_info.device_errors; the host-buffer calls return QMMM_ERR_CUDA).
 constexpr int PUSH_SLOT_WORDS = 8;
 constexpr long long PUSH_HARD_NS = 2000000000ll;
 __device__ __forceinline__ long long push_global_ns() {
@@ -357,26 +372,25 @@ __device__ __forceinline__ long long push_global_ns() {
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return t;
 }
-// Warps with ws == 0 call this with all 32 lanes: lane 4 e + c holds value c of the warp's
-// point e (first point pbase); EPT <= 4.
-template <int EPT>
-__device__ __forceinline__ void push_records(const PairParams &prm, double a, int pbase, int lane) {
-    static_assert(EPT <= 4, "six record words per point in one warp");
-    const int e = lane / 6, w = lane - 6 * e;
-    const int src = e < EPT ? 4 * e + (w == 0 || w == 5 ? 0 : w - 1) : 0;
-    const double v = __shfl_sync(0xffffffffu, a, src);
-    const unsigned long long word = (w == 0 || w == 5) ? prm.push_seq
-                                                       : static_cast<unsigned long long>(__double_as_longlong(v));
-    const int p = pbase + e;
-    if (e < EPT && p < prm.P)
-        *reinterpret_cast<volatile unsigned long long *>(
-            prm.push_slots + (static_cast<int64_t>(blockIdx.y) * prm.P + p) * PUSH_SLOT_WORDS + w) = word;
-}
 struct push_u64x2 { unsigned long long x, y; };
 __device__ __forceinline__ push_u64x2 push_ld_v2(const unsigned long long *p) {
     push_u64x2 r;
     asm volatile("ld.volatile.global.v2.u64 {%0, %1}, [%2];" : "=l"(r.x), "=l"(r.y) : "l"(p));
     return r;
+}
+__device__ __forceinline__ void push_st_v2(unsigned long long *p, unsigned long long a, unsigned long long b) {
+    asm volatile("st.volatile.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");
+}
+// Warps with ws == 0 call this with all 32 lanes: lane 4 e + c holds value c of the warp's
+// point e (first point pbase); EPT <= 4.  One 16-byte store {tag, value} per lane.
+template <int EPT>
+__device__ __forceinline__ void push_records(const PairParams &prm, double a, int pbase, int lane) {
+    static_assert(EPT <= 4, "four units per point, at most sixteen lanes");
+    const int e = lane >> 2, c = lane & 3;
+    const int p = pbase + e;
+    if (lane < 4 * EPT && p < prm.P)
+        push_st_v2(prm.push_slots + (static_cast<int64_t>(blockIdx.y) * prm.P + p) * PUSH_SLOT_WORDS + 2 * c,
+                   prm.push_seq, static_cast<unsigned long long>(__double_as_longlong(a)));
 }
 // All NT threads of every CTA call this after the records are pushed.  rec_s: shared memory
 // for slices * ppb * 4 doubles (the idle stage buffers), scratch: NT doubles, flag: one int.
@@ -393,17 +407,25 @@ __device__ __forceinline__ void finish_point_block_push(const PairParams &prm, i
         const int p = blockIdx.x * ppb + pp;
         double *dst = rec_s + 4 * r;
         if (p >= prm.P) { dst[0] = dst[1] = dst[2] = dst[3] = 0.0; continue; }
-        const unsigned long long *q = prm.push_slots + (static_cast<int64_t>(sl) * prm.P + p) * PUSH_SLOT_WORDS;
+        unsigned long long *q = prm.push_slots + (static_cast<int64_t>(sl) * prm.P + p) * PUSH_SLOT_WORDS;
         for (;;) {
-            const push_u64x2 a = push_ld_v2(q), b = push_ld_v2(q + 2), c = push_ld_v2(q + 4);
-            if (a.x == prm.push_seq && c.y == prm.push_seq) {
+            const push_u64x2 a = push_ld_v2(q), b = push_ld_v2(q + 2), c = push_ld_v2(q + 4), d = push_ld_v2(q + 6);
+            if (a.x == prm.push_seq && b.x == prm.push_seq && c.x == prm.push_seq && d.x == prm.push_seq) {
                 dst[0] = __longlong_as_double(static_cast<long long>(a.y));
-                dst[1] = __longlong_as_double(static_cast<long long>(b.x));
-                dst[2] = __longlong_as_double(static_cast<long long>(b.y));
-                dst[3] = __longlong_as_double(static_cast<long long>(c.x));
+                dst[1] = __longlong_as_double(static_cast<long long>(b.y));
+                dst[2] = __longlong_as_double(static_cast<long long>(c.y));
+                dst[3] = __longlong_as_double(static_cast<long long>(d.y));
+                // consumed: untag, so that a replay of this launch (CUDA graph: same tag) waits
+                // for its own records
+#pragma unroll
+                for (int u = 0; u < 4; ++u) push_st_v2(q + 2 * u, 0ull, 0ull);
                 break;
             }
-            if (push_global_ns() - t0 > PUSH_HARD_NS) { *flag = 0; break; }
+            if (push_global_ns() - t0 > PUSH_HARD_NS) {
+                *flag = 0;
+                if (prm.dev_err) *reinterpret_cast<volatile int *>(prm.dev_err) = 1;
+                break;
+            }
         }
     }
     sync();
@@ -432,23 +454,11 @@ __device__ __forceinline__ void finish_point_block_push(const PairParams &prm, i
         if (!ok) r = __longlong_as_double(0x7ff8000000000000ll);
     }
     if (prm.host_records) {
-        // threads 0 .. nval-1 hold value (tid & 3) of the CTA's point tid >> 2: eight points per
-        // warp, written as two groups of four records (six lanes each, one store instruction)
-        if (tid < ((nval + 31) & ~31)) {
-            const int lane = tid & 31, wbase = (tid >> 5) * 8;
-#pragma unroll
-            for (int half = 0; half < 2; ++half) {
-                const int e = lane / 6, w = lane - 6 * e;
-                const int src = (4 * half + (e < 4 ? e : 0)) * 4 + ((w == 0 || w == 5) ? 0 : w - 1);
-                const double val = __shfl_sync(0xffffffffu, r, src);
-                const unsigned long long word =
-                    (w == 0 || w == 5) ? prm.push_seq : static_cast<unsigned long long>(__double_as_longlong(val));
-                const int lp = wbase + 4 * half + e, gp = blockIdx.x * ppb + lp;
-                if (e < 4 && lp < ppb && gp < prm.P)
-                    *reinterpret_cast<volatile unsigned long long *>(
-                        prm.host_records + static_cast<int64_t>(gp) * PUSH_SLOT_WORDS + w) = word;
-            }
-        }
+        // thread (g == 0, v) holds value v & 3 of the CTA's point v >> 2: one 16-byte store
+        // {tag, value} into the point's record in pinned host memory
+        if (mine)
+            push_st_v2(prm.host_records + static_cast<int64_t>(p) * PUSH_SLOT_WORDS + 2 * (v & 3), prm.push_seq,
+                       static_cast<unsigned long long>(__double_as_longlong(r)));
     } else if (mine) {
         if ((v & 3) == 0) prm.V[p] = r;
         else if (prm.E) prm.E[3 * static_cast<int64_t>(p) + (v & 3) - 1] = r;
@@ -1008,6 +1018,19 @@ __global__ void __launch_bounds__(256) walker_energy_kernel(const double *V, int
     for (; i < N; i += 32) a0 += v[i];
     const double s = warp_sum((a0 + a1) + (a2 + a3));
     if (lane == 0) U[w] = -s;
+}
+
+// ----------------------------------------------------------------------------- rank partials
+// Eq. 5 across devices (U = B[1] + ... + B[N_B], one block per GPU): the
+// per-rank partials parts[r][n] are added in RANK ORDER 0, 1, 2, ... (a plain left-to-right
+// sum), so every rank that holds the same gathered partials gets bitwise the same result.
+__global__ void __launch_bounds__(256) sum_rank_partials_kernel(const double *parts, int R, int64_t n,
+                                                                double *out) {
+    const int64_t i = blockIdx.x * 256ll + threadIdx.x;
+    if (i >= n) return;
+    double a = parts[i];
+    for (int r = 1; r < R; ++r) a += parts[static_cast<int64_t>(r) * n + i];
+    out[i] = a;
 }
 
 // ----------------------------------------------------------------------------- packing

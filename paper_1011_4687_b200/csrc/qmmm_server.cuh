@@ -9,9 +9,10 @@
 //   leader : one warp of CTA 0 polls the request line over PCIe (one transaction), copies r
 //            to device memory, publishes s in cmd
 //   all    : poll cmd (L2), run their source slice exactly like pair_kernel<REAL,1> (TMA ring,
-//            FP64 or FP32-acc64 pair math, in-CTA reduction), store their partial, take a ticket
-//   last   : the CTA with the last ticket adds the partials in a fixed order and stores
-//            {s, V, E, s} to the answer line in one transaction
+//            FP64 or FP32-acc64 pair math, in-CTA reduction)
+//   all    : push their partial as one tagged record (four 16-byte units {s, value})
+//   leader : collects the records, adds them in a fixed order and stores {s, V} {s, Ex}
+//            {s, Ey} {s, Ez} to the answer line
 //
 // The producer warp prefetches the first ring stages of the NEXT move while the CTA waits
 // (the sources do not depend on r), so a move starts on data that is already in shared memory.
@@ -28,8 +29,10 @@ struct ServerMailbox {                 // pinned host memory, device-mapped
     // the host writes seq_a, then r, then seq_b (x86 stores are ordered); the device accepts
     // a snapshot only when seq_a == seq_b (a seqlock), so r always belongs to that move
     volatile unsigned long long req[8];    // [0] seq_a  [1..3] r_new (as bits)  [4] seq_b; EXIT = retire
-    // answer line, written by the device with ONE coalesced store of 6 lanes and validated by
-    // the host the same way: [0] ack_a  [1..4] V, Ex, Ey, Ez (as bits)  [5] ack_b
+                                           // [5] yield: another handle wants the device -- retire
+    // answer line: four self-validating 16-byte units {s, V} {s, Ex} {s, Ey} {s, Ez} (values as
+    // bits), each written by the device with one aligned 16-byte store; the host takes the
+    // answer when all four carry the move number s
     volatile unsigned long long ans[8];
     volatile unsigned long long exited;    // device -> host: launch id that has retired
     volatile unsigned long long pad[7];
@@ -59,31 +62,22 @@ __device__ __forceinline__ long long global_ns() {
     return t;
 }
 
-// Cross-CTA sum of one move, push model.  Every CTA stores its partial as one tagged 48-byte
-// record {s, V, Ex, Ey, Ez, s} (six lanes, one store instruction, one L2 write packet) into
-// its own slot -- no fence, no atomic ticket, and it is free for the next move at once.  The
-// leader CTA collects: thread t polls slot t with three 16-byte volatile loads until both tags
-// carry s, the records go to shared memory, and the slices are added in exactly the order of
-// finish_point_block (so the result is bitwise that of the launch path).  Threads 0..3 then
-// hold V, Ex, Ey, Ez and lanes 0..5 of warp 0 store {s, V, E, s} to the mapped answer line in
-// one transaction -- no system-scope fence (a PCIe round trip each) on the critical path.
+// Cross-CTA sum of one move, push model.  Every CTA stores its partial as one tagged 64-byte
+// record of four self-validating 16-byte units {s, V} {s, Ex} {s, Ey} {s, Ez} (one aligned
+// 16-byte store per lane, as push_records in qmmm_kernels.cuh) into its own slot -- no fence, no
+// atomic ticket, and it is free for the next move at once.  The leader CTA collects: thread t
+// polls slot t with four 16-byte volatile loads until all four tags carry s (move numbers only
+// grow, so nothing is reset), the records go to shared memory, and the slices are added in
+// exactly the order of finish_point_block (so the result is bitwise that of the launch path).
+// Threads 0..3 then hold V, Ex, Ey, Ez and store {s, value} to the mapped answer line -- no
+// system-scope fence (a PCIe round trip each) on the critical path.
 constexpr int SLOT_WORDS = 8;              // 64-byte slots in the partials workspace
 
 __device__ __forceinline__ void server_push(unsigned long long *slots, int lane, double acc,
                                             unsigned long long seq) {
-    // lanes 0..3 hold V, Ex, Ey, Ez; shift them to lanes 1..4, tags in lanes 0 and 5
-    const double up = __shfl_up_sync(0xffffffffu, acc, 1);
-    unsigned long long w = static_cast<unsigned long long>(__double_as_longlong(up));
-    if (lane == 0 || lane == 5) w = seq;
-    if (lane < 6)
-        *reinterpret_cast<volatile unsigned long long *>(slots + blockIdx.y * SLOT_WORDS + lane) = w;
-}
-
-struct u64x2 { unsigned long long x, y; };
-__device__ __forceinline__ u64x2 ld_volatile_v2(const unsigned long long *p) {
-    u64x2 r;
-    asm volatile("ld.volatile.global.v2.u64 {%0, %1}, [%2];" : "=l"(r.x), "=l"(r.y) : "l"(p));
-    return r;
+    if (lane < 4)                          // lanes 0..3 hold V, Ex, Ey, Ez
+        push_st_v2(slots + blockIdx.y * SLOT_WORDS + 2 * lane, seq,
+                   static_cast<unsigned long long>(__double_as_longlong(acc)));
 }
 
 // Leader CTA only; all 256 consumer threads call it.  part_s: [slices][4] doubles of shared
@@ -99,12 +93,12 @@ __device__ __forceinline__ bool server_collect(const PairParams &prm, ServerMail
     for (int sl = tid; sl < prm.slices; sl += NT) {
         const unsigned long long *p = slots + sl * SLOT_WORDS;
         for (;;) {
-            const u64x2 a = ld_volatile_v2(p), b = ld_volatile_v2(p + 2), c = ld_volatile_v2(p + 4);
-            if (a.x == seq && c.y == seq) {
+            const push_u64x2 a = push_ld_v2(p), b = push_ld_v2(p + 2), c = push_ld_v2(p + 4), d = push_ld_v2(p + 6);
+            if (a.x == seq && b.x == seq && c.x == seq && d.x == seq) {
                 part_s[4 * sl + 0] = __longlong_as_double(static_cast<long long>(a.y));
-                part_s[4 * sl + 1] = __longlong_as_double(static_cast<long long>(b.x));
-                part_s[4 * sl + 2] = __longlong_as_double(static_cast<long long>(b.y));
-                part_s[4 * sl + 3] = __longlong_as_double(static_cast<long long>(c.x));
+                part_s[4 * sl + 1] = __longlong_as_double(static_cast<long long>(b.y));
+                part_s[4 * sl + 2] = __longlong_as_double(static_cast<long long>(c.y));
+                part_s[4 * sl + 3] = __longlong_as_double(static_cast<long long>(d.y));
                 break;
             }
             if (global_ns() - t_start > SERVER_HARD_NS) { *flag = 0; break; }
@@ -125,14 +119,11 @@ __device__ __forceinline__ bool server_collect(const PairParams &prm, ServerMail
     }
     scratch[tid] = ((a[0] + a[1]) + (a[2] + a[3])) + ((a[4] + a[5]) + (a[6] + a[7]));
     sync();
-    if (tid < 32) {
+    if (tid < 4) {
         double r = 0.0;
-        if (tid < 4)
-            for (int k = 0; k < G; ++k) r += scratch[k * 4 + tid];
-        const double up = __shfl_up_sync(0xffffffffu, r, 1);
-        unsigned long long w = static_cast<unsigned long long>(__double_as_longlong(up));
-        if (tid == 0 || tid == 5) w = seq;
-        if (tid < 6) mail->ans[tid] = w;
+        for (int k = 0; k < G; ++k) r += scratch[k * 4 + tid];
+        push_st_v2(const_cast<unsigned long long *>(mail->ans) + 2 * tid, seq,
+                   static_cast<unsigned long long>(__double_as_longlong(r)));
     }
     return true;
 }
@@ -225,10 +216,14 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) move_server_kernel(const Serve
                 // lanes 0..4 read the request line over PCIe in one transaction
                 const long long t_idle = global_ns();
                 for (;;) {
-                    w = lane < 5 ? sp.mail->req[lane] : 0ull;
+                    w = lane < 6 ? sp.mail->req[lane] : 0ull;
                     const unsigned long long a = __shfl_sync(0xffffffffu, w, 0);
                     const unsigned long long b = __shfl_sync(0xffffffffu, w, 4);
                     if (a == b && a != last) { c = a; break; }
+                    if (__shfl_sync(0xffffffffu, w, 5) != 0ull) {      // another handle wants the device
+                        c = SERVER_EXIT;
+                        break;
+                    }
                     const long long now = __shfl_sync(0xffffffffu, global_ns(), 0);
                     if (now - t_idle > SERVER_IDLE_NS || now - t_start > SERVER_LIFE_NS) {
                         c = SERVER_EXIT;

@@ -50,13 +50,7 @@ def rel_errors(ref, V, E):
     return eV, eE
 
 
-def check(ref, V, E, tol):
-    eV, eE = rel_errors(ref, V, E)
-    kV = ref.absV / np.abs(ref.V)
-    assert np.all((eV <= tol) | ((kV > 1e3) & (eV / kV <= tol * 1e-3))), f"V: max rel err {eV.max():.3e}"
-    if E is not None:
-        kE = ref.absE / np.linalg.norm(ref.E, axis=1)
-        assert np.all((eE <= tol) | ((kE > 1e3) & (eE / kE <= tol * 1e-3))), f"E: max rel err {eE.max():.3e}"
+from parity_check import check  # noqa: E402  (tests/parity_check.py: the tolerance rule)
 
 
 def random_grid(rng, n, h, origin, fill=0.8, hole=None, signed=False):
@@ -253,11 +247,9 @@ def test_point_on_an_empty_node_is_harmless(torch_cuda, B, oracle_mod, precision
     try:
         V, E = run(torch_cuda, B, hnd, pts, precision)
         assert np.all(np.isfinite(V)) and np.all(np.isfinite(E))
-        eV, _ = rel_errors(ref, V, None)
-        assert eV.max() <= (TOL64 if precision == "fp64" else TOL32)
-        # E at the centre of a symmetric hole is a small difference of large terms: absolute bound
-        scale = ref.absE.max()
-        assert np.max(np.linalg.norm(E - ref.E, axis=1)) <= (1e-12 if precision == "fp64" else 1e-5) * scale
+        # E at the centre of a symmetric hole is a small difference of large terms (kappa_E far
+        # above 1e3): check() holds it to err / kappa, everything else to the plain tolerance
+        check(ref, V, E, TOL64 if precision == "fp64" else TOL32)
     finally:
         B.qmmm_field_destroy(hnd)
 
@@ -292,7 +284,7 @@ def test_grid_symmetry_pins_without_the_oracle(torch_cuda, B):
 
 
 # ------------------------------------------------------------ the bench configurations
-def test_config3_grid_fp32_full_energy(torch_cuda, B, oracle_mod):
+def test_config3_grid_fp32_full_energy(torch_cuda, B, oracle_mod, full_oracle):
     """Config 3 in the launch configuration bench.py times (AUTO -> grid kernels): V and E on a
     seeded 1 % subsample, the total energy per walker and whole batch against the oracle on
     all 16,384 points; the list layout on the same handle for comparison."""
@@ -305,10 +297,9 @@ def test_config3_grid_fp32_full_energy(torch_cuda, B, oracle_mod):
         Vl, El = run(torch_cuda, B, h, pts, "fp32", layout="list")
     finally:
         B.qmmm_field_destroy(h)
-    idx = subsample_points(w.P, 0.01, seed=3)
-    ref = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, pts[idx], want_abs=True)
-    check(ref, V[idx], E[idx], TOL32)
-    full = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, pts, want_E=False)
+    full = full_oracle(3)                         # every point, V and E
+    check(full, V, E, TOL32)
+    check(full, Vl, El, TOL32)
     for name, v in (("grid", V), ("list", Vl)):
         per_walker = np.abs(v.reshape(w.W, w.N).sum(1) - full.V.reshape(w.W, w.N).sum(1))
         batch = abs(v.sum() - full.V.sum())
@@ -318,13 +309,17 @@ def test_config3_grid_fp32_full_energy(torch_cuda, B, oracle_mod):
         assert per_walker.max() <= E_TOL
         assert batch / w.W <= E_TOL
         assert batch <= 1e-4
-    eE = np.linalg.norm(E[idx] - ref.E, axis=1) / np.linalg.norm(ref.E, axis=1)
-    print(f"config3 fp32 grid: max rel err of |E| on the subsample {eE.max():.3e}")
+    for name, e in (("grid", E), ("list", El)):
+        eE = np.linalg.norm(e - full.E, axis=1) / np.linalg.norm(full.E, axis=1)
+        kE = full.absE / np.linalg.norm(full.E, axis=1)
+        print(f"config3 fp32 {name}: max rel err of |E| over all points {eE.max():.3e} "
+              f"(kappa_E max {kE.max():.1f}; E uses the raw MUFU.RSQ value, DESIGN.md reading 21)")
 
 
-def test_config4_grid_fp64(torch_cuda, B, oracle_mod):
+def test_config4_grid_fp64(torch_cuda, B, full_oracle):
     """Config 4 (16.7 M cells x 2,048 points, FP64) in bench.py's launch configuration
-    (AUTO -> grid kernels); oracle on 24 sampled points; list layout for comparison."""
+    (AUTO -> grid kernels): V and E of all 2,048 points against the oracle, for the grid
+    kernel and its potential-only variant (the list kernels: tests/test_parity_gpu.py)."""
     w = make_workload(4)
     pts = w.elec_xyz.reshape(-1, 3)
     h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, len(pts))
@@ -333,17 +328,14 @@ def test_config4_grid_fp64(torch_cuda, B, oracle_mod):
         assert gi["present"] and gi["n"] == (256, 256, 256)
         V, E = run(torch_cuda, B, h, pts, "fp64")
         assert B.qmmm_field_get_grid_info(h)["last_layout"] == "grid"
+        assert B.qmmm_field_get_info(h)["last_dz_table"]
         Vp, _ = run(torch_cuda, B, h, pts, "fp64", want_E=False)
-        Vl, El = run(torch_cuda, B, h, pts, "fp64", layout="list")
+        assert B.qmmm_field_get_grid_info(h)["last_layout"] == "grid"
     finally:
         B.qmmm_field_destroy(h)
-    idx = subsample_points(w.P, 24 / w.P, seed=4)
-    ref = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, pts[idx], want_abs=True)
-    check(ref, V[idx], E[idx], TOL64)
-    check(ref, Vp[idx], None, TOL64)
-    assert np.all(np.isfinite(V)) and np.all(np.isfinite(E))
-    assert np.max(np.abs(V - Vl) / np.abs(Vl)) <= 1e-12
-    assert np.max(np.linalg.norm(E - El, axis=1) / np.linalg.norm(El, axis=1)) <= 1e-11
+    ref = full_oracle(4)
+    check(ref, V, E, TOL64)
+    check(ref, Vp, None, TOL64)
 
 
 # ------------------------------------------------------------------ per-walker energy (Eq. 4)
@@ -415,13 +407,11 @@ def test_random_grids_plans_and_precisions(torch_cuda, B, oracle_mod):
                         slices=int(rng.choice([0, 1, 3, 37, 200])), stages=int(rng.choice([0, 2, 5, 8])))
             want_E = bool(rng.random() < 0.8)
             V, E = run(torch_cuda, B, hnd, pts, precision, want_E=want_E, layout="grid", plan=plan)
-            eV, eE = rel_errors(ref, V, E)
-            kV = ref.absV / np.abs(ref.V)
-            kE = ref.absE / np.linalg.norm(ref.E, axis=1)
             msg = f"case {case}: n={n} h={h} P={P} {precision} plan={plan} list={use_list}"
-            assert np.all(eV <= tol * np.maximum(1.0, kV)), f"{msg}: V rel err {eV.max():.3e}"
-            if want_E:
-                assert np.all(eE <= tol * np.maximum(1.0, kE)), f"{msg}: E rel err {eE.max():.3e}"
+            try:
+                check(ref, V, E if want_E else None, tol)
+            except AssertionError as exc:
+                raise AssertionError(f"{msg}: {exc}") from None
         finally:
             B.qmmm_field_destroy(hnd)
 

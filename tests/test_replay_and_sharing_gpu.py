@@ -1,0 +1,161 @@
+"""Robustness of the few-point machinery (tagged records, CUDA-graph replay, shared handles on
+several host threads, resident move servers) -- every result against the CPU oracle.
+
+* A CUDA graph that holds ONE evaluation is replayed with new positions in the same buffer:
+  the record tags are kernel parameters, i.e. frozen in the graph, so a replay must not take
+  the previous replay's records for its own (the collector clears the tags it has consumed;
+  qmmm_kernels.cuh "Tags").
+* Several host threads, each with its own handle on one environment (qmmm_field_share;
+  PAPER.md:23, :242: OpenMP on the host code, several ranks per GPU), make single-point
+  host-buffer calls at once: one resident move server per device at most, nobody times out.
+"""
+import threading
+import time
+
+import numpy as np
+import pytest
+
+from paper_1011_4687_b200.workloads import make_workload
+from parity_check import check
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"fp64": 1e-12, "fp32": 1e-5}
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1011_4687_b200 import binding
+    return binding
+
+
+@pytest.mark.parametrize("layout", ["grid", "list"])
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("P", [1, 4, 32])
+@pytest.mark.parametrize("overlap", [False, True])
+def test_single_evaluation_graph_replayed_with_changing_inputs(torch_cuda, B, oracle_mod, layout, precision,
+                                                               P, overlap):
+    torch = torch_cuda
+    w = make_workload(1)
+    rng = np.random.default_rng(100 + P)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, P)
+    try:
+        B.qmmm_field_set_layout(h, layout)
+        B.qmmm_field_set_overlap(h, overlap)
+        batches = [np.ascontiguousarray(rng.normal(size=(P, 3)) * 0.8) for _ in range(6)]
+        refs = [oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, b, want_abs=True) for b in batches]
+        pts = torch.from_numpy(batches[0]).cuda()
+        V = torch.zeros(P, dtype=torch.float64, device="cuda")
+        E = torch.zeros((P, 3), dtype=torch.float64, device="cuda")
+        B.qmmm_field_eval(h, pts, 1, P, V, E, precision)              # eager warm-up
+        torch.cuda.synchronize()
+        eager = (V.cpu().numpy().copy(), E.cpu().numpy().copy())
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            B.qmmm_field_eval(h, pts, 1, P, V, E, precision)          # ONE evaluation in the graph
+        for rep in range(3):                                          # same inputs: bitwise the eager result
+            V.fill_(float("nan")); E.fill_(float("nan"))
+            g.replay()
+            torch.cuda.synchronize()
+            assert np.array_equal(V.cpu().numpy(), eager[0]) and np.array_equal(E.cpu().numpy(), eager[1])
+        for i in list(range(6)) * 4:                                  # the input buffer changes between replays
+            pts.copy_(torch.from_numpy(batches[i]))
+            g.replay()
+            g.replay()                                                # back to back, no sync in between
+            torch.cuda.synchronize()
+            check(refs[i], V.cpu().numpy(), E.cpu().numpy(), TOL[precision])
+        assert B.qmmm_field_get_info(h)["device_errors"] == 0
+    finally:
+        B.qmmm_field_destroy(h)
+
+
+def test_eval_moves_single_move_graph_replay(torch_cuda, B, oracle_mod):
+    """qmmm_field_eval_moves with n = 1 inside a graph (the other call the tags matter for)."""
+    torch = torch_cuda
+    w = make_workload(2, n_points=(8, 1))
+    walk = w.elec_xyz.reshape(-1, 3)
+    ref = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, walk, want_abs=True)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 1)
+    try:
+        for precision in ("fp32", "fp64"):
+            pts = torch.from_numpy(walk[:1].copy()).cuda()
+            V = torch.zeros(1, dtype=torch.float64, device="cuda")
+            E = torch.zeros((1, 3), dtype=torch.float64, device="cuda")
+            B.qmmm_field_eval_moves(h, pts, 1, 1, V, E, precision)
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                B.qmmm_field_eval_moves(h, pts, 1, 1, V, E, precision)
+            got_V, got_E = [], []
+            for i in range(len(walk)):
+                pts.copy_(torch.from_numpy(walk[i:i + 1].copy()))
+                g.replay()
+                torch.cuda.synchronize()
+                got_V.append(V.cpu().numpy()[0]); got_E.append(E.cpu().numpy()[0])
+            check(ref, np.array(got_V), np.array(got_E), TOL[precision])
+    finally:
+        B.qmmm_field_destroy(h)
+
+
+@pytest.mark.parametrize("precision", ["fp32", "fp64"])
+def test_host_threads_with_shared_handles_single_point_calls(torch_cuda, B, oracle_mod, precision):
+    """Six host threads, one handle each on the same environment, 150 single-point
+    qmmm_field_eval_host calls each, all at once.  A resident move server holds every SM, so
+    the library keeps at most one per device and none while several handles are active; every
+    answer must match the oracle and nobody may wait for another handle's server to expire."""
+    w = make_workload(2, n_points=(150, 1))
+    walk = np.ascontiguousarray(w.elec_xyz.reshape(-1, 3))
+    ref = oracle_mod.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, walk, want_abs=True)
+    nthreads = 6
+    parent = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 1)
+    handles = [parent] + [B.qmmm_field_share(parent, 1) for _ in range(nthreads - 1)]
+    results = [None] * nthreads
+    errors = []
+
+    def worker(k):
+        try:
+            import torch
+            torch.cuda.set_device(0)
+            stream = torch.cuda.Stream()
+            V = np.full(len(walk), np.nan); E = np.full((len(walk), 3), np.nan)
+            order = np.roll(np.arange(len(walk)), 17 * k)             # every thread its own order
+            for i in order:
+                v = np.zeros(1); e = np.zeros((1, 3))
+                B.qmmm_field_eval_host(handles[k], walk[i:i + 1], 1, 1, v, e, precision, stream)
+                V[i] = v[0]; E[i] = e[0]
+            results[k] = (V, E)
+        except Exception as exc:                                      # noqa: BLE001
+            errors.append((k, repr(exc)))
+
+    try:
+        t0 = time.perf_counter()
+        threads = [threading.Thread(target=worker, args=(k,)) for k in range(nthreads)]
+        for t in threads:
+            t.start()
+        for t in threads:
+            t.join()
+        elapsed = time.perf_counter() - t0
+        assert not errors, errors
+        for k in range(nthreads):
+            check(ref, results[k][0], results[k][1], TOL[precision])
+        # 900 calls of ~15-60 us each; a thread stuck behind a foreign server would need seconds
+        assert elapsed < 5.0, f"{elapsed:.2f} s for {nthreads * len(walk)} calls"
+        # afterwards a single active handle gets its resident server back (bitwise the launch path
+        # of the LIST layout is checked elsewhere; here: still correct)
+        time.sleep(0.1)
+        v = np.zeros(1); e = np.zeros((1, 3))
+        for i in range(20):
+            B.qmmm_field_eval_host(handles[1], walk[i:i + 1], 1, 1, v, e, precision)
+            assert abs(v[0] - ref.V[i]) <= TOL[precision] * abs(ref.V[i])
+        assert all(B.qmmm_field_get_info(hd)["device_errors"] == 0 for hd in handles)
+    finally:
+        for hd in handles[1:]:
+            B.qmmm_field_destroy(hd)
+        B.qmmm_field_destroy(parent)
