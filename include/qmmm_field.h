@@ -240,6 +240,22 @@ qmmm_status qmmm_field_share(const qmmm_field *parent, int64_t max_points, qmmm_
  */
 qmmm_status qmmm_sum_rank_partials(const double *parts, int64_t R, int64_t n, double *out, void *stream);
 
+/*
+ * FP32 grid kernels: granularity of the coordinate lattice.  The FP32 path keeps every
+ * difference (point - node) EXACT by rounding the point's coordinates to a power-of-two lattice
+ * and corrects V for the rounding residual to first order; E is evaluated at the lattice point
+ * (relative error about 3 x residual / distance per cell).  With one lattice per grid axis the
+ * residual is up to 2^-25 of the axis length in nodes: fine for axes of up to 128 nodes (all FP32
+ * BASELINE configurations), too coarse for long axes with points next to cells.  With a lattice
+ * per work unit (32 rows x 64 z nodes) the residual is 2^-25 of the distance to THAT unit's
+ * farthest node, i.e. a few 1e-6 nodes next to the point whatever the size of the grid, at about
+ * 3 % more time.  mode -1 (default): per work unit when an axis has more than 128 nodes; 0: never;
+ * 1: always.  The source-list FP32 kernels always use a lattice per 2,048-source block.
+ * With it the FP32 tolerances (1e-5 relative per point on V and E) hold for points at least one
+ * cell edge away from every charged cell.  Sticky; INVALID_ARG on another mode.
+ */
+qmmm_status qmmm_field_set_local_lattice(qmmm_field *h, int mode);
+
 /* qmmm_field_destroy -- frees the handle and its device buffers.  NULL is a no-op. */
 qmmm_status qmmm_field_destroy(qmmm_field *h);
 
@@ -269,7 +285,8 @@ typedef struct {
     int32_t device_errors;       /* nonzero: a kernel of this handle gave up a bounded wait (a cross-CTA
                                   * record never arrived; never expected) and wrote NaN results.  Read
                                   * without synchronising; the host-buffer calls return QMMM_ERR_CUDA. */
-    int32_t reserved;
+    int32_t last_local_lattice;  /* 1: the most recent eval ran the FP32 grid kernel with a coordinate
+                                  * lattice per work unit (qmmm_field_set_local_lattice) */
     char last_kernel[192];       /* mangled name of the kernel the most recent evaluation launched (or of
                                   * the move server it started): which template instantiation ran */
 } qmmm_field_info;

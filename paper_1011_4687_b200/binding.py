@@ -32,6 +32,7 @@ EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_hos
                     "qmmm_field_set_layout", "qmmm_field_get_grid_info",
                     "qmmm_field_destroy", "qmmm_field_set_plan", "qmmm_field_get_info",
                     "qmmm_field_set_timing", "qmmm_field_last_timing", "qmmm_field_set_overlap",
+                    "qmmm_field_set_local_lattice",
                     "qmmm_sum_rank_partials", "qmmm_probe_peak", "qmmm_last_error")
 
 
@@ -53,7 +54,7 @@ class qmmm_field_info(ctypes.Structure):
                 ("last_plan", qmmm_plan), ("last_point_blocks", ctypes.c_int32),
                 ("last_launches", ctypes.c_int32), ("sm_count", ctypes.c_int32),
                 ("last_dz_table", ctypes.c_int32), ("device_errors", ctypes.c_int32),
-                ("reserved", ctypes.c_int32), ("last_kernel", ctypes.c_char * 192)]
+                ("last_local_lattice", ctypes.c_int32), ("last_kernel", ctypes.c_char * 192)]
 
 
 class qmmm_grid_info(ctypes.Structure):
@@ -113,6 +114,8 @@ def _load() -> ctypes.CDLL:
     lib.qmmm_field_set_timing.argtypes = [vp, ci]
     lib.qmmm_field_set_overlap.restype = ci
     lib.qmmm_field_set_overlap.argtypes = [vp, ci]
+    lib.qmmm_field_set_local_lattice.restype = ci
+    lib.qmmm_field_set_local_lattice.argtypes = [vp, ci]
     lib.qmmm_field_last_timing.restype = ci
     lib.qmmm_field_last_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_double),
                                            ctypes.POINTER(ctypes.c_double)]
@@ -283,6 +286,11 @@ def qmmm_field_set_overlap(handle: int, enable: bool) -> None:
     """Back-to-back evaluations on one stream may overlap (programmatic dependent launch); see
     include/qmmm_field.h for the precondition on elec_xyz."""
     _check(_lib.qmmm_field_set_overlap(handle, int(bool(enable))))
+
+
+def qmmm_field_set_local_lattice(handle: int, mode: int = -1) -> None:
+    """FP32 grid kernels: coordinate lattice per work unit (-1 automatic, 0 never, 1 always)."""
+    _check(_lib.qmmm_field_set_local_lattice(handle, int(mode)))
 
 
 def qmmm_field_last_timing(handle: int) -> Tuple[float, float]:

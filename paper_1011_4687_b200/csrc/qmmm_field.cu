@@ -220,6 +220,9 @@ struct qmmm_field {
     double *nuclei_u = nullptr;    // [K][4] nuclei in grid units
     int layout = QMMM_LAYOUT_AUTO, last_layout = QMMM_LAYOUT_LIST;
     double bb_lo[3] = {0, 0, 0}, bb_hi[3] = {0, 0, 0};   // bounding box of the cells
+    double q_scale = 1.0;          // power of two applied to the cell charges of the FP32 copies
+    int local_lattice = -1;        // FP32 grid kernel, lattice per gchunk: -1 automatic, 0 off, 1 on
+    int last_local_lattice = 0;
     const char *last_kernel = "";  // mangled name of the kernel the most recent evaluation ran
     // device error word (pinned, device-mapped): set by a kernel whose bounded wait gave up
     int *dev_err_h = nullptr, *dev_err_d = nullptr;
@@ -530,6 +533,31 @@ cudaError_t to_device(const double *src, int64_t n, double **dev, bool *owned) {
 }
 
 
+// Power of two 2^k with 2^k * max|q| in [0.5, 1) (1 when all charges are zero): the scale of the
+// cell charges in the FP32 copies (PairParams::q_unscale).
+cudaError_t charge_scale(const double *dq, int64_t n, double *scale) {
+    *scale = 1.0;
+    if (n <= 0) return cudaSuccess;
+    unsigned long long *dmax = nullptr, hmax = 0;
+    cudaError_t e = cudaMalloc(&dmax, sizeof(hmax));
+    if (e == cudaSuccess) e = cudaMemset(dmax, 0, sizeof(hmax));
+    if (e == cudaSuccess) {
+        absmax_kernel<<<static_cast<unsigned>(std::min<int64_t>(1024, (n + 255) / 256)), 256>>>(dq, n, dmax);
+        e = cudaMemcpy(&hmax, dmax, sizeof(hmax), cudaMemcpyDeviceToHost);
+    }
+    cudaFree(dmax);
+    if (e != cudaSuccess) return e;
+    double m;
+    std::memcpy(&m, &hmax, 8);
+    if (m > 0.0 && std::isfinite(m)) {
+        int ex = 0;
+        std::frexp(m, &ex);                       // m = f * 2^ex, 0.5 <= f < 1
+        ex = std::max(-1000, std::min(1000, ex));
+        *scale = std::ldexp(1.0, -ex);
+    }
+    return cudaSuccess;
+}
+
 // ------------------------------------------------------------------ grid layout (8(f)-1)
 // Packs dense charges [nx][ny][nz] (device) into the FP32 and FP64 gchunk copies and converts
 // the packed nuclei (h->nuclei) to grid units.
@@ -546,9 +574,9 @@ cudaError_t build_grid(qmmm_field *h, const double *ddense, const GridGeom &gg) 
     if (e != cudaSuccess) return e;
     const unsigned nb = static_cast<unsigned>((rows_padded + 63) / 64);
     grid_pack_kernel<float><<<nb, 64>>>(ddense, h->g_rows, gg.n[2], static_cast<int>(h->g_segs),
-                                        rows_padded, h->gcells32);
+                                        rows_padded, h->q_scale, h->gcells32);
     grid_pack_kernel<double><<<nb, 64>>>(ddense, h->g_rows, gg.n[2], static_cast<int>(h->g_segs),
-                                         rows_padded, h->gcells64);
+                                         rows_padded, 1.0, h->gcells64);
     if (h->K > 0) {
         e = cudaMalloc(&h->nuclei_u, h->K * 4 * sizeof(double));
         if (e != cudaSuccess) return e;
@@ -787,6 +815,7 @@ qmmm_status server_start(qmmm_field *h, int prec, bool *usable) {
     prm.inv_lattice = 1.0 / h->lattice;
     prm.nuc = h->nuclei;
     prm.K = f32 ? static_cast<int>(h->K) : 0;
+    prm.q_unscale = f32 ? 1.0 / h->q_scale : 1.0;
     prm.counters = h->counters;
     sp.mail = h->srv_mail_d;
     sp.dev = h->srv_dev;
@@ -979,6 +1008,7 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
         if (e == cudaSuccess) e = to_device(nuc_xyz, 3 * K, &dnxyz, &own[2]);
         if (e == cudaSuccess) e = to_device(nuc_Z, K, &dnz, &own[3]);
         const int T = 256;
+        if (e == cudaSuccess) e = charge_scale(dq, M, &h->q_scale);
         if (e == cudaSuccess && M + K > 0) {
             // FP64 copy: cells then nuclei, one SoA chunk array (the nuclei are ordinary FP64 sources)
             const int64_t Mpad = h->n_chunks64 * CHUNK;
@@ -1026,7 +1056,7 @@ qmmm_status qmmm_field_create(const double *src_xyz, const double *src_q, int64_
                 origins_kernel<<<static_cast<unsigned>((h->n_blocks * 32 + T - 1) / T), T>>>(
                     dxyz, M, h->n_blocks, h->lattice, h->origins);
                 pack_f32_kernel<<<static_cast<unsigned>((h->n_chunks + 63) / 64), 64>>>(
-                    dxyz, dq, M, h->n_chunks, h->origins, h->lattice, h->chunks32);
+                    dxyz, dq, M, h->n_chunks, h->origins, h->lattice, h->q_scale, h->chunks32);
             }
         }
         if (e == cudaSuccess) e = cudaGetLastError();
@@ -1112,6 +1142,7 @@ qmmm_status qmmm_field_create_grid3(const double *origin, const double *spacing,
         grid_count_kernel<<<1024, 256>>>(dq, ntot, dcnt);
         e = cudaMemcpy(&cnt, dcnt, sizeof(cnt), cudaMemcpyDeviceToHost);
     }
+    if (e == cudaSuccess) e = charge_scale(dq, ntot, &h->q_scale);
     if (e == cudaSuccess) e = build_grid(h, dq, gg);
     cudaFree(dcnt);
     if (own[0]) cudaFree(dq);
@@ -1155,11 +1186,12 @@ qmmm_status qmmm_field_share(const qmmm_field *parent, int64_t max_points, qmmm_
     h->n_chunks = parent->n_chunks; h->n_chunks64 = parent->n_chunks64; h->n_blocks = parent->n_blocks;
     h->device = parent->device; h->sm_count = parent->sm_count;
     h->chunks64 = parent->chunks64; h->chunks32 = parent->chunks32; h->origins = parent->origins;
-    h->lattice = parent->lattice; h->nuclei = parent->nuclei;
+    h->lattice = parent->lattice; h->nuclei = parent->nuclei; h->q_scale = parent->q_scale;
     h->has_list = parent->has_list; h->has_grid = parent->has_grid; h->grid = parent->grid;
     h->g_rows = parent->g_rows; h->g_tiles = parent->g_tiles; h->g_segs = parent->g_segs; h->n_g = parent->n_g;
     h->gcells32 = parent->gcells32; h->gcells64 = parent->gcells64; h->nuclei_u = parent->nuclei_u;
     h->layout = parent->layout;
+    h->local_lattice = parent->local_lattice;
     for (int k = 0; k < 3; ++k) { h->bb_lo[k] = parent->bb_lo[k]; h->bb_hi[k] = parent->bb_hi[k]; }
     // its own mutable part: workspace, tickets, mailboxes, move server, staging, plan
     qmmm_status rs = alloc_runtime(h);
@@ -1261,6 +1293,13 @@ qmmm_status qmmm_field_set_timing(qmmm_field *h, int enable) {
     return QMMM_OK;
 }
 
+qmmm_status qmmm_field_set_local_lattice(qmmm_field *h, int mode) {
+    if (!h) return fail(QMMM_ERR_INVALID_ARG, "set_local_lattice: NULL handle");
+    if (mode < -1 || mode > 1) return fail(QMMM_ERR_INVALID_ARG, "set_local_lattice: mode must be -1, 0 or 1");
+    h->local_lattice = mode;
+    return QMMM_OK;
+}
+
 qmmm_status qmmm_field_set_overlap(qmmm_field *h, int enable) {
     if (!h) return fail(QMMM_ERR_INVALID_ARG, "set_overlap: NULL handle");
     h->overlap = enable != 0;
@@ -1292,6 +1331,7 @@ qmmm_status qmmm_field_get_info(const qmmm_field *h, qmmm_field_info *info) {
     info->last_launches = h->last_launches;
     info->sm_count = h->sm_count;
     info->last_dz_table = h->last_dz_table;
+    info->last_local_lattice = h->last_local_lattice;
     info->device_errors = h->dev_err_h ? *reinterpret_cast<volatile int *>(h->dev_err_h) : 0;
     std::strncpy(info->last_kernel, h->last_kernel ? h->last_kernel : "", sizeof(info->last_kernel) - 1);
     return QMMM_OK;
@@ -1369,6 +1409,7 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
         prm.done = h->counters + h->max_points;
         // overlap with the previous evaluation on this stream (not with the timing events in
         // between, and not for the mailbox path, whose host reads V and E behind a flag)
+        prm.q_unscale = f32 ? 1.0 / h->q_scale : 1.0;
         prm.pdl = pdl_attr ? 1 : 0;
         prm.dev_err = h->dev_err_d;
         // Few points, all CTAs of the launch resident together (at most
@@ -1414,6 +1455,11 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
             prm.g_segs = static_cast<int>(h->g_segs);
             prm.g_dzt = use_dzt ? 1 : 0;
             prm.g_light = light ? 1 : 0;
+            // FP32: the whole-grid lattice quantum is 2^-24 of the axis (in nodes); beyond 128 nodes
+            // the field of cells next to a point would lose accuracy (qmmm_grid.cuh, on_lattice)
+            const int nmax = std::max({h->grid.n[0], h->grid.n[1], h->grid.n[2]});
+            prm.g_fine = (f32 && (h->local_lattice == 1 || (h->local_lattice < 0 && nmax > 128))) ? 1 : 0;
+            h->last_local_lattice = prm.g_fine;
         } else {
             prm.chunks = f32 ? reinterpret_cast<const char *>(h->chunks32)
                              : reinterpret_cast<const char *>(h->chunks64);

@@ -39,32 +39,40 @@ struct GridF32Layout {
     static constexpr int NT = 32 * NW;
     static constexpr int STAGE_BYTES = GRID_NODES * sizeof(float);          // 8 KB
     static constexpr int BAR_BYTES = 18 * sizeof(uint64_t);                 // 8 full, 8 empty, flag
-    static constexpr int ELEC_BYTES = NW * EPT * 3 * sizeof(double);
-    static constexpr int SCRATCH_BYTES = NW * 2 * 3 * EPT * sizeof(float);     // lattice a, dd
+    static constexpr int ELEC_BYTES = 2 * NW * EPT * 3 * sizeof(double);    // points in units of hz, and in node units
+    // whole-grid lattice a, dd per CTA point; per-warp lattice a[3][EPT], dd[3][EPT]; per-warp reference node [4]
+    static constexpr int SCRATCH_BYTES = NW * 2 * 3 * EPT * sizeof(float) + NW * 6 * EPT * sizeof(float) +
+                                         NW * 4 * sizeof(int);
     static constexpr int ACC_BYTES = EPT * 4 * NT * sizeof(double);
     __host__ __device__ static constexpr size_t total(int stages) {
         return static_cast<size_t>(stages) * STAGE_BYTES + BAR_BYTES + ELEC_BYTES + SCRATCH_BYTES +
                ACC_BYTES;
     }
-    // dz table (DZT kernels), after everything else: [z nodes padded to whole gchunks + 1][NW][EPT]
+    // dz table (DZT kernels), after everything else: [z nodes padded to whole gchunks + 1][NW][EPT],
+    // then (local lattice) a_z relative to the segment's first node and its residual: 2 x [segs][NW][EPT]
     __host__ __device__ static constexpr size_t dzt_bytes(int segs) {
-        return static_cast<size_t>(segs * 64 + 1) * NW * EPT * sizeof(float);
+        return static_cast<size_t>(segs * 64 + 1 + 2 * segs) * NW * EPT * sizeof(float);
     }
 };
 
-// Coordinate of an evaluation point along one axis (grid units) on a power-of-two lattice
-// fine enough that every difference a - k to a node index k = 0..n-1 is EXACT in FP32: the
-// quantum is 2^-24 of the power of two above the farthest node.  dd = u - a is the residual;
-// it enters once, at the end, as the first-order correction V(a + dd) = V(a) - E(a) . dd
-// (DESIGN.md "FP32 path").  Plain FP32 rounding of the differences would be coherent over a
-// regular grid and bias V.
-__device__ __forceinline__ void on_lattice(double u, int n, float &a, float &dd) {
-    const double far = fmax(fmax(fabs(u), fabs(u - (n - 1))), 1.0);
+// Coordinate of an evaluation point along one axis (node units) on a power-of-two lattice fine
+// enough that every difference a - k to the node indices k = i_lo..i_hi is EXACT in FP32: the
+// quantum is 2^-24 of the power of two above the farthest of those nodes.  a is returned
+// relative to i_lo (a_rel = a - i_lo, itself exact in FP32); dd = u - a is the residual, which
+// enters V as the first-order correction V(a + dd) = V(a) - E(a) . dd.
+// Plain FP32 rounding of the differences would be coherent over a regular grid and bias V.
+//   whole grid (i_lo = 0, i_hi = n - 1): one quantum per axis and point, 2^-24 of the axis;
+//   one gchunk (the 32 rows / 64 z nodes a warp is about to walk): the quantum follows the
+//     distance to THOSE nodes, so next to a point it is 2^-24 of a few dozen nodes however long
+//     the axis is.  E has no first-order correction (it is evaluated at a, relative error about
+//     3 |dd| / distance per term), so long axes with points close to cells need this one.
+__device__ __forceinline__ void on_lattice(double u, int i_lo, int i_hi, float &a_rel, float &dd) {
+    const double far = fmax(fmax(fabs(u - i_lo), fabs(u - i_hi)), 1.0);
     const int ex = ((__double2hiint(far) >> 20) & 0x7ff) - 1022;          // far < 2^ex
     const double lam = __hiloint2double((ex - 24 + 1023) << 20, 0);
     const double inv = __hiloint2double((24 - ex + 1023) << 20, 0);
     const double al = rint(u * inv) * lam;
-    a = static_cast<float>(al);                                // exact: |al| <= 2^24 quanta
+    a_rel = static_cast<float>(al - i_lo);                     // exact: a multiple of lam, at most 2^24 quanta
     dd = static_cast<float>(u - al);
 }
 
@@ -338,9 +346,12 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     uint64_t *empty = full + 8;
     int *flag = reinterpret_cast<int *>(empty + 8);
     ptr += L::BAR_BYTES;
-    double *elec_s = reinterpret_cast<double *>(ptr);          // [WP*EPT][3], grid units
+    double *elec_s = reinterpret_cast<double *>(ptr);          // [WP*EPT][3], units of hz (for the nuclei)
+    double *u_s = elec_s + NW * EPT * 3;                       // [WP*EPT][3], node units of each axis
     ptr += L::ELEC_BYTES;
-    float *lat_s = reinterpret_cast<float *>(ptr);             // a[WP*EPT][3], then dd[WP*EPT][3]
+    float *lat_s = reinterpret_cast<float *>(ptr);             // whole-grid lattice: a[WP*EPT][3], then dd[WP*EPT][3]
+    float *warp_s = lat_s + NW * EPT * 6;                      // per warp: a[3][EPT], dd[3][EPT] of the gchunk at hand
+    int *iref_s = reinterpret_cast<int *>(warp_s + NW * EPT * 6);   // per warp: reference node of a, per axis
     ptr += L::SCRATCH_BYTES;
     double2 *acc = reinterpret_cast<double2 *>(ptr);           // [EPT*2][NT] double2
 
@@ -399,6 +410,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     }
     const int ppb = WP * EPT;
     float *dd_all = lat_s + NW * EPT * 3;
+    const bool fine = prm.g_fine != 0;                          // local lattice per gchunk (uniform)
     for (int i = threadIdx.x; i < ppb * 3; i += NT) {
         int p = blockIdx.x * ppb + i / 3;
         p = p < prm.P ? p : prm.P - 1;                          // clamp: duplicates are not written
@@ -406,18 +418,33 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
         const double u = (point_coord(prm, static_cast<int64_t>(p) * 3 + comp) - prm.g_org[comp]) * prm.g_inv_h[comp];
         const double sc = comp == 0 ? prm.g_sx : (comp == 1 ? prm.g_sy : 1.0);
         elec_s[i] = u * sc;                                     // units of hz (for the nuclei)
+        u_s[i] = u;
         float dd;
-        on_lattice(u, prm.g_n[comp], lat_s[i], dd);             // node index units of this axis
+        on_lattice(u, 0, prm.g_n[comp] - 1, lat_s[i], dd);      // node index units of this axis
         dd_all[i] = dd * static_cast<float>(sc);                // residual in units of hz
     }
     __syncthreads();
     constexpr int TS = DZT ? NW * EP2 : 0;                      // float2 per z node of the table
     float *dzt = reinterpret_cast<float *>(acc + EPT * 2 * NT); // [segs * ZS + 1][NW][EPT]
+    float *azrel_t = dzt + (prm.g_segs * GRID_ZS + 1) * NW * EPT;   // local lattice: [segs][NW][EPT]
+    float *ddz_t = azrel_t + prm.g_segs * NW * EPT;                 //                [segs][NW][EPT]
     if constexpr (DZT) {                                        // a_z - k: exact on the lattice
+        if (fine) {                                             // one lattice per (z segment, point)
+            for (int i = threadIdx.x; i < prm.g_segs * NW * EPT; i += NT) {
+                const int sg = i / (NW * EPT), pp = i - sg * (NW * EPT);
+                on_lattice(u_s[pp * 3 + 2], sg * GRID_ZS, sg * GRID_ZS + GRID_ZS - 1, azrel_t[i], ddz_t[i]);
+            }
+            __syncthreads();
+        }
         const int nent = (prm.g_segs * GRID_ZS + 1) * NW * EPT;
         for (int i = threadIdx.x; i < nent; i += NT) {
             const int kz = i / (NW * EPT), pp = i - kz * (NW * EPT);
-            dzt[i] = lat_s[pp * 3 + 2] - static_cast<float>(kz);
+            if (fine) {
+                const int sg = min(kz / GRID_ZS, prm.g_segs - 1);
+                dzt[i] = azrel_t[sg * (NW * EPT) + pp] - static_cast<float>(kz - sg * GRID_ZS);
+            } else {
+                dzt[i] = lat_s[pp * 3 + 2] - static_cast<float>(kz);
+            }
         }
         __syncthreads();
     }
@@ -429,26 +456,71 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
 #pragma unroll
     for (int i = 0; i < EPT * 2; ++i) my[i * NT] = make_double2(0.0, 0.0);
     const double *pe = elec_s + wp * EPT * 3;
-    // lattice coordinates of this thread's points, packed two points per register pair
-    float2 ax[EP2], ay[EP2], az[EP2];
-#pragma unroll
-    for (int e = 0; e < EP2; ++e) {
-        const float *a0 = lat_s + (wp * EPT + 2 * e) * 3;
-        ax[e] = f2(a0[0], a0[3]);
-        ay[e] = f2(a0[1], a0[4]);
-        az[e] = f2(a0[2], a0[5]);
+    // Lattice coordinates of this warp's points, two points per register pair, relative to the
+    // reference node (irx, iry, irz), and their residuals dd (units of hz) in the warp's scratch.
+    // Whole-grid lattice: reference node 0, filled once.  Local lattice (fine): refilled for
+    // every gchunk by relattice() below.
+    float *a_w = warp_s + warp * 6 * EPT, *dd_w = a_w + 3 * EPT;
+    int *iref_w = iref_s + warp * 4;
+    if (lane < 3 * EPT) {
+        const int comp = lane / EPT, pt = lane - comp * EPT;
+        a_w[lane] = lat_s[(wp * EPT + pt) * 3 + comp];
+        dd_w[lane] = dd_all[(wp * EPT + pt) * 3 + comp];
     }
-    // FP32 accumulators over up to GRID_FLUSH gchunks, then FP64 columns
-    float2 vv[EP2], tt[EP2], ex[EP2], ey[EP2], ez[EP2];
+    if (lane < 3) iref_w[lane] = 0;
+    __syncwarp();
+    float2 ax[EP2], ay[EP2], az[EP2];
+    int irx = 0, iry = 0, irz = 0;
+    auto load_lattice = [&]() {
 #pragma unroll
-    for (int e = 0; e < EP2; ++e) vv[e] = tt[e] = ex[e] = ey[e] = ez[e] = f2(0.0f, 0.0f);
+        for (int e = 0; e < EP2; ++e) {
+            ax[e] = *reinterpret_cast<const float2 *>(a_w + 2 * e);
+            ay[e] = *reinterpret_cast<const float2 *>(a_w + EPT + 2 * e);
+            az[e] = *reinterpret_cast<const float2 *>(a_w + 2 * EPT + 2 * e);
+        }
+        irx = iref_w[0]; iry = iref_w[1]; irz = iref_w[2];
+    };
+    load_lattice();
+    const int n_rows = prm.g_n[0] * prm.g_n[1];
+    // fine: the lattice of the nodes of ONE gchunk -- rows tile_ * 32 .. + 31, z nodes
+    // seg_ * ZS + zlo .. zhi -- computed in FP64 by the first 3 EPT (with a dz table: 2 EPT) lanes
+    auto relattice = [&](int tile_, int seg_, int zlo, int zhi) {
+        __syncwarp();
+        if (lane < (DZT ? 2 : 3) * EPT) {
+            const int comp = lane / EPT, pt = lane - comp * EPT;
+            int i_lo, i_hi;
+            if (comp == 2) {
+                i_lo = seg_ * GRID_ZS + zlo;
+                i_hi = seg_ * GRID_ZS + zhi;
+            } else {
+                const int nyy = prm.g_n[1];
+                const int r0 = tile_ * 32, r1 = min(r0 + 31, n_rows - 1);
+                const int x0 = r0 / nyy, x1 = r1 / nyy;
+                if (comp == 0) { i_lo = x0; i_hi = x1; }
+                else if (x0 == x1) { i_lo = r0 - x0 * nyy; i_hi = r1 - x0 * nyy; }
+                else { i_lo = 0; i_hi = nyy - 1; }
+            }
+            float a, dd;
+            on_lattice(u_s[(wp * EPT + pt) * 3 + comp], i_lo, i_hi, a, dd);
+            a_w[lane] = a;
+            dd_w[lane] = dd * static_cast<float>(comp == 0 ? prm.g_sx : (comp == 1 ? prm.g_sy : 1.0));
+            if (pt == 0) iref_w[comp] = i_lo;
+        }
+        __syncwarp();
+        load_lattice();
+    };
+    // FP32 accumulators over up to GRID_FLUSH gchunks, then FP64 columns.  cc: the first-order
+    // correction for the lattice residual, sum over gchunks of E_gchunk(a) . dd
+    float2 vv[EP2], tt[EP2], ex[EP2], ey[EP2], ez[EP2], cc[EP2];
+#pragma unroll
+    for (int e = 0; e < EP2; ++e) vv[e] = tt[e] = ex[e] = ey[e] = ez[e] = cc[e] = f2(0.0f, 0.0f);
     auto flush = [&]() {
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
             double2 t;
             t = my[(4 * e + 0) * NT];            // V = (3 sum a - sum c r^2) / 2: the Newton step
-            t.x += 1.5 * static_cast<double>(vv[e].x) - 0.5 * static_cast<double>(tt[e].x);
-            t.y += 1.5 * static_cast<double>(vv[e].y) - 0.5 * static_cast<double>(tt[e].y);
+            t.x += 1.5 * static_cast<double>(vv[e].x) - 0.5 * static_cast<double>(tt[e].x) - static_cast<double>(cc[e].x);
+            t.y += 1.5 * static_cast<double>(vv[e].y) - 0.5 * static_cast<double>(tt[e].y) - static_cast<double>(cc[e].y);
             my[(4 * e + 0) * NT] = t;
             t = my[(4 * e + 1) * NT];
             t.x += static_cast<double>(ex[e].x);
@@ -462,7 +534,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
             t.x += static_cast<double>(ez[e].x);
             t.y += static_cast<double>(ez[e].y);
             my[(4 * e + 3) * NT] = t;
-            vv[e] = tt[e] = ex[e] = ey[e] = ez[e] = f2(0.0f, 0.0f);
+            vv[e] = tt[e] = ex[e] = ey[e] = ez[e] = cc[e] = f2(0.0f, 0.0f);
         }
     };
 
@@ -481,12 +553,13 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
             const int sl = 2 * warp + (it & 1);
             const int tl = g / segs, sg = g - tl * segs;
             const int rw = tl * 32 + lane, rx = rw / ny;
-            const float fxs = static_cast<float>(rx), fys = static_cast<float>(rw - rx * ny);
-            const float fzs = static_cast<float>(sg * GRID_ZS);
+            if (fine) relattice(tl, sg, 0, GRID_ZS - 1);
+            const float fxs = static_cast<float>(rx - irx), fys = static_cast<float>(rw - rx * ny - iry);
+            const float fzs = static_cast<float>(sg * GRID_ZS - irz);
             mbar_wait(&full[sl], (it >> 1) & 1);
             const float *data = reinterpret_cast<const float *>(smem + static_cast<size_t>(sl) * STAGE_BYTES);
-            auto one_point = [&](float axs, float ays, float azs, float &vvc, float &ttc, float &exc,
-                                 float &eyc, float &ezc) {
+            auto one_point = [&](float axs, float ays, float azs, int pt, float &vvc, float &ttc, float &exc,
+                                 float &eyc, float &ezc, float &ccc) {
                 const float dxs = (axs - fxs) * static_cast<float>(prm.g_sx);   // exact difference (lattice), then hx/hz
                 const float dys = (ays - fys) * static_cast<float>(prm.g_sy);
                 GridRowF32N row;
@@ -494,14 +567,17 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
                 float v1, t1;
                 row.run(data + 4 * lane, GRID_ZS / 4, v1, t1);
                 const float s1 = row.S.x + row.S.y;
+                const float exg = dxs * s1, eyg = dys * s1, ezg = row.SZ.x + row.SZ.y;
                 vvc += v1;
                 ttc += t1;
-                exc = fmaf(dxs, s1, exc);
-                eyc = fmaf(dys, s1, eyc);
-                ezc += row.SZ.x + row.SZ.y;
+                exc += exg;
+                eyc += eyg;
+                ezc += ezg;
+                if (fine)           // this gchunk was seen from its own lattice point: E_gchunk . dd
+                    ccc = fmaf(exg, dd_w[pt], fmaf(eyg, dd_w[EPT + pt], fmaf(ezg, dd_w[2 * EPT + pt], ccc)));
             };
-            one_point(ax[0].x, ay[0].x, az[0].x, vv[0].x, tt[0].x, ex[0].x, ey[0].x, ez[0].x);
-            if (second) one_point(ax[0].y, ay[0].y, az[0].y, vv[0].y, tt[0].y, ex[0].y, ey[0].y, ez[0].y);
+            one_point(ax[0].x, ay[0].x, az[0].x, 0, vv[0].x, tt[0].x, ex[0].x, ey[0].x, ez[0].x, cc[0].x);
+            if (second) one_point(ax[0].y, ay[0].y, az[0].y, 1, vv[0].y, tt[0].y, ex[0].y, ey[0].y, ez[0].y, cc[0].y);
             __syncwarp();                          // every lane has read the slot
             if (lane == 0 && g + 2 * NW < hi) {    // refill it with the gchunk after next
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -517,8 +593,9 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     uint32_t phase = 0;
     for (int g = lo; g < hi; ++g) {
         if (warp == 0) produce();          // gchunk g + stages - 1 into the slot freed by g - 1
-        const float2 fx = bc(static_cast<float>(ix)), fy = bc(static_cast<float>(iy));
-        const float2 fz = bc(static_cast<float>(seg * GRID_ZS + z0));
+        if (fine) relattice(tile, seg, z0, z0 + ZL - 1);
+        const float2 fx = bc(static_cast<float>(ix - irx)), fy = bc(static_cast<float>(iy - iry));
+        const float2 fz = bc(static_cast<float>(seg * GRID_ZS + z0 - irz));
         float2 dx[EP2], dy[EP2], rxy2[EP2], azb[EP2], v[EP2], tq[EP2];
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
@@ -546,13 +623,31 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[slot]);
         // Ex = dx sum(s), Ey = dy sum(s), Ez = sum(s dz)
+        if (fine) {
+            // this gchunk was seen from its own lattice point a = u - dd: V -= E_gchunk(a) . dd
 #pragma unroll
-        for (int e = 0; e < EP2; ++e) {
-            vv[e] = __fadd2_rn(vv[e], v[e]);
-            tt[e] = __fadd2_rn(tt[e], tq[e]);
-            ex[e] = __ffma2_rn(dx[e], row.S[e], ex[e]);
-            ey[e] = __ffma2_rn(dy[e], row.S[e], ey[e]);
-            ez[e] = __fadd2_rn(ez[e], row.SZ[e]);
+            for (int e = 0; e < EP2; ++e) {
+                const float2 exg = __fmul2_rn(dx[e], row.S[e]), eyg = __fmul2_rn(dy[e], row.S[e]);
+                const float2 ddx = *reinterpret_cast<const float2 *>(dd_w + 2 * e);
+                const float2 ddy = *reinterpret_cast<const float2 *>(dd_w + EPT + 2 * e);
+                const float2 ddz = DZT ? *reinterpret_cast<const float2 *>(ddz_t + seg * (NW * EPT) + wp * EPT + 2 * e)
+                                       : *reinterpret_cast<const float2 *>(dd_w + 2 * EPT + 2 * e);
+                vv[e] = __fadd2_rn(vv[e], v[e]);
+                tt[e] = __fadd2_rn(tt[e], tq[e]);
+                ex[e] = __fadd2_rn(ex[e], exg);
+                ey[e] = __fadd2_rn(ey[e], eyg);
+                ez[e] = __fadd2_rn(ez[e], row.SZ[e]);
+                cc[e] = __ffma2_rn(exg, ddx, __ffma2_rn(eyg, ddy, __ffma2_rn(row.SZ[e], ddz, cc[e])));
+            }
+        } else {
+#pragma unroll
+            for (int e = 0; e < EP2; ++e) {
+                vv[e] = __fadd2_rn(vv[e], v[e]);
+                tt[e] = __fadd2_rn(tt[e], tq[e]);
+                ex[e] = __ffma2_rn(dx[e], row.S[e], ex[e]);
+                ey[e] = __ffma2_rn(dy[e], row.S[e], ey[e]);
+                ez[e] = __fadd2_rn(ez[e], row.SZ[e]);
+            }
         }
         if (++pending == GRID_FLUSH) {
             flush();
@@ -577,8 +672,10 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     }
     if (pending) flush();
     QMMM_MARK(3);
-    // the cells were seen from the lattice point a = u - dd: V(u) = V(a) - E(a) . dd, applied to
-    // this thread's FP64 sums (before the nuclei, which are evaluated at u itself)
+    // whole-grid lattice: the cells were seen from ONE lattice point a = u - dd: V(u) = V(a) - E(a) . dd,
+    // applied to this thread's FP64 sums (before the nuclei, which are evaluated at u itself); the
+    // local lattice has applied its corrections gchunk by gchunk (cc)
+    if (!fine)
 #pragma unroll
     for (int e = 0; e < EP2; ++e) {
         const float *d0 = dd_all + (wp * EPT + 2 * e) * 3;
@@ -598,10 +695,12 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
             double2 t;
-            t = my[(4 * e + 0) * NT]; t.x += nV[2 * e]; t.y += nV[2 * e + 1]; my[(4 * e + 0) * NT] = t;
-            t = my[(4 * e + 1) * NT]; t.x += nEx[2 * e]; t.y += nEx[2 * e + 1]; my[(4 * e + 1) * NT] = t;
-            t = my[(4 * e + 2) * NT]; t.x += nEy[2 * e]; t.y += nEy[2 * e + 1]; my[(4 * e + 2) * NT] = t;
-            t = my[(4 * e + 3) * NT]; t.x += nEz[2 * e]; t.y += nEz[2 * e + 1]; my[(4 * e + 3) * NT] = t;
+            // (the cells' sums carry the power-of-two scale of the FP32 charges: q_unscale)
+            const double qu = prm.q_unscale;
+            t = my[(4 * e + 0) * NT]; t.x = fma(t.x, qu, nV[2 * e]); t.y = fma(t.y, qu, nV[2 * e + 1]); my[(4 * e + 0) * NT] = t;
+            t = my[(4 * e + 1) * NT]; t.x = fma(t.x, qu, nEx[2 * e]); t.y = fma(t.y, qu, nEx[2 * e + 1]); my[(4 * e + 1) * NT] = t;
+            t = my[(4 * e + 2) * NT]; t.x = fma(t.x, qu, nEy[2 * e]); t.y = fma(t.y, qu, nEy[2 * e + 1]); my[(4 * e + 2) * NT] = t;
+            t = my[(4 * e + 3) * NT]; t.x = fma(t.x, qu, nEz[2 * e]); t.y = fma(t.y, qu, nEz[2 * e + 1]); my[(4 * e + 3) * NT] = t;
         }
     }
 
@@ -972,7 +1071,7 @@ __global__ void grid_scatter_kernel(const double *xyz, const double *q, int64_t 
 // residual below one rounding unit).  Cells beyond the grid are 0.
 template <typename REAL>
 __global__ void grid_pack_kernel(const double *dense, int64_t rows, int nz, int segs,
-                                 int64_t rows_padded, REAL *out) {
+                                 int64_t rows_padded, double q_scale, REAL *out) {
     constexpr int PER = sizeof(REAL) == 4 ? 4 : 2;       // nodes per 128-bit load
     const int64_t row = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x;
     if (row >= rows_padded) return;
@@ -983,7 +1082,7 @@ __global__ void grid_pack_kernel(const double *dense, int64_t rows, int nz, int 
         REAL *o = out + (tile * segs + seg) * GRID_NODES;
         for (int k = 0; k < GRID_ZS; ++k) {
             const int iz = seg * GRID_ZS + k;
-            const double qd = (row < rows && iz < nz) ? dense[row * nz + iz] : 0.0;
+            const double qd = (row < rows && iz < nz) ? dense[row * nz + iz] * q_scale : 0.0;   // 2^k: exact
             REAL v;
             if constexpr (sizeof(REAL) == 4) {
                 const double want = qd + carry;

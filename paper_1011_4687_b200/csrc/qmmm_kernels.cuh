@@ -61,6 +61,11 @@ struct PairParams {
     double g_scaleV, g_scaleE;   // 1/hz, 1/hz^2
     int g_n[3], g_segs;      // nodes per axis (row = ix * ny + iy); z segments (gchunks) per row tile
     int g_dzt;               // grid kernels: dz table in shared memory (qmmm_grid.cuh, DZT)
+    int g_fine;              // FP32 grid kernel: coordinate lattice per gchunk instead of per grid (long axes)
+    // FP32 copies (list and grid) store q_j * 2^k with 2^k * max|q| in [0.5, 1): tiny charges keep
+    // their full FP32 precision (no denormals, no flush), and the result does not depend on the
+    // unit of charge.  q_unscale = 2^-k multiplies the cells' FP64 sums before the nuclei are added.
+    double q_unscale;
     int g_light;             // host side only: FP64 grid kernel with 4 consumer warps (overlapped few-point evaluations)
     // push-model collection (overlapped few-point evaluations): tagged 64-byte records instead
     // of partials + fence + ticket; NULL = the ticket path
@@ -178,6 +183,25 @@ __device__ __forceinline__ double rsqrt_mufu_f64(double x) {        // MUFU.RSQ6
 // a regular grid and biases V by ~2e-8 hartree per point.
 __device__ __forceinline__ float lattice_round(double a64, double lattice, double inv_lattice) {
     return static_cast<float>(rint(a64 * inv_lattice) * lattice);
+}
+// The same with a quantum chosen per (point, origin block): the block's sources lie within
+// `radius` of its origin on every axis, so every |a - o| < |a| + radius =: reach < 2^ex, and a
+// lattice of 2^(ex - 24) -- never coarser than the handle's, of which the source offsets are
+// multiples -- still makes d = a - o exact.  For the blocks NEAR a point this is far finer than
+// the handle's quantum (2^-24 of the whole environment's extent), and those are the blocks
+// that matter for the residual dd = (r - c) - a: V is corrected for it to first order
+// (V(a + dd) = V(a) - E(a) . dd) but E itself is evaluated at a, with a relative error of about
+// 3 |dd| / (distance to the cell) per term.  Returns a, sets dd.
+__device__ __forceinline__ float lattice_round_local(double a64, double radius, double lattice,
+                                                     double inv_lattice, float &dd) {
+    const double reach = fabs(a64) + radius;                                  // radius >= 2 lattice > 0
+    const int ex = ((__double2hiint(reach) >> 20) & 0x7ff) - 1022;            // reach < 2^ex
+    double lam = __hiloint2double((ex - 24 + 1023) << 20, 0);
+    double inv = __hiloint2double((24 - ex + 1023) << 20, 0);
+    if (lam > lattice) { lam = lattice; inv = inv_lattice; }
+    const double al = rint(a64 * inv) * lam;
+    dd = static_cast<float>(a64 - al);
+    return static_cast<float>(al);                                            // exact: |al| < 2^24 quanta
 }
 
 // ----------------------------------------------------------------------------- pair math
@@ -567,20 +591,17 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
             // the rounding residual delta is applied as a first-order correction at the flush:
             // V(a_hat + delta) = V(a_hat) - E(a_hat) . delta.
             const double *org = reinterpret_cast<const double *>(st);
-            const double cx = org[0], cy = org[1], cz = org[2];
+            const double cx = org[0], cy = org[1], cz = org[2], rad = org[3];
             float v32[EPT], ex32[EPT], ey32[EPT], ez32[EPT];
-            float ddx[EPT], ddy[EPT], ddz[EPT];   // rounding residuals (|delta| <= ulp/2 of a)
+            float ddx[EPT], ddy[EPT], ddz[EPT];   // lattice residuals (|delta| <= half a local quantum)
 #pragma unroll
             for (int e = 0; e < EPT; ++e) {
                 const double a0 = elec_s[(wp * EPT + e) * 3 + 0] - cx;
                 const double a1 = elec_s[(wp * EPT + e) * 3 + 1] - cy;
                 const double a2 = elec_s[(wp * EPT + e) * 3 + 2] - cz;
-                rx[e] = lattice_round(a0, prm.lattice, prm.inv_lattice);
-                ry[e] = lattice_round(a1, prm.lattice, prm.inv_lattice);
-                rz[e] = lattice_round(a2, prm.lattice, prm.inv_lattice);
-                ddx[e] = static_cast<float>(a0 - static_cast<double>(rx[e]));
-                ddy[e] = static_cast<float>(a1 - static_cast<double>(ry[e]));
-                ddz[e] = static_cast<float>(a2 - static_cast<double>(rz[e]));
+                rx[e] = lattice_round_local(a0, rad, prm.lattice, prm.inv_lattice, ddx[e]);
+                ry[e] = lattice_round_local(a1, rad, prm.lattice, prm.inv_lattice, ddy[e]);
+                rz[e] = lattice_round_local(a2, rad, prm.lattice, prm.inv_lattice, ddz[e]);
                 v32[e] = ex32[e] = ey32[e] = ez32[e] = 0.0f;
             }
             for (int ch = ws; ch < nch; ch += WS) {
@@ -639,7 +660,14 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
 
     QMMM_MARK(3);
     // FP64 path: the nuclei are ordinary sources at the end of the FP64 chunk array
-    if constexpr (F32) nuclei_share<EPT>(prm, elec_s + wp * EPT * 3, ws, WS, lane, V, Ex, Ey, Ez);
+    if constexpr (F32) {
+        // the FP32 copy stores the cell charges times a power of two (PairParams::q_unscale)
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {
+            V[e] *= prm.q_unscale; Ex[e] *= prm.q_unscale; Ey[e] *= prm.q_unscale; Ez[e] *= prm.q_unscale;
+        }
+        nuclei_share<EPT>(prm, elec_s + wp * EPT * 3, ws, WS, lane, V, Ex, Ey, Ez);
+    }
 
     QMMM_MARK(4);
     // ---- in-CTA reduction (paper: shared memory; here shuffle + smem) ----
@@ -871,9 +899,10 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
         if (lane < 3 * EPT) {
             const int comp = lane / EPT, pt = lane % EPT;
             const double a64 = pe[3 * pt + comp] - reinterpret_cast<const double *>(st)[comp];
-            const float a32 = lattice_round(a64, prm.lattice, prm.inv_lattice);
-            a_s[lane] = a32;
-            dd_s[lane] = static_cast<float>(a64 - static_cast<double>(a32));
+            float dd32;
+            a_s[lane] = lattice_round_local(a64, reinterpret_cast<const double *>(st)[3], prm.lattice,
+                                            prm.inv_lattice, dd32);
+            dd_s[lane] = dd32;
         }
         __syncwarp();
         float2 rx[EP2], ry[EP2], rz[EP2], v[EP2], tq[EP2], ex[EP2], ey[EP2], ez[EP2];
@@ -944,10 +973,12 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
             double2 t;
-            t = my[(4 * e + 0) * NT]; t.x += nV[2 * e]; t.y += nV[2 * e + 1]; my[(4 * e + 0) * NT] = t;
-            t = my[(4 * e + 1) * NT]; t.x += nEx[2 * e]; t.y += nEx[2 * e + 1]; my[(4 * e + 1) * NT] = t;
-            t = my[(4 * e + 2) * NT]; t.x += nEy[2 * e]; t.y += nEy[2 * e + 1]; my[(4 * e + 2) * NT] = t;
-            t = my[(4 * e + 3) * NT]; t.x += nEz[2 * e]; t.y += nEz[2 * e + 1]; my[(4 * e + 3) * NT] = t;
+            // (the cells' sums carry the power-of-two scale of the FP32 charges: q_unscale)
+            const double qu = prm.q_unscale;
+            t = my[(4 * e + 0) * NT]; t.x = fma(t.x, qu, nV[2 * e]); t.y = fma(t.y, qu, nV[2 * e + 1]); my[(4 * e + 0) * NT] = t;
+            t = my[(4 * e + 1) * NT]; t.x = fma(t.x, qu, nEx[2 * e]); t.y = fma(t.y, qu, nEx[2 * e + 1]); my[(4 * e + 1) * NT] = t;
+            t = my[(4 * e + 2) * NT]; t.x = fma(t.x, qu, nEy[2 * e]); t.y = fma(t.y, qu, nEy[2 * e + 1]); my[(4 * e + 2) * NT] = t;
+            t = my[(4 * e + 3) * NT]; t.x = fma(t.x, qu, nEz[2 * e]); t.y = fma(t.y, qu, nEz[2 * e + 1]); my[(4 * e + 3) * NT] = t;
         }
     }
 
@@ -1084,6 +1115,18 @@ __global__ void __launch_bounds__(256) bbox_kernel(const double *xyz, int64_t M,
     }
 }
 
+// max |q| over n values (as the bits of the non-negative double: an integer maximum)
+__global__ void __launch_bounds__(256) absmax_kernel(const double *q, int64_t n, unsigned long long *out) {
+    double m = 0.0;
+    for (int64_t j = blockIdx.x * 256ll + threadIdx.x; j < n; j += 256ll * gridDim.x) {
+        const double v = fabs(q[j]);
+        if (v > m && v < 1e300) m = v;
+    }
+    for (int k = 16; k >= 1; k >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, k));
+    if ((threadIdx.x & 31) == 0 && m > 0.0)
+        atomicMax(out, static_cast<unsigned long long>(__double_as_longlong(m)));
+}
+
 // One warp per origin block: centre of the bounding box of the block's real sources.
 __global__ void origins_kernel(const double *xyz, int64_t M, int64_t n_blocks, double lattice,
                                double *origins) {
@@ -1114,7 +1157,11 @@ __global__ void origins_kernel(const double *xyz, int64_t M, int64_t n_blocks, d
             const double u = static_cast<double>(hsh >> 11) * (1.0 / 9007199254740992.0) - 0.5;
             origins[4 * b + k] = 0.5 * (lo[k] + hi[k]) + u * lattice;
         }
-        origins[4 * b + 3] = 0.0;
+        // reach of the block: its sources (after rounding to the lattice) lie within this
+        // distance of the origin on every axis (lattice_round_local)
+        double rad = 0.0;
+        for (int k = 0; k < 3; ++k) rad = fmax(rad, 0.5 * (hi[k] - lo[k]));
+        origins[4 * b + 3] = rad + 2.0 * lattice;
     }
 }
 
@@ -1144,7 +1191,7 @@ __device__ __forceinline__ float round_feedback(double exact, double q, double &
 }
 
 __global__ void pack_f32_kernel(const double *xyz, const double *q, int64_t M, int64_t n_chunks,
-                                const double *origins, double lattice, float *chunks) {
+                                const double *origins, double lattice, double q_scale, float *chunks) {
     const double inv_lattice = 1.0 / lattice;
     const int64_t ch = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x;
     if (ch >= n_chunks) return;
@@ -1154,7 +1201,7 @@ __global__ void pack_f32_kernel(const double *xyz, const double *q, int64_t M, i
     for (int i = 0; i < CHUNK; ++i) {
         const int64_t j = ch * CHUNK + i;
         const int64_t src = j < M ? j : M - 1;           // pads: last real source, charge 0
-        const double qj = j < M ? q[src] : 0.0;
+        const double qj = j < M ? q[src] * q_scale : 0.0;   // power-of-two scale: exact
         c[i] = round_feedback(xyz[3 * src + 0] - o[0], qj, cx, lattice, inv_lattice);
         c[CHUNK + i] = round_feedback(xyz[3 * src + 1] - o[1], qj, cy, lattice, inv_lattice);
         c[2 * CHUNK + i] = round_feedback(xyz[3 * src + 2] - o[2], qj, cz, lattice, inv_lattice);

@@ -281,12 +281,10 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) move_server_kernel(const Serve
             if constexpr (F32) {
                 const double *org = reinterpret_cast<const double *>(st);
                 const double a0 = px - org[0], a1 = py - org[1], a2 = pz - org[2];
-                const float rx = lattice_round(a0, prm.lattice, prm.inv_lattice);
-                const float ry = lattice_round(a1, prm.lattice, prm.inv_lattice);
-                const float rz = lattice_round(a2, prm.lattice, prm.inv_lattice);
-                const float ddx = static_cast<float>(a0 - static_cast<double>(rx));
-                const float ddy = static_cast<float>(a1 - static_cast<double>(ry));
-                const float ddz = static_cast<float>(a2 - static_cast<double>(rz));
+                float ddx, ddy, ddz;
+                const float rx = lattice_round_local(a0, org[3], prm.lattice, prm.inv_lattice, ddx);
+                const float ry = lattice_round_local(a1, org[3], prm.lattice, prm.inv_lattice, ddy);
+                const float rz = lattice_round_local(a2, org[3], prm.lattice, prm.inv_lattice, ddz);
                 float v32 = 0.f, ex32 = 0.f, ey32 = 0.f, ez32 = 0.f;
                 const float *data = reinterpret_cast<const float *>(st + STAGE_HDR);
                 for (int ch = ws; ch < nch; ch += WS) {
@@ -324,7 +322,10 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) move_server_kernel(const Serve
             if (lane == 0) mbar_arrive(&empty[slot]);
             c = ce;
         }
-        if constexpr (F32) nuclei_share<1>(prm, elec_s, ws, WS, lane, V, Ex, Ey, Ez);
+        if constexpr (F32) {
+            V[0] *= prm.q_unscale; Ex[0] *= prm.q_unscale; Ey[0] *= prm.q_unscale; Ez[0] *= prm.q_unscale;
+            nuclei_share<1>(prm, elec_s, ws, WS, lane, V, Ex, Ey, Ez);
+        }
         const double sV = warp_sum(V[0]), sEx = warp_sum(Ex[0]), sEy = warp_sum(Ey[0]), sEz = warp_sum(Ez[0]);
         if (lane == 0) {
             double *r = red + warp * 4;

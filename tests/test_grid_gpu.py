@@ -520,10 +520,6 @@ def test_dz_table_and_stepped_dz_kernels(torch_cuda, B, oracle_mod, nz, P, preci
     rng = np.random.default_rng(1000 + nz + P)
     origin = np.array([-1.0, -0.9, -0.5 * h * (nz - 1)]) + rng.normal(size=3) * 0.1
     centre = origin + 0.5 * h * (np.array(n) - 1)
-    # FP32: the point coordinates live on a lattice of 2^-24 of the axis extent and only V gets
-    # the first-order correction for the residual, so the relative error
-    # of E grows with (nodes along the axis) / (distance to the nearest cell in nodes): keep
-    # the points four cells away from the cells, as the BASELINE configurations do
     dense, pos, q = random_grid(rng, n, h, origin, fill=0.8, hole=(centre, 1.6))
     nuc = centre + np.array([3.0, -2.5, 4.0]) + rng.normal(size=(4, 3))
     Z = np.array([1.0, 6.0, 7.0, 8.0])
@@ -540,6 +536,80 @@ def test_dz_table_and_stepped_dz_kernels(torch_cuda, B, oracle_mod, nz, P, preci
             check(ref, V0, None, tol)
     finally:
         B.qmmm_field_destroy(hnd)
+
+
+@pytest.mark.parametrize("layout", ["grid", "list"])
+@pytest.mark.parametrize("nz", [400, 130])
+def test_fp32_field_next_to_cells_on_a_long_axis(torch_cuda, B, oracle_mod, layout, nz):
+    """FP32 evaluates the field at the point's LATTICE position (only V is corrected for the
+    residual).  With one lattice per grid axis the residual is 2^-25 of the
+    axis length: on a 400-node axis, 1.2 nodes from a charged cell, |E| was off by 1.5e-5 in
+    round 1.  The lattice per work unit (grid kernels; automatic beyond 128 nodes) and per
+    2,048-source block (list kernels) keeps the plain 1e-5: points 1.2 nodes from charged
+    cells, both layouts, no clearance clause."""
+    n, h = (12, 11, nz), 0.25
+    rng = np.random.default_rng(7 + nz)
+    origin = np.array([-1.4, -1.3, -0.5 * h * (nz - 1)]) + rng.normal(size=3) * 0.05
+    centre = origin + 0.5 * h * (np.array(n) - 1)
+    dense, pos, q = random_grid(rng, n, h, origin, fill=0.9, hole=(centre, 1.0))
+    # points 1.2 nodes (0.3 bohr) from charged cells on the rim of the hole, on the inner side
+    d = pos - centre
+    r = np.linalg.norm(d, axis=1)
+    rim = np.argsort(r)[:96]
+    pts = pos[rim] - d[rim] / r[rim, None] * (1.2 * h)
+    pts = np.concatenate([pts, centre + rng.normal(size=(32, 3)) * 0.2])
+    nearest = np.min(np.linalg.norm(pts[:, None, :] - pos[None, rim, :], axis=2), axis=1)
+    assert 1.0 * h <= nearest.min() <= 1.2001 * h
+    nuc = centre + np.array([3.0, -2.5, 4.0]) + rng.normal(size=(4, 3))
+    Z = np.array([1.0, 6.0, 7.0, 8.0])
+    ref = oracle_mod.field(pos, q, nuc, Z, pts, want_abs=True)
+    hnd = B.qmmm_field_create(pos, q, nuc, Z, len(pts))
+    try:
+        assert B.qmmm_field_get_grid_info(hnd)["present"]
+        for plan in (dict(), dict(points_per_thread=8), dict(points_per_thread=2, point_warps=4, slices=9)):
+            V, E = run(torch_cuda, B, hnd, pts, "fp32", layout=layout, plan=plan)
+            if layout == "grid":
+                assert bool(B.qmmm_field_get_info(hnd)["last_local_lattice"]) == (nz > 128)
+            check(ref, V, E, TOL32)
+        for npts in (1, 2):                                         # the node-packed single-point walk
+            V, E = run(torch_cuda, B, hnd, pts[:npts], "fp32", layout=layout)
+            eV, eE = rel_errors(ref, np.concatenate([V, ref.V[npts:]]), np.concatenate([E, ref.E[npts:]]))
+            assert eV.max() <= TOL32 and eE.max() <= TOL32
+        if layout == "grid" and nz <= 128 + 2:
+            # forcing the lattice per work unit on a short axis changes nothing but rounding
+            B.qmmm_field_set_local_lattice(hnd, 1)
+            V1, E1 = run(torch_cuda, B, hnd, pts, "fp32", layout=layout)
+            assert B.qmmm_field_get_info(hnd)["last_local_lattice"] == 1
+            check(ref, V1, E1, TOL32)
+            B.qmmm_field_set_local_lattice(hnd, -1)
+        V64, E64 = run(torch_cuda, B, hnd, pts, "fp64", layout=layout)
+        check(ref, V64, E64, TOL64)
+    finally:
+        B.qmmm_field_destroy(hnd)
+
+
+@pytest.mark.parametrize("layout", ["grid", "list"])
+def test_unit_of_charge_does_not_matter(torch_cuda, B, layout):
+    """Scaling every charge by 2^k scales V and E by 2^k BITWISE (the oracle has the same pin):
+    FP64 trivially; FP32 because its copies store the cell charges relative to a power of two
+    near the largest one, so tiny charges (below FP32's normal range, 1.2e-38) keep their
+    precision instead of being flushed."""
+    w = make_workload(1, n_points=(1, 24))
+    pts = w.elec_xyz.reshape(-1, 3)
+    out = {}
+    for k in (0, -100, -140, 60):
+        f = 2.0 ** k
+        hnd = B.qmmm_field_create(w.src_xyz, w.src_q * f, w.nuc_xyz, w.nuc_Z * f, len(pts))
+        try:
+            for prec in ("fp64", "fp32"):
+                out[(k, prec)] = run(torch_cuda, B, hnd, pts, prec, layout=layout)
+        finally:
+            B.qmmm_field_destroy(hnd)
+    for prec in ("fp64", "fp32"):
+        V0, E0 = out[(0, prec)]
+        for k in (-100, -140, 60):
+            V, E = out[(k, prec)]
+            assert np.array_equal(V, V0 * 2.0 ** k) and np.array_equal(E, E0 * 2.0 ** k), (prec, k)
 
 
 # ----------------------------------------------- overlapped back-to-back evaluations (PDL)
