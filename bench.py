@@ -138,8 +138,9 @@ class ClockSampler(threading.Thread):
 
 
 # ------------------------------------------------------------------------ oracle timing
-def oracle_sample_rate(w, sample_pairs: float, seed: int = 99):
-    """Times the CPU oracle (as it stands) on a seeded subsample of the evaluation points."""
+def oracle_sample_rate(w, sample_pairs: float, seed: int = 99, nthreads: int = 0):
+    """Times the CPU oracle (as it stands) on a seeded subsample of the evaluation points
+    (nthreads = 0: all host cores this process may use)."""
     import oracle
     oracle.build()
     pts = w.elec_xyz.reshape(-1, 3)
@@ -151,7 +152,7 @@ def oracle_sample_rate(w, sample_pairs: float, seed: int = 99):
     t0 = time.perf_counter()
     # all host cores this process may use (torchrun sets OMP_NUM_THREADS=1 by default)
     res = oracle.field(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, sub,
-                       nthreads=len(os.sched_getaffinity(0)))
+                       nthreads=nthreads or len(os.sched_getaffinity(0)))
     dt = time.perf_counter() - t0
     pairs = n * per_point
     return dict(pairs=pairs, seconds=dt, rate=pairs / dt, threads=res.threads, n_points=n,
@@ -212,6 +213,23 @@ def probe_peaks(B):
     return {"ffma_lane_ops_per_s": ffma, "dfma_lane_ops_per_s": dfma, "mufu_lane_ops_per_s": mufu}
 
 
+def probe_memory_and_launch(B):
+    """SURVEY.md 8(d) "Timing protocol": empty-kernel launch + sync latency and the read
+    bandwidth over a 33 MB (L2-resident) and a 537 MB (HBM) buffer, same process."""
+    launch_s, _ = B.qmmm_probe_peak(3)
+    l2, _ = B.qmmm_probe_peak(4)
+    hbm, _ = B.qmmm_probe_peak(5)
+    out = {"empty_launch_plus_sync_us": launch_s * 1e6, "l2_read_GBps_33MB": l2 / 1e9,
+           "hbm_read_GBps_537MB": hbm / 1e9}
+    mp = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(mp):
+        try:
+            out["measured_peaks_hbm_GBps"] = json.load(open(mp))["hbm_gbs"]
+        except Exception:
+            pass
+    return out
+
+
 def time_steps(torch, B, h, batches, W, N, prec, steps, warmup, flush, stream, want_E=True):
     """Per-step CUDA events on the launch stream; returns (step_ms list, pair_ms list)."""
     P = W * N
@@ -234,7 +252,7 @@ def time_steps(torch, B, h, batches, W, N, prec, steps, warmup, flush, stream, w
     return [a.elapsed_time(b) for a, b in evs], pair_ms, (V, E)
 
 
-def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
+def sweep_all_configs(torch, B, peaks, main_cfg, main_result, mem=None):
     """Per-config table (N=1): ms per evaluation, Gpair/s and FMA-pipe fraction for every
     BASELINE.json configuration and precision; config 2 also as the QMC host loop."""
     out = []
@@ -350,6 +368,14 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result):
                     row["source_GBps_back_to_back"] = bytes_eval / (row["us_per_eval_1000_back_to_back"] * 1e-6) / 1e9
                     row["source_GBps_cuda_graph"] = bytes_eval / (row["us_per_eval_1000_cuda_graph"] * 1e-6) / 1e9
                     row["source_GBps_cuda_graph_overlap"] = bytes_eval / (row["us_per_eval_1000_cuda_graph_overlap"] * 1e-6) / 1e9
+                    if mem:
+                        # the single-electron path is bound by source bandwidth and latency, not by
+                        # the FMA pipe: its rates against the measured read bandwidths
+                        for k in ("back_to_back", "cuda_graph", "cuda_graph_overlap"):
+                            row[f"frac_of_l2_read_bw_{k}"] = row[f"source_GBps_{k}"] / mem["l2_read_GBps_33MB"]
+                            row[f"frac_of_hbm_read_bw_{k}"] = row[f"source_GBps_{k}"] / mem["hbm_read_GBps_537MB"]
+                        row["source_bytes_fit_l2"] = bool(bytes_eval < 100e6)
+                        row["empty_launch_plus_sync_us"] = mem["empty_launch_plus_sync_us"]
                 if not w.sequential and idx <= 1:
                     # launch-free figure for the small configurations (an evaluation is of the
                     # size of one kernel launch): 200 evaluations captured once in a CUDA graph
@@ -528,7 +554,8 @@ def run_ours(args):
             "gpu_launches": info["last_launches"] * args.steps,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
                          "frac": achieved / peak_tf, "traffic": traffic,
-                         "kernel": KERNEL[(layout, prec)], "kernel_ms": pair_s * 1e3,
+                         "kernel": KERNEL[(layout, prec)], "kernel_symbol": info.get("last_kernel", ""),
+                         "kernel_ms": pair_s * 1e3,
                          "slots_per_pair": slots, "dz_table": bool(info.get("last_dz_table")),
                          # the same launch against SURVEY.md 8(d)'s fixed per-pair figure (17 FP32 /
                          # 18 FP64 slots: list of positions, per-pair refinement); above 1 when the
@@ -544,18 +571,52 @@ def run_ours(args):
                          "mufu_lane_ops_per_s": peaks1["mufu_lane_ops_per_s"],
                          "probe_before": peaks0, "probe_after": peaks1},
         }
+        if traffic is not None:
+            line["roofline"]["traffic_source"] = ("ncu --set full capture summarised in profiles/ "
+                                                  "(pair_kernel_traffic.csv); looked up, not measured in this run")
         if world == 1:
             cb = oracle_sample_rate(w, args.cpu_sample_pairs)
             line["cpu_baseline"] = {
                 "value": cb["rate"] / 1e9, "unit": UNIT, "cores": cb["threads"], "kind": "oracle",
                 "sample": f"{cb['n_points']} of {cb['n_total']} evaluation points x all "
                           f"{w.M}+{w.K} sources ({cb['pairs']:.3g} pairs, {cb['seconds']:.1f} s)"}
-            line["paper_context"] = "GTX 275 vs one i7-920 core: 23.6x (SP), 11.0x (DP), whole run (PAPER.md:13)"
+            # the same oracle on ONE core (SURVEY.md 8(d) "CPU baseline" (b)): 1 % of the points, the
+            # rate scales linearly in the points; the paper's speed-ups are quoted per one core
+            c1 = oracle_sample_rate(w, 0.01 * P * (w.M + w.K), seed=98, nthreads=1)
+            line["cpu_baseline_one_core"] = {
+                "value": c1["rate"] / 1e9, "unit": UNIT, "cores": c1["threads"], "kind": "oracle",
+                "sample": f"{c1['n_points']} of {c1['n_total']} evaluation points (1 %) x all {w.M}+{w.K} "
+                          f"sources ({c1['pairs']:.3g} pairs, {c1['seconds']:.1f} s); rate is per pair, "
+                          f"so it carries over to the full batch"}
+            line["paper_context"] = {
+                "paper_gpu_vs_one_cpu_core": {"sp": 23.6, "dp": 11.0,
+                                              "what": "GTX 275 vs one Core i7 920 core, whole QMC run incl. upload "
+                                                      "(PAPER.md:13, :165); another machine and a whole program: context only"},
+                "this_run_gpu_vs_one_cpu_core": {"precision": prec, "ratio": value / (c1["rate"] / 1e9),
+                                                 "what": "this kernel path (device-resident) vs the FP64 oracle on one "
+                                                         "host core of this box"}}
+            mem = probe_memory_and_launch(B)
+            line["probes"] = mem
             if not args.no_sweep:
                 B.qmmm_field_destroy(h)
                 h = None
                 del batches
-                line["configs"] = sweep_all_configs(torch, B, peaks1, args.config, line)
+                line["configs"] = sweep_all_configs(torch, B, peaks1, args.config, line, mem)
+                # configs[4] in FP64 is the roofline case of the FP64 kernels: its
+                # own block, from the sweep's row (same process, same DFMA probe)
+                for r in line["configs"]:
+                    if r["config"] == 4 and r["precision"] == "fp64" and r["layout_choice"] == "auto":
+                        ach = r["pairs_per_eval"] * r["slots_per_pair"] * 2 / (r["pair_kernel_ms_median"] * 1e-3) / 1e12
+                        pk = 2 * peaks1["dfma_lane_ops_per_s"] / 1e12
+                        line["roofline_fp64"] = {
+                            "workload": WORKLOAD_NAME[4], "bound": "alu", "achieved": ach, "peak": pk,
+                            "unit": "TFLOP/s", "frac": ach / pk, "kernel": KERNEL[(r["layout"], "fp64")],
+                            "kernel_ms": r["pair_kernel_ms_median"], "slots_per_pair": r["slots_per_pair"],
+                            "dz_table": r["dz_table"], "gpairs_per_s": r["gpairs_per_s"],
+                            "frac_at_survey_slots": r["pairs_per_eval"] * 18 / (r["pair_kernel_ms_median"] * 1e-3)
+                                                    / peaks1["dfma_lane_ops_per_s"],
+                            "traffic": None,
+                            "peak_source": "measured DFMA lane rate, same process (qmmm_probe_peak)"}
         print(json.dumps(line), flush=True)
     if h is not None:
         B.qmmm_field_destroy(h)
