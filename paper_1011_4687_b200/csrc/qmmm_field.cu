@@ -418,16 +418,19 @@ cudaError_t launch_pair_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
     return cudaErrorInvalidValue;
 }
 
-template <int EP2, int NW, bool NODEPACK = false, bool FULL = false, bool DZT = false>
+template <int EP2, int NW, bool NODEPACK = false, bool FULL = false, bool DZT = false, int FINE = -1>
 cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
     if constexpr (!NODEPACK && !FULL) {            // every warp its own point group: no z split
         if constexpr (EP2 == 2 && (NW == GRID_NW_EPT4 || NW == GRID_NW_EPT4_LIGHT)) {
             if (prm.point_warps == NW && prm.g_dzt)
-                return launch_grid_f32<EP2, NW, false, true, true>(prm, grid, smem, st);
+                return prm.g_fine ? launch_grid_f32<EP2, NW, false, true, true, 1>(prm, grid, smem, st)
+                                  : launch_grid_f32<EP2, NW, false, true, true, 0>(prm, grid, smem, st);
         }
-        if (prm.point_warps == NW) return launch_grid_f32<EP2, NW, false, true>(prm, grid, smem, st);
+        if (prm.point_warps == NW)
+            return prm.g_fine ? launch_grid_f32<EP2, NW, false, true, false, 1>(prm, grid, smem, st)
+                              : launch_grid_f32<EP2, NW, false, true, false, 0>(prm, grid, smem, st);
     }
-    auto kern = grid_kernel_f32x2<EP2, NW, NODEPACK, FULL, DZT>;
+    auto kern = grid_kernel_f32x2<EP2, NW, NODEPACK, FULL, DZT, FINE>;
     static SmemConfig configured;
     static const char *const name = kernel_name(reinterpret_cast<const void *>(kern));
     g_launched = name;

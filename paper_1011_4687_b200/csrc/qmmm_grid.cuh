@@ -327,8 +327,11 @@ constexpr int GRID_FLUSH = QMMM_GRID_FLUSH;                       // gchunks per
 // slower and is not used there).
 // DZT (FULL only): dz from a per-CTA table in shared memory (GridRowF32<EP2, TS>), chosen by
 // the launcher when the table fits beside two CTAs per SM.
-template <int EP2, int NW, bool NODEPACK = false, bool FULL = false, bool DZT = false>
+// FINE: coordinate lattice per gchunk (on_lattice) -- 1 on, 0 off (the batched FULL kernels are
+// compiled both ways: the switch costs registers in their loop), -1 decided by prm.g_fine.
+template <int EP2, int NW, bool NODEPACK = false, bool FULL = false, bool DZT = false, int FINE = -1>
 __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 16 / NW : 1) grid_kernel_f32x2(const PairParams prm) {
+    static_assert(FINE == -1 || FULL, "the compile-time switch is for the batched FULL kernels");
     static_assert(!DZT || (FULL && !NODEPACK), "dz table: every warp walks whole gchunks of its own points");
     static_assert(!NODEPACK || EP2 == 1, "node packing walks single points");
     static_assert(!(NODEPACK && FULL), "FULL is a mode of the point-packed walk");
@@ -410,7 +413,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     }
     const int ppb = WP * EPT;
     float *dd_all = lat_s + NW * EPT * 3;
-    const bool fine = prm.g_fine != 0;                          // local lattice per gchunk (uniform)
+    const bool fine = FINE >= 0 ? FINE == 1 : prm.g_fine != 0;  // local lattice per gchunk (uniform)
     for (int i = threadIdx.x; i < ppb * 3; i += NT) {
         int p = blockIdx.x * ppb + i / 3;
         p = p < prm.P ? p : prm.P - 1;                          // clamp: duplicates are not written
