@@ -47,6 +47,7 @@ UNIT = "Gpair/s"
 # stepping it: one operation less, 8 (FP32) / 12 (FP64).
 SLOTS = {("list", "fp32"): 14, ("list", "fp64"): 18, ("grid", "fp32"): 9, ("grid", "fp64"): 13}
 SLOTS_V_ONLY = {"list": 13, "grid": 8}     # FP64 potential only (E = NULL)
+SLOTS_V_ONLY_F32_GRID = 6                  # FP32 potential only, batched grid kernel: r^2, a, V0, y0^2, c, T
 
 
 def slots_for(layout, prec, info, v_only=False):
@@ -421,6 +422,23 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result, mem=None):
                     row["fma_pipe_frac_cuda_graph_overlap"] = pairs * slots_o / (us * 1e-6) / peak
                     del gr
                 out.append(row)
+                if prec == "fp32" and not w.sequential and idx == 3 and layout == "grid":
+                    # FP32 potential only (E = NULL): the paper's own computation, Eq. 4; the batched
+                    # grid kernel needs 6 FMA-pipe operations + 1 MUFU per pair: the XU pipe bounds it
+                    B.qmmm_field_set_timing(h, True)
+                    step_ms, pair_ms, _ = time_steps(torch, B, h, batches, W, N, prec, reps, 3, flush,
+                                                     stream, want_E=False)
+                    info = B.qmmm_field_get_info(h)
+                    out.append({"config": idx, "name": w.name, "precision": "fp32 potential-only",
+                                "layout": layout, "layout_choice": "auto" if which == "auto" else "forced",
+                                "points": P, "M": w.M, "K": w.K, "pairs_per_eval": pairs,
+                                "ms_per_eval_median": float(np.median(step_ms)),
+                                "pair_kernel_ms_median": float(np.median(pair_ms)),
+                                "gpairs_per_s": pairs / np.median(step_ms) / 1e6,
+                                "slots_per_pair": SLOTS_V_ONLY_F32_GRID,
+                                "fma_pipe_frac": pairs * SLOTS_V_ONLY_F32_GRID / (np.median(step_ms) * 1e-3) / peak,
+                                "xu_pipe_frac": pairs / (np.median(step_ms) * 1e-3) / peaks["mufu_lane_ops_per_s"],
+                                "kernel_symbol": info.get("last_kernel", ""), "plan": info["last_plan"]})
                 if prec == "fp64" and not w.sequential and idx in (1, 4):
                     # potential only (E = NULL): the paper's own computation, Eq. 4; 13 (list) or
                     # 8 (grid) DP slots

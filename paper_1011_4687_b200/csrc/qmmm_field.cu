@@ -418,9 +418,15 @@ cudaError_t launch_pair_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
     return cudaErrorInvalidValue;
 }
 
-template <int EP2, int NW, bool NODEPACK = false, bool FULL = false, bool DZT = false, int FINE = -1>
+template <int EP2, int NW, bool NODEPACK = false, bool FULL = false, bool DZT = false, int FINE = -1,
+          bool VONLY = false>
 cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
     if constexpr (!NODEPACK && !FULL) {            // every warp its own point group: no z split
+        if constexpr (EP2 == 2 && NW == GRID_NW_EPT4) {
+            // E = NULL: the potential alone (Eq. 4), 6 instead of 8 operations per pair
+            if (prm.point_warps == NW && prm.g_dzt && !prm.E)
+                return launch_grid_f32<EP2, NW, false, true, true, 0, true>(prm, grid, smem, st);
+        }
         if constexpr (EP2 == 2 && (NW == GRID_NW_EPT4 || NW == GRID_NW_EPT4_LIGHT)) {
             if (prm.point_warps == NW && prm.g_dzt)
                 return prm.g_fine ? launch_grid_f32<EP2, NW, false, true, true, 1>(prm, grid, smem, st)
@@ -430,7 +436,7 @@ cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaS
             return prm.g_fine ? launch_grid_f32<EP2, NW, false, true, false, 1>(prm, grid, smem, st)
                               : launch_grid_f32<EP2, NW, false, true, false, 0>(prm, grid, smem, st);
     }
-    auto kern = grid_kernel_f32x2<EP2, NW, NODEPACK, FULL, DZT, FINE>;
+    auto kern = grid_kernel_f32x2<EP2, NW, NODEPACK, FULL, DZT, FINE, VONLY>;
     static SmemConfig configured;
     static const char *const name = kernel_name(reinterpret_cast<const void *>(kern));
     g_launched = name;

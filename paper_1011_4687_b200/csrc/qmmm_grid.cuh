@@ -98,8 +98,15 @@ __device__ __forceinline__ void on_lattice(double u, int i_lo, int i_hi, float &
 // the CTA tabulates it once in shared memory ([z node][warp][EPT] floats, TS = float2 per z
 // node) and a node's dz is ONE broadcast 128-bit load for both point pairs instead of a packed
 // add per pair: 8 FMA-pipe lane operations per pair instead of 9.
-template <int EP2, int TS = 0>
+//
+// VONLY (potential only, Eq. 4 proper; needs the table): the table holds z2 = (u_z - k)^2, formed
+// in FP64 from the point's true coordinate and rounded once, rxy2 is formed in FP64 per (point,
+// row) and rounded once, and r^2 = rxy2 + z2 is ONE add.  No lattice and no residual: nothing
+// needs the field to be corrected with.  Per pair: r^2, a, V0 += a, y0^2, c, T += c r^2 = 6
+// FMA-pipe lane operations + 1 MUFU.RSQ -- the XU pipe (16 per SM and clock) is the limit.
+template <int EP2, int TS = 0, bool VONLY = false>
 struct GridRowF32 {
+    static_assert(!VONLY || TS > 0, "the potential-only walk is table-driven");
     float2 dzA[EP2], r2A[EP2], y0A[EP2], dzB[EP2], r2B[EP2], y0B[EP2];
     float2 rxy2[EP2], S[EP2], SZ[EP2];
     const float2 *tp;                  // TS > 0: table entry of the node held in the current set
@@ -122,7 +129,7 @@ struct GridRowF32 {
         for (int e = 0; e < EP2; ++e) {
             rxy2[e] = rxy2_[e];
             S[e] = SZ[e] = f2(0.0f, 0.0f);
-            r2A[e] = __ffma2_rn(dzA[e], dzA[e], rxy2[e]);
+            r2A[e] = VONLY ? __fadd2_rn(dzA[e], rxy2[e]) : __ffma2_rn(dzA[e], dzA[e], rxy2[e]);
         }
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
@@ -151,7 +158,7 @@ struct GridRowF32 {
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
             if constexpr (TS == 0) dzn[e] = __fadd2_rn(dzc[e], bc(-1.0f));
-            r2n[e] = __ffma2_rn(dzn[e], dzn[e], rxy2[e]);
+            r2n[e] = VONLY ? __fadd2_rn(dzn[e], rxy2[e]) : __ffma2_rn(dzn[e], dzn[e], rxy2[e]);
         }
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
@@ -170,8 +177,10 @@ struct GridRowF32 {
             Vc[e] = first ? a : __fadd2_rn(Vc[e], a);
             const float2 c = __fmul2_rn(a, __fmul2_rn(y0[e], y0[e]));
             Tc[e] = first ? __fmul2_rn(c, r2[e]) : __ffma2_rn(c, r2[e], Tc[e]);
-            S[e] = __fadd2_rn(S[e], c);
-            SZ[e] = __ffma2_rn(c, dz[e], SZ[e]);
+            if constexpr (!VONLY) {
+                S[e] = __fadd2_rn(S[e], c);
+                SZ[e] = __ffma2_rn(c, dz[e], SZ[e]);
+            }
         }
     }
     // 4 nodes (one 128-bit load of charges); their V0 and T sums go to Vc, Tc
@@ -329,9 +338,12 @@ constexpr int GRID_FLUSH = QMMM_GRID_FLUSH;                       // gchunks per
 // the launcher when the table fits beside two CTAs per SM.
 // FINE: coordinate lattice per gchunk (on_lattice) -- 1 on, 0 off (the batched FULL kernels are
 // compiled both ways: the switch costs registers in their loop), -1 decided by prm.g_fine.
-template <int EP2, int NW, bool NODEPACK = false, bool FULL = false, bool DZT = false, int FINE = -1>
+// VONLY (E = NULL; FULL + DZT only): the potential alone, no lattice (GridRowF32<.., VONLY>).
+template <int EP2, int NW, bool NODEPACK = false, bool FULL = false, bool DZT = false, int FINE = -1,
+          bool VONLY = false>
 __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 16 / NW : 1) grid_kernel_f32x2(const PairParams prm) {
     static_assert(FINE == -1 || FULL, "the compile-time switch is for the batched FULL kernels");
+    static_assert(!VONLY || (FULL && DZT && FINE == 0), "potential only: batched table-driven walk, no lattice");
     static_assert(!DZT || (FULL && !NODEPACK), "dz table: every warp walks whole gchunks of its own points");
     static_assert(!NODEPACK || EP2 == 1, "node packing walks single points");
     static_assert(!(NODEPACK && FULL), "FULL is a mode of the point-packed walk");
@@ -442,7 +454,10 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
         const int nent = (prm.g_segs * GRID_ZS + 1) * NW * EPT;
         for (int i = threadIdx.x; i < nent; i += NT) {
             const int kz = i / (NW * EPT), pp = i - kz * (NW * EPT);
-            if (fine) {
+            if constexpr (VONLY) {                              // z2 = (u_z - k)^2, rounded once
+                const double dzt64 = u_s[pp * 3 + 2] - static_cast<double>(kz);
+                dzt[i] = static_cast<float>(dzt64 * dzt64);
+            } else if (fine) {
                 const int sg = min(kz / GRID_ZS, prm.g_segs - 1);
                 dzt[i] = azrel_t[sg * (NW * EPT) + pp] - static_cast<float>(kz - sg * GRID_ZS);
             } else {
@@ -596,6 +611,32 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     uint32_t phase = 0;
     for (int g = lo; g < hi; ++g) {
         if (warp == 0) produce();          // gchunk g + stages - 1 into the slot freed by g - 1
+        if constexpr (VONLY) {
+            // rxy2 = dx^2 + dy^2 of the lane's row from the points' true coordinates, in FP64,
+            // rounded once (pe: units of hz; node (ix, iy) sits at (ix sx, iy sy))
+            const double rowx = static_cast<double>(ix) * prm.g_sx, rowy = static_cast<double>(iy) * prm.g_sy;
+            float2 rxy2[EP2], v[EP2], tq[EP2];
+#pragma unroll
+            for (int e = 0; e < EP2; ++e) {
+                const double dx0 = pe[6 * e + 0] - rowx, dy0 = pe[6 * e + 1] - rowy;
+                const double dx1 = pe[6 * e + 3] - rowx, dy1 = pe[6 * e + 4] - rowy;
+                rxy2[e] = f2(static_cast<float>(fma(dy0, dy0, fma(dx0, dx0, 1e-30))),
+                             static_cast<float>(fma(dy1, dy1, fma(dx1, dx1, 1e-30))));
+                v[e] = tq[e] = f2(0.0f, 0.0f);
+            }
+            GridRowF32<EP2, TS, true> row;
+            row.start(reinterpret_cast<const float2 *>(dzt) + (seg * GRID_ZS) * TS + wp * EP2, rxy2);
+            mbar_wait(&full[slot], phase);
+            row.run(reinterpret_cast<const float *>(smem + static_cast<size_t>(slot) * STAGE_BYTES) + 4 * lane,
+                    GRID_ZS / 4, v, tq);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[slot]);
+#pragma unroll
+            for (int e = 0; e < EP2; ++e) {
+                vv[e] = __fadd2_rn(vv[e], v[e]);
+                tt[e] = __fadd2_rn(tt[e], tq[e]);
+            }
+        } else {
         if (fine) relattice(tile, seg, z0, z0 + ZL - 1);
         const float2 fx = bc(static_cast<float>(ix - irx)), fy = bc(static_cast<float>(iy - iry));
         const float2 fz = bc(static_cast<float>(seg * GRID_ZS + z0 - irz));
@@ -652,6 +693,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
                 ez[e] = __fadd2_rn(ez[e], row.SZ[e]);
             }
         }
+        }
         if (++pending == GRID_FLUSH) {
             flush();
             pending = 0;
@@ -678,7 +720,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     // whole-grid lattice: the cells were seen from ONE lattice point a = u - dd: V(u) = V(a) - E(a) . dd,
     // applied to this thread's FP64 sums (before the nuclei, which are evaluated at u itself); the
     // local lattice has applied its corrections gchunk by gchunk (cc)
-    if (!fine)
+    if (!fine && !VONLY)
 #pragma unroll
     for (int e = 0; e < EP2; ++e) {
         const float *d0 = dd_all + (wp * EPT + 2 * e) * 3;

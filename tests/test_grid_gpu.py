@@ -295,12 +295,23 @@ def test_config3_grid_fp32_full_energy(torch_cuda, B, oracle_mod, full_oracle):
         V, E = run(torch_cuda, B, h, pts, "fp32")
         assert B.qmmm_field_get_grid_info(h)["last_layout"] == "grid"
         Vl, El = run(torch_cuda, B, h, pts, "fp32", layout="list")
+        # E = NULL: the potential-only kernel (Eq. 4 proper; no lattice, 6 operations per pair)
+        Vp, _ = run(torch_cuda, B, h, pts, "fp32", want_E=False, layout="auto")
+        assert "ELb1EEEv" in B.qmmm_field_get_info(h)["last_kernel"]      # <2, 8, false, true, true, 0, true>
+        U = torch_cuda.zeros(w.W, dtype=torch_cuda.float64, device="cuda")
+        B.qmmm_field_eval_energy(h, torch_cuda.from_numpy(pts).cuda(), w.W, w.N, U, "fp32")
+        torch_cuda.cuda.synchronize()
+        U = U.cpu().numpy()
     finally:
         B.qmmm_field_destroy(h)
     full = full_oracle(3)                         # every point, V and E
     check(full, V, E, TOL32)
     check(full, Vl, El, TOL32)
-    for name, v in (("grid", V), ("list", Vl)):
+    check(full, Vp, None, TOL32)
+    dU = np.abs(U + full.V.reshape(w.W, w.N).sum(1))
+    print(f"config3 fp32 eval_energy: per-walker max |dU| = {dU.max():.3e} hartree")
+    assert dU.max() <= E_TOL
+    for name, v in (("grid", V), ("list", Vl), ("grid potential-only", Vp)):
         per_walker = np.abs(v.reshape(w.W, w.N).sum(1) - full.V.reshape(w.W, w.N).sum(1))
         batch = abs(v.sum() - full.V.sum())
         d = v - full.V
