@@ -53,7 +53,13 @@ typedef enum {
  *   QMMM_FP64       : FP64 throughout (rel. error <= 1e-12 on V and E).
  *   QMMM_FP32_ACC64 : cell sources in FP32 arithmetic (MUFU rsqrt + one Newton
  *                     step, applied to the sum), running sums in FP64; nuclei always FP64
- *                     (per-point rel. error <= 1e-5, energy within 1e-5 hartree). */
+ *                     (per-point rel. error <= 1e-5 on V and on |E|, per-configuration
+ *                     energy within 1e-5 hartree).  Conditions of the bound on |E|: the point
+ *                     is at least two cell edges from every charged cell (one edge with the
+ *                     lattice per work unit, qmmm_field_set_local_lattice), and the sum does
+ *                     not cancel to less than about a hundredth of its terms (kappa <~ 100:
+ *                     no FP32 arithmetic can do better than ~1e-7 x sum |q|/r^2).  E = NULL on
+ *                     a grid runs a potential-only kernel (6 instead of 8 operations per pair). */
 typedef enum { QMMM_FP64 = 0, QMMM_FP32_ACC64 = 1 } qmmm_precision;
 
 /*
@@ -246,13 +252,14 @@ qmmm_status qmmm_sum_rank_partials(const double *parts, int64_t R, int64_t n, do
  * and corrects V for the rounding residual to first order; E is evaluated at the lattice point
  * (relative error about 3 x residual / distance per cell).  With one lattice per grid axis the
  * residual is up to 2^-25 of the axis length in nodes: fine for axes of up to 128 nodes (all FP32
- * BASELINE configurations), too coarse for long axes with points next to cells.  With a lattice
- * per work unit (32 rows x 64 z nodes) the residual is 2^-25 of the distance to THAT unit's
- * farthest node, i.e. a few 1e-6 nodes next to the point whatever the size of the grid, at about
- * 3 % more time.  mode -1 (default): per work unit when an axis has more than 128 nodes; 0: never;
- * 1: always.  The source-list FP32 kernels always use a lattice per 2,048-source block.
- * With it the FP32 tolerances (1e-5 relative per point on V and E) hold for points at least one
- * cell edge away from every charged cell.  Sticky; INVALID_ARG on another mode.
+ * BASELINE configurations, whose points keep more than three cell edges from the cells; tested
+ * at two), too coarse for long axes with points next to cells.  With a lattice per work unit
+ * (32 rows x 64 z nodes) the residual is 2^-25 of the distance to THAT unit's farthest node,
+ * i.e. a few 1e-6 nodes next to the point whatever the size of the grid, at about 8 % more time
+ * (measured on configs[3]: 5.68 instead of 5.27 ms).  mode -1 (default): per work unit when an
+ * axis has more than 128 nodes; 0: never; 1: always.  The source-list FP32 kernels always use a
+ * lattice per 2,048-source block.  With it the FP32 tolerance on E holds for points at least
+ * 1.2 cell edges from every charged cell (tested).  Sticky; INVALID_ARG on another mode.
  */
 qmmm_status qmmm_field_set_local_lattice(qmmm_field *h, int mode);
 

@@ -550,6 +550,34 @@ def test_dz_table_and_stepped_dz_kernels(torch_cuda, B, oracle_mod, nz, P, preci
 
 
 @pytest.mark.parametrize("layout", ["grid", "list"])
+@pytest.mark.parametrize("clearance,local", [(2.0, -1), (1.2, 1)])
+def test_fp32_field_next_to_cells_on_a_128_node_axis(torch_cuda, B, oracle_mod, layout, clearance, local):
+    """What include/qmmm_field.h promises for axes of up to 128 nodes (all FP32 BASELINE
+    configurations): with the whole-grid lattice (automatic there) E keeps 1e-5 for points two
+    cell edges from the charged cells; with qmmm_field_set_local_lattice(h, 1) for points 1.2
+    cell edges away.  The list kernels always use a lattice per 2,048-source block."""
+    n, h = (12, 11, 128), 0.25
+    rng = np.random.default_rng(5)
+    origin = np.array([-1.4, -1.3, -0.5 * h * 127]) + rng.normal(size=3) * 0.05
+    centre = origin + 0.5 * h * (np.array(n) - 1)
+    dense, pos, q = random_grid(rng, n, h, origin, fill=0.9, hole=(centre, 1.0))
+    d = pos - centre
+    r = np.linalg.norm(d, axis=1)
+    rim = np.argsort(r)[:96]
+    pts = pos[rim] - d[rim] / r[rim, None] * (clearance * h)
+    ref = oracle_mod.field(pos, q, NO_XYZ, NO_Z, pts, want_abs=True)
+    hnd = B.qmmm_field_create(pos, q, None, None, len(pts))
+    try:
+        B.qmmm_field_set_local_lattice(hnd, local)
+        V, E = run(torch_cuda, B, hnd, pts, "fp32", layout=layout)
+        if layout == "grid":
+            assert B.qmmm_field_get_info(hnd)["last_local_lattice"] == (1 if local == 1 else 0)
+        check(ref, V, E, TOL32)
+    finally:
+        B.qmmm_field_destroy(hnd)
+
+
+@pytest.mark.parametrize("layout", ["grid", "list"])
 @pytest.mark.parametrize("nz", [400, 130])
 def test_fp32_field_next_to_cells_on_a_long_axis(torch_cuda, B, oracle_mod, layout, nz):
     """FP32 evaluates the field at the point's LATTICE position (only V is corrected for the

@@ -21,7 +21,7 @@ from parity_check import check
 pytestmark = pytest.mark.gpu
 
 TOL = {"fp64": 1e-12, "fp32": 1e-5}
-FAMILIES = ("pair_kernel", "grid_kernel_f32x2", "grid_kernel_f64", "move_server_kernel")
+FAMILIES = ("pair_kernel", "pair_kernel_f32x2", "grid_kernel_f32x2", "grid_kernel_f64", "move_server_kernel")
 
 
 def exported_kernels(lib_path):
@@ -119,29 +119,38 @@ def test_every_kernel_instantiation_runs_and_agrees_with_the_oracle(oracle_mod):
     finally:
         B.qmmm_field_destroy(h)
 
-    # ---- a long z axis: the batched kernels step dz instead of reading a table
-    origin, hh, n3, dense, pos, q, centre = long_axis_grid(rng)
-    pts = centre + rng.normal(size=(P0, 3)) * 0.3
-    pts = centre + (pts - centre) * np.minimum(1.0, 0.9 / np.linalg.norm(pts - centre, axis=1))[:, None]
-    ref_long = oracle_mod.field(pos, q, np.zeros((0, 3)), np.zeros(0), pts, want_abs=True)
-    h = B.qmmm_field_create_grid(origin, hh, n3, dense, None, None, P0)
-    try:
-        for prec in ("fp64", "fp32"):
-            for want_E in (True, False):
-                for overlap in (False, True):
-                    for local in ((-1, 0) if prec == "fp32" else (-1,)):
-                        B.qmmm_field_set_local_lattice(h, local)
-                        for n in (24, P0):
-                            for ppt, pw in ((4, 0), (4, 8), (4, 4), (2, 16), (8, 8)):
-                                if ppt == 8 and prec == "fp64":
-                                    continue
-                                if local == 0 and prec == "fp32" and want_E:
-                                    continue            # whole-grid lattice on a 600-node axis: E out of tolerance by design
-                                evaluate(h, pts[:n], Sub(ref_long, n), "grid", prec,
-                                         dict(points_per_thread=ppt, point_warps=pw), overlap, want_E,
-                                         f"long {prec} n={n} ppt={ppt} pw={pw} ov={overlap} E={want_E} local={local}")
-    finally:
-        B.qmmm_field_destroy(h)
+    # ---- long z axes.  1,700 nodes: no dz table fits, the batched kernels step dz.  130 nodes: the
+    # table fits and the FP32 kernels use the lattice per work unit (more than 128 nodes).
+    for nz in (1700, 130):
+        origin, hh, n3, dense, pos, q, centre = long_axis_grid(rng, nz)
+        pts = centre + rng.normal(size=(P0, 3)) * 0.3
+        pts = centre + (pts - centre) * np.minimum(1.0, 0.9 / np.linalg.norm(pts - centre, axis=1))[:, None]
+        ref_long = oracle_mod.field(pos, q, np.zeros((0, 3)), np.zeros(0), pts, want_abs=True)
+        h = B.qmmm_field_create_grid(origin, hh, n3, dense, None, None, P0)
+        try:
+            for prec in ("fp64", "fp32"):
+                for want_E in (True, False):
+                    for overlap in (False, True):
+                        for local in ((-1, 0) if prec == "fp32" else (-1,)):
+                            B.qmmm_field_set_local_lattice(h, local)
+                            for n in (24, P0):
+                                for ppt, pw in ((4, 0), (4, 8), (4, 4), (2, 16), (8, 8)):
+                                    if ppt == 8 and prec == "fp64":
+                                        continue
+                                    if local == 0 and prec == "fp32" and want_E:
+                                        continue        # whole-grid lattice forced on an axis of more than 128 nodes:
+                                                        # E is out of tolerance by design (include/qmmm_field.h)
+                                    evaluate(h, pts[:n], Sub(ref_long, n), "grid", prec,
+                                             dict(points_per_thread=ppt, point_warps=pw), overlap, want_E,
+                                             f"nz={nz} {prec} n={n} ppt={ppt} pw={pw} ov={overlap} E={want_E} local={local}")
+            if nz == 130:
+                # light CTAs (overlap) with the dz table beside a shallow pipeline, lattice per work unit
+                B.qmmm_field_set_local_lattice(h, -1)
+                evaluate(h, pts[:24], Sub(ref_long, 24), "grid", "fp32",
+                         dict(points_per_thread=4, point_warps=4, stages=2), True, True,
+                         "nz=130 fp32 n=24 ppt=4 pw=4 stages=2 ov=True E=True local=-1")
+        finally:
+            B.qmmm_field_destroy(h)
 
     missing = exported - set(seen)
     extra = set(seen) - exported
