@@ -787,6 +787,8 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
         if (prm.push_slots) {                    // (uniform over the grid)
             finish_point_block_push<NT>(prm, WP * EPT, threadIdx.x, flag, reinterpret_cast<double *>(smem), red,
                                         [] { __syncthreads(); });
+            QMMM_MARK(6);
+            QMMM_MARK_GT(9);
             return;
         }
     }
@@ -820,6 +822,8 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
     constexpr int STAGE_BYTES = GRID_STAGE_BYTES_F64;
     extern __shared__ __align__(128) unsigned char smem[];
     pdl_launch_dependents();
+    QMMM_MARK_GT(8);
+    QMMM_MARK(0);
     const int stages = WARPOWN ? NW : prm.stages;
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + static_cast<size_t>(stages) * STAGE_BYTES);
     uint64_t *empty = full + 8;
@@ -884,6 +888,7 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
         }
     }
     __syncthreads();
+    QMMM_MARK(1);
 
     if (warp == NW) {
         if constexpr (!WARPOWN) {
@@ -963,6 +968,7 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
     };
 
     const int segs = prm.g_segs, ny = prm.g_n[1];
+    QMMM_MARK(2);
     if constexpr (WARPOWN) {
         int it = 0;
         for (int g = lo + warp; g < hi; g += NW, ++it) {
@@ -1007,6 +1013,7 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
         }
     }
 
+    QMMM_MARK(3);
     // nuclei (units of hz), FP64
     if constexpr (WITH_E) {
         nuclei_share<EPT>(prm, pe, ws, WS, lane, V, Ex, Ey, Ez);
@@ -1017,6 +1024,7 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
         nuclei_share<EPT>(prm, pe, ws, WS, lane, V, nEx, nEy, nEz);
     }
 
+    QMMM_MARK(4);
 #pragma unroll
     for (int e = 0; e < EPT; ++e) {
         V[e] = warp_sum(V[e]);
@@ -1044,13 +1052,18 @@ __global__ void __launch_bounds__(32 * (NW + 1), 1) grid_kernel_f64(const PairPa
         else if (lane < EPT * 4 && p < prm.P)
             prm.partial[(static_cast<int64_t>(blockIdx.y) * prm.P + p) * 4 + (lane & 3)] = a;
     }
+    QMMM_MARK(5);
     if (prm.push_slots) {                        // (uniform over the grid)
         finish_point_block_push<32 * NW>(prm, WP * EPT, threadIdx.x, flag, reinterpret_cast<double *>(smem), red,
                                          [] { consumer_sync<NW>(); });
+        QMMM_MARK(6);
+        QMMM_MARK_GT(9);
         return;
     }
     finish_point_block<32 * NW>(prm, WP * EPT, threadIdx.x, flag, red, [] { consumer_sync<NW>(); },
                                 prm.seq);
+    QMMM_MARK(6);
+    QMMM_MARK_GT(9);
 }
 
 // ----------------------------------------------------------------------------- create: detect

@@ -703,6 +703,8 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) pair_kernel(const PairParams p
         finish_point_block_push<32 * COMPUTE_WARPS>(prm, WP * EPT, threadIdx.x, flag,
                                                     reinterpret_cast<double *>(smem), red,
                                                     [] { compute_warps_sync(); });
+        QMMM_MARK(6);
+        QMMM_MARK_GT(9);
         return;
     }
     finish_point_block<32 * COMPUTE_WARPS>(prm, WP * EPT, threadIdx.x, flag, red,
@@ -1023,6 +1025,8 @@ __global__ void __launch_bounds__(32 * NW, 1) pair_kernel_f32x2(const PairParams
         if (prm.push_slots) {                    // (uniform over the grid)
             finish_point_block_push<NT>(prm, WP * EPT, threadIdx.x, flag, reinterpret_cast<double *>(smem), red,
                                         [] { __syncthreads(); });
+            QMMM_MARK(6);
+            QMMM_MARK_GT(9);
             return;
         }
     }
