@@ -117,7 +117,14 @@ qmmm_status qmmm_field_eval_energy(qmmm_field *h, const double *elec_xyz, int64_
  *               writes {V, E} back -- no kernel launch, copy or synchronisation per move.
  *               It retires by itself after 2 ms without a request (and after 1 s in any
  *               case) and is restarted transparently; any other call on the handle retires
- *               it first.  While it is resident it occupies every SM.  `stream` is not used.
+ *               it first.  While it is resident it occupies every SM, so there is at most
+ *               one per device: when several handles make host-buffer calls at the same time
+ *               (qmmm_field_share) a resident server is asked to yield and everybody uses the
+ *               launch path below until the device is quiet again.  `stream` is not used.
+ *               Environments with the grid-aware copy are served by the grid-aware server
+ *               (every warp keeps its work units of charges in shared memory: configs[2]
+ *               needs no source traffic at all per move), others -- and layout LIST -- by
+ *               the source-list server.
  *   W*N <= 64 : one kernel launch on `stream`, no copies and no stream synchronisation: up to
  *               32 points travel as kernel parameters (more are read by the kernel from a
  *               pinned, device-mapped mailbox), and the results come back as one tagged
@@ -125,8 +132,9 @@ qmmm_status qmmm_field_eval_energy(qmmm_field *h, const double *elec_xyz, int64_
  *               host memory, which the call polls (or, for launch shapes the record
  *               collection does not cover, as V, E followed by a sequence number).
  *   otherwise : host->device copy, kernel, device->host copy on `stream`, synchronisation.
- * All three give bitwise the result of qmmm_field_eval with the same plan and layout (the
- * move server always reads the source list: layout LIST).
+ * The launch paths and the source-list server give bitwise the result of qmmm_field_eval with
+ * the same plan and layout; the grid-aware server splits the work units over its warps in its
+ * own way and agrees to rounding (deterministic from call to call).
  * Same argument meaning and errors as qmmm_field_eval.
  */
 qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int64_t W,
@@ -179,8 +187,7 @@ qmmm_status qmmm_field_eval_moves(qmmm_field *h, const double *elec_xyz, int64_t
  *   cell_q [n0][n1][n2]         cell CHARGES, C order (z fastest), host or device pointer;
  *                               0 = no cell there
  *   nuclei, max_points, out     as qmmm_field_create
- * A handle made by qmmm_field_create_grid has no source list (layout LIST is refused; the
- * single-point move server is not used).  Precondition of the grid layout: no evaluation
+ * A handle made by qmmm_field_create_grid has no source list (layout LIST is refused).  Precondition of the grid layout: no evaluation
  * point coincides with a node that carries charge (empty nodes are harmless).
  * Errors as qmmm_field_create.
  */

@@ -675,6 +675,29 @@ cudaError_t detect_grid(qmmm_field *h, const double *dxyz, const double *dq, int
 
 namespace {
 
+// Grid layout: cells as charges only, coordinates from the indices; everything in grid units.
+void fill_grid_params(qmmm_field *h, PairParams &prm, bool f32) {
+    prm.chunks = f32 ? reinterpret_cast<const char *>(h->gcells32)
+                     : reinterpret_cast<const char *>(h->gcells64);
+    prm.n_chunks = static_cast<int>(h->n_g);
+    prm.nuc = h->nuclei_u;
+    prm.K = static_cast<int>(h->K);
+    for (int k = 0; k < 3; ++k) prm.g_org[k] = h->grid.org[k];
+    for (int k = 0; k < 3; ++k) prm.g_inv_h[k] = 1.0 / h->grid.h[k];
+    prm.g_sx = h->grid.h[0] / h->grid.h[2];        // exactly 1 for cubic cells
+    prm.g_sy = h->grid.h[1] / h->grid.h[2];
+    prm.g_ortho = (prm.g_sx != 1.0 || prm.g_sy != 1.0) ? 1 : 0;
+    prm.g_scaleV = 1.0 / h->grid.h[2];
+    prm.g_scaleE = 1.0 / (h->grid.h[2] * h->grid.h[2]);
+    for (int k = 0; k < 3; ++k) prm.g_n[k] = h->grid.n[k];
+    prm.g_segs = static_cast<int>(h->g_segs);
+    // FP32: the whole-grid lattice quantum is 2^-24 of the axis (in nodes); beyond 128 nodes
+    // the field of cells next to a point would lose accuracy (qmmm_grid.cuh, on_lattice)
+    const int nmax = std::max({h->grid.n[0], h->grid.n[1], h->grid.n[2]});
+    prm.g_fine = (f32 && (h->local_lattice == 1 || (h->local_lattice < 0 && nmax > 128))) ? 1 : 0;
+    h->last_local_lattice = prm.g_fine;
+}
+
 // ------------------------------------------------------------------ resident move server
 double now_seconds() {
     struct timespec t;
@@ -780,18 +803,46 @@ cudaError_t server_launch(const ServerParams &sp, int slices, size_t smem, cudaS
                                        dim3(CTA_THREADS), args, smem, st);
 }
 
+template <bool F32>
+cudaError_t server_grid_launch(const ServerParams &sp, int slices, size_t smem, cudaStream_t st) {
+    auto kern = move_server_grid_kernel<F32>;
+    static SmemConfig configured;
+    static const char *const name = kernel_name(reinterpret_cast<const void *>(kern));
+    g_launched = name;
+    cudaError_t e = configured.ensure(kern, smem);
+    if (e != cudaSuccess) return e;
+    void *args[] = {const_cast<ServerParams *>(&sp)};
+    return cudaLaunchCooperativeKernel(reinterpret_cast<void *>(kern), dim3(1, slices),
+                                       dim3(32 * SERVER_GRID_NW), args, smem, st);
+}
+
 // Starts the server for `prec`; *usable = false when this problem cannot be served (the
 // caller then uses the launch path).
 qmmm_status server_start(qmmm_field *h, int prec, bool *usable) {
     const bool f32 = prec == QMMM_FP32_ACC64;
     *usable = false;
-    const int64_t n_chunks = f32 ? h->n_chunks : h->n_chunks64;
-    if (!h->srv_ok || n_chunks < 1 || h->timing || !h->has_list || h->layout == QMMM_LAYOUT_GRID) return QMMM_OK;
+    // the grid-aware server when the handle has the compact copy (and LIST is not forced), else
+    // the source-list server
+    const bool grid = h->has_grid && h->layout != QMMM_LAYOUT_LIST;
+    const int64_t n_chunks = grid ? h->n_g : (f32 ? h->n_chunks : h->n_chunks64);
+    if (!h->srv_ok || n_chunks < 1 || h->timing || (!grid && !h->has_list)) return QMMM_OK;
     qmmm_plan pl = choose_plan(h, 1, f32);
-    if (pl.points_per_thread != 1 || pl.point_warps != 1 || pl.slices > h->sm_count) return QMMM_OK;
+    size_t smem = 0;
+    if (grid) {
+        pl.points_per_thread = 1;
+        pl.point_warps = 1;
+        pl.slices = static_cast<int>(std::min<int64_t>(h->sm_count, std::max<int64_t>(h->n_g, (h->K + 31) / 32)));
+        pl.stages = f32 ? 2 : 1;
+        smem = f32 ? ServerGridLayout<true>::total(pl.slices) : ServerGridLayout<false>::total(pl.slices);
+        if (static_cast<int64_t>(pl.slices) * SLOT_WORDS > h->workspace_doubles) return QMMM_OK;
+    } else {
+        if (pl.points_per_thread != 1 || pl.point_warps != 1 || pl.slices > h->sm_count) return QMMM_OK;
+    }
     const size_t extra = 128 + static_cast<size_t>(pl.slices) * 4 * sizeof(double);   // cmd, go, collected partials
-    size_t smem = pair_smem_bytes(f32, pl.stages, 1, 1) + extra;
-    while (smem > 227 * 1024 && pl.stages > 2) smem = pair_smem_bytes(f32, --pl.stages, 1, 1) + extra;
+    if (!grid) {
+        smem = pair_smem_bytes(f32, pl.stages, 1, 1) + extra;
+        while (smem > 227 * 1024 && pl.stages > 2) smem = pair_smem_bytes(f32, --pl.stages, 1, 1) + extra;
+    }
 
     {
         // one resident server per device, and none while several handles make host-path calls
@@ -811,21 +862,26 @@ qmmm_status server_start(qmmm_field *h, int prec, bool *usable) {
     ServerParams sp;
     std::memset(&sp, 0, sizeof(sp));
     PairParams &prm = sp.pair;
-    prm.chunks = f32 ? reinterpret_cast<const char *>(h->chunks32)
-                     : reinterpret_cast<const char *>(h->chunks64);
-    prm.origins = h->origins;
     prm.partial = h->workspace;
     prm.P = 1;
     prm.n_chunks = static_cast<int>(n_chunks);
     prm.slices = pl.slices;
     prm.point_warps = 1;
     prm.stages = pl.stages;
-    prm.lattice = h->lattice;
-    prm.inv_lattice = 1.0 / h->lattice;
-    prm.nuc = h->nuclei;
-    prm.K = f32 ? static_cast<int>(h->K) : 0;
     prm.q_unscale = f32 ? 1.0 / h->q_scale : 1.0;
     prm.counters = h->counters;
+    prm.dev_err = h->dev_err_d;
+    if (grid) {
+        fill_grid_params(h, prm, f32);
+    } else {
+        prm.chunks = f32 ? reinterpret_cast<const char *>(h->chunks32)
+                         : reinterpret_cast<const char *>(h->chunks64);
+        prm.origins = h->origins;
+        prm.lattice = h->lattice;
+        prm.inv_lattice = 1.0 / h->lattice;
+        prm.nuc = h->nuclei;
+        prm.K = f32 ? static_cast<int>(h->K) : 0;
+    }
     sp.mail = h->srv_mail_d;
     sp.dev = h->srv_dev;
     sp.start_seq = h->srv_seq;
@@ -843,8 +899,10 @@ qmmm_status server_start(qmmm_field *h, int prec, bool *usable) {
             return cuda_fail(e0, "move server set-up");
         }
     }
-    cudaError_t e = f32 ? server_launch<float>(sp, pl.slices, smem, h->srv_stream)
-                        : server_launch<double>(sp, pl.slices, smem, h->srv_stream);
+    cudaError_t e = grid ? (f32 ? server_grid_launch<true>(sp, pl.slices, smem, h->srv_stream)
+                                : server_grid_launch<false>(sp, pl.slices, smem, h->srv_stream))
+                         : (f32 ? server_launch<float>(sp, pl.slices, smem, h->srv_stream)
+                                : server_launch<double>(sp, pl.slices, smem, h->srv_stream));
     if (e != cudaSuccess) {                    // e.g. the GPU is shared and cannot hold the grid
         cudaGetLastError();
         h->srv_ok = false;
@@ -853,6 +911,7 @@ qmmm_status server_start(qmmm_field *h, int prec, bool *usable) {
     }
     h->srv_alive = true;
     h->last_kernel = g_launched;
+    h->last_layout = grid ? QMMM_LAYOUT_GRID : QMMM_LAYOUT_LIST;
     h->srv_prec = prec;
     h->last_plan = pl;
     h->last_point_blocks = 1;
@@ -1305,6 +1364,7 @@ qmmm_status qmmm_field_set_timing(qmmm_field *h, int enable) {
 qmmm_status qmmm_field_set_local_lattice(qmmm_field *h, int mode) {
     if (!h) return fail(QMMM_ERR_INVALID_ARG, "set_local_lattice: NULL handle");
     if (mode < -1 || mode > 1) return fail(QMMM_ERR_INVALID_ARG, "set_local_lattice: mode must be -1, 0 or 1");
+    server_stop(h);
     h->local_lattice = mode;
     return QMMM_OK;
 }
@@ -1447,28 +1507,9 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
             }
         }
         if (grid) {
-            // cells: charges only, coordinates from the indices; everything in grid units
-            prm.chunks = f32 ? reinterpret_cast<const char *>(h->gcells32)
-                             : reinterpret_cast<const char *>(h->gcells64);
-            prm.n_chunks = static_cast<int>(h->n_g);
-            prm.nuc = h->nuclei_u;
-            prm.K = static_cast<int>(h->K);
-            for (int k = 0; k < 3; ++k) prm.g_org[k] = h->grid.org[k];
-            for (int k = 0; k < 3; ++k) prm.g_inv_h[k] = 1.0 / h->grid.h[k];
-            prm.g_sx = h->grid.h[0] / h->grid.h[2];        // exactly 1 for cubic cells
-            prm.g_sy = h->grid.h[1] / h->grid.h[2];
-            prm.g_ortho = (prm.g_sx != 1.0 || prm.g_sy != 1.0) ? 1 : 0;
-            prm.g_scaleV = 1.0 / h->grid.h[2];
-            prm.g_scaleE = 1.0 / (h->grid.h[2] * h->grid.h[2]);
-            for (int k = 0; k < 3; ++k) prm.g_n[k] = h->grid.n[k];
-            prm.g_segs = static_cast<int>(h->g_segs);
+            fill_grid_params(h, prm, f32);
             prm.g_dzt = use_dzt ? 1 : 0;
             prm.g_light = light ? 1 : 0;
-            // FP32: the whole-grid lattice quantum is 2^-24 of the axis (in nodes); beyond 128 nodes
-            // the field of cells next to a point would lose accuracy (qmmm_grid.cuh, on_lattice)
-            const int nmax = std::max({h->grid.n[0], h->grid.n[1], h->grid.n[2]});
-            prm.g_fine = (f32 && (h->local_lattice == 1 || (h->local_lattice < 0 && nmax > 128))) ? 1 : 0;
-            h->last_local_lattice = prm.g_fine;
         } else {
             prm.chunks = f32 ? reinterpret_cast<const char *>(h->chunks32)
                              : reinterpret_cast<const char *>(h->chunks64);

@@ -21,6 +21,7 @@
 // Results are bitwise those of the launch path with the same partition.
 #pragma once
 #include "qmmm_kernels.cuh"
+#include "qmmm_grid.cuh"
 
 namespace qmmm {
 
@@ -128,6 +129,58 @@ __device__ __forceinline__ bool server_collect(const PairParams &prm, ServerMail
     return true;
 }
 
+// Warp 0 of every CTA waits here for the next move.  Leader CTA: polls the request line in pinned
+// host memory, relays r_new through device memory and publishes the move number; the others
+// poll that number.  Returns the move number (or SERVER_EXIT) in every lane; elec_s[0..2] = r_new.
+__device__ __forceinline__ unsigned long long server_next_move(const ServerParams &sp, bool leader, int lane,
+                                                               unsigned long long last, long long t_start,
+                                                               double *elec_s) {
+    unsigned long long c = 0, w = 0;
+    if (leader) {
+        // lanes 0..4 read the request line over PCIe in one transaction
+        const long long t_idle = global_ns();
+        for (;;) {
+            w = lane < 6 ? sp.mail->req[lane] : 0ull;
+            const unsigned long long a = __shfl_sync(0xffffffffu, w, 0);
+            const unsigned long long b = __shfl_sync(0xffffffffu, w, 4);
+            if (a == b && a != last) { c = a; break; }
+            if (__shfl_sync(0xffffffffu, w, 5) != 0ull) {      // another handle wants the device
+                c = SERVER_EXIT;
+                break;
+            }
+            const long long now = __shfl_sync(0xffffffffu, global_ns(), 0);
+            if (now - t_idle > SERVER_IDLE_NS || now - t_start > SERVER_LIFE_NS) {
+                c = SERVER_EXIT;
+                break;
+            }
+        }
+        if (c != SERVER_EXIT && lane >= 1 && lane <= 3) {
+            const double v = __longlong_as_double(static_cast<long long>(w));
+            elec_s[lane - 1] = v;
+            sp.dev->elec[lane - 1] = v;
+            __threadfence();
+        }
+        __syncwarp();
+        if (lane == 0) *reinterpret_cast<volatile unsigned long long *>(&sp.dev->cmd) = c;
+    } else {
+        for (;;) {
+            if (lane == 0) c = *reinterpret_cast<volatile unsigned long long *>(&sp.dev->cmd);
+            c = __shfl_sync(0xffffffffu, c, 0);
+            if (c != last) break;
+            const long long now = __shfl_sync(0xffffffffu, global_ns(), 0);
+            if (now - t_start > SERVER_HARD_NS) {
+                c = SERVER_EXIT;
+                break;
+            }
+        }
+        if (c != SERVER_EXIT) {
+            __threadfence();
+            if (lane < 3) elec_s[lane] = __ldcg(&sp.dev->elec[lane]);
+        }
+    }
+    return c;
+}
+
 // grid = (1, slices) with slices <= SM count, launched cooperatively (all CTAs resident).
 template <typename REAL>
 __global__ void __launch_bounds__(CTA_THREADS, 1) move_server_kernel(const ServerParams sp) {
@@ -211,49 +264,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) move_server_kernel(const Serve
     const long long t_start = global_ns();
     for (;;) {
         if (warp == 0) {
-            unsigned long long c = 0, w = 0;
-            if (leader) {
-                // lanes 0..4 read the request line over PCIe in one transaction
-                const long long t_idle = global_ns();
-                for (;;) {
-                    w = lane < 6 ? sp.mail->req[lane] : 0ull;
-                    const unsigned long long a = __shfl_sync(0xffffffffu, w, 0);
-                    const unsigned long long b = __shfl_sync(0xffffffffu, w, 4);
-                    if (a == b && a != last) { c = a; break; }
-                    if (__shfl_sync(0xffffffffu, w, 5) != 0ull) {      // another handle wants the device
-                        c = SERVER_EXIT;
-                        break;
-                    }
-                    const long long now = __shfl_sync(0xffffffffu, global_ns(), 0);
-                    if (now - t_idle > SERVER_IDLE_NS || now - t_start > SERVER_LIFE_NS) {
-                        c = SERVER_EXIT;
-                        break;
-                    }
-                }
-                if (c != SERVER_EXIT && lane >= 1 && lane <= 3) {
-                    const double v = __longlong_as_double(static_cast<long long>(w));
-                    elec_s[lane - 1] = v;
-                    sp.dev->elec[lane - 1] = v;
-                    __threadfence();
-                }
-                __syncwarp();
-                if (lane == 0) *reinterpret_cast<volatile unsigned long long *>(&sp.dev->cmd) = c;
-            } else {
-                for (;;) {
-                    if (lane == 0) c = *reinterpret_cast<volatile unsigned long long *>(&sp.dev->cmd);
-                    c = __shfl_sync(0xffffffffu, c, 0);
-                    if (c != last) break;
-                    const long long now = __shfl_sync(0xffffffffu, global_ns(), 0);
-                    if (now - t_start > SERVER_HARD_NS) {
-                        c = SERVER_EXIT;
-                        break;
-                    }
-                }
-                if (c != SERVER_EXIT) {
-                    __threadfence();
-                    if (lane < 3) elec_s[lane] = __ldcg(&sp.dev->elec[lane]);
-                }
-            }
+            const unsigned long long c = server_next_move(sp, leader, lane, last, t_start, elec_s);
             if (lane == 0) {
                 *cmd_s = c;
                 *go_s = c == SERVER_EXIT ? SERVER_EXIT : ++released;    // release the producer
@@ -349,6 +360,241 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) move_server_kernel(const Serve
             compute_warps_sync();
             for (int s = 0; s < npre; ++s, ++k)
                 mbar_wait(&full[k % stages], static_cast<uint32_t>(k / stages) & 1u);
+            break;
+        }
+    }
+    if (leader && threadIdx.x == 0) {
+        __threadfence_system();
+        sp.mail->exited = sp.launch_id;
+    }
+}
+
+// ----------------------------------------------------------------------------- grid-aware server
+// The same resident server for environments that have the grid-aware compact copy (charges
+// only, qmmm_grid.cuh): 4 / 8 B per cell instead of 16 / 32 B, and the single-point walks of the
+// grid kernels (FP32: two z nodes per register pair, GridRowF32N; FP64: the scalar row walk).
+// Every warp owns the gchunks lo + w, lo + w + NW, ... of its CTA's slice and loads them itself
+// into private slots (FP32 two, FP64 one): no producer warp, no waiting on other warps.  The
+// assignment never changes, so a warp whose share fits its slots (configs[2]: 1,024 gchunks over
+// 148 CTAs x 8 warps: at most one each) loads it ONCE when the server starts and serves every
+// move from shared memory -- no source traffic at all per move; larger shares stream, with the
+// first gchunks of the next move prefetched while the CTA waits for it.
+constexpr int SERVER_GRID_NW = 8;
+template <bool F32>
+struct ServerGridLayout {
+    static constexpr int SLOTS = F32 ? 2 : 1;                       // per warp
+    static constexpr int SLOT_BYTES = F32 ? GRID_NODES * 4 : GRID_NODES * 8;
+    static constexpr int STAGE_BYTES = SERVER_GRID_NW * SLOTS * SLOT_BYTES;     // 128 KB
+    static constexpr int FIXED_BYTES = 16 * 8 /* barriers */ + 256 * 8 /* red / scratch */ + 8 * 8 /* r_new, cmd, flag */;
+    __host__ __device__ static constexpr size_t total(int slices) {
+        return static_cast<size_t>(STAGE_BYTES) + FIXED_BYTES + static_cast<size_t>(slices) * 4 * sizeof(double);
+    }
+};
+
+// prm: grid fields as for the grid kernels (chunks = gchunks, n_chunks = their number, nuc = nuclei
+// in units of hz, g_*), P = 1; grid = (1, slices), slices <= SM count, launched cooperatively.
+template <bool F32>
+__global__ void __launch_bounds__(32 * SERVER_GRID_NW, 1) move_server_grid_kernel(const ServerParams sp) {
+    using L = ServerGridLayout<F32>;
+    constexpr int NW = SERVER_GRID_NW, NT = 32 * NW, S = L::SLOTS, SB = L::SLOT_BYTES;
+    const PairParams &prm = sp.pair;
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + L::STAGE_BYTES);          // [NW][S]
+    double *red = reinterpret_cast<double *>(full + 16);                           // [256]
+    double *elec_s = red + 256;                                                    // [3] r_new, bohr
+    volatile unsigned long long *cmd_s = reinterpret_cast<volatile unsigned long long *>(elec_s + 4);
+    int *flag = reinterpret_cast<int *>(elec_s + 6);
+    double *part_s = elec_s + 8;                                                   // leader: [slices][4]
+    unsigned long long *slots = reinterpret_cast<unsigned long long *>(prm.partial);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int lo, hi;
+    slice_range(prm.n_chunks, prm.slices, blockIdx.y, lo, hi);
+    const int cnt = hi - lo > warp ? (hi - lo - warp + NW - 1) / NW : 0;           // gchunks of this warp
+    const int segs = prm.g_segs, ny = prm.g_n[1];
+    unsigned char *my_slots = smem + static_cast<size_t>(warp) * S * SB;
+    uint64_t *my_full = full + warp * S;
+    uint32_t phase = 0, pending = 0;                     // bit per slot (warp-uniform)
+    // Shares larger than the slots stream through them round robin: the n-th gchunk this warp
+    // walks since the server started (its gchunk number n % cnt) sits in slot n % S, and the
+    // slot is refilled at once with the gchunk that is walked S steps later.
+    unsigned nrun = 0;
+    auto load_into = [&](int i, int slot) {              // gchunk number i of this warp -> slot
+        if (lane == 0) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            mbar_expect_tx(&my_full[slot], SB);
+            tma_bulk_g2s(my_slots + static_cast<size_t>(slot) * SB,
+                         prm.chunks + static_cast<size_t>(lo + warp + i * NW) * SB, SB, &my_full[slot]);
+        }
+        pending |= 1u << slot;
+    };
+    if (lane == 0) {
+        for (int k = 0; k < S; ++k) mbar_init(&my_full[k], 1);
+        fence_barrier_init();
+    }
+    if (threadIdx.x == 0) *cmd_s = sp.start_seq;
+    __syncwarp();
+    for (int i = 0; i < cnt && i < S; ++i) load_into(i, i);
+    __syncthreads();
+
+    unsigned long long last = sp.start_seq;
+    const bool leader = blockIdx.y == 0;
+    const long long t_start = global_ns();
+    const bool fine = F32 && prm.g_fine != 0;
+    const int n_rows = prm.g_n[0] * prm.g_n[1];
+    for (;;) {
+        if (warp == 0) {
+            const unsigned long long c = server_next_move(sp, leader, lane, last, t_start, elec_s);
+            if (lane == 0) *cmd_s = c;
+        }
+        __syncthreads();
+        const unsigned long long cmd = *cmd_s;
+        if (cmd == SERVER_EXIT) {
+            for (int k = 0; k < S; ++k)                  // no bulk copy may be in flight when the CTA ends
+                if (pending & (1u << k)) mbar_wait(&my_full[k], (phase >> k) & 1u);
+            break;
+        }
+        last = cmd;
+
+        // the point in node units (u) and in units of hz (uh: the nuclei, the FP64 walk)
+        double u[3], uh[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            u[k] = (elec_s[k] - prm.g_org[k]) * prm.g_inv_h[k];
+            uh[k] = u[k] * (k == 0 ? prm.g_sx : (k == 1 ? prm.g_sy : 1.0));
+        }
+        double V = 0.0, Ex = 0.0, Ey = 0.0, Ez = 0.0;    // this thread's sums, grid units
+        if constexpr (F32) {
+            // lattice coordinates a (relative to the reference node ir) and residuals dd (units of hz)
+            // of the point: lanes 0..2 compute one axis each, everybody gets all three
+            float ax, ay, az, ddx, ddy, ddz;
+            int irx, iry, irz;
+            auto lattice = [&](int xl, int xh, int yl, int yh, int zl, int zh) {
+                float a = 0.0f, dd = 0.0f;
+                int il = 0;
+                if (lane < 3) {
+                    il = lane == 0 ? xl : (lane == 1 ? yl : zl);
+                    on_lattice(u[lane], il, lane == 0 ? xh : (lane == 1 ? yh : zh), a, dd);
+                    dd *= static_cast<float>(lane == 0 ? prm.g_sx : (lane == 1 ? prm.g_sy : 1.0));
+                }
+                ax = __shfl_sync(0xffffffffu, a, 0); ay = __shfl_sync(0xffffffffu, a, 1); az = __shfl_sync(0xffffffffu, a, 2);
+                ddx = __shfl_sync(0xffffffffu, dd, 0); ddy = __shfl_sync(0xffffffffu, dd, 1); ddz = __shfl_sync(0xffffffffu, dd, 2);
+                irx = __shfl_sync(0xffffffffu, il, 0); iry = __shfl_sync(0xffffffffu, il, 1); irz = __shfl_sync(0xffffffffu, il, 2);
+            };
+            if (!fine) lattice(0, prm.g_n[0] - 1, 0, prm.g_n[1] - 1, 0, prm.g_n[2] - 1);
+            float vv = 0.0f, tt = 0.0f, ex = 0.0f, ey = 0.0f, ez = 0.0f, cc = 0.0f;
+            int run = 0;
+            auto flush = [&]() {
+                V += 1.5 * static_cast<double>(vv) - 0.5 * static_cast<double>(tt) - static_cast<double>(cc);
+                Ex += static_cast<double>(ex); Ey += static_cast<double>(ey); Ez += static_cast<double>(ez);
+                vv = tt = ex = ey = ez = cc = 0.0f;
+                run = 0;
+            };
+            for (int i = 0; i < cnt; ++i, ++nrun) {
+                const int slot = cnt > S ? static_cast<int>(nrun % S) : i, g = lo + warp + i * NW;
+                const int tl = g / segs, sg = g - tl * segs;
+                const int rw = tl * 32 + lane, rx = rw / ny;
+                if (fine) {                              // the lattice of THIS gchunk's nodes
+                    const int r0 = tl * 32, r1 = min(r0 + 31, n_rows - 1), x0 = r0 / ny, x1 = r1 / ny;
+                    lattice(x0, x1, x0 == x1 ? r0 - x0 * ny : 0, x0 == x1 ? r1 - x0 * ny : ny - 1,
+                            sg * GRID_ZS, sg * GRID_ZS + GRID_ZS - 1);
+                }
+                if (pending & (1u << slot)) {
+                    mbar_wait(&my_full[slot], (phase >> slot) & 1u);
+                    phase ^= 1u << slot;
+                    pending &= ~(1u << slot);
+                }
+                const float *data = reinterpret_cast<const float *>(my_slots + static_cast<size_t>(slot) * SB);
+                const float dxs = (ax - static_cast<float>(rx - irx)) * static_cast<float>(prm.g_sx);   // exact, then hx/hz
+                const float dys = (ay - static_cast<float>(rw - rx * ny - iry)) * static_cast<float>(prm.g_sy);
+                GridRowF32N row;
+                row.start(az - static_cast<float>(sg * GRID_ZS - irz), fmaf(dys, dys, fmaf(dxs, dxs, 1e-30f)));
+                float v1, t1;
+                row.run(data + 4 * lane, GRID_ZS / 4, v1, t1);
+                const float s1 = row.S.x + row.S.y;
+                const float exg = dxs * s1, eyg = dys * s1, ezg = row.SZ.x + row.SZ.y;
+                vv += v1; tt += t1; ex += exg; ey += eyg; ez += ezg;
+                if (fine) cc = fmaf(exg, ddx, fmaf(eyg, ddy, fmaf(ezg, ddz, cc)));
+                __syncwarp();                            // every lane has read the slot
+                if (cnt > S) load_into(i + S < cnt ? i + S : i + S - cnt, slot);   // (wraps to the next move)
+                if (++run == GRID_FLUSH) flush();
+            }
+            if (run) flush();
+            // whole-grid lattice: V(u) = V(a) - E(a) . dd (the local lattice did it gchunk by gchunk)
+            if (!fine) V -= Ex * static_cast<double>(ddx) + Ey * static_cast<double>(ddy) + Ez * static_cast<double>(ddz);
+            V *= prm.q_unscale; Ex *= prm.q_unscale; Ey *= prm.q_unscale; Ez *= prm.q_unscale;
+        } else {
+            for (int i = 0; i < cnt; ++i, ++nrun) {
+                const int slot = cnt > S ? static_cast<int>(nrun % S) : i, g = lo + warp + i * NW;
+                const int tl = g / segs, sg = g - tl * segs;
+                const int rw = tl * 32 + lane, rx = rw / ny;
+                if (pending & (1u << slot)) {
+                    mbar_wait(&my_full[slot], (phase >> slot) & 1u);
+                    phase ^= 1u << slot;
+                    pending &= ~(1u << slot);
+                }
+                const double *b = reinterpret_cast<const double *>(my_slots + static_cast<size_t>(slot) * SB) + 2 * lane;
+                const double dx = uh[0] - static_cast<double>(rx) * prm.g_sx;
+                const double dy = uh[1] - static_cast<double>(rw - rx * ny) * prm.g_sy;
+                const double rxy2 = fma(dy, dy, fma(dx, dx, 1e-200));
+                double azb = uh[2] - static_cast<double>(sg * GRID_ZS), Sx = 0.0, SZ = 0.0;
+#pragma unroll 1
+                for (int k4 = 0; k4 < GRID_ZS / 4; ++k4) {
+                    const double2 Qa = *reinterpret_cast<const double2 *>(b + (2 * k4) * 64);
+                    const double2 Qb = *reinterpret_cast<const double2 *>(b + (2 * k4 + 1) * 64);
+                    const double qs[4] = {Qa.x, Qa.y, Qb.x, Qb.y};
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) {
+                        const double dz = t == 0 ? azb : azb - static_cast<double>(t);
+                        const double y = rsqrt_refined_f64(fma(dz, dz, rxy2));
+                        const double p = qs[t] * y;
+                        V += p;
+                        const double sv = p * (y * y);
+                        Sx += sv;
+                        SZ = fma(sv, dz, SZ);
+                    }
+                    azb -= 4.0;
+                }
+                Ex = fma(dx, Sx, Ex);
+                Ey = fma(dy, Sx, Ey);
+                Ez += SZ;
+                __syncwarp();
+                if (cnt > S) load_into(i + S < cnt ? i + S : i + S - cnt, slot);
+            }
+        }
+        // nuclei of this CTA's share (units of hz), FP64, thread-strided
+        {
+            int klo, khi;
+            slice_range(prm.K, prm.slices, blockIdx.y, klo, khi);
+            for (int j = klo + threadIdx.x; j < khi; j += NT) {
+                const double2 a = *reinterpret_cast<const double2 *>(prm.nuc + 4 * static_cast<int64_t>(j));
+                const double2 b2 = *reinterpret_cast<const double2 *>(prm.nuc + 4 * static_cast<int64_t>(j) + 2);
+                pair_f64(uh[0], uh[1], uh[2], a.x, a.y, b2.x, b2.y, V, Ex, Ey, Ez);
+            }
+        }
+        const double sV = warp_sum(V), sEx = warp_sum(Ex), sEy = warp_sum(Ey), sEz = warp_sum(Ez);
+        if (lane == 0) {
+            double *r = red + warp * 4;
+            r[0] = sV; r[1] = sEx; r[2] = sEy; r[3] = sEz;
+        }
+        __syncthreads();
+        if (warp == 0) {
+            double acc = 0.0;
+            if (lane < 4) {
+                for (int w = 0; w < NW; ++w) acc += red[w * 4 + lane];
+                acc *= lane ? prm.g_scaleE : prm.g_scaleV;       // grid units -> hartree, hartree / bohr
+            }
+            server_push(slots, lane, acc, cmd);
+        }
+        __syncthreads();                                 // red is reused by the collection
+        if (leader && !server_collect(prm, sp.mail, slots, threadIdx.x, part_s, red, flag,
+                                      [] { __syncthreads(); }, cmd, t_start)) {
+            if (threadIdx.x == 0) {                      // a slot never arrived (not expected): retire everybody
+                *reinterpret_cast<volatile unsigned long long *>(&sp.dev->cmd) = SERVER_EXIT;
+                if (prm.dev_err) *reinterpret_cast<volatile int *>(prm.dev_err) = 1;
+            }
+            for (int k = 0; k < S; ++k)
+                if (pending & (1u << k)) mbar_wait(&my_full[k], (phase >> k) & 1u);
             break;
         }
     }

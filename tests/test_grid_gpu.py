@@ -187,7 +187,13 @@ def test_create_grid_ragged_shapes(torch_cuda, B, oracle_mod, n, h, P, precision
             assert np.array_equal(V, V2) and np.array_equal(E, E2)
             Vh = np.zeros(P); Eh = np.zeros((P, 3))
             B.qmmm_field_eval_host(hd, np.ascontiguousarray(pts), 1, P, Vh, Eh, precision)
-            assert np.array_equal(V, Vh) and np.array_equal(E, Eh)
+            if P == 1:
+                # one point: the grid-aware move server, which splits the work units over its warps
+                # in its own way (equal to rounding, checked against the oracle)
+                assert "move_server_grid_kernel" in B.qmmm_field_get_info(hd)["last_kernel"]
+                check(ref, Vh, Eh, tol)
+            else:
+                assert np.array_equal(V, Vh) and np.array_equal(E, Eh)
         finally:
             B.qmmm_field_destroy(hd)
     finally:

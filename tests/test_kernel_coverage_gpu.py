@@ -21,7 +21,8 @@ from parity_check import check
 pytestmark = pytest.mark.gpu
 
 TOL = {"fp64": 1e-12, "fp32": 1e-5}
-FAMILIES = ("pair_kernel", "pair_kernel_f32x2", "grid_kernel_f32x2", "grid_kernel_f64", "move_server_kernel")
+FAMILIES = ("pair_kernel", "pair_kernel_f32x2", "grid_kernel_f32x2", "grid_kernel_f64", "move_server_kernel",
+            "move_server_grid_kernel")
 
 
 def exported_kernels(lib_path):
@@ -107,15 +108,19 @@ def test_every_kernel_instantiation_runs_and_agrees_with_the_oracle(oracle_mod):
                                         continue        # the list kernels have no overlap / FULL variants
                                     evaluate(h, base[:n], Sub(ref_all, n), layout, prec, plan, overlap, want_E,
                                              f"cfg1 {layout} {prec} n={n} ppt={ppt} pw={pw} ov={overlap} E={want_E}")
-        # the move servers (single-point host calls on the source list)
-        for prec in ("fp64", "fp32"):
-            B.qmmm_field_set_layout(h, "auto")
-            B.qmmm_field_set_plan(h)
-            v = np.zeros(1); e = np.zeros((1, 3))
-            B.qmmm_field_eval_host(h, np.ascontiguousarray(base[:1]), 1, 1, v, e, prec)
-            name = B.qmmm_field_get_info(h)["last_kernel"]
-            check(Sub(ref_all, 1), v, e, TOL[prec])
-            seen.setdefault(name, f"move server {prec}")
+        # the move servers (single-point host calls): grid-aware on this handle, source list when forced
+        for layout in ("auto", "list"):
+            for prec in ("fp64", "fp32"):
+                B.qmmm_field_set_layout(h, layout)
+                B.qmmm_field_set_plan(h)
+                for i in range(3):
+                    v = np.zeros(1); e = np.zeros((1, 3))
+                    B.qmmm_field_eval_host(h, np.ascontiguousarray(base[i:i + 1]), 1, 1, v, e, prec)
+                    name = B.qmmm_field_get_info(h)["last_kernel"]
+                    sub = Sub(ref_all, i + 1)
+                    sub.V, sub.E, sub.absV, sub.absE = sub.V[i:], sub.E[i:], sub.absV[i:], sub.absE[i:]
+                    check(sub, v, e, TOL[prec])
+                seen.setdefault(name, f"move server {layout} {prec}")
     finally:
         B.qmmm_field_destroy(h)
 

@@ -356,6 +356,51 @@ def test_repeatability_stress_all_kernel_variants(torch_cuda, B):
         B.qmmm_field_destroy(h)
 
 
+@pytest.mark.parametrize("handle_kind", ["list+grid", "create_grid"])
+def test_grid_aware_move_server(torch_cuda, B, oracle_mod, handle_kind):
+    """Single-point eval_host calls on an environment with the grid-aware copy are served by the
+    grid-aware resident server (charges only; every warp keeps its own work units in shared
+    memory): 60 moves of config 2's random walk per precision against the oracle, across idle
+    retirement, precision switches and a device-path call; handles made by qmmm_field_create
+    (list detected as a grid) and by qmmm_field_create_grid (no list at all)."""
+    import time
+    w = make_workload(2, n_points=(60, 1))
+    pts = np.ascontiguousarray(w.elec_xyz.reshape(-1, 3))
+    ref = oracle_of(oracle_mod, w, pts)
+    if handle_kind == "create_grid":
+        n, hh = 128, 0.25
+        origin = -0.5 * hh * (n - 1) * np.ones(3)
+        dense = np.zeros((n, n, n))
+        idx = np.rint((w.src_xyz - origin) / hh).astype(np.int64)
+        dense[idx[:, 0], idx[:, 1], idx[:, 2]] = w.src_q
+        h = B.qmmm_field_create_grid(origin, hh, (n, n, n), dense, w.nuc_xyz, w.nuc_Z, 4)
+    else:
+        h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 4)
+    try:
+        for prec, tol in (("fp32", TOL32), ("fp64", TOL64), ("fp32", TOL32)):
+            V = np.full(len(pts), np.nan); E = np.full((len(pts), 3), np.nan)
+            for i in range(len(pts)):
+                v = np.zeros(1); e = np.zeros((1, 3))
+                B.qmmm_field_eval_host(h, pts[i:i + 1], 1, 1, v, e, prec)
+                V[i] = v[0]; E[i] = e[0]
+                if i == 0:
+                    assert "move_server_grid_kernel" in B.qmmm_field_get_info(h)["last_kernel"]
+                if i == 20:
+                    time.sleep(0.02)                     # the server retires after 2 ms idle
+                if i == 40:                              # a device-path call in between retires it too
+                    Vd, _ = gpu_eval(torch_cuda, B, w, pts[:3], prec, handle=h)
+                    assert np.all(np.isfinite(Vd))
+            check(ref, V, E, tol)
+            # twice the same move: bitwise the same answer (deterministic)
+            v1 = np.zeros(1); e1 = np.zeros((1, 3)); v2 = np.zeros(1); e2 = np.zeros((1, 3))
+            B.qmmm_field_eval_host(h, pts[7:8], 1, 1, v1, e1, prec)
+            B.qmmm_field_eval_host(h, pts[7:8], 1, 1, v2, e2, prec)
+            assert np.array_equal(v1, v2) and np.array_equal(e1, e2) and v1[0] == V[7]
+        assert B.qmmm_field_get_info(h)["device_errors"] == 0
+    finally:
+        B.qmmm_field_destroy(h)
+
+
 def test_move_server_bitwise_equals_launch_path_and_survives_idle_and_switches(torch_cuda, B):
     """Single-point eval_host calls are served by the resident move server (one cooperative
     launch, pinned mailbox).  Its results must be bitwise those of the launch path (same
@@ -372,7 +417,7 @@ def test_move_server_bitwise_equals_launch_path_and_survives_idle_and_switches(t
         B.qmmm_field_set_layout(h, "list")
         for prec in ("fp64", "fp32"):
             ref[prec] = [gpu_eval(torch_cuda, B, w, pts[i:i + 1], prec, handle=h) for i in range(len(pts))]
-        B.qmmm_field_set_layout(h, "auto")
+        # (with AUTO the grid-aware server would answer: test_grid_aware_move_server)
         order = ["fp64", "fp64", "fp32", "fp64", "fp32", "fp32"] * 2
         for i, prec in enumerate(order):
             V = np.full(1, np.nan); E = np.full((1, 3), np.nan)
