@@ -428,9 +428,9 @@ cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaS
                 return launch_grid_f32<EP2, NW, false, true, true, 0, true>(prm, grid, smem, st);
         }
         if constexpr (EP2 == 2 && (NW == GRID_NW_EPT4 || NW == GRID_NW_EPT4_LIGHT)) {
+            // (the dz-table kernels work from the point's true position: no lattice to refine)
             if (prm.point_warps == NW && prm.g_dzt)
-                return prm.g_fine ? launch_grid_f32<EP2, NW, false, true, true, 1>(prm, grid, smem, st)
-                                  : launch_grid_f32<EP2, NW, false, true, true, 0>(prm, grid, smem, st);
+                return launch_grid_f32<EP2, NW, false, true, true, 0>(prm, grid, smem, st);
         }
         if (prm.point_warps == NW)
             return prm.g_fine ? launch_grid_f32<EP2, NW, false, true, false, 1>(prm, grid, smem, st)

@@ -48,10 +48,9 @@ struct GridF32Layout {
         return static_cast<size_t>(stages) * STAGE_BYTES + BAR_BYTES + ELEC_BYTES + SCRATCH_BYTES +
                ACC_BYTES;
     }
-    // dz table (DZT kernels), after everything else: [z nodes padded to whole gchunks + 1][NW][EPT],
-    // then (local lattice) a_z relative to the segment's first node and its residual: 2 x [segs][NW][EPT]
+    // dz table (DZT kernels), after everything else: [z nodes padded to whole gchunks + 1][NW][EPT]
     __host__ __device__ static constexpr size_t dzt_bytes(int segs) {
-        return static_cast<size_t>(segs * 64 + 1 + 2 * segs) * NW * EPT * sizeof(float);
+        return static_cast<size_t>(segs * 64 + 1) * NW * EPT * sizeof(float);
     }
 };
 
@@ -94,10 +93,11 @@ __device__ __forceinline__ void on_lattice(double u, int i_lo, int i_hi, float &
 // y0^2, c = a y0^2, sum c, sum c dz, T += c r^2 = 9 FMA-pipe lane operations + 1 MUFU.RSQ
 // (+ 10/16 for the two summation trees).
 //
-// TS > 0 (dz table): dz = a_z - k depends on the point and the z node only, not on the row, so
+// TS > 0 (dz table): dz = u_z - k depends on the point and the z node only, not on the row, so
 // the CTA tabulates it once in shared memory ([z node][warp][EPT] floats, TS = float2 per z
-// node) and a node's dz is ONE broadcast 128-bit load for both point pairs instead of a packed
-// add per pair: 8 FMA-pipe lane operations per pair instead of 9.
+// node; formed in FP64 from the point's true coordinate, rounded once) and a node's dz is ONE
+// broadcast 128-bit load for both point pairs instead of a packed add per pair: 8 FMA-pipe
+// lane operations per pair instead of 9.
 //
 // VONLY (potential only, Eq. 4 proper; needs the table): the table holds z2 = (u_z - k)^2, formed
 // in FP64 from the point's true coordinate and rounded once, rxy2 is formed in FP64 per (point,
@@ -426,6 +426,11 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     const int ppb = WP * EPT;
     float *dd_all = lat_s + NW * EPT * 3;
     const bool fine = FINE >= 0 ? FINE == 1 : prm.g_fine != 0;  // local lattice per gchunk (uniform)
+    // TRUEPT (the batched dz-table kernels): r^2 and the differences are those of the point's TRUE
+    // position, not of its lattice position -- see the walk below; no residual, no correction, no
+    // dependence of E on the length of the axes (FINE is moot: instantiated with FINE = 0 only)
+    constexpr bool TRUEPT = FULL && DZT && !VONLY;
+    static_assert(!(DZT && FINE == 1), "the dz-table kernels have no lattice residual to refine");
     for (int i = threadIdx.x; i < ppb * 3; i += NT) {
         int p = blockIdx.x * ppb + i / 3;
         p = p < prm.P ? p : prm.P - 1;                          // clamp: duplicates are not written
@@ -441,28 +446,14 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     __syncthreads();
     constexpr int TS = DZT ? NW * EP2 : 0;                      // float2 per z node of the table
     float *dzt = reinterpret_cast<float *>(acc + EPT * 2 * NT); // [segs * ZS + 1][NW][EPT]
-    float *azrel_t = dzt + (prm.g_segs * GRID_ZS + 1) * NW * EPT;   // local lattice: [segs][NW][EPT]
-    float *ddz_t = azrel_t + prm.g_segs * NW * EPT;                 //                [segs][NW][EPT]
-    if constexpr (DZT) {                                        // a_z - k: exact on the lattice
-        if (fine) {                                             // one lattice per (z segment, point)
-            for (int i = threadIdx.x; i < prm.g_segs * NW * EPT; i += NT) {
-                const int sg = i / (NW * EPT), pp = i - sg * (NW * EPT);
-                on_lattice(u_s[pp * 3 + 2], sg * GRID_ZS, sg * GRID_ZS + GRID_ZS - 1, azrel_t[i], ddz_t[i]);
-            }
-            __syncthreads();
-        }
+    if constexpr (DZT) {
+        // one entry per (z node, point of the CTA), formed in FP64 from the point's TRUE coordinate
+        // and rounded once: dz = u_z - k, or (potential only) z2 = (u_z - k)^2
         const int nent = (prm.g_segs * GRID_ZS + 1) * NW * EPT;
         for (int i = threadIdx.x; i < nent; i += NT) {
             const int kz = i / (NW * EPT), pp = i - kz * (NW * EPT);
-            if constexpr (VONLY) {                              // z2 = (u_z - k)^2, rounded once
-                const double dzt64 = u_s[pp * 3 + 2] - static_cast<double>(kz);
-                dzt[i] = static_cast<float>(dzt64 * dzt64);
-            } else if (fine) {
-                const int sg = min(kz / GRID_ZS, prm.g_segs - 1);
-                dzt[i] = azrel_t[sg * (NW * EPT) + pp] - static_cast<float>(kz - sg * GRID_ZS);
-            } else {
-                dzt[i] = lat_s[pp * 3 + 2] - static_cast<float>(kz);
-            }
+            const double dzt64 = u_s[pp * 3 + 2] - static_cast<double>(kz);
+            dzt[i] = static_cast<float>(VONLY ? dzt64 * dzt64 : dzt64);
         }
         __syncthreads();
     }
@@ -501,10 +492,10 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     load_lattice();
     const int n_rows = prm.g_n[0] * prm.g_n[1];
     // fine: the lattice of the nodes of ONE gchunk -- rows tile_ * 32 .. + 31, z nodes
-    // seg_ * ZS + zlo .. zhi -- computed in FP64 by the first 3 EPT (with a dz table: 2 EPT) lanes
+    // seg_ * ZS + zlo .. zhi -- computed in FP64 by the first 3 EPT lanes
     auto relattice = [&](int tile_, int seg_, int zlo, int zhi) {
         __syncwarp();
-        if (lane < (DZT ? 2 : 3) * EPT) {
+        if (lane < 3 * EPT) {
             const int comp = lane / EPT, pt = lane - comp * EPT;
             int i_lo, i_hi;
             if (comp == 2) {
@@ -636,6 +627,45 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
                 vv[e] = __fadd2_rn(vv[e], v[e]);
                 tt[e] = __fadd2_rn(tt[e], tq[e]);
             }
+        } else if constexpr (TRUEPT) {
+            // r^2 of the TRUE point without FP64 in the loop: dx = a_x - ix is exact on the lattice
+            // and u_x = a_x + dd_x, so (u_x - ix)^2 = dx^2 + 2 dx dd_x (+ dd_x^2 ~ 1e-11 dx^2); the
+            // cross terms join rxy2 before it is rounded.  dz of the true point comes from the
+            // table (rounded once).  No residual is left: nothing to correct V with afterwards, and E is
+            // formed from the true differences (dx + dd_x, rounded) whatever the length of the axes.
+            const float2 fx = bc(static_cast<float>(ix)), fy = bc(static_cast<float>(iy));
+            float2 dx[EP2], dy[EP2], rxy2[EP2], v[EP2], tq[EP2];
+#pragma unroll
+            for (int e = 0; e < EP2; ++e) {
+                dx[e] = __fadd2_rn(ax[e], f2(-fx.x, -fx.y));          // exact (lattice), node units
+                dy[e] = __fadd2_rn(ay[e], f2(-fy.x, -fy.y));
+                if (prm.g_ortho) {                                    // cells that are not cubic: hx/hz, hy/hz
+                    dx[e] = __fmul2_rn(dx[e], bc(static_cast<float>(prm.g_sx)));
+                    dy[e] = __fmul2_rn(dy[e], bc(static_cast<float>(prm.g_sy)));
+                }
+                const float2 ddx = *reinterpret_cast<const float2 *>(dd_w + 2 * e);        // units of hz
+                const float2 ddy = *reinterpret_cast<const float2 *>(dd_w + EPT + 2 * e);
+                const float2 cross = __ffma2_rn(dx[e], ddx, __fmul2_rn(dy[e], ddy));
+                rxy2[e] = __ffma2_rn(dy[e], dy[e], __ffma2_rn(dx[e], dx[e], __ffma2_rn(cross, bc(2.0f), bc(1e-30f))));
+                dx[e] = __fadd2_rn(dx[e], ddx);                       // the true differences, for the field
+                dy[e] = __fadd2_rn(dy[e], ddy);
+                v[e] = tq[e] = f2(0.0f, 0.0f);
+            }
+            GridRowF32<EP2, TS> row;
+            row.start(reinterpret_cast<const float2 *>(dzt) + (seg * GRID_ZS) * TS + wp * EP2, rxy2);
+            mbar_wait(&full[slot], phase);
+            row.run(reinterpret_cast<const float *>(smem + static_cast<size_t>(slot) * STAGE_BYTES) + 4 * lane,
+                    GRID_ZS / 4, v, tq);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[slot]);
+#pragma unroll
+            for (int e = 0; e < EP2; ++e) {
+                vv[e] = __fadd2_rn(vv[e], v[e]);
+                tt[e] = __fadd2_rn(tt[e], tq[e]);
+                ex[e] = __ffma2_rn(dx[e], row.S[e], ex[e]);
+                ey[e] = __ffma2_rn(dy[e], row.S[e], ey[e]);
+                ez[e] = __fadd2_rn(ez[e], row.SZ[e]);
+            }
         } else {
         if (fine) relattice(tile, seg, z0, z0 + ZL - 1);
         const float2 fx = bc(static_cast<float>(ix - irx)), fy = bc(static_cast<float>(iy - iry));
@@ -674,8 +704,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
                 const float2 exg = __fmul2_rn(dx[e], row.S[e]), eyg = __fmul2_rn(dy[e], row.S[e]);
                 const float2 ddx = *reinterpret_cast<const float2 *>(dd_w + 2 * e);
                 const float2 ddy = *reinterpret_cast<const float2 *>(dd_w + EPT + 2 * e);
-                const float2 ddz = DZT ? *reinterpret_cast<const float2 *>(ddz_t + seg * (NW * EPT) + wp * EPT + 2 * e)
-                                       : *reinterpret_cast<const float2 *>(dd_w + 2 * EPT + 2 * e);
+                const float2 ddz = *reinterpret_cast<const float2 *>(dd_w + 2 * EPT + 2 * e);
                 vv[e] = __fadd2_rn(vv[e], v[e]);
                 tt[e] = __fadd2_rn(tt[e], tq[e]);
                 ex[e] = __fadd2_rn(ex[e], exg);
@@ -720,7 +749,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     // whole-grid lattice: the cells were seen from ONE lattice point a = u - dd: V(u) = V(a) - E(a) . dd,
     // applied to this thread's FP64 sums (before the nuclei, which are evaluated at u itself); the
     // local lattice has applied its corrections gchunk by gchunk (cc)
-    if (!fine && !VONLY)
+    if (!fine && !VONLY && !TRUEPT)
 #pragma unroll
     for (int e = 0; e < EP2; ++e) {
         const float *d0 = dd_all + (wp * EPT + 2 * e) * 3;
