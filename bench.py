@@ -547,13 +547,15 @@ def run_ours(args):
         achieved = P * w.M * slots * 2 / pair_s / 1e12
         peak_tf = 2 * peak_lane / 1e12
         # DRAM bytes per pair-kernel launch from the committed ncu capture (profiles/), if any
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "pair_kernel_traffic.csv")
-        if os.path.exists(tpath):
-            for ln in open(tpath):
-                f = ln.strip().split(",")
-                if len(f) >= 2 and f[0] == f"config{args.config}_{prec}_{layout}":
-                    traffic = float(f[1])
+        def lookup_traffic(key):
+            tpath = os.path.join(ROOT, "profiles", "pair_kernel_traffic.csv")
+            if os.path.exists(tpath):
+                for ln in open(tpath):
+                    f = ln.strip().split(",")
+                    if len(f) >= 3 and f[0] == key:
+                        return float(f[1]), f[2]
+            return None, None
+        traffic, traffic_file = lookup_traffic(f"config{args.config}_{prec}_{layout}")
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
@@ -590,8 +592,8 @@ def run_ours(args):
                          "probe_before": peaks0, "probe_after": peaks1},
         }
         if traffic is not None:
-            line["roofline"]["traffic_source"] = ("ncu --set full capture summarised in profiles/ "
-                                                  "(pair_kernel_traffic.csv); looked up, not measured in this run")
+            line["roofline"]["traffic_source"] = (f"ncu --set full capture profiles/{traffic_file}; looked up "
+                                                  "(profiles/pair_kernel_traffic.csv), not measured in this run")
         if world == 1:
             cb = oracle_sample_rate(w, args.cpu_sample_pairs)
             line["cpu_baseline"] = {
@@ -633,7 +635,8 @@ def run_ours(args):
                             "dz_table": r["dz_table"], "gpairs_per_s": r["gpairs_per_s"],
                             "frac_at_survey_slots": r["pairs_per_eval"] * 18 / (r["pair_kernel_ms_median"] * 1e-3)
                                                     / peaks1["dfma_lane_ops_per_s"],
-                            "traffic": None,
+                            "traffic": lookup_traffic(f"config4_fp64_{r['layout']}")[0],
+                            "traffic_source": "ncu --set full capture under profiles/ (pair_kernel_traffic.csv); looked up",
                             "peak_source": "measured DFMA lane rate, same process (qmmm_probe_peak)"}
         print(json.dumps(line), flush=True)
     if h is not None:
