@@ -160,9 +160,11 @@ qmmm_status qmmm_field_eval_moves_host(qmmm_field *h, const double *elec_xyz_hos
  * random walk): move s evaluates the N points elec_xyz[s][N][3] (device) into V[s][N] and
  * E[s][N][3] (device; E may be NULL).  Equivalent to n calls of qmmm_field_eval with W = 1,
  * issued from C (no per-call binding cost) and always with overlapped launches
- * (qmmm_field_set_overlap, whose precondition holds by construction here): each move is its
- * own kernel, move s + 1 starts while move s finishes.  Asynchronous on `stream`; capturable
- * into a CUDA graph.  Errors as qmmm_field_eval.
+ * (qmmm_field_set_overlap): each move is its own kernel, move s + 1 starts while move s
+ * finishes.  The FIRST move is launched with plain stream serialization, so elec_xyz may be
+ * produced by whatever precedes the call on the stream; the later moves follow this library's
+ * own kernels, which do not write elec_xyz.  Asynchronous on `stream`; capturable into a CUDA
+ * graph.  Errors as qmmm_field_eval.
  */
 qmmm_status qmmm_field_eval_moves(qmmm_field *h, const double *elec_xyz, int64_t n, int64_t N,
                                   double *V, double *E, int prec, void *stream);
@@ -335,10 +337,14 @@ qmmm_status qmmm_field_set_timing(qmmm_field *h, int enable);
  * 8-warp CTAs so that several evaluations share an SM -- the period of a sequence is a CTA's
  * lifetime divided by the CTAs an SM holds -- i.e. another association of the same sums:
  * equal to rounding, and still deterministic from run to run.
- * Precondition while enabled: elec_xyz of an evaluation is not produced by the evaluation
- * immediately before it on the same stream (it is read before the wait); work of other
- * libraries in between serialises as usual.  Ignored (plain serialization) while timing is on
- * and by the host-buffer paths.  Works inside CUDA-graph capture.
+ * Precondition while enabled: elec_xyz of an evaluation must not be written by the kernel that
+ * immediately precedes the evaluation on the stream, WHATEVER that kernel is (this library's
+ * previous evaluation, or a caller's kernel that proposes the next positions): the points are
+ * read before the wait, and CUDA gives a programmatically launched kernel no visibility of its
+ * predecessor's writes before that wait.  Put any other kernel (or an event) in between, or
+ * leave overlap off for evaluations whose points the preceding kernel produces.  Ignored (plain
+ * serialization) while timing is on and by the host-buffer paths.  Works inside CUDA-graph
+ * capture.
  */
 qmmm_status qmmm_field_set_overlap(qmmm_field *h, int enable);
 qmmm_status qmmm_field_last_timing(qmmm_field *h, double *pair_ms, double *finalize_ms);
