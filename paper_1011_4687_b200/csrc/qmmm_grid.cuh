@@ -321,12 +321,13 @@ struct GridRowF32N {
 // point groups, the WS source-split warps different z runs (ZS / WS nodes) of the same 32
 // rows.  Per gchunk a thread only forms dx, dy (exact FP32 differences on the point's
 // lattice) and adds the row's sums into FP32 accumulators, flushed to the FP64 columns in
-// shared memory every 4th gchunk.  prm.chunks = gchunks [n_chunks][ZS/4][32][4] float;
+// shared memory after every gchunk (GRID_FLUSH).  prm.chunks = gchunks [n_chunks][ZS/4][32][4] float;
 // prm.nuc = nuclei in grid units; prm.elec in bohr (converted to grid units when staged).
 #ifndef QMMM_GRID_FLUSH
-#define QMMM_GRID_FLUSH 4
+#define QMMM_GRID_FLUSH 1
 #endif
-constexpr int GRID_FLUSH = QMMM_GRID_FLUSH;                       // gchunks per FP32 -> FP64 flush
+constexpr int GRID_FLUSH = QMMM_GRID_FLUSH;                       // gchunks per FP32 -> FP64 flush (round 2: 1; 4 measured the
+                                                                  // same time on config 3 and 10 - 40 % more rounding noise in V)
 
 // NODEPACK (EP2 = 1 only): each of the thread's two points is walked on its own with two NODES
 // per register pair (GridRowF32N); a second point beyond P is skipped.  For one or two points
@@ -723,7 +724,9 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
             }
         }
         }
-        if (++pending == GRID_FLUSH) {
+        // (the potential-only kernel is bound by the XU pipe, which also does the FP32 -> FP64
+        // conversions of a flush: every 4th gchunk there, 4.30 instead of 4.40 ms on config 3)
+        if (++pending == (VONLY ? 4 : GRID_FLUSH)) {
             flush();
             pending = 0;
         }
