@@ -276,6 +276,36 @@ qmmm_status qmmm_sum_rank_partials(const double *parts, int64_t R, int64_t n, do
  */
 qmmm_status qmmm_field_set_local_lattice(qmmm_field *h, int mode);
 
+/*
+ * qmmm_field_eval_noalloc -- V and E (Eq. 4, and its field) for callers that
+ * cannot allocate: code under CUDA-graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc.  No handle (qmmm_field_create allocates): the environment is passed with every
+ * call as it is, FP64, all pointers DEVICE pointers:
+ *   src_xyz [M][3], src_q [M]   cells (charges q_j = -rho_j dV);   nuc_xyz [K][3], nuc_Z [K]  nuclei (+Z)
+ *   elec_xyz [P][3]             evaluation points, 1 <= P <= QMMM_NOALLOC_MAX_POINTS
+ *   V [P], E [P][3] (E may be NULL)   out
+ * FP64 arithmetic throughout (relative error <= 1e-12 as QMMM_FP64), deterministic, one kernel
+ * launch (plus a memset of a few hundred bytes) on `stream`, asynchronous.  The call makes NO
+ * cudaMalloc / cudaFree / allocating library call: its scratch memory -- the per-slice partial
+ * sums of Eq. 5-6 and the arrival tickets -- is a fixed file-scope __device__ array of 2 MiB +
+ * 4 KiB that every GPU loading the library holds until the process exits.  The first call on a
+ * device resolves that array's device address (cudaGetSymbolAddress, once per device); make
+ * one call outside any graph capture first.
+ * Sharing: every call of the process on a device uses the SAME array.  Calls that overlap on the
+ * GPU (different streams or host threads with two calls in flight at once) race on it and give
+ * wrong results: serialise them.  The array keeps the last call's contents; what must start at
+ * zero (the tickets) is cleared on `stream` at the start of each call.
+ * It is the plain formulation (sources read from the caller's arrays, no packed copy, no grid
+ * detection): about half the FP64 rate of the handle-based list kernels.  M = 0 and/or K = 0 are
+ * valid.  Errors: INVALID_ARG (NULL where not allowed, negative M or K, P < 1, P beyond the
+ * maximum -- the message names the limit), UNSUPPORTED_DEVICE, CUDA.
+ */
+#define QMMM_NOALLOC_MAX_POINTS 4096
+qmmm_status qmmm_field_eval_noalloc(const double *src_xyz, const double *src_q, int64_t M,
+                                    const double *nuc_xyz, const double *nuc_Z, int64_t K,
+                                    const double *elec_xyz, int64_t P, double *V, double *E,
+                                    void *stream);
+
 /* qmmm_field_destroy -- frees the handle and its device buffers.  NULL is a no-op. */
 qmmm_status qmmm_field_destroy(qmmm_field *h);
 

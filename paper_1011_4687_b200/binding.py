@@ -32,7 +32,7 @@ EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_hos
                     "qmmm_field_set_layout", "qmmm_field_get_grid_info",
                     "qmmm_field_destroy", "qmmm_field_set_plan", "qmmm_field_get_info",
                     "qmmm_field_set_timing", "qmmm_field_last_timing", "qmmm_field_set_overlap",
-                    "qmmm_field_set_local_lattice",
+                    "qmmm_field_set_local_lattice", "qmmm_field_eval_noalloc",
                     "qmmm_sum_rank_partials", "qmmm_probe_peak", "qmmm_last_error")
 
 
@@ -122,6 +122,8 @@ def _load() -> ctypes.CDLL:
     lib.qmmm_probe_peak.restype = ci
     lib.qmmm_probe_peak.argtypes = [ci, ci, ctypes.POINTER(ctypes.c_double),
                                     ctypes.POINTER(ctypes.c_double), vp]
+    lib.qmmm_field_eval_noalloc.restype = ci
+    lib.qmmm_field_eval_noalloc.argtypes = [vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, vp]
     lib.qmmm_sum_rank_partials.restype = ci
     lib.qmmm_sum_rank_partials.argtypes = [vp, i64, i64, vp, vp]
     lib.qmmm_last_error.restype = ctypes.c_char_p
@@ -250,6 +252,21 @@ def qmmm_field_eval_moves(handle: int, elec_xyz, n: int, N: int, V, E=None, prec
     issued from C.  Asynchronous on the stream."""
     _check(_lib.qmmm_field_eval_moves(handle, _ptr(elec_xyz), int(n), int(N), _ptr(V), _ptr(E),
                                       _PREC[precision], _stream(stream)))
+
+
+QMMM_NOALLOC_MAX_POINTS = 4096
+
+
+def qmmm_field_eval_noalloc(src_xyz, src_q, nuc_xyz, nuc_Z, elec_xyz, V, E=None, stream=None) -> None:
+    """V and E without a handle and without any allocation (fixed __device__ scratch array in
+    the library; include/qmmm_field.h): all arguments are DEVICE FP64 tensors, src_xyz [M,3],
+    src_q [M], nuc_xyz [K,3], nuc_Z [K] (either pair may be None), elec_xyz [P,3] with
+    P <= QMMM_NOALLOC_MAX_POINTS, V [P], E [P,3] or None.  Asynchronous on the stream."""
+    M = int(src_q.shape[0]) if src_q is not None else 0
+    K = int(nuc_Z.shape[0]) if nuc_Z is not None else 0
+    P = int(elec_xyz.shape[0])
+    _check(_lib.qmmm_field_eval_noalloc(_ptr(src_xyz), _ptr(src_q), M, _ptr(nuc_xyz), _ptr(nuc_Z), K,
+                                        _ptr(elec_xyz), P, _ptr(V), _ptr(E), _stream(stream)))
 
 
 def qmmm_sum_rank_partials(parts, out, stream=None) -> None:

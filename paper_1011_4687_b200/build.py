@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libqmmm_field.so")
-SOURCES = ["qmmm_field.cu", "qmmm_probe.cu"]
+SOURCES = ["qmmm_field.cu", "qmmm_probe.cu", "qmmm_noalloc.cu"]
 HEADERS = [os.path.join(CSRC, "qmmm_kernels.cuh"), os.path.join(CSRC, "qmmm_grid.cuh"),
            os.path.join(CSRC, "qmmm_server.cuh"),
            os.path.join(os.path.dirname(HERE), "include", "qmmm_field.h")]
