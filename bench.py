@@ -222,6 +222,22 @@ def probe_memory_and_launch(B):
     hbm, _ = B.qmmm_probe_peak(5)
     out = {"empty_launch_plus_sync_us": launch_s * 1e6, "l2_read_GBps_33MB": l2 / 1e9,
            "hbm_read_GBps_537MB": hbm / 1e9}
+    # Floor of the per-move host path (r_new in, U_ES out, every step): 1,000
+    # sequential single-point moves through the resident move server against an environment of
+    # ONE cell -- request written by the host, answer visible to the host, next to no evaluation
+    # in between: what the pinned-mailbox round trip over PCIe costs by itself.
+    one_xyz = np.array([[7.0, 0.0, 0.0]]); one_q = np.array([-0.5])
+    h1 = B.qmmm_field_create(one_xyz, one_q, None, None, 1)
+    try:
+        rng = np.random.default_rng(5)
+        walk = np.ascontiguousarray(rng.normal(size=(1000, 3)) * 0.5)
+        hV = np.zeros(1000); hE = np.zeros((1000, 3))
+        for prec in ("fp32", "fp64"):
+            B.qmmm_field_eval_moves_host(h1, walk[:50], 50, 1, hV, hE, prec)
+            secs = B.qmmm_field_eval_moves_host(h1, walk, 1000, 1, hV, hE, prec)
+            out[f"host_move_round_trip_us_one_cell_{prec}"] = secs * 1e6 / 1000
+    finally:
+        B.qmmm_field_destroy(h1)
     mp = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(mp):
         try:
@@ -377,6 +393,10 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result, mem=None):
                             row[f"frac_of_hbm_read_bw_{k}"] = row[f"source_GBps_{k}"] / mem["hbm_read_GBps_537MB"]
                         row["source_bytes_fit_l2"] = bool(bytes_eval < 100e6)
                         row["empty_launch_plus_sync_us"] = mem["empty_launch_plus_sync_us"]
+                        # the host loop against its floor (the same loop on a one-cell environment)
+                        row["us_per_eval_host_loop_floor"] = mem[f"host_move_round_trip_us_one_cell_{prec}"]
+                        row["us_per_eval_host_loop_above_floor"] = (row["us_per_eval_host_loop"]
+                                                                    - mem[f"host_move_round_trip_us_one_cell_{prec}"])
                 if not w.sequential and idx <= 1:
                     # launch-free figure for the small configurations (an evaluation is of the
                     # size of one kernel launch): 200 evaluations captured once in a CUDA graph

@@ -889,7 +889,7 @@ qmmm_status server_start(qmmm_field *h, int prec, bool *usable) {
     post_request(h->srv_mail_h, h->srv_seq, nullptr);
     ServerDevice init;
     std::memset(&init, 0, sizeof(init));
-    init.cmd = h->srv_seq;
+    for (int u = 0; u < 3; ++u) init.rec[2 * u] = h->srv_seq;       // tags of the last answered move
     {
         cudaError_t e0 = cudaMemcpy(h->srv_dev, &init, sizeof(init), cudaMemcpyHostToDevice);
         if (e0 == cudaSuccess)

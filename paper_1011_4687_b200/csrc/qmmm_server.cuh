@@ -6,9 +6,9 @@
 // resident) and then serves moves from a pinned, device-mapped mailbox:
 //
 //   host   : writes {s, r, s} into the request line; spins until the answer line carries s
-//   leader : one warp of CTA 0 polls the request line over PCIe (one transaction), copies r
-//            to device memory, publishes s in cmd
-//   all    : poll cmd (L2), run their source slice exactly like pair_kernel<REAL,1> (TMA ring,
+//   leader : one warp of CTA 0 polls the request line over PCIe (one transaction) and publishes
+//            the move as three tagged 16-byte units {s, x} {s, y} {s, z} in device memory
+//   all    : poll those units (L2), run their source slice exactly like pair_kernel<REAL,1> (TMA ring,
 //            FP64 or FP32-acc64 pair math, in-CTA reduction)
 //   all    : push their partial as one tagged record (four 16-byte units {s, value})
 //   leader : collects the records, adds them in a fixed order and stores {s, V} {s, Ex}
@@ -40,8 +40,13 @@ struct ServerMailbox {                 // pinned host memory, device-mapped
 };
 
 struct ServerDevice {                  // device memory shared by the CTAs of the server
-    double elec[3];                        // r_new of the published move
-    unsigned long long cmd;                // last published move number, or EXIT
+    // The published move: three self-validating 16-byte units {s, x} {s, y} {s, z} (s = move
+    // number, or SERVER_EXIT; x, y, z = r_new as bits), each written by the leader with ONE
+    // aligned 16-byte store and polled by the other CTAs with 16-byte loads until all three tags
+    // agree and differ from the last move -- no fence on either side (round 1 wrote r_new, fenced,
+    // then wrote the move number, and the readers fenced and loaded r_new after seeing the number:
+    // two more L2 round trips per move).
+    unsigned long long rec[8];
 };
 
 constexpr unsigned long long SERVER_EXIT = ~0ull;
@@ -154,29 +159,26 @@ __device__ __forceinline__ unsigned long long server_next_move(const ServerParam
                 break;
             }
         }
-        if (c != SERVER_EXIT && lane >= 1 && lane <= 3) {
-            const double v = __longlong_as_double(static_cast<long long>(w));
-            elec_s[lane - 1] = v;
-            sp.dev->elec[lane - 1] = v;
-            __threadfence();
+        if (lane >= 1 && lane <= 3) {                        // lanes 1..3 hold x, y, z (as bits)
+            if (c != SERVER_EXIT) elec_s[lane - 1] = __longlong_as_double(static_cast<long long>(w));
+            push_st_v2(sp.dev->rec + 2 * (lane - 1), c, c != SERVER_EXIT ? w : 0ull);
         }
         __syncwarp();
-        if (lane == 0) *reinterpret_cast<volatile unsigned long long *>(&sp.dev->cmd) = c;
     } else {
+        push_u64x2 r = {0ull, 0ull};
         for (;;) {
-            if (lane == 0) c = *reinterpret_cast<volatile unsigned long long *>(&sp.dev->cmd);
-            c = __shfl_sync(0xffffffffu, c, 0);
-            if (c != last) break;
+            if (lane < 3) r = push_ld_v2(sp.dev->rec + 2 * lane);
+            const unsigned long long t0 = __shfl_sync(0xffffffffu, r.x, 0), t1 = __shfl_sync(0xffffffffu, r.x, 1),
+                                     t2 = __shfl_sync(0xffffffffu, r.x, 2);
+            if (t0 == t1 && t1 == t2 && t0 != last) { c = t0; break; }
             const long long now = __shfl_sync(0xffffffffu, global_ns(), 0);
             if (now - t_start > SERVER_HARD_NS) {
                 c = SERVER_EXIT;
                 break;
             }
         }
-        if (c != SERVER_EXIT) {
-            __threadfence();
-            if (lane < 3) elec_s[lane] = __ldcg(&sp.dev->elec[lane]);
-        }
+        if (c != SERVER_EXIT && lane < 3) elec_s[lane] = __longlong_as_double(static_cast<long long>(r.y));
+        __syncwarp();
     }
     return c;
 }
@@ -354,7 +356,7 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) move_server_kernel(const Serve
                             [] { compute_warps_sync(); }, cmd, t_start)) {
             // a slot never arrived (not expected): retire everybody
             if (threadIdx.x == 0) {
-                *reinterpret_cast<volatile unsigned long long *>(&sp.dev->cmd) = SERVER_EXIT;
+                for (int u = 0; u < 3; ++u) push_st_v2(sp.dev->rec + 2 * u, SERVER_EXIT, 0ull);
                 *go_s = SERVER_EXIT;
             }
             compute_warps_sync();
@@ -385,7 +387,9 @@ struct ServerGridLayout {
     static constexpr int SLOTS = F32 ? 2 : 1;                       // per warp
     static constexpr int SLOT_BYTES = F32 ? GRID_NODES * 4 : GRID_NODES * 8;
     static constexpr int STAGE_BYTES = SERVER_GRID_NW * SLOTS * SLOT_BYTES;     // 128 KB
-    static constexpr int FIXED_BYTES = 16 * 8 /* barriers */ + 256 * 8 /* red / scratch */ + 8 * 8 /* r_new, cmd, flag */;
+    static constexpr int NUC_STAGED = 64;                           // nuclei of the CTA's share kept in shared memory
+    static constexpr int FIXED_BYTES = 16 * 8 /* barriers */ + 256 * 8 /* red / scratch */ + 8 * 8 /* r_new, cmd, flag */ +
+                                       NUC_STAGED * 4 * 8 /* staged nuclei */;
     __host__ __device__ static constexpr size_t total(int slices) {
         return static_cast<size_t>(STAGE_BYTES) + FIXED_BYTES + static_cast<size_t>(slices) * 4 * sizeof(double);
     }
@@ -404,7 +408,8 @@ __global__ void __launch_bounds__(32 * SERVER_GRID_NW, 1) move_server_grid_kerne
     double *elec_s = red + 256;                                                    // [3] r_new, bohr
     volatile unsigned long long *cmd_s = reinterpret_cast<volatile unsigned long long *>(elec_s + 4);
     int *flag = reinterpret_cast<int *>(elec_s + 6);
-    double *part_s = elec_s + 8;                                                   // leader: [slices][4]
+    double *nuc_s = elec_s + 8;                                                    // [NUC_STAGED][4]: this CTA's nuclei
+    double *part_s = nuc_s + L::NUC_STAGED * 4;                                    // leader: [slices][4]
     unsigned long long *slots = reinterpret_cast<unsigned long long *>(prm.partial);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -435,6 +440,12 @@ __global__ void __launch_bounds__(32 * SERVER_GRID_NW, 1) move_server_grid_kerne
     if (threadIdx.x == 0) *cmd_s = sp.start_seq;
     __syncwarp();
     for (int i = 0; i < cnt && i < S; ++i) load_into(i, i);
+    // the CTA's share of the nuclei never changes either: its first NUC_STAGED go to shared memory
+    // once (a global load and its latency less per move), any more are read from global memory
+    int klo, khi;
+    slice_range(prm.K, prm.slices, blockIdx.y, klo, khi);
+    const int kst = min(khi - klo, L::NUC_STAGED);
+    for (int i = threadIdx.x; i < kst * 4; i += NT) nuc_s[i] = prm.nuc[4 * static_cast<int64_t>(klo) + i];
     __syncthreads();
 
     unsigned long long last = sp.start_seq;
@@ -563,14 +574,11 @@ __global__ void __launch_bounds__(32 * SERVER_GRID_NW, 1) move_server_grid_kerne
             }
         }
         // nuclei of this CTA's share (units of hz), FP64, thread-strided
-        {
-            int klo, khi;
-            slice_range(prm.K, prm.slices, blockIdx.y, klo, khi);
-            for (int j = klo + threadIdx.x; j < khi; j += NT) {
-                const double2 a = *reinterpret_cast<const double2 *>(prm.nuc + 4 * static_cast<int64_t>(j));
-                const double2 b2 = *reinterpret_cast<const double2 *>(prm.nuc + 4 * static_cast<int64_t>(j) + 2);
-                pair_f64(uh[0], uh[1], uh[2], a.x, a.y, b2.x, b2.y, V, Ex, Ey, Ez);
-            }
+        for (int j = threadIdx.x; j < khi - klo; j += NT) {
+            const double *nu = j < kst ? nuc_s + 4 * j : prm.nuc + 4 * static_cast<int64_t>(klo + j);
+            const double2 a = *reinterpret_cast<const double2 *>(nu);
+            const double2 b2 = *reinterpret_cast<const double2 *>(nu + 2);
+            pair_f64(uh[0], uh[1], uh[2], a.x, a.y, b2.x, b2.y, V, Ex, Ey, Ez);
         }
         const double sV = warp_sum(V), sEx = warp_sum(Ex), sEy = warp_sum(Ey), sEz = warp_sum(Ez);
         if (lane == 0) {
@@ -590,7 +598,7 @@ __global__ void __launch_bounds__(32 * SERVER_GRID_NW, 1) move_server_grid_kerne
         if (leader && !server_collect(prm, sp.mail, slots, threadIdx.x, part_s, red, flag,
                                       [] { __syncthreads(); }, cmd, t_start)) {
             if (threadIdx.x == 0) {                      // a slot never arrived (not expected): retire everybody
-                *reinterpret_cast<volatile unsigned long long *>(&sp.dev->cmd) = SERVER_EXIT;
+                for (int u = 0; u < 3; ++u) push_st_v2(sp.dev->rec + 2 * u, SERVER_EXIT, 0ull);
                 if (prm.dev_err) *reinterpret_cast<volatile int *>(prm.dev_err) = 1;
             }
             for (int k = 0; k < S; ++k)
