@@ -381,6 +381,9 @@ __global__ void __launch_bounds__(CTA_THREADS, 1) move_server_kernel(const Serve
 // 148 CTAs x 8 warps: at most one each) loads it ONCE when the server starts and serves every
 // move from shared memory -- no source traffic at all per move; larger shares stream, with the
 // first gchunks of the next move prefetched while the CTA waits for it.
+// (Measured and rejected in round 2: 16 warps with half a gchunk -- 32 z nodes -- each.  The walk
+// halves, but 512-thread barriers, the 16-warp reduction and the barrier around the 256-thread
+// collection cost more: 6.52 / 7.14 us per move on configs[2] against 6.05 / 6.83 us.)
 constexpr int SERVER_GRID_NW = 8;
 template <bool F32>
 struct ServerGridLayout {
