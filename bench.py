@@ -46,7 +46,9 @@ UNIT = "Gpair/s"
 # node only; qmmm_field_info.last_dz_table says whether the last launch did) load it instead of
 # stepping it: one operation less, 8 (FP32) / 12 (FP64).
 SLOTS = {("list", "fp32"): 14, ("list", "fp64"): 18, ("grid", "fp32"): 9, ("grid", "fp64"): 13}
-SLOTS_V_ONLY = {"list": 13, "grid": 8}     # FP64 potential only (E = NULL)
+# FP64 potential only (E = NULL).  List: 3 sub, 3 for r^2, 5 for the refinement, fma(q, y, V) = 12
+# (round 1 printed 13; the SASS count of tests/test_sass_slots.py says 12).
+SLOTS_V_ONLY = {"list": 12, "grid": 8}
 SLOTS_V_ONLY_F32_GRID = 6                  # FP32 potential only, batched grid kernel: r^2, a, V0, y0^2, c, T
 
 
@@ -460,8 +462,8 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result, mem=None):
                                 "xu_pipe_frac": pairs / (np.median(step_ms) * 1e-3) / peaks["mufu_lane_ops_per_s"],
                                 "kernel_symbol": info.get("last_kernel", ""), "plan": info["last_plan"]})
                 if prec == "fp64" and not w.sequential and idx in (1, 4):
-                    # potential only (E = NULL): the paper's own computation, Eq. 4; 13 (list) or
-                    # 8 (grid) DP slots
+                    # potential only (E = NULL): the paper's own computation, Eq. 4; 12 (list) or
+                    # 8 (grid; 7 with the dz table) DP slots
                     B.qmmm_field_set_timing(h, True)
                     step_ms, pair_ms, _ = time_steps(torch, B, h, batches, W, N, prec, reps, 3, flush,
                                                      stream, want_E=False)
