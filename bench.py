@@ -74,6 +74,8 @@ def parse_args():
                     help="source copy the kernels read: list of positions, or the grid-aware "
                          "compact format (auto: grid when the cells are grid nodes and the "
                          "batch has many points)")
+    ap.add_argument("--potential-only", action="store_true",
+                    help="E = NULL: the potential alone (PAPER.md Eq. 4 proper); fewer operations per pair")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-sweep", action="store_true",
                     help="skip the per-config table (all five configs) at N=1")
@@ -531,7 +533,7 @@ def run_ours(args):
     barrier()
     sampler.start()
     step_ms, pair_ms, _ = time_steps(torch, B, h, batches, W, N, prec, args.steps, args.warmup,
-                                     flush, stream)
+                                     flush, stream, want_E=not args.potential_only)
     barrier()
     clocks = sampler.stop()
     peaks1 = probe_peaks(B)
@@ -548,7 +550,7 @@ def run_ours(args):
     B.qmmm_field_set_timing(h, False)
     pin_in = [torch.from_numpy(b.copy()).pin_memory() for b in host_batches]
     pin_out = torch.zeros(P * 4, dtype=torch.float64).pin_memory()
-    hV, hE = pin_out[:P], pin_out[P:].reshape(P, 3)
+    hV, hE = pin_out[:P], (None if args.potential_only else pin_out[P:].reshape(P, 3))
     for i in range(args.warmup):
         B.qmmm_field_eval_host(h, pin_in[i % n_batches], W, N, hV, hE, prec, stream)
     barrier()
@@ -565,7 +567,13 @@ def run_ours(args):
         peak_key = "ffma_lane_ops_per_s" if prec == "fp32" else "dfma_lane_ops_per_s"
         peak_lane = 0.5 * (peaks0[peak_key] + peaks1[peak_key])
         pair_s = float(np.mean(pair_ms)) * 1e-3
-        slots = slots_for(layout, prec, info)
+        if args.potential_only and prec == "fp32":
+            # only the batched grid kernel has an FP32 potential-only variant (its symbol ends in
+            # ...ELb1EEEv...); every other FP32 path runs its V + E kernel with E = NULL
+            v_kernel = "ELb1EEEvNS_10PairParamsE" in info.get("last_kernel", "") and "grid_kernel_f32x2" in info.get("last_kernel", "")
+            slots = SLOTS_V_ONLY_F32_GRID if v_kernel else slots_for(layout, prec, info)
+        else:
+            slots = slots_for(layout, prec, info, v_only=args.potential_only)
         achieved = P * w.M * slots * 2 / pair_s / 1e12
         peak_tf = 2 * peak_lane / 1e12
         # DRAM bytes per pair-kernel launch from the committed ncu capture (profiles/), if any
@@ -587,12 +595,12 @@ def run_ours(args):
                        "M_nominal": w.M_nominal, "K": w.K, "W": W, "N": N,
                        "pairs_per_step_per_gpu": pairs_step_rank,
                        "parallelism": f"walkers sharded x{world}, sources replicated, no collective",
-                       "layout": layout,
+                       "layout": layout, "outputs": "V only (E = NULL)" if args.potential_only else "V and E",
                        "l2": "flushed between timed steps (256 MB write)", "plan": info["last_plan"],
                        "point_blocks": info["last_point_blocks"]},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": P * 24,
-                    "d2h_bytes_per_step": P * 32},
+                    "d2h_bytes_per_step": P * (8 if args.potential_only else 32)},
             "gpu_launches": info["last_launches"] * args.steps,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
                          "frac": achieved / peak_tf, "traffic": traffic,
