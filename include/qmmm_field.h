@@ -296,7 +296,9 @@ qmmm_status qmmm_field_set_local_lattice(qmmm_field *h, int mode);
  * wrong results: serialise them.  The array keeps the last call's contents; what must start at
  * zero (the tickets) is cleared on `stream` at the start of each call.
  * It is the plain formulation (sources read from the caller's arrays, no packed copy, no grid
- * detection): about half the FP64 rate of the handle-based list kernels.  M = 0 and/or K = 0 are
+ * detection): about half the FP64 rate of the handle-based list kernels (measured on B200, 4,096
+ * points x 1.04 M cells: 0.40 against 0.86 T pair interactions per second; 1.20 T with the grid
+ * kernels).  M = 0 and/or K = 0 are
  * valid.  Errors: INVALID_ARG (NULL where not allowed, negative M or K, P < 1, P beyond the
  * maximum -- the message names the limit), UNSUPPORTED_DEVICE, CUDA.
  */
