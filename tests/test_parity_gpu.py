@@ -356,6 +356,37 @@ def test_repeatability_stress_all_kernel_variants(torch_cuda, B):
         B.qmmm_field_destroy(h)
 
 
+def test_config2_all_1000_moves_host_loop_and_device_sequence(torch_cuda, B, oracle_mod):
+    """configs[2] as BASELINE.json states it -- 1,000 sequential single-electron evaluations --
+    in the two launch configurations bench.py times: the host loop (qmmm_field_eval_moves_host:
+    resident grid-aware move server) and the device-resident sequence (qmmm_field_eval_moves:
+    overlapped launches).  EVERY move against the oracle, both precisions."""
+    torch = torch_cuda
+    w = make_workload(2)
+    pts = np.ascontiguousarray(w.elec_xyz.reshape(-1, 3))
+    assert len(pts) == 1000
+    ref = oracle_of(oracle_mod, w, pts)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 1)
+    try:
+        d = torch.from_numpy(pts).cuda()
+        for prec, tol in (("fp32", TOL32), ("fp64", TOL64)):
+            V = np.full(1000, np.nan); E = np.full((1000, 3), np.nan)
+            B.qmmm_field_eval_moves_host(h, pts, 1000, 1, V, E, prec)
+            assert "move_server_grid_kernel" in B.qmmm_field_get_info(h)["last_kernel"]
+            check(ref, V, E, tol)
+            Vd = torch.full((1000,), float("nan"), dtype=torch.float64, device="cuda")
+            Ed = torch.full((1000, 3), float("nan"), dtype=torch.float64, device="cuda")
+            B.qmmm_field_eval_moves(h, d, 1000, 1, Vd, Ed, prec)
+            torch.cuda.synchronize()
+            check(ref, Vd.cpu().numpy(), Ed.cpu().numpy(), tol)
+            dU = abs(V.sum() - ref.V.sum())
+            print(f"config2 {prec}: sum over the 1,000-move walk deviates by {dU:.3e} hartree "
+                  f"(max per move {np.abs(V - ref.V).max():.3e})")
+        assert B.qmmm_field_get_info(h)["device_errors"] == 0
+    finally:
+        B.qmmm_field_destroy(h)
+
+
 @pytest.mark.parametrize("handle_kind", ["list+grid", "create_grid"])
 def test_grid_aware_move_server(torch_cuda, B, oracle_mod, handle_kind):
     """Single-point eval_host calls on an environment with the grid-aware copy are served by the
