@@ -128,9 +128,10 @@ qmmm_status qmmm_field_eval_energy(qmmm_field *h, const double *elec_xyz, int64_
  *   W*N <= 64 : one kernel launch on `stream`, no copies and no stream synchronisation: up to
  *               32 points travel as kernel parameters (more are read by the kernel from a
  *               pinned, device-mapped mailbox), and the results come back as one tagged
- *               record {tag, V, E, tag} per point written by the kernel straight into pinned
- *               host memory, which the call polls (or, for launch shapes the record
- *               collection does not cover, as V, E followed by a sequence number).
+ *               record per point -- four self-validating 16-byte units {tag, V} {tag, Ex}
+ *               {tag, Ey} {tag, Ez} -- written by the kernel straight into pinned host memory,
+ *               which the call polls (or, for launch shapes the record collection does not
+ *               cover, as V, E followed by a sequence number).
  *   otherwise : host->device copy, kernel, device->host copy on `stream`, synchronisation.
  * The launch paths and the source-list server give bitwise the result of qmmm_field_eval with
  * the same plan and layout; the grid-aware server splits the work units over its warps in its
