@@ -269,11 +269,11 @@ qmmm_status qmmm_sum_rank_partials(const double *parts, int64_t R, int64_t n, do
  * (measured on configs[3]: 5.68 instead of 5.27 ms).  mode -1 (default): per work unit when an
  * axis has more than 128 nodes; 0: never; 1: always.  The source-list FP32 kernels always use a
  * lattice per 2,048-source block.  With it the FP32 tolerance on E holds for points at least
- * 1.2 cell edges from every charged cell (tested).  The batched kernels that tabulate dz per
- * CTA (a few dozen points and more, z axes of up to a few hundred nodes: all batched BASELINE
- * configurations) do not evaluate at a lattice position at all -- they fold the residual into
- * r^2 and into the differences -- so the setting does not concern them.  Sticky; INVALID_ARG
- * on another mode.
+ * 1.2 cell edges from every charged cell (tested).  The kernels that tabulate dz per CTA
+ * (evaluations of three points and more with the automatic plan, z axes of up to about 1,500
+ * nodes: configs[1] and all batched BASELINE configurations) do not evaluate at a lattice
+ * position at all -- they fold the residual into r^2 and into the differences -- so the
+ * setting does not concern them.  Sticky; INVALID_ARG on another mode.
  */
 qmmm_status qmmm_field_set_local_lattice(qmmm_field *h, int mode);
 

@@ -140,9 +140,9 @@ int grid_f32_warps(int ept, int64_t P, bool light) {
 #define QMMM_GRID_F32_DZT 1
 #endif
 size_t grid_dzt_bytes(bool f32, int ept, int wp, int64_t P, int64_t g_segs, bool light) {
-    if (f32) {      // 4 points per thread, every warp its own point group (the FULL kernel)
+    if (f32) {      // 4 points per thread; every warp its own point group, or z-split warps: the same table
         if (!QMMM_GRID_F32_DZT || ept != 4 || g_segs > 4096) return 0;
-        if (wp != (light ? GRID_NW_EPT4_LIGHT : GRID_NW_EPT4)) return 0;
+        (void)wp;
         return light ? GridF32Layout<2, GRID_NW_EPT4_LIGHT>::dzt_bytes(static_cast<int>(g_segs))
                      : GridF32Layout<2, GRID_NW_EPT4>::dzt_bytes(static_cast<int>(g_segs));
     }
@@ -435,6 +435,10 @@ cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaS
         if (prm.point_warps == NW)
             return prm.g_fine ? launch_grid_f32<EP2, NW, false, true, false, 1>(prm, grid, smem, st)
                               : launch_grid_f32<EP2, NW, false, true, false, 0>(prm, grid, smem, st);
+        if constexpr (EP2 == 2 && !DZT && (NW == GRID_NW_EPT4 || NW == GRID_NW_EPT4_LIGHT)) {
+            // few-point plans (z-split warps): the same table and true-point walk
+            if (prm.g_dzt) return launch_grid_f32<EP2, NW, false, false, true>(prm, grid, smem, st);
+        }
     }
     auto kern = grid_kernel_f32x2<EP2, NW, NODEPACK, FULL, DZT, FINE, VONLY>;
     static SmemConfig configured;

@@ -345,7 +345,7 @@ template <int EP2, int NW, bool NODEPACK = false, bool FULL = false, bool DZT = 
 __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 16 / NW : 1) grid_kernel_f32x2(const PairParams prm) {
     static_assert(FINE == -1 || FULL, "the compile-time switch is for the batched FULL kernels");
     static_assert(!VONLY || (FULL && DZT && FINE == 0), "potential only: batched table-driven walk, no lattice");
-    static_assert(!DZT || (FULL && !NODEPACK), "dz table: every warp walks whole gchunks of its own points");
+    static_assert(!DZT || !NODEPACK, "dz table: the point-packed walks (every warp its own points, or z-split warps)");
     static_assert(!NODEPACK || EP2 == 1, "node packing walks single points");
     static_assert(!(NODEPACK && FULL), "FULL is a mode of the point-packed walk");
     using L = GridF32Layout<EP2, NW>;
@@ -430,7 +430,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
     // TRUEPT (the batched dz-table kernels): r^2 and the differences are those of the point's TRUE
     // position, not of its lattice position -- see the walk below; no residual, no correction, no
     // dependence of E on the length of the axes (FINE is moot: instantiated with FINE = 0 only)
-    constexpr bool TRUEPT = FULL && DZT && !VONLY;
+    constexpr bool TRUEPT = DZT && !VONLY;
     static_assert(!(DZT && FINE == 1), "the dz-table kernels have no lattice residual to refine");
     for (int i = threadIdx.x; i < ppb * 3; i += NT) {
         int p = blockIdx.x * ppb + i / 3;
@@ -453,6 +453,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
         const int nent = (prm.g_segs * GRID_ZS + 1) * NW * EPT;
         for (int i = threadIdx.x; i < nent; i += NT) {
             const int kz = i / (NW * EPT), pp = i - kz * (NW * EPT);
+            if (pp >= ppb) continue;                            // (z-split plans stage fewer than NW point groups)
             const double dzt64 = u_s[pp * 3 + 2] - static_cast<double>(kz);
             dzt[i] = static_cast<float>(VONLY ? dzt64 * dzt64 : dzt64);
         }
@@ -653,10 +654,14 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
                 v[e] = tq[e] = f2(0.0f, 0.0f);
             }
             GridRowF32<EP2, TS> row;
-            row.start(reinterpret_cast<const float2 *>(dzt) + (seg * GRID_ZS) * TS + wp * EP2, rxy2);
+            // (z-split warps start at their own z run z0 of the gchunk; FULL: z0 = 0, ZL = 64)
+            row.start(reinterpret_cast<const float2 *>(dzt) + (seg * GRID_ZS + z0) * TS + wp * EP2, rxy2);
             mbar_wait(&full[slot], phase);
-            row.run(reinterpret_cast<const float *>(smem + static_cast<size_t>(slot) * STAGE_BYTES) + 4 * lane,
-                    GRID_ZS / 4, v, tq);
+            const float *data = reinterpret_cast<const float *>(smem + static_cast<size_t>(slot) * STAGE_BYTES);
+            if constexpr (FULL)
+                row.run(data + 4 * lane, GRID_ZS / 4, v, tq);
+            else
+                row.run(data + (z0 / 4) * 128 + 4 * lane, ZL / 4, v, tq);
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[slot]);
 #pragma unroll

@@ -527,11 +527,12 @@ def test_eval_is_cuda_graph_capturable(torch_cuda, B, layout, precision):
 @pytest.mark.parametrize("nz,P,precision,tol,table", [
     (64, 128, "fp32", TOL32, True), (130, 128, "fp32", TOL32, True), (400, 128, "fp32", TOL32, False),
     (64, 128, "fp64", TOL64, True), (300, 128, "fp64", TOL64, True), (600, 128, "fp64", TOL64, False),
-    (64, 8, "fp32", TOL32, False), (64, 3, "fp64", TOL64, False)])
+    (64, 8, "fp32", TOL32, True), (1700, 8, "fp32", TOL32, False), (64, 3, "fp64", TOL64, False)])
 def test_dz_table_and_stepped_dz_kernels(torch_cuda, B, oracle_mod, nz, P, precision, tol, table):
-    """The batched grid kernels tabulate dz = u_z - k per CTA in shared memory when the table
-    fits (qmmm_field_info.last_dz_table) and step it per pair otherwise (long z axes; few-point
-    plans): both against the oracle, on z extents with ragged last gchunks."""
+    """The grid kernels tabulate dz = u_z - k per CTA in shared memory when the table fits
+    (qmmm_field_info.last_dz_table; FP32: batched and few-point plans alike, FP64: the batched
+    plan) and step it per pair otherwise (long z axes; the FP64 few-point walks): both against
+    the oracle, on z extents with ragged last gchunks."""
     n = (9, 8, nz)
     h = 0.25
     rng = np.random.default_rng(1000 + nz + P)

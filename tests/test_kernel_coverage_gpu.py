@@ -139,7 +139,7 @@ def test_every_kernel_instantiation_runs_and_agrees_with_the_oracle(oracle_mod):
                         for local in ((-1, 0) if prec == "fp32" else (-1,)):
                             B.qmmm_field_set_local_lattice(h, local)
                             for n in (24, P0):
-                                for ppt, pw in ((4, 0), (4, 8), (4, 4), (2, 16), (8, 8)):
+                                for ppt, pw in ((4, 0), (4, 8), (4, 4), (4, 1), (2, 16), (8, 8)):
                                     if ppt == 8 and prec == "fp64":
                                         continue
                                     if local == 0 and prec == "fp32" and want_E:
