@@ -159,3 +159,29 @@ def test_host_threads_with_shared_handles_single_point_calls(torch_cuda, B, orac
         for hd in handles[1:]:
             B.qmmm_field_destroy(hd)
         B.qmmm_field_destroy(parent)
+
+
+@pytest.mark.parametrize("layout", ["auto", "list"])
+def test_move_server_relay_soak_bitwise_repeatable(torch_cuda, B, layout):
+    """The resident servers relay every move to their 148 CTAs as three tagged 16-byte units and
+    collect 148 tagged records, without fences (qmmm_server.cuh).  A stale or torn unit would
+    evaluate a move at a mixed or previous position: 30 repetitions of configs[2]'s 1,000-move
+    walk per precision (60,000 moves per server kind) must reproduce the first pass bit for bit
+    (the first pass itself is checked against the oracle in tests/test_parity_gpu.py)."""
+    w = make_workload(2)
+    pts = np.ascontiguousarray(w.elec_xyz.reshape(-1, 3))
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 1)
+    try:
+        B.qmmm_field_set_layout(h, layout)
+        for precision in ("fp32", "fp64"):
+            V0 = np.zeros(len(pts)); E0 = np.zeros((len(pts), 3))
+            B.qmmm_field_eval_moves_host(h, pts, len(pts), 1, V0, E0, precision)
+            want = "move_server_grid_kernel" if layout == "auto" else "move_server_kernel"
+            assert want in B.qmmm_field_get_info(h)["last_kernel"]
+            for rep in range(30):
+                V = np.full(len(pts), np.nan); E = np.full((len(pts), 3), np.nan)
+                B.qmmm_field_eval_moves_host(h, pts, len(pts), 1, V, E, precision)
+                assert np.array_equal(V, V0) and np.array_equal(E, E0), (layout, precision, rep)
+        assert B.qmmm_field_get_info(h)["device_errors"] == 0
+    finally:
+        B.qmmm_field_destroy(h)
