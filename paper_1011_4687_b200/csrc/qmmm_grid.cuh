@@ -75,6 +75,18 @@ __device__ __forceinline__ void on_lattice(double u, int i_lo, int i_hi, float &
     dd = static_cast<float>(u - al);
 }
 
+// v += x with the rounding error of the sum kept (fast two-sum: exact when v's exponent is not
+// below x's, which holds from the second partial sum on; else the error term is itself rounded),
+// and d += dx - 2 error: V = v - d / 2 then holds the exact sum.  4 operations more than two
+// plain adds, once per 16 nodes: a quarter operation per pair.
+__device__ __forceinline__ void add_run(float2 &v, float2 &d, float2 x, float2 dx) {
+    const float2 s = __fadd2_rn(v, x);
+    const float2 bb = __ffma2_rn(v, bc(-1.0f), s);              // s - v
+    const float2 er = __ffma2_rn(x, bc(-1.0f), bb);             // (s - v) - x = -(rounding error of s)
+    v = s;
+    d = __fadd2_rn(d, __ffma2_rn(er, bc(2.0f), dx));
+}
+
 // A run of z nodes of the lane's row for EP2 packed point pairs, software-pipelined: while
 // the FMA pipe works on node n the MUFU.RSQ of node n + 1 is already in flight (two register
 // sets A / B in turn).
@@ -196,11 +208,24 @@ struct GridRowF32 {
         acc(dzB, r2B, y0B, Q.w, Vc, Tc, false);
         if constexpr (TS > 0) tp += 4 * TS;
     }
-    // n4 * 4 nodes starting at b ([k4][32][4] floats); V0 and T are summed as trees of short
-    // FP32 runs (4 nodes -> 16 -> run): a long FP32 running sum of slowly varying same-sign
-    // terms drifts
-    __device__ __forceinline__ void run(const float *b, int n4, float2 (&v)[EP2], float2 (&t)[EP2]) {
+    // n4 * 4 nodes starting at b ([k4][32][4] floats).  v receives the row's sum of a (V0), d the
+    // sum of c r^2 - a (T - V0: the Newton term, V = V0 - d / 2).  V0 and T are summed as trees
+    // of short FP32 runs (4 nodes -> 16 -> run): a long FP32 running sum of slowly varying
+    // same-sign terms drifts; T - V0 is formed once per run (16 nodes
+    // when compensated) and is exact, the two agree to 1e-6.
+    // VONLY: the last level (16 -> run) is where the row sum reaches its full size.  It carries
+    // 60 % of the tree's rounding variance and, on config 3, a systematic +6e-10 hartree per
+    // point (partial sums 1 : 2 : 3 : 4 of nearly equal terms; reproduced by a CPU emulation
+    // of the tree in IEEE float32), so there it is added with a fast
+    // two-sum whose error term goes to d: a quarter operation per pair, +2.3 % time, rms of V
+    // on config 3 4.5e-8 -> 2.7e-8 and the batch total inside 1e-5 hartree.  The V + E kernel
+    // keeps plain adds: its error is dominated by the FP32 dz table and rxy2 (6.7e-8 -> 6.4e-8
+    // with the two-sum, at +3 % time: measured, not taken).
+    __device__ __forceinline__ void run(const float *b, int n4, float2 (&v)[EP2], float2 (&d)[EP2]) {
         if ((n4 & 3) == 0) {
+            float2 t[EP2];
+#pragma unroll
+            for (int e = 0; e < EP2; ++e) t[e] = f2(0.0f, 0.0f);
 #pragma unroll 1
             for (int g = 0; g < n4; g += 4) {
                 float2 v16[EP2], t16[EP2], Vc[EP2], Tc[EP2];
@@ -216,19 +241,27 @@ struct GridRowF32 {
                 }
 #pragma unroll
                 for (int e = 0; e < EP2; ++e) {
-                    v[e] = __fadd2_rn(v[e], v16[e]);
-                    t[e] = __fadd2_rn(t[e], t16[e]);
+                    if constexpr (VONLY) {
+                        add_run(v[e], d[e], v16[e], __ffma2_rn(v16[e], bc(-1.0f), t16[e]));
+                    } else {
+                        v[e] = __fadd2_rn(v[e], v16[e]);
+                        t[e] = __fadd2_rn(t[e], t16[e]);
+                    }
                 }
+            }
+            if constexpr (!VONLY) {
+#pragma unroll
+                for (int e = 0; e < EP2; ++e) d[e] = __fadd2_rn(d[e], __ffma2_rn(v[e], bc(-1.0f), t[e]));
             }
         } else {
 #pragma unroll 1
-            for (int k4 = 0; k4 < n4; ++k4) {
+            for (int k4 = 0; k4 < n4; ++k4) {            // short z runs of the z-split plans
                 float2 Vc[EP2], Tc[EP2];
                 four(b + k4 * 128, Vc, Tc);
 #pragma unroll
                 for (int e = 0; e < EP2; ++e) {
                     v[e] = __fadd2_rn(v[e], Vc[e]);
-                    t[e] = __fadd2_rn(t[e], Tc[e]);
+                    d[e] = __fadd2_rn(d[e], __ffma2_rn(Vc[e], bc(-1.0f), Tc[e]));
                 }
             }
         }
@@ -529,9 +562,9 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
             double2 t;
-            t = my[(4 * e + 0) * NT];            // V = (3 sum a - sum c r^2) / 2: the Newton step
-            t.x += 1.5 * static_cast<double>(vv[e].x) - 0.5 * static_cast<double>(tt[e].x) - static_cast<double>(cc[e].x);
-            t.y += 1.5 * static_cast<double>(vv[e].y) - 0.5 * static_cast<double>(tt[e].y) - static_cast<double>(cc[e].y);
+            t = my[(4 * e + 0) * NT];            // V = (3 sum a - sum c r^2) / 2, the Newton step, as V0 - (T - V0) / 2
+            t.x += static_cast<double>(vv[e].x) - 0.5 * static_cast<double>(tt[e].x) - static_cast<double>(cc[e].x);
+            t.y += static_cast<double>(vv[e].y) - 0.5 * static_cast<double>(tt[e].y) - static_cast<double>(cc[e].y);
             my[(4 * e + 0) * NT] = t;
             t = my[(4 * e + 1) * NT];
             t.x += static_cast<double>(ex[e].x);
@@ -580,7 +613,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
                 const float s1 = row.S.x + row.S.y;
                 const float exg = dxs * s1, eyg = dys * s1, ezg = row.SZ.x + row.SZ.y;
                 vvc += v1;
-                ttc += t1;
+                ttc += t1 - v1;                    // T - V0 (exact: the two agree to 1e-6)
                 exc += exg;
                 eyc += eyg;
                 ezc += ezg;
@@ -625,10 +658,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[slot]);
 #pragma unroll
-            for (int e = 0; e < EP2; ++e) {
-                vv[e] = __fadd2_rn(vv[e], v[e]);
-                tt[e] = __fadd2_rn(tt[e], tq[e]);
-            }
+            for (int e = 0; e < EP2; ++e) add_run(vv[e], tt[e], v[e], tq[e]);    // four rows per flush: compensated
         } else if constexpr (TRUEPT) {
             // r^2 of the TRUE point without FP64 in the loop: dx = a_x - ix is exact on the lattice
             // and u_x = a_x + dd_x, so (u_x - ix)^2 = dx^2 + 2 dx dd_x (+ dd_x^2 ~ 1e-11 dx^2); the
@@ -1161,33 +1191,38 @@ __global__ void grid_scatter_kernel(const double *xyz, const double *q, int64_t 
     dense[at] = q[j];
 }
 
-// Pack the dense charges into gchunks: one thread per (padded) row.  REAL = float: each
-// charge absorbs the rounding residual of the previous one along the row (running monopole
-// residual below one rounding unit).  Cells beyond the grid are 0.
+// Pack the dense charges into gchunks: one thread per (padded) row.  Cells beyond the grid are 0.
+// REAL = float: each charge absorbs the rounding residual of the previous one (running monopole
+// residual below one rounding unit); the residual runs along the row and
+// on into the next row of the same tile of 32 rows (one thread per tile: a residual dropped at
+// the end of every ROW left 16,384 of them on config 3, +1.4e-10 hartree at every point).
 template <typename REAL>
 __global__ void grid_pack_kernel(const double *dense, int64_t rows, int nz, int segs,
                                  int64_t rows_padded, double q_scale, REAL *out) {
     constexpr int PER = sizeof(REAL) == 4 ? 4 : 2;       // nodes per 128-bit load
-    const int64_t row = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x;
-    if (row >= rows_padded) return;
-    const int64_t tile = row / 32;
-    const int lane = static_cast<int>(row % 32);
+    constexpr int ROWS = sizeof(REAL) == 4 ? 32 : 1;     // rows per thread
+    const int64_t row0 = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x;
+    if (row0 >= rows_padded || row0 % ROWS != 0) return;
     double carry = 0.0;
-    for (int seg = 0; seg < segs; ++seg) {
-        REAL *o = out + (tile * segs + seg) * GRID_NODES;
-        for (int k = 0; k < GRID_ZS; ++k) {
-            const int iz = seg * GRID_ZS + k;
-            const double qd = (row < rows && iz < nz) ? dense[row * nz + iz] * q_scale : 0.0;   // 2^k: exact
-            REAL v;
-            if constexpr (sizeof(REAL) == 4) {
-                const double want = qd + carry;
-                v = static_cast<float>(want);
-                carry = qd != 0.0 ? want - static_cast<double>(v) : carry;
-                if (qd == 0.0) v = 0.0f;                 // empty cells stay exactly empty
-            } else {
-                v = qd;
+    for (int64_t row = row0; row < row0 + ROWS; ++row) {
+        const int64_t tile = row / 32;
+        const int lane = static_cast<int>(row % 32);
+        for (int seg = 0; seg < segs; ++seg) {
+            REAL *o = out + (tile * segs + seg) * GRID_NODES;
+            for (int k = 0; k < GRID_ZS; ++k) {
+                const int iz = seg * GRID_ZS + k;
+                const double qd = (row < rows && iz < nz) ? dense[row * nz + iz] * q_scale : 0.0;   // 2^k: exact
+                REAL v;
+                if constexpr (sizeof(REAL) == 4) {
+                    const double want = qd + carry;
+                    v = static_cast<float>(want);
+                    carry = qd != 0.0 ? want - static_cast<double>(v) : carry;
+                    if (qd == 0.0) v = 0.0f;                 // empty cells stay exactly empty
+                } else {
+                    v = qd;
+                }
+                o[(k / PER) * 32 * PER + lane * PER + (k % PER)] = v;
             }
-            o[(k / PER) * 32 * PER + lane * PER + (k % PER)] = v;
         }
     }
 }

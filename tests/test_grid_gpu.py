@@ -326,6 +326,15 @@ def test_config3_grid_fp32_full_energy(torch_cuda, B, oracle_mod, full_oracle):
         assert per_walker.max() <= E_TOL
         assert batch / w.W <= E_TOL
         assert batch <= 1e-4
+        if name == "grid potential-only":
+            # the energy path (Eq. 4 needs V only; qmmm_field_eval_energy runs this kernel): the
+            # north star's criterion taken literally -- the sum over all 16,384 points within
+            # 1e-5 hartree of the oracle's, 4e-12 of the 2.5e6 hartree it adds up
+            assert batch <= E_TOL, batch
+    # and through the entry point that returns energies: sum over walkers of U[w]
+    batch_U = abs(U.sum() + full.V.sum())
+    print(f"config3 fp32 eval_energy: whole batch |dU| = {batch_U:.3e} hartree")
+    assert batch_U <= E_TOL
     for name, e in (("grid", E), ("list", El)):
         eE = np.linalg.norm(e - full.E, axis=1) / np.linalg.norm(full.E, axis=1)
         kE = full.absE / np.linalg.norm(full.E, axis=1)

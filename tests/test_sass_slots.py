@@ -5,7 +5,7 @@ holds the reciprocal-square-root seeds (MUFU.RSQ / MUFU.RSQ64H: exactly one per 
 the arithmetic-pipe lane operations in it are counted per seed: packed FFMA2 / FMUL2 / FADD2 count
 two (two points per instruction), scalar FP32 and every DP instruction one.  The count must equal
 the table's figure, plus at most the summation-tree adds of the FP32 kernels (a quarter operation
-per pair); a kernel that silently did more -- or less -- work per pair than the roofline assumes
+per pair; half of one in the potential-only kernel, whose last tree level is compensated); a kernel that silently did more -- or less -- work per pair than the roofline assumes
 would fail here.
 """
 import os
@@ -75,8 +75,11 @@ def test_lane_operations_per_pair_match_the_roofline_table(sym, layout, prec, v_
         lane_ops = 2 * sum(ops.count(k) for k in PACKED) + sum(ops.count(k) for k in SCALAR)
         assert sum(ops.count(k) for k in DP) == 0, "FP64 arithmetic inside the FP32 hot loop"
         per_pair = lane_ops / seeds
-        # one seed per pair; the V0 / T summation trees add at most a quarter operation per pair
-        assert claimed <= per_pair <= claimed + 0.25 + 1e-9, (sym, per_pair, claimed)
+        # one seed per pair; the V0 / T summation trees add at most a quarter operation per pair,
+        # the compensated last tree level of the potential-only kernel (fast two-sum, once per 16
+        # nodes) another quarter
+        extra = 0.5 if v_only else 0.25
+        assert claimed <= per_pair <= claimed + extra + 1e-9, (sym, per_pair, claimed)
     else:
         per_pair = sum(ops.count(k) for k in DP) / seeds
         assert per_pair == pytest.approx(claimed, abs=1e-9), (sym, per_pair, claimed)
