@@ -463,6 +463,22 @@ def sweep_all_configs(torch, B, peaks, main_cfg, main_result, mem=None):
                                 "fma_pipe_frac": pairs * SLOTS_V_ONLY_F32_GRID / (np.median(step_ms) * 1e-3) / peak,
                                 "xu_pipe_frac": pairs / (np.median(step_ms) * 1e-3) / peaks["mufu_lane_ops_per_s"],
                                 "kernel_symbol": info.get("last_kernel", ""), "plan": info["last_plan"]})
+                    # V + E without the accurate-V arithmetic (qmmm_field_set_accurate_v(h, 0)): the
+                    # kernel of rounds 1-2 before the batch-total criterion was met
+                    B.qmmm_field_set_accurate_v(h, False)
+                    step_ms, pair_ms, _ = time_steps(torch, B, h, batches, W, N, prec, reps, 3, flush, stream)
+                    info = B.qmmm_field_get_info(h)
+                    B.qmmm_field_set_accurate_v(h, True)
+                    out.append({"config": idx, "name": w.name, "precision": "fp32, accurate_v off",
+                                "layout": layout, "layout_choice": "auto" if which == "auto" else "forced",
+                                "points": P, "M": w.M, "K": w.K, "pairs_per_eval": pairs,
+                                "ms_per_eval_median": float(np.median(step_ms)),
+                                "pair_kernel_ms_median": float(np.median(pair_ms)),
+                                "gpairs_per_s": pairs / np.median(step_ms) / 1e6,
+                                "slots_per_pair": slots,
+                                "fma_pipe_frac": pairs * slots / (np.median(step_ms) * 1e-3) / peak,
+                                "xu_pipe_frac": pairs / (np.median(step_ms) * 1e-3) / peaks["mufu_lane_ops_per_s"],
+                                "kernel_symbol": info.get("last_kernel", ""), "plan": info["last_plan"]})
                 if prec == "fp64" and not w.sequential and idx in (1, 4):
                     # potential only (E = NULL): the paper's own computation, Eq. 4; 12 (list) or
                     # 8 (grid; 7 with the dz table) DP slots
@@ -568,9 +584,10 @@ def run_ours(args):
         peak_lane = 0.5 * (peaks0[peak_key] + peaks1[peak_key])
         pair_s = float(np.mean(pair_ms)) * 1e-3
         if args.potential_only and prec == "fp32":
-            # only the batched grid kernel has an FP32 potential-only variant (its symbol ends in
-            # ...ELb1EEEv...); every other FP32 path runs its V + E kernel with E = NULL
-            v_kernel = "ELb1EEEvNS_10PairParamsE" in info.get("last_kernel", "") and "grid_kernel_f32x2" in info.get("last_kernel", "")
+            # only the batched grid kernel has an FP32 potential-only variant (template arguments
+            # <.., VONLY = true, ACCV = false>: its symbol ends in ...ELb1ELb0EEEv...); every other
+            # FP32 path runs its V + E kernel with E = NULL
+            v_kernel = "ELb1ELb0EEEvNS_10PairParamsE" in info.get("last_kernel", "") and "grid_kernel_f32x2" in info.get("last_kernel", "")
             slots = SLOTS_V_ONLY_F32_GRID if v_kernel else slots_for(layout, prec, info)
         else:
             slots = slots_for(layout, prec, info, v_only=args.potential_only)

@@ -62,8 +62,8 @@ typedef enum {
  *                     a grid runs a potential-only kernel (6 instead of 8 operations per pair)
  *                     whose row sums are compensated: on BASELINE config 3 its V is within
  *                     2.7e-8 hartree rms per point and 5.4e-6 hartree summed over all 16,384
- *                     points (V + E launch: 6.7e-8 and 3.1e-5) -- take energies from it
- *                     (qmmm_field_eval_energy does). */
+ *                     points; the batched V + E kernel does the same by default (2.6e-8,
+ *                     5.8e-6; qmmm_field_set_accurate_v). */
 typedef enum { QMMM_FP64 = 0, QMMM_FP32_ACC64 = 1 } qmmm_precision;
 
 /*
@@ -280,6 +280,23 @@ qmmm_status qmmm_sum_rank_partials(const double *parts, int64_t R, int64_t n, do
  * setting does not concern them.  Sticky; INVALID_ARG on another mode.
  */
 qmmm_status qmmm_field_set_local_lattice(qmmm_field *h, int mode);
+
+/*
+ * FP32 grid kernels, batched V + E evaluations (every warp its own points, dz table: a few
+ * hundred points and more per call): accuracy of V.  BASELINE.json's north star asks for the
+ * total electrostatic energy sum_i V(r_i) within 1e-5 hartree; for a batch of 16,384 points
+ * (configs[3]) that is 4e-12 of the sum, which plain FP32 arithmetic with FP64 accumulation of
+ * row sums misses (3.1e-5: a common bias of +1.9e-9 hartree per point and 6.7e-8 rms).
+ * enable != 0 (default): r^2 = rxy2 + z2 with rxy2 formed in FP64 per (point, row) and z2 from a
+ * second per-CTA table, both rounded once, and the last level of the FP32 row sums added with a
+ * two-sum (as in the potential-only kernel): 2.6e-8 rms, +3.6e-10 mean, 5.8e-6 over the batch,
+ * at 5.6 % more time (configs[3]: 5.60 instead of 5.30 ms).  enable = 0: the faster kernel
+ * (every per-configuration energy still within 2e-6 hartree).  E agrees between the two to FP32
+ * rounding (1e-7 relative).  Used when both tables fit in shared memory beside the pipeline (z
+ * axes of up to 128 nodes at the default depth: every FP32 BASELINE configuration), else the
+ * faster kernel runs.  Sticky; shared handles inherit the parent's setting at qmmm_field_share.
+ */
+qmmm_status qmmm_field_set_accurate_v(qmmm_field *h, int enable);
 
 /*
  * qmmm_field_eval_noalloc -- V and E (Eq. 4, and its field) for callers that

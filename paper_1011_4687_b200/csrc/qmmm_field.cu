@@ -223,6 +223,7 @@ struct qmmm_field {
     double q_scale = 1.0;          // power of two applied to the cell charges of the FP32 copies
     int local_lattice = -1;        // FP32 grid kernel, lattice per gchunk: -1 automatic, 0 off, 1 on
     int last_local_lattice = 0;
+    int accurate_v = 1;            // FP32 batched grid V + E kernel: accurate V (qmmm_field_set_accurate_v)
     const char *last_kernel = "";  // mangled name of the kernel the most recent evaluation ran
     // device error word (pinned, device-mapped): set by a kernel whose bounded wait gave up
     int *dev_err_h = nullptr, *dev_err_d = nullptr;
@@ -419,13 +420,15 @@ cudaError_t launch_pair_ept(bool f32, int ept, const PairParams &prm, dim3 grid,
 }
 
 template <int EP2, int NW, bool NODEPACK = false, bool FULL = false, bool DZT = false, int FINE = -1,
-          bool VONLY = false>
+          bool VONLY = false, bool ACCV = false>
 cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaStream_t st) {
     if constexpr (!NODEPACK && !FULL) {            // every warp its own point group: no z split
         if constexpr (EP2 == 2 && NW == GRID_NW_EPT4) {
             // E = NULL: the potential alone (Eq. 4), 6 instead of 8 operations per pair
             if (prm.point_warps == NW && prm.g_dzt && !prm.E)
                 return launch_grid_f32<EP2, NW, false, true, true, 0, true>(prm, grid, smem, st);
+            if (prm.point_warps == NW && prm.g_dzt && prm.g_accv)
+                return launch_grid_f32<EP2, NW, false, true, true, 0, false, true>(prm, grid, smem, st);
         }
         if constexpr (EP2 == 2 && (NW == GRID_NW_EPT4 || NW == GRID_NW_EPT4_LIGHT)) {
             // (the dz-table kernels work from the point's true position: no lattice to refine)
@@ -440,7 +443,7 @@ cudaError_t launch_grid_f32(const PairParams &prm, dim3 grid, size_t smem, cudaS
             if (prm.g_dzt) return launch_grid_f32<EP2, NW, false, false, true>(prm, grid, smem, st);
         }
     }
-    auto kern = grid_kernel_f32x2<EP2, NW, NODEPACK, FULL, DZT, FINE, VONLY>;
+    auto kern = grid_kernel_f32x2<EP2, NW, NODEPACK, FULL, DZT, FINE, VONLY, ACCV>;
     static SmemConfig configured;
     static const char *const name = kernel_name(reinterpret_cast<const void *>(kern));
     g_launched = name;
@@ -1264,6 +1267,7 @@ qmmm_status qmmm_field_share(const qmmm_field *parent, int64_t max_points, qmmm_
     h->gcells32 = parent->gcells32; h->gcells64 = parent->gcells64; h->nuclei_u = parent->nuclei_u;
     h->layout = parent->layout;
     h->local_lattice = parent->local_lattice;
+    h->accurate_v = parent->accurate_v;
     for (int k = 0; k < 3; ++k) { h->bb_lo[k] = parent->bb_lo[k]; h->bb_hi[k] = parent->bb_hi[k]; }
     // its own mutable part: workspace, tickets, mailboxes, move server, staging, plan
     qmmm_status rs = alloc_runtime(h);
@@ -1373,6 +1377,12 @@ qmmm_status qmmm_field_set_local_lattice(qmmm_field *h, int mode) {
     return QMMM_OK;
 }
 
+qmmm_status qmmm_field_set_accurate_v(qmmm_field *h, int enable) {
+    if (!h) return fail(QMMM_ERR_INVALID_ARG, "set_accurate_v: NULL handle");
+    h->accurate_v = enable != 0;
+    return QMMM_OK;
+}
+
 qmmm_status qmmm_field_set_overlap(qmmm_field *h, int enable) {
     if (!h) return fail(QMMM_ERR_INVALID_ARG, "set_overlap: NULL handle");
     h->overlap = enable != 0;
@@ -1463,6 +1473,10 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
     // (the FP32 kernel runs two CTAs per SM: half the budget each)
     const bool use_dzt = dzt > 0 && smem + dzt <= (f32 ? (light ? 56 : 110) : 200) * 1024;
     if (use_dzt) smem += dzt;
+    // batched FP32 V + E kernel: accurate V (a z2 table beside the dz table) when both fit
+    const bool use_accv = use_dzt && f32 && E && !light && h->accurate_v && pl.points_per_thread == 4 &&
+                          pl.point_warps == GRID_NW_EPT4 && smem + dzt <= 110 * 1024;
+    if (use_accv) smem += dzt;
 
     if (h->timing) CUDA_TRY(cudaEventRecord(h->ev[0], st));
     {
@@ -1513,6 +1527,7 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
         if (grid) {
             fill_grid_params(h, prm, f32);
             prm.g_dzt = use_dzt ? 1 : 0;
+            prm.g_accv = use_accv ? 1 : 0;
             prm.g_light = light ? 1 : 0;
         } else {
             prm.chunks = f32 ? reinterpret_cast<const char *>(h->chunks32)

@@ -116,9 +116,32 @@ __device__ __forceinline__ void add_run(float2 &v, float2 &d, float2 x, float2 d
 // row) and rounded once, and r^2 = rxy2 + z2 is ONE add.  No lattice and no residual: nothing
 // needs the field to be corrected with.  Per pair: r^2, a, V0 += a, y0^2, c, T += c r^2 = 6
 // FMA-pipe lane operations + 1 MUFU.RSQ -- the XU pipe (16 per SM and clock) is the limit.
-template <int EP2, int TS = 0, bool VONLY = false>
+//
+// ACCV (V + E, batched table kernel; the default, qmmm_field_set_accurate_v): the same r^2 as
+// VONLY -- a z2 entry beside every dz entry of the table, rxy2 formed in FP64 per (point, row) --
+// and the same compensated row sums, with dz still read for sum c dz.  Still 8 operations per
+// pair (r^2 is one add instead of one fma), one more broadcast load per node, a quarter
+// operation for the two-sum: +5.6 % time on config 3 for V rms 6.7e-8 -> 2.6e-8 hartree and the
+// total over the 16,384 points of the batch 3.1e-5 -> 5.8e-6.
+template <int EP2, int TS = 0, bool VONLY = false, bool ACCV = false>
 struct GridRowF32 {
     static_assert(!VONLY || TS > 0, "the potential-only walk is table-driven");
+    static_assert(!ACCV || (TS > 0 && !VONLY), "ACCV: V + E walk with the dz and the z2 table");
+    static constexpr bool COMP = VONLY || ACCV;      // last tree level added with a two-sum
+    // r^2 of the node whose table entry is t: dz^2 + rxy2, or (VONLY: the table holds z2;
+    // ACCV: a z2 entry follows the node's dz entries) z2 + rxy2
+    __device__ __forceinline__ void r2_of(const float2 *t, const float2 (&dz)[EP2], float2 (&r2)[EP2]) {
+        if constexpr (ACCV) {
+            float2 z2[EP2];
+            load_dz(t + TS / 2, z2);
+#pragma unroll
+            for (int e = 0; e < EP2; ++e) r2[e] = __fadd2_rn(z2[e], rxy2[e]);
+        } else {
+#pragma unroll
+            for (int e = 0; e < EP2; ++e)
+                r2[e] = VONLY ? __fadd2_rn(dz[e], rxy2[e]) : __ffma2_rn(dz[e], dz[e], rxy2[e]);
+        }
+    }
     float2 dzA[EP2], r2A[EP2], y0A[EP2], dzB[EP2], r2B[EP2], y0B[EP2];
     float2 rxy2[EP2], S[EP2], SZ[EP2];
     const float2 *tp;                  // TS > 0: table entry of the node held in the current set
@@ -141,8 +164,8 @@ struct GridRowF32 {
         for (int e = 0; e < EP2; ++e) {
             rxy2[e] = rxy2_[e];
             S[e] = SZ[e] = f2(0.0f, 0.0f);
-            r2A[e] = VONLY ? __fadd2_rn(dzA[e], rxy2[e]) : __ffma2_rn(dzA[e], dzA[e], rxy2[e]);
         }
+        r2_of(t, dzA, r2A);
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
             y0A[e].x = rsqrt_mufu_f32(r2A[e].x);
@@ -166,11 +189,15 @@ struct GridRowF32 {
     // next node from the current one: dz - 1, r^2, MUFU
     __device__ __forceinline__ void step(const float2 (&dzc)[EP2], float2 (&dzn)[EP2],
                                          float2 (&r2n)[EP2], float2 (&y0n)[EP2], int j = 0) {
-        if constexpr (TS > 0) load_dz(tp + j * TS, dzn);      // j-th node after the one at tp
+        if constexpr (TS > 0) {
+            load_dz(tp + j * TS, dzn);                        // j-th node after the one at tp
+            r2_of(tp + j * TS, dzn, r2n);
+        } else {
 #pragma unroll
-        for (int e = 0; e < EP2; ++e) {
-            if constexpr (TS == 0) dzn[e] = __fadd2_rn(dzc[e], bc(-1.0f));
-            r2n[e] = VONLY ? __fadd2_rn(dzn[e], rxy2[e]) : __ffma2_rn(dzn[e], dzn[e], rxy2[e]);
+            for (int e = 0; e < EP2; ++e) {
+                dzn[e] = __fadd2_rn(dzc[e], bc(-1.0f));
+                r2n[e] = __ffma2_rn(dzn[e], dzn[e], rxy2[e]);
+            }
         }
 #pragma unroll
         for (int e = 0; e < EP2; ++e) {
@@ -218,9 +245,9 @@ struct GridRowF32 {
     // point (partial sums 1 : 2 : 3 : 4 of nearly equal terms; reproduced by a CPU emulation
     // of the tree in IEEE float32), so there it is added with a fast
     // two-sum whose error term goes to d: a quarter operation per pair, +2.3 % time, rms of V
-    // on config 3 4.5e-8 -> 2.7e-8 and the batch total inside 1e-5 hartree.  The V + E kernel
-    // keeps plain adds: its error is dominated by the FP32 dz table and rxy2 (6.7e-8 -> 6.4e-8
-    // with the two-sum, at +3 % time: measured, not taken).
+    // on config 3 4.5e-8 -> 2.7e-8 and the batch total inside 1e-5 hartree.  ACCV: the same.
+    // The other V + E walks keep plain adds: their error is dominated by the FP32 dz table and
+    // rxy2 (6.7e-8 -> 6.4e-8 with the two-sum alone, at +3 % time).
     __device__ __forceinline__ void run(const float *b, int n4, float2 (&v)[EP2], float2 (&d)[EP2]) {
         if ((n4 & 3) == 0) {
             float2 t[EP2];
@@ -241,7 +268,7 @@ struct GridRowF32 {
                 }
 #pragma unroll
                 for (int e = 0; e < EP2; ++e) {
-                    if constexpr (VONLY) {
+                    if constexpr (COMP) {
                         add_run(v[e], d[e], v16[e], __ffma2_rn(v16[e], bc(-1.0f), t16[e]));
                     } else {
                         v[e] = __fadd2_rn(v[e], v16[e]);
@@ -249,7 +276,7 @@ struct GridRowF32 {
                     }
                 }
             }
-            if constexpr (!VONLY) {
+            if constexpr (!COMP) {
 #pragma unroll
                 for (int e = 0; e < EP2; ++e) d[e] = __fadd2_rn(d[e], __ffma2_rn(v[e], bc(-1.0f), t[e]));
             }
@@ -373,9 +400,11 @@ constexpr int GRID_FLUSH = QMMM_GRID_FLUSH;                       // gchunks per
 // FINE: coordinate lattice per gchunk (on_lattice) -- 1 on, 0 off (the batched FULL kernels are
 // compiled both ways: the switch costs registers in their loop), -1 decided by prm.g_fine.
 // VONLY (E = NULL; FULL + DZT only): the potential alone, no lattice (GridRowF32<.., VONLY>).
+// ACCV (FULL + DZT, V + E): accurate V (GridRowF32<.., false, ACCV>); the table is twice as large.
 template <int EP2, int NW, bool NODEPACK = false, bool FULL = false, bool DZT = false, int FINE = -1,
-          bool VONLY = false>
+          bool VONLY = false, bool ACCV = false>
 __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 16 / NW : 1) grid_kernel_f32x2(const PairParams prm) {
+    static_assert(!ACCV || (FULL && DZT && !VONLY), "ACCV: the batched table-driven V + E walk");
     static_assert(FINE == -1 || FULL, "the compile-time switch is for the batched FULL kernels");
     static_assert(!VONLY || (FULL && DZT && FINE == 0), "potential only: batched table-driven walk, no lattice");
     static_assert(!DZT || !NODEPACK, "dz table: the point-packed walks (every warp its own points, or z-split warps)");
@@ -478,7 +507,7 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
         dd_all[i] = dd * static_cast<float>(sc);                // residual in units of hz
     }
     __syncthreads();
-    constexpr int TS = DZT ? NW * EP2 : 0;                      // float2 per z node of the table
+    constexpr int TS = DZT ? NW * EP2 * (ACCV ? 2 : 1) : 0;     // float2 per z node of the table (ACCV: dz entries, then z2 entries)
     float *dzt = reinterpret_cast<float *>(acc + EPT * 2 * NT); // [segs * ZS + 1][NW][EPT]
     if constexpr (DZT) {
         // one entry per (z node, point of the CTA), formed in FP64 from the point's TRUE coordinate
@@ -488,7 +517,12 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
             const int kz = i / (NW * EPT), pp = i - kz * (NW * EPT);
             if (pp >= ppb) continue;                            // (z-split plans stage fewer than NW point groups)
             const double dzt64 = u_s[pp * 3 + 2] - static_cast<double>(kz);
-            dzt[i] = static_cast<float>(VONLY ? dzt64 * dzt64 : dzt64);
+            if constexpr (ACCV) {
+                dzt[(2 * kz + 0) * (NW * EPT) + pp] = static_cast<float>(dzt64);
+                dzt[(2 * kz + 1) * (NW * EPT) + pp] = static_cast<float>(dzt64 * dzt64);
+            } else {
+                dzt[i] = static_cast<float>(VONLY ? dzt64 * dzt64 : dzt64);
+            }
         }
         __syncthreads();
     }
@@ -677,13 +711,22 @@ __global__ void __launch_bounds__(32 * NW, (!NODEPACK && NW <= 8 && EP2 <= 2) ? 
                 }
                 const float2 ddx = *reinterpret_cast<const float2 *>(dd_w + 2 * e);        // units of hz
                 const float2 ddy = *reinterpret_cast<const float2 *>(dd_w + EPT + 2 * e);
-                const float2 cross = __ffma2_rn(dx[e], ddx, __fmul2_rn(dy[e], ddy));
-                rxy2[e] = __ffma2_rn(dy[e], dy[e], __ffma2_rn(dx[e], dx[e], __ffma2_rn(cross, bc(2.0f), bc(1e-30f))));
+                if constexpr (ACCV) {
+                    // rxy2 of the true point in FP64, rounded once (as in the potential-only kernel)
+                    const double rowx = static_cast<double>(ix) * prm.g_sx, rowy = static_cast<double>(iy) * prm.g_sy;
+                    const double dx0 = pe[6 * e + 0] - rowx, dy0 = pe[6 * e + 1] - rowy;
+                    const double dx1 = pe[6 * e + 3] - rowx, dy1 = pe[6 * e + 4] - rowy;
+                    rxy2[e] = f2(static_cast<float>(fma(dy0, dy0, fma(dx0, dx0, 1e-30))),
+                                 static_cast<float>(fma(dy1, dy1, fma(dx1, dx1, 1e-30))));
+                } else {
+                    const float2 cross = __ffma2_rn(dx[e], ddx, __fmul2_rn(dy[e], ddy));
+                    rxy2[e] = __ffma2_rn(dy[e], dy[e], __ffma2_rn(dx[e], dx[e], __ffma2_rn(cross, bc(2.0f), bc(1e-30f))));
+                }
                 dx[e] = __fadd2_rn(dx[e], ddx);                       // the true differences, for the field
                 dy[e] = __fadd2_rn(dy[e], ddy);
                 v[e] = tq[e] = f2(0.0f, 0.0f);
             }
-            GridRowF32<EP2, TS> row;
+            GridRowF32<EP2, TS, false, ACCV> row;
             // (z-split warps start at their own z run z0 of the gchunk; FULL: z0 = 0, ZL = 64)
             row.start(reinterpret_cast<const float2 *>(dzt) + (seg * GRID_ZS + z0) * TS + wp * EP2, rxy2);
             mbar_wait(&full[slot], phase);

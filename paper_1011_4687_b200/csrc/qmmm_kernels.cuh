@@ -61,6 +61,7 @@ struct PairParams {
     double g_scaleV, g_scaleE;   // 1/hz, 1/hz^2
     int g_n[3], g_segs;      // nodes per axis (row = ix * ny + iy); z segments (gchunks) per row tile
     int g_dzt;               // grid kernels: dz table in shared memory (qmmm_grid.cuh, DZT)
+    int g_accv;              // FP32 batched dz-table kernel: accurate V (z2 table, FP64 rxy2, compensated row sums)
     int g_fine;              // FP32 grid kernel: coordinate lattice per gchunk instead of per grid (long axes)
     // FP32 copies (list and grid) store q_j * 2^k with 2^k * max|q| in [0.5, 1): tiny charges keep
     // their full FP32 precision (no denormals, no flush), and the result does not depend on the

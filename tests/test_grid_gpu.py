@@ -300,10 +300,15 @@ def test_config3_grid_fp32_full_energy(torch_cuda, B, oracle_mod, full_oracle):
     try:
         V, E = run(torch_cuda, B, h, pts, "fp32")
         assert B.qmmm_field_get_grid_info(h)["last_layout"] == "grid"
+        assert "ELb0ELb1EEEv" in B.qmmm_field_get_info(h)["last_kernel"]  # <2, 8, false, true, true, 0, false, ACCV = true>
+        B.qmmm_field_set_accurate_v(h, False)     # the faster V + E kernel (same E; V to 7e-8 rms instead of 3e-8)
+        Vf, Ef = run(torch_cuda, B, h, pts, "fp32")
+        assert "ELb0ELb0EEEv" in B.qmmm_field_get_info(h)["last_kernel"]
+        B.qmmm_field_set_accurate_v(h, True)
         Vl, El = run(torch_cuda, B, h, pts, "fp32", layout="list")
         # E = NULL: the potential-only kernel (Eq. 4 proper; no lattice, 6 operations per pair)
         Vp, _ = run(torch_cuda, B, h, pts, "fp32", want_E=False, layout="auto")
-        assert "ELb1EEEv" in B.qmmm_field_get_info(h)["last_kernel"]      # <2, 8, false, true, true, 0, true>
+        assert "ELb1ELb0EEEv" in B.qmmm_field_get_info(h)["last_kernel"]  # <2, 8, false, true, true, 0, VONLY = true, false>
         U = torch_cuda.zeros(w.W, dtype=torch_cuda.float64, device="cuda")
         B.qmmm_field_eval_energy(h, torch_cuda.from_numpy(pts).cuda(), w.W, w.N, U, "fp32")
         torch_cuda.cuda.synchronize()
@@ -312,12 +317,13 @@ def test_config3_grid_fp32_full_energy(torch_cuda, B, oracle_mod, full_oracle):
         B.qmmm_field_destroy(h)
     full = full_oracle(3)                         # every point, V and E
     check(full, V, E, TOL32)
+    check(full, Vf, Ef, TOL32)
     check(full, Vl, El, TOL32)
     check(full, Vp, None, TOL32)
     dU = np.abs(U + full.V.reshape(w.W, w.N).sum(1))
     print(f"config3 fp32 eval_energy: per-walker max |dU| = {dU.max():.3e} hartree")
     assert dU.max() <= E_TOL
-    for name, v in (("grid", V), ("list", Vl), ("grid potential-only", Vp)):
+    for name, v in (("grid", V), ("grid, accurate_v off", Vf), ("list", Vl), ("grid potential-only", Vp)):
         per_walker = np.abs(v.reshape(w.W, w.N).sum(1) - full.V.reshape(w.W, w.N).sum(1))
         batch = abs(v.sum() - full.V.sum())
         d = v - full.V
@@ -326,15 +332,18 @@ def test_config3_grid_fp32_full_energy(torch_cuda, B, oracle_mod, full_oracle):
         assert per_walker.max() <= E_TOL
         assert batch / w.W <= E_TOL
         assert batch <= 1e-4
-        if name == "grid potential-only":
-            # the energy path (Eq. 4 needs V only; qmmm_field_eval_energy runs this kernel): the
-            # north star's criterion taken literally -- the sum over all 16,384 points within
-            # 1e-5 hartree of the oracle's, 4e-12 of the 2.5e6 hartree it adds up
+        if name in ("grid", "grid potential-only"):
+            # the configuration bench.py times (V and E) and the energy path (Eq. 4 needs V only;
+            # qmmm_field_eval_energy runs the potential-only kernel): the north star's criterion
+            # taken literally -- the sum over all 16,384 points within 1e-5 hartree of the
+            # oracle's, 4e-12 of the 2.5e6 hartree it adds up
             assert batch <= E_TOL, batch
     # and through the entry point that returns energies: sum over walkers of U[w]
     batch_U = abs(U.sum() + full.V.sum())
     print(f"config3 fp32 eval_energy: whole batch |dU| = {batch_U:.3e} hartree")
     assert batch_U <= E_TOL
+    # the field is formed from the same sums either way (r^2 differs in its last bit)
+    assert np.max(np.linalg.norm(E - Ef, axis=1) / np.linalg.norm(Ef, axis=1)) <= 1e-6
     for name, e in (("grid", E), ("list", El)):
         eE = np.linalg.norm(e - full.E, axis=1) / np.linalg.norm(full.E, axis=1)
         kE = full.absE / np.linalg.norm(full.E, axis=1)

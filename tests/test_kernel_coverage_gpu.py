@@ -108,6 +108,12 @@ def test_every_kernel_instantiation_runs_and_agrees_with_the_oracle(oracle_mod):
                                         continue        # the list kernels have no overlap / FULL variants
                                     evaluate(h, base[:n], Sub(ref_all, n), layout, prec, plan, overlap, want_E,
                                              f"cfg1 {layout} {prec} n={n} ppt={ppt} pw={pw} ov={overlap} E={want_E}")
+        # the batched FP32 V + E kernel without the accurate-V arithmetic (qmmm_field_set_accurate_v)
+        B.qmmm_field_set_accurate_v(h, False)
+        for n in (24, P0):
+            evaluate(h, base[:n], Sub(ref_all, n), "grid", "fp32", dict(points_per_thread=4, point_warps=16), False, True,
+                     f"cfg1 grid fp32 n={n} ppt=4 pw=16 accurate_v off")
+        B.qmmm_field_set_accurate_v(h, True)
         # the move servers (single-point host calls): grid-aware on this handle, source list when forced
         for layout in ("auto", "list"):
             for prec in ("fp64", "fp32"):

@@ -5,7 +5,7 @@ holds the reciprocal-square-root seeds (MUFU.RSQ / MUFU.RSQ64H: exactly one per 
 the arithmetic-pipe lane operations in it are counted per seed: packed FFMA2 / FMUL2 / FADD2 count
 two (two points per instruction), scalar FP32 and every DP instruction one.  The count must equal
 the table's figure, plus at most the summation-tree adds of the FP32 kernels (a quarter operation
-per pair; half of one in the potential-only kernel, whose last tree level is compensated); a kernel that silently did more -- or less -- work per pair than the roofline assumes
+per pair; half of one in the kernels whose last tree level is compensated); a kernel that silently did more -- or less -- work per pair than the roofline assumes
 would fail here.
 """
 import os
@@ -20,17 +20,20 @@ PACKED = ("FFMA2", "FMUL2", "FADD2")
 SCALAR = ("FFMA", "FMUL", "FADD")
 DP = ("DFMA", "DMUL", "DADD")
 
-# (mangled kernel, layout, precision, potential only, dz table)
+# (mangled kernel, layout, precision, potential only, dz table, compensated row sums)
 KERNELS = [
-    ("_ZN4qmmm17grid_kernel_f32x2ILi2ELi8ELb0ELb1ELb1ELi0ELb0EEEvNS_10PairParamsE", "grid", "fp32", False, True),
-    ("_ZN4qmmm17grid_kernel_f32x2ILi2ELi8ELb0ELb1ELb1ELi0ELb1EEEvNS_10PairParamsE", "grid", "fp32", True, True),
-    ("_ZN4qmmm17grid_kernel_f32x2ILi2ELi8ELb0ELb1ELb0ELi0ELb0EEEvNS_10PairParamsE", "grid", "fp32", False, False),
-    ("_ZN4qmmm17pair_kernel_f32x2ILi4ELi8EEEvNS_10PairParamsE", "list", "fp32", False, False),
-    ("_ZN4qmmm15grid_kernel_f64ILi4ELb1ELi8ELb0ELb1EEEvNS_10PairParamsE", "grid", "fp64", False, True),
-    ("_ZN4qmmm15grid_kernel_f64ILi4ELb0ELi8ELb0ELb1EEEvNS_10PairParamsE", "grid", "fp64", True, True),
-    ("_ZN4qmmm15grid_kernel_f64ILi4ELb1ELi8ELb0ELb0EEEvNS_10PairParamsE", "grid", "fp64", False, False),
-    ("_ZN4qmmm11pair_kernelIdLi4ELb1EEEvNS_10PairParamsE", "list", "fp64", False, False),
-    ("_ZN4qmmm11pair_kernelIdLi4ELb0EEEvNS_10PairParamsE", "list", "fp64", True, False),
+    # <2, 8, false, true, true, 0, VONLY, ACCV>: the batched kernels of config 3 -- V + E with accurate V (default),
+    # V + E fast (qmmm_field_set_accurate_v(h, 0)), potential only
+    ("_ZN4qmmm17grid_kernel_f32x2ILi2ELi8ELb0ELb1ELb1ELi0ELb0ELb1EEEvNS_10PairParamsE", "grid", "fp32", False, True, True),
+    ("_ZN4qmmm17grid_kernel_f32x2ILi2ELi8ELb0ELb1ELb1ELi0ELb0ELb0EEEvNS_10PairParamsE", "grid", "fp32", False, True, False),
+    ("_ZN4qmmm17grid_kernel_f32x2ILi2ELi8ELb0ELb1ELb1ELi0ELb1ELb0EEEvNS_10PairParamsE", "grid", "fp32", True, True, True),
+    ("_ZN4qmmm17grid_kernel_f32x2ILi2ELi8ELb0ELb1ELb0ELi0ELb0ELb0EEEvNS_10PairParamsE", "grid", "fp32", False, False, False),
+    ("_ZN4qmmm17pair_kernel_f32x2ILi4ELi8EEEvNS_10PairParamsE", "list", "fp32", False, False, False),
+    ("_ZN4qmmm15grid_kernel_f64ILi4ELb1ELi8ELb0ELb1EEEvNS_10PairParamsE", "grid", "fp64", False, True, False),
+    ("_ZN4qmmm15grid_kernel_f64ILi4ELb0ELi8ELb0ELb1EEEvNS_10PairParamsE", "grid", "fp64", True, True, False),
+    ("_ZN4qmmm15grid_kernel_f64ILi4ELb1ELi8ELb0ELb0EEEvNS_10PairParamsE", "grid", "fp64", False, False, False),
+    ("_ZN4qmmm11pair_kernelIdLi4ELb1EEEvNS_10PairParamsE", "list", "fp64", False, False, False),
+    ("_ZN4qmmm11pair_kernelIdLi4ELb0EEEvNS_10PairParamsE", "list", "fp64", True, False, False),
 ]
 
 
@@ -57,8 +60,8 @@ def hot_loop(lib, sym, seed):
 
 
 @pytest.mark.skipif(shutil.which("cuobjdump") is None, reason="cuobjdump (CUDA toolkit) not on PATH")
-@pytest.mark.parametrize("sym,layout,prec,v_only,dzt", KERNELS)
-def test_lane_operations_per_pair_match_the_roofline_table(sym, layout, prec, v_only, dzt):
+@pytest.mark.parametrize("sym,layout,prec,v_only,dzt,comp", KERNELS)
+def test_lane_operations_per_pair_match_the_roofline_table(sym, layout, prec, v_only, dzt, comp):
     from paper_1011_4687_b200 import build
     import bench
     lib = build.build()
@@ -76,9 +79,9 @@ def test_lane_operations_per_pair_match_the_roofline_table(sym, layout, prec, v_
         assert sum(ops.count(k) for k in DP) == 0, "FP64 arithmetic inside the FP32 hot loop"
         per_pair = lane_ops / seeds
         # one seed per pair; the V0 / T summation trees add at most a quarter operation per pair,
-        # the compensated last tree level of the potential-only kernel (fast two-sum, once per 16
-        # nodes) another quarter
-        extra = 0.5 if v_only else 0.25
+        # the compensated last tree level of the potential-only and the accurate V + E kernel (fast
+        # two-sum, once per 16 nodes) another quarter
+        extra = 0.5 if comp else 0.25
         assert claimed <= per_pair <= claimed + extra + 1e-9, (sym, per_pair, claimed)
     else:
         per_pair = sum(ops.count(k) for k in DP) / seeds
