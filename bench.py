@@ -613,6 +613,10 @@ def run_ours(args):
                        "pairs_per_step_per_gpu": pairs_step_rank,
                        "parallelism": f"walkers sharded x{world}, sources replicated, no collective",
                        "layout": layout, "outputs": "V only (E = NULL)" if args.potential_only else "V and E",
+                       "accurate_v": ("on (library default): batched FP32 grid V + E kernel with the z2 table, FP64-formed rxy2 "
+                                      "and compensated row sums -- the batch's total energy within 1e-5 hartree of the oracle's "
+                                      "(tests/test_grid_gpu.py::test_config3_grid_fp32_full_energy); the sweep row "
+                                      "'fp32, accurate_v off' times the faster kernel") if prec == "fp32" else "n/a (FP64)",
                        "l2": "flushed between timed steps (256 MB write)", "plan": info["last_plan"],
                        "point_blocks": info["last_point_blocks"]},
             "clocks": clocks,
