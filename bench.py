@@ -689,6 +689,13 @@ def run_ours(args):
                             "traffic": lookup_traffic(f"config4_fp64_{r['layout']}")[0],
                             "traffic_source": "ncu --set full capture under profiles/ (pair_kernel_traffic.csv); looked up",
                             "peak_source": "measured DFMA lane rate, same process (qmmm_probe_peak)"}
+                    if (r["config"] == args.config and r["precision"] == "fp32, accurate_v off"
+                            and r["layout_choice"] == "auto" and prec == "fp32"):
+                        # the same workload with qmmm_field_set_accurate_v(h, 0): the faster kernel that
+                        # misses the batch-total energy criterion (context for roofline.frac)
+                        line["roofline"]["accurate_v_off"] = {
+                            "frac": r["fma_pipe_frac"], "gpairs_per_s": r["gpairs_per_s"],
+                            "kernel_ms": r["pair_kernel_ms_median"], "kernel_symbol": r["kernel_symbol"]}
         print(json.dumps(line), flush=True)
     if h is not None:
         B.qmmm_field_destroy(h)
