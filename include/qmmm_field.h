@@ -292,8 +292,8 @@ qmmm_status qmmm_field_set_local_lattice(qmmm_field *h, int mode);
  * two-sum (as in the potential-only kernel): 2.6e-8 rms, +3.6e-10 mean, 5.8e-6 over the batch,
  * at 5.6 % more time (configs[3]: 5.60 instead of 5.30 ms).  enable = 0: the faster kernel
  * (every per-configuration energy still within 2e-6 hartree).  E agrees between the two to FP32
- * rounding (1e-7 relative).  Used when both tables fit in shared memory beside the pipeline (z
- * axes of up to 128 nodes at the default depth: every FP32 BASELINE configuration), else the
+ * rounding (1e-7 relative).  Used when both tables fit in shared memory beside a pipeline of at
+ * least two stages (z axes of up to 192 nodes: every FP32 BASELINE configuration), else the
  * faster kernel runs.  Sticky; shared handles inherit the parent's setting at qmmm_field_share.
  */
 qmmm_status qmmm_field_set_accurate_v(qmmm_field *h, int enable);
