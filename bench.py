@@ -76,6 +76,9 @@ def parse_args():
                          "batch has many points)")
     ap.add_argument("--potential-only", action="store_true",
                     help="E = NULL: the potential alone (PAPER.md Eq. 4 proper); fewer operations per pair")
+    ap.add_argument("--fast-v", action="store_true",
+                    help="qmmm_field_set_accurate_v(h, 0): the batched FP32 grid V + E kernel without the accurate-V "
+                         "arithmetic (5.6 %% faster; misses the batch-total energy criterion, DESIGN.md section 6)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-sweep", action="store_true",
                     help="skip the per-config table (all five configs) at N=1")
@@ -537,6 +540,8 @@ def run_ours(args):
     h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, P)
     B.qmmm_field_set_layout(h, args.layout)
     B.qmmm_field_set_timing(h, True)
+    if args.fast_v:
+        B.qmmm_field_set_accurate_v(h, False)
     n_batches = 4
     host_batches = [draw_points(args.config, W, N, seed=1 + 97 * rank + b).reshape(-1, 3)
                     for b in range(n_batches)]
@@ -613,7 +618,7 @@ def run_ours(args):
                        "pairs_per_step_per_gpu": pairs_step_rank,
                        "parallelism": f"walkers sharded x{world}, sources replicated, no collective",
                        "layout": layout, "outputs": "V only (E = NULL)" if args.potential_only else "V and E",
-                       "accurate_v": ("on (library default): batched FP32 grid V + E kernel with the z2 table, FP64-formed rxy2 "
+                       "accurate_v": "off (--fast-v)" if args.fast_v else ("on (library default): batched FP32 grid V + E kernel with the z2 table, FP64-formed rxy2 "
                                       "and compensated row sums -- the batch's total energy within 1e-5 hartree of the oracle's "
                                       "(tests/test_grid_gpu.py::test_config3_grid_fp32_full_energy); the sweep row "
                                       "'fp32, accurate_v off' times the faster kernel") if prec == "fp32" else "n/a (FP64)",
