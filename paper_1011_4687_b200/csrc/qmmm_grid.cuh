@@ -76,9 +76,10 @@ __device__ __forceinline__ void on_lattice(double u, int i_lo, int i_hi, float &
 }
 
 // v += x with the rounding error of the sum kept (fast two-sum: exact when v's exponent is not
-// below x's, which holds from the second partial sum on; else the error term is itself rounded),
-// and d += dx - 2 error: V = v - d / 2 then holds the exact sum.  4 operations more than two
-// plain adds, once per 16 nodes: a quarter operation per pair.
+// below x's, which always holds from the third 16-node sum of a row on; where the second sum is
+// the larger one the error term may itself round -- an eighth of an ulp of the row sum at most,
+// tests/test_row_sum_identity.py), and d += dx - 2 error: V = v - d / 2 then holds the exact
+// sum.  4 operations more than two plain adds, once per 16 nodes: a quarter operation per pair.
 __device__ __forceinline__ void add_run(float2 &v, float2 &d, float2 x, float2 dx) {
     const float2 s = __fadd2_rn(v, x);
     const float2 bb = __ffma2_rn(v, bc(-1.0f), s);              // s - v
