@@ -289,7 +289,8 @@ qmmm_status qmmm_field_set_local_lattice(qmmm_field *h, int mode);
  * row sums misses (3.1e-5: a common bias of +1.9e-9 hartree per point and 6.7e-8 rms).
  * enable != 0 (default): r^2 = rxy2 + z2 with rxy2 formed in FP64 per (point, row) and z2 from a
  * second per-CTA table, both rounded once, and the last level of the FP32 row sums added with a
- * two-sum (as in the potential-only kernel): 2.6e-8 rms, +3.6e-10 mean, 5.8e-6 over the batch,
+ * two-sum (as in the potential-only kernel): 2.6e-8 rms, +3.6e-10 mean, 5.8e-6 over the batch
+ * (1.5e-6 ... 1.3e-5 over six seeded batches of that size: 24-bit r^2 leaves about 6e-6 +- 3.4e-6),
  * at 5.6 % more time (configs[3]: 5.60 instead of 5.30 ms).  enable = 0: the faster kernel
  * (every per-configuration energy still within 2e-6 hartree).  E agrees between the two to FP32
  * rounding (1e-7 relative).  Used when both tables fit in shared memory beside a pipeline of at
