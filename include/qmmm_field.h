@@ -295,7 +295,8 @@ qmmm_status qmmm_field_set_local_lattice(qmmm_field *h, int mode);
  * (every per-configuration energy still within 2e-6 hartree).  E agrees between the two to FP32
  * rounding (1e-7 relative).  Used when both tables fit in shared memory beside a pipeline of at
  * least two stages (z axes of up to 192 nodes: every FP32 BASELINE configuration), else the
- * faster kernel runs.  Sticky; shared handles inherit the parent's setting at qmmm_field_share.
+ * faster kernel runs (qmmm_field_info.last_accurate_v tells which one the last evaluation ran).
+ * Sticky; shared handles inherit the parent's setting at qmmm_field_share.
  */
 qmmm_status qmmm_field_set_accurate_v(qmmm_field *h, int enable);
 
@@ -362,6 +363,8 @@ typedef struct {
                                   * without synchronising; the host-buffer calls return QMMM_ERR_CUDA. */
     int32_t last_local_lattice;  /* 1: the most recent eval ran the FP32 grid kernel with a coordinate
                                   * lattice per work unit (qmmm_field_set_local_lattice) */
+    int32_t last_accurate_v;     /* 1: the most recent eval ran an FP32 grid kernel with the accurate-V
+                                  * arithmetic (qmmm_field_set_accurate_v; also the potential-only kernel) */
     char last_kernel[192];       /* mangled name of the kernel the most recent evaluation launched (or of
                                   * the move server it started): which template instantiation ran */
 } qmmm_field_info;

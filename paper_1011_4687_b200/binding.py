@@ -54,7 +54,8 @@ class qmmm_field_info(ctypes.Structure):
                 ("last_plan", qmmm_plan), ("last_point_blocks", ctypes.c_int32),
                 ("last_launches", ctypes.c_int32), ("sm_count", ctypes.c_int32),
                 ("last_dz_table", ctypes.c_int32), ("device_errors", ctypes.c_int32),
-                ("last_local_lattice", ctypes.c_int32), ("last_kernel", ctypes.c_char * 192)]
+                ("last_local_lattice", ctypes.c_int32), ("last_accurate_v", ctypes.c_int32),
+                ("last_kernel", ctypes.c_char * 192)]
 
 
 class qmmm_grid_info(ctypes.Structure):

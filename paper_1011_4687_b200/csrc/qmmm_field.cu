@@ -224,6 +224,7 @@ struct qmmm_field {
     int local_lattice = -1;        // FP32 grid kernel, lattice per gchunk: -1 automatic, 0 off, 1 on
     int last_local_lattice = 0;
     int accurate_v = 1;            // FP32 batched grid V + E kernel: accurate V (qmmm_field_set_accurate_v)
+    int last_accurate_v = 0;
     const char *last_kernel = "";  // mangled name of the kernel the most recent evaluation ran
     // device error word (pinned, device-mapped): set by a kernel whose bounded wait gave up
     int *dev_err_h = nullptr, *dev_err_d = nullptr;
@@ -1415,6 +1416,7 @@ qmmm_status qmmm_field_get_info(const qmmm_field *h, qmmm_field_info *info) {
     info->sm_count = h->sm_count;
     info->last_dz_table = h->last_dz_table;
     info->last_local_lattice = h->last_local_lattice;
+    info->last_accurate_v = h->last_accurate_v;
     info->device_errors = h->dev_err_h ? *reinterpret_cast<volatile int *>(h->dev_err_h) : 0;
     std::strncpy(info->last_kernel, h->last_kernel ? h->last_kernel : "", sizeof(info->last_kernel) - 1);
     return QMMM_OK;
@@ -1571,6 +1573,9 @@ qmmm_status eval_impl(qmmm_field *h, const double *elec_xyz, int64_t W, int64_t 
     h->last_point_blocks = pb;
     h->last_launches = launches;
     h->last_dz_table = use_dzt ? 1 : 0;
+    // (potential-only evaluations of batched FP32 grids always run the compensated kernel)
+    h->last_accurate_v = (use_accv || (use_dzt && f32 && !E && !light && pl.points_per_thread == 4 &&
+                                       pl.point_warps == GRID_NW_EPT4)) ? 1 : 0;
     return QMMM_OK;
 }
 }  // namespace

@@ -301,14 +301,17 @@ def test_config3_grid_fp32_full_energy(torch_cuda, B, oracle_mod, full_oracle):
         V, E = run(torch_cuda, B, h, pts, "fp32")
         assert B.qmmm_field_get_grid_info(h)["last_layout"] == "grid"
         assert "ELb0ELb1EEEv" in B.qmmm_field_get_info(h)["last_kernel"]  # <2, 8, false, true, true, 0, false, ACCV = true>
+        assert B.qmmm_field_get_info(h)["last_accurate_v"] == 1
         B.qmmm_field_set_accurate_v(h, False)     # the faster V + E kernel (same E; V to 7e-8 rms instead of 3e-8)
         Vf, Ef = run(torch_cuda, B, h, pts, "fp32")
         assert "ELb0ELb0EEEv" in B.qmmm_field_get_info(h)["last_kernel"]
+        assert B.qmmm_field_get_info(h)["last_accurate_v"] == 0
         B.qmmm_field_set_accurate_v(h, True)
         Vl, El = run(torch_cuda, B, h, pts, "fp32", layout="list")
         # E = NULL: the potential-only kernel (Eq. 4 proper; no lattice, 6 operations per pair)
         Vp, _ = run(torch_cuda, B, h, pts, "fp32", want_E=False, layout="auto")
         assert "ELb1ELb0EEEv" in B.qmmm_field_get_info(h)["last_kernel"]  # <2, 8, false, true, true, 0, VONLY = true, false>
+        assert B.qmmm_field_get_info(h)["last_accurate_v"] == 1
         U = torch_cuda.zeros(w.W, dtype=torch_cuda.float64, device="cuda")
         B.qmmm_field_eval_energy(h, torch_cuda.from_numpy(pts).cuda(), w.W, w.N, U, "fp32")
         torch_cuda.cuda.synchronize()
