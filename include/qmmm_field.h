@@ -147,6 +147,30 @@ qmmm_status qmmm_field_eval_host(qmmm_field *h, const double *elec_xyz_host, int
                                  void *stream);
 
 /*
+ * qmmm_field_eval_move_host -- one single-electron move of the QMC loop (the
+ * Metropolis step needs U_ES(r_new) - U_ES(r_old), Eq. 4): the potential and field
+ * at r_new and their change from r_old, dV = V(r_new) - V(r_old) (the change of the electron's
+ * electrostatic energy is -dV) and dE = E(r_new) - E(r_old), in one call with HOST buffers.
+ *   r_old, r_new   HOST [3]       the electron's position before and after the proposed move
+ *   V_old, E_old   HOST [1], [3]  V and E at r_old as a previous call returned them (V_new, E_new
+ *                                 of the accepted move), or NULL: then r_old is evaluated too, in
+ *                                 the SAME launch as r_new (one two-point evaluation, not two)
+ *   V_new, E_new   HOST [1], [3]  out: V(r_new), E(r_new); E_new may be NULL (potential only:
+ *                                 E_old and dE are then ignored)
+ *   dV, dE         HOST [1], [3]  out: the differences; each may be NULL
+ * With V_old (and E_old when E_new is wanted) this is the one-point call of qmmm_field_eval_host
+ * -- the resident move server, 6-7 us per move on configs[2] -- plus a subtraction on the host;
+ * without them it is the two-point launch path of qmmm_field_eval_host.  Accuracy: V and E as for
+ * qmmm_field_eval; dV carries the absolute error of the two potentials (a difference of nearly
+ * equal numbers), not a relative one.  Errors as qmmm_field_eval_host (the handle needs
+ * max_points >= 2 for the two-point form).
+ */
+qmmm_status qmmm_field_eval_move_host(qmmm_field *h, const double *r_old, const double *r_new,
+                                      const double *V_old, const double *E_old, double *V_new,
+                                      double *E_new, double *dV, double *dE, int precision,
+                                      void *stream);
+
+/*
  * qmmm_field_eval_moves_host -- n successive single-configuration evaluations, the loop the
  * paper deploys (every Monte-Carlo step sends r_new and receives U_ES).  Step s
  * evaluates the N points elec_xyz_host[s][N][3] and writes V_host[s][N] (and E_host[s][N][3]

@@ -26,7 +26,7 @@ _STATUS = {0: "QMMM_OK", 1: "QMMM_ERR_INVALID_ARG", 2: "QMMM_ERR_ALLOC", 3: "QMM
 LIB_PATH = os.environ.get("QMMM_FIELD_LIB") or os.path.join(
     os.path.dirname(os.path.abspath(__file__)), "libqmmm_field.so")
 EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_host",
-                    "qmmm_field_eval_moves_host", "qmmm_field_create_grid", "qmmm_field_eval_energy",
+                    "qmmm_field_eval_moves_host", "qmmm_field_eval_move_host", "qmmm_field_create_grid", "qmmm_field_eval_energy",
                     "qmmm_field_eval_moves",
                     "qmmm_field_share", "qmmm_field_create_grid3",
                     "qmmm_field_set_layout", "qmmm_field_get_grid_info",
@@ -86,6 +86,8 @@ def _load() -> ctypes.CDLL:
     lib.qmmm_field_eval_energy.argtypes = [vp, vp, i64, i64, vp, ci, vp]
     lib.qmmm_field_eval_host.restype = ci
     lib.qmmm_field_eval_host.argtypes = [vp, vp, i64, i64, vp, vp, ci, vp]
+    lib.qmmm_field_eval_move_host.restype = ci
+    lib.qmmm_field_eval_move_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, ci, vp]
     lib.qmmm_field_eval_moves_host.restype = ci
     lib.qmmm_field_eval_moves_host.argtypes = [vp, vp, i64, i64, vp, vp, ci, vp,
                                                ctypes.POINTER(ctypes.c_double)]
@@ -235,6 +237,16 @@ def qmmm_field_eval_host(handle: int, elec_xyz, W: int, N: int, V, E=None, preci
     """Per-step host loop of PAPER.md:117: host buffers in/out, synchronises the stream."""
     _check(_lib.qmmm_field_eval_host(handle, _ptr(elec_xyz), int(W), int(N), _ptr(V), _ptr(E),
                                      _PREC[precision], _stream(stream)))
+
+
+def qmmm_field_eval_move_host(handle: int, r_old, r_new, V_old=None, E_old=None, V_new=None, E_new=None,
+                              dV=None, dE=None, precision="fp64", stream=None) -> None:
+    """One single-electron move: V, E at r_new and their change from r_old; host
+    arrays (numpy float64).  V_old / E_old = the values a previous call returned at r_old, or None:
+    then both points are evaluated in one launch.  Argument marshalling only."""
+    _check(_lib.qmmm_field_eval_move_host(handle, _ptr(r_old), _ptr(r_new), _ptr(V_old), _ptr(E_old),
+                                          _ptr(V_new), _ptr(E_new), _ptr(dV), _ptr(dE),
+                                          _PREC[precision], _stream(stream)))
 
 
 def qmmm_field_eval_moves_host(handle: int, elec_xyz, n: int, N: int, V, E=None, precision="fp64",

@@ -1747,6 +1747,38 @@ qmmm_status qmmm_debug_phases(qmmm_field *h, long long *out, int n) {
 }
 #endif
 
+qmmm_status qmmm_field_eval_move_host(qmmm_field *h, const double *r_old, const double *r_new,
+                                      const double *V_old, const double *E_old, double *V_new,
+                                      double *E_new, double *dV, double *dE, int prec, void *stream) {
+    if (!h) return fail(QMMM_ERR_INVALID_ARG, "eval_move_host: NULL handle");
+    if (!r_old || !r_new || !V_new) return fail(QMMM_ERR_INVALID_ARG, "eval_move_host: NULL r_old, r_new or V_new");
+    double Vo = 0.0, Eo[3] = {0.0, 0.0, 0.0};
+    if (V_old && (!E_new || E_old)) {
+        // the caller knows the old values: one point, the resident move server
+        qmmm_status s = qmmm_field_eval_host(h, r_new, 1, 1, V_new, E_new, prec, stream);
+        if (s != QMMM_OK) return s;
+        Vo = *V_old;
+        if (E_new) std::memcpy(Eo, E_old, sizeof(Eo));
+    } else {
+        // both points in one launch
+        double pts[6], V2[2], E2[6];
+        std::memcpy(pts, r_old, 3 * sizeof(double));
+        std::memcpy(pts + 3, r_new, 3 * sizeof(double));
+        qmmm_status s = qmmm_field_eval_host(h, pts, 1, 2, V2, E_new ? E2 : nullptr, prec, stream);
+        if (s != QMMM_OK) return s;
+        Vo = V2[0];
+        *V_new = V2[1];
+        if (E_new) {
+            std::memcpy(Eo, E2, sizeof(Eo));
+            std::memcpy(E_new, E2 + 3, 3 * sizeof(double));
+        }
+    }
+    if (dV) *dV = *V_new - Vo;
+    if (dE && E_new)
+        for (int k = 0; k < 3; ++k) dE[k] = E_new[k] - Eo[k];
+    return QMMM_OK;
+}
+
 qmmm_status qmmm_field_eval_moves_host(qmmm_field *h, const double *elec_xyz_host, int64_t n,
                                        int64_t N, double *V_host, double *E_host, int prec,
                                        void *stream, double *seconds) {

@@ -387,6 +387,50 @@ def test_config2_all_1000_moves_host_loop_and_device_sequence(torch_cuda, B, ora
         B.qmmm_field_destroy(h)
 
 
+def test_eval_move_host_against_the_oracle(torch_cuda, B, oracle_mod):
+    """qmmm_field_eval_move_host (dU = U(r_new) - U(r_old) in one call): 40
+    moves of configs[2]'s random walk.  Both forms -- the old values handed back in (one-point
+    evaluation, resident move server) and NULL (both points in one launch) -- both precisions,
+    potential only as well; V_new, E_new as qmmm_field_eval, dV and dE within the absolute error of
+    the two values they are differences of."""
+    w = make_workload(2, n_points=(41, 1))
+    pts = np.ascontiguousarray(w.elec_xyz.reshape(-1, 3))
+    ref = oracle_of(oracle_mod, w, pts)
+    h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 2)
+    try:
+        for prec, tol in (("fp32", TOL32), ("fp64", TOL64)):
+            for form in ("old values given", "both evaluated"):
+                Vn = np.full(41, np.nan); En = np.full((41, 3), np.nan)
+                dV = np.full(41, np.nan); dE = np.full((41, 3), np.nan)
+                B.qmmm_field_eval_host(h, pts[0:1], 1, 1, Vn[0:1], En[0:1], prec)        # the walk's start
+                for i in range(1, 41):
+                    given = form == "old values given"
+                    B.qmmm_field_eval_move_host(h, pts[i - 1], pts[i],
+                                                Vn[i - 1:i] if given else None, En[i - 1] if given else None,
+                                                Vn[i:i + 1], En[i], dV[i:i + 1], dE[i], prec)
+                    name = B.qmmm_field_get_info(h)["last_kernel"]
+                    assert ("move_server" in name) == given, (form, name)
+                check(ref, Vn, En, tol)
+                # differences: absolute error of the two values
+                want_dV = ref.V[1:] - ref.V[:-1]
+                want_dE = ref.E[1:] - ref.E[:-1]
+                assert np.all(np.abs(dV[1:] - want_dV) <= tol * (np.abs(ref.V[1:]) + np.abs(ref.V[:-1]))), (prec, form)
+                nE = np.linalg.norm(ref.E[1:], axis=1) + np.linalg.norm(ref.E[:-1], axis=1)
+                assert np.all(np.linalg.norm(dE[1:] - want_dE, axis=1) <= tol * nE), (prec, form)
+                if given:         # exactly the difference of the values handed in and out
+                    assert np.array_equal(dV[1:], Vn[1:] - Vn[:-1]) and np.array_equal(dE[1:], En[1:] - En[:-1])
+            # potential only: E_new = NULL, E_old and dE ignored
+            v = np.zeros(1); d = np.zeros(1)
+            B.qmmm_field_eval_move_host(h, pts[3], pts[4], None, None, v, None, d, None, prec)
+            assert abs(v[0] - ref.V[4]) <= tol * abs(ref.V[4])
+            assert abs(d[0] - (ref.V[4] - ref.V[3])) <= tol * (abs(ref.V[4]) + abs(ref.V[3]))
+        with pytest.raises(B.QmmmError):
+            B.qmmm_field_eval_move_host(h, None, pts[1], None, None, np.zeros(1), None, None, None, "fp64")
+        assert B.qmmm_field_get_info(h)["device_errors"] == 0
+    finally:
+        B.qmmm_field_destroy(h)
+
+
 @pytest.mark.parametrize("handle_kind", ["list+grid", "create_grid"])
 def test_grid_aware_move_server(torch_cuda, B, oracle_mod, handle_kind):
     """Single-point eval_host calls on an environment with the grid-aware copy are served by the
