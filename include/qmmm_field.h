@@ -285,6 +285,21 @@ qmmm_status qmmm_field_share(const qmmm_field *parent, int64_t max_points, qmmm_
 qmmm_status qmmm_sum_rank_partials(const double *parts, int64_t R, int64_t n, double *out, void *stream);
 
 /*
+ * qmmm_field_min_distance -- debug helper, not part of the hot path (SURVEY.md 8(b) "r = 0"): the
+ * smallest distance, in bohr, between the P evaluation points and the CHARGED sources of the
+ * handle (cells with q != 0 and nuclei with Z != 0).  The evaluation has no softening and no
+ * exclusion (PAPER.md:59 has none): a point on a source gives IEEE inf / NaN, and the FP32 bound
+ * on |E| asks for a clearance of two cell edges (qmmm_precision above); this is the call that
+ * checks such preconditions.  Brute force over all pairs in FP64, one kernel on `stream`, then a
+ * stream synchronisation; allocates and frees 8 bytes of device memory.
+ *   elec_xyz           DEVICE [P][3] FP64
+ *   min_distance_host  HOST   [1]    out; +inf for an environment without charged sources
+ * INVALID_ARG for NULL pointers or P < 1 (P is not limited by max_points).
+ */
+qmmm_status qmmm_field_min_distance(qmmm_field *h, const double *elec_xyz, int64_t P,
+                                    double *min_distance_host, void *stream);
+
+/*
  * FP32 grid kernels: granularity of the coordinate lattice.  The FP32 path keeps every
  * difference (point - node) EXACT by rounding the point's coordinates to a power-of-two lattice
  * and corrects V for the rounding residual to first order; E is evaluated at the lattice point

@@ -33,7 +33,7 @@ EXPORTED_SYMBOLS = ("qmmm_field_create", "qmmm_field_eval", "qmmm_field_eval_hos
                     "qmmm_field_destroy", "qmmm_field_set_plan", "qmmm_field_get_info",
                     "qmmm_field_set_timing", "qmmm_field_last_timing", "qmmm_field_set_overlap",
                     "qmmm_field_set_local_lattice", "qmmm_field_set_accurate_v", "qmmm_field_eval_noalloc",
-                    "qmmm_sum_rank_partials", "qmmm_probe_peak", "qmmm_last_error")
+                    "qmmm_field_min_distance", "qmmm_sum_rank_partials", "qmmm_probe_peak", "qmmm_last_error")
 
 
 class QmmmError(RuntimeError):
@@ -86,6 +86,8 @@ def _load() -> ctypes.CDLL:
     lib.qmmm_field_eval_energy.argtypes = [vp, vp, i64, i64, vp, ci, vp]
     lib.qmmm_field_eval_host.restype = ci
     lib.qmmm_field_eval_host.argtypes = [vp, vp, i64, i64, vp, vp, ci, vp]
+    lib.qmmm_field_min_distance.restype = ci
+    lib.qmmm_field_min_distance.argtypes = [vp, vp, i64, ctypes.POINTER(ctypes.c_double), vp]
     lib.qmmm_field_eval_move_host.restype = ci
     lib.qmmm_field_eval_move_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, ci, vp]
     lib.qmmm_field_eval_moves_host.restype = ci
@@ -237,6 +239,15 @@ def qmmm_field_eval_host(handle: int, elec_xyz, W: int, N: int, V, E=None, preci
     """Per-step host loop of PAPER.md:117: host buffers in/out, synchronises the stream."""
     _check(_lib.qmmm_field_eval_host(handle, _ptr(elec_xyz), int(W), int(N), _ptr(V), _ptr(E),
                                      _PREC[precision], _stream(stream)))
+
+
+def qmmm_field_min_distance(handle: int, elec_xyz, stream=None) -> float:
+    """Debug helper: smallest distance (bohr) between the points (device tensor [P,3]) and the
+    charged sources of the handle."""
+    out = ctypes.c_double()
+    _check(_lib.qmmm_field_min_distance(handle, _ptr(elec_xyz), int(elec_xyz.numel() // 3), ctypes.byref(out),
+                                        _stream(stream)))
+    return out.value
 
 
 def qmmm_field_eval_move_host(handle: int, r_old, r_new, V_old=None, E_old=None, V_new=None, E_new=None,

@@ -1747,6 +1747,89 @@ qmmm_status qmmm_debug_phases(qmmm_field *h, long long *out, int n) {
 }
 #endif
 
+// ---- debug helper: smallest distance between the evaluation points and the charged sources ----
+namespace {
+constexpr int MIND_POINTS = 64;       // points per CTA (shared memory)
+// Sources are enumerated from the FP64 list copy ([chunk][x, y, z, q][128], cells then nuclei) or,
+// for handles without one, from the FP64 grid copy ([gchunk][ZS/2][32 rows][2]) plus the nuclei.
+// Squared distances are >= 0, so their bit patterns order like unsigned integers: the minimum is
+// taken with an integer atomic (order-independent, hence deterministic).
+__global__ void __launch_bounds__(256) min_distance_kernel(const double *elec, int64_t P, const double *chunks64,
+                                                           int64_t n_list, const double *gcells64, int64_t n_nodes,
+                                                           qmmm::GridGeom gg, int g_segs, const double *nuclei,
+                                                           int64_t K, unsigned long long *out) {
+    __shared__ double pt[MIND_POINTS][3];
+    const int64_t p0 = static_cast<int64_t>(blockIdx.x) * MIND_POINTS;
+    const int np = static_cast<int>(P - p0 < MIND_POINTS ? P - p0 : MIND_POINTS);
+    for (int i = threadIdx.x; i < np * 3; i += blockDim.x) pt[i / 3][i % 3] = elec[p0 * 3 + i];
+    __syncthreads();
+    double best = __longlong_as_double(0x7ff0000000000000ll);            // +inf
+    auto visit = [&](double x, double y, double z) {
+        for (int i = 0; i < np; ++i) {
+            const double dx = pt[i][0] - x, dy = pt[i][1] - y, dz = pt[i][2] - z;
+            const double d2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            best = d2 < best ? d2 : best;
+        }
+    };
+    const int64_t stride = static_cast<int64_t>(gridDim.y) * blockDim.x;
+    const int64_t first = static_cast<int64_t>(blockIdx.y) * blockDim.x + threadIdx.x;
+    if (chunks64) {
+        for (int64_t j = first; j < n_list; j += stride) {
+            const double *c = chunks64 + (j / 128) * 512 + (j % 128);
+            if (c[384] != 0.0) visit(c[0], c[128], c[256]);
+        }
+    } else {
+        const int ny = gg.n[1];
+        for (int64_t j = first; j < n_nodes; j += stride) {
+            if (gcells64[j] == 0.0) continue;
+            const int64_t c = j / qmmm::GRID_NODES;
+            const int i = static_cast<int>(j % qmmm::GRID_NODES);
+            const int64_t row = (c / g_segs) * 32 + (i / 2) % 32;
+            const int iz = static_cast<int>(c % g_segs) * qmmm::GRID_ZS + 2 * (i / 64) + (i & 1);
+            visit(gg.org[0] + gg.h[0] * static_cast<double>(row / ny), gg.org[1] + gg.h[1] * static_cast<double>(row % ny),
+                  gg.org[2] + gg.h[2] * static_cast<double>(iz));
+        }
+        for (int64_t j = first; j < K; j += stride)
+            if (nuclei[4 * j + 3] != 0.0) visit(nuclei[4 * j], nuclei[4 * j + 1], nuclei[4 * j + 2]);
+    }
+    for (int m = 16; m >= 1; m >>= 1) {
+        const double o = __shfl_xor_sync(0xffffffffu, best, m);
+        best = o < best ? o : best;
+    }
+    if ((threadIdx.x & 31) == 0) atomicMin(out, static_cast<unsigned long long>(__double_as_longlong(best)));
+}
+}  // namespace
+
+qmmm_status qmmm_field_min_distance(qmmm_field *h, const double *elec_xyz, int64_t P, double *min_distance_host,
+                                    void *stream) {
+    if (!h) return fail(QMMM_ERR_INVALID_ARG, "min_distance: NULL handle");
+    if (!elec_xyz || !min_distance_host) return fail(QMMM_ERR_INVALID_ARG, "min_distance: NULL elec_xyz or result");
+    if (P < 1) return fail(QMMM_ERR_INVALID_ARG, "min_distance: P must be >= 1");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    unsigned long long *out_d = nullptr, out_h = 0x7ff0000000000000ull;
+    CUDA_TRY(cudaMalloc(&out_d, sizeof(out_h)));
+    cudaError_t e = cudaMemcpyAsync(out_d, &out_h, sizeof(out_h), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && h->M + h->K > 0) {
+        const bool list = h->has_list && h->chunks64;
+        const int64_t n_list = h->n_chunks64 * 128, n_nodes = h->n_g * qmmm::GRID_NODES;
+        const int64_t n_src = list ? n_list : n_nodes + h->K;
+        const unsigned gx = static_cast<unsigned>((P + MIND_POINTS - 1) / MIND_POINTS);
+        unsigned gy = static_cast<unsigned>(std::min<int64_t>((n_src + 255) / 256, std::max<int64_t>(1, 8 * h->sm_count / gx)));
+        if (gy < 1) gy = 1;
+        min_distance_kernel<<<dim3(gx, gy), 256, 0, st>>>(elec_xyz, P, list ? h->chunks64 : nullptr, n_list, h->gcells64,
+                                                        n_nodes, h->grid, static_cast<int>(h->g_segs), h->nuclei, h->K, out_d);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&out_h, out_d, sizeof(out_h), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(out_d);
+    if (e != cudaSuccess) return cuda_fail(e, "min_distance");
+    double d2;
+    std::memcpy(&d2, &out_h, sizeof(d2));
+    *min_distance_host = std::sqrt(d2);
+    return QMMM_OK;
+}
+
 qmmm_status qmmm_field_eval_move_host(qmmm_field *h, const double *r_old, const double *r_new,
                                       const double *V_old, const double *E_old, double *V_new,
                                       double *E_new, double *dV, double *dE, int prec, void *stream) {

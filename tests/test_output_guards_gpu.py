@@ -103,3 +103,62 @@ def test_noalloc_outputs_stay_inside_their_buffers():
         assert guards_intact(vb, P) and guards_intact(eb, 3 * P), P
         assert bool(torch.isfinite(V).all()) and bool(torch.isfinite(Ef).all()), P
         assert not bool((V == SENTINEL).any()) and not bool((Ef == SENTINEL).any()), P
+
+
+def test_min_distance_helper_against_brute_force():
+    """qmmm_field_min_distance (debug helper, SURVEY.md 8(b) "r = 0"): the smallest distance between
+    the points and the CHARGED sources -- source-list handles (cells and nuclei; pads and empty
+    cells do not count), grid-only handles (qmmm_field_create_grid), ragged point counts, a point
+    placed on a cell, and an environment without sources -- against numpy."""
+    import torch
+    from paper_1011_4687_b200 import binding as B
+    rng = np.random.default_rng(77)
+
+    def brute(pts, *sources):
+        best = np.inf
+        for xyz, q in sources:
+            keep = np.asarray(q) != 0.0
+            if keep.any():
+                d = np.linalg.norm(pts[:, None, :] - np.asarray(xyz)[keep][None, :, :], axis=2)
+                best = min(best, float(d.min()))
+        return best
+
+    for idx in (0, 1):
+        w = make_workload(idx)
+        h = B.qmmm_field_create(w.src_xyz, w.src_q, w.nuc_xyz, w.nuc_Z, 8)
+        try:
+            for P in (1, 5, 64, 65, 200):                       # P is not limited by max_points
+                pts = rng.normal(size=(P, 3)) * 1.5
+                got = B.qmmm_field_min_distance(h, torch.from_numpy(pts).cuda())
+                want = brute(pts, (w.src_xyz, w.src_q), (w.nuc_xyz, w.nuc_Z))
+                assert abs(got - want) <= 1e-12 * want, (idx, P, got, want)
+            pts = rng.normal(size=(7, 3))
+            pts[3] = w.src_xyz[np.flatnonzero(w.src_q)[11]]      # a point ON a charged cell
+            assert B.qmmm_field_min_distance(h, torch.from_numpy(pts).cuda()) == 0.0
+        finally:
+            B.qmmm_field_destroy(h)
+    # grid-only handle: 20 x 13 x 70 nodes with empty cells, orthorhombic spacing, 3 nuclei
+    n, hh, origin = (20, 13, 70), np.array([0.3, 0.25, 0.2]), np.array([-3.0, -1.5, -7.0])
+    dense = -rng.random(n) * 1e-2
+    dense[rng.random(n) > 0.6] = 0.0
+    idx3 = np.stack(np.meshgrid(*[np.arange(k) for k in n], indexing="ij"), axis=-1)
+    pos = (origin + hh * idx3).reshape(-1, 3)
+    nuc = rng.normal(size=(3, 3)) * 2.0
+    Z = np.array([1.0, 0.0, 8.0])                                # a nucleus of charge 0 does not count
+    h = B.qmmm_field_create_grid(origin, tuple(hh), n, np.ascontiguousarray(dense), nuc, Z, 4)
+    try:
+        assert not B.qmmm_field_get_grid_info(h)["has_list"]
+        for P in (1, 33, 130):
+            pts = rng.normal(size=(P, 3)) * 2.0
+            got = B.qmmm_field_min_distance(h, torch.from_numpy(pts).cuda())
+            want = brute(pts, (pos, dense.reshape(-1)), (nuc, Z))
+            assert abs(got - want) <= 1e-12 * want, (P, got, want)
+    finally:
+        B.qmmm_field_destroy(h)
+    h = B.qmmm_field_create(None, None, None, None, 4)           # nothing to be near to
+    try:
+        assert B.qmmm_field_min_distance(h, torch.zeros((3, 3), dtype=torch.float64, device="cuda")) == np.inf
+        with pytest.raises(B.QmmmError):
+            B.qmmm_field_min_distance(h, torch.zeros((0, 3), dtype=torch.float64, device="cuda"))
+    finally:
+        B.qmmm_field_destroy(h)
