@@ -50,6 +50,22 @@ SLOTS = {("list", "fp32"): 14, ("list", "fp64"): 18, ("grid", "fp32"): 9, ("grid
 # (round 1 printed 13; the SASS count of tests/test_sass_slots.py says 12).
 SLOTS_V_ONLY = {"list": 12, "grid": 8}
 SLOTS_V_ONLY_F32_GRID = 6                  # FP32 potential only, batched grid kernel: r^2, a, V0, y0^2, c, T
+# Floating-point operations per pair of the same kernels (an fma counts 2), for readers who count
+# flops (SURVEY.md 8(d) "eta_flop").  (layout, precision, dz table, potential only).  FP32 grid with
+# the table, V + E: r^2 2 (1 when it is an add: accurate V), a 1, V0 1, y0^2 1, c 1, T 2, S 1, SZ 2 = 11;
+# FP64 grid with the table: r^2 2, refinement 8, p 1, V 1, y^2 1, s 1, S 1, SZ 2 = 17.
+FLOPS = {("list", "fp32", False, False): 21, ("list", "fp64", False, False): 27, ("list", "fp64", False, True): 19,
+         ("grid", "fp32", False, False): 12, ("grid", "fp32", True, False): 11, ("grid", "fp32", True, True): 7,
+         ("grid", "fp64", False, False): 18, ("grid", "fp64", True, False): 17,
+         ("grid", "fp64", False, True): 12, ("grid", "fp64", True, True): 11}
+
+
+def flops_for(layout, prec, info, v_only=False):
+    key = (layout, prec, bool(info.get("last_dz_table")) and layout == "grid", bool(v_only))
+    n = FLOPS.get(key, FLOPS.get((layout, prec, key[2], False)))
+    if key == ("grid", "fp32", True, False) and info.get("last_accurate_v"):
+        n -= 1                                   # accurate V: r^2 = rxy2 + z2 is an add, not an fma
+    return n
 
 
 def slots_for(layout, prec, info, v_only=False):
@@ -637,6 +653,11 @@ def run_ours(args):
                          # 18 FP64 slots: list of positions, per-pair refinement); above 1 when the
                          # kernel needs fewer operations than that formulation
                          "frac_at_survey_slots": P * w.M * (17 if prec == "fp32" else 18) / pair_s / peak_lane,
+                         # the flop-counting view (SURVEY.md 8(d) eta_flop): the kernel's own flops per
+                         # pair (an fma = 2) and, for FP32, the survey's fixed 24, over 2 x the lane rate
+                         "flops_per_pair": flops_for(layout, prec, info, v_only=args.potential_only),
+                         "eta_flop": P * w.M * flops_for(layout, prec, info, v_only=args.potential_only) / pair_s / (2 * peak_lane),
+                         "eta_flop_at_survey_24": (P * w.M * 24 / pair_s / (2 * peak_lane)) if prec == "fp32" else None,
                          # one MUFU (RSQ / RSQ64H) per pair against the measured MUFU rate: the
                          # co-limiter of the FP32 grid kernel
                          "xu_frac": P * w.M / pair_s / (0.5 * (peaks0["mufu_lane_ops_per_s"] + peaks1["mufu_lane_ops_per_s"])),
