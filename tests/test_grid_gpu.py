@@ -858,3 +858,33 @@ def test_config2_single_point_device_evaluations(torch_cuda, B, oracle_mod, prec
         assert abs(Vl[0] - V[0]) <= 2 * tol * abs(V[0])
     finally:
         B.qmmm_field_destroy(h)
+
+
+def test_accurate_v_and_potential_only_on_orthorhombic_cells(torch_cuda, B, oracle_mod):
+    """The batched FP32 table kernels that form rxy2 in FP64 from the points' true coordinates
+    (accurate V, the default; potential only) on cells that are not cubic (0.3 x 0.2 x 0.25 bohr,
+    24 x 40 x 70 nodes: two z segments, empty cells): against the oracle, with the faster V + E
+    kernel beside them; qmmm_field_info.last_accurate_v says which one ran."""
+    rng = np.random.default_rng(5)
+    n, hh = (24, 40, 70), np.array([0.3, 0.2, 0.25])
+    origin = np.array([1.0, -2.0, 0.5])
+    centre = origin + 0.5 * hh * (np.array(n) - 1)
+    dense, pos, q = random_grid(rng, n, hh, origin, fill=0.7, hole=(centre, 1.6))
+    P = 300
+    pts = centre + rng.normal(size=(P, 3)) * 0.5
+    pts = centre + (pts - centre) * np.minimum(1.0, 1.1 / np.linalg.norm(pts - centre, axis=1))[:, None]
+    ref = oracle_mod.field(pos, q, NO_XYZ, NO_Z, pts, want_abs=True)
+    h = B.qmmm_field_create_grid(origin, tuple(hh), n, dense, None, None, P)
+    try:
+        rms = {}
+        for want_E, accurate in ((True, True), (True, False), (False, True)):
+            B.qmmm_field_set_accurate_v(h, accurate)
+            V, E = run(torch_cuda, B, h, pts, "fp32", want_E=want_E, plan=dict(points_per_thread=4, point_warps=16))
+            check(ref, V, E, TOL32)
+            assert B.qmmm_field_get_info(h)["last_accurate_v"] == int(accurate)
+            assert B.qmmm_field_get_info(h)["last_dz_table"] == 1
+            rms[(want_E, accurate)] = float(np.std(V - ref.V))
+        assert rms[(True, True)] < 0.8 * rms[(True, False)]        # measured: 6.6e-8 against 1.2e-7
+        assert rms[(False, True)] < 0.8 * rms[(True, False)]
+    finally:
+        B.qmmm_field_destroy(h)
