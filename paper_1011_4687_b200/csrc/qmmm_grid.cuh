@@ -77,7 +77,7 @@ __device__ __forceinline__ void on_lattice(double u, int i_lo, int i_hi, float &
 
 // v += x with the rounding error of the sum kept (fast two-sum: exact when v's exponent is not
 // below x's, which always holds from the third 16-node sum of a row on; where the second sum is
-// the larger one the error term may itself round -- an eighth of an ulp of the row sum at most,
+// the larger one the error term may itself round -- half an ulp of that sum, in a minority of rows:
 // tests/test_row_sum_identity.py), and d += dx - 2 error: V = v - d / 2 then holds the exact
 // sum.  4 operations more than two plain adds, once per 16 nodes: a quarter operation per pair.
 __device__ __forceinline__ void add_run(float2 &v, float2 &d, float2 x, float2 dx) {
@@ -246,7 +246,9 @@ struct GridRowF32 {
     // point (partial sums 1 : 2 : 3 : 4 of nearly equal terms; reproduced by a CPU emulation
     // of the tree in IEEE float32), so there it is added with a fast
     // two-sum whose error term goes to d: a quarter operation per pair, +2.3 % time, rms of V
-    // on config 3 4.5e-8 -> 2.7e-8 and the batch total inside 1e-5 hartree.  ACCV: the same.
+    // on config 3 4.5e-8 -> 2.7e-8 and the batch total inside 1e-5 hartree; the level below it
+    // (4 -> 16) is added pairwise there, which takes its share of the drift away for nothing.
+    // ACCV: the same.
     // The other V + E walks keep plain adds: their error is dominated by the FP32 dz table and
     // rxy2 (6.7e-8 -> 6.4e-8 with the two-sum alone, at +3 % time).
     __device__ __forceinline__ void run(const float *b, int n4, float2 (&v)[EP2], float2 (&d)[EP2]) {
@@ -258,13 +260,33 @@ struct GridRowF32 {
             for (int g = 0; g < n4; g += 4) {
                 float2 v16[EP2], t16[EP2], Vc[EP2], Tc[EP2];
                 four(b + g * 128, v16, t16);
-#pragma unroll
-                for (int k4 = 1; k4 < 4; ++k4) {
-                    four(b + (g + k4) * 128, Vc, Tc);
+                if constexpr (COMP) {
+                    // the four 4-node sums pairwise, (f0 + f1) + (f2 + f3): the same three adds as
+                    // one after the other, without the 1 : 2 : 3 : 4 partial sums that drift
+                    // (+1.5e-10 hartree per point on config 3 at this level; 8 more live registers)
+                    float2 w[EP2], tw[EP2];
+                    four(b + (g + 1) * 128, Vc, Tc);
 #pragma unroll
                     for (int e = 0; e < EP2; ++e) {
                         v16[e] = __fadd2_rn(v16[e], Vc[e]);
                         t16[e] = __fadd2_rn(t16[e], Tc[e]);
+                    }
+                    four(b + (g + 2) * 128, w, tw);
+                    four(b + (g + 3) * 128, Vc, Tc);
+#pragma unroll
+                    for (int e = 0; e < EP2; ++e) {
+                        v16[e] = __fadd2_rn(v16[e], __fadd2_rn(w[e], Vc[e]));
+                        t16[e] = __fadd2_rn(t16[e], __fadd2_rn(tw[e], Tc[e]));
+                    }
+                } else {
+#pragma unroll
+                    for (int k4 = 1; k4 < 4; ++k4) {
+                        four(b + (g + k4) * 128, Vc, Tc);
+#pragma unroll
+                        for (int e = 0; e < EP2; ++e) {
+                            v16[e] = __fadd2_rn(v16[e], Vc[e]);
+                            t16[e] = __fadd2_rn(t16[e], Tc[e]);
+                        }
                     }
                 }
 #pragma unroll

@@ -9,8 +9,8 @@ compensated they keep, for every add s = fl(v + x), the error term er = (s - v) 
 
 * the fast two-sum is exact whenever |v| >= |x| (always from the third 16-node sum on): s - er ==
   v + x in exact arithmetic, so the compensated V equals the exactly summed 16-node sums; where
-  the second sum is the larger one the error term may itself round (an eighth of an ulp of the
-  row sum at most, in a minority of rows);
+  the second sum is the larger one the error term may itself round (half an ulp of that sum,
+  in a minority of rows);
 * T16 - V16 is exact (Sterbenz) when the two agree to a factor of two, as they do to 1e-6;
 * on slowly varying same-sign terms -- the shape of a row's terms -- the plain last level is
   off by rounding errors of the size the error terms account for, and the compensated value is
@@ -45,7 +45,8 @@ def row_terms(rng, n=64):
 
 
 def tree_16(a, t):
-    """The two lower levels (4 -> 16) in float32; t enters through an fma chain."""
+    """The two lower levels (4 -> 16) in float32: four nodes one after the other (t through an fma
+    chain), the four 4-node sums pairwise."""
     v16, t16 = [], []
     for g in range(0, len(a), 16):
         vs, ts = [], []
@@ -55,8 +56,8 @@ def tree_16(a, t):
             for j in range(k + 1, k + 4):
                 acc = f32(np.float64(acc) + t[j])                                    # fma(c, r2, acc): one rounding
             ts.append(acc)
-        v16.append(seq(vs))
-        t16.append(seq(ts))
+        v16.append(f32(f32(vs[0] + vs[1]) + f32(vs[2] + vs[3])))                    # pairwise, as the compensated kernels
+        t16.append(f32(f32(ts[0] + ts[1]) + f32(ts[2] + ts[3])))
     return v16, t16
 
 
@@ -91,9 +92,10 @@ def test_two_sum_last_level_returns_the_exact_sum_of_the_16_node_sums():
         V_plain = 1.5 * float(vp) - 0.5 * float(tp)
         ulp = float(np.spacing(f32(abs(V_exact))))
         # d's own rounding only -- or, where the one two-sum outside the exact regime was inexact,
-        # half an ulp of the FIRST 16-node sum, an eighth of the row sum's
+        # half an ulp of the SECOND 16-node sum (at most half an ulp of the row sum, when that
+        # group holds most of the row)
         inexact_rows += not all_exact
-        assert abs(V_comp - V_exact) <= (0.02 if all_exact else 0.3) * ulp, (V_comp, V_exact, ulp)
+        assert abs(V_comp - V_exact) <= (0.02 if all_exact else 0.51) * ulp, (V_comp, V_exact, ulp)
         assert abs(V_plain - V_exact) <= 2.5 * ulp
         worse += abs(V_plain - V_exact) > abs(V_comp - V_exact)
     assert worse >= 200           # the plain level is off by a good fraction of an ulp in most rows
