@@ -61,9 +61,9 @@ typedef enum {
  *                     no FP32 arithmetic can do better than ~1e-7 x sum |q|/r^2).  E = NULL on
  *                     a grid runs a potential-only kernel (6 instead of 8 operations per pair)
  *                     whose row sums are compensated: on BASELINE config 3 its V is within
- *                     2.7e-8 hartree rms per point and 5.4e-6 hartree summed over all 16,384
+ *                     2.7e-8 hartree rms per point and 2.4e-6 hartree summed over all 16,384
  *                     points; the batched V + E kernel does the same by default (2.6e-8,
- *                     5.8e-6; qmmm_field_set_accurate_v). */
+ *                     2.6e-6; qmmm_field_set_accurate_v). */
 typedef enum { QMMM_FP64 = 0, QMMM_FP32_ACC64 = 1 } qmmm_precision;
 
 /*
@@ -327,10 +327,11 @@ qmmm_status qmmm_field_set_local_lattice(qmmm_field *h, int mode);
  * (configs[3]) that is 4e-12 of the sum, which plain FP32 arithmetic with FP64 accumulation of
  * row sums misses (3.1e-5: a common bias of +1.9e-9 hartree per point and 6.7e-8 rms).
  * enable != 0 (default): r^2 = rxy2 + z2 with rxy2 formed in FP64 per (point, row) and z2 from a
- * second per-CTA table, both rounded once, and the last level of the FP32 row sums added with a
- * two-sum (as in the potential-only kernel): 2.6e-8 rms, +3.6e-10 mean, 5.8e-6 over the batch
- * (1.5e-6 ... 1.3e-5 over six seeded batches of that size: 24-bit r^2 leaves about 6e-6 +- 3.4e-6),
- * at 5.6 % more time (configs[3]: 5.60 instead of 5.30 ms).  enable = 0: the faster kernel
+ * second per-CTA table, both rounded once, the last level of the FP32 row sums added with a
+ * two-sum and the one below it pairwise (as in the potential-only kernel): 2.6e-8 rms, +1.6e-10
+ * mean, 2.6e-6 over the batch (0.9e-6 ... 9.3e-6 over seven seeded batches of that size: 24-bit
+ * r^2 leaves about 3.6e-6 +- 3.4e-6, so larger batches will exceed 1e-5), at 6 % more time
+ * (configs[3]: 5.62 instead of 5.30 ms).  enable = 0: the faster kernel
  * (every per-configuration energy still within 2e-6 hartree).  E agrees between the two to FP32
  * rounding (1e-7 relative).  Used when both tables fit in shared memory beside a pipeline of at
  * least two stages (z axes of up to 192 nodes: every FP32 BASELINE configuration), else the

@@ -122,8 +122,8 @@ __device__ __forceinline__ void add_run(float2 &v, float2 &d, float2 x, float2 d
 // VONLY -- a z2 entry beside every dz entry of the table, rxy2 formed in FP64 per (point, row) --
 // and the same compensated row sums, with dz still read for sum c dz.  Still 8 operations per
 // pair (r^2 is one add instead of one fma), one more broadcast load per node, a quarter
-// operation for the two-sum: +5.6 % time on config 3 for V rms 6.7e-8 -> 2.6e-8 hartree and the
-// total over the 16,384 points of the batch 3.1e-5 -> 5.8e-6.
+// operation for the two-sum: +6 % time on config 3 for V rms 6.7e-8 -> 2.6e-8 hartree and the
+// total over the 16,384 points of the batch 3.1e-5 -> 2.6e-6.
 template <int EP2, int TS = 0, bool VONLY = false, bool ACCV = false>
 struct GridRowF32 {
     static_assert(!VONLY || TS > 0, "the potential-only walk is table-driven");
