@@ -94,7 +94,7 @@ def parse_args():
                     help="E = NULL: the potential alone (PAPER.md Eq. 4 proper); fewer operations per pair")
     ap.add_argument("--fast-v", action="store_true",
                     help="qmmm_field_set_accurate_v(h, 0): the batched FP32 grid V + E kernel without the accurate-V "
-                         "arithmetic (5.6 %% faster; misses the batch-total energy criterion, DESIGN.md section 6)")
+                         "arithmetic (6 %% faster; misses the batch-total energy criterion, DESIGN.md section 6)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-sweep", action="store_true",
                     help="skip the per-config table (all five configs) at N=1")

@@ -337,7 +337,7 @@ def qmmm_field_set_local_lattice(handle: int, mode: int = -1) -> None:
 
 
 def qmmm_field_set_accurate_v(handle: int, enable: bool = True) -> None:
-    """FP32 batched grid V + E kernel: accurate V (default on; off = the 5.6 % faster kernel)."""
+    """FP32 batched grid V + E kernel: accurate V (default on; off = the 6 % faster kernel)."""
     _check(_lib.qmmm_field_set_accurate_v(handle, int(bool(enable))))
 
 
